@@ -1,0 +1,240 @@
+"""ctypes front-end of the CPU oracle (oracle.c).  TEST INFRASTRUCTURE ONLY.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
+import this.  It never imports paper_2502_15253_b200 and vice versa; the only module both sides
+use is `workloads` (seeded inputs, no arithmetic of the method).
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+from typing import List, Sequence
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "oracle.c")
+_LIB = os.path.join(_HERE, "liboracle.so")
+_CFLAGS = ["-O2", "-std=c11", "-mfma", "-ffp-contract=off", "-fopenmp", "-shared", "-fPIC"]
+
+
+def build(force: bool = False) -> str:
+    """Compile oracle.c with gcc (building the checker is not using it)."""
+    stale = (not os.path.exists(_LIB)) or any(
+        os.path.getmtime(os.path.join(_HERE, f)) > os.path.getmtime(_LIB) for f in ("oracle.c", "oracle.h"))
+    if force or stale:
+        tmp = _LIB + f".tmp{os.getpid()}"
+        subprocess.check_call(["gcc", *_CFLAGS, _SRC, "-o", tmp, "-lm"])
+        os.replace(tmp, _LIB)
+    return _LIB
+
+
+class _Events(C.Structure):
+    _fields_ = [("n", C.c_int64), ("e_nu", C.c_void_p), ("e_vis", C.c_void_p), ("w", C.c_void_p),
+                ("core", C.c_void_p), ("n_cores", C.c_int32), ("L_m", C.c_void_p),
+                ("n_bins", C.c_int32), ("edges", C.c_void_p)]
+
+
+class _Bkg(C.Structure):
+    _fields_ = [("idx_rate", C.c_int32), ("tmpl", C.c_void_p), ("idx_shape", C.c_void_p)]
+
+
+class _Dataset(C.Structure):
+    _fields_ = [("n_bins", C.c_int32), ("idx_a", C.c_int32 * 3), ("idx_signorm", C.c_int32),
+                ("norm", C.c_double), ("idx_flux", C.c_void_p), ("n_bkg", C.c_int32),
+                ("bkg", C.POINTER(_Bkg))]
+
+
+class _Model(C.Structure):
+    _fields_ = [("osc_model", C.c_int32), ("ordering", C.c_int32), ("n_params", C.c_int32),
+                ("n_datasets", C.c_int32), ("idx_osc", C.c_int32 * 6), ("fixed_osc", C.c_double * 6),
+                ("datasets", C.POINTER(_Dataset)), ("prior_mean", C.c_void_p), ("prior_sigma", C.c_void_p)]
+
+
+_lib = None
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        lib = C.CDLL(build())
+        dp = C.POINTER(C.c_double)
+        lib.orc_terms.restype = C.c_int
+        lib.orc_terms.argtypes = [C.POINTER(_Model), dp, dp, dp]
+        lib.orc_pee.restype = C.c_double
+        lib.orc_pee.argtypes = [C.c_int, dp, dp, C.c_double, C.c_double]
+        lib.orc_escale.restype = C.c_double
+        lib.orc_escale.argtypes = [C.c_double] * 4
+        lib.orc_bin.restype = C.c_int32
+        lib.orc_bin.argtypes = [dp, C.c_int32, C.c_double]
+        lib.orc_dev.restype = C.c_double
+        lib.orc_dev.argtypes = [C.c_double, C.c_double]
+        lib.orc_spectra.restype = C.c_int
+        lib.orc_spectra.argtypes = [C.POINTER(_Model), C.POINTER(_Events), C.c_int32, dp, dp, C.c_int]
+        lib.orc_event_bins.restype = C.c_int
+        lib.orc_event_bins.argtypes = [C.POINTER(_Model), C.POINTER(_Events), C.c_int32, dp,
+                                       C.POINTER(C.c_int32)]
+        lib.orc_expectation.restype = C.c_int
+        lib.orc_expectation.argtypes = [C.POINTER(_Model), C.c_int32, dp, dp, dp]
+        lib.orc_nll_from_mu.restype = C.c_int
+        lib.orc_nll_from_mu.argtypes = [C.POINTER(_Model), C.c_int32, dp, dp, dp, dp]
+        lib.orc_nll.restype = C.c_int
+        lib.orc_nll.argtypes = [C.POINTER(_Model), C.POINTER(_Events), C.c_int32, dp, dp, dp, C.c_int]
+        lib.orc_max_threads.restype = C.c_int
+        _lib = lib
+    return _lib
+
+
+def _dp(a: np.ndarray):
+    return a.ctypes.data_as(C.POINTER(C.c_double))
+
+
+def _f64(a) -> np.ndarray:
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+class Oracle:
+    """Binds one `workloads.ModelSpec` (+ optionally its event lists) to the C oracle."""
+
+    def __init__(self, model, events: Sequence = ()):
+        self._keep: List[object] = []          # numpy arrays the C structs point into
+        self.model = model
+        self._m = self._marshal_model(model)
+        self._ev = self._marshal_events(events) if len(events) else None
+        self.n_params = model.n_params
+        self.total_bins = sum(d.n_bins for d in model.datasets)
+        self.n_events = sum(e.n for e in events)
+
+    # -- marshalling ---------------------------------------------------------------------------
+    def _arr(self, a, dtype):
+        a = np.ascontiguousarray(a, dtype=dtype)
+        self._keep.append(a)
+        return a.ctypes.data
+
+    def _marshal_model(self, model) -> _Model:
+        ds_arr = (_Dataset * len(model.datasets))()
+        for d, ds in enumerate(model.datasets):
+            bk_arr = (_Bkg * max(1, len(ds.bkg)))()
+            for k, bk in enumerate(ds.bkg):
+                bk_arr[k].idx_rate = int(bk.idx_rate)
+                bk_arr[k].tmpl = self._arr(bk.tmpl, np.float64)
+                bk_arr[k].idx_shape = None if bk.idx_shape is None else self._arr(bk.idx_shape, np.int32)
+            self._keep.append(bk_arr)
+            ds_arr[d].n_bins = int(ds.n_bins)
+            ds_arr[d].idx_a = (C.c_int32 * 3)(*[int(i) for i in ds.idx_a])
+            ds_arr[d].idx_signorm = int(ds.idx_signorm)
+            ds_arr[d].norm = float(ds.norm)
+            ds_arr[d].idx_flux = None if ds.idx_flux is None else self._arr(ds.idx_flux, np.int32)
+            ds_arr[d].n_bkg = len(ds.bkg)
+            ds_arr[d].bkg = C.cast(bk_arr, C.POINTER(_Bkg))
+        self._keep.append(ds_arr)
+        m = _Model()
+        m.osc_model = int(model.osc_model)
+        m.ordering = int(model.ordering)
+        m.n_params = int(model.n_params)
+        m.n_datasets = len(model.datasets)
+        m.idx_osc = (C.c_int32 * 6)(*[int(i) for i in model.idx_osc])
+        m.fixed_osc = (C.c_double * 6)(*[float(x) for x in model.fixed_osc])
+        m.datasets = C.cast(ds_arr, C.POINTER(_Dataset))
+        m.prior_mean = None if model.prior_mean is None else self._arr(model.prior_mean, np.float64)
+        m.prior_sigma = None if model.prior_sigma is None else self._arr(model.prior_sigma, np.float64)
+        return m
+
+    def _marshal_events(self, events):
+        arr = (_Events * len(events))()
+        for d, e in enumerate(events):
+            arr[d].n = e.n
+            arr[d].e_nu = self._arr(e.e_nu, np.float32)
+            arr[d].e_vis = self._arr(e.e_vis, np.float32)
+            arr[d].w = None if e.w is None else self._arr(e.w, np.float32)
+            arr[d].core = None if e.core is None else self._arr(e.core, np.int32)
+            arr[d].n_cores = len(e.L_m)
+            arr[d].L_m = self._arr(e.L_m, np.float64)
+            arr[d].n_bins = e.n_bins
+            arr[d].edges = self._arr(e.edges, np.float64)
+        return arr
+
+    def _params(self, params):
+        p = _f64(params)
+        if p.ndim == 1:
+            p = p[None, :]
+        assert p.shape[1] == self.n_params, (p.shape, self.n_params)
+        return p
+
+    # -- O1/O2 ---------------------------------------------------------------------------------
+    def terms(self, theta):
+        th = _f64(theta)
+        A = np.zeros(3)
+        m = np.zeros(3)
+        S = _load().orc_terms(C.byref(self._m), _dp(th), _dp(A), _dp(m))
+        assert S > 0
+        return A[:S].copy(), m[:S].copy()
+
+    # -- O3 ------------------------------------------------------------------------------------
+    def spectra(self, params, n_threads: int = 0) -> np.ndarray:
+        p = self._params(params)
+        hist = np.zeros((p.shape[0], self.total_bins))
+        rc = _load().orc_spectra(C.byref(self._m), self._ev, p.shape[0], _dp(p), _dp(hist), n_threads)
+        assert rc == 0, rc
+        return hist
+
+    def event_bins(self, params) -> np.ndarray:
+        p = self._params(params)
+        bins = np.zeros((p.shape[0], self.n_events), dtype=np.int32)
+        rc = _load().orc_event_bins(C.byref(self._m), self._ev, p.shape[0], _dp(p),
+                                    bins.ctypes.data_as(C.POINTER(C.c_int32)))
+        assert rc == 0, rc
+        return bins
+
+    # -- O4 / O5 -------------------------------------------------------------------------------
+    def expectation(self, params, hist) -> np.ndarray:
+        p = self._params(params)
+        h = _f64(hist).reshape(p.shape[0], self.total_bins)
+        mu = np.zeros_like(h)
+        rc = _load().orc_expectation(C.byref(self._m), p.shape[0], _dp(p), _dp(h), _dp(mu))
+        assert rc == 0, rc
+        return mu
+
+    def nll_from_mu(self, params, mu, data) -> np.ndarray:
+        p = self._params(params)
+        mu = _f64(mu).reshape(p.shape[0], self.total_bins)
+        data = _f64(data)
+        assert data.shape == (self.total_bins,)
+        out = np.zeros(p.shape[0])
+        rc = _load().orc_nll_from_mu(C.byref(self._m), p.shape[0], _dp(p), _dp(mu), _dp(data), _dp(out))
+        assert rc == 0, rc
+        return out
+
+    def nll(self, params, data, n_threads: int = 0) -> np.ndarray:
+        p = self._params(params)
+        data = _f64(data)
+        assert data.shape == (self.total_bins,)
+        out = np.zeros(p.shape[0])
+        rc = _load().orc_nll(C.byref(self._m), self._ev, p.shape[0], _dp(p), _dp(data), _dp(out), n_threads)
+        assert rc == 0, rc
+        return out
+
+
+# -- scalar helpers (pins) ----------------------------------------------------------------------
+def pee(A, dm2, L_m: float, E_MeV: float) -> float:
+    A = _f64(A)
+    dm2 = _f64(dm2)
+    return float(_load().orc_pee(len(A), _dp(A), _dp(dm2), float(L_m), float(E_MeV)))
+
+
+def escale(a0: float, a1: float, a2: float, v: float) -> float:
+    return float(_load().orc_escale(a0, a1, a2, v))
+
+
+def bin_index(edges, e: float) -> int:
+    ed = _f64(edges)
+    return int(_load().orc_bin(_dp(ed), len(ed) - 1, float(e)))
+
+
+def dev(n: float, mu: float) -> float:
+    return float(_load().orc_dev(float(n), float(mu)))
+
+
+def max_threads() -> int:
+    return int(_load().orc_max_threads())

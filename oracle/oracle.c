@@ -1,0 +1,294 @@
+/*
+ * oracle.c -- see oracle.h.  TEST INFRASTRUCTURE ONLY; shares nothing with the CUDA path.
+ *
+ * Build: gcc -O2 -std=c11 -mfma -ffp-contract=off -fopenmp -shared -fPIC oracle.c -o liboracle.so -lm
+ *   -ffp-contract=off : no a*b+c is fused unless written as fma(); the only fma() calls are the
+ *                       two in orc_escale(), whose rounding sequence is normative (R8).
+ *   -mfma             : fma() compiles to one vfmadd instead of the (equally correctly rounded)
+ *                       libm software routine.
+ *
+ * Steps follow SURVEY.md 8(c) O1-O5, which restate PAPER.md:34-39 (Eq. 1-2), :67-83 (Eq. 3-6),
+ * :119-125 (Eq. 9) and :177 (signal step 1).
+ */
+#include "oracle.h"
+
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+/* phase = 1.267 * dm2[eV^2] * L[m] / E[MeV]  (R1: the literal 1.267, as north_star states) */
+static const double K_PHASE = 1.267;
+
+static double par(const orc_model *m, const double *theta, int slot)
+{
+    int idx = m->idx_osc[slot];
+    return idx >= 0 ? theta[idx] : m->fixed_osc[slot];
+}
+
+/* first-octant branch theta < pi/4 (R4): cos 2theta = +sqrt(1 - sin^2 2theta) */
+static void mixing(double s22, double *cos2, double *sin2, double *cos4)
+{
+    double c2t = sqrt(1.0 - s22);
+    *cos2 = (1.0 + c2t) / 2.0;
+    *sin2 = (1.0 - c2t) / 2.0;
+    *cos4 = (*cos2) * (*cos2);
+}
+
+int orc_terms(const orc_model *m, const double *theta, double A[ORC_MAX_TERMS], double dm2[ORC_MAX_TERMS])
+{
+    double s13 = par(m, theta, 0), mee = par(m, theta, 1);
+    double s12 = par(m, theta, 2), m21 = par(m, theta, 3);
+    double c2_13, s2_13, c4_13, c2_12, s2_12, c4_12;
+    mixing(s13, &c2_13, &s2_13, &c4_13);
+    mixing(s12, &c2_12, &s2_12, &c4_12);
+    (void)s2_13; (void)c4_12;
+
+    switch (m->osc_model) {
+    case ORC_EQ1:
+        /* PAPER.md:34 Eq. 1:  1 - sin^2(2th13) sin^2(D_ee) - cos^4(th13) sin^2(2th12) sin^2(D_21) */
+        A[0] = s13;          dm2[0] = mee;
+        A[1] = c4_13 * s12;  dm2[1] = m21;
+        return 2;
+    case ORC_FULL3: {
+        /* exact 3-flavour vacuum P_ee (BASELINE.json config 4 "with dm2_31, dm2_32"):
+         *   1 - cos^4(th13) sin^2(2th12) sin^2(D_21)
+         *     - sin^2(2th13) [cos^2(th12) sin^2(D_31) + sin^2(th12) sin^2(D_32)]
+         * with |dm2_31|, |dm2_32| from inverting PAPER.md:39 Eq. 2 under dm2_31 - dm2_32 = dm2_21:
+         *   normal   (o=+1): dm31 = mee + sin^2(th12) m21,  dm32 = mee - cos^2(th12) m21
+         *   inverted (o=-1): |dm31| = mee - sin^2(th12) m21, |dm32| = mee + cos^2(th12) m21     */
+        double o = m->ordering >= 0 ? 1.0 : -1.0;
+        A[0] = c4_13 * s12;  dm2[0] = m21;
+        A[1] = s13 * c2_12;  dm2[1] = mee + o * s2_12 * m21;
+        A[2] = s13 * s2_12;  dm2[2] = mee - o * c2_12 * m21;
+        return 3;
+    }
+    case ORC_STERILE4: {
+        /* BASELINE.json config 5 (the paper prints no 3+1 formula):
+         *   1 - cos^4(th14) sin^2(2th13) sin^2(D_ee) - sin^2(2th14) sin^2(D_41)
+         *     - cos^4(th13) sin^2(2th12) sin^2(D_21)                                             */
+        double s14 = par(m, theta, 4), m41 = par(m, theta, 5);
+        double c2_14, s2_14, c4_14;
+        mixing(s14, &c2_14, &s2_14, &c4_14);
+        (void)c2_14; (void)s2_14;
+        A[0] = c4_14 * s13;  dm2[0] = mee;
+        A[1] = s14;          dm2[1] = m41;
+        A[2] = c4_13 * s12;  dm2[2] = m21;
+        return 3;
+    }
+    default:
+        return -1;
+    }
+}
+
+double orc_pee(int S, const double *A, const double *dm2, double L_m, double E_MeV)
+{
+    double x = L_m / E_MeV;
+    double p = 1.0;
+    for (int k = 0; k < S; ++k) {
+        double c = K_PHASE * dm2[k];
+        double s = sin(c * x);
+        p -= A[k] * (s * s);
+    }
+    return p;
+}
+
+double orc_escale(double a0, double a1, double a2, double e_vis)
+{
+    return fma(fma(a2, e_vis, a1), e_vis, a0);
+}
+
+int32_t orc_bin(const double *edges, int32_t n_bins, double e)
+{
+    if (e < edges[0] || !(e < edges[n_bins])) return -1;   /* also drops NaN */
+    /* upper_bound(edges, e) - 1 : last j with edges[j] <= e */
+    int32_t lo = 0, hi = n_bins;                            /* invariant edges[lo] <= e < edges[hi] */
+    while (hi - lo > 1) {
+        int32_t mid = lo + (hi - lo) / 2;
+        if (edges[mid] <= e) lo = mid; else hi = mid;
+    }
+    return lo;
+}
+
+/* Neumaier-compensated running sum: keeps the oracle's own rounding << 1e-9 of a bin. */
+static inline void nsum(double *s, double *c, double y)
+{
+    double t = *s + y;
+    if (!isfinite(t)) { *s = t; return; }        /* inf / NaN: nothing to compensate */
+    if (fabs(*s) >= fabs(y)) *c += (*s - t) + y;
+    else                     *c += (y - t) + *s;
+    *s = t;
+}
+
+static int64_t total_bins(const orc_model *m)
+{
+    int64_t t = 0;
+    for (int d = 0; d < m->n_datasets; ++d) t += m->datasets[d].n_bins;
+    return t;
+}
+
+static void get_a(const orc_dataset *ds, const double *theta, double a[3])
+{
+    static const double dflt[3] = {0.0, 1.0, 0.0};
+    for (int j = 0; j < 3; ++j) a[j] = ds->idx_a[j] >= 0 ? theta[ds->idx_a[j]] : dflt[j];
+}
+
+static int check(const orc_model *m, const orc_events *ev)
+{
+    if (!m || !ev || m->n_datasets <= 0) return -1;
+    for (int d = 0; d < m->n_datasets; ++d)
+        if (m->datasets[d].n_bins != ev[d].n_bins || ev[d].n_bins <= 0) return -2;
+    return 0;
+}
+
+/* one point: signal step 1 of PAPER.md:177 -- weight every MC event with P_ee and sum per bin */
+static void spectra_point(const orc_model *m, const orc_events *ev, const double *theta,
+                          double *hist, double *comp, int32_t *bins_out)
+{
+    double A[ORC_MAX_TERMS], dm2[ORC_MAX_TERMS];
+    int S = orc_terms(m, theta, A, dm2);
+    int64_t off = 0, ev_off = 0;
+    for (int d = 0; d < m->n_datasets; ++d) {
+        const orc_events *e = &ev[d];
+        const orc_dataset *ds = &m->datasets[d];
+        double a[3];
+        get_a(ds, theta, a);
+        for (int b = 0; b < e->n_bins; ++b) { hist[off + b] = 0.0; comp[off + b] = 0.0; }
+        for (int64_t i = 0; i < e->n; ++i) {
+            double E = (double)e->e_nu[i];
+            double L = e->L_m[e->core ? e->core[i] : 0];
+            double p = orc_pee(S, A, dm2, L, E);
+            double v = (double)e->e_vis[i];
+            double ep = orc_escale(a[0], a[1], a[2], v);
+            int32_t b = orc_bin(e->edges, e->n_bins, ep);
+            if (bins_out) bins_out[ev_off + i] = b;
+            if (b < 0) continue;
+            double wi = e->w ? (double)e->w[i] : 1.0;
+            nsum(&hist[off + b], &comp[off + b], wi * p);
+        }
+        for (int b = 0; b < e->n_bins; ++b) hist[off + b] += comp[off + b];
+        off += e->n_bins;
+        ev_off += e->n;
+    }
+}
+
+int orc_max_threads(void)
+{
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+
+int orc_spectra(const orc_model *m, const orc_events *ev, int32_t P, const double *params,
+                double *hist, int n_threads)
+{
+    int rc = check(m, ev);
+    if (rc) return rc;
+    int64_t TB = total_bins(m);
+    int nt = n_threads > 0 ? n_threads : orc_max_threads();
+    (void)nt;
+#pragma omp parallel num_threads(nt)
+    {
+        double *comp = (double *)malloc(sizeof(double) * (size_t)TB);
+#pragma omp for schedule(dynamic, 1)
+        for (int32_t p = 0; p < P; ++p)
+            spectra_point(m, ev, params + (int64_t)p * m->n_params, hist + (int64_t)p * TB, comp, NULL);
+        free(comp);
+    }
+    return 0;
+}
+
+int orc_event_bins(const orc_model *m, const orc_events *ev, int32_t P, const double *params,
+                   int32_t *bins)
+{
+    int rc = check(m, ev);
+    if (rc) return rc;
+    int64_t TB = total_bins(m), NE = 0;
+    for (int d = 0; d < m->n_datasets; ++d) NE += ev[d].n;
+    double *h = (double *)malloc(sizeof(double) * (size_t)TB * 2);
+    for (int32_t p = 0; p < P; ++p)
+        spectra_point(m, ev, params + (int64_t)p * m->n_params, h, h + TB, bins + (int64_t)p * NE);
+    free(h);
+    return 0;
+}
+
+int orc_expectation(const orc_model *m, int32_t P, const double *params, const double *hist, double *mu)
+{
+    int64_t TB = total_bins(m);
+    for (int32_t p = 0; p < P; ++p) {
+        const double *theta = params + (int64_t)p * m->n_params;
+        int64_t off = 0;
+        for (int d = 0; d < m->n_datasets; ++d) {
+            const orc_dataset *ds = &m->datasets[d];
+            double eps = ds->idx_signorm >= 0 ? theta[ds->idx_signorm] : 1.0;
+            for (int b = 0; b < ds->n_bins; ++b) {
+                double f = (ds->idx_flux && ds->idx_flux[b] >= 0) ? theta[ds->idx_flux[b]] : 1.0;
+                double v = eps * ds->norm * f * hist[p * TB + off + b];      /* signal */
+                for (int k = 0; k < ds->n_bkg; ++k) {                        /* + backgrounds */
+                    const orc_bkg *bk = &ds->bkg[k];
+                    double r = bk->idx_rate >= 0 ? theta[bk->idx_rate] : 1.0;
+                    double s = (bk->idx_shape && bk->idx_shape[b] >= 0) ? theta[bk->idx_shape[b]] : 1.0;
+                    v += r * s * bk->tmpl[b];
+                }
+                mu[p * TB + off + b] = v;
+            }
+            off += ds->n_bins;
+        }
+    }
+    return 0;
+}
+
+double orc_dev(double n, double mu)
+{
+    /* -ln L + ln L_saturated for one Poisson bin (Eq. 3 over PAPER.md:96 Eq. 8's
+     * saturated model mu = n): the n! cancels.  DESIGN.md R9 (normalisation), R10 (edge cases). */
+    if (isnan(n) || isnan(mu)) return NAN;
+    if (mu < 0.0) return INFINITY;
+    if (n > 0.0) {
+        if (mu == 0.0) return INFINITY;
+        return mu - n + n * log(n / mu);
+    }
+    if (n == 0.0) return mu;
+    return NAN;                                  /* negative counts are not data */
+}
+
+int orc_nll_from_mu(const orc_model *m, int32_t P, const double *params, const double *mu,
+                    const double *data, double *nll)
+{
+    int64_t TB = total_bins(m);
+    for (int32_t p = 0; p < P; ++p) {
+        const double *theta = params + (int64_t)p * m->n_params;
+        double s = 0.0, c = 0.0;
+        for (int64_t i = 0; i < TB; ++i) nsum(&s, &c, orc_dev(data[i], mu[p * TB + i]));
+        if (m->prior_mean && m->prior_sigma) {
+            /* uncorrelated Gaussian priors G(b - b_bar, sigma) (Eq. 6):
+             * -ln G = 1/2 ((b - b_bar)/sigma)^2 + const, constant dropped (R9) */
+            for (int j = 0; j < m->n_params; ++j) {
+                double sg = m->prior_sigma[j];
+                if (!(sg > 0.0) || isinf(sg)) continue;
+                double z = (theta[j] - m->prior_mean[j]) / sg;
+                nsum(&s, &c, 0.5 * z * z);
+            }
+        }
+        nll[p] = s + c;
+    }
+    return 0;
+}
+
+int orc_nll(const orc_model *m, const orc_events *ev, int32_t P, const double *params,
+            const double *data, double *nll, int n_threads)
+{
+    int64_t TB = total_bins(m);
+    double *hist = (double *)malloc(sizeof(double) * (size_t)TB * (size_t)P * 2);
+    if (!hist) return -3;
+    double *mu = hist + (size_t)TB * (size_t)P;
+    int rc = orc_spectra(m, ev, P, params, hist, n_threads);
+    if (!rc) rc = orc_expectation(m, P, params, hist, mu);
+    if (!rc) rc = orc_nll_from_mu(m, P, params, mu, data, nll);
+    free(hist);
+    return rc;
+}

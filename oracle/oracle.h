@@ -1,0 +1,115 @@
+/*
+ * oracle.h -- plain CPU oracle for the oscillation-weighted event spectrum and the binned
+ * Poisson negative log-likelihood of arXiv 2502.15253 (PhyLiNO).
+ *
+ * TEST INFRASTRUCTURE ONLY.  Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+ * --impl reference legs may build, load or call this.  It shares no code, header, table or
+ * constant with the CUDA path under paper_2502_15253_b200/ and neither includes the other.
+ *
+ * Everything is straight double-precision loops in the caller's event order, libm sin/log/sqrt,
+ * std fma() where the rounding sequence is normative.  Citations are PAPER.md line numbers
+ * and DESIGN.md reading numbers (R1...).
+ *
+ * Pins (tests/test_oracle_*.py): every function below is pinned by closed forms, invariants,
+ * mpmath / exact-rational brute force and textbook identities; none is "parity unpinned".
+ * End-to-end numeric values are NOT pinned against the paper: it prints no spectrum or
+ * likelihood value and its inputs are not public ("What pins the oracle").
+ */
+#ifndef PHYLINO_ORACLE_H
+#define PHYLINO_ORACLE_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum { ORC_EQ1 = 0, ORC_FULL3 = 1, ORC_STERILE4 = 2 };
+enum { ORC_MAX_TERMS = 3 };
+
+/* MC events of one dataset, caller order. */
+typedef struct {
+    int64_t        n;
+    const float   *e_nu;     /* [n] true neutrino energy, MeV */
+    const float   *e_vis;    /* [n] reconstructed energy, MeV */
+    const float   *w;        /* [n] MC weight, NULL => 1 */
+    const int32_t *core;     /* [n] reactor-core index, NULL => 0 */
+    int32_t        n_cores;
+    const double  *L_m;      /* [n_cores] baselines, metres */
+    int32_t        n_bins;
+    const double  *edges;    /* [n_bins+1] strictly ascending */
+} orc_events;
+
+typedef struct {
+    int32_t        idx_rate;   /* -1 => 1 */
+    const double  *tmpl;       /* [n_bins] */
+    const int32_t *idx_shape;  /* [n_bins] or NULL => 1 */
+} orc_bkg;
+
+typedef struct {
+    int32_t        n_bins;
+    int32_t        idx_a[3];     /* -1 => (0,1,0) */
+    int32_t        idx_signorm;  /* -1 => 1 */
+    double         norm;
+    const int32_t *idx_flux;     /* [n_bins] or NULL => 1 */
+    int32_t        n_bkg;
+    const orc_bkg *bkg;
+} orc_dataset;
+
+typedef struct {
+    int32_t            osc_model;    /* ORC_EQ1 / ORC_FULL3 / ORC_STERILE4 */
+    int32_t            ordering;     /* +1 normal, -1 inverted (FULL3) */
+    int32_t            n_params;
+    int32_t            n_datasets;
+    int32_t            idx_osc[6];   /* s13, mee, s12, m21, s14, m41; -1 => fixed_osc */
+    double             fixed_osc[6];
+    const orc_dataset *datasets;
+    const double      *prior_mean;   /* [n_params] or NULL */
+    const double      *prior_sigma;  /* [n_params] or NULL; <=0, inf or NaN => unconstrained */
+} orc_model;
+
+/* O1-O2: amplitudes A_k and mass splittings m_k [eV^2] of the oscillation terms at one point.
+ * Returns the number of terms S (2 or 3).  PAPER.md:34 (Eq. 1), :39 (Eq. 2), BASELINE.json config 5. */
+int orc_terms(const orc_model *m, const double *theta, double A[ORC_MAX_TERMS], double dm2[ORC_MAX_TERMS]);
+
+/* P_ee = 1 - sum_k A_k sin^2(1.267 dm2_k L/E)   (Eq. 1; phase constant: DESIGN.md R1). */
+double orc_pee(int S, const double *A, const double *dm2, double L_m, double E_MeV);
+
+/* Energy-scale map E' = fma(fma(a2,v,a1),v,a0)  (R8). */
+double orc_escale(double a0, double a1, double a2, double e_vis);
+
+/* Bin of E' in half-open bins [edges[b], edges[b+1]); -1 if outside or NaN (R7). */
+int32_t orc_bin(const double *edges, int32_t n_bins, double e);
+
+/* O3: hist[p][off_d + b] = sum_i w_i P_ee(i,p) over events of dataset d landing in bin b.
+ * hist is [P][total_bins] row-major, dataset-major inside a point.  n_threads <= 0 => all cores
+ * (parallel over points only; each point sums its events sequentially in input order). */
+int orc_spectra(const orc_model *m, const orc_events *ev, int32_t P, const double *params,
+                double *hist, int n_threads);
+
+/* Same, additionally writing the bin index of every event of every dataset at point p
+ * (bins[p][i] over the concatenated events, -1 = dropped).  For bit-exact bin-assignment parity. */
+int orc_event_bins(const orc_model *m, const orc_events *ev, int32_t P, const double *params,
+                   int32_t *bins);
+
+/* O4: mu[p][off_d+b] = eps_d norm_d f_db H + sum_k r_dk s_dkb T_dkb. */
+int orc_expectation(const orc_model *m, int32_t P, const double *params, const double *hist, double *mu);
+
+/* Half-deviance of one bin, mu - n + n ln(n/mu)  (PAPER.md:67 Eq. 3, :96 Eq. 8; R9-R10). */
+double orc_dev(double n, double mu);
+
+/* O5: nll[p] = sum_bins dev(n, mu) + 1/2 sum_j ((theta_j - mean_j)/sigma_j)^2  (PAPER.md:82 Eq. 6, :119 Eq. 9). */
+int orc_nll_from_mu(const orc_model *m, int32_t P, const double *params, const double *mu,
+                    const double *data, double *nll);
+
+/* O3+O4+O5 in one call. */
+int orc_nll(const orc_model *m, const orc_events *ev, int32_t P, const double *params,
+            const double *data, double *nll, int n_threads);
+
+/* Number of threads orc_spectra would use for n_threads <= 0. */
+int orc_max_threads(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,92 @@
+"""Plain data containers describing a fit model and its inputs (no arithmetic).
+
+Names follow the paper: datasets d, bins i, parameter
+vector theta, signal/background contributions.
+"""
+from __future__ import annotations
+
+from dataclasses import dataclass, field
+from typing import List, Optional
+
+import numpy as np
+
+# oscillation models (BASELINE.json configs 1-3 / 4 / 5)
+OSC_EQ1 = 0        # PAPER.md:34 Eq. 1 (two terms)
+OSC_FULL3 = 1      # exact 3-flavour vacuum P_ee with dm31, dm32 (config 4; Eq. 2 inverted)
+OSC_STERILE4 = 2   # 3+1 extension (formula from BASELINE.json config 5)
+
+# slots of the six oscillation parameters in idx_osc / fixed_osc
+S13, MEE, S12, M21, S14, M41 = range(6)   # sin^2 2theta13, dm2_ee, sin^2 2theta12, dm2_21, sin^2 2theta14, dm2_41
+
+
+@dataclass
+class BkgSpec:
+    """One background contribution of one dataset: rate * shape_i * template_i."""
+    tmpl: np.ndarray                       # float64 [n_bins] expected counts at rate = shape = 1
+    idx_rate: int = -1                     # index into theta, -1 => 1
+    idx_shape: Optional[np.ndarray] = None  # int32 [n_bins] indices into theta (-1 => 1), None => all 1
+
+
+@dataclass
+class DatasetSpec:
+    """How theta acts on one dataset's signal spectrum and backgrounds."""
+    n_bins: int
+    idx_a: tuple = (-1, -1, -1)            # energy-scale a0,a1,a2; -1 => (0,1,0)
+    idx_signorm: int = -1                  # detection-efficiency-like multiplier; -1 => 1
+    norm: float = 1.0                      # constant MC -> data normalisation
+    idx_flux: Optional[np.ndarray] = None  # int32 [n_bins] per-bin flux scale; None => all 1
+    bkg: List[BkgSpec] = field(default_factory=list)
+
+
+@dataclass
+class DatasetEvents:
+    """MC event list of one dataset in the caller's (unsorted) order."""
+    e_nu: np.ndarray      # float32 [n] true neutrino energy, MeV
+    e_vis: np.ndarray     # float32 [n] reconstructed (visible) energy, MeV
+    w: np.ndarray         # float32 [n] MC weight
+    core: np.ndarray      # int32 [n] reactor-core index (two reactors => two baselines)
+    L_m: np.ndarray       # float64 [n_cores] baseline per core, metres
+    edges: np.ndarray     # float64 [n_bins+1] strictly ascending reco-energy bin edges, MeV
+
+    @property
+    def n(self) -> int:
+        return int(self.e_nu.shape[0])
+
+    @property
+    def n_bins(self) -> int:
+        return int(self.edges.shape[0] - 1)
+
+
+@dataclass
+class ModelSpec:
+    osc_model: int
+    n_params: int
+    idx_osc: tuple                          # 6 indices into theta, -1 => use fixed_osc
+    fixed_osc: tuple                        # 6 fixed values
+    datasets: List[DatasetSpec]
+    ordering: int = +1                      # +1 normal, -1 inverted (FULL3 only)
+    prior_mean: Optional[np.ndarray] = None   # float64 [n_params]
+    prior_sigma: Optional[np.ndarray] = None  # float64 [n_params]; <= 0 or inf => unconstrained
+
+    @property
+    def total_bins(self) -> int:
+        return sum(d.n_bins for d in self.datasets)
+
+
+@dataclass
+class Workload:
+    name: str
+    model: ModelSpec
+    events: List[DatasetEvents]
+    params: np.ndarray        # float64 [P, n_params] batch of parameter points
+    theta0: np.ndarray        # float64 [n_params] the point pseudo-data is drawn at
+    seed: int
+    note: str = ""
+
+    @property
+    def n_points(self) -> int:
+        return int(self.params.shape[0])
+
+    @property
+    def n_events(self) -> int:
+        return sum(e.n for e in self.events)
