@@ -1,0 +1,192 @@
+/*
+ * phylino.h -- C-ABI of the B200 (sm_100a) hot path of PhyLiNO's forward-folding likelihood
+ * fit (arXiv 2502.15253): the oscillation-weighted MC event spectrum, batched over parameter
+ * points, and the binned Poisson negative log-likelihood with Gaussian priors.
+ *
+ * Citations are line numbers of /root/reference/PAPER.md and reading numbers (R1...) of DESIGN.md.
+ *
+ * What the library computes, for every parameter point p of a batch (signal step 1):
+ *
+ *   P_ee(e,p) = 1 - sum_k A_k(p) sin^2( 1.267 dm2_k(p)[eV^2] L_core(e)[m] / E_nu(e)[MeV] )
+ *               (PAPER.md:34 Eq. 1, :39 Eq. 2; 3-flavour and 3+1 forms: DESIGN.md R2, R15)
+ *   E'(e,p)   = fma(fma(a2, v, a1), v, a0),  v = (double)E_vis(e)          (R8)
+ *   H[p,d,b]  = sum over MC events e of dataset d with edges[b] <= E' < edges[b+1] of w(e) P_ee(e,p)
+ *   mu[p,d,b] = eps_d norm_d f_db H[p,d,b] + sum_k r_dk s_dkb T_dkb
+ *   nll[p]    = sum_{d,b} [mu - n + n ln(n/mu)] + 1/2 sum_j ((theta_j - mean_j)/sigma_j)^2
+ *               (PAPER.md:67-83 Eq. 3-6, :96 Eq. 8, :119-125 Eq. 9; R9, R10)
+ *
+ * Conventions
+ *   Pointers  : every pointer argument says HOST or DEVICE.  DEVICE pointers must belong to the
+ *               CUDA device the context was created on.
+ *   Ownership : the context deep-copies everything handed to phylino_set_model and
+ *               phylino_load_events and owns all device memory it allocates.  The caller owns
+ *               `params`, `data` and the outputs; they must stay alive until the stream has
+ *               passed the call.
+ *   Async     : phylino_spectra / phylino_nll / phylino_event_bins only enqueue work on the
+ *               context's stream and return; they never synchronise and never touch host-visible
+ *               output.  phylino_load_events / phylino_set_model synchronise the stream.
+ *   Errors    : every entry point returns a phylino_status; nothing throws across the ABI.
+ *               Shape / state problems are detected on the host before any launch.  The text of
+ *               the last error of a context is kept in phylino_last_error().  VALUE problems in
+ *               device-resident `params` (NaN, sin^2 2theta outside [0,1]) are not errors: they
+ *               propagate as NaN into that point's outputs, as sqrt of a negative does.
+ *   Threads   : one context must not be used from two host threads at once; any number of
+ *               contexts may coexist (independent fits).
+ *   Determinism: identical inputs give bit-identical outputs on every call (64-bit fixed-point
+ *               bin accumulators: integer addition is associative).
+ *   No CPU fallback: without a CUDA device phylino_create fails with PHYLINO_ERR_CUDA.
+ */
+#ifndef PHYLINO_H
+#define PHYLINO_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#if defined(__GNUC__)
+#define PHYLINO_API __attribute__((visibility("default")))
+#else
+#define PHYLINO_API
+#endif
+
+#define PHYLINO_MAX_DATASETS 32     /* PAPER.md:209 splits Double Chooz into 18 histograms */
+#define PHYLINO_MAX_BINS     2048   /* per dataset */
+#define PHYLINO_MAX_BKG      8      /* background contributions per dataset (3-4) */
+
+typedef struct phylino_ctx phylino_ctx;   /* opaque */
+
+typedef enum {
+    PHYLINO_OK        = 0,
+    PHYLINO_ERR_ARG   = 1,   /* NULL pointer, negative size, non-finite weight or baseline, ... */
+    PHYLINO_ERR_SHAPE = 2,   /* sizes disagree with the model (n_bins, dataset index, P < 0, ...) */
+    PHYLINO_ERR_STATE = 3,   /* call order: set_model -> load_events (all datasets) -> spectra/nll */
+    PHYLINO_ERR_OOM   = 4,   /* host or device allocation failed */
+    PHYLINO_ERR_CUDA  = 5    /* any other CUDA runtime error (text in phylino_last_error) */
+} phylino_status;
+
+typedef enum {
+    PHYLINO_OSC_EQ1      = 0,  /* PAPER.md:34 Eq. 1: terms (sin^2 2th13, dm2_ee), (cos^4 th13 sin^2 2th12, dm2_21) */
+    PHYLINO_OSC_FULL3    = 1,  /* exact 3-flavour vacuum P_ee with dm2_31, dm2_32 from Eq. 2 (R2) */
+    PHYLINO_OSC_STERILE4 = 2   /* 3+1 extension (formula of BASELINE.json config 5; R15) */
+} phylino_osc_model;
+
+/* slots of idx_osc / fixed_osc */
+enum { PHYLINO_S13 = 0, PHYLINO_MEE = 1, PHYLINO_S12 = 2, PHYLINO_M21 = 3, PHYLINO_S14 = 4, PHYLINO_M41 = 5 };
+
+/* One background contribution of a dataset: rate * shape_b * template_b. HOST pointers. */
+typedef struct {
+    int32_t        idx_rate;     /* index into theta of the rate multiplier, -1 => 1 */
+    const double  *tmpl;         /* HOST [n_bins] expected counts at rate = shape = 1 */
+    const int32_t *idx_shape;    /* HOST [n_bins] indices into theta (-1 => 1), or NULL => all 1 */
+} phylino_bkg_desc;
+
+/* How theta acts on one dataset. HOST pointers. */
+typedef struct {
+    int32_t        n_bins;
+    int32_t        idx_a[3];     /* energy-scale a0,a1,a2; -1 => 0,1,0 */
+    int32_t        idx_signorm;  /* signal normalisation multiplier eps_d; -1 => 1 */
+    double         norm;         /* constant MC -> data normalisation (R16) */
+    const int32_t *idx_flux;     /* HOST [n_bins] per-bin flux scale f_db, or NULL => all 1 */
+    int32_t        n_bkg;        /* 0 ... PHYLINO_MAX_BKG */
+    const phylino_bkg_desc *bkg; /* HOST [n_bkg] */
+} phylino_dataset_desc;
+
+typedef struct {
+    int32_t  osc_model;          /* phylino_osc_model */
+    int32_t  ordering;           /* +1 normal, -1 inverted; PHYLINO_OSC_FULL3 only (R5) */
+    int32_t  n_params;           /* NPAR, length of one parameter point theta */
+    int32_t  n_datasets;         /* D, 1 ... PHYLINO_MAX_DATASETS */
+    int32_t  idx_osc[6];         /* indices into theta of sin^2 2th13, dm2_ee, sin^2 2th12, dm2_21,
+                                    sin^2 2th14, dm2_41; -1 => fixed_osc[slot] */
+    double   fixed_osc[6];
+    const phylino_dataset_desc *datasets;   /* HOST [n_datasets] */
+    const double *prior_mean;    /* HOST [n_params] or NULL (no priors) */
+    const double *prior_sigma;   /* HOST [n_params] or NULL; sigma <= 0, inf or NaN => unconstrained
+                                    (sin^2 2th13 is left free) */
+} phylino_model_desc;
+
+/* Create a context on CUDA device `device`.  `cuda_stream` is a cudaStream_t (0 = default stream)
+ * on which all later work of this context is enqueued.  Fails with PHYLINO_ERR_CUDA when there is
+ * no such device (there is no CPU fallback). */
+PHYLINO_API phylino_status phylino_create(int device, void *cuda_stream, phylino_ctx **out);
+
+/* Frees everything the context owns.  NULL is allowed. */
+PHYLINO_API void phylino_destroy(phylino_ctx *ctx);
+
+/* Deep-copies the model.  Drops events loaded under an earlier model. */
+PHYLINO_API phylino_status phylino_set_model(phylino_ctx *ctx, const phylino_model_desc *model);
+
+/* Event store of dataset `dataset` (MC events with the full detector response;
+ * :191 "copied to the GPU memory only once").  All pointers HOST; arrays are copied.
+ *   e_nu_MeV  [n] true neutrino energy (finite, > 0)
+ *   e_vis_MeV [n] reconstructed energy (NaN allowed: such an event never lands in a bin)
+ *   weight    [n] MC weight (finite), NULL => 1
+ *   core      [n] reactor-core index in [0, n_cores), NULL => 0       (R13)
+ *   baseline_m[n_cores] L in metres (finite, >= 0)
+ *   edges     [n_bins+1] strictly ascending reco-energy bin edges; n_bins must equal the model's.
+ * The store is structure-of-arrays, sorted by reconstructed energy ("sorted according
+ * to their energy"; R14): x = L_core/E_nu as fp64, E_vis and w as fp32.
+ * n = 0 is allowed (empty dataset).  Reloading a dataset replaces it. */
+PHYLINO_API phylino_status phylino_load_events(phylino_ctx *ctx, int dataset, int64_t n,
+                                   const float *e_nu_MeV, const float *e_vis_MeV, const float *weight,
+                                   const int32_t *core, int n_cores, const double *baseline_m,
+                                   int n_bins, const double *edges);
+
+/* H[p, off_d + b] for P parameter points (PAPER.md:177 step 1; Eq. 1).
+ *   params DEVICE [P x n_params] row-major;  hist DEVICE [P x total_bins], dataset-major inside a point.
+ * P = 0 is a no-op. */
+PHYLINO_API phylino_status phylino_spectra(phylino_ctx *ctx, int P, const double *params, double *hist);
+
+/* nll[p] (PAPER.md:67-83 Eq. 3-6, :119-125 Eq. 9): spectra, expectation assembly and the
+ * Poisson half-deviance + prior reduction, all on the device.
+ *   params DEVICE [P x n_params]; data DEVICE [total_bins] observed counts n_db; nll DEVICE [P]. */
+PHYLINO_API phylino_status phylino_nll(phylino_ctx *ctx, int P, const double *params, const double *data, double *nll);
+
+/* mu[p, off_d + b]: the spectra followed by the expectation assembly (PAPER.md:105-107, :177 step 2
+ * reduced to per-bin multipliers): mu = eps_d norm_d f_db H + sum_k r_dk s_dkb T_dkb.
+ *   params DEVICE [P x n_params]; mu DEVICE [P x total_bins]. */
+PHYLINO_API phylino_status phylino_expectation(phylino_ctx *ctx, int P, const double *params, double *mu);
+
+/* Diagnostic for the bit-exact bin-assignment parity test: bins[p, i] = bin index b (within its
+ * dataset) of event i at point p, -1 if E' falls outside [edges[0], edges[n_bins]) or is NaN.
+ * i runs over the datasets' events concatenated in the CALLER's original order.
+ *   params DEVICE [P x n_params]; bins DEVICE int32 [P x total_events]. */
+PHYLINO_API phylino_status phylino_event_bins(phylino_ctx *ctx, int P, const double *params, int32_t *bins);
+
+/* Same as phylino_nll / phylino_spectra but with HOST buffers: pinned staging, H2D of params (and
+ * data), the kernels, D2H of the result, and a stream synchronise -- the end-to-end call a host
+ * minimiser makes once per batch (parameters go to the GPU, the result comes back). */
+PHYLINO_API phylino_status phylino_nll_host(phylino_ctx *ctx, int P, const double *params_host,
+                                const double *data_host, double *nll_host);
+PHYLINO_API phylino_status phylino_spectra_host(phylino_ctx *ctx, int P, const double *params_host, double *hist_host);
+
+/* Sizes the caller needs for its buffers. */
+PHYLINO_API int64_t phylino_total_bins(const phylino_ctx *ctx);     /* sum_d n_bins, 0 before set_model */
+PHYLINO_API int64_t phylino_total_events(const phylino_ctx *ctx);   /* sum_d n over loaded datasets */
+
+/* Tuning knob (0 => library default): parameter points per CTA pass over an event tile. */
+PHYLINO_API phylino_status phylino_set_point_chunk(phylino_ctx *ctx, int points_per_cta);
+
+/* Device timing of the two kernels of a call (CUDA events on the context's stream, recorded around
+ * the spectra kernel and the finalize kernel of every later call).  phylino_last_kernel_ms waits for
+ * the last call to finish and returns its two durations in milliseconds (HOST pointers). */
+PHYLINO_API phylino_status phylino_set_timing(phylino_ctx *ctx, int on);
+PHYLINO_API phylino_status phylino_last_kernel_ms(phylino_ctx *ctx, float *spectra_ms, float *finalize_ms);
+
+/* Kernel launches enqueued by this context so far (bench.py's `gpu_launches`). */
+PHYLINO_API int64_t phylino_launch_count(const phylino_ctx *ctx);
+
+/* Text of the last error of this context ("" if none).  Valid until the next call on ctx. */
+PHYLINO_API const char *phylino_last_error(const phylino_ctx *ctx);
+
+/* Microbenchmark of the pipe that bounds the batched path: issues
+ * `iters` dependent-chain DFMA per thread over a full-chip grid on the context's stream and
+ * returns the achieved fp64 FMA instructions per second (lane-operations/s) in *dfma_per_s. */
+PHYLINO_API phylino_status phylino_peak_fp64(phylino_ctx *ctx, int iters, double *dfma_per_s_host);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PHYLINO_H */

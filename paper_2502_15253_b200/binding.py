@@ -1,0 +1,317 @@
+"""ctypes binding of include/phylino.h.  Argument marshalling only.
+
+PyTorch is used for what the caller hands in and gets back (device tensors, the current CUDA
+stream); nothing here computes.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional, Sequence
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "libphylino.so")
+
+# every symbol include/phylino.h declares
+abi_symbols = (
+    "phylino_create", "phylino_destroy", "phylino_set_model", "phylino_load_events",
+    "phylino_spectra", "phylino_nll", "phylino_event_bins", "phylino_nll_host",
+    "phylino_spectra_host", "phylino_total_bins", "phylino_total_events",
+    "phylino_set_point_chunk", "phylino_launch_count", "phylino_last_error", "phylino_peak_fp64",
+    "phylino_expectation", "phylino_set_timing", "phylino_last_kernel_ms",
+)
+
+_STATUS = {0: "OK", 1: "ERR_ARG", 2: "ERR_SHAPE", 3: "ERR_STATE", 4: "ERR_OOM", 5: "ERR_CUDA"}
+
+
+class PhylinoError(RuntimeError):
+    def __init__(self, status: int, text: str):
+        super().__init__(f"phylino: {_STATUS.get(status, status)}: {text}")
+        self.status = status
+
+
+class _Bkg(C.Structure):
+    _fields_ = [("idx_rate", C.c_int32), ("tmpl", C.c_void_p), ("idx_shape", C.c_void_p)]
+
+
+class _Dataset(C.Structure):
+    _fields_ = [("n_bins", C.c_int32), ("idx_a", C.c_int32 * 3), ("idx_signorm", C.c_int32),
+                ("norm", C.c_double), ("idx_flux", C.c_void_p), ("n_bkg", C.c_int32),
+                ("bkg", C.POINTER(_Bkg))]
+
+
+class _Model(C.Structure):
+    _fields_ = [("osc_model", C.c_int32), ("ordering", C.c_int32), ("n_params", C.c_int32),
+                ("n_datasets", C.c_int32), ("idx_osc", C.c_int32 * 6), ("fixed_osc", C.c_double * 6),
+                ("datasets", C.POINTER(_Dataset)), ("prior_mean", C.c_void_p),
+                ("prior_sigma", C.c_void_p)]
+
+
+_lib = None
+
+
+def lib_path() -> str:
+    return _LIB_PATH
+
+
+def load_library():
+    """dlopen libphylino.so.  Fails loudly if it has not been built (no fallback of any kind)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(_LIB_PATH):
+        raise RuntimeError(
+            f"{_LIB_PATH} is missing: build it with `python -m paper_2502_15253_b200.build` "
+            "(nvcc, sm_100a).  There is no CPU or PyTorch fallback for this path.")
+    lib = C.CDLL(_LIB_PATH)
+    vp, i32, i64, dbl = C.c_void_p, C.c_int, C.c_int64, C.c_double
+    lib.phylino_create.restype = i32
+    lib.phylino_create.argtypes = [i32, vp, C.POINTER(vp)]
+    lib.phylino_destroy.restype = None
+    lib.phylino_destroy.argtypes = [vp]
+    lib.phylino_set_model.restype = i32
+    lib.phylino_set_model.argtypes = [vp, C.POINTER(_Model)]
+    lib.phylino_load_events.restype = i32
+    lib.phylino_load_events.argtypes = [vp, i32, i64, vp, vp, vp, vp, i32, vp, i32, vp]
+    lib.phylino_spectra.restype = i32
+    lib.phylino_spectra.argtypes = [vp, i32, vp, vp]
+    lib.phylino_nll.restype = i32
+    lib.phylino_nll.argtypes = [vp, i32, vp, vp, vp]
+    lib.phylino_expectation.restype = i32
+    lib.phylino_expectation.argtypes = [vp, i32, vp, vp]
+    lib.phylino_set_timing.restype = i32
+    lib.phylino_set_timing.argtypes = [vp, i32]
+    lib.phylino_last_kernel_ms.restype = i32
+    lib.phylino_last_kernel_ms.argtypes = [vp, C.POINTER(C.c_float), C.POINTER(C.c_float)]
+    lib.phylino_event_bins.restype = i32
+    lib.phylino_event_bins.argtypes = [vp, i32, vp, vp]
+    lib.phylino_nll_host.restype = i32
+    lib.phylino_nll_host.argtypes = [vp, i32, vp, vp, vp]
+    lib.phylino_spectra_host.restype = i32
+    lib.phylino_spectra_host.argtypes = [vp, i32, vp, vp]
+    lib.phylino_total_bins.restype = i64
+    lib.phylino_total_bins.argtypes = [vp]
+    lib.phylino_total_events.restype = i64
+    lib.phylino_total_events.argtypes = [vp]
+    lib.phylino_set_point_chunk.restype = i32
+    lib.phylino_set_point_chunk.argtypes = [vp, i32]
+    lib.phylino_launch_count.restype = i64
+    lib.phylino_launch_count.argtypes = [vp]
+    lib.phylino_last_error.restype = C.c_char_p
+    lib.phylino_last_error.argtypes = [vp]
+    lib.phylino_peak_fp64.restype = i32
+    lib.phylino_peak_fp64.argtypes = [vp, i32, C.POINTER(dbl)]
+    _lib = lib
+    return lib
+
+
+def _np_ptr(a: Optional[np.ndarray]):
+    return None if a is None else a.ctypes.data
+
+
+class Phylino:
+    """One fit context (phylino_ctx).  Method names follow the C entry points.
+
+    `model` / `events` are `workloads.ModelSpec` / `workloads.DatasetEvents`-shaped objects (plain
+    attribute containers); device-side arguments are float64 CUDA tensors.
+    """
+
+    def __init__(self, device: int = 0, stream: Optional[int] = None):
+        import torch
+        self._torch = torch
+        self._lib = load_library()
+        if not torch.cuda.is_available():
+            raise PhylinoError(5, "no CUDA device: this path has no CPU fallback")
+        self.device = int(device)
+        if stream is None:
+            stream = torch.cuda.current_stream(self.device).cuda_stream
+        self._ctx = C.c_void_p()
+        st = self._lib.phylino_create(self.device, C.c_void_p(stream), C.byref(self._ctx))
+        if st != 0:
+            raise PhylinoError(st, "phylino_create failed")
+        self.n_params = 0
+
+    # -- plumbing ------------------------------------------------------------------------------
+    def _check(self, st: int):
+        if st != 0:
+            raise PhylinoError(st, self._lib.phylino_last_error(self._ctx).decode())
+
+    def close(self):
+        if getattr(self, "_ctx", None) is not None and self._ctx:
+            self._lib.phylino_destroy(self._ctx)
+            self._ctx = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    def _dev_params(self, params):
+        t = self._torch
+        if not (isinstance(params, t.Tensor) and params.is_cuda and params.dtype == t.float64
+                and params.is_contiguous() and params.device.index == self.device):
+            raise TypeError("params must be a contiguous float64 CUDA tensor on the context's device")
+        if params.dim() != 2 or params.shape[1] != self.n_params:
+            raise ValueError(f"params must be [P, {self.n_params}], got {tuple(params.shape)}")
+        return params
+
+    # -- phylino_set_model ---------------------------------------------------------------------
+    def set_model(self, model):
+        keep = []
+
+        def arr(a, dt):
+            a = np.ascontiguousarray(a, dtype=dt)
+            keep.append(a)
+            return a.ctypes.data
+
+        n_ds = len(model.datasets)
+        ds_arr = (_Dataset * n_ds)()
+        for d, ds in enumerate(model.datasets):
+            bk_arr = (_Bkg * max(1, len(ds.bkg)))()
+            for k, bk in enumerate(ds.bkg):
+                bk_arr[k].idx_rate = int(bk.idx_rate)
+                bk_arr[k].tmpl = arr(bk.tmpl, np.float64)
+                bk_arr[k].idx_shape = None if bk.idx_shape is None else arr(bk.idx_shape, np.int32)
+            keep.append(bk_arr)
+            ds_arr[d].n_bins = int(ds.n_bins)
+            ds_arr[d].idx_a = (C.c_int32 * 3)(*[int(i) for i in ds.idx_a])
+            ds_arr[d].idx_signorm = int(ds.idx_signorm)
+            ds_arr[d].norm = float(ds.norm)
+            ds_arr[d].idx_flux = None if ds.idx_flux is None else arr(ds.idx_flux, np.int32)
+            ds_arr[d].n_bkg = len(ds.bkg)
+            ds_arr[d].bkg = C.cast(bk_arr, C.POINTER(_Bkg))
+        m = _Model()
+        m.osc_model = int(model.osc_model)
+        m.ordering = int(model.ordering)
+        m.n_params = int(model.n_params)
+        m.n_datasets = n_ds
+        m.idx_osc = (C.c_int32 * 6)(*[int(i) for i in model.idx_osc])
+        m.fixed_osc = (C.c_double * 6)(*[float(x) for x in model.fixed_osc])
+        m.datasets = C.cast(ds_arr, C.POINTER(_Dataset))
+        m.prior_mean = None if model.prior_mean is None else arr(model.prior_mean, np.float64)
+        m.prior_sigma = None if model.prior_sigma is None else arr(model.prior_sigma, np.float64)
+        self._check(self._lib.phylino_set_model(self._ctx, C.byref(m)))
+        self.n_params = int(model.n_params)
+        del keep
+
+    # -- phylino_load_events -------------------------------------------------------------------
+    def load_events(self, dataset: int, e_nu, e_vis, weight, core, baseline_m, edges):
+        e_nu = np.ascontiguousarray(e_nu, dtype=np.float32)
+        e_vis = np.ascontiguousarray(e_vis, dtype=np.float32)
+        w = None if weight is None else np.ascontiguousarray(weight, dtype=np.float32)
+        c = None if core is None else np.ascontiguousarray(core, dtype=np.int32)
+        L = np.ascontiguousarray(baseline_m, dtype=np.float64)
+        ed = np.ascontiguousarray(edges, dtype=np.float64)
+        if e_vis.shape != e_nu.shape or (w is not None and w.shape != e_nu.shape) \
+                or (c is not None and c.shape != e_nu.shape):
+            raise ValueError("event arrays must have the same length")
+        self._check(self._lib.phylino_load_events(
+            self._ctx, int(dataset), int(e_nu.shape[0]), _np_ptr(e_nu), _np_ptr(e_vis), _np_ptr(w),
+            _np_ptr(c), int(L.shape[0]), _np_ptr(L), int(ed.shape[0] - 1), _np_ptr(ed)))
+
+    def load_workload(self, wl):
+        """set_model + load_events for every dataset of a `workloads.Workload`."""
+        self.set_model(wl.model)
+        for d, e in enumerate(wl.events):
+            self.load_events(d, e.e_nu, e.e_vis, e.w, e.core, e.L_m, e.edges)
+
+    # -- sizes ---------------------------------------------------------------------------------
+    @property
+    def total_bins(self) -> int:
+        return int(self._lib.phylino_total_bins(self._ctx))
+
+    @property
+    def total_events(self) -> int:
+        return int(self._lib.phylino_total_events(self._ctx))
+
+    @property
+    def launch_count(self) -> int:
+        return int(self._lib.phylino_launch_count(self._ctx))
+
+    def set_point_chunk(self, points_per_cta: int):
+        self._check(self._lib.phylino_set_point_chunk(self._ctx, int(points_per_cta)))
+
+    # -- phylino_spectra / phylino_nll / phylino_event_bins (device buffers, asynchronous) -------
+    def spectra(self, params, out=None):
+        t = self._torch
+        p = self._dev_params(params)
+        if out is None:
+            out = t.empty((p.shape[0], self.total_bins), dtype=t.float64, device=p.device)
+        assert out.is_cuda and out.dtype == t.float64 and out.is_contiguous() \
+            and out.numel() == p.shape[0] * self.total_bins
+        self._check(self._lib.phylino_spectra(self._ctx, int(p.shape[0]), p.data_ptr(), out.data_ptr()))
+        return out
+
+    def nll(self, params, data, out=None):
+        t = self._torch
+        p = self._dev_params(params)
+        if not (isinstance(data, t.Tensor) and data.is_cuda and data.dtype == t.float64
+                and data.is_contiguous() and data.numel() == self.total_bins):
+            raise TypeError(f"data must be a contiguous float64 CUDA tensor of {self.total_bins} counts")
+        if out is None:
+            out = t.empty((p.shape[0],), dtype=t.float64, device=p.device)
+        assert out.is_cuda and out.dtype == t.float64 and out.is_contiguous() and out.numel() == p.shape[0]
+        self._check(self._lib.phylino_nll(self._ctx, int(p.shape[0]), p.data_ptr(), data.data_ptr(),
+                                          out.data_ptr()))
+        return out
+
+    def expectation(self, params, out=None):
+        t = self._torch
+        p = self._dev_params(params)
+        if out is None:
+            out = t.empty((p.shape[0], self.total_bins), dtype=t.float64, device=p.device)
+        assert out.is_cuda and out.dtype == t.float64 and out.is_contiguous() \
+            and out.numel() == p.shape[0] * self.total_bins
+        self._check(self._lib.phylino_expectation(self._ctx, int(p.shape[0]), p.data_ptr(), out.data_ptr()))
+        return out
+
+    def set_timing(self, on: bool = True):
+        self._check(self._lib.phylino_set_timing(self._ctx, int(bool(on))))
+
+    def last_kernel_ms(self):
+        """(spectra kernel ms, finalize kernel ms) of the last call; waits for it to finish."""
+        a, b = C.c_float(0.0), C.c_float(0.0)
+        self._check(self._lib.phylino_last_kernel_ms(self._ctx, C.byref(a), C.byref(b)))
+        return float(a.value), float(b.value)
+
+    def event_bins(self, params):
+        t = self._torch
+        p = self._dev_params(params)
+        out = t.empty((p.shape[0], self.total_events), dtype=t.int32, device=p.device)
+        self._check(self._lib.phylino_event_bins(self._ctx, int(p.shape[0]), p.data_ptr(), out.data_ptr()))
+        return out
+
+    # -- host-buffer entry points (synchronous, copies inside) ---------------------------------
+    def nll_host(self, params: np.ndarray, data: np.ndarray, out: Optional[np.ndarray] = None) -> np.ndarray:
+        p = np.ascontiguousarray(params, dtype=np.float64)
+        d = np.ascontiguousarray(data, dtype=np.float64)
+        if p.ndim != 2 or p.shape[1] != self.n_params or d.shape != (self.total_bins,):
+            raise ValueError("bad shapes")
+        if out is None:
+            out = np.empty(p.shape[0], dtype=np.float64)
+        self._check(self._lib.phylino_nll_host(self._ctx, int(p.shape[0]), p.ctypes.data, d.ctypes.data,
+                                               out.ctypes.data))
+        return out
+
+    def spectra_host(self, params: np.ndarray, out: Optional[np.ndarray] = None) -> np.ndarray:
+        p = np.ascontiguousarray(params, dtype=np.float64)
+        if p.ndim != 2 or p.shape[1] != self.n_params:
+            raise ValueError("bad shapes")
+        if out is None:
+            out = np.empty((p.shape[0], self.total_bins), dtype=np.float64)
+        self._check(self._lib.phylino_spectra_host(self._ctx, int(p.shape[0]), p.ctypes.data, out.ctypes.data))
+        return out
+
+    def peak_fp64(self, iters: int = 4096) -> float:
+        v = C.c_double(0.0)
+        self._check(self._lib.phylino_peak_fp64(self._ctx, int(iters), C.byref(v)))
+        return float(v.value)

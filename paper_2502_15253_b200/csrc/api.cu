@@ -1,0 +1,559 @@
+/*
+ * api.cu -- the C-ABI of include/phylino.h: context, model tables, event store, launches.
+ * Host logic only; the arithmetic of the path lives in spectra.cu / finalize.cu.
+ */
+#include <algorithm>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <numeric>
+
+#include "internal.h"
+
+using namespace phylino;
+
+namespace {
+
+struct DeviceGuard {
+    int prev = -1;
+    bool ok = true;
+    explicit DeviceGuard(int dev)
+    {
+        if (cudaGetDevice(&prev) != cudaSuccess) { prev = -1; ok = false; return; }
+        if (prev != dev && cudaSetDevice(dev) != cudaSuccess) ok = false;
+    }
+    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+
+phylino_status fail(phylino_ctx *c, phylino_status s, const char *fmt, ...)
+{
+    char buf[512];
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(buf, sizeof buf, fmt, ap);
+    va_end(ap);
+    if (c) c->err = buf;
+    return s;
+}
+
+phylino_status cuda_fail(phylino_ctx *c, cudaError_t e, const char *what)
+{
+    cudaGetLastError();     /* clear the sticky-less error state */
+    return fail(c, e == cudaErrorMemoryAllocation ? PHYLINO_ERR_OOM : PHYLINO_ERR_CUDA, "%s: %s", what,
+                cudaGetErrorString(e));
+}
+
+#define CU(call)                                                    \
+    do {                                                            \
+        cudaError_t e_ = (call);                                    \
+        if (e_ != cudaSuccess) return cuda_fail(ctx, e_, #call);    \
+    } while (0)
+
+template <class T> cudaError_t upload(T **dst, const std::vector<T> &src, cudaStream_t st)
+{
+    *dst = nullptr;
+    size_t n = std::max<size_t>(src.size(), 1);
+    cudaError_t e = cudaMalloc((void **)dst, n * sizeof(T));
+    if (e != cudaSuccess) return e;
+    if (!src.empty()) e = cudaMemcpyAsync(*dst, src.data(), src.size() * sizeof(T), cudaMemcpyHostToDevice, st);
+    return e;
+}
+
+void free_events(phylino_dataset_host &d)
+{
+    cudaFree(d.d_x); cudaFree(d.d_v); cudaFree(d.d_w); cudaFree(d.d_edges); cudaFree(d.d_perm);
+    d.d_x = nullptr; d.d_v = nullptr; d.d_w = nullptr; d.d_edges = nullptr; d.d_perm = nullptr;
+    d.loaded = false; d.n = d.n_pad = 0;
+}
+
+void free_tables(phylino_ctx *c)
+{
+    FinalizeArgs &f = c->fin;
+    cudaFree((void *)f.bin_ds); cudaFree((void *)f.idx_flux); cudaFree((void *)f.inv_scale);
+    cudaFree((void *)f.norm); cudaFree((void *)f.idx_signorm); cudaFree((void *)f.n_bkg);
+    cudaFree((void *)f.idx_rate); cudaFree((void *)f.idx_shape); cudaFree((void *)f.tmpl);
+    cudaFree((void *)f.prior_mean); cudaFree((void *)f.prior_sigma);
+    f = FinalizeArgs{};
+}
+
+void free_all(phylino_ctx *c)
+{
+    for (auto &d : c->ds) free_events(d);
+    c->ds.clear();
+    free_tables(c);
+    cudaFree(c->d_acc); cudaFree(c->d_flags);
+    c->d_acc = nullptr; c->d_flags = nullptr; c->acc_capacity = 0;
+    cudaFree(c->d_stage); c->d_stage = nullptr;
+    if (c->h_pin) cudaFreeHost(c->h_pin);
+    c->h_pin = nullptr; c->stage_capacity = 0;
+    c->have_model = false;
+}
+
+void free_events_timing(phylino_ctx *c)
+{
+    for (auto &e : c->ev) { if (e) cudaEventDestroy(e); e = nullptr; }
+    c->timing = false;
+}
+
+bool idx_ok(int32_t i, int32_t n) { return i >= -1 && i < n; }
+
+phylino_status check_ready(phylino_ctx *ctx, int P, const void *params, const void *out)
+{
+    if (!ctx) return PHYLINO_ERR_ARG;
+    if (!ctx->have_model) return fail(ctx, PHYLINO_ERR_STATE, "phylino_set_model has not been called");
+    for (int d = 0; d < ctx->n_datasets; ++d)
+        if (!ctx->ds[d].loaded) return fail(ctx, PHYLINO_ERR_STATE, "dataset %d has no events loaded", d);
+    if (P < 0) return fail(ctx, PHYLINO_ERR_SHAPE, "P = %d is negative", P);
+    if ((int64_t)P * ctx->total_bins > (int64_t)1 << 40) return fail(ctx, PHYLINO_ERR_SHAPE, "P x total_bins too large");
+    if (P > 0 && (!params || !out)) return fail(ctx, PHYLINO_ERR_ARG, "NULL params or output pointer");
+    return PHYLINO_OK;
+}
+
+phylino_status ensure_acc(phylino_ctx *ctx, int P)
+{
+    int64_t need = (int64_t)P * ctx->total_bins;
+    if (need <= ctx->acc_capacity) return PHYLINO_OK;
+    /* the stream may still use the old buffers */
+    CU(cudaStreamSynchronize(ctx->stream));
+    cudaFree(ctx->d_acc); cudaFree(ctx->d_flags);
+    ctx->d_acc = nullptr; ctx->d_flags = nullptr; ctx->acc_capacity = 0;
+    CU(cudaMalloc((void **)&ctx->d_acc, need * sizeof(long long)));
+    CU(cudaMalloc((void **)&ctx->d_flags, need * sizeof(unsigned)));
+    CU(cudaMemsetAsync(ctx->d_acc, 0, need * sizeof(long long), ctx->stream));
+    CU(cudaMemsetAsync(ctx->d_flags, 0, need * sizeof(unsigned), ctx->stream));
+    ctx->acc_capacity = need;
+    return PHYLINO_OK;
+}
+
+int default_points_per_cta(const phylino_ctx *ctx, int P)
+{
+    if (ctx->points_per_cta > 0) return std::min(ctx->points_per_cta, std::max(P, 1));
+    return std::min(P, 16);
+}
+
+/* enqueue the spectra kernel (rows a1-a4) for P points */
+phylino_status enqueue_spectra(phylino_ctx *ctx, int P, const double *params)
+{
+    SpectraArgs a{};
+    int tiles = 0;
+    for (int d = 0; d < ctx->n_datasets; ++d) {
+        const phylino_dataset_host &h = ctx->ds[d];
+        DatasetDev &v = a.ds[d];
+        v.x = h.d_x; v.v = h.d_v; v.w = h.d_w; v.edges = h.d_edges;
+        v.n_bins = h.n_bins;
+        v.bin_off = d == 0 ? 0 : a.ds[d - 1].bin_off + a.ds[d - 1].n_bins;
+        v.tile_begin = tiles;
+        for (int j = 0; j < 3; ++j) v.idx_a[j] = h.idx_a[j];
+        v.fx_scale = std::ldexp(1.0, h.fx_exp);
+        tiles += (int)(h.n_pad / EV_PER_CTA);
+    }
+    /* empty datasets own no tile: make sure the lookup in the kernel skips them */
+    a.osc.osc_model = ctx->osc_model;
+    a.osc.ordering = ctx->ordering;
+    for (int j = 0; j < 6; ++j) { a.osc.idx_osc[j] = ctx->idx_osc[j]; a.osc.fixed_osc[j] = ctx->fixed_osc[j]; }
+    a.n_datasets = ctx->n_datasets;
+    a.n_params = ctx->n_params;
+    a.P = P;
+    a.points_per_cta = default_points_per_cta(ctx, P);
+    a.total_bins = ctx->total_bins;
+    a.params = params;
+    a.acc = ctx->d_acc;
+    a.flags = ctx->d_flags;
+    if (ctx->timing) CU(cudaEventRecord(ctx->ev[0], ctx->stream));
+    if (tiles > 0 && P > 0) {
+        CU(launch_spectra(a, tiles, ctx->n_terms, ctx->per_point_binning, ctx->max_bins, ctx->stream));
+        ctx->launches += 1;
+    }
+    return PHYLINO_OK;
+}
+
+phylino_status enqueue_finalize(phylino_ctx *ctx, int P, const double *params, const double *data,
+                                double *hist, double *nll, int mode = -1)
+{
+    if (mode < 0) mode = nll ? 2 : 0;
+    FinalizeArgs f = ctx->fin;
+    f.P = P;
+    f.params = params;
+    f.acc = ctx->d_acc;
+    f.flags = ctx->d_flags;
+    f.data = data;
+    f.hist = hist;
+    f.nll = nll;
+    if (ctx->timing) CU(cudaEventRecord(ctx->ev[1], ctx->stream));
+    CU(launch_finalize(f, mode, ctx->stream));
+    ctx->launches += 1;
+    if (ctx->timing) CU(cudaEventRecord(ctx->ev[2], ctx->stream));
+    return PHYLINO_OK;
+}
+
+phylino_status ensure_stage(phylino_ctx *ctx, int64_t doubles)
+{
+    if (doubles <= ctx->stage_capacity) return PHYLINO_OK;
+    CU(cudaStreamSynchronize(ctx->stream));
+    cudaFree(ctx->d_stage); ctx->d_stage = nullptr;
+    if (ctx->h_pin) cudaFreeHost(ctx->h_pin);
+    ctx->h_pin = nullptr; ctx->stage_capacity = 0;
+    CU(cudaMalloc((void **)&ctx->d_stage, doubles * sizeof(double)));
+    CU(cudaHostAlloc((void **)&ctx->h_pin, doubles * sizeof(double), cudaHostAllocDefault));
+    ctx->stage_capacity = doubles;
+    return PHYLINO_OK;
+}
+
+} // namespace
+
+extern "C" {
+
+phylino_status phylino_create(int device, void *cuda_stream, phylino_ctx **out)
+{
+    if (!out) return PHYLINO_ERR_ARG;
+    *out = nullptr;
+    int n = 0;
+    cudaError_t e = cudaGetDeviceCount(&n);
+    if (e != cudaSuccess || device < 0 || device >= n) { cudaGetLastError(); return PHYLINO_ERR_CUDA; }
+    phylino_ctx *c = new (std::nothrow) phylino_ctx;
+    if (!c) return PHYLINO_ERR_OOM;
+    c->device = device;
+    c->stream = (cudaStream_t)cuda_stream;
+    DeviceGuard g(device);
+    if (!g.ok || cudaFree(0) != cudaSuccess) { cudaGetLastError(); delete c; return PHYLINO_ERR_CUDA; }
+    *out = c;
+    return PHYLINO_OK;
+}
+
+void phylino_destroy(phylino_ctx *ctx)
+{
+    if (!ctx) return;
+    DeviceGuard g(ctx->device);
+    cudaStreamSynchronize(ctx->stream);
+    free_all(ctx);
+    free_events_timing(ctx);
+    delete ctx;
+}
+
+phylino_status phylino_set_model(phylino_ctx *ctx, const phylino_model_desc *m)
+{
+    if (!ctx) return PHYLINO_ERR_ARG;
+    if (!m || !m->datasets) return fail(ctx, PHYLINO_ERR_ARG, "NULL model");
+    if (m->osc_model < PHYLINO_OSC_EQ1 || m->osc_model > PHYLINO_OSC_STERILE4)
+        return fail(ctx, PHYLINO_ERR_ARG, "unknown osc_model %d", m->osc_model);
+    if (m->n_params < 0) return fail(ctx, PHYLINO_ERR_SHAPE, "n_params = %d", m->n_params);
+    if (m->n_datasets < 1 || m->n_datasets > PHYLINO_MAX_DATASETS)
+        return fail(ctx, PHYLINO_ERR_SHAPE, "n_datasets = %d not in 1..%d", m->n_datasets, PHYLINO_MAX_DATASETS);
+    const int n_used_osc = m->osc_model == PHYLINO_OSC_STERILE4 ? 6 : 4;
+    for (int j = 0; j < n_used_osc; ++j)
+        if (!idx_ok(m->idx_osc[j], m->n_params)) return fail(ctx, PHYLINO_ERR_SHAPE, "idx_osc[%d] = %d out of range", j, m->idx_osc[j]);
+    int64_t tb = 0;
+    int max_bkg = 0, max_bins = 0;
+    bool perpoint = false;
+    for (int d = 0; d < m->n_datasets; ++d) {
+        const phylino_dataset_desc &s = m->datasets[d];
+        if (s.n_bins < 1 || s.n_bins > PHYLINO_MAX_BINS)
+            return fail(ctx, PHYLINO_ERR_SHAPE, "dataset %d: n_bins = %d not in 1..%d", d, s.n_bins, PHYLINO_MAX_BINS);
+        if (s.n_bkg < 0 || s.n_bkg > PHYLINO_MAX_BKG || (s.n_bkg > 0 && !s.bkg))
+            return fail(ctx, PHYLINO_ERR_SHAPE, "dataset %d: n_bkg = %d", d, s.n_bkg);
+        for (int j = 0; j < 3; ++j) {
+            if (!idx_ok(s.idx_a[j], m->n_params)) return fail(ctx, PHYLINO_ERR_SHAPE, "dataset %d: idx_a[%d] out of range", d, j);
+            perpoint |= s.idx_a[j] >= 0;
+        }
+        if (!idx_ok(s.idx_signorm, m->n_params)) return fail(ctx, PHYLINO_ERR_SHAPE, "dataset %d: idx_signorm out of range", d);
+        if (s.idx_flux)
+            for (int b = 0; b < s.n_bins; ++b)
+                if (!idx_ok(s.idx_flux[b], m->n_params)) return fail(ctx, PHYLINO_ERR_SHAPE, "dataset %d: idx_flux[%d] out of range", d, b);
+        for (int k = 0; k < s.n_bkg; ++k) {
+            const phylino_bkg_desc &bk = s.bkg[k];
+            if (!bk.tmpl) return fail(ctx, PHYLINO_ERR_ARG, "dataset %d bkg %d: NULL template", d, k);
+            if (!idx_ok(bk.idx_rate, m->n_params)) return fail(ctx, PHYLINO_ERR_SHAPE, "dataset %d bkg %d: idx_rate out of range", d, k);
+            if (bk.idx_shape)
+                for (int b = 0; b < s.n_bins; ++b)
+                    if (!idx_ok(bk.idx_shape[b], m->n_params)) return fail(ctx, PHYLINO_ERR_SHAPE, "dataset %d bkg %d: idx_shape[%d] out of range", d, k, b);
+        }
+        tb += s.n_bins;
+        max_bkg = std::max(max_bkg, s.n_bkg);
+        max_bins = std::max(max_bins, s.n_bins);
+    }
+
+    DeviceGuard g(ctx->device);
+    CU(cudaStreamSynchronize(ctx->stream));
+    free_all(ctx);
+
+    ctx->osc_model = m->osc_model;
+    ctx->ordering = m->ordering >= 0 ? 1 : -1;
+    ctx->n_params = m->n_params;
+    ctx->n_datasets = m->n_datasets;
+    ctx->n_terms = m->osc_model == PHYLINO_OSC_EQ1 ? 2 : 3;
+    for (int j = 0; j < 6; ++j) { ctx->idx_osc[j] = j < n_used_osc ? m->idx_osc[j] : -1; ctx->fixed_osc[j] = m->fixed_osc[j]; }
+    ctx->per_point_binning = perpoint;
+    ctx->total_bins = (int32_t)tb;
+    ctx->max_bkg = max_bkg;
+    ctx->max_bins = max_bins;
+    ctx->ds.resize(m->n_datasets);
+
+    std::vector<int32_t> bin_ds(tb), idx_flux(tb, -1), idx_signorm(m->n_datasets), n_bkg(m->n_datasets);
+    std::vector<int32_t> idx_rate((size_t)m->n_datasets * std::max(max_bkg, 1), -1);
+    std::vector<int32_t> idx_shape((size_t)std::max(max_bkg, 1) * tb, -1);
+    std::vector<double> tmpl((size_t)std::max(max_bkg, 1) * tb, 0.0), norm(m->n_datasets), inv_scale(m->n_datasets, 1.0);
+    int64_t off = 0;
+    for (int d = 0; d < m->n_datasets; ++d) {
+        const phylino_dataset_desc &s = m->datasets[d];
+        phylino_dataset_host &h = ctx->ds[d];
+        h.n_bins = s.n_bins;
+        for (int j = 0; j < 3; ++j) h.idx_a[j] = s.idx_a[j];
+        h.idx_signorm = s.idx_signorm;
+        h.norm = s.norm;
+        idx_signorm[d] = s.idx_signorm;
+        norm[d] = s.norm;
+        n_bkg[d] = s.n_bkg;
+        for (int b = 0; b < s.n_bins; ++b) {
+            bin_ds[off + b] = d;
+            if (s.idx_flux) idx_flux[off + b] = s.idx_flux[b];
+        }
+        for (int k = 0; k < s.n_bkg; ++k) {
+            const phylino_bkg_desc &bk = s.bkg[k];
+            idx_rate[(size_t)d * max_bkg + k] = bk.idx_rate;
+            for (int b = 0; b < s.n_bins; ++b) {
+                tmpl[(size_t)k * tb + off + b] = bk.tmpl[b];
+                if (bk.idx_shape) idx_shape[(size_t)k * tb + off + b] = bk.idx_shape[b];
+            }
+        }
+        off += s.n_bins;
+    }
+    FinalizeArgs &f = ctx->fin;
+    f.n_params = m->n_params;
+    f.total_bins = (int32_t)tb;
+    f.n_datasets = m->n_datasets;
+    f.max_bkg = max_bkg;
+    cudaStream_t st = ctx->stream;
+    CU(upload((int32_t **)&f.bin_ds, bin_ds, st));
+    CU(upload((int32_t **)&f.idx_flux, idx_flux, st));
+    CU(upload((double **)&f.inv_scale, inv_scale, st));
+    CU(upload((double **)&f.norm, norm, st));
+    CU(upload((int32_t **)&f.idx_signorm, idx_signorm, st));
+    CU(upload((int32_t **)&f.n_bkg, n_bkg, st));
+    CU(upload((int32_t **)&f.idx_rate, idx_rate, st));
+    CU(upload((int32_t **)&f.idx_shape, idx_shape, st));
+    CU(upload((double **)&f.tmpl, tmpl, st));
+    if (m->prior_mean && m->prior_sigma && m->n_params > 0) {
+        std::vector<double> pm(m->prior_mean, m->prior_mean + m->n_params);
+        std::vector<double> ps(m->prior_sigma, m->prior_sigma + m->n_params);
+        CU(upload((double **)&f.prior_mean, pm, st));
+        CU(upload((double **)&f.prior_sigma, ps, st));
+    }
+    CU(cudaStreamSynchronize(st));      /* the host vectors above die here */
+    ctx->have_model = true;
+    ctx->err.clear();
+    return PHYLINO_OK;
+}
+
+phylino_status phylino_load_events(phylino_ctx *ctx, int dataset, int64_t n, const float *e_nu,
+                                   const float *e_vis, const float *weight, const int32_t *core,
+                                   int n_cores, const double *baseline_m, int n_bins, const double *edges)
+{
+    if (!ctx) return PHYLINO_ERR_ARG;
+    if (!ctx->have_model) return fail(ctx, PHYLINO_ERR_STATE, "phylino_set_model must come before phylino_load_events");
+    if (dataset < 0 || dataset >= ctx->n_datasets) return fail(ctx, PHYLINO_ERR_SHAPE, "dataset %d not in 0..%d", dataset, ctx->n_datasets - 1);
+    phylino_dataset_host &h = ctx->ds[dataset];
+    if (n_bins != h.n_bins) return fail(ctx, PHYLINO_ERR_SHAPE, "dataset %d: n_bins = %d, model says %d", dataset, n_bins, h.n_bins);
+    if (n < 0 || n > 0x7fff0000ll) return fail(ctx, PHYLINO_ERR_SHAPE, "n = %lld out of range", (long long)n);
+    if (!edges || n_cores < 1 || !baseline_m || (n > 0 && (!e_nu || !e_vis)))
+        return fail(ctx, PHYLINO_ERR_ARG, "NULL array or n_cores < 1");
+    for (int b = 0; b <= n_bins; ++b)
+        if (!std::isfinite(edges[b]) || (b > 0 && !(edges[b] > edges[b - 1])))
+            return fail(ctx, PHYLINO_ERR_ARG, "edges must be finite and strictly ascending (at %d)", b);
+    for (int c = 0; c < n_cores; ++c)
+        if (!std::isfinite(baseline_m[c]) || baseline_m[c] < 0.0) return fail(ctx, PHYLINO_ERR_ARG, "baseline %d is not finite >= 0", c);
+    for (int64_t i = 0; i < n; ++i) {
+        if (!(e_nu[i] > 0.0f) || !std::isfinite(e_nu[i])) return fail(ctx, PHYLINO_ERR_ARG, "e_nu[%lld] is not finite > 0", (long long)i);
+        if (weight && !std::isfinite(weight[i])) return fail(ctx, PHYLINO_ERR_ARG, "weight[%lld] is not finite", (long long)i);
+        if (core && (core[i] < 0 || core[i] >= n_cores)) return fail(ctx, PHYLINO_ERR_ARG, "core[%lld] = %d out of range", (long long)i, core[i]);
+    }
+
+    /* sort by reconstructed energy (R14), NaN last, stable */
+    std::vector<int32_t> perm((size_t)n);
+    std::iota(perm.begin(), perm.end(), 0);
+    std::stable_sort(perm.begin(), perm.end(), [e_vis](int32_t a, int32_t b) {
+        float x = e_vis[a], y = e_vis[b];
+        if (x != x) return false;
+        if (y != y) return true;
+        return x < y;
+    });
+    const int64_t n_pad = (n + EV_PER_CTA - 1) / EV_PER_CTA * EV_PER_CTA;
+    std::vector<double> x((size_t)n_pad, 0.0);
+    std::vector<float> v((size_t)n_pad, std::nanf("")), w((size_t)n_pad, 0.0f);
+    double wsum = 0.0;
+    for (int64_t i = 0; i < n; ++i) {
+        int32_t s = perm[i];
+        x[i] = baseline_m[core ? core[s] : 0] / (double)e_nu[s];
+        v[i] = e_vis[s];
+        w[i] = weight ? weight[s] : 1.0f;
+        wsum += std::fabs((double)w[i]);
+    }
+    /* fixed-point scale 2^e with 8 * sum|w| * 2^e <= 2^62 (|P_ee| <= 4 is enforced per point) */
+    int ex = 0;
+    if (wsum > 0.0) std::frexp(wsum, &ex);
+    int fx = std::max(-1000, std::min(1000, 59 - ex));
+
+    DeviceGuard g(ctx->device);
+    CU(cudaStreamSynchronize(ctx->stream));
+    free_events(h);
+    cudaStream_t st = ctx->stream;
+    std::vector<double> ed(edges, edges + n_bins + 1);
+    CU(upload(&h.d_x, x, st));
+    CU(upload(&h.d_v, v, st));
+    CU(upload(&h.d_w, w, st));
+    CU(upload(&h.d_edges, ed, st));
+    CU(upload(&h.d_perm, perm, st));
+    double inv = std::ldexp(1.0, -fx);
+    CU(cudaMemcpyAsync((void *)(ctx->fin.inv_scale + dataset), &inv, sizeof(double), cudaMemcpyHostToDevice, st));
+    CU(cudaStreamSynchronize(st));
+    h.n = n; h.n_pad = n_pad; h.wsum_abs = wsum; h.fx_exp = fx; h.loaded = true;
+    ctx->err.clear();
+    return PHYLINO_OK;
+}
+
+phylino_status phylino_spectra(phylino_ctx *ctx, int P, const double *params, double *hist)
+{
+    phylino_status s = check_ready(ctx, P, params, hist);
+    if (s != PHYLINO_OK || P == 0) return s;
+    DeviceGuard g(ctx->device);
+    if ((s = ensure_acc(ctx, P)) != PHYLINO_OK) return s;
+    if ((s = enqueue_spectra(ctx, P, params)) != PHYLINO_OK) return s;
+    return enqueue_finalize(ctx, P, params, nullptr, hist, nullptr);
+}
+
+phylino_status phylino_nll(phylino_ctx *ctx, int P, const double *params, const double *data, double *nll)
+{
+    phylino_status s = check_ready(ctx, P, params, nll);
+    if (s != PHYLINO_OK || P == 0) return s;
+    if (!data) return fail(ctx, PHYLINO_ERR_ARG, "NULL data pointer");
+    DeviceGuard g(ctx->device);
+    if ((s = ensure_acc(ctx, P)) != PHYLINO_OK) return s;
+    if ((s = enqueue_spectra(ctx, P, params)) != PHYLINO_OK) return s;
+    return enqueue_finalize(ctx, P, params, data, nullptr, nll);
+}
+
+phylino_status phylino_expectation(phylino_ctx *ctx, int P, const double *params, double *mu)
+{
+    phylino_status s = check_ready(ctx, P, params, mu);
+    if (s != PHYLINO_OK || P == 0) return s;
+    DeviceGuard g(ctx->device);
+    if ((s = ensure_acc(ctx, P)) != PHYLINO_OK) return s;
+    if ((s = enqueue_spectra(ctx, P, params)) != PHYLINO_OK) return s;
+    return enqueue_finalize(ctx, P, params, nullptr, mu, nullptr, 1);
+}
+
+phylino_status phylino_event_bins(phylino_ctx *ctx, int P, const double *params, int32_t *bins)
+{
+    phylino_status s = check_ready(ctx, P, params, bins);
+    if (s != PHYLINO_OK || P == 0) return s;
+    DeviceGuard g(ctx->device);
+    int64_t total = phylino_total_events(ctx), off = 0, boff = 0;
+    for (int d = 0; d < ctx->n_datasets; ++d) {
+        const phylino_dataset_host &h = ctx->ds[d];
+        EventBinsArgs a{};
+        a.ds.v = h.d_v; a.ds.edges = h.d_edges; a.ds.n_bins = h.n_bins; a.ds.bin_off = (int32_t)boff;
+        for (int j = 0; j < 3; ++j) a.ds.idx_a[j] = h.idx_a[j];
+        a.perm = h.d_perm; a.n = h.n; a.ev_off = off; a.total_events = total;
+        a.P = P; a.n_params = ctx->n_params; a.params = params; a.bins = bins;
+        if (h.n > 0) {
+            CU(launch_event_bins(a, ctx->stream));
+            ctx->launches += 1;
+        }
+        off += h.n;
+        boff += h.n_bins;
+    }
+    return PHYLINO_OK;
+}
+
+phylino_status phylino_nll_host(phylino_ctx *ctx, int P, const double *params_host, const double *data_host,
+                                double *nll_host)
+{
+    phylino_status s = check_ready(ctx, P, params_host, nll_host);
+    if (s != PHYLINO_OK || P == 0) return s;
+    if (!data_host) return fail(ctx, PHYLINO_ERR_ARG, "NULL data pointer");
+    DeviceGuard g(ctx->device);
+    const int64_t np = (int64_t)P * ctx->n_params, tb = ctx->total_bins;
+    if ((s = ensure_stage(ctx, np + tb + P)) != PHYLINO_OK) return s;
+    if ((s = ensure_acc(ctx, P)) != PHYLINO_OK) return s;
+    std::memcpy(ctx->h_pin, params_host, np * sizeof(double));
+    std::memcpy(ctx->h_pin + np, data_host, tb * sizeof(double));
+    CU(cudaMemcpyAsync(ctx->d_stage, ctx->h_pin, (np + tb) * sizeof(double), cudaMemcpyHostToDevice, ctx->stream));
+    if ((s = enqueue_spectra(ctx, P, ctx->d_stage)) != PHYLINO_OK) return s;
+    if ((s = enqueue_finalize(ctx, P, ctx->d_stage, ctx->d_stage + np, nullptr, ctx->d_stage + np + tb)) != PHYLINO_OK) return s;
+    CU(cudaMemcpyAsync(ctx->h_pin + np + tb, ctx->d_stage + np + tb, P * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    std::memcpy(nll_host, ctx->h_pin + np + tb, P * sizeof(double));
+    return PHYLINO_OK;
+}
+
+phylino_status phylino_spectra_host(phylino_ctx *ctx, int P, const double *params_host, double *hist_host)
+{
+    phylino_status s = check_ready(ctx, P, params_host, hist_host);
+    if (s != PHYLINO_OK || P == 0) return s;
+    DeviceGuard g(ctx->device);
+    const int64_t np = (int64_t)P * ctx->n_params, nh = (int64_t)P * ctx->total_bins;
+    if ((s = ensure_stage(ctx, np + nh)) != PHYLINO_OK) return s;
+    if ((s = ensure_acc(ctx, P)) != PHYLINO_OK) return s;
+    std::memcpy(ctx->h_pin, params_host, np * sizeof(double));
+    CU(cudaMemcpyAsync(ctx->d_stage, ctx->h_pin, np * sizeof(double), cudaMemcpyHostToDevice, ctx->stream));
+    if ((s = enqueue_spectra(ctx, P, ctx->d_stage)) != PHYLINO_OK) return s;
+    if ((s = enqueue_finalize(ctx, P, ctx->d_stage, nullptr, ctx->d_stage + np, nullptr)) != PHYLINO_OK) return s;
+    CU(cudaMemcpyAsync(ctx->h_pin + np, ctx->d_stage + np, nh * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    std::memcpy(hist_host, ctx->h_pin + np, nh * sizeof(double));
+    return PHYLINO_OK;
+}
+
+int64_t phylino_total_bins(const phylino_ctx *ctx) { return ctx && ctx->have_model ? ctx->total_bins : 0; }
+
+int64_t phylino_total_events(const phylino_ctx *ctx)
+{
+    int64_t t = 0;
+    if (ctx) for (const auto &d : ctx->ds) if (d.loaded) t += d.n;
+    return t;
+}
+
+phylino_status phylino_set_point_chunk(phylino_ctx *ctx, int points_per_cta)
+{
+    if (!ctx) return PHYLINO_ERR_ARG;
+    if (points_per_cta < 0 || points_per_cta > CTA_THREADS) return fail(ctx, PHYLINO_ERR_ARG, "points_per_cta = %d not in 0..%d", points_per_cta, CTA_THREADS);
+    ctx->points_per_cta = points_per_cta;
+    return PHYLINO_OK;
+}
+
+phylino_status phylino_set_timing(phylino_ctx *ctx, int on)
+{
+    if (!ctx) return PHYLINO_ERR_ARG;
+    DeviceGuard g(ctx->device);
+    if (on && !ctx->ev[0])
+        for (auto &e : ctx->ev) CU(cudaEventCreate(&e));
+    ctx->timing = on != 0;
+    return PHYLINO_OK;
+}
+
+phylino_status phylino_last_kernel_ms(phylino_ctx *ctx, float *spectra_ms, float *finalize_ms)
+{
+    if (!ctx || !spectra_ms || !finalize_ms) return PHYLINO_ERR_ARG;
+    if (!ctx->timing) return fail(ctx, PHYLINO_ERR_STATE, "phylino_set_timing(ctx, 1) has not been called");
+    DeviceGuard g(ctx->device);
+    CU(cudaEventSynchronize(ctx->ev[2]));
+    CU(cudaEventElapsedTime(spectra_ms, ctx->ev[0], ctx->ev[1]));
+    CU(cudaEventElapsedTime(finalize_ms, ctx->ev[1], ctx->ev[2]));
+    return PHYLINO_OK;
+}
+
+int64_t phylino_launch_count(const phylino_ctx *ctx) { return ctx ? ctx->launches : 0; }
+
+const char *phylino_last_error(const phylino_ctx *ctx) { return ctx ? ctx->err.c_str() : ""; }
+
+phylino_status phylino_peak_fp64(phylino_ctx *ctx, int iters, double *dfma_per_s_host)
+{
+    if (!ctx || !dfma_per_s_host || iters < 1) return PHYLINO_ERR_ARG;
+    DeviceGuard g(ctx->device);
+    CU(run_peak_fp64(iters, ctx->stream, dfma_per_s_host));
+    ctx->launches += 2;
+    return PHYLINO_OK;
+}
+
+} // extern "C"

@@ -1,0 +1,111 @@
+/*
+ * devmath.cuh -- device arithmetic of the hot path: oscillation terms, sin^2 of the phase,
+ * energy-scale map, bin search.  Compiled with -fmad=false: every fused multiply-add below is
+ * written as fma() on purpose, nothing else is contracted (bit-exact bin assignment, R8).
+ */
+#ifndef PHYLINO_DEVMATH_CUH
+#define PHYLINO_DEVMATH_CUH
+
+#include "internal.h"
+
+namespace phylino {
+
+/* first-octant branch theta < pi/4 (R4): cos 2theta = +sqrt(1 - sin^2 2theta) */
+__device__ __forceinline__ void mixing(double s22, double &cos2, double &sin2, double &cos4)
+{
+    double c2t = sqrt(1.0 - s22);
+    cos2 = (1.0 + c2t) / 2.0;
+    sin2 = (1.0 - c2t) / 2.0;
+    cos4 = cos2 * cos2;
+}
+
+__device__ __forceinline__ double osc_par(const OscDev &o, const double *theta, int slot)
+{
+    int idx = o.idx_osc[slot];
+    return idx >= 0 ? theta[idx] : o.fixed_osc[slot];
+}
+
+/* Amplitudes A_k and mass splittings dm2_k [eV^2] of the S oscillation terms at one point.
+ *   EQ1      PAPER.md:34 Eq. 1
+ *   FULL3    exact 3-flavour vacuum P_ee; |dm2_31|, |dm2_32| from inverting PAPER.md:39 Eq. 2 (R2, R5)
+ *   STERILE4 BASELINE.json config 5 (PAPER.md:199 prints none; R15) */
+__device__ __forceinline__ void osc_terms(const OscDev &o, const double *theta, double A[MAX_TERMS],
+                                          double dm2[MAX_TERMS])
+{
+    double s13 = osc_par(o, theta, PHYLINO_S13), mee = osc_par(o, theta, PHYLINO_MEE);
+    double s12 = osc_par(o, theta, PHYLINO_S12), m21 = osc_par(o, theta, PHYLINO_M21);
+    double c2_13, s2_13, c4_13, c2_12, s2_12, c4_12;
+    mixing(s13, c2_13, s2_13, c4_13);
+    mixing(s12, c2_12, s2_12, c4_12);
+    if (o.osc_model == PHYLINO_OSC_EQ1) {
+        A[0] = s13;          dm2[0] = mee;
+        A[1] = c4_13 * s12;  dm2[1] = m21;
+        A[2] = 0.0;          dm2[2] = 0.0;
+    } else if (o.osc_model == PHYLINO_OSC_FULL3) {
+        double sgn = o.ordering >= 0 ? 1.0 : -1.0;
+        A[0] = c4_13 * s12;  dm2[0] = m21;
+        A[1] = s13 * c2_12;  dm2[1] = mee + sgn * s2_12 * m21;
+        A[2] = s13 * s2_12;  dm2[2] = mee - sgn * c2_12 * m21;
+    } else {
+        double s14 = osc_par(o, theta, PHYLINO_S14), m41 = osc_par(o, theta, PHYLINO_M41);
+        double c2_14, s2_14, c4_14;
+        mixing(s14, c2_14, s2_14, c4_14);
+        A[0] = c4_14 * s13;  dm2[0] = mee;
+        A[1] = s14;          dm2[1] = m41;
+        A[2] = c4_13 * s12;  dm2[2] = m21;
+    }
+}
+
+/* Phase in half-turns per unit x = L/E:  phase = 1.267 dm2 x  (R1)  =  (pi/2) (h x),
+ * h = 1.267 dm2 (2/pi). */
+__device__ __forceinline__ double halfturn_coeff(double dm2)
+{
+    return (1.267 * dm2) * 0.63661977236758134308;   /* 2/pi */
+}
+
+/* sin^2((pi/2) h x), |h x| < 2^51.
+ *   n = rint(h x) by the 1.5*2^52 trick, f = h x - n in [-1/2, 1/2] with ONE rounding (fma), so the
+ *   range reduction is exact for phases of thousands of radians (config 5: 7.8e3 rad);
+ *   q = sin^2((pi/2) f) = z Q(z), z = f^2: degree-5 minimax Q, |error| <= 4.1e-13 absolute
+ *   (Remez fit made for this file);
+ *   n odd  =>  sin^2 = 1 - q.  Parity, sign flip and the constant are integer-pipe work.
+ * 11 fp64 instructions including the final A-weighted update done by the caller. */
+__device__ __forceinline__ double sin2_halfturns(double h, double x)
+{
+    const double MAGIC = 6755399441055744.0;        /* 1.5 * 2^52 */
+    double t = fma(h, x, MAGIC);
+    double n = t - MAGIC;
+    double f = fma(h, x, -n);
+    double z = f * f;
+    double q = -0x1.e2a4cab0973aep-11;
+    q = fma(q, z,  0x1.a65598e5b8576p-7);
+    q = fma(q, z, -0x1.e1f273f3e9df0p-4);
+    q = fma(q, z,  0x1.55d3c0fdef250p-1);
+    q = fma(q, z, -0x1.03c1f070b1413p+1);
+    q = fma(q, z,  0x1.3bd3cc9bac6fep+1);
+    unsigned odd = (unsigned)__double2loint(t) & 1u;
+    double sz   = __hiloint2double(__double2hiint(z) ^ (int)(odd << 31), __double2loint(z));
+    double oddf = __hiloint2double((int)(odd * 0x3FF00000u), 0);
+    return fma(sz, q, oddf);
+}
+
+/* E' = fma(fma(a2, v, a1), v, a0): the normative rounding sequence of the energy-scale map (R8). */
+__device__ __forceinline__ double escale(double a0, double a1, double a2, double v)
+{
+    return fma(fma(a2, v, a1), v, a0);
+}
+
+/* Half-open bins [edges[b], edges[b+1]): largest b with edges[b] <= e; -1 outside or NaN (R7). */
+__device__ __forceinline__ int bin_search(const double *edges, int n_bins, double e)
+{
+    if (!(e >= edges[0]) || !(e < edges[n_bins])) return -1;
+    int lo = 0, hi = n_bins;
+    while (hi - lo > 1) {
+        int mid = (lo + hi) >> 1;
+        if (edges[mid] <= e) lo = mid; else hi = mid;
+    }
+    return lo;
+}
+
+} // namespace phylino
+#endif

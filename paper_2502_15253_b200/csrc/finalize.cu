@@ -1,0 +1,109 @@
+/*
+ * finalize.cu -- SURVEY.md 8(a) rows a5-a7: fixed-point accumulators -> fp64 spectra, expectation
+ * assembly, and the Poisson half-deviance + Gaussian-prior reduction.
+ *
+ *   mu[p,d,b] = eps_d norm_d f_db H[p,d,b] + sum_k r_dk s_dkb T_dkb
+ *   nll[p]    = sum_{d,b} dev(n, mu) + 1/2 sum_j ((theta_j - mean_j)/sigma_j)^2
+ *   dev(n,mu) = mu - n + n ln(n/mu)   (Eq. 3 over the saturated model of :96 Eq. 8; R9, R10)
+ *
+ * One CTA per parameter point.  Every thread sums a fixed strided subset of the bins and of the
+ * priors, the warps combine by a fixed shuffle tree and warp 0 adds the warp totals in index
+ * order: the result is bitwise reproducible.  The kernel re-zeroes the accumulators it reads so
+ * the next call needs no memset launch.
+ */
+#include "internal.h"
+
+namespace phylino {
+
+namespace {
+
+constexpr int FIN_THREADS = 128;
+
+__device__ __forceinline__ double half_deviance(double n, double mu)
+{
+    if (n != n || mu != mu) return __longlong_as_double(0x7ff8000000000000ll);
+    if (mu < 0.0) return __longlong_as_double(0x7ff0000000000000ll);
+    if (n > 0.0) {
+        if (mu == 0.0) return __longlong_as_double(0x7ff0000000000000ll);
+        return mu - n + n * log(n / mu);
+    }
+    if (n == 0.0) return mu;
+    return __longlong_as_double(0x7ff8000000000000ll);     /* negative counts are not data */
+}
+
+template <int MODE>   /* 0 = spectra H, 1 = expectation mu, 2 = NLL */
+__global__ void __launch_bounds__(FIN_THREADS) finalize_kernel(const __grid_constant__ FinalizeArgs a)
+{
+    const int p = blockIdx.x;
+    const double *theta = a.params + (size_t)p * a.n_params;
+    const size_t row = (size_t)p * a.total_bins;
+    double part = 0.0;
+
+    for (int g = threadIdx.x; g < a.total_bins; g += FIN_THREADS) {
+        long long q = a.acc[row + g];
+        unsigned fl = a.flags[row + g];
+        if (q) a.acc[row + g] = 0;
+        if (fl) a.flags[row + g] = 0;
+        const int d = a.bin_ds[g];
+        double H = (double)q * a.inv_scale[d];              /* 2^-e: exact scaling */
+        if (fl) {
+            if ((fl & FLAG_NAN) || ((fl & FLAG_PINF) && (fl & FLAG_NINF)))
+                H = __longlong_as_double(0x7ff8000000000000ll);
+            else
+                H = __longlong_as_double((fl & FLAG_PINF) ? 0x7ff0000000000000ll : 0xfff0000000000000ll);
+        }
+        if (MODE == 0) {
+            a.hist[row + g] = H;
+        } else {
+            double eps = a.idx_signorm[d] >= 0 ? theta[a.idx_signorm[d]] : 1.0;
+            double f = a.idx_flux[g] >= 0 ? theta[a.idx_flux[g]] : 1.0;
+            double mu = eps * a.norm[d] * f * H;
+            const int nb = a.n_bkg[d];
+            for (int k = 0; k < nb; ++k) {
+                int ir = a.idx_rate[d * a.max_bkg + k];
+                int is = a.idx_shape[(size_t)k * a.total_bins + g];
+                double r = ir >= 0 ? theta[ir] : 1.0;
+                double s = is >= 0 ? theta[is] : 1.0;
+                mu += r * s * a.tmpl[(size_t)k * a.total_bins + g];
+            }
+            if (MODE == 1) a.hist[row + g] = mu;
+            else part += half_deviance(a.data[g], mu);
+        }
+    }
+    if (MODE != 2) return;
+
+    if (a.prior_mean && a.prior_sigma) {
+        /* uncorrelated Gaussian priors (Eq. 6), constants dropped (R9) */
+        for (int j = threadIdx.x; j < a.n_params; j += FIN_THREADS) {
+            double sg = a.prior_sigma[j];
+            if (!(sg > 0.0) || sg > 1.79769313486231570e308) continue;
+            double z = (theta[j] - a.prior_mean[j]) / sg;
+            part += 0.5 * z * z;
+        }
+    }
+
+    __shared__ double wsum[FIN_THREADS / 32];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) part += __shfl_xor_sync(0xffffffffu, part, o);
+    if ((threadIdx.x & 31) == 0) wsum[threadIdx.x >> 5] = part;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double s = 0.0;
+#pragma unroll
+        for (int i = 0; i < FIN_THREADS / 32; ++i) s += wsum[i];
+        a.nll[p] = s;
+    }
+}
+
+} // namespace
+
+cudaError_t launch_finalize(const FinalizeArgs &a, int mode, cudaStream_t st)
+{
+    if (a.P <= 0) return cudaSuccess;
+    if (mode == 2)      finalize_kernel<2><<<a.P, FIN_THREADS, 0, st>>>(a);
+    else if (mode == 1) finalize_kernel<1><<<a.P, FIN_THREADS, 0, st>>>(a);
+    else                finalize_kernel<0><<<a.P, FIN_THREADS, 0, st>>>(a);
+    return cudaGetLastError();
+}
+
+} // namespace phylino

@@ -1,0 +1,152 @@
+/*
+ * internal.h -- host/device structures shared by the translation units of libphylino.so.
+ * Not part of the ABI (include/phylino.h is); private to the CUDA path.
+ */
+#ifndef PHYLINO_INTERNAL_H
+#define PHYLINO_INTERNAL_H
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <string>
+#include <vector>
+
+#include "phylino.h"
+
+namespace phylino {
+
+/* ---- tiling of the event store --------------------------------------------------------------
+ * One CTA owns EV_PER_CTA consecutive (E_vis-sorted) events of ONE dataset and walks a chunk of
+ * parameter points over them; thread t keeps events [t*K, t*K+K) of the tile in registers. */
+constexpr int K_EV       = 8;                       /* events per thread */
+constexpr int CTA_THREADS = 256;
+constexpr int EV_PER_CTA = K_EV * CTA_THREADS;      /* 2048; every dataset is padded to a multiple */
+constexpr int MAX_TERMS  = 3;
+
+/* flag bits of a (point, bin) accumulator whose value left the fixed-point domain */
+enum : unsigned { FLAG_NAN = 1u, FLAG_PINF = 2u, FLAG_NINF = 4u };
+
+/* Per-dataset entry of the table that travels by value in the kernel parameters. */
+struct DatasetDev {
+    const double *x;        /* [n_pad] L_core/E_nu  [m/MeV], fp64 (phase range reduction needs it) */
+    const float  *v;        /* [n_pad] E_vis [MeV]; padding = NaN */
+    const float  *w;        /* [n_pad] MC weight;   padding = 0   */
+    const double *edges;    /* [n_bins+1] */
+    int32_t n_bins;
+    int32_t bin_off;        /* offset of this dataset inside a point's total_bins */
+    int32_t tile_begin;     /* first CTA tile (blockIdx.x) of this dataset */
+    int32_t idx_a[3];       /* energy-scale indices into theta, -1 => (0,1,0) */
+    double  fx_scale;       /* 2^e: fixed-point scale of the bin accumulators */
+};
+
+struct OscDev {
+    int32_t osc_model, ordering;
+    int32_t idx_osc[6];
+    double  fixed_osc[6];
+};
+
+struct SpectraArgs {
+    DatasetDev ds[PHYLINO_MAX_DATASETS];
+    OscDev  osc;
+    int32_t n_datasets;
+    int32_t n_params;
+    int32_t P;              /* points in the batch */
+    int32_t points_per_cta;
+    int32_t total_bins;
+    const double *params;   /* DEVICE [P x n_params] */
+    long long    *acc;      /* DEVICE [P x total_bins] fixed-point accumulators (zero on entry) */
+    unsigned     *flags;    /* DEVICE [P x total_bins] FLAG_* (zero on entry) */
+};
+
+/* Model tables of the expectation / NLL stage, all DEVICE pointers. */
+struct FinalizeArgs {
+    int32_t P, n_params, total_bins, n_datasets, max_bkg;
+    const double  *params;        /* [P x n_params] */
+    long long     *acc;           /* [P x total_bins]; re-zeroed by the kernel */
+    unsigned      *flags;         /* [P x total_bins]; re-zeroed by the kernel */
+    const int32_t *bin_ds;        /* [total_bins] dataset of a global bin */
+    const int32_t *idx_flux;      /* [total_bins] */
+    const double  *inv_scale;     /* [n_datasets] 2^-e */
+    const double  *norm;          /* [n_datasets] */
+    const int32_t *idx_signorm;   /* [n_datasets] */
+    const int32_t *n_bkg;         /* [n_datasets] */
+    const int32_t *idx_rate;      /* [n_datasets x max_bkg] */
+    const int32_t *idx_shape;     /* [max_bkg x total_bins] */
+    const double  *tmpl;          /* [max_bkg x total_bins] */
+    const double  *prior_mean;    /* [n_params] or NULL */
+    const double  *prior_sigma;   /* [n_params] or NULL */
+    const double  *data;          /* [total_bins] (NLL mode) */
+    double        *hist;          /* [P x total_bins] (spectra / expectation mode) */
+    double        *nll;           /* [P] (NLL mode) */
+};
+
+struct EventBinsArgs {
+    DatasetDev ds;
+    const int32_t *perm;          /* [n] sorted position -> caller's index */
+    int64_t n;                    /* real events of the dataset */
+    int64_t ev_off;               /* offset of this dataset in the concatenated caller order */
+    int64_t total_events;
+    int32_t P, n_params;
+    const double *params;
+    int32_t *bins;
+};
+
+/* kernel launchers (spectra.cu, finalize.cu, peaks.cu) */
+cudaError_t launch_spectra(const SpectraArgs &a, int n_tiles, int S, bool per_point_binning,
+                           int max_bins, cudaStream_t st);
+cudaError_t launch_finalize(const FinalizeArgs &a, int mode /*0 H, 1 mu, 2 nll*/, cudaStream_t st);
+cudaError_t launch_event_bins(const EventBinsArgs &a, cudaStream_t st);
+cudaError_t run_peak_fp64(int iters, cudaStream_t st, double *dfma_per_s);
+
+} // namespace phylino
+
+/* ---- host-side context ---------------------------------------------------------------------- */
+struct phylino_dataset_host {
+    /* model */
+    int32_t n_bins = 0;
+    int32_t idx_a[3] = {-1, -1, -1};
+    int32_t idx_signorm = -1;
+    double  norm = 1.0;
+    std::vector<int32_t> idx_flux;                 /* empty => all -1 */
+    struct Bkg { int32_t idx_rate; std::vector<double> tmpl; std::vector<int32_t> idx_shape; };
+    std::vector<Bkg> bkg;
+    /* events */
+    bool     loaded = false;
+    int64_t  n = 0, n_pad = 0;
+    double   wsum_abs = 0.0;
+    int      fx_exp = 0;
+    double  *d_x = nullptr;
+    float   *d_v = nullptr, *d_w = nullptr;
+    double  *d_edges = nullptr;
+    int32_t *d_perm = nullptr;
+};
+
+struct phylino_ctx {
+    int device = 0;
+    cudaStream_t stream = nullptr;
+    std::string err;
+    bool have_model = false;
+    int32_t osc_model = 0, ordering = 1, n_params = 0, n_datasets = 0, n_terms = 2;
+    int32_t idx_osc[6] = {-1, -1, -1, -1, -1, -1};
+    double  fixed_osc[6] = {0, 0, 0, 0, 0, 0};
+    bool    per_point_binning = false;
+    int32_t total_bins = 0, max_bkg = 0, max_bins = 0;
+    std::vector<phylino_dataset_host> ds;
+    /* device model tables */
+    void *d_tables = nullptr;                      /* one allocation, carved up below */
+    phylino::FinalizeArgs fin{};                   /* table pointers filled by set_model */
+    /* accumulators */
+    int64_t   acc_capacity = 0;                    /* in (point, bin) cells */
+    long long *d_acc = nullptr;
+    unsigned  *d_flags = nullptr;
+    /* host-buffer entry points: pinned + device staging */
+    double *h_pin = nullptr, *d_stage = nullptr;
+    int64_t stage_capacity = 0;                    /* doubles */
+    int points_per_cta = 0;
+    /* optional device timing of the two kernels of a call (phylino_set_timing) */
+    bool timing = false;
+    cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};
+    int64_t launches = 0;
+};
+
+#endif

@@ -1,0 +1,331 @@
+"""-m gpu: the CUDA path (through the C-ABI binding) against the CPU oracle on the same seeded inputs.
+
+Tolerances are north_star's: bin assignment bit-exact, per-bin relative error <= 1e-7,
+NLL absolute error <= 1e-6."""
+import numpy as np
+import pytest
+
+import workloads
+from workloads.spec import OSC_EQ1, OSC_FULL3, OSC_STERILE4
+
+pytestmark = pytest.mark.gpu
+
+REL_BIN = 1e-7
+ABS_NLL = 1e-6
+
+
+def _dev(a):
+    import torch
+    return torch.as_tensor(np.ascontiguousarray(a, dtype=np.float64), device="cuda")
+
+
+def _data_for(orc, wl, oracle_mod):
+    """Pseudo-data n ~ Poisson(mu(theta0)) with mu from the ORACLE (never from the CUDA path)."""
+    h0 = orc.spectra(wl.theta0[None, :])
+    mu0 = orc.expectation(wl.theta0[None, :], h0)[0]
+    return workloads.poisson_counts(mu0, wl.seed + 7)
+
+
+def _check_hist(h_gpu, h_orc):
+    assert h_gpu.shape == h_orc.shape
+    zero = h_orc == 0.0
+    assert np.array_equal(h_gpu[zero], h_orc[zero])              # empty bins are exactly empty
+    rel = np.abs(h_gpu[~zero] - h_orc[~zero]) / np.abs(h_orc[~zero])
+    assert rel.size == 0 or rel.max() <= REL_BIN, rel.max()
+    return 0.0 if rel.size == 0 else float(rel.max())
+
+
+def _run_case(gpu, oracle_mod, wl, check_bins=True, points=None, ppc=None):
+    import torch
+    params = wl.params if points is None else wl.params[points]
+    orc = oracle_mod.Oracle(wl.model, wl.events)
+    data = _data_for(orc, wl, oracle_mod)
+    with gpu.Phylino() as ph:
+        ph.load_workload(wl)
+        if ppc:
+            ph.set_point_chunk(ppc)
+        dp = _dev(params)
+        h = ph.spectra(dp).cpu().numpy()
+        nll = ph.nll(dp, _dev(data)).cpu().numpy()
+        bins = ph.event_bins(dp).cpu().numpy() if check_bins else None
+        torch.cuda.synchronize()
+    h_o = orc.spectra(params)
+    nll_o = orc.nll(params, data)
+    rel = _check_hist(h, h_o)
+    fin = np.isfinite(nll_o)
+    assert np.array_equal(np.isfinite(nll), fin)
+    assert np.array_equal(nll[~fin], nll_o[~fin], equal_nan=True)
+    err = np.abs(nll[fin] - nll_o[fin]).max() if fin.any() else 0.0
+    assert err <= ABS_NLL, err
+    if check_bins:
+        assert np.array_equal(bins, orc.event_bins(params))       # bit-exact bin assignment
+    return rel, err
+
+
+@pytest.mark.parametrize("osc", [OSC_EQ1, OSC_FULL3, OSC_STERILE4])
+@pytest.mark.parametrize("n_datasets", [1, 3])
+def test_tiny_inputs(gpu, oracle_mod, osc, n_datasets):
+    wl = workloads.make_tiny(seed=40 + osc, osc_model=osc, n_events=100, n_points=5, n_datasets=n_datasets)
+    _run_case(gpu, oracle_mod, wl)
+
+
+# scaled-down copies of the five BASELINE.json configs: several CTA tiles (2048 events) per dataset
+# and a ragged tail, a point count that is not a multiple of the point chunk
+@pytest.mark.parametrize("k,scale,n_points", [(1, 0.137, 3), (2, 0.0123, 19), (3, 0.0051, 41),
+                                               (4, 0.00217, 9), (5, 0.0097, 37)])
+def test_configs_scaled(gpu, oracle_mod, k, scale, n_points):
+    wl = workloads.make_config(k, scale=scale, n_points=n_points)
+    _run_case(gpu, oracle_mod, wl)
+
+
+def test_config1_full(gpu, oracle_mod):
+    _run_case(gpu, oracle_mod, workloads.make_config(1))
+
+
+# full BASELINE.json sizes in the launch configuration bench.py times (default point chunk),
+# checked on sampled points the oracle can compute one by one
+@pytest.mark.parametrize("k,n_sample", [(2, 6), (3, 6), (4, 3), (5, 6)])
+def test_configs_full_size_sampled_points(gpu, oracle_mod, k, n_sample):
+    import torch
+    wl = workloads.make_config(k)
+    P = wl.n_points
+    rng = np.random.Generator(np.random.PCG64(99 + k))
+    pts = np.unique(np.concatenate([[0, P - 1], rng.integers(0, P, n_sample)]))
+    if k == 3:
+        pts = np.unique(np.concatenate([pts, np.arange(0, 27)[::5]]))   # oscillation / energy-scale shifts
+    orc = oracle_mod.Oracle(wl.model, wl.events)
+    data = _data_for(orc, wl, oracle_mod)
+    with gpu.Phylino() as ph:
+        ph.load_workload(wl)
+        dp = _dev(wl.params)
+        h = ph.spectra(dp)[torch.as_tensor(pts, device="cuda")].cpu().numpy()
+        nll = ph.nll(dp, _dev(data)).cpu().numpy()
+    h_o = orc.spectra(wl.params[pts])
+    nll_o = orc.nll(wl.params[pts], data)
+    _check_hist(h, h_o)
+    assert np.abs(nll[pts] - nll_o).max() <= ABS_NLL, np.abs(nll[pts] - nll_o).max()
+    # properties that hold at any size: every point finite, NLL >= 0 (half-deviance + priors)
+    assert np.isfinite(nll).all() and (nll >= 0).all()
+
+
+def test_bitwise_reproducible_and_chunk_independent(gpu, oracle_mod):
+    import torch
+    wl = workloads.make_config(2, scale=0.02, n_points=23)
+    orc = oracle_mod.Oracle(wl.model, wl.events)
+    data = _dev(_data_for(orc, wl, oracle_mod))
+    dp = _dev(wl.params)
+    outs = []
+    with gpu.Phylino() as ph:
+        ph.load_workload(wl)
+        for ppc in (0, 0, 1, 5, 16, 23):
+            ph.set_point_chunk(ppc)
+            outs.append((ph.spectra(dp).cpu().numpy().tobytes(), ph.nll(dp, data).cpu().numpy().tobytes()))
+    torch.cuda.synchronize()
+    assert all(o == outs[0] for o in outs[1:])
+    # a second context on a permuted copy of the events gives the same bits: the fixed-point
+    # accumulators do not depend on arrival order, the sort is by E_vis
+    wl2 = workloads.make_config(2, scale=0.02, n_points=23)
+    rng = np.random.Generator(np.random.PCG64(5))
+    for e in wl2.events:
+        perm = rng.permutation(e.n)
+        e.e_nu, e.e_vis, e.w, e.core = e.e_nu[perm], e.e_vis[perm], e.w[perm], e.core[perm]
+    with gpu.Phylino() as ph:
+        ph.load_workload(wl2)
+        h2 = ph.spectra(dp).cpu().numpy()
+    h1 = np.frombuffer(outs[0][0], dtype=np.float64).reshape(h2.shape)
+    # equal E_vis keys may be ordered differently inside a thread's run -> allow rounding-level difference
+    assert np.allclose(h1, h2, rtol=1e-13, atol=0)
+
+
+def test_host_entry_points_match_device_ones(gpu, oracle_mod):
+    wl = workloads.make_config(2, scale=0.01, n_points=7)
+    orc = oracle_mod.Oracle(wl.model, wl.events)
+    data = _data_for(orc, wl, oracle_mod)
+    with gpu.Phylino() as ph:
+        ph.load_workload(wl)
+        dp = _dev(wl.params)
+        h_d = ph.spectra(dp).cpu().numpy()
+        n_d = ph.nll(dp, _dev(data)).cpu().numpy()
+        h_h = ph.spectra_host(wl.params)
+        n_h = ph.nll_host(wl.params, data)
+        assert ph.launch_count == 8
+    assert h_d.tobytes() == h_h.tobytes() and n_d.tobytes() == n_h.tobytes()
+
+
+# ---- edge cases ------------------------------------------------------------------------------
+def _one_dataset_model(n_bins, osc=OSC_EQ1, idx_a=(-1, -1, -1), n_params=4):
+    from workloads.spec import DatasetSpec, ModelSpec
+    return ModelSpec(osc_model=osc, n_params=n_params, idx_osc=(0, 1, 2, 3, -1, -1), fixed_osc=(0,) * 6,
+                     datasets=[DatasetSpec(n_bins=n_bins, idx_a=idx_a)])
+
+
+THETA = np.array([[0.1, 2.5e-3, 0.85, 7.5e-5]])
+
+
+def _events(e_nu, e_vis, w, edges, L=(1050.0,), core=None):
+    from workloads.spec import DatasetEvents
+    n = len(e_nu)
+    return DatasetEvents(e_nu=np.asarray(e_nu, np.float32), e_vis=np.asarray(e_vis, np.float32),
+                         w=np.asarray(w, np.float32),
+                         core=np.zeros(n, np.int32) if core is None else np.asarray(core, np.int32),
+                         L_m=np.asarray(L, np.float64), edges=np.asarray(edges, np.float64))
+
+
+def _both(gpu, oracle_mod, model, evs, params, check_bins=True):
+    from workloads.spec import Workload
+    wl = Workload(name="edge", model=model, events=evs, params=np.asarray(params, np.float64),
+                  theta0=np.asarray(params[0], np.float64), seed=1)
+    orc = oracle_mod.Oracle(model, evs)
+    with gpu.Phylino() as ph:
+        ph.load_workload(wl)
+        dp = _dev(wl.params)
+        h = ph.spectra(dp).cpu().numpy()
+        b = ph.event_bins(dp).cpu().numpy() if (check_bins and wl.n_events) else None
+    h_o = orc.spectra(wl.params)
+    if b is not None:
+        assert np.array_equal(b, orc.event_bins(wl.params))
+    return h, h_o
+
+
+def test_empty_dataset_and_single_event(gpu, oracle_mod):
+    edges = np.linspace(1.0, 8.0, 8)
+    h, h_o = _both(gpu, oracle_mod, _one_dataset_model(7), [_events([], [], [], edges)], THETA, check_bins=False)
+    assert np.array_equal(h, np.zeros((1, 7))) and np.array_equal(h_o, h)
+    h, h_o = _both(gpu, oracle_mod, _one_dataset_model(7), [_events([3.5], [2.7], [1.25], edges)], THETA)
+    _check_hist(h, h_o)
+    assert np.count_nonzero(h) == 1
+
+
+def test_edges_underflow_overflow_nan(gpu, oracle_mod):
+    edges = np.array([1.0, 1.5, 2.25, 3.0, 3.5, 4.75, 6.0, 9.0])
+    below = np.nextafter(np.float32(1.0), np.float32(0.0))
+    e_vis = [1.0, below, 9.0, np.nextafter(np.float32(9.0), np.float32(0.0)), 2.25, 3.5, np.nan, -1.0, 50.0, 6.0]
+    n = len(e_vis)
+    h, h_o = _both(gpu, oracle_mod, _one_dataset_model(7), [_events([3.0 + 0.1 * i for i in range(n)], e_vis,
+                                                                     [1.0 + 0.01 * i for i in range(n)], edges)], THETA)
+    _check_hist(h, h_o)
+    # all events out of range
+    h, h_o = _both(gpu, oracle_mod, _one_dataset_model(7), [_events([3.0] * 5, [0.1, 0.2, 20.0, 30.0, np.nan],
+                                                                     [1.0] * 5, edges)], THETA)
+    assert np.array_equal(h, np.zeros((1, 7))) and np.array_equal(h_o, h)
+
+
+def test_energy_scale_moves_events_across_edges(gpu, oracle_mod):
+    """events sit exactly on edges; a0 shifts of +-1 ulp-scale and of one bin width."""
+    rng = np.random.Generator(np.random.PCG64(3))
+    edges = 1.0 + 0.25 * np.arange(30)
+    e_vis = np.concatenate([edges[:-1], edges[:-1] + 0.125, rng.uniform(0.5, 9.0, 3000)]).astype(np.float32)
+    n = len(e_vis)
+    evs = [_events(rng.uniform(2.0, 8.0, n), e_vis, rng.uniform(0.5, 1.5, n), edges, L=(400.0, 1100.0),
+                   core=rng.integers(0, 2, n))]
+    model = _one_dataset_model(29, idx_a=(4, 5, 6), n_params=7)
+    base = np.array([0.1, 2.5e-3, 0.85, 7.5e-5, 0.0, 1.0, 0.0])
+    pts = [base.copy() for _ in range(9)]
+    pts[1][4] = 0.25; pts[2][4] = -0.25; pts[3][4] = 1e-16; pts[4][4] = -1e-16
+    pts[5][5] = 1.0 + 2 ** -52; pts[6][5] = 1.0 - 2 ** -53; pts[7][6] = 1e-3; pts[8][5:7] = (-1.0, 0.3)
+    h, h_o = _both(gpu, oracle_mod, model, evs, np.array(pts))
+    _check_hist(h, h_o)
+
+
+def test_nan_and_unphysical_points_propagate(gpu, oracle_mod):
+    wl = workloads.make_tiny(seed=77, osc_model=OSC_EQ1, n_events=100, n_points=6)
+    wl.params[1, 0] = np.nan           # sin^2 2theta13 = NaN
+    wl.params[2, 2] = 1.5              # sin^2 2theta12 > 1: sqrt of a negative
+    wl.params[3, 1] = np.nan           # dm2_ee = NaN
+    wl.params[4, 6] = np.nan           # a0 = NaN: every event of dataset 0 leaves the histogram
+    orc = oracle_mod.Oracle(wl.model, wl.events)
+    data = _data_for(orc, wl, oracle_mod)
+    with gpu.Phylino() as ph:
+        ph.load_workload(wl)
+        dp = _dev(wl.params)
+        h = ph.spectra(dp).cpu().numpy()
+        nll = ph.nll(dp, _dev(data)).cpu().numpy()
+        # the accumulators were left clean: a following good batch is unaffected
+        good = workloads.make_tiny(seed=77, osc_model=OSC_EQ1, n_events=100, n_points=6).params
+        h2 = ph.spectra(_dev(good)).cpu().numpy()
+    h_o = orc.spectra(wl.params)
+    assert np.array_equal(np.isnan(h), np.isnan(h_o))
+    ok = ~np.isnan(h_o)
+    _check_hist(h[ok], h_o[ok])
+    nll_o = orc.nll(wl.params, data)
+    assert np.array_equal(np.isnan(nll), np.isnan(nll_o))
+    fin = np.isfinite(nll_o)
+    assert np.abs(nll[fin] - nll_o[fin]).max() <= ABS_NLL
+    _check_hist(h2, orc.spectra(good))
+
+
+def test_zero_count_and_zero_mu_bins(gpu, oracle_mod):
+    wl = workloads.make_tiny(seed=78, osc_model=OSC_EQ1, n_events=60, n_points=3)
+    orc = oracle_mod.Oracle(wl.model, wl.events)
+    data = _data_for(orc, wl, oracle_mod)
+    data[::2] = 0.0
+    with gpu.Phylino() as ph:
+        ph.load_workload(wl)
+        nll = ph.nll(_dev(wl.params), _dev(data)).cpu().numpy()
+    assert np.abs(nll - orc.nll(wl.params, data)).max() <= ABS_NLL
+    # no backgrounds + an empty bin with observed counts -> mu = 0, n > 0 -> +inf on both sides
+    edges = np.linspace(1.0, 8.0, 8)
+    model = _one_dataset_model(7)
+    evs = [_events([3.5, 4.0], [2.7, 2.8], [1.0, 1.0], edges)]
+    orc = oracle_mod.Oracle(model, evs)
+    d = np.array([0, 2, 0, 0, 3, 0, 0], dtype=np.float64)
+    from workloads.spec import Workload
+    with gpu.Phylino() as ph:
+        ph.load_workload(Workload("z", model, evs, THETA, THETA[0], 1))
+        nll = ph.nll(_dev(THETA), _dev(d)).cpu().numpy()
+    assert np.isposinf(nll).all() and np.isposinf(orc.nll(THETA, d)).all()
+
+
+def test_eighteen_datasets_and_odd_bin_counts(gpu, oracle_mod):
+    """splitting gives 18 histograms; bin counts that are not multiples of 32."""
+    from workloads.spec import DatasetSpec, ModelSpec, Workload
+    rng = np.random.Generator(np.random.PCG64(18))
+    D = 18
+    evs, dss = [], []
+    for d in range(D):
+        B = 5 + 3 * d
+        edges = np.sort(rng.uniform(0.8, 9.5, B + 1))
+        edges[0], edges[-1] = 0.8, 9.5
+        evs.append(workloads.reactor_events(rng, 300 + 411 * d, [355.0, 469.0, 1050.0], [0.3, 0.3, 0.4], 0.08,
+                                            edges, weights="uniform"))
+        dss.append(DatasetSpec(n_bins=B, idx_a=(4 + 3 * (d % 2), 5 + 3 * (d % 2), 6 + 3 * (d % 2)), norm=0.5))
+    model = ModelSpec(osc_model=OSC_EQ1, n_params=10, idx_osc=(0, 1, 2, 3, -1, -1), fixed_osc=(0,) * 6, datasets=dss)
+    base = np.array([0.1, 2.5e-3, 0.85, 7.5e-5, 0.0, 1.0, 0.0, 0.01, 0.99, 0.001])
+    params = base[None, :] + rng.standard_normal((11, 10)) * np.array([0.01, 5e-5, 0.02, 2e-6, .02, .01, .001, .02, .01, .001])
+    h, h_o = _both(gpu, oracle_mod, model, evs, params)
+    _check_hist(h, h_o)
+
+
+def test_error_reporting(gpu):
+    import torch
+    wl = workloads.make_tiny(seed=5, n_events=10, n_points=2, n_datasets=2)
+    with gpu.Phylino() as ph:
+        dp = _dev(wl.params)
+        with pytest.raises(gpu.PhylinoError) as e:
+            ph.load_events(0, wl.events[0].e_nu, wl.events[0].e_vis, None, None, [1000.0], wl.events[0].edges)
+        assert e.value.status == 3                                   # ERR_STATE: no model
+        ph.set_model(wl.model)
+        ph.load_events(0, wl.events[0].e_nu, wl.events[0].e_vis, None, None, [1000.0], wl.events[0].edges)
+        out = torch.empty((2, ph.total_bins), dtype=torch.float64, device="cuda")
+        with pytest.raises(gpu.PhylinoError) as e:
+            ph.spectra(dp, out)
+        assert e.value.status == 3 and "dataset 1" in str(e.value)    # dataset 1 not loaded
+        with pytest.raises(gpu.PhylinoError) as e:
+            ph.load_events(1, wl.events[1].e_nu, wl.events[1].e_vis, None, None, [1000.0], wl.events[1].edges[:-1])
+        assert e.value.status == 2                                   # ERR_SHAPE: n_bins
+        with pytest.raises(gpu.PhylinoError) as e:
+            ph.load_events(5, wl.events[1].e_nu, wl.events[1].e_vis, None, None, [1000.0], wl.events[1].edges)
+        assert e.value.status == 2
+        bad = wl.events[1].e_nu.copy(); bad[3] = -1.0
+        with pytest.raises(gpu.PhylinoError) as e:
+            ph.load_events(1, bad, wl.events[1].e_vis, None, None, [1000.0], wl.events[1].edges)
+        assert e.value.status == 1                                   # ERR_ARG
+        with pytest.raises(gpu.PhylinoError) as e:
+            ph.load_events(1, wl.events[1].e_nu, wl.events[1].e_vis, None, None, [1000.0], wl.events[1].edges[::-1])
+        assert e.value.status == 1
+
+
+def test_peak_fp64_microbenchmark_runs(gpu):
+    with gpu.Phylino() as ph:
+        r = ph.peak_fp64(2048)
+    assert 1e12 < r < 1e14
