@@ -127,16 +127,9 @@ phylino_status ensure_acc(phylino_ctx *ctx, int P)
     return PHYLINO_OK;
 }
 
-int default_points_per_cta(const phylino_ctx *ctx, int P)
+/* fill the by-value kernel arguments that do not depend on the batch */
+int fill_datasets(const phylino_ctx *ctx, SpectraArgs &a)
 {
-    if (ctx->points_per_cta > 0) return std::min(ctx->points_per_cta, std::max(P, 1));
-    return std::min(P, 16);
-}
-
-/* enqueue the spectra kernel (rows a1-a4) for P points */
-phylino_status enqueue_spectra(phylino_ctx *ctx, int P, const double *params)
-{
-    SpectraArgs a{};
     int tiles = 0;
     for (int d = 0; d < ctx->n_datasets; ++d) {
         const phylino_dataset_host &h = ctx->ds[d];
@@ -146,24 +139,59 @@ phylino_status enqueue_spectra(phylino_ctx *ctx, int P, const double *params)
         v.bin_off = d == 0 ? 0 : a.ds[d - 1].bin_off + a.ds[d - 1].n_bins;
         v.tile_begin = tiles;
         for (int j = 0; j < 3; ++j) v.idx_a[j] = h.idx_a[j];
+        v.v_pos_min = h.v_pos_min;
+        v.v_max = h.v_max;
         v.fx_scale = std::ldexp(1.0, h.fx_exp);
         tiles += (int)(h.n_pad / EV_PER_CTA);
     }
-    /* empty datasets own no tile: make sure the lookup in the kernel skips them */
     a.osc.osc_model = ctx->osc_model;
     a.osc.ordering = ctx->ordering;
     for (int j = 0; j < 6; ++j) { a.osc.idx_osc[j] = ctx->idx_osc[j]; a.osc.fixed_osc[j] = ctx->fixed_osc[j]; }
     a.n_datasets = ctx->n_datasets;
     a.n_params = ctx->n_params;
-    a.P = P;
-    a.points_per_cta = default_points_per_cta(ctx, P);
     a.total_bins = ctx->total_bins;
+    a.max_bins = ctx->max_bins;
+    a.per_point_binning = ctx->per_point_binning ? 1 : 0;
+    a.n_tiles = tiles;
+    /* stride permutation of the tile blocks: close to the golden section of the block count and
+     * coprime to it, so that consecutive virtual blocks are far apart in energy */
+    const int nb = (tiles + TILE_BLOCK - 1) / TILE_BLOCK;
+    int stride = std::max(1, (int)std::lround(nb * 0.6180339887));
+    while (stride > 1 && std::gcd(stride, std::max(nb, 1)) != 1) --stride;
+    a.block_stride = stride;
+    return tiles;
+}
+
+constexpr int CTAS_PER_SM = 2;                       /* __launch_bounds__(CTA_THREADS, 2) */
+constexpr size_t SMEM_BUDGET = 110 * 1024;           /* per CTA, so that two fit in 227 KB */
+
+/* Points per chunk: as many as shared memory allows (<= 16), then fewer while the persistent grid
+ * would get less than ~24 (chunk, tile) units per CTA to balance. */
+int choose_points_per_cta(const phylino_ctx *ctx, int P, int tiles)
+{
+    int ppc = ctx->points_per_cta > 0 ? ctx->points_per_cta : 16;
+    ppc = std::max(1, std::min(ppc, P));
+    while (ppc > 1 && spectra_smem_bytes(ctx->n_terms, ctx->max_bins, ppc, ctx->per_point_binning) > SMEM_BUDGET) --ppc;
+    if (ctx->points_per_cta > 0) return ppc;
+    const long long slots = (long long)ctx->sm_count * CTAS_PER_SM;
+    while (ppc > 4 && (long long)tiles * ((P + ppc - 1) / ppc) < 24 * slots) ppc = (ppc + 1) / 2;
+    return ppc;
+}
+
+/* enqueue the spectra kernel (rows a1-a4) for P points */
+phylino_status enqueue_spectra(phylino_ctx *ctx, int P, const double *params)
+{
+    SpectraArgs a{};
+    const int tiles = fill_datasets(ctx, a);
+    a.P = P;
+    a.points_per_cta = choose_points_per_cta(ctx, P, tiles);
+    a.n_chunks = (P + a.points_per_cta - 1) / a.points_per_cta;
     a.params = params;
     a.acc = ctx->d_acc;
     a.flags = ctx->d_flags;
     if (ctx->timing) CU(cudaEventRecord(ctx->ev[0], ctx->stream));
     if (tiles > 0 && P > 0) {
-        CU(launch_spectra(a, tiles, ctx->n_terms, ctx->per_point_binning, ctx->max_bins, ctx->stream));
+        CU(launch_spectra(a, ctx->n_terms, ctx->sm_count, ctx->stream));
         ctx->launches += 1;
     }
     return PHYLINO_OK;
@@ -217,7 +245,12 @@ phylino_status phylino_create(int device, void *cuda_stream, phylino_ctx **out)
     c->device = device;
     c->stream = (cudaStream_t)cuda_stream;
     DeviceGuard g(device);
-    if (!g.ok || cudaFree(0) != cudaSuccess) { cudaGetLastError(); delete c; return PHYLINO_ERR_CUDA; }
+    if (!g.ok || cudaFree(0) != cudaSuccess ||
+        cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, device) != cudaSuccess) {
+        cudaGetLastError();
+        delete c;
+        return PHYLINO_ERR_CUDA;
+    }
     *out = c;
     return PHYLINO_OK;
 }
@@ -382,12 +415,17 @@ phylino_status phylino_load_events(phylino_ctx *ctx, int dataset, int64_t n, con
     std::vector<double> x((size_t)n_pad, 0.0);
     std::vector<float> v((size_t)n_pad, std::nanf("")), w((size_t)n_pad, 0.0f);
     double wsum = 0.0;
+    float v_pos_min = INFINITY, v_max = -INFINITY;
     for (int64_t i = 0; i < n; ++i) {
         int32_t s = perm[i];
         x[i] = baseline_m[core ? core[s] : 0] / (double)e_nu[s];
         v[i] = e_vis[s];
         w[i] = weight ? weight[s] : 1.0f;
         wsum += std::fabs((double)w[i]);
+        if (std::isfinite(v[i])) {
+            if (v[i] > 0.0f && v[i] < v_pos_min) v_pos_min = v[i];
+            if (v[i] > v_max) v_max = v[i];
+        }
     }
     /* fixed-point scale 2^e with 8 * sum|w| * 2^e <= 2^62 (|P_ee| <= 4 is enforced per point) */
     int ex = 0;
@@ -408,6 +446,7 @@ phylino_status phylino_load_events(phylino_ctx *ctx, int dataset, int64_t n, con
     CU(cudaMemcpyAsync((void *)(ctx->fin.inv_scale + dataset), &inv, sizeof(double), cudaMemcpyHostToDevice, st));
     CU(cudaStreamSynchronize(st));
     h.n = n; h.n_pad = n_pad; h.wsum_abs = wsum; h.fx_exp = fx; h.loaded = true;
+    h.v_pos_min = v_pos_min; h.v_max = v_max;
     ctx->err.clear();
     return PHYLINO_OK;
 }
@@ -448,20 +487,20 @@ phylino_status phylino_event_bins(phylino_ctx *ctx, int P, const double *params,
     phylino_status s = check_ready(ctx, P, params, bins);
     if (s != PHYLINO_OK || P == 0) return s;
     DeviceGuard g(ctx->device);
-    int64_t total = phylino_total_events(ctx), off = 0, boff = 0;
+    SpectraArgs a{};
+    fill_datasets(ctx, a);
+    a.P = P;
+    a.points_per_cta = 1;
+    a.n_chunks = P;
+    a.params = params;
+    int64_t total = phylino_total_events(ctx), off = 0;
     for (int d = 0; d < ctx->n_datasets; ++d) {
         const phylino_dataset_host &h = ctx->ds[d];
-        EventBinsArgs a{};
-        a.ds.v = h.d_v; a.ds.edges = h.d_edges; a.ds.n_bins = h.n_bins; a.ds.bin_off = (int32_t)boff;
-        for (int j = 0; j < 3; ++j) a.ds.idx_a[j] = h.idx_a[j];
-        a.perm = h.d_perm; a.n = h.n; a.ev_off = off; a.total_events = total;
-        a.P = P; a.n_params = ctx->n_params; a.params = params; a.bins = bins;
         if (h.n > 0) {
-            CU(launch_event_bins(a, ctx->stream));
+            CU(launch_event_bins(a, d, h.d_perm, h.n, off, total, bins, ctx->stream));
             ctx->launches += 1;
         }
         off += h.n;
-        boff += h.n_bins;
     }
     return PHYLINO_OK;
 }

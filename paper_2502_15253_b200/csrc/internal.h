@@ -22,6 +22,7 @@ constexpr int K_EV       = 8;                       /* events per thread */
 constexpr int CTA_THREADS = 256;
 constexpr int EV_PER_CTA = K_EV * CTA_THREADS;      /* 2048; every dataset is padded to a multiple */
 constexpr int MAX_TERMS  = 3;
+constexpr int TILE_BLOCK = 8;                       /* tiles per block = longest context */
 
 /* flag bits of a (point, bin) accumulator whose value left the fixed-point domain */
 enum : unsigned { FLAG_NAN = 1u, FLAG_PINF = 2u, FLAG_NINF = 4u };
@@ -36,6 +37,8 @@ struct DatasetDev {
     int32_t bin_off;        /* offset of this dataset inside a point's total_bins */
     int32_t tile_begin;     /* first CTA tile (blockIdx.x) of this dataset */
     int32_t idx_a[3];       /* energy-scale indices into theta, -1 => (0,1,0) */
+    float   v_pos_min;      /* smallest positive finite E_vis of the dataset (+inf if none) */
+    float   v_max;          /* largest finite E_vis (-inf if none) */
     double  fx_scale;       /* 2^e: fixed-point scale of the bin accumulators */
 };
 
@@ -51,7 +54,12 @@ struct SpectraArgs {
     int32_t n_datasets;
     int32_t n_params;
     int32_t P;              /* points in the batch */
-    int32_t points_per_cta;
+    int32_t points_per_cta; /* points per chunk */
+    int32_t n_chunks;       /* ceil(P / points_per_cta) */
+    int32_t n_tiles;        /* CTA tiles over all datasets */
+    int32_t block_stride;   /* stride permutation of the tile blocks (coprime to the block count) */
+    int32_t max_bins;       /* largest n_bins: fixes the shared-memory layout */
+    int32_t per_point_binning; /* some dataset's energy scale depends on theta */
     int32_t total_bins;
     const double *params;   /* DEVICE [P x n_params] */
     long long    *acc;      /* DEVICE [P x total_bins] fixed-point accumulators (zero on entry) */
@@ -80,22 +88,12 @@ struct FinalizeArgs {
     double        *nll;           /* [P] (NLL mode) */
 };
 
-struct EventBinsArgs {
-    DatasetDev ds;
-    const int32_t *perm;          /* [n] sorted position -> caller's index */
-    int64_t n;                    /* real events of the dataset */
-    int64_t ev_off;               /* offset of this dataset in the concatenated caller order */
-    int64_t total_events;
-    int32_t P, n_params;
-    const double *params;
-    int32_t *bins;
-};
-
 /* kernel launchers (spectra.cu, finalize.cu, peaks.cu) */
-cudaError_t launch_spectra(const SpectraArgs &a, int n_tiles, int S, bool per_point_binning,
-                           int max_bins, cudaStream_t st);
+size_t spectra_smem_bytes(int S, int max_bins, int ppc, bool per_point);
+cudaError_t launch_spectra(const SpectraArgs &a, int S, int sm_count, cudaStream_t st);
 cudaError_t launch_finalize(const FinalizeArgs &a, int mode /*0 H, 1 mu, 2 nll*/, cudaStream_t st);
-cudaError_t launch_event_bins(const EventBinsArgs &a, cudaStream_t st);
+cudaError_t launch_event_bins(const SpectraArgs &a, int d, const int32_t *perm, long long n, long long ev_off,
+                              long long total_events, int32_t *bins, cudaStream_t st);
 cudaError_t run_peak_fp64(int iters, cudaStream_t st, double *dfma_per_s);
 
 } // namespace phylino
@@ -114,6 +112,7 @@ struct phylino_dataset_host {
     bool     loaded = false;
     int64_t  n = 0, n_pad = 0;
     double   wsum_abs = 0.0;
+    float    v_pos_min = 0.f, v_max = 0.f;
     int      fx_exp = 0;
     double  *d_x = nullptr;
     float   *d_v = nullptr, *d_w = nullptr;
@@ -123,6 +122,7 @@ struct phylino_dataset_host {
 
 struct phylino_ctx {
     int device = 0;
+    int sm_count = 0;
     cudaStream_t stream = nullptr;
     std::string err;
     bool have_model = false;
