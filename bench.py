@@ -32,10 +32,10 @@ import workloads  # noqa: E402
 
 METRIC = "oscillated event x param-point/s (batched spectra+NLL)"
 UNIT = "event*point/s"
-# fp64-pipe instructions per event x point executed by the spectra kernel:
-# 11 per oscillation term + 1 accumulate, + 4 (E' and the two edge compares) when the energy scale
-# differs per point.
-FP64_PER_TERM, FP64_ACC, FP64_BINNING = 11, 1, 4
+# ALGORITHMIC fp64-pipe instructions per event x point: per oscillation term
+# 11 for 1/2 cos(2 phase) (3 range reduction, 1 square, 7 Horner) + 1 multiply-accumulate into the run.
+# The bin/weight bookkeeping is per batch of events and per run, not per event x point.
+FP64_PER_TERM = 12
 # nominal fp64 pipe: 64 lanes/clk/SM x 148 SMs x 1.965 GHz (B200_PROFILING.md table)
 PEAK_FP64_INST = 64 * 148 * 1.965e9
 L2_FLUSH_BYTES = 256 << 20
@@ -43,8 +43,7 @@ L2_FLUSH_BYTES = 256 << 20
 
 def fp64_inst_per_evpt(model) -> int:
     S = 2 if model.osc_model == 0 else 3
-    per_point = any(i >= 0 for d in model.datasets for i in d.idx_a)
-    return FP64_PER_TERM * S + FP64_ACC + (FP64_BINNING if per_point else 0)
+    return FP64_PER_TERM * S
 
 
 class ClockSampler(threading.Thread):
@@ -149,7 +148,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json config, 1-based (default 2 = configs[1])")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--points-per-cta", type=int, default=0)
+    ap.add_argument("--slice-events", type=int, default=0, help="tuning: events per L2-resident slice")
+    ap.add_argument("--max-warps", type=int, default=0, help="tuning: cap on the persistent grid's warps")
     ap.add_argument("--ref-points", type=int, default=16, help="points per step of --impl reference")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
@@ -182,8 +182,8 @@ def main():
         params = wl.theta0[None, :] + rng.uniform(-1, 1, wl.params.shape) * spread[None, :]
     ph = pkg.Phylino(device=local)
     ph.load_workload(wl)
-    if args.points_per_cta:
-        ph.set_point_chunk(args.points_per_cta)
+    if args.slice_events or args.max_warps:
+        ph.set_tuning(args.slice_events, args.max_warps)
     ph.set_timing(True)
     P, NPAR, TB = wl.n_points, wl.model.n_params, ph.total_bins
     d_params = torch.as_tensor(params, device="cuda")
@@ -206,7 +206,7 @@ def main():
     # ---- device-resident timed region: K steps, CUDA events per step, L2 flushed in between ----
     starts = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps)]
     ends = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps)]
-    sp_ms, fin_ms = [], []
+    su_ms, sp_ms, fin_ms = [], [], []
     sampler = ClockSampler(physical_gpu_index(local))
     launches0 = ph.launch_count
     barrier()
@@ -216,9 +216,10 @@ def main():
         starts[i].record()
         ph.nll(d_params, d_data, d_nll)
         ends[i].record()
-        a, b = ph.last_kernel_ms()          # waits for this step; per-kernel device times
-        sp_ms.append(a)
-        fin_ms.append(b)
+        a, b, c = ph.last_kernel_ms()       # waits for this step; per-kernel device times
+        su_ms.append(a)
+        sp_ms.append(b)
+        fin_ms.append(c)
         flush.zero_()
     torch.cuda.synchronize()
     clocks = sampler.stop()
@@ -269,8 +270,8 @@ def main():
             "measured_dfma_peak": None if measured_peak is None else measured_peak / 1e9,
             "frac_of_measured": None if not measured_peak else achieved / measured_peak,
             "fp64_inst_per_event_point": inst, "kernel_ms": sp_avg, "kernel_share_of_step": sp_avg / ms_per_step,
-            "finalize_kernel_ms": sum(fin_ms) / len(fin_ms),
-            "hbm_bytes_per_launch": 16 * wl.n_events + 8 * P * NPAR,
+            "setup_kernel_ms": sum(su_ms) / len(su_ms), "finalize_kernel_ms": sum(fin_ms) / len(fin_ms),
+            "hbm_bytes_per_launch": 20 * wl.n_events + 8 * P * TB,
         }
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,

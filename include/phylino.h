@@ -127,7 +127,7 @@ PHYLINO_API phylino_status phylino_set_model(phylino_ctx *ctx, const phylino_mod
  *   baseline_m[n_cores] L in metres (finite, >= 0)
  *   edges     [n_bins+1] strictly ascending reco-energy bin edges; n_bins must equal the model's.
  * The store is structure-of-arrays, sorted by reconstructed energy ("sorted according
- * to their energy"; R14): x = L_core/E_nu as fp64, E_vis and w as fp32.
+ * to their energy"; R14): x = L_core/E_nu and w as fp64, E_vis as fp32.
  * n = 0 is allowed (empty dataset).  Reloading a dataset replaces it. */
 PHYLINO_API phylino_status phylino_load_events(phylino_ctx *ctx, int dataset, int64_t n,
                                    const float *e_nu_MeV, const float *e_vis_MeV, const float *weight,
@@ -166,14 +166,18 @@ PHYLINO_API phylino_status phylino_spectra_host(phylino_ctx *ctx, int P, const d
 PHYLINO_API int64_t phylino_total_bins(const phylino_ctx *ctx);     /* sum_d n_bins, 0 before set_model */
 PHYLINO_API int64_t phylino_total_events(const phylino_ctx *ctx);   /* sum_d n over loaded datasets */
 
-/* Tuning knob (0 => library default): parameter points per CTA pass over an event tile. */
-PHYLINO_API phylino_status phylino_set_point_chunk(phylino_ctx *ctx, int points_per_cta);
+/* Tuning knobs (0 => library default).  slice_events: events a warp walks for every group of 32
+ * parameter points before it moves on (keeps the re-read events in L2); max_warps: cap on the warps
+ * of the persistent grid of the spectra kernel.  Results are bit-identical from call to call for
+ * fixed knobs; other values regroup the fp64 partial sums (rounding-level differences only). */
+PHYLINO_API phylino_status phylino_set_tuning(phylino_ctx *ctx, int slice_events, int max_warps);
 
-/* Device timing of the two kernels of a call (CUDA events on the context's stream, recorded around
- * the spectra kernel and the finalize kernel of every later call).  phylino_last_kernel_ms waits for
- * the last call to finish and returns its two durations in milliseconds (HOST pointers). */
+/* Device timing of the three kernels of a call (CUDA events on the context's stream, recorded
+ * around the setup, spectra and finalize kernels of every later call).  phylino_last_kernel_ms
+ * waits for the last call to finish and writes its three durations in milliseconds to ms[0..2]
+ * (HOST pointer): per-point setup (records + bin thresholds), spectra, finalize. */
 PHYLINO_API phylino_status phylino_set_timing(phylino_ctx *ctx, int on);
-PHYLINO_API phylino_status phylino_last_kernel_ms(phylino_ctx *ctx, float *spectra_ms, float *finalize_ms);
+PHYLINO_API phylino_status phylino_last_kernel_ms(phylino_ctx *ctx, float *ms);
 
 /* Kernel launches enqueued by this context so far (bench.py's `gpu_launches`). */
 PHYLINO_API int64_t phylino_launch_count(const phylino_ctx *ctx);

@@ -19,7 +19,7 @@ abi_symbols = (
     "phylino_create", "phylino_destroy", "phylino_set_model", "phylino_load_events",
     "phylino_spectra", "phylino_nll", "phylino_event_bins", "phylino_nll_host",
     "phylino_spectra_host", "phylino_total_bins", "phylino_total_events",
-    "phylino_set_point_chunk", "phylino_launch_count", "phylino_last_error", "phylino_peak_fp64",
+    "phylino_set_tuning", "phylino_launch_count", "phylino_last_error", "phylino_peak_fp64",
     "phylino_expectation", "phylino_set_timing", "phylino_last_kernel_ms",
 )
 
@@ -84,7 +84,7 @@ def load_library():
     lib.phylino_set_timing.restype = i32
     lib.phylino_set_timing.argtypes = [vp, i32]
     lib.phylino_last_kernel_ms.restype = i32
-    lib.phylino_last_kernel_ms.argtypes = [vp, C.POINTER(C.c_float), C.POINTER(C.c_float)]
+    lib.phylino_last_kernel_ms.argtypes = [vp, C.POINTER(C.c_float)]
     lib.phylino_event_bins.restype = i32
     lib.phylino_event_bins.argtypes = [vp, i32, vp, vp]
     lib.phylino_nll_host.restype = i32
@@ -95,8 +95,8 @@ def load_library():
     lib.phylino_total_bins.argtypes = [vp]
     lib.phylino_total_events.restype = i64
     lib.phylino_total_events.argtypes = [vp]
-    lib.phylino_set_point_chunk.restype = i32
-    lib.phylino_set_point_chunk.argtypes = [vp, i32]
+    lib.phylino_set_tuning.restype = i32
+    lib.phylino_set_tuning.argtypes = [vp, i32, i32]
     lib.phylino_launch_count.restype = i64
     lib.phylino_launch_count.argtypes = [vp]
     lib.phylino_last_error.restype = C.c_char_p
@@ -237,8 +237,8 @@ class Phylino:
     def launch_count(self) -> int:
         return int(self._lib.phylino_launch_count(self._ctx))
 
-    def set_point_chunk(self, points_per_cta: int):
-        self._check(self._lib.phylino_set_point_chunk(self._ctx, int(points_per_cta)))
+    def set_tuning(self, slice_events: int = 0, max_warps: int = 0):
+        self._check(self._lib.phylino_set_tuning(self._ctx, int(slice_events), int(max_warps)))
 
     # -- phylino_spectra / phylino_nll / phylino_event_bins (device buffers, asynchronous) -------
     def spectra(self, params, out=None):
@@ -278,10 +278,10 @@ class Phylino:
         self._check(self._lib.phylino_set_timing(self._ctx, int(bool(on))))
 
     def last_kernel_ms(self):
-        """(spectra kernel ms, finalize kernel ms) of the last call; waits for it to finish."""
-        a, b = C.c_float(0.0), C.c_float(0.0)
-        self._check(self._lib.phylino_last_kernel_ms(self._ctx, C.byref(a), C.byref(b)))
-        return float(a.value), float(b.value)
+        """(setup, spectra, finalize) kernel ms of the last call; waits for it to finish."""
+        ms = (C.c_float * 3)()
+        self._check(self._lib.phylino_last_kernel_ms(self._ctx, ms))
+        return float(ms[0]), float(ms[1]), float(ms[2])
 
     def event_bins(self, params):
         t = self._torch

@@ -63,8 +63,8 @@ template <class T> cudaError_t upload(T **dst, const std::vector<T> &src, cudaSt
 
 void free_events(phylino_dataset_host &d)
 {
-    cudaFree(d.d_x); cudaFree(d.d_v); cudaFree(d.d_w); cudaFree(d.d_edges); cudaFree(d.d_perm);
-    d.d_x = nullptr; d.d_v = nullptr; d.d_w = nullptr; d.d_edges = nullptr; d.d_perm = nullptr;
+    cudaFree(d.d_x); cudaFree(d.d_v); cudaFree(d.d_w); cudaFree(d.d_wsum); cudaFree(d.d_edges); cudaFree(d.d_perm);
+    d.d_x = nullptr; d.d_v = nullptr; d.d_w = nullptr; d.d_wsum = nullptr; d.d_edges = nullptr; d.d_perm = nullptr;
     d.loaded = false; d.n = d.n_pad = 0;
 }
 
@@ -85,6 +85,8 @@ void free_all(phylino_ctx *c)
     free_tables(c);
     cudaFree(c->d_acc); cudaFree(c->d_flags);
     c->d_acc = nullptr; c->d_flags = nullptr; c->acc_capacity = 0;
+    cudaFree(c->d_rec); cudaFree(c->d_thr); cudaFree(c->d_safe);
+    c->d_rec = nullptr; c->d_thr = nullptr; c->d_safe = nullptr; c->point_capacity = 0;
     cudaFree(c->d_stage); c->d_stage = nullptr;
     if (c->h_pin) cudaFreeHost(c->h_pin);
     c->h_pin = nullptr; c->stage_capacity = 0;
@@ -114,35 +116,50 @@ phylino_status check_ready(phylino_ctx *ctx, int P, const void *params, const vo
 phylino_status ensure_acc(phylino_ctx *ctx, int P)
 {
     int64_t need = (int64_t)P * ctx->total_bins;
-    if (need <= ctx->acc_capacity) return PHYLINO_OK;
-    /* the stream may still use the old buffers */
-    CU(cudaStreamSynchronize(ctx->stream));
-    cudaFree(ctx->d_acc); cudaFree(ctx->d_flags);
-    ctx->d_acc = nullptr; ctx->d_flags = nullptr; ctx->acc_capacity = 0;
-    CU(cudaMalloc((void **)&ctx->d_acc, need * sizeof(long long)));
-    CU(cudaMalloc((void **)&ctx->d_flags, need * sizeof(unsigned)));
-    CU(cudaMemsetAsync(ctx->d_acc, 0, need * sizeof(long long), ctx->stream));
-    CU(cudaMemsetAsync(ctx->d_flags, 0, need * sizeof(unsigned), ctx->stream));
-    ctx->acc_capacity = need;
+    if (need > ctx->acc_capacity) {
+        /* the stream may still use the old buffers */
+        CU(cudaStreamSynchronize(ctx->stream));
+        cudaFree(ctx->d_acc); cudaFree(ctx->d_flags);
+        ctx->d_acc = nullptr; ctx->d_flags = nullptr; ctx->acc_capacity = 0;
+        CU(cudaMalloc((void **)&ctx->d_acc, need * sizeof(long long)));
+        CU(cudaMalloc((void **)&ctx->d_flags, need * sizeof(unsigned)));
+        CU(cudaMemsetAsync(ctx->d_acc, 0, need * sizeof(long long), ctx->stream));
+        CU(cudaMemsetAsync(ctx->d_flags, 0, need * sizeof(unsigned), ctx->stream));
+        ctx->acc_capacity = need;
+    }
+    if (P > ctx->point_capacity) {
+        /* per-point records and threshold rows written by the setup kernel of every call */
+        CU(cudaStreamSynchronize(ctx->stream));
+        cudaFree(ctx->d_rec); cudaFree(ctx->d_thr); cudaFree(ctx->d_safe);
+        ctx->d_rec = nullptr; ctx->d_thr = nullptr; ctx->d_safe = nullptr; ctx->point_capacity = 0;
+        const int64_t rows = ctx->per_point_binning ? P : 1;
+        CU(cudaMalloc((void **)&ctx->d_rec, (size_t)rec_fields(ctx->n_terms) * P * sizeof(double)));
+        CU(cudaMalloc((void **)&ctx->d_thr, (size_t)rows * (ctx->total_bins + ctx->n_datasets) * sizeof(float)));
+        CU(cudaMalloc((void **)&ctx->d_safe, (size_t)rows * ctx->n_datasets * sizeof(float2)));
+        ctx->point_capacity = P;
+    }
     return PHYLINO_OK;
 }
 
 /* fill the by-value kernel arguments that do not depend on the batch */
-int fill_datasets(const phylino_ctx *ctx, SpectraArgs &a)
+void fill_datasets(const phylino_ctx *ctx, SpectraArgs &a)
 {
-    int tiles = 0;
+    int64_t batches = 0;
     for (int d = 0; d < ctx->n_datasets; ++d) {
         const phylino_dataset_host &h = ctx->ds[d];
         DatasetDev &v = a.ds[d];
-        v.x = h.d_x; v.v = h.d_v; v.w = h.d_w; v.edges = h.d_edges;
+        v.x = h.d_x; v.w = h.d_w; v.v = h.d_v; v.wsum = h.d_wsum; v.edges = h.d_edges;
         v.n_bins = h.n_bins;
         v.bin_off = d == 0 ? 0 : a.ds[d - 1].bin_off + a.ds[d - 1].n_bins;
-        v.tile_begin = tiles;
+        v.thr_off = v.bin_off + d;
+        v.per_point = (h.idx_a[0] >= 0 || h.idx_a[1] >= 0 || h.idx_a[2] >= 0) ? 1 : 0;
+        v.batch_begin = (int32_t)batches;
+        v.n_batches = (int32_t)(h.n_pad / EB);
         for (int j = 0; j < 3; ++j) v.idx_a[j] = h.idx_a[j];
         v.v_pos_min = h.v_pos_min;
         v.v_max = h.v_max;
         v.fx_scale = std::ldexp(1.0, h.fx_exp);
-        tiles += (int)(h.n_pad / EV_PER_CTA);
+        batches += h.n_pad / EB;
     }
     a.osc.osc_model = ctx->osc_model;
     a.osc.ordering = ctx->ordering;
@@ -150,48 +167,52 @@ int fill_datasets(const phylino_ctx *ctx, SpectraArgs &a)
     a.n_datasets = ctx->n_datasets;
     a.n_params = ctx->n_params;
     a.total_bins = ctx->total_bins;
-    a.max_bins = ctx->max_bins;
-    a.per_point_binning = ctx->per_point_binning ? 1 : 0;
-    a.n_tiles = tiles;
-    /* stride permutation of the tile blocks: close to the golden section of the block count and
-     * coprime to it, so that consecutive virtual blocks are far apart in energy */
-    const int nb = (tiles + TILE_BLOCK - 1) / TILE_BLOCK;
-    int stride = std::max(1, (int)std::lround(nb * 0.6180339887));
-    while (stride > 1 && std::gcd(stride, std::max(nb, 1)) != 1) --stride;
-    a.block_stride = stride;
-    return tiles;
+    a.thr_stride = ctx->total_bins + ctx->n_datasets;
+    a.n_batches = (int32_t)batches;
+    a.rec = ctx->d_rec;
+    a.thr = ctx->d_thr;
+    a.safe = ctx->d_safe;
+    a.acc = ctx->d_acc;
+    a.flags = ctx->d_flags;
 }
 
-constexpr int CTAS_PER_SM = 2;                       /* __launch_bounds__(CTA_THREADS, 2) */
-constexpr size_t SMEM_BUDGET = 110 * 1024;           /* per CTA, so that two fit in 227 KB */
-
-/* Points per chunk: as many as shared memory allows (<= 16), then fewer while the persistent grid
- * would get less than ~24 (chunk, tile) units per CTA to balance. */
-int choose_points_per_cta(const phylino_ctx *ctx, int P, int tiles)
+void fill_batch(const phylino_ctx *ctx, SpectraArgs &a, int P, const double *params)
 {
-    int ppc = ctx->points_per_cta > 0 ? ctx->points_per_cta : 16;
-    ppc = std::max(1, std::min(ppc, P));
-    while (ppc > 1 && spectra_smem_bytes(ctx->n_terms, ctx->max_bins, ppc, ctx->per_point_binning) > SMEM_BUDGET) --ppc;
-    if (ctx->points_per_cta > 0) return ppc;
-    const long long slots = (long long)ctx->sm_count * CTAS_PER_SM;
-    while (ppc > 4 && (long long)tiles * ((P + ppc - 1) / ppc) < 24 * slots) ppc = (ppc + 1) / 2;
-    return ppc;
+    a.P = P;
+    a.params = params;
+    a.thr_rows = ctx->per_point_binning ? P : 1;
+    const int slice_events = ctx->slice_events > 0 ? ctx->slice_events : 512;
+    a.slice_batches = std::max(1, slice_events / EB);
 }
 
-/* enqueue the spectra kernel (rows a1-a4) for P points */
+/* Warps of the persistent grid: all the chip holds at once, fewer while a lane's sub-stream would
+ * get less than two batches (tiny inputs are launch-latency bound anyway). */
+int choose_warps(const phylino_ctx *ctx, int P, int64_t batches)
+{
+    int streams = 1;                                   /* sub-streams per warp of the (only) point group */
+    if (P < 32) { int pl = 1; while (pl < P) pl <<= 1; streams = 32 / pl; }
+    int64_t w = std::max<int64_t>(1, batches / (2 * streams));
+    int cap = ctx->resident_warps;
+    if (ctx->max_warps > 0) cap = std::min(cap, ctx->max_warps);
+    return (int)std::min<int64_t>(w, std::max(cap, 1));
+}
+
+/* enqueue the setup and spectra kernels (rows a1-a4) for P points */
 phylino_status enqueue_spectra(phylino_ctx *ctx, int P, const double *params)
 {
     SpectraArgs a{};
-    const int tiles = fill_datasets(ctx, a);
-    a.P = P;
-    a.points_per_cta = choose_points_per_cta(ctx, P, tiles);
-    a.n_chunks = (P + a.points_per_cta - 1) / a.points_per_cta;
-    a.params = params;
-    a.acc = ctx->d_acc;
-    a.flags = ctx->d_flags;
+    fill_datasets(ctx, a);
+    fill_batch(ctx, a, P, params);
+    if (ctx->resident_warps == 0)
+        CU(spectra_max_warps(ctx->n_terms, ctx->sm_count, &ctx->resident_warps));
     if (ctx->timing) CU(cudaEventRecord(ctx->ev[0], ctx->stream));
-    if (tiles > 0 && P > 0) {
-        CU(launch_spectra(a, ctx->n_terms, ctx->sm_count, ctx->stream));
+    if (a.n_batches > 0 && P > 0) {
+        CU(launch_setup(a, ctx->n_terms, ctx->stream));
+        ctx->launches += 1;
+    }
+    if (ctx->timing) CU(cudaEventRecord(ctx->ev[1], ctx->stream));
+    if (a.n_batches > 0 && P > 0) {
+        CU(launch_spectra(a, ctx->n_terms, choose_warps(ctx, P, a.n_batches), ctx->stream));
         ctx->launches += 1;
     }
     return PHYLINO_OK;
@@ -209,10 +230,10 @@ phylino_status enqueue_finalize(phylino_ctx *ctx, int P, const double *params, c
     f.data = data;
     f.hist = hist;
     f.nll = nll;
-    if (ctx->timing) CU(cudaEventRecord(ctx->ev[1], ctx->stream));
+    if (ctx->timing) CU(cudaEventRecord(ctx->ev[2], ctx->stream));
     CU(launch_finalize(f, mode, ctx->stream));
     ctx->launches += 1;
-    if (ctx->timing) CU(cudaEventRecord(ctx->ev[2], ctx->stream));
+    if (ctx->timing) CU(cudaEventRecord(ctx->ev[3], ctx->stream));
     return PHYLINO_OK;
 }
 
@@ -411,17 +432,18 @@ phylino_status phylino_load_events(phylino_ctx *ctx, int dataset, int64_t n, con
         if (y != y) return true;
         return x < y;
     });
-    const int64_t n_pad = (n + EV_PER_CTA - 1) / EV_PER_CTA * EV_PER_CTA;
-    std::vector<double> x((size_t)n_pad, 0.0);
-    std::vector<float> v((size_t)n_pad, std::nanf("")), w((size_t)n_pad, 0.0f);
+    const int64_t n_pad = (n + EB - 1) / EB * EB;
+    std::vector<double> x((size_t)n_pad, 0.0), w((size_t)n_pad, 0.0), ws((size_t)(n_pad / EB), 0.0);
+    std::vector<float> v((size_t)n_pad, std::nanf(""));
     double wsum = 0.0;
     float v_pos_min = INFINITY, v_max = -INFINITY;
     for (int64_t i = 0; i < n; ++i) {
         int32_t s = perm[i];
         x[i] = baseline_m[core ? core[s] : 0] / (double)e_nu[s];
         v[i] = e_vis[s];
-        w[i] = weight ? weight[s] : 1.0f;
-        wsum += std::fabs((double)w[i]);
+        w[i] = weight ? (double)weight[s] : 1.0;
+        ws[i / EB] += w[i];                     /* in event order: the batch total the hot kernel adds */
+        wsum += std::fabs(w[i]);
         if (std::isfinite(v[i])) {
             if (v[i] > 0.0f && v[i] < v_pos_min) v_pos_min = v[i];
             if (v[i] > v_max) v_max = v[i];
@@ -440,6 +462,7 @@ phylino_status phylino_load_events(phylino_ctx *ctx, int dataset, int64_t n, con
     CU(upload(&h.d_x, x, st));
     CU(upload(&h.d_v, v, st));
     CU(upload(&h.d_w, w, st));
+    CU(upload(&h.d_wsum, ws, st));
     CU(upload(&h.d_edges, ed, st));
     CU(upload(&h.d_perm, perm, st));
     double inv = std::ldexp(1.0, -fx);
@@ -487,12 +510,14 @@ phylino_status phylino_event_bins(phylino_ctx *ctx, int P, const double *params,
     phylino_status s = check_ready(ctx, P, params, bins);
     if (s != PHYLINO_OK || P == 0) return s;
     DeviceGuard g(ctx->device);
+    if ((s = ensure_acc(ctx, P)) != PHYLINO_OK) return s;
     SpectraArgs a{};
     fill_datasets(ctx, a);
-    a.P = P;
-    a.points_per_cta = 1;
-    a.n_chunks = P;
-    a.params = params;
+    fill_batch(ctx, a, P, params);
+    if (a.n_batches > 0) {                      /* the threshold rows the hot kernel would use */
+        CU(launch_setup(a, ctx->n_terms, ctx->stream));
+        ctx->launches += 1;
+    }
     int64_t total = phylino_total_events(ctx), off = 0;
     for (int d = 0; d < ctx->n_datasets; ++d) {
         const phylino_dataset_host &h = ctx->ds[d];
@@ -553,11 +578,12 @@ int64_t phylino_total_events(const phylino_ctx *ctx)
     return t;
 }
 
-phylino_status phylino_set_point_chunk(phylino_ctx *ctx, int points_per_cta)
+phylino_status phylino_set_tuning(phylino_ctx *ctx, int slice_events, int max_warps)
 {
     if (!ctx) return PHYLINO_ERR_ARG;
-    if (points_per_cta < 0 || points_per_cta > CTA_THREADS) return fail(ctx, PHYLINO_ERR_ARG, "points_per_cta = %d not in 0..%d", points_per_cta, CTA_THREADS);
-    ctx->points_per_cta = points_per_cta;
+    if (slice_events < 0 || max_warps < 0) return fail(ctx, PHYLINO_ERR_ARG, "negative tuning value");
+    ctx->slice_events = slice_events;
+    ctx->max_warps = max_warps;
     return PHYLINO_OK;
 }
 
@@ -571,14 +597,13 @@ phylino_status phylino_set_timing(phylino_ctx *ctx, int on)
     return PHYLINO_OK;
 }
 
-phylino_status phylino_last_kernel_ms(phylino_ctx *ctx, float *spectra_ms, float *finalize_ms)
+phylino_status phylino_last_kernel_ms(phylino_ctx *ctx, float *ms)
 {
-    if (!ctx || !spectra_ms || !finalize_ms) return PHYLINO_ERR_ARG;
+    if (!ctx || !ms) return PHYLINO_ERR_ARG;
     if (!ctx->timing) return fail(ctx, PHYLINO_ERR_STATE, "phylino_set_timing(ctx, 1) has not been called");
     DeviceGuard g(ctx->device);
-    CU(cudaEventSynchronize(ctx->ev[2]));
-    CU(cudaEventElapsedTime(spectra_ms, ctx->ev[0], ctx->ev[1]));
-    CU(cudaEventElapsedTime(finalize_ms, ctx->ev[1], ctx->ev[2]));
+    CU(cudaEventSynchronize(ctx->ev[3]));
+    for (int i = 0; i < 3; ++i) CU(cudaEventElapsedTime(ms + i, ctx->ev[i], ctx->ev[i + 1]));
     return PHYLINO_OK;
 }
 

@@ -63,30 +63,31 @@ __device__ __forceinline__ double halfturn_coeff(double dm2)
     return (1.267 * dm2) * 0.63661977236758134308;   /* 2/pi */
 }
 
-/* sin^2((pi/2) h x), |h x| < 2^51.
+/* g(h, x) = 1/2 cos(pi h x) = 1/2 - sin^2((pi/2) h x), |h x| < 2^51, so that
+ *   P_ee = 1 - sum_k A_k sin^2(phase_k) = (1 - 1/2 sum_k A_k) + sum_k A_k g(h_k, x).
  *   n = rint(h x) by the 1.5*2^52 trick, f = h x - n in [-1/2, 1/2] with ONE rounding (fma), so the
  *   range reduction is exact for phases of thousands of radians (config 5: 7.8e3 rad);
- *   q = sin^2((pi/2) f) = z Q(z), z = f^2: degree-5 minimax Q, |error| <= 4.1e-13 absolute
- *   (Remez fit made for this file);
- *   n odd  =>  sin^2 = 1 - q.  Parity, sign flip and the constant are integer-pipe work.
- * 11 fp64 instructions including the final A-weighted update done by the caller. */
-__device__ __forceinline__ double sin2_halfturns(double h, double x)
+ *   1/2 cos(pi f) = 1/2 - z Q(z), z = f^2: degree-5 minimax Q, |error| <= 4.1e-13 absolute
+ *   (Remez fit made for this file, checked against mpmath);
+ *   cos(pi (n + f)) = (-1)^n cos(pi f): the parity of n is bit 0 of the low word of t, moved onto
+ *   the sign bit of the result by ONE integer multiply-add on the high word.
+ * 10 fp64 instructions + 1 integer instruction. */
+__device__ __forceinline__ double half_cos_halfturns(double h, double x)
 {
     const double MAGIC = 6755399441055744.0;        /* 1.5 * 2^52 */
     double t = fma(h, x, MAGIC);
     double n = t - MAGIC;
     double f = fma(h, x, -n);
     double z = f * f;
-    double q = -0x1.e2a4cab0973aep-11;
-    q = fma(q, z,  0x1.a65598e5b8576p-7);
-    q = fma(q, z, -0x1.e1f273f3e9df0p-4);
-    q = fma(q, z,  0x1.55d3c0fdef250p-1);
-    q = fma(q, z, -0x1.03c1f070b1413p+1);
-    q = fma(q, z,  0x1.3bd3cc9bac6fep+1);
-    unsigned odd = (unsigned)__double2loint(t) & 1u;
-    double sz   = __hiloint2double(__double2hiint(z) ^ (int)(odd << 31), __double2loint(z));
-    double oddf = __hiloint2double((int)(odd * 0x3FF00000u), 0);
-    return fma(sz, q, oddf);
+    double q =  0x1.e2a4cab0973aep-11;               /* -Q(z), Horner */
+    q = fma(q, z, -0x1.a65598e5b8576p-7);
+    q = fma(q, z,  0x1.e1f273f3e9df0p-4);
+    q = fma(q, z, -0x1.55d3c0fdef250p-1);
+    q = fma(q, z,  0x1.03c1f070b1413p+1);
+    q = fma(q, z, -0x1.3bd3cc9bac6fep+1);
+    double c = fma(q, z, 0.5);
+    unsigned hi = (unsigned)__double2hiint(c) + ((unsigned)__double2loint(t) << 31);
+    return __hiloint2double((int)hi, __double2loint(c));
 }
 
 /* E' = fma(fma(a2, v, a1), v, a0): the normative rounding sequence of the energy-scale map (R8). */

@@ -15,14 +15,14 @@
 
 namespace phylino {
 
-/* ---- tiling of the event store --------------------------------------------------------------
- * One CTA owns EV_PER_CTA consecutive (E_vis-sorted) events of ONE dataset and walks a chunk of
- * parameter points over them; thread t keeps events [t*K, t*K+K) of the tile in registers. */
-constexpr int K_EV       = 8;                       /* events per thread */
-constexpr int CTA_THREADS = 256;
-constexpr int EV_PER_CTA = K_EV * CTA_THREADS;      /* 2048; every dataset is padded to a multiple */
-constexpr int MAX_TERMS  = 3;
-constexpr int TILE_BLOCK = 8;                       /* tiles per block = longest context */
+/* ---- layout of the event store and of a launch -------------------------------------------------
+ * The events of a dataset, sorted by E_vis, are cut into batches of EB consecutive events; a warp
+ * owns a contiguous range of batches and walks it once per group of 32 parameter points, ONE
+ * POINT PER LANE (spectra.cu). */
+constexpr int EB          = 4;                      /* events per batch; every dataset is padded to a multiple */
+constexpr int WARPS       = 4;                      /* warps per CTA of the spectra kernel */
+constexpr int MAX_TERMS   = 3;
+constexpr int SETUP_THREADS = 128;
 
 /* flag bits of a (point, bin) accumulator whose value left the fixed-point domain */
 enum : unsigned { FLAG_NAN = 1u, FLAG_PINF = 2u, FLAG_NINF = 4u };
@@ -30,12 +30,16 @@ enum : unsigned { FLAG_NAN = 1u, FLAG_PINF = 2u, FLAG_NINF = 4u };
 /* Per-dataset entry of the table that travels by value in the kernel parameters. */
 struct DatasetDev {
     const double *x;        /* [n_pad] L_core/E_nu  [m/MeV], fp64 (phase range reduction needs it) */
+    const double *w;        /* [n_pad] MC weight as fp64 (exact copy of the fp32 input); padding = 0 */
     const float  *v;        /* [n_pad] E_vis [MeV]; padding = NaN */
-    const float  *w;        /* [n_pad] MC weight;   padding = 0   */
+    const double *wsum;     /* [n_pad / EB] sum of the weights of a batch */
     const double *edges;    /* [n_bins+1] */
     int32_t n_bins;
     int32_t bin_off;        /* offset of this dataset inside a point's total_bins */
-    int32_t tile_begin;     /* first CTA tile (blockIdx.x) of this dataset */
+    int32_t thr_off;        /* offset of this dataset inside a threshold row: sum of (n_bins+1) before it */
+    int32_t per_point;      /* the energy scale of this dataset depends on theta */
+    int32_t batch_begin;    /* first global batch of this dataset */
+    int32_t n_batches;
     int32_t idx_a[3];       /* energy-scale indices into theta, -1 => (0,1,0) */
     float   v_pos_min;      /* smallest positive finite E_vis of the dataset (+inf if none) */
     float   v_max;          /* largest finite E_vis (-inf if none) */
@@ -48,20 +52,24 @@ struct OscDev {
     double  fixed_osc[6];
 };
 
+/* per-point record written by the setup kernel, structure-of-arrays: rec[field * P + p] */
+constexpr int rec_fields(int S) { return 2 * S + 2; }       /* h_k, A_k, P0, bad */
+
 struct SpectraArgs {
     DatasetDev ds[PHYLINO_MAX_DATASETS];
     OscDev  osc;
     int32_t n_datasets;
     int32_t n_params;
     int32_t P;              /* points in the batch */
-    int32_t points_per_cta; /* points per chunk */
-    int32_t n_chunks;       /* ceil(P / points_per_cta) */
-    int32_t n_tiles;        /* CTA tiles over all datasets */
-    int32_t block_stride;   /* stride permutation of the tile blocks (coprime to the block count) */
-    int32_t max_bins;       /* largest n_bins: fixes the shared-memory layout */
-    int32_t per_point_binning; /* some dataset's energy scale depends on theta */
+    int32_t n_batches;      /* event batches over all datasets */
+    int32_t slice_batches;  /* batches a warp walks for all point groups before moving on */
+    int32_t thr_stride;     /* floats per threshold row: total_bins + n_datasets */
+    int32_t thr_rows;       /* P if some dataset's energy scale depends on theta, else 1 */
     int32_t total_bins;
     const double *params;   /* DEVICE [P x n_params] */
+    double       *rec;      /* DEVICE [rec_fields x P] per-point records (setup kernel) */
+    float        *thr;      /* DEVICE [thr_rows x thr_stride] fp32 bin thresholds (setup kernel) */
+    float2       *safe;     /* DEVICE [thr_rows x n_datasets] fp32 interval on which a row holds */
     long long    *acc;      /* DEVICE [P x total_bins] fixed-point accumulators (zero on entry) */
     unsigned     *flags;    /* DEVICE [P x total_bins] FLAG_* (zero on entry) */
 };
@@ -89,8 +97,9 @@ struct FinalizeArgs {
 };
 
 /* kernel launchers (spectra.cu, finalize.cu, peaks.cu) */
-size_t spectra_smem_bytes(int S, int max_bins, int ppc, bool per_point);
-cudaError_t launch_spectra(const SpectraArgs &a, int S, int sm_count, cudaStream_t st);
+cudaError_t launch_setup(const SpectraArgs &a, int S, cudaStream_t st);
+cudaError_t spectra_max_warps(int S, int sm_count, int *warps);
+cudaError_t launch_spectra(const SpectraArgs &a, int S, int n_warps, cudaStream_t st);
 cudaError_t launch_finalize(const FinalizeArgs &a, int mode /*0 H, 1 mu, 2 nll*/, cudaStream_t st);
 cudaError_t launch_event_bins(const SpectraArgs &a, int d, const int32_t *perm, long long n, long long ev_off,
                               long long total_events, int32_t *bins, cudaStream_t st);
@@ -114,8 +123,8 @@ struct phylino_dataset_host {
     double   wsum_abs = 0.0;
     float    v_pos_min = 0.f, v_max = 0.f;
     int      fx_exp = 0;
-    double  *d_x = nullptr;
-    float   *d_v = nullptr, *d_w = nullptr;
+    double  *d_x = nullptr, *d_w = nullptr, *d_wsum = nullptr;
+    float   *d_v = nullptr;
     double  *d_edges = nullptr;
     int32_t *d_perm = nullptr;
 };
@@ -135,17 +144,23 @@ struct phylino_ctx {
     /* device model tables */
     void *d_tables = nullptr;                      /* one allocation, carved up below */
     phylino::FinalizeArgs fin{};                   /* table pointers filled by set_model */
-    /* accumulators */
+    /* accumulators and per-call point tables */
     int64_t   acc_capacity = 0;                    /* in (point, bin) cells */
     long long *d_acc = nullptr;
     unsigned  *d_flags = nullptr;
+    int64_t   point_capacity = 0;                  /* points the tables below hold */
+    double   *d_rec = nullptr;                     /* [rec_fields x point_capacity] */
+    float    *d_thr = nullptr;                     /* [thr_rows x (total_bins + n_datasets)] */
+    float2   *d_safe = nullptr;                    /* [thr_rows x n_datasets] */
     /* host-buffer entry points: pinned + device staging */
     double *h_pin = nullptr, *d_stage = nullptr;
     int64_t stage_capacity = 0;                    /* doubles */
-    int points_per_cta = 0;
-    /* optional device timing of the two kernels of a call (phylino_set_timing) */
+    /* tuning knobs, 0 => default (phylino_set_tuning) */
+    int slice_events = 0, max_warps = 0;
+    int resident_warps = 0;                        /* warps of the spectra kernel the chip holds at once */
+    /* optional device timing of the three kernels of a call (phylino_set_timing) */
     bool timing = false;
-    cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};
+    cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
     int64_t launches = 0;
 };
 

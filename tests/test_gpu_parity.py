@@ -35,15 +35,15 @@ def _check_hist(h_gpu, h_orc):
     return 0.0 if rel.size == 0 else float(rel.max())
 
 
-def _run_case(gpu, oracle_mod, wl, check_bins=True, points=None, ppc=None):
+def _run_case(gpu, oracle_mod, wl, check_bins=True, points=None, tuning=None):
     import torch
     params = wl.params if points is None else wl.params[points]
     orc = oracle_mod.Oracle(wl.model, wl.events)
     data = _data_for(orc, wl, oracle_mod)
     with gpu.Phylino() as ph:
         ph.load_workload(wl)
-        if ppc:
-            ph.set_point_chunk(ppc)
+        if tuning:
+            ph.set_tuning(*tuning)
         dp = _dev(params)
         h = ph.spectra(dp).cpu().numpy()
         nll = ph.nll(dp, _dev(data)).cpu().numpy()
@@ -117,20 +117,20 @@ def test_bitwise_reproducible(gpu, oracle_mod):
     outs = {}
     with gpu.Phylino() as ph:
         ph.load_workload(wl)
-        for ppc in (0, 0, 1, 5, 16, 5, 1, 0):
-            ph.set_point_chunk(ppc)
-            outs.setdefault(ppc, []).append((ph.spectra(dp).cpu().numpy(), ph.nll(dp, data).cpu().numpy()))
+        for tun in ((0, 0), (0, 0), (64, 0), (0, 37), (4096, 1000), (0, 37), (64, 0), (0, 0)):
+            ph.set_tuning(*tun)
+            outs.setdefault(tun, []).append((ph.spectra(dp).cpu().numpy(), ph.nll(dp, data).cpu().numpy()))
     torch.cuda.synchronize()
     # same inputs, same launch configuration => the same bits, call after call
-    for ppc, runs in outs.items():
+    for tun, runs in outs.items():
         for h, n in runs[1:]:
-            assert h.tobytes() == runs[0][0].tobytes() and n.tobytes() == runs[0][1].tobytes(), ppc
-    # another point chunk changes which events a thread sums in fp64 before the (exact) integer
+            assert h.tobytes() == runs[0][0].tobytes() and n.tobytes() == runs[0][1].tobytes(), tun
+    # another slice length / grid changes which events a lane sums in fp64 before the (exact) integer
     # accumulation: rounding-level differences only
-    for ppc, runs in outs.items():
-        assert np.allclose(runs[0][0], outs[0][0][0], rtol=1e-13, atol=0)
-        assert np.allclose(runs[0][1], outs[0][0][1], rtol=0, atol=1e-9)
-    outs = [(outs[0][0][0].tobytes(), None)]
+    for tun, runs in outs.items():
+        assert np.allclose(runs[0][0], outs[(0, 0)][0][0], rtol=1e-13, atol=0)
+        assert np.allclose(runs[0][1], outs[(0, 0)][0][1], rtol=0, atol=1e-9)
+    outs = [(outs[(0, 0)][0][0].tobytes(), None)]
     # a second context on a permuted copy of the events gives the same bits: the fixed-point
     # accumulators do not depend on arrival order, the sort is by E_vis
     wl2 = workloads.make_config(2, scale=0.02, n_points=23)
@@ -157,7 +157,7 @@ def test_host_entry_points_match_device_ones(gpu, oracle_mod):
         n_d = ph.nll(dp, _dev(data)).cpu().numpy()
         h_h = ph.spectra_host(wl.params)
         n_h = ph.nll_host(wl.params, data)
-        assert ph.launch_count == 8
+        assert ph.launch_count == 12             # setup + spectra + finalize per call
     assert h_d.tobytes() == h_h.tobytes() and n_d.tobytes() == n_h.tobytes()
 
 
