@@ -148,7 +148,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json config, 1-based (default 2 = configs[1])")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--slice-events", type=int, default=0, help="tuning: events per L2-resident slice")
+    ap.add_argument("--unit-events", type=int, default=0, help="tuning: events per unit of the event store")
+    ap.add_argument("--chunk-groups", type=int, default=0, help="tuning: groups of 32 points per work item")
     ap.add_argument("--max-warps", type=int, default=0, help="tuning: cap on the persistent grid's warps")
     ap.add_argument("--ref-points", type=int, default=16, help="points per step of --impl reference")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -182,8 +183,8 @@ def main():
         params = wl.theta0[None, :] + rng.uniform(-1, 1, wl.params.shape) * spread[None, :]
     ph = pkg.Phylino(device=local)
     ph.load_workload(wl)
-    if args.slice_events or args.max_warps:
-        ph.set_tuning(args.slice_events, args.max_warps)
+    if args.unit_events or args.chunk_groups or args.max_warps:
+        ph.set_tuning(args.unit_events, args.chunk_groups, args.max_warps)
     ph.set_timing(True)
     P, NPAR, TB = wl.n_points, wl.model.n_params, ph.total_bins
     d_params = torch.as_tensor(params, device="cuda")
@@ -271,7 +272,7 @@ def main():
             "frac_of_measured": None if not measured_peak else achieved / measured_peak,
             "fp64_inst_per_event_point": inst, "kernel_ms": sp_avg, "kernel_share_of_step": sp_avg / ms_per_step,
             "setup_kernel_ms": sum(su_ms) / len(su_ms), "finalize_kernel_ms": sum(fin_ms) / len(fin_ms),
-            "hbm_bytes_per_launch": 20 * wl.n_events + 8 * P * TB,
+            "hbm_bytes_per_launch": 24 * wl.n_events + 8 * P * TB,
         }
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,

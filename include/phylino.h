@@ -126,8 +126,9 @@ PHYLINO_API phylino_status phylino_set_model(phylino_ctx *ctx, const phylino_mod
  *   core      [n] reactor-core index in [0, n_cores), NULL => 0       (R13)
  *   baseline_m[n_cores] L in metres (finite, >= 0)
  *   edges     [n_bins+1] strictly ascending reco-energy bin edges; n_bins must equal the model's.
- * The store is structure-of-arrays, sorted by reconstructed energy ("sorted according
- * to their energy"; R14): x = L_core/E_nu and w as fp64, E_vis as fp32.
+ * The store is sorted by reconstructed energy ("sorted according to their energy";
+ * R14) and cut into 96-byte records of 4 events: x = L_core/E_nu and w as fp64, E_vis as fp32
+ * (DESIGN.md "Event store").
  * n = 0 is allowed (empty dataset).  Reloading a dataset replaces it. */
 PHYLINO_API phylino_status phylino_load_events(phylino_ctx *ctx, int dataset, int64_t n,
                                    const float *e_nu_MeV, const float *e_vis_MeV, const float *weight,
@@ -166,11 +167,12 @@ PHYLINO_API phylino_status phylino_spectra_host(phylino_ctx *ctx, int P, const d
 PHYLINO_API int64_t phylino_total_bins(const phylino_ctx *ctx);     /* sum_d n_bins, 0 before set_model */
 PHYLINO_API int64_t phylino_total_events(const phylino_ctx *ctx);   /* sum_d n over loaded datasets */
 
-/* Tuning knobs (0 => library default).  slice_events: events a warp walks for every group of 32
- * parameter points before it moves on (keeps the re-read events in L2); max_warps: cap on the warps
- * of the persistent grid of the spectra kernel.  Results are bit-identical from call to call for
- * fixed knobs; other values regroup the fp64 partial sums (rounding-level differences only). */
-PHYLINO_API phylino_status phylino_set_tuning(phylino_ctx *ctx, int slice_events, int max_warps);
+/* Tuning knobs (0 => library default).  unit_events: events per unit of the event store;
+ * chunk_groups: groups of 32 parameter points per work item (a warp of the spectra kernel walks one
+ * unit for every group of an item, then claims the next item); max_warps: cap on the warps of the
+ * persistent grid.  Results are bit-identical from call to call for fixed knobs; other values
+ * regroup the fp64 partial sums (rounding-level differences only). */
+PHYLINO_API phylino_status phylino_set_tuning(phylino_ctx *ctx, int unit_events, int chunk_groups, int max_warps);
 
 /* Device timing of the three kernels of a call (CUDA events on the context's stream, recorded
  * around the setup, spectra and finalize kernels of every later call).  phylino_last_kernel_ms

@@ -96,7 +96,7 @@ def load_library():
     lib.phylino_total_events.restype = i64
     lib.phylino_total_events.argtypes = [vp]
     lib.phylino_set_tuning.restype = i32
-    lib.phylino_set_tuning.argtypes = [vp, i32, i32]
+    lib.phylino_set_tuning.argtypes = [vp, i32, i32, i32]
     lib.phylino_launch_count.restype = i64
     lib.phylino_launch_count.argtypes = [vp]
     lib.phylino_last_error.restype = C.c_char_p
@@ -237,8 +237,8 @@ class Phylino:
     def launch_count(self) -> int:
         return int(self._lib.phylino_launch_count(self._ctx))
 
-    def set_tuning(self, slice_events: int = 0, max_warps: int = 0):
-        self._check(self._lib.phylino_set_tuning(self._ctx, int(slice_events), int(max_warps)))
+    def set_tuning(self, unit_events: int = 0, chunk_groups: int = 0, max_warps: int = 0):
+        self._check(self._lib.phylino_set_tuning(self._ctx, int(unit_events), int(chunk_groups), int(max_warps)))
 
     # -- phylino_spectra / phylino_nll / phylino_event_bins (device buffers, asynchronous) -------
     def spectra(self, params, out=None):

@@ -63,8 +63,8 @@ template <class T> cudaError_t upload(T **dst, const std::vector<T> &src, cudaSt
 
 void free_events(phylino_dataset_host &d)
 {
-    cudaFree(d.d_x); cudaFree(d.d_v); cudaFree(d.d_w); cudaFree(d.d_wsum); cudaFree(d.d_edges); cudaFree(d.d_perm);
-    d.d_x = nullptr; d.d_v = nullptr; d.d_w = nullptr; d.d_wsum = nullptr; d.d_edges = nullptr; d.d_perm = nullptr;
+    cudaFree(d.d_ev); cudaFree(d.d_edges); cudaFree(d.d_perm);
+    d.d_ev = nullptr; d.d_edges = nullptr; d.d_perm = nullptr;
     d.loaded = false; d.n = d.n_pad = 0;
 }
 
@@ -85,8 +85,8 @@ void free_all(phylino_ctx *c)
     free_tables(c);
     cudaFree(c->d_acc); cudaFree(c->d_flags);
     c->d_acc = nullptr; c->d_flags = nullptr; c->acc_capacity = 0;
-    cudaFree(c->d_rec); cudaFree(c->d_thr); cudaFree(c->d_safe);
-    c->d_rec = nullptr; c->d_thr = nullptr; c->d_safe = nullptr; c->point_capacity = 0;
+    cudaFree(c->d_rec); cudaFree(c->d_thr); cudaFree(c->d_safe); cudaFree(c->d_counter);
+    c->d_rec = nullptr; c->d_thr = nullptr; c->d_safe = nullptr; c->d_counter = nullptr; c->point_capacity = 0;
     cudaFree(c->d_stage); c->d_stage = nullptr;
     if (c->h_pin) cudaFreeHost(c->h_pin);
     c->h_pin = nullptr; c->stage_capacity = 0;
@@ -127,6 +127,10 @@ phylino_status ensure_acc(phylino_ctx *ctx, int P)
         CU(cudaMemsetAsync(ctx->d_flags, 0, need * sizeof(unsigned), ctx->stream));
         ctx->acc_capacity = need;
     }
+    if (!ctx->d_counter) {
+        CU(cudaMalloc((void **)&ctx->d_counter, sizeof(unsigned)));
+        CU(cudaMemsetAsync(ctx->d_counter, 0, sizeof(unsigned), ctx->stream));
+    }
     if (P > ctx->point_capacity) {
         /* per-point records and threshold rows written by the setup kernel of every call */
         CU(cudaStreamSynchronize(ctx->stream));
@@ -144,22 +148,19 @@ phylino_status ensure_acc(phylino_ctx *ctx, int P)
 /* fill the by-value kernel arguments that do not depend on the batch */
 void fill_datasets(const phylino_ctx *ctx, SpectraArgs &a)
 {
-    int64_t batches = 0;
     for (int d = 0; d < ctx->n_datasets; ++d) {
         const phylino_dataset_host &h = ctx->ds[d];
         DatasetDev &v = a.ds[d];
-        v.x = h.d_x; v.w = h.d_w; v.v = h.d_v; v.wsum = h.d_wsum; v.edges = h.d_edges;
+        v.ev = h.d_ev; v.edges = h.d_edges;
         v.n_bins = h.n_bins;
         v.bin_off = d == 0 ? 0 : a.ds[d - 1].bin_off + a.ds[d - 1].n_bins;
         v.thr_off = v.bin_off + d;
         v.per_point = (h.idx_a[0] >= 0 || h.idx_a[1] >= 0 || h.idx_a[2] >= 0) ? 1 : 0;
-        v.batch_begin = (int32_t)batches;
         v.n_batches = (int32_t)(h.n_pad / EB);
         for (int j = 0; j < 3; ++j) v.idx_a[j] = h.idx_a[j];
         v.v_pos_min = h.v_pos_min;
         v.v_max = h.v_max;
         v.fx_scale = std::ldexp(1.0, h.fx_exp);
-        batches += h.n_pad / EB;
     }
     a.osc.osc_model = ctx->osc_model;
     a.osc.ordering = ctx->ordering;
@@ -168,51 +169,72 @@ void fill_datasets(const phylino_ctx *ctx, SpectraArgs &a)
     a.n_params = ctx->n_params;
     a.total_bins = ctx->total_bins;
     a.thr_stride = ctx->total_bins + ctx->n_datasets;
-    a.n_batches = (int32_t)batches;
     a.rec = ctx->d_rec;
     a.thr = ctx->d_thr;
     a.safe = ctx->d_safe;
     a.acc = ctx->d_acc;
     a.flags = ctx->d_flags;
+    a.counter = ctx->d_counter;
 }
 
+/* Cut of the batch into work items (spectra.cu): U batches per unit, G point groups per item.
+ * Aim: about 24 items per resident warp (dynamic balance, short tail) of at least 16 batch-groups
+ * each (the per-item cost -- first bin search, one flush per point -- stays a few percent). */
 void fill_batch(const phylino_ctx *ctx, SpectraArgs &a, int P, const double *params)
 {
     a.P = P;
     a.params = params;
     a.thr_rows = ctx->per_point_binning ? P : 1;
-    const int slice_events = ctx->slice_events > 0 ? ctx->slice_events : 512;
-    a.slice_batches = std::max(1, slice_events / EB);
-}
-
-/* Warps of the persistent grid: all the chip holds at once, fewer while a lane's sub-stream would
- * get less than two batches (tiny inputs are launch-latency bound anyway). */
-int choose_warps(const phylino_ctx *ctx, int P, int64_t batches)
-{
-    int streams = 1;                                   /* sub-streams per warp of the (only) point group */
+    const int64_t n_groups = (P + 31) / 32;
+    int streams = 1;                                    /* sub-streams per warp when P < 32 */
     if (P < 32) { int pl = 1; while (pl < P) pl <<= 1; streams = 32 / pl; }
-    int64_t w = std::max<int64_t>(1, batches / (2 * streams));
-    int cap = ctx->resident_warps;
-    if (ctx->max_warps > 0) cap = std::min(cap, ctx->max_warps);
-    return (int)std::min<int64_t>(w, std::max(cap, 1));
+    int64_t batches = 0;
+    for (int d = 0; d < ctx->n_datasets; ++d) batches += ctx->ds[d].n_pad / EB;
+    int cap = std::max(ctx->resident_warps, WARPS);
+    if (ctx->max_warps > 0) cap = std::max(WARPS, std::min(cap, ctx->max_warps / WARPS * WARPS));
+    const int64_t work = std::max<int64_t>(1, batches * n_groups / (24ll * cap));
+    int64_t U = 16;
+    while (U < 64 && U * 2 <= work) U *= 2;
+    U = std::max<int64_t>(U, 4 * streams);
+    if (ctx->unit_events > 0) U = std::max(1, ctx->unit_events / EB);
+    int64_t G = std::max<int64_t>(1, std::min<int64_t>(std::min<int64_t>(work, 512) / U, n_groups));
+    if (ctx->chunk_groups > 0) G = std::min<int64_t>(ctx->chunk_groups, n_groups);
+    int64_t units, chunks;
+    for (;;) {
+        units = 0;
+        for (int d = 0; d < ctx->n_datasets; ++d) {
+            a.ds[d].unit_begin = (int32_t)units;
+            units += (ctx->ds[d].n_pad / EB + U - 1) / U;
+        }
+        chunks = (n_groups + G - 1) / G;
+        if (units * chunks < (1ll << 31) - 2ll * cap) break;
+        if (G < n_groups) G *= 2; else U *= 2;          /* keep items and tickets inside 32 bits */
+    }
+    a.unit_batches = (int32_t)U;
+    a.chunk_groups = (int32_t)G;
+    a.n_units = (int32_t)units;
+    a.n_chunks = (int32_t)chunks;
+    a.n_items = (int32_t)(units * chunks);
+    const int64_t warps = std::min<int64_t>(cap, (a.n_items + WARPS - 1) / WARPS * WARPS);
+    a.n_warps = (int32_t)std::max<int64_t>(warps, WARPS);
 }
 
 /* enqueue the setup and spectra kernels (rows a1-a4) for P points */
 phylino_status enqueue_spectra(phylino_ctx *ctx, int P, const double *params)
 {
+    if (ctx->resident_warps == 0)
+        CU(spectra_max_warps(ctx->n_terms, ctx->sm_count, &ctx->resident_warps));
     SpectraArgs a{};
     fill_datasets(ctx, a);
     fill_batch(ctx, a, P, params);
-    if (ctx->resident_warps == 0)
-        CU(spectra_max_warps(ctx->n_terms, ctx->sm_count, &ctx->resident_warps));
     if (ctx->timing) CU(cudaEventRecord(ctx->ev[0], ctx->stream));
-    if (a.n_batches > 0 && P > 0) {
+    if (a.n_items > 0 && P > 0) {
         CU(launch_setup(a, ctx->n_terms, ctx->stream));
         ctx->launches += 1;
     }
     if (ctx->timing) CU(cudaEventRecord(ctx->ev[1], ctx->stream));
-    if (a.n_batches > 0 && P > 0) {
-        CU(launch_spectra(a, ctx->n_terms, choose_warps(ctx, P, a.n_batches), ctx->stream));
+    if (a.n_items > 0 && P > 0) {
+        CU(launch_spectra(a, ctx->n_terms, ctx->stream));
         ctx->launches += 1;
     }
     return PHYLINO_OK;
@@ -433,20 +455,24 @@ phylino_status phylino_load_events(phylino_ctx *ctx, int dataset, int64_t n, con
         return x < y;
     });
     const int64_t n_pad = (n + EB - 1) / EB * EB;
-    std::vector<double> x((size_t)n_pad, 0.0), w((size_t)n_pad, 0.0), ws((size_t)(n_pad / EB), 0.0);
-    std::vector<float> v((size_t)n_pad, std::nanf(""));
+    EventBatch blank{};
+    for (int j = 0; j < EB; ++j) blank.v[j] = std::nanf("");
+    std::vector<EventBatch> ev((size_t)(n_pad / EB), blank);
     double wsum = 0.0;
     float v_pos_min = INFINITY, v_max = -INFINITY;
     for (int64_t i = 0; i < n; ++i) {
         int32_t s = perm[i];
-        x[i] = baseline_m[core ? core[s] : 0] / (double)e_nu[s];
-        v[i] = e_vis[s];
-        w[i] = weight ? (double)weight[s] : 1.0;
-        ws[i / EB] += w[i];                     /* in event order: the batch total the hot kernel adds */
-        wsum += std::fabs(w[i]);
-        if (std::isfinite(v[i])) {
-            if (v[i] > 0.0f && v[i] < v_pos_min) v_pos_min = v[i];
-            if (v[i] > v_max) v_max = v[i];
+        EventBatch &b = ev[(size_t)(i / EB)];
+        const int j = (int)(i % EB);
+        const float vi = e_vis[s];
+        b.x[j] = baseline_m[core ? core[s] : 0] / (double)e_nu[s];
+        b.v[j] = vi;
+        b.w[j] = weight ? (double)weight[s] : 1.0;
+        b.wsum += b.w[j];                       /* in event order: the batch total the hot kernel adds */
+        wsum += std::fabs(b.w[j]);
+        if (std::isfinite(vi)) {
+            if (vi > 0.0f && vi < v_pos_min) v_pos_min = vi;
+            if (vi > v_max) v_max = vi;
         }
     }
     /* fixed-point scale 2^e with 8 * sum|w| * 2^e <= 2^62 (|P_ee| <= 4 is enforced per point) */
@@ -459,10 +485,7 @@ phylino_status phylino_load_events(phylino_ctx *ctx, int dataset, int64_t n, con
     free_events(h);
     cudaStream_t st = ctx->stream;
     std::vector<double> ed(edges, edges + n_bins + 1);
-    CU(upload(&h.d_x, x, st));
-    CU(upload(&h.d_v, v, st));
-    CU(upload(&h.d_w, w, st));
-    CU(upload(&h.d_wsum, ws, st));
+    CU(upload(&h.d_ev, ev, st));
     CU(upload(&h.d_edges, ed, st));
     CU(upload(&h.d_perm, perm, st));
     double inv = std::ldexp(1.0, -fx);
@@ -514,7 +537,7 @@ phylino_status phylino_event_bins(phylino_ctx *ctx, int P, const double *params,
     SpectraArgs a{};
     fill_datasets(ctx, a);
     fill_batch(ctx, a, P, params);
-    if (a.n_batches > 0) {                      /* the threshold rows the hot kernel would use */
+    if (a.n_items > 0) {                        /* the threshold rows the hot kernel would use */
         CU(launch_setup(a, ctx->n_terms, ctx->stream));
         ctx->launches += 1;
     }
@@ -578,11 +601,12 @@ int64_t phylino_total_events(const phylino_ctx *ctx)
     return t;
 }
 
-phylino_status phylino_set_tuning(phylino_ctx *ctx, int slice_events, int max_warps)
+phylino_status phylino_set_tuning(phylino_ctx *ctx, int unit_events, int chunk_groups, int max_warps)
 {
     if (!ctx) return PHYLINO_ERR_ARG;
-    if (slice_events < 0 || max_warps < 0) return fail(ctx, PHYLINO_ERR_ARG, "negative tuning value");
-    ctx->slice_events = slice_events;
+    if (unit_events < 0 || chunk_groups < 0 || max_warps < 0) return fail(ctx, PHYLINO_ERR_ARG, "negative tuning value");
+    ctx->unit_events = unit_events;
+    ctx->chunk_groups = chunk_groups;
     ctx->max_warps = max_warps;
     return PHYLINO_OK;
 }

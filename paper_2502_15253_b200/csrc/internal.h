@@ -16,9 +16,10 @@
 namespace phylino {
 
 /* ---- layout of the event store and of a launch -------------------------------------------------
- * The events of a dataset, sorted by E_vis, are cut into batches of EB consecutive events; a warp
- * owns a contiguous range of batches and walks it once per group of 32 parameter points, ONE
- * POINT PER LANE (spectra.cu). */
+ * The events of a dataset, sorted by E_vis, are cut into batches of EB consecutive events, one
+ * 96-byte record each; `unit_batches` consecutive batches form a unit.  A work item is one unit x
+ * `chunk_groups` groups of 32 parameter points; the warps of a persistent grid claim items from a
+ * global counter and walk the unit once per group, ONE POINT PER LANE (spectra.cu). */
 constexpr int EB          = 4;                      /* events per batch; every dataset is padded to a multiple */
 constexpr int WARPS       = 4;                      /* warps per CTA of the spectra kernel */
 constexpr int MAX_TERMS   = 3;
@@ -27,19 +28,26 @@ constexpr int SETUP_THREADS = 128;
 /* flag bits of a (point, bin) accumulator whose value left the fixed-point domain */
 enum : unsigned { FLAG_NAN = 1u, FLAG_PINF = 2u, FLAG_NINF = 4u };
 
+/* EB consecutive events of the E_vis-sorted store: everything the hot loop reads, behind one pointer */
+struct __align__(16) EventBatch {
+    double x[EB];           /* L_core/E_nu  [m/MeV], fp64 (phase range reduction needs it) */
+    double w[EB];           /* MC weight as fp64 (exact copy of the fp32 input); padding = 0 */
+    float  v[EB];           /* E_vis [MeV]; padding = NaN */
+    double wsum;            /* w[0] + ... + w[EB-1], summed in that order */
+    double reserved;
+};
+static_assert(sizeof(EventBatch) == 96, "EventBatch is read with fixed 16-byte offsets");
+
 /* Per-dataset entry of the table that travels by value in the kernel parameters. */
 struct DatasetDev {
-    const double *x;        /* [n_pad] L_core/E_nu  [m/MeV], fp64 (phase range reduction needs it) */
-    const double *w;        /* [n_pad] MC weight as fp64 (exact copy of the fp32 input); padding = 0 */
-    const float  *v;        /* [n_pad] E_vis [MeV]; padding = NaN */
-    const double *wsum;     /* [n_pad / EB] sum of the weights of a batch */
+    const EventBatch *ev;   /* [n_batches] */
     const double *edges;    /* [n_bins+1] */
     int32_t n_bins;
     int32_t bin_off;        /* offset of this dataset inside a point's total_bins */
     int32_t thr_off;        /* offset of this dataset inside a threshold row: sum of (n_bins+1) before it */
     int32_t per_point;      /* the energy scale of this dataset depends on theta */
-    int32_t batch_begin;    /* first global batch of this dataset */
     int32_t n_batches;
+    int32_t unit_begin;     /* first global unit of this dataset (units never straddle datasets) */
     int32_t idx_a[3];       /* energy-scale indices into theta, -1 => (0,1,0) */
     float   v_pos_min;      /* smallest positive finite E_vis of the dataset (+inf if none) */
     float   v_max;          /* largest finite E_vis (-inf if none) */
@@ -61,8 +69,13 @@ struct SpectraArgs {
     int32_t n_datasets;
     int32_t n_params;
     int32_t P;              /* points in the batch */
-    int32_t n_batches;      /* event batches over all datasets */
-    int32_t slice_batches;  /* batches a warp walks for all point groups before moving on */
+    int32_t n_units;        /* units over all datasets */
+    int32_t unit_batches;   /* U: batches per unit (the last unit of a dataset may be shorter) */
+    int32_t chunk_groups;   /* G: point groups per work item */
+    int32_t n_chunks;       /* ceil(n_groups / G) */
+    int32_t n_items;        /* n_units x n_chunks; item = unit * n_chunks + chunk */
+    int32_t n_warps;        /* warps of the persistent grid (a multiple of WARPS) */
+    unsigned *counter;      /* DEVICE work counter; the setup kernel sets it to 2 n_warps */
     int32_t thr_stride;     /* floats per threshold row: total_bins + n_datasets */
     int32_t thr_rows;       /* P if some dataset's energy scale depends on theta, else 1 */
     int32_t total_bins;
@@ -99,7 +112,7 @@ struct FinalizeArgs {
 /* kernel launchers (spectra.cu, finalize.cu, peaks.cu) */
 cudaError_t launch_setup(const SpectraArgs &a, int S, cudaStream_t st);
 cudaError_t spectra_max_warps(int S, int sm_count, int *warps);
-cudaError_t launch_spectra(const SpectraArgs &a, int S, int n_warps, cudaStream_t st);
+cudaError_t launch_spectra(const SpectraArgs &a, int S, cudaStream_t st);
 cudaError_t launch_finalize(const FinalizeArgs &a, int mode /*0 H, 1 mu, 2 nll*/, cudaStream_t st);
 cudaError_t launch_event_bins(const SpectraArgs &a, int d, const int32_t *perm, long long n, long long ev_off,
                               long long total_events, int32_t *bins, cudaStream_t st);
@@ -123,8 +136,7 @@ struct phylino_dataset_host {
     double   wsum_abs = 0.0;
     float    v_pos_min = 0.f, v_max = 0.f;
     int      fx_exp = 0;
-    double  *d_x = nullptr, *d_w = nullptr, *d_wsum = nullptr;
-    float   *d_v = nullptr;
+    phylino::EventBatch *d_ev = nullptr;
     double  *d_edges = nullptr;
     int32_t *d_perm = nullptr;
 };
@@ -155,8 +167,9 @@ struct phylino_ctx {
     /* host-buffer entry points: pinned + device staging */
     double *h_pin = nullptr, *d_stage = nullptr;
     int64_t stage_capacity = 0;                    /* doubles */
+    unsigned *d_counter = nullptr;                 /* work counter of the spectra kernel */
     /* tuning knobs, 0 => default (phylino_set_tuning) */
-    int slice_events = 0, max_warps = 0;
+    int unit_events = 0, chunk_groups = 0, max_warps = 0;
     int resident_warps = 0;                        /* warps of the spectra kernel the chip holds at once */
     /* optional device timing of the three kernels of a call (phylino_set_timing) */
     bool timing = false;

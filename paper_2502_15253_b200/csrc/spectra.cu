@@ -2,14 +2,16 @@
  * spectra.cu -- the batched oscillation-weight + histogram kernels (
  * PAPER.md:177 signal step 1, :183 "the most time-demanding computational step").
  *
- * Layout of the work: ONE PARAMETER POINT PER LANE.  The E_vis-sorted events of all datasets are cut
- * into batches of EB events and the batches into equal contiguous ranges, one per warp of a
- * persistent grid (no tail wave).  A warp walks its range once per group of 32 points: the event
- * data (x = L/E, w, E_vis) are warp-uniform broadcast loads, everything that depends on the point
- * (half-turn coefficients h_k, the run accumulators, the current bin and its fp32 upper threshold)
- * lives in the lane's registers.  No shared memory, no shuffles, no barriers.  A last group of
- * fewer than 32 points splits the warp's range into 32/PL sub-streams (PL = points rounded up to
- * a power of two), so that a batch of 1 point still uses all 32 lanes (event-parallel).
+ * Layout of the work: ONE PARAMETER POINT PER LANE.  The E_vis-sorted events of a dataset are cut
+ * into 96-byte batches of EB events and the batches into units; a work item is one unit x a chunk
+ * of point groups (32 points each).  The warps of a persistent grid claim items from a global
+ * counter (dynamic balance: units that contain bin edges cost more) and walk the unit once per
+ * group: the event data (x = L/E, w, E_vis) are warp-uniform broadcast loads from one pointer,
+ * everything that depends on the point (half-turn coefficients h_k, the run accumulators, the
+ * current bin and its fp32 upper threshold) lives in the lane's registers.  No shared memory, no
+ * shuffles in the loop, no barriers.  The next item's unit is prefetched into L2 while the current
+ * one is walked.  A group of fewer than 32 points splits the unit into 32/PL sub-streams (PL =
+ * points rounded up to a power of two), so that a batch of 1 point still uses all 32 lanes.
  *
  * Oscillation weight (row a2).  P_ee = P0 + sum_k A_k g_k with g = 1/2 cos(2 phase) (devmath.cuh):
  * the lane accumulates C_k = sum_e w_e g_k(e) and W = sum_e w_e over a run of events that share a
@@ -25,10 +27,11 @@
  * batch.  Events outside the interval on which a table is proven (and points that fail the
  * monotonicity check) take the per-event fp64 map.
  *
- * Histogram (rows a4, a5).  When a run ends (bin edge, end of the slice) its fp64 total is converted
+ * Histogram (rows a4, a5).  When a run ends (bin edge, end of the unit) its fp64 total is converted
  * once to 64-bit fixed point and added to the (point, bin) accumulator with an integer RED.
- * Integer addition is associative: the result does not depend on which warp arrives first, i.e.
- * bitwise reproducible with no float atomics anywhere.
+ * Integer addition is associative: the result depends neither on which warp walks an item nor on
+ * the order of arrival, i.e. bitwise reproducible with no float atomics anywhere (the cut of the
+ * events into items is a function of the sizes only).
  */
 #include "devmath.cuh"
 
@@ -104,6 +107,7 @@ __global__ void __launch_bounds__(SETUP_THREADS) setup_kernel(const __grid_const
 {
     if ((int)blockIdx.x < rec_blocks) {
         const int p = blockIdx.x * SETUP_THREADS + threadIdx.x;
+        if (p == 0) *a.counter = 2u * (unsigned)a.n_warps;     /* see spectra_kernel */
         if (p >= a.P) return;
         const double *theta = a.params + (size_t)p * a.n_params;
         double A[MAX_TERMS], dm2[MAX_TERMS];
@@ -186,10 +190,10 @@ __device__ __forceinline__ void flush_run(const SpectraArgs &a, const DatasetDev
     r.W = 0.0;
 }
 
-/* One warp, batches [b0, b1) of dataset ds, point group g (points 32 g ... 32 g + 31). */
+/* One warp, batches [b0, b1) of dataset ds (one unit), point group g (points 32 g ... 32 g + 31). */
 template <int S>
-__device__ __forceinline__ void walk_slice(const SpectraArgs &a, const DatasetDev &ds, int d, int b0, int b1, int g,
-                                           int lane)
+__device__ __forceinline__ void walk_unit(const SpectraArgs &a, const DatasetDev &ds, int d, int b0, int b1, int g,
+                                          int lane)
 {
     /* lane -> (point, sub-stream): a group of np < 32 points uses PL = 2^ceil(log2 np) point lanes
      * and splits the batches into NS = 32 / PL contiguous sub-streams */
@@ -201,8 +205,8 @@ __device__ __forceinline__ void walk_slice(const SpectraArgs &a, const DatasetDe
     const bool active = pl < np;
     const int p = 32 * g + (active ? pl : 0);
     const int nb = b1 - b0;
-    const int my0 = b0 + (int)((long long)nb * s / NS), my1 = b0 + (int)((long long)nb * (s + 1) / NS);
-    const int iters = (nb + NS - 1) / NS;                  /* >= my1 - my0 for every lane */
+    const int my0 = b0 + nb * s / NS, mine = b0 + nb * (s + 1) / NS - my0;
+    const int iters = (nb + NS - 1) / NS;                  /* >= mine for every lane */
 
     double h[S];
 #pragma unroll
@@ -210,7 +214,7 @@ __device__ __forceinline__ void walk_slice(const SpectraArgs &a, const DatasetDe
     const int row = a.thr_rows > 1 ? p : 0;
     const float *thr = a.thr + (size_t)row * a.thr_stride + ds.thr_off;
     const float2 safe = a.safe[(size_t)row * a.n_datasets + d];
-    const double *theta = a.params + (size_t)p * a.n_params;
+    const int B = ds.n_bins;
 
     Run<S> r;
 #pragma unroll
@@ -219,23 +223,21 @@ __device__ __forceinline__ void walk_slice(const SpectraArgs &a, const DatasetDe
     r.cur = -1;
     r.hi = -pos_inf();
 
+    const EventBatch *bp = ds.ev + my0;
 #pragma unroll 1
-    for (int i = 0; i < iters; ++i) {
-        const int bi = my0 + i;
-        if (bi >= my1) continue;
-        const size_t e0 = (size_t)bi * EB;
+    for (int i = 0; i < iters; ++i, ++bp) {
+        if (i >= mine) continue;
         double x[EB], w[EB];
         {
-            const double2 *xp = reinterpret_cast<const double2 *>(ds.x + e0);
-            const double2 *wp = reinterpret_cast<const double2 *>(ds.w + e0);
+            const double2 *q = reinterpret_cast<const double2 *>(bp);
 #pragma unroll
             for (int j = 0; j < EB / 2; ++j) {
-                double2 t = __ldg(xp + j), u = __ldg(wp + j);
+                double2 t = __ldg(q + j), u = __ldg(q + EB / 2 + j);
                 x[2 * j] = t.x; x[2 * j + 1] = t.y;
                 w[2 * j] = u.x; w[2 * j + 1] = u.y;
             }
         }
-        const float v_last = __ldg(ds.v + e0 + EB - 1);
+        const float v_last = __ldg(&bp->v[EB - 1]);
 
         /* row a2: g_k of every event of the batch */
         double gk[S][EB];
@@ -250,16 +252,24 @@ __device__ __forceinline__ void walk_slice(const SpectraArgs &a, const DatasetDe
             for (int j = 0; j < EB; ++j)
 #pragma unroll
                 for (int k = 0; k < S; ++k) r.C[k] = fma(w[j], gk[k][j], r.C[k]);
-            r.W += __ldg(ds.wsum + bi);
+            r.W += __ldg(&bp->wsum);
         } else {
             /* a run ends inside the batch (or none is open yet): walk its events one by one */
-            const float4 v4 = __ldg(reinterpret_cast<const float4 *>(ds.v + e0));
+            const float4 v4 = __ldg(reinterpret_cast<const float4 *>(bp->v));
             const float v[EB] = {v4.x, v4.y, v4.z, v4.w};
 #pragma unroll
             for (int j = 0; j < EB; ++j) {
                 if (!(v[j] < r.hi)) {
+                    int b;
                     float nhi;
-                    const int b = locate_bin(ds, thr, safe, theta, v[j], nhi);
+                    if (r.hi > -pos_inf() && r.hi < pos_inf() && v[j] <= safe.y) {
+                        /* r.hi = thr[cur + 1] <= v inside the table's interval: scan forward */
+                        b = r.cur + 1;
+                        nhi = b < B ? __ldg(thr + b + 1) : pos_inf();
+                        while (!(v[j] < nhi)) { ++b; nhi = b < B ? __ldg(thr + b + 1) : pos_inf(); }
+                    } else {
+                        b = locate_bin(ds, thr, safe, a.params + (size_t)p * a.n_params, v[j], nhi);
+                    }
                     if (b != r.cur) {
                         flush_run<S>(a, ds, p, active, r);
                         r.cur = b;
@@ -275,37 +285,63 @@ __device__ __forceinline__ void walk_slice(const SpectraArgs &a, const DatasetDe
     flush_run<S>(a, ds, p, active, r);
 }
 
+/* lane 0 takes the next ticket of the work counter; the value is needed one item later */
+__device__ __forceinline__ unsigned take_ticket(unsigned *counter, int lane)
+{
+    unsigned t = 0;
+    if (lane == 0) t = atomicAdd(counter, 1u);
+    return t;
+}
+
+/* item -> (dataset, batches [b0, b1), chunk) */
+__device__ __forceinline__ void decode_item(const SpectraArgs &a, unsigned item, int &d, int &b0, int &b1, int &chunk)
+{
+    const int unit = (int)(item / (unsigned)a.n_chunks);
+    chunk = (int)(item - (unsigned)unit * (unsigned)a.n_chunks);
+    d = 0;
+    for (int i = 1; i < a.n_datasets; ++i)
+        if (unit >= a.ds[i].unit_begin) d = i;
+    b0 = (unit - a.ds[d].unit_begin) * a.unit_batches;
+    b1 = min(b0 + a.unit_batches, a.ds[d].n_batches);
+}
+
 template <int S>
 __global__ void __launch_bounds__(WARPS * 32, 4) spectra_kernel(const __grid_constant__ SpectraArgs a)
 {
-    static_assert(EB == 4, "the batch loads below are written for EB = 4");
+    static_assert(EB == 4, "the batch loads are written for EB = 4");
     const int lane = threadIdx.x & 31;
-    const long long nW = (long long)gridDim.x * WARPS;
-    const long long gw = (long long)blockIdx.x * WARPS + (threadIdx.x >> 5);
-    /* this warp's equal share of the batches of all datasets */
-    const long long B0 = gw * a.n_batches / nW, B1 = (gw + 1) * a.n_batches / nW;
-    if (B0 >= B1) return;
+    const unsigned nW = gridDim.x * WARPS;
     const int n_groups = (a.P + 31) >> 5;
-    /* with several point groups the range is walked in slices that stay in L2 between groups */
-    const int slice = n_groups > 1 ? a.slice_batches : 0x7fffffff;
+    const unsigned n_items = (unsigned)a.n_items;
+    /* the first two items of a warp are static, later ones come from the counter (which the setup
+     * kernel left at 2 nW): warps that meet expensive units (bin edges) simply claim fewer */
+    unsigned cur = blockIdx.x * WARPS + (threadIdx.x >> 5), nxt = cur + nW;
 #pragma unroll 1
-    for (int d = 0; d < a.n_datasets; ++d) {
-        const DatasetDev &ds = a.ds[d];
-        const long long db = ds.batch_begin;
-        const long long s0 = max(B0, db) - db, s1 = min(B1, db + ds.n_batches) - db;
-#pragma unroll 1
-        for (long long sb = s0; sb < s1; sb += slice) {
-            const int se = (int)min(sb + slice, s1);
-#pragma unroll 1
-            for (int g = 0; g < n_groups; ++g) walk_slice<S>(a, ds, d, (int)sb, se, g, lane);
+    while (cur < n_items) {
+        const unsigned ticket = take_ticket(a.counter, lane);
+        int d, b0, b1, chunk;
+        decode_item(a, cur, d, b0, b1, chunk);
+        if (nxt < n_items && nxt / (unsigned)a.n_chunks != cur / (unsigned)a.n_chunks) {
+            /* pull the next unit towards the SM while this one is being walked */
+            int nd, nb0, nb1, nc;
+            decode_item(a, nxt, nd, nb0, nb1, nc);
+            const char *base = reinterpret_cast<const char *>(a.ds[nd].ev + nb0);
+            const int bytes = (nb1 - nb0) * (int)sizeof(EventBatch);
+            for (int o = lane * 128; o < bytes; o += 32 * 128)
+                asm volatile("prefetch.global.L2 [%0];" ::"l"(base + o));
         }
+        const DatasetDev &ds = a.ds[d];
+        const int g1 = min((chunk + 1) * a.chunk_groups, n_groups);
+#pragma unroll 1
+        for (int g = chunk * a.chunk_groups; g < g1; ++g) walk_unit<S>(a, ds, d, b0, b1, g, lane);
+        cur = nxt;
+        nxt = __shfl_sync(0xffffffffu, ticket, 0);
     }
 }
 
-template <int S> cudaError_t launch_t(const SpectraArgs &a, int n_warps, cudaStream_t st)
+template <int S> cudaError_t launch_t(const SpectraArgs &a, cudaStream_t st)
 {
-    const int grid = (n_warps + WARPS - 1) / WARPS;
-    spectra_kernel<S><<<grid, WARPS * 32, 0, st>>>(a);
+    spectra_kernel<S><<<a.n_warps / WARPS, WARPS * 32, 0, st>>>(a);
     return cudaGetLastError();
 }
 
@@ -335,11 +371,11 @@ cudaError_t launch_setup(const SpectraArgs &a, int S, cudaStream_t st)
     return cudaGetLastError();
 }
 
-/* persistent grid of n_warps warps (a multiple of WARPS is used), each with an equal range of batches */
-cudaError_t launch_spectra(const SpectraArgs &a, int S, int n_warps, cudaStream_t st)
+/* persistent grid of a.n_warps warps (a multiple of WARPS) that claim the a.n_items work items */
+cudaError_t launch_spectra(const SpectraArgs &a, int S, cudaStream_t st)
 {
-    if (a.n_batches <= 0 || a.P <= 0 || n_warps <= 0) return cudaSuccess;
-    return S == 2 ? launch_t<2>(a, n_warps, st) : launch_t<3>(a, n_warps, st);
+    if (a.n_items <= 0 || a.P <= 0 || a.n_warps < WARPS) return cudaSuccess;
+    return S == 2 ? launch_t<2>(a, st) : launch_t<3>(a, st);
 }
 
 /* ---- diagnostic: bin index of every event at every point (bit-exact parity of row a3) ----
@@ -357,7 +393,7 @@ __global__ void __launch_bounds__(256) event_bins_kernel(const __grid_constant__
     const int row = a.thr_rows > 1 ? p : 0;
     float hi;
     int b = locate_bin(ds, a.thr + (size_t)row * a.thr_stride + ds.thr_off, a.safe[(size_t)row * a.n_datasets + d],
-                       a.params + (size_t)p * a.n_params, ds.v[i], hi);
+                       a.params + (size_t)p * a.n_params, ds.ev[i / EB].v[i % EB], hi);
     bins[(size_t)p * total_events + ev_off + perm[i]] = (b >= 0 && b < ds.n_bins) ? b : -1;
 }
 } // namespace

@@ -117,7 +117,7 @@ def test_bitwise_reproducible(gpu, oracle_mod):
     outs = {}
     with gpu.Phylino() as ph:
         ph.load_workload(wl)
-        for tun in ((0, 0), (0, 0), (64, 0), (0, 37), (4096, 1000), (0, 37), (64, 0), (0, 0)):
+        for tun in ((0, 0, 0), (0, 0, 0), (64, 0, 0), (0, 0, 37), (4096, 3, 1000), (0, 0, 37), (64, 0, 0), (0, 0, 0)):
             ph.set_tuning(*tun)
             outs.setdefault(tun, []).append((ph.spectra(dp).cpu().numpy(), ph.nll(dp, data).cpu().numpy()))
     torch.cuda.synchronize()
@@ -125,12 +125,12 @@ def test_bitwise_reproducible(gpu, oracle_mod):
     for tun, runs in outs.items():
         for h, n in runs[1:]:
             assert h.tobytes() == runs[0][0].tobytes() and n.tobytes() == runs[0][1].tobytes(), tun
-    # another slice length / grid changes which events a lane sums in fp64 before the (exact) integer
+    # another unit length / grid changes which events a lane sums in fp64 before the (exact) integer
     # accumulation: rounding-level differences only
     for tun, runs in outs.items():
-        assert np.allclose(runs[0][0], outs[(0, 0)][0][0], rtol=1e-13, atol=0)
-        assert np.allclose(runs[0][1], outs[(0, 0)][0][1], rtol=0, atol=1e-9)
-    outs = [(outs[(0, 0)][0][0].tobytes(), None)]
+        assert np.allclose(runs[0][0], outs[(0, 0, 0)][0][0], rtol=1e-13, atol=0)
+        assert np.allclose(runs[0][1], outs[(0, 0, 0)][0][1], rtol=0, atol=1e-9)
+    outs = [(outs[(0, 0, 0)][0][0].tobytes(), None)]
     # a second context on a permuted copy of the events gives the same bits: the fixed-point
     # accumulators do not depend on arrival order, the sort is by E_vis
     wl2 = workloads.make_config(2, scale=0.02, n_points=23)
