@@ -103,11 +103,14 @@ def physical_gpu_index(local: int) -> int:
     return local
 
 
-def traffic_from_profile():
-    """dram bytes per launch of the spectra kernel from the committed ncu capture, or None."""
-    p = os.path.join(ROOT, "profiles", "spectra_kernel_traffic.json")
+def traffic_from_profile(config: int):
+    """dram bytes (read + write) per launch of the spectra kernel for this config, from the committed
+    summary of the ncu --set full capture (profiles/spectra_kernel_traffic.csv), or None."""
+    import csv
+    p = os.path.join(ROOT, "profiles", "spectra_kernel_traffic.csv")
     try:
-        return json.load(open(p))["dram_bytes_per_launch"]
+        rows = [r for r in csv.DictReader(open(p)) if int(r["config"]) == config]
+        return int(rows[-1]["dram_bytes_read"]) + int(rows[-1]["dram_bytes_write"])
     except Exception:
         return None
 
@@ -266,7 +269,7 @@ def main():
             measured_peak = None
         roofline = {
             "bound": "alu", "kernel": "spectra_kernel", "achieved": achieved / 1e9, "peak": PEAK_FP64_INST / 1e9,
-            "unit": "fp64 Ginst/s", "frac": achieved / PEAK_FP64_INST, "traffic": traffic_from_profile(),
+            "unit": "fp64 Ginst/s", "frac": achieved / PEAK_FP64_INST, "traffic": traffic_from_profile(args.config),
             "peak_source": "nominal: 64 fp64 lanes/clk/SM x 148 SMs x 1.965 GHz (DESIGN.md)",
             "measured_dfma_peak": None if measured_peak is None else measured_peak / 1e9,
             "frac_of_measured": None if not measured_peak else achieved / measured_peak,
