@@ -197,6 +197,7 @@ void fill_batch(const phylino_ctx *ctx, SpectraArgs &a, int P, const double *par
     while (U < 64 && U * 2 <= work) U *= 2;
     U = std::max<int64_t>(U, 4 * streams);
     if (ctx->unit_events > 0) U = std::max(1, ctx->unit_events / EB);
+    U = std::min<int64_t>(U, MAX_UNIT_BATCHES);         /* a unit must fit the warp's staging buffer */
     int64_t G = std::max<int64_t>(1, std::min<int64_t>(std::min<int64_t>(work, 512) / U, n_groups));
     if (ctx->chunk_groups > 0) G = std::min<int64_t>(ctx->chunk_groups, n_groups);
     int64_t units, chunks;

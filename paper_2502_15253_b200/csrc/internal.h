@@ -22,6 +22,7 @@ namespace phylino {
  * global counter and walk the unit once per group, ONE POINT PER LANE (spectra.cu). */
 constexpr int EB          = 4;                      /* events per batch; every dataset is padded to a multiple */
 constexpr int WARPS       = 4;                      /* warps per CTA of the spectra kernel */
+constexpr int MAX_UNIT_BATCHES = 64;                /* a unit is staged in shared memory: <= 6 KB */
 constexpr int MAX_TERMS   = 3;
 constexpr int SETUP_THREADS = 128;
 

@@ -41,6 +41,34 @@ namespace {
 
 __device__ __forceinline__ float pos_inf() { return __int_as_float(0x7f800000); }
 
+/* ---- per-warp staging of a unit in shared memory: one bulk async copy (TMA engine, no tensor map),
+ * completion signalled on an mbarrier that the 32 lanes poll.  (PTX ISA cp.async.bulk / mbarrier.) */
+__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(unsigned long long *bar, unsigned count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+
+/* lane 0 of the warp: expect `bytes` on `bar` and start the copy global -> shared */
+__device__ __forceinline__ void bulk_load(void *dst, const void *src, unsigned bytes, unsigned long long *bar)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+
+__device__ __forceinline__ void mbar_wait(unsigned long long *bar, unsigned parity)
+{
+    unsigned done;
+    do {
+        asm volatile("{\n\t.reg .pred p;\n\t"
+                     "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+                     "selp.u32 %0, 1, 0, p;\n\t}"
+                     : "=r"(done) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+    } while (!done);
+}
+
 /* run total -> fixed point; values outside the domain become flag bits */
 __device__ __forceinline__ long long to_fixed(double s, double scale, bool bad, unsigned &fl)
 {
@@ -190,10 +218,11 @@ __device__ __forceinline__ void flush_run(const SpectraArgs &a, const DatasetDev
     r.W = 0.0;
 }
 
-/* One warp, batches [b0, b1) of dataset ds (one unit), point group g (points 32 g ... 32 g + 31). */
+/* One warp, the nb batches of one unit of dataset ds staged at `unit` (SHARED memory), point group g
+ * (points 32 g ... 32 g + 31). */
 template <int S>
-__device__ __forceinline__ void walk_unit(const SpectraArgs &a, const DatasetDev &ds, int d, int b0, int b1, int g,
-                                          int lane)
+__device__ __forceinline__ void walk_unit(const SpectraArgs &a, const DatasetDev &ds, int d, const EventBatch *unit,
+                                          int nb, int g, int lane)
 {
     /* lane -> (point, sub-stream): a group of np < 32 points uses PL = 2^ceil(log2 np) point lanes
      * and splits the batches into NS = 32 / PL contiguous sub-streams */
@@ -204,8 +233,7 @@ __device__ __forceinline__ void walk_unit(const SpectraArgs &a, const DatasetDev
     const int pl = lane & (PL - 1), s = lane / PL;
     const bool active = pl < np;
     const int p = 32 * g + (active ? pl : 0);
-    const int nb = b1 - b0;
-    const int my0 = b0 + nb * s / NS, mine = b0 + nb * (s + 1) / NS - my0;
+    const int my0 = nb * s / NS, mine = nb * (s + 1) / NS - my0;
     const int iters = (nb + NS - 1) / NS;                  /* >= mine for every lane */
 
     double h[S];
@@ -223,7 +251,7 @@ __device__ __forceinline__ void walk_unit(const SpectraArgs &a, const DatasetDev
     r.cur = -1;
     r.hi = -pos_inf();
 
-    const EventBatch *bp = ds.ev + my0;
+    const EventBatch *bp = unit + my0;
 #pragma unroll 1
     for (int i = 0; i < iters; ++i, ++bp) {
         if (i >= mine) continue;
@@ -232,12 +260,12 @@ __device__ __forceinline__ void walk_unit(const SpectraArgs &a, const DatasetDev
             const double2 *q = reinterpret_cast<const double2 *>(bp);
 #pragma unroll
             for (int j = 0; j < EB / 2; ++j) {
-                double2 t = __ldg(q + j), u = __ldg(q + EB / 2 + j);
+                double2 t = q[j], u = q[EB / 2 + j];
                 x[2 * j] = t.x; x[2 * j + 1] = t.y;
                 w[2 * j] = u.x; w[2 * j + 1] = u.y;
             }
         }
-        const float v_last = __ldg(&bp->v[EB - 1]);
+        const float v_last = bp->v[EB - 1];
 
         /* row a2: g_k of every event of the batch */
         double gk[S][EB];
@@ -252,10 +280,10 @@ __device__ __forceinline__ void walk_unit(const SpectraArgs &a, const DatasetDev
             for (int j = 0; j < EB; ++j)
 #pragma unroll
                 for (int k = 0; k < S; ++k) r.C[k] = fma(w[j], gk[k][j], r.C[k]);
-            r.W += __ldg(&bp->wsum);
+            r.W += bp->wsum;
         } else {
             /* a run ends inside the batch (or none is open yet): walk its events one by one */
-            const float4 v4 = __ldg(reinterpret_cast<const float4 *>(bp->v));
+            const float4 v4 = *reinterpret_cast<const float4 *>(bp->v);
             const float v[EB] = {v4.x, v4.y, v4.z, v4.w};
 #pragma unroll
             for (int j = 0; j < EB; ++j) {
@@ -309,46 +337,70 @@ template <int S>
 __global__ void __launch_bounds__(WARPS * 32, 4) spectra_kernel(const __grid_constant__ SpectraArgs a)
 {
     static_assert(EB == 4, "the batch loads are written for EB = 4");
-    const int lane = threadIdx.x & 31;
+    extern __shared__ __align__(128) unsigned char stage[];       /* [WARPS][2][unit_batches] EventBatch */
+    __shared__ unsigned long long bars[WARPS][2];
+    const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
     const unsigned nW = gridDim.x * WARPS;
     const int n_groups = (a.P + 31) >> 5;
     const unsigned n_items = (unsigned)a.n_items;
+    EventBatch *const buf0 = reinterpret_cast<EventBatch *>(stage) + (size_t)(2 * wib) * a.unit_batches;
+    if (lane == 0) {
+        mbar_init(&bars[wib][0], 1);
+        mbar_init(&bars[wib][1], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncwarp();
     /* the first two items of a warp are static, later ones come from the counter (which the setup
-     * kernel left at 2 nW): warps that meet expensive units (bin edges) simply claim fewer */
-    unsigned cur = blockIdx.x * WARPS + (threadIdx.x >> 5), nxt = cur + nW;
+     * kernel left at 2 nW): warps that meet expensive units (bin edges) simply claim fewer.  The
+     * unit of item i + 1 is copied into the warp's other buffer while item i is walked. */
+    unsigned cur = blockIdx.x * WARPS + wib, nxt = cur + nW;
+    unsigned phase = 0u;                                /* bit b: parity of the next completion of buffer b */
+    int b = 0;
+    if (cur < n_items && lane == 0) {
+        int d, b0, b1, chunk;
+        decode_item(a, cur, d, b0, b1, chunk);
+        bulk_load(buf0, a.ds[d].ev + b0, (unsigned)(b1 - b0) * (unsigned)sizeof(EventBatch), &bars[wib][0]);
+    }
 #pragma unroll 1
     while (cur < n_items) {
         const unsigned ticket = take_ticket(a.counter, lane);
         int d, b0, b1, chunk;
         decode_item(a, cur, d, b0, b1, chunk);
-        if (nxt < n_items && nxt / (unsigned)a.n_chunks != cur / (unsigned)a.n_chunks) {
-            /* pull the next unit towards the SM while this one is being walked */
+        if (nxt < n_items && lane == 0) {
+            /* the other buffer was last read one item ago; every lane has passed the __syncwarp below */
             int nd, nb0, nb1, nc;
             decode_item(a, nxt, nd, nb0, nb1, nc);
-            const char *base = reinterpret_cast<const char *>(a.ds[nd].ev + nb0);
-            const int bytes = (nb1 - nb0) * (int)sizeof(EventBatch);
-            for (int o = lane * 128; o < bytes; o += 32 * 128)
-                asm volatile("prefetch.global.L2 [%0];" ::"l"(base + o));
+            bulk_load(buf0 + (b ^ 1) * a.unit_batches, a.ds[nd].ev + nb0, (unsigned)(nb1 - nb0) * (unsigned)sizeof(EventBatch),
+                      &bars[wib][b ^ 1]);
         }
+        mbar_wait(&bars[wib][b], (phase >> b) & 1u);
+        phase ^= 1u << b;
         const DatasetDev &ds = a.ds[d];
         const int g1 = min((chunk + 1) * a.chunk_groups, n_groups);
 #pragma unroll 1
-        for (int g = chunk * a.chunk_groups; g < g1; ++g) walk_unit<S>(a, ds, d, b0, b1, g, lane);
+        for (int g = chunk * a.chunk_groups; g < g1; ++g) walk_unit<S>(a, ds, d, buf0 + b * a.unit_batches, b1 - b0, g, lane);
         cur = nxt;
-        nxt = __shfl_sync(0xffffffffu, ticket, 0);
+        nxt = __shfl_sync(0xffffffffu, ticket, 0);      /* also orders this item's reads before the next copy */
+        b ^= 1;
     }
 }
 
+/* dynamic shared memory of one CTA: two unit buffers per warp, sized for the largest unit */
+constexpr size_t STAGE_BYTES = (size_t)WARPS * 2 * MAX_UNIT_BATCHES * sizeof(EventBatch);
+
 template <int S> cudaError_t launch_t(const SpectraArgs &a, cudaStream_t st)
 {
-    spectra_kernel<S><<<a.n_warps / WARPS, WARPS * 32, 0, st>>>(a);
+    spectra_kernel<S><<<a.n_warps / WARPS, WARPS * 32, STAGE_BYTES, st>>>(a);
     return cudaGetLastError();
 }
 
 template <int S> cudaError_t max_warps_t(int sm_count, int *warps)
 {
     int per_sm = 0;
-    cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, spectra_kernel<S>, WARPS * 32, 0);
+    cudaError_t e = cudaFuncSetAttribute(spectra_kernel<S>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         (int)STAGE_BYTES);
+    if (e != cudaSuccess) return e;
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, spectra_kernel<S>, WARPS * 32, STAGE_BYTES);
     if (e != cudaSuccess) return e;
     if (per_sm < 1) return cudaErrorLaunchOutOfResources;
     *warps = sm_count * per_sm * WARPS;
