@@ -178,7 +178,7 @@ void fill_datasets(const phylino_ctx *ctx, SpectraArgs &a)
 }
 
 /* Cut of the batch into work items (spectra.cu): U batches per unit, G point groups per item.
- * Aim: about 24 items per resident warp (dynamic balance, short tail) of at least 16 batch-groups
+ * Aim: about 12 items per resident warp (dynamic balance, short tail) of at least 16 batch-groups
  * each (the per-item cost -- first bin search, one flush per point -- stays a few percent). */
 void fill_batch(const phylino_ctx *ctx, SpectraArgs &a, int P, const double *params)
 {
@@ -192,7 +192,7 @@ void fill_batch(const phylino_ctx *ctx, SpectraArgs &a, int P, const double *par
     for (int d = 0; d < ctx->n_datasets; ++d) batches += ctx->ds[d].n_pad / EB;
     int cap = std::max(ctx->resident_warps, WARPS);
     if (ctx->max_warps > 0) cap = std::max(WARPS, std::min(cap, ctx->max_warps / WARPS * WARPS));
-    const int64_t work = std::max<int64_t>(1, batches * n_groups / (24ll * cap));
+    const int64_t work = std::max<int64_t>(1, batches * n_groups / (12ll * cap));
     int64_t U = 16;
     while (U < 64 && U * 2 <= work) U *= 2;
     U = std::max<int64_t>(U, 4 * streams);
@@ -470,6 +470,8 @@ phylino_status phylino_load_events(phylino_ctx *ctx, int dataset, int64_t n, con
         b.v[j] = vi;
         b.w[j] = weight ? (double)weight[s] : 1.0;
         b.wsum += b.w[j];                       /* in event order: the batch total the hot kernel adds */
+        if (j == 0)                             /* where a lane starts looking for its bin (a hint, never trusted) */
+            b.bin0 = vi == vi ? (int32_t)(std::upper_bound(edges, edges + n_bins + 1, (double)vi) - edges) - 1 : n_bins;
         wsum += std::fabs(b.w[j]);
         if (std::isfinite(vi)) {
             if (vi > 0.0f && vi < v_pos_min) v_pos_min = vi;

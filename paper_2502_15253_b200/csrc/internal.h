@@ -35,7 +35,8 @@ struct __align__(16) EventBatch {
     double w[EB];           /* MC weight as fp64 (exact copy of the fp32 input); padding = 0 */
     float  v[EB];           /* E_vis [MeV]; padding = NaN */
     double wsum;            /* w[0] + ... + w[EB-1], summed in that order */
-    double reserved;
+    int32_t bin0;           /* hint: bin of v[0] under the identity energy scale, -1 below, n_bins above / NaN */
+    int32_t reserved;
 };
 static_assert(sizeof(EventBatch) == 96, "EventBatch is read with fixed 16-byte offsets");
 

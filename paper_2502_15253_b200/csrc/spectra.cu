@@ -197,6 +197,8 @@ template <int S> struct Run {
     double W;       /* sum of w over the run */
     int    cur;     /* its bin; < 0 or >= n_bins: events that land in no bin (never flushed) */
     float  hi;      /* later events below hi stay in the run (-inf: re-locate at the next event) */
+    float  hi2;     /* threshold after hi (+inf past the last edge), loaded when the run opened so that the
+                     * end of the run does not wait for it; meaningful only while hi is a table threshold */
 };
 
 template <int S>
@@ -218,23 +220,98 @@ __device__ __forceinline__ void flush_run(const SpectraArgs &a, const DatasetDev
     r.W = 0.0;
 }
 
-/* One warp, the nb batches of one unit of dataset ds staged at `unit` (SHARED memory), point group g
- * (points 32 g ... 32 g + 31). */
+/* threshold row entry with the conventions thr[-1] = -inf, thr[B + 1] = +inf */
+__device__ __forceinline__ float thr_at(const float *thr, int B, int i)
+{
+    return i < 0 ? -pos_inf() : (i > B ? pos_inf() : __ldg(thr + i));
+}
+
+/* One batch of the lane's stream (rows a2-a4). */
 template <int S>
+__device__ __forceinline__ void walk_batch(const SpectraArgs &a, const DatasetDev &ds, const EventBatch *bp,
+                                           const double (&h)[S], const float *thr, float2 safe, int p, bool active,
+                                           Run<S> &r)
+{
+    const int B = ds.n_bins;
+    double x[EB], w[EB];
+    {
+        const double2 *q = reinterpret_cast<const double2 *>(bp);
+#pragma unroll
+        for (int j = 0; j < EB / 2; ++j) {
+            double2 t = q[j], u = q[EB / 2 + j];
+            x[2 * j] = t.x; x[2 * j + 1] = t.y;
+            w[2 * j] = u.x; w[2 * j + 1] = u.y;
+        }
+    }
+    const float v_last = bp->v[EB - 1];
+
+    /* row a2: g_k of every event of the batch */
+    double gk[S][EB];
+#pragma unroll
+    for (int j = 0; j < EB; ++j)
+#pragma unroll
+        for (int k = 0; k < S; ++k) gk[k][j] = half_cos_halfturns(h[k], x[j]);
+
+    if (v_last < r.hi) {
+        /* rows a3 + a4: the store is sorted, so the whole batch lies in the run's bin */
+#pragma unroll
+        for (int j = 0; j < EB; ++j)
+#pragma unroll
+            for (int k = 0; k < S; ++k) r.C[k] = fma(w[j], gk[k][j], r.C[k]);
+        r.W += bp->wsum;
+    } else {
+        /* a run ends inside the batch (or none is open yet): walk its events one by one */
+        const float4 v4 = *reinterpret_cast<const float4 *>(bp->v);
+        const float v[EB] = {v4.x, v4.y, v4.z, v4.w};
+#pragma unroll
+        for (int j = 0; j < EB; ++j) {
+            if (!(v[j] < r.hi)) {
+                int b;
+                float nhi;
+                if (r.hi > -pos_inf() && r.hi < pos_inf() && v[j] <= safe.y) {
+                    /* r.hi = thr[cur + 1] <= v inside the table's interval: scan forward */
+                    b = r.cur + 1;
+                    nhi = r.hi2;
+                    while (b < B && !(v[j] < nhi)) { ++b; nhi = thr_at(thr, B, b + 1); }
+                } else {
+                    b = locate_bin(ds, thr, safe, a.params + (size_t)p * a.n_params, v[j], nhi);
+                }
+                if (b != r.cur) {
+                    flush_run<S>(a, ds, p, active, r);
+                    r.cur = b;
+                }
+                r.hi = nhi;
+                r.hi2 = thr_at(thr, B, b + 2);
+            }
+#pragma unroll
+            for (int k = 0; k < S; ++k) r.C[k] = fma(w[j], gk[k][j], r.C[k]);
+            r.W += w[j];
+        }
+    }
+}
+
+/* One warp, the nb batches of one unit of dataset ds staged at `unit` (SHARED memory), point group g
+ * (points 32 g ... 32 g + 31).  FULL: the group has 32 points, every lane walks all batches. */
+template <int S, bool FULL>
 __device__ __forceinline__ void walk_unit(const SpectraArgs &a, const DatasetDev &ds, int d, const EventBatch *unit,
                                           int nb, int g, int lane)
 {
     /* lane -> (point, sub-stream): a group of np < 32 points uses PL = 2^ceil(log2 np) point lanes
      * and splits the batches into NS = 32 / PL contiguous sub-streams */
-    const int np = min(32, a.P - 32 * g);
-    int PL = 32;
-    if (np < 32) { PL = 1; while (PL < np) PL <<= 1; }
-    const int NS = 32 / PL;
-    const int pl = lane & (PL - 1), s = lane / PL;
-    const bool active = pl < np;
-    const int p = 32 * g + (active ? pl : 0);
-    const int my0 = nb * s / NS, mine = nb * (s + 1) / NS - my0;
-    const int iters = (nb + NS - 1) / NS;                  /* >= mine for every lane */
+    int my0 = 0, mine = nb, iters = nb, p = 32 * g + lane;
+    bool active = true;
+    if (!FULL) {
+        const int np = min(32, a.P - 32 * g);
+        int PL = 1;
+        while (PL < np) PL <<= 1;
+        const int NS = 32 / PL;
+        const int pl = lane & (PL - 1), s = lane / PL;
+        active = pl < np;
+        p = 32 * g + (active ? pl : 0);
+        my0 = nb * s / NS;
+        mine = nb * (s + 1) / NS - my0;
+        iters = (nb + NS - 1) / NS;                        /* >= mine for every lane */
+    }
 
     double h[S];
 #pragma unroll
@@ -250,64 +327,32 @@ __device__ __forceinline__ void walk_unit(const SpectraArgs &a, const DatasetDev
     r.W = 0.0;
     r.cur = -1;
     r.hi = -pos_inf();
+    r.hi2 = pos_inf();
 
     const EventBatch *bp = unit + my0;
-#pragma unroll 1
-    for (int i = 0; i < iters; ++i, ++bp) {
-        if (i >= mine) continue;
-        double x[EB], w[EB];
-        {
-            const double2 *q = reinterpret_cast<const double2 *>(bp);
-#pragma unroll
-            for (int j = 0; j < EB / 2; ++j) {
-                double2 t = q[j], u = q[EB / 2 + j];
-                x[2 * j] = t.x; x[2 * j + 1] = t.y;
-                w[2 * j] = u.x; w[2 * j + 1] = u.y;
-            }
+    if (mine > 0) {
+        /* open the run at the lane's first event: start from the load-time hint (its bin under the
+         * identity energy scale) and step to the bin the lane's own thresholds give -- the same
+         * decision as the binary search of locate_bin, usually without a single dependent load */
+        const float v0 = bp->v[0];
+        if (v0 >= safe.x && v0 <= safe.y) {
+            int b = max(-1, min(bp->bin0, B));
+            float lo = thr_at(thr, B, b), hi = thr_at(thr, B, b + 1);
+            while (b >= 0 && v0 < lo) { --b; hi = lo; lo = thr_at(thr, B, b); }
+            while (b < B && !(v0 < hi)) { ++b; hi = thr_at(thr, B, b + 1); }
+            r.cur = b;
+            r.hi = hi;
+            r.hi2 = thr_at(thr, B, b + 2);
         }
-        const float v_last = bp->v[EB - 1];
-
-        /* row a2: g_k of every event of the batch */
-        double gk[S][EB];
-#pragma unroll
-        for (int j = 0; j < EB; ++j)
-#pragma unroll
-            for (int k = 0; k < S; ++k) gk[k][j] = half_cos_halfturns(h[k], x[j]);
-
-        if (v_last < r.hi) {
-            /* rows a3 + a4: the store is sorted, so the whole batch lies in the run's bin */
-#pragma unroll
-            for (int j = 0; j < EB; ++j)
-#pragma unroll
-                for (int k = 0; k < S; ++k) r.C[k] = fma(w[j], gk[k][j], r.C[k]);
-            r.W += bp->wsum;
-        } else {
-            /* a run ends inside the batch (or none is open yet): walk its events one by one */
-            const float4 v4 = *reinterpret_cast<const float4 *>(bp->v);
-            const float v[EB] = {v4.x, v4.y, v4.z, v4.w};
-#pragma unroll
-            for (int j = 0; j < EB; ++j) {
-                if (!(v[j] < r.hi)) {
-                    int b;
-                    float nhi;
-                    if (r.hi > -pos_inf() && r.hi < pos_inf() && v[j] <= safe.y) {
-                        /* r.hi = thr[cur + 1] <= v inside the table's interval: scan forward */
-                        b = r.cur + 1;
-                        nhi = b < B ? __ldg(thr + b + 1) : pos_inf();
-                        while (!(v[j] < nhi)) { ++b; nhi = b < B ? __ldg(thr + b + 1) : pos_inf(); }
-                    } else {
-                        b = locate_bin(ds, thr, safe, a.params + (size_t)p * a.n_params, v[j], nhi);
-                    }
-                    if (b != r.cur) {
-                        flush_run<S>(a, ds, p, active, r);
-                        r.cur = b;
-                    }
-                    r.hi = nhi;
-                }
-#pragma unroll
-                for (int k = 0; k < S; ++k) r.C[k] = fma(w[j], gk[k][j], r.C[k]);
-                r.W += w[j];
-            }
+    }
+    if (FULL) {
+#pragma unroll 1
+        for (int i = 0; i < nb; ++i, ++bp) walk_batch<S>(a, ds, bp, h, thr, safe, p, active, r);
+    } else {
+#pragma unroll 1
+        for (int i = 0; i < iters; ++i, ++bp) {
+            if (i >= mine) continue;
+            walk_batch<S>(a, ds, bp, h, thr, safe, p, active, r);
         }
     }
     flush_run<S>(a, ds, p, active, r);
@@ -317,7 +362,9 @@ __device__ __forceinline__ void walk_unit(const SpectraArgs &a, const DatasetDev
 __device__ __forceinline__ unsigned take_ticket(unsigned *counter, int lane)
 {
     unsigned t = 0;
-    if (lane == 0) t = atomicAdd(counter, 1u);
+    /* written in PTX so that the compiler does not turn it into its warp-aggregated form, whose
+     * shuffle would wait for the atomic right here */
+    if (lane == 0) asm volatile("atom.global.add.u32 %0, [%1], 1;" : "=r"(t) : "l"(counter) : "memory");
     return t;
 }
 
@@ -378,7 +425,10 @@ __global__ void __launch_bounds__(WARPS * 32, 4) spectra_kernel(const __grid_con
         const DatasetDev &ds = a.ds[d];
         const int g1 = min((chunk + 1) * a.chunk_groups, n_groups);
 #pragma unroll 1
-        for (int g = chunk * a.chunk_groups; g < g1; ++g) walk_unit<S>(a, ds, d, buf0 + b * a.unit_batches, b1 - b0, g, lane);
+        for (int g = chunk * a.chunk_groups; g < g1; ++g) {
+            if (32 * g + 32 <= a.P) walk_unit<S, true>(a, ds, d, buf0 + b * a.unit_batches, b1 - b0, g, lane);
+            else                    walk_unit<S, false>(a, ds, d, buf0 + b * a.unit_batches, b1 - b0, g, lane);
+        }
         cur = nxt;
         nxt = __shfl_sync(0xffffffffu, ticket, 0);      /* also orders this item's reads before the next copy */
         b ^= 1;
