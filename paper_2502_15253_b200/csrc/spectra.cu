@@ -290,6 +290,26 @@ __device__ __forceinline__ void walk_batch(const SpectraArgs &a, const DatasetDe
     }
 }
 
+/* Two consecutive batches known to lie inside the lane's open run (the store is sorted: the last
+ * event of the second batch is below r.hi): rows a2 + a4 only, straight-line. */
+template <int S>
+__device__ __forceinline__ void walk_pair_inside(const EventBatch *bp, const double (&h)[S], Run<S> &r)
+{
+#pragma unroll
+    for (int u = 0; u < 2; ++u) {
+        const double2 *q = reinterpret_cast<const double2 *>(bp + u);
+#pragma unroll
+        for (int j = 0; j < EB / 2; ++j) {
+            const double2 t = q[j], w = q[EB / 2 + j];
+#pragma unroll
+            for (int k = 0; k < S; ++k) r.C[k] = fma(w.x, half_cos_halfturns(h[k], t.x), r.C[k]);
+#pragma unroll
+            for (int k = 0; k < S; ++k) r.C[k] = fma(w.y, half_cos_halfturns(h[k], t.y), r.C[k]);
+        }
+        r.W += bp[u].wsum;
+    }
+}
+
 /* One warp, the nb batches of one unit of dataset ds staged at `unit` (SHARED memory), point group g
  * (points 32 g ... 32 g + 31).  FULL: the group has 32 points, every lane walks all batches. */
 template <int S, bool FULL>
@@ -346,8 +366,19 @@ __device__ __forceinline__ void walk_unit(const SpectraArgs &a, const DatasetDev
         }
     }
     if (FULL) {
+        int i = 0;
 #pragma unroll 1
-        for (int i = 0; i < nb; ++i, ++bp) walk_batch<S>(a, ds, bp, h, thr, safe, p, active, r);
+        while (i < nb) {
+            if (i + 2 <= nb && bp[1].v[EB - 1] < r.hi) {
+                walk_pair_inside<S>(bp, h, r);
+                i += 2;
+                bp += 2;
+            } else {
+                walk_batch<S>(a, ds, bp, h, thr, safe, p, active, r);
+                ++i;
+                ++bp;
+            }
+        }
     } else {
 #pragma unroll 1
         for (int i = 0; i < iters; ++i, ++bp) {
@@ -362,9 +393,10 @@ __device__ __forceinline__ void walk_unit(const SpectraArgs &a, const DatasetDev
 __device__ __forceinline__ unsigned take_ticket(unsigned *counter, int lane)
 {
     unsigned t = 0;
-    /* written in PTX so that the compiler does not turn it into its warp-aggregated form, whose
-     * shuffle would wait for the atomic right here */
-    if (lane == 0) asm volatile("atom.global.add.u32 %0, [%1], 1;" : "=r"(t) : "l"(counter) : "memory");
+    /* atom.inc with a limit the counter never reaches (items + tickets stay below 2^31, fill_batch):
+     * ptxas turns a uniform-address atom.add into its warp-aggregated form, whose shuffle would wait
+     * for the atomic right here instead of one item later */
+    if (lane == 0) asm volatile("atom.global.inc.u32 %0, [%1], 0x7fffffff;" : "=r"(t) : "l"(counter) : "memory");
     return t;
 }
 
