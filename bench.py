@@ -33,9 +33,10 @@ import workloads  # noqa: E402
 METRIC = "oscillated event x param-point/s (batched spectra+NLL)"
 UNIT = "event*point/s"
 # ALGORITHMIC fp64-pipe instructions per event x point: per oscillation term
-# 11 for 1/2 cos(2 phase) (3 range reduction, 1 square, 7 Horner) + 1 multiply-accumulate into the run.
+# 10 for 1/2 cos(2 phase) (3 range reduction, 1 square, 6 Horner) + 1 multiply-accumulate into the run;
+# the SASS of the hot loop has exactly these (9 DFMA + 1 DADD + 1 DMUL per event x point x term).
 # The bin/weight bookkeeping is per batch of events and per run, not per event x point.
-FP64_PER_TERM = 12
+FP64_PER_TERM = 11
 # nominal fp64 pipe: 64 lanes/clk/SM x 148 SMs x 1.965 GHz (B200_PROFILING.md table)
 PEAK_FP64_INST = 64 * 148 * 1.965e9
 L2_FLUSH_BYTES = 256 << 20
