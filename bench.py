@@ -260,6 +260,34 @@ def main():
         e2e_s = float(t.item())
     e2e_value = world * evpt_step * args.steps / e2e_s
 
+    # ---- cross-point caching, reported beside the dense numbers, never instead of
+    # them: the same host-buffer call with phylino_set_caching(1); wall time of one whole batch (config 3: one
+    # central-difference gradient step; config 5: one grid scan), every step a fresh batch.
+    cached = None
+    ph.set_caching(True)
+    ph.nll_host(h_params, data, out)
+    vp, classes = ph.last_plan()
+    if vp > 0:
+        for _ in range(args.warmup):
+            ph.nll_host(h_params, data, out)
+        torch.cuda.synchronize()
+        c_s = 0.0
+        for i in range(args.steps):
+            h_params[:, 0] = params[:, 0] * (1.0 + 1e-9 * (i + 1))
+            t0 = time.perf_counter()
+            ph.nll_host(h_params, data, out)
+            c_s += time.perf_counter() - t0
+            flush.zero_()
+            torch.cuda.synchronize()
+        dense_ref = np.empty(P)
+        ph.set_caching(False)
+        ph.nll_host(h_params, data, dense_ref)
+        cached = {"ms_per_step": c_s / args.steps * 1e3, "virtual_points": vp, "energy_scale_classes": classes,
+                  "points": P, "max_abs_nll_diff_vs_dense": float(np.nanmax(np.abs(out - dense_ref))),
+                  "note": "phylino_nll_host with phylino_set_caching(1): H2D + plan + kernels + D2H; "
+                          "not comparable with the dense roofline (fewer event x point evaluations are executed)"}
+    ph.set_caching(False)
+
     if rank == 0:
         inst = fp64_inst_per_evpt(wl.model)
         sp_avg = sum(sp_ms) / len(sp_ms)
@@ -291,6 +319,8 @@ def main():
                     "d2h_bytes_per_step": 8 * P, "ms_per_step": e2e_s / args.steps * 1e3},
             "roofline": roofline,
         }
+        if cached is not None:
+            line["cached"] = cached
         if world == 1 and not args.no_cpu_baseline:
             import oracle                                   # the cpu_baseline leg (test infrastructure)
             orc = oracle.Oracle(wl.model, wl.events)

@@ -174,6 +174,22 @@ PHYLINO_API int64_t phylino_total_events(const phylino_ctx *ctx);   /* sum_d n o
  * regroup the fp64 partial sums (rounding-level differences only). */
 PHYLINO_API phylino_status phylino_set_tuning(phylino_ctx *ctx, int unit_events, int chunk_groups, int max_warps);
 
+/* Cross-point caching for the HOST-buffer entry points (the paper's "caching, where
+ * costly recalculations are only triggered upon relevant parameter changes").  For a fixed
+ * energy scale and fixed mass splittings the spectrum is affine in the oscillation amplitudes (PAPER.md:34
+ * Eq. 1): H[p,b] = P0(p) W[b] + sum_k A_k(p) C_k[b].  With caching on, phylino_nll_host / phylino_spectra_host
+ * group the points of the batch by the BIT PATTERNS of the parameters that enter the energy scale and each
+ * mass splitting, evaluate W and C_k once per group (packed as "virtual points" for the same kernels), and
+ * combine them per point.  Points whose parameters differ only in amplitudes, flux/background nuisances or
+ * rates share all of the event work: a 603-point central-difference batch of a 301-parameter fit needs 21
+ * virtual points.  Results agree with the dense path to rounding (within the same per-bin and NLL tolerances) and
+ * are bitwise reproducible; a cell that left the fixed-point domain reads NaN (the dense path tells +-inf
+ * apart).  If the batch does not shrink to at most half, the dense path runs.  Off by default; the
+ * DEVICE-pointer entry points are always dense.  phylino_last_plan: virtual points and energy-scale classes
+ * of the last host call that used the cache (0, 0 if it ran dense). */
+PHYLINO_API phylino_status phylino_set_caching(phylino_ctx *ctx, int on);
+PHYLINO_API phylino_status phylino_last_plan(const phylino_ctx *ctx, int64_t *virtual_points, int64_t *classes);
+
 /* Device timing of the three kernels of a call (CUDA events on the context's stream, recorded
  * around the setup, spectra and finalize kernels of every later call).  phylino_last_kernel_ms
  * waits for the last call to finish and writes its three durations in milliseconds to ms[0..2]

@@ -21,6 +21,7 @@ abi_symbols = (
     "phylino_spectra_host", "phylino_total_bins", "phylino_total_events",
     "phylino_set_tuning", "phylino_launch_count", "phylino_last_error", "phylino_peak_fp64",
     "phylino_expectation", "phylino_set_timing", "phylino_last_kernel_ms",
+    "phylino_set_caching", "phylino_last_plan",
 )
 
 _STATUS = {0: "OK", 1: "ERR_ARG", 2: "ERR_SHAPE", 3: "ERR_STATE", 4: "ERR_OOM", 5: "ERR_CUDA"}
@@ -95,6 +96,10 @@ def load_library():
     lib.phylino_total_bins.argtypes = [vp]
     lib.phylino_total_events.restype = i64
     lib.phylino_total_events.argtypes = [vp]
+    lib.phylino_set_caching.restype = i32
+    lib.phylino_set_caching.argtypes = [vp, i32]
+    lib.phylino_last_plan.restype = i32
+    lib.phylino_last_plan.argtypes = [vp, C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
     lib.phylino_set_tuning.restype = i32
     lib.phylino_set_tuning.argtypes = [vp, i32, i32, i32]
     lib.phylino_launch_count.restype = i64
@@ -273,6 +278,15 @@ class Phylino:
             and out.numel() == p.shape[0] * self.total_bins
         self._check(self._lib.phylino_expectation(self._ctx, int(p.shape[0]), p.data_ptr(), out.data_ptr()))
         return out
+
+    def set_caching(self, on: bool = True):
+        self._check(self._lib.phylino_set_caching(self._ctx, int(bool(on))))
+
+    def last_plan(self):
+        """(virtual points, energy-scale classes) of the last host call that used the cache; (0, 0) if dense."""
+        v, c = C.c_int64(0), C.c_int64(0)
+        self._check(self._lib.phylino_last_plan(self._ctx, C.byref(v), C.byref(c)))
+        return int(v.value), int(c.value)
 
     def set_timing(self, on: bool = True):
         self._check(self._lib.phylino_set_timing(self._ctx, int(bool(on))))

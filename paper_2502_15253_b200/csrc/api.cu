@@ -9,6 +9,7 @@
 #include <cstring>
 #include <new>
 #include <numeric>
+#include <vector>
 
 #include "internal.h"
 
@@ -87,6 +88,7 @@ void free_all(phylino_ctx *c)
     c->d_acc = nullptr; c->d_flags = nullptr; c->acc_capacity = 0;
     cudaFree(c->d_rec); cudaFree(c->d_thr); cudaFree(c->d_safe); cudaFree(c->d_counter);
     c->d_rec = nullptr; c->d_thr = nullptr; c->d_safe = nullptr; c->d_counter = nullptr; c->point_capacity = 0;
+    cudaFree(c->d_plan); c->d_plan = nullptr; c->plan_capacity = 0;
     cudaFree(c->d_stage); c->d_stage = nullptr;
     if (c->h_pin) cudaFreeHost(c->h_pin);
     c->h_pin = nullptr; c->stage_capacity = 0;
@@ -270,6 +272,199 @@ phylino_status ensure_stage(phylino_ctx *ctx, int64_t doubles)
     CU(cudaMalloc((void **)&ctx->d_stage, doubles * sizeof(double)));
     CU(cudaHostAlloc((void **)&ctx->h_pin, doubles * sizeof(double), cudaHostAllocDefault));
     ctx->stage_capacity = doubles;
+    return PHYLINO_OK;
+}
+
+/* ---- cross-point caching ("costly recalculations are only
+ * triggered upon relevant parameter changes") ---------------------------------------------------
+ * For a fixed energy scale and fixed mass splittings the histogram is affine in the amplitudes:
+ *   H[p,b] = P0(p) W[b] + sum_k A_k(p) C_k[b],  W[b] = sum_e w_e,  C_k[b] = sum_e w_e g(h_k x_e),
+ * so a batch needs one W per distinct energy-scale tuple ("class") and one C per distinct
+ * (class, splitting).  The plan groups the caller's points by the BIT PATTERNS of the parameters
+ * these depend on (never by value tolerance), packs the distinct (class, splitting) pairs S at a
+ * time into virtual points for the spectra kernel, and tells the finalize kernel which cells each
+ * real point combines.  A 603-point central-difference batch of config 3 becomes 21 virtual
+ * points, the 4096-point grid of config 5 becomes 22. */
+struct ComponentPlan {
+    int V = 0, C = 0;
+    std::vector<int32_t> vp_class, vp_src, class_rep, pt_comp;
+};
+
+/* parameters the half-turn coefficient of term k depends on (devmath.cuh osc_terms) */
+int term_deps(int osc_model, int k, int slots[3])
+{
+    if (osc_model == PHYLINO_OSC_EQ1) { slots[0] = k == 0 ? PHYLINO_MEE : PHYLINO_M21; return 1; }
+    if (osc_model == PHYLINO_OSC_STERILE4) { slots[0] = k == 0 ? PHYLINO_MEE : (k == 1 ? PHYLINO_M41 : PHYLINO_M21); return 1; }
+    if (k == 0) { slots[0] = PHYLINO_M21; return 1; }
+    slots[0] = PHYLINO_MEE; slots[1] = PHYLINO_S12; slots[2] = PHYLINO_M21;
+    return 3;
+}
+
+uint64_t bits_of(double x) { uint64_t u; std::memcpy(&u, &x, sizeof u); return u; }
+
+uint64_t mix64(uint64_t h, uint64_t x)
+{
+    h ^= x + 0x9e3779b97f4a7c15ull + (h << 6) + (h >> 2);
+    h *= 0xff51afd7ed558ccdull;
+    return h ^ (h >> 32);
+}
+
+/* open-addressing set of ids; equality is decided by the caller on the ACTUAL key bits (the hash only
+ * picks the probe start), so two different keys are never merged */
+struct IdTable {
+    std::vector<int32_t> slot;
+    uint64_t mask;
+    explicit IdTable(size_t n) { size_t c = 16; while (c < 2 * n + 2) c <<= 1; slot.assign(c, -1); mask = c - 1; }
+    template <class Eq> int32_t find_or_insert(uint64_t h, int32_t fresh, Eq same, bool &inserted)
+    {
+        for (uint64_t i = h & mask;; i = (i + 1) & mask) {
+            if (slot[i] < 0) { slot[i] = fresh; inserted = true; return fresh; }
+            if (same(slot[i])) { inserted = false; return slot[i]; }
+        }
+    }
+};
+
+/* false: caching would not pay (more than half as many virtual points as points) -- use the dense path */
+bool plan_components(const phylino_ctx *ctx, int P, const double *params, ComponentPlan &pl)
+{
+    const int S = ctx->n_terms, NP = ctx->n_params;
+    /* columns of the parameter vector that enter the energy scale of any dataset */
+    std::vector<int32_t> acols;
+    for (int d = 0; d < ctx->n_datasets; ++d)
+        for (int j = 0; j < 3; ++j)
+            if (ctx->ds[d].idx_a[j] >= 0) acols.push_back(ctx->ds[d].idx_a[j]);
+    std::vector<int32_t> cls((size_t)P);
+    {
+        IdTable tab((size_t)P);
+        for (int p = 0; p < P; ++p) {
+            const double *th = params + (size_t)p * NP;
+            uint64_t h = 0x243f6a8885a308d3ull;
+            for (int32_t c : acols) h = mix64(h, bits_of(th[c]));
+            bool ins;
+            const int32_t id = tab.find_or_insert(h, (int32_t)pl.class_rep.size(), [&](int32_t other) {
+                const double *to = params + (size_t)pl.class_rep[other] * NP;
+                for (int32_t c : acols) if (bits_of(th[c]) != bits_of(to[c])) return false;
+                return true;
+            }, ins);
+            if (ins) pl.class_rep.push_back(p);
+            cls[p] = id;
+        }
+    }
+    pl.C = (int)pl.class_rep.size();
+    /* distinct (class, formula, dependency bits) -> pair id, in order of first appearance */
+    std::vector<int32_t> pair_class, pair_src, pt_pair((size_t)P * S);
+    {
+        IdTable tab((size_t)P * S);
+        auto dep = [&](int p, int k, int j, int n_slots, const int *slots) -> uint64_t {
+            (void)k; (void)n_slots;
+            const int idx = ctx->idx_osc[slots[j]];
+            return bits_of(idx >= 0 ? params[(size_t)p * NP + idx] : ctx->fixed_osc[slots[j]]);
+        };
+        for (int p = 0; p < P; ++p) {
+            for (int k = 0; k < S; ++k) {
+                int slots[3];
+                const int n = term_deps(ctx->osc_model, k, slots);
+                const int formula = n == 1 ? 0 : k;             /* single-parameter terms share one formula */
+                uint64_t h = mix64(mix64(0x13198a2e03707344ull, (uint64_t)cls[p]), (uint64_t)formula);
+                for (int j = 0; j < n; ++j) h = mix64(h, dep(p, k, j, n, slots));
+                bool ins;
+                const int32_t id = tab.find_or_insert(h, (int32_t)pair_src.size(), [&](int32_t other) {
+                    const int op = pair_src[other] >> 2, ok = pair_src[other] & 3;
+                    int oslots[3];
+                    const int on = term_deps(ctx->osc_model, ok, oslots);
+                    if (pair_class[other] != cls[p] || on != n || (on == 1 ? 0 : ok) != formula) return false;
+                    for (int j = 0; j < n; ++j) if (dep(p, k, j, n, slots) != dep(op, ok, j, on, oslots)) return false;
+                    return true;
+                }, ins);
+                if (ins) { pair_class.push_back(cls[p]); pair_src.push_back(p * 4 + k); }
+                pt_pair[(size_t)p * S + k] = id;
+            }
+        }
+    }
+    /* pack the pairs of a class S at a time */
+    const int n_pairs = (int)pair_class.size();
+    std::vector<int32_t> fill((size_t)pl.C, 0), open_vp((size_t)pl.C, -1), pair_cell((size_t)n_pairs);
+    for (int q = 0; q < n_pairs; ++q) {
+        const int c = pair_class[q];
+        if (open_vp[c] < 0 || fill[c] == S) {
+            open_vp[c] = pl.V++;
+            fill[c] = 0;
+            pl.vp_class.push_back(c);
+            for (int s = 0; s < S; ++s) pl.vp_src.push_back(pair_src[q]);   /* unused slots repeat the first pair */
+        }
+        pl.vp_src[(size_t)open_vp[c] * S + fill[c]] = pair_src[q];
+        pair_cell[q] = open_vp[c] * (S + 1) + 1 + fill[c];
+        ++fill[c];
+    }
+    if (2 * (int64_t)pl.V > P) return false;
+    pl.pt_comp.resize((size_t)P * (S + 1));
+    for (int p = 0; p < P; ++p) {
+        int32_t *row = &pl.pt_comp[(size_t)p * (S + 1)];
+        for (int k = 0; k < S; ++k) row[k + 1] = pair_cell[pt_pair[(size_t)p * S + k]];
+        row[0] = (row[1] - 1) / (S + 1) * (S + 1);          /* W of the virtual point that holds term 0 */
+    }
+    return true;
+}
+
+/* enqueue rows a1-a7 for a host-resident batch already copied to d_params, through the component
+ * plan; hist xor nll as in enqueue_finalize */
+phylino_status enqueue_cached(phylino_ctx *ctx, int P, const double *h_params, const double *d_params,
+                              const double *d_data, double *d_hist, double *d_nll, bool *used)
+{
+    *used = false;
+    ctx->last_virtual_points = ctx->last_classes = 0;
+    ComponentPlan pl;
+    if (!plan_components(ctx, P, h_params, pl)) return PHYLINO_OK;
+    const int S = ctx->n_terms, V = pl.V;
+    phylino_status s;
+    /* accumulator rows: V (S + 1); threshold rows and records: sized by ensure_acc for max(P, .) points */
+    if ((s = ensure_acc(ctx, std::max(P, V * (S + 1)))) != PHYLINO_OK) return s;
+    const int64_t n_int = (int64_t)V + (int64_t)V * S + pl.C + (int64_t)P * (S + 1);
+    if (n_int > ctx->plan_capacity) {
+        CU(cudaStreamSynchronize(ctx->stream));
+        cudaFree(ctx->d_plan); ctx->d_plan = nullptr; ctx->plan_capacity = 0;
+        CU(cudaMalloc((void **)&ctx->d_plan, n_int * sizeof(int32_t)));
+        ctx->plan_capacity = n_int;
+    }
+    std::vector<int32_t> blob;
+    blob.reserve((size_t)n_int);
+    blob.insert(blob.end(), pl.vp_class.begin(), pl.vp_class.end());
+    blob.insert(blob.end(), pl.vp_src.begin(), pl.vp_src.end());
+    blob.insert(blob.end(), pl.class_rep.begin(), pl.class_rep.end());
+    blob.insert(blob.end(), pl.pt_comp.begin(), pl.pt_comp.end());
+    /* pageable source: the copy is staged by the driver before the call returns */
+    CU(cudaMemcpyAsync(ctx->d_plan, blob.data(), n_int * sizeof(int32_t), cudaMemcpyHostToDevice, ctx->stream));
+
+    if (ctx->resident_warps == 0) CU(spectra_max_warps(ctx->n_terms, ctx->sm_count, &ctx->resident_warps));
+    SpectraArgs a{};
+    fill_datasets(ctx, a);
+    fill_batch(ctx, a, V, d_params);
+    a.comp = 1;
+    a.thr_rows = pl.C;
+    a.vp_class = ctx->d_plan;
+    a.vp_src = ctx->d_plan + V;
+    a.class_rep = ctx->d_plan + V + (int64_t)V * S;
+    if (ctx->timing) CU(cudaEventRecord(ctx->ev[0], ctx->stream));
+    if (a.n_items > 0) { CU(launch_setup(a, S, ctx->stream)); ctx->launches += 1; }
+    if (ctx->timing) CU(cudaEventRecord(ctx->ev[1], ctx->stream));
+    if (a.n_items > 0) { CU(launch_spectra(a, S, ctx->stream)); ctx->launches += 1; }
+
+    FinalizeArgs f = ctx->fin;
+    f.P = P; f.params = d_params; f.acc = ctx->d_acc; f.flags = ctx->d_flags;
+    f.data = d_data; f.hist = d_hist; f.nll = d_nll;
+    f.comp = 1; f.n_terms = S; f.osc = a.osc;
+    f.pt_comp = ctx->d_plan + V + (int64_t)V * S + pl.C;
+    if (ctx->timing) CU(cudaEventRecord(ctx->ev[2], ctx->stream));
+    CU(launch_finalize(f, d_nll ? 2 : 0, ctx->stream));
+    ctx->launches += 1;
+    if (ctx->timing) CU(cudaEventRecord(ctx->ev[3], ctx->stream));
+    /* the cells are shared between points: cleared here, not by the finalize kernel */
+    const size_t cells = (size_t)V * (S + 1) * ctx->total_bins;
+    CU(cudaMemsetAsync(ctx->d_acc, 0, cells * sizeof(long long), ctx->stream));
+    CU(cudaMemsetAsync(ctx->d_flags, 0, cells * sizeof(unsigned), ctx->stream));
+    ctx->last_virtual_points = V;
+    ctx->last_classes = pl.C;
+    *used = true;
     return PHYLINO_OK;
 }
 
@@ -569,8 +764,14 @@ phylino_status phylino_nll_host(phylino_ctx *ctx, int P, const double *params_ho
     std::memcpy(ctx->h_pin, params_host, np * sizeof(double));
     std::memcpy(ctx->h_pin + np, data_host, tb * sizeof(double));
     CU(cudaMemcpyAsync(ctx->d_stage, ctx->h_pin, (np + tb) * sizeof(double), cudaMemcpyHostToDevice, ctx->stream));
-    if ((s = enqueue_spectra(ctx, P, ctx->d_stage)) != PHYLINO_OK) return s;
-    if ((s = enqueue_finalize(ctx, P, ctx->d_stage, ctx->d_stage + np, nullptr, ctx->d_stage + np + tb)) != PHYLINO_OK) return s;
+    bool cached = false;
+    if (ctx->caching &&
+        (s = enqueue_cached(ctx, P, params_host, ctx->d_stage, ctx->d_stage + np, nullptr, ctx->d_stage + np + tb, &cached)) != PHYLINO_OK)
+        return s;
+    if (!cached) {
+        if ((s = enqueue_spectra(ctx, P, ctx->d_stage)) != PHYLINO_OK) return s;
+        if ((s = enqueue_finalize(ctx, P, ctx->d_stage, ctx->d_stage + np, nullptr, ctx->d_stage + np + tb)) != PHYLINO_OK) return s;
+    }
     CU(cudaMemcpyAsync(ctx->h_pin + np + tb, ctx->d_stage + np + tb, P * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
     CU(cudaStreamSynchronize(ctx->stream));
     std::memcpy(nll_host, ctx->h_pin + np + tb, P * sizeof(double));
@@ -587,8 +788,14 @@ phylino_status phylino_spectra_host(phylino_ctx *ctx, int P, const double *param
     if ((s = ensure_acc(ctx, P)) != PHYLINO_OK) return s;
     std::memcpy(ctx->h_pin, params_host, np * sizeof(double));
     CU(cudaMemcpyAsync(ctx->d_stage, ctx->h_pin, np * sizeof(double), cudaMemcpyHostToDevice, ctx->stream));
-    if ((s = enqueue_spectra(ctx, P, ctx->d_stage)) != PHYLINO_OK) return s;
-    if ((s = enqueue_finalize(ctx, P, ctx->d_stage, nullptr, ctx->d_stage + np, nullptr)) != PHYLINO_OK) return s;
+    bool cached = false;
+    if (ctx->caching &&
+        (s = enqueue_cached(ctx, P, params_host, ctx->d_stage, nullptr, ctx->d_stage + np, nullptr, &cached)) != PHYLINO_OK)
+        return s;
+    if (!cached) {
+        if ((s = enqueue_spectra(ctx, P, ctx->d_stage)) != PHYLINO_OK) return s;
+        if ((s = enqueue_finalize(ctx, P, ctx->d_stage, nullptr, ctx->d_stage + np, nullptr)) != PHYLINO_OK) return s;
+    }
     CU(cudaMemcpyAsync(ctx->h_pin + np, ctx->d_stage + np, nh * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
     CU(cudaStreamSynchronize(ctx->stream));
     std::memcpy(hist_host, ctx->h_pin + np, nh * sizeof(double));
@@ -611,6 +818,21 @@ phylino_status phylino_set_tuning(phylino_ctx *ctx, int unit_events, int chunk_g
     ctx->unit_events = unit_events;
     ctx->chunk_groups = chunk_groups;
     ctx->max_warps = max_warps;
+    return PHYLINO_OK;
+}
+
+phylino_status phylino_set_caching(phylino_ctx *ctx, int on)
+{
+    if (!ctx) return PHYLINO_ERR_ARG;
+    ctx->caching = on != 0;
+    return PHYLINO_OK;
+}
+
+phylino_status phylino_last_plan(const phylino_ctx *ctx, int64_t *virtual_points, int64_t *classes)
+{
+    if (!ctx || !virtual_points || !classes) return PHYLINO_ERR_ARG;
+    *virtual_points = ctx->last_virtual_points;
+    *classes = ctx->last_classes;
     return PHYLINO_OK;
 }
 

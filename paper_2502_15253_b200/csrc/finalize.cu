@@ -10,8 +10,14 @@
  * priors, the warps combine by a fixed shuffle tree and warp 0 adds the warp totals in index
  * order: the result is bitwise reproducible.  The kernel re-zeroes the accumulators it reads so
  * the next call needs no memset launch.
+ *
+ * Component mode (cross-point caching): the spectra kernel summed, per
+ * energy-scale class and distinct mass splitting, W[b] = sum_e w_e and C[b] = sum_e w_e g(h x_e);
+ * here H[p,b] = P0(p) W[b] + sum_k A_k(p) C_k[b] -- the histogram is affine in the amplitudes
+ * (Eq. 1; the paper's own "caching").  Cells are shared between points, so
+ * the caller clears them after this kernel.
  */
-#include "internal.h"
+#include "devmath.cuh"
 
 namespace phylino {
 
@@ -38,14 +44,38 @@ __global__ void __launch_bounds__(FIN_THREADS) finalize_kernel(const __grid_cons
     const double *theta = a.params + (size_t)p * a.n_params;
     const size_t row = (size_t)p * a.total_bins;
     double part = 0.0;
+    double A[MAX_TERMS] = {0.0, 0.0, 0.0}, P0 = 1.0;
+    bool bad = false;
+    if (a.comp) {
+        double dm2[MAX_TERMS], asum = 0.0, half = 0.0;
+        osc_terms(a.osc, theta, A, dm2);
+        for (int k = 0; k < a.n_terms; ++k) { asum += fabs(A[k]); half += A[k]; }
+        P0 = 1.0 - 0.5 * half;
+        bad = !(asum <= 3.0);                               /* as the setup kernel's per-point check */
+    }
 
     for (int g = threadIdx.x; g < a.total_bins; g += FIN_THREADS) {
-        long long q = a.acc[row + g];
-        unsigned fl = a.flags[row + g];
-        if (q) a.acc[row + g] = 0;
-        if (fl) a.flags[row + g] = 0;
         const int d = a.bin_ds[g];
-        double H = (double)q * a.inv_scale[d];              /* 2^-e: exact scaling */
+        double H;
+        unsigned fl = 0;
+        if (a.comp) {
+            const int32_t *rows = a.pt_comp + (size_t)p * (a.n_terms + 1);
+            const size_t c0 = (size_t)rows[0] * a.total_bins + g;
+            fl = a.flags[c0];
+            H = P0 * ((double)a.acc[c0] * a.inv_scale[d]);
+            for (int k = 0; k < a.n_terms; ++k) {
+                const size_t ck = (size_t)rows[k + 1] * a.total_bins + g;
+                fl |= a.flags[ck];
+                H = fma(A[k], (double)a.acc[ck] * a.inv_scale[d], H);
+            }
+            if (fl || bad) fl = FLAG_NAN;
+        } else {
+            long long q = a.acc[row + g];
+            fl = a.flags[row + g];
+            if (q) a.acc[row + g] = 0;
+            if (fl) a.flags[row + g] = 0;
+            H = (double)q * a.inv_scale[d];                 /* 2^-e: exact scaling */
+        }
         if (fl) {
             if ((fl & FLAG_NAN) || ((fl & FLAG_PINF) && (fl & FLAG_NINF)))
                 H = __longlong_as_double(0x7ff8000000000000ll);

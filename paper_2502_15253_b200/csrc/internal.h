@@ -87,6 +87,14 @@ struct SpectraArgs {
     float2       *safe;     /* DEVICE [thr_rows x n_datasets] fp32 interval on which a row holds */
     long long    *acc;      /* DEVICE [P x total_bins] fixed-point accumulators (zero on entry) */
     unsigned     *flags;    /* DEVICE [P x total_bins] FLAG_* (zero on entry) */
+    /* component mode (cross-point caching; api.cu plan_components): the P
+     * "points" of this launch are VIRTUAL points -- an energy-scale class (threshold row) plus S
+     * half-turn coefficients, each taken from (real point, term) of the caller's batch -- and a run
+     * is flushed as S + 1 separate sums (W, C_1..C_S) into acc[(p (S+1) + j) x total_bins + bin]. */
+    int32_t comp;
+    const int32_t *vp_class;    /* DEVICE [P] threshold row of a virtual point */
+    const int32_t *vp_src;      /* DEVICE [P x S] source of slot s: real point * 4 + term */
+    const int32_t *class_rep;   /* DEVICE [thr_rows] real point whose energy scale defines the row */
 };
 
 /* Model tables of the expectation / NLL stage, all DEVICE pointers. */
@@ -109,6 +117,10 @@ struct FinalizeArgs {
     const double  *data;          /* [total_bins] (NLL mode) */
     double        *hist;          /* [P x total_bins] (spectra / expectation mode) */
     double        *nll;           /* [P] (NLL mode) */
+    /* component mode: H[p,b] = P0(p) W[b] + sum_k A_k(p) C_k[b] from the cells pt_comp names */
+    int32_t comp, n_terms;
+    OscDev  osc;
+    const int32_t *pt_comp;       /* [P x (n_terms + 1)] accumulator rows: W, then the row of each term's C */
 };
 
 /* kernel launchers (spectra.cu, finalize.cu, peaks.cu) */
@@ -166,6 +178,11 @@ struct phylino_ctx {
     double   *d_rec = nullptr;                     /* [rec_fields x point_capacity] */
     float    *d_thr = nullptr;                     /* [thr_rows x (total_bins + n_datasets)] */
     float2   *d_safe = nullptr;                    /* [thr_rows x n_datasets] */
+    /* cross-point caching of the host-buffer entry points (phylino_set_caching) */
+    bool caching = false;
+    int32_t *d_plan = nullptr;                     /* vp_class | vp_src | class_rep | pt_comp */
+    int64_t plan_capacity = 0;                     /* int32 entries */
+    int64_t last_virtual_points = 0, last_classes = 0;
     /* host-buffer entry points: pinned + device staging */
     double *h_pin = nullptr, *d_stage = nullptr;
     int64_t stage_capacity = 0;                    /* doubles */

@@ -103,6 +103,17 @@ __device__ __forceinline__ void energy_scale_of(const DatasetDev &ds, const doub
     a2 = ds.idx_a[2] >= 0 ? theta[ds.idx_a[2]] : 0.0;
 }
 
+/* threshold row of launch point p, and the parameter vector its energy scale comes from */
+__device__ __forceinline__ int row_of(const SpectraArgs &a, int p)
+{
+    return a.comp ? a.vp_class[p] : (a.thr_rows > 1 ? p : 0);
+}
+
+__device__ __forceinline__ const double *theta_of(const SpectraArgs &a, int p)
+{
+    return a.params + (size_t)(a.comp ? a.class_rep[a.vp_class[p]] : p) * a.n_params;
+}
+
 /* Bin of one event of dataset ds at one point, and the fp32 bound `hi` below which later (larger)
  * events are known to stay in that bin (-inf: not known, ask again).
  *   table : thr[b] <= v decides E'(v) >= edges[b] for v in [safe.x, safe.y]; the result is the number
@@ -137,6 +148,17 @@ __global__ void __launch_bounds__(SETUP_THREADS) setup_kernel(const __grid_const
         const int p = blockIdx.x * SETUP_THREADS + threadIdx.x;
         if (p == 0) *a.counter = 2u * (unsigned)a.n_warps;     /* see spectra_kernel */
         if (p >= a.P) return;
+        if (a.comp) {
+            /* virtual point: slot s computes the half-turn coefficient of (real point, term) vp_src */
+#pragma unroll
+            for (int k = 0; k < S; ++k) {
+                const int src = a.vp_src[(size_t)p * S + k];
+                double A[MAX_TERMS], dm2[MAX_TERMS];
+                osc_terms(a.osc, a.params + (size_t)(src >> 2) * a.n_params, A, dm2);
+                a.rec[(size_t)k * a.P + p] = halfturn_coeff(dm2[src & 3]);
+            }
+            return;
+        }
         const double *theta = a.params + (size_t)p * a.n_params;
         double A[MAX_TERMS], dm2[MAX_TERMS];
         osc_terms(a.osc, theta, A, dm2);
@@ -154,7 +176,8 @@ __global__ void __launch_bounds__(SETUP_THREADS) setup_kernel(const __grid_const
         return;
     }
     const int row = blockIdx.x - rec_blocks;
-    const double *theta = a.params + (size_t)row * a.n_params;         /* only read where idx_a >= 0 */
+    /* only read where idx_a >= 0 */
+    const double *theta = a.params + (size_t)(a.comp ? a.class_rep[row] : row) * a.n_params;
     for (int e = threadIdx.x; e < a.thr_stride; e += SETUP_THREADS) {
         int d = 0;
         for (int i = 1; i < a.n_datasets; ++i)
@@ -204,7 +227,17 @@ template <int S> struct Run {
 template <int S>
 __device__ __forceinline__ void flush_run(const SpectraArgs &a, const DatasetDev &ds, int p, bool active, Run<S> &r)
 {
-    if (active && r.cur >= 0 && r.cur < ds.n_bins) {
+    if (a.comp && active && r.cur >= 0 && r.cur < ds.n_bins) {
+        /* component mode: W and every C_k go to cells of their own (the amplitudes come later) */
+        const size_t cell = (size_t)p * (S + 1) * a.total_bins + ds.bin_off + r.cur;
+#pragma unroll
+        for (int j = 0; j <= S; ++j) {
+            unsigned fl;
+            const long long q = to_fixed(j == 0 ? r.W : r.C[j - 1], ds.fx_scale, false, fl);
+            if (q) atomicAdd((unsigned long long *)a.acc + cell + (size_t)j * a.total_bins, (unsigned long long)q);
+            if (fl) atomicOr(a.flags + cell + (size_t)j * a.total_bins, fl);
+        }
+    } else if (active && r.cur >= 0 && r.cur < ds.n_bins) {
         double tot = a.rec[(size_t)(2 * S) * a.P + p] * r.W;                 /* P0 W */
 #pragma unroll
         for (int k = 0; k < S; ++k) tot = fma(a.rec[(size_t)(S + k) * a.P + p], r.C[k], tot);
@@ -274,7 +307,7 @@ __device__ __forceinline__ void walk_batch(const SpectraArgs &a, const DatasetDe
                     nhi = r.hi2;
                     while (b < B && !(v[j] < nhi)) { ++b; nhi = thr_at(thr, B, b + 1); }
                 } else {
-                    b = locate_bin(ds, thr, safe, a.params + (size_t)p * a.n_params, v[j], nhi);
+                    b = locate_bin(ds, thr, safe, theta_of(a, p), v[j], nhi);
                 }
                 if (b != r.cur) {
                     flush_run<S>(a, ds, p, active, r);
@@ -336,7 +369,7 @@ __device__ __forceinline__ void walk_unit(const SpectraArgs &a, const DatasetDev
     double h[S];
 #pragma unroll
     for (int k = 0; k < S; ++k) h[k] = a.rec[(size_t)k * a.P + p];
-    const int row = a.thr_rows > 1 ? p : 0;
+    const int row = row_of(a, p);
     const float *thr = a.thr + (size_t)row * a.thr_stride + ds.thr_off;
     const float2 safe = a.safe[(size_t)row * a.n_datasets + d];
     const int B = ds.n_bins;
@@ -524,10 +557,10 @@ __global__ void __launch_bounds__(256) event_bins_kernel(const __grid_constant__
     const int p = blockIdx.y;
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
-    const int row = a.thr_rows > 1 ? p : 0;
+    const int row = row_of(a, p);
     float hi;
     int b = locate_bin(ds, a.thr + (size_t)row * a.thr_stride + ds.thr_off, a.safe[(size_t)row * a.n_datasets + d],
-                       a.params + (size_t)p * a.n_params, ds.ev[i / EB].v[i % EB], hi);
+                       theta_of(a, p), ds.ev[i / EB].v[i % EB], hi);
     bins[(size_t)p * total_events + ev_off + perm[i]] = (b >= 0 && b < ds.n_bins) ? b : -1;
 }
 } // namespace
