@@ -237,7 +237,7 @@ phylino_status enqueue_spectra(phylino_ctx *ctx, int P, const double *params)
     }
     if (ctx->timing) CU(cudaEventRecord(ctx->ev[1], ctx->stream));
     if (a.n_items > 0 && P > 0) {
-        CU(launch_spectra(a, ctx->n_terms, ctx->stream));
+        CU(launch_spectra(a, ctx->n_terms, ctx->stream, !ctx->timing));
         ctx->launches += 1;
     }
     return PHYLINO_OK;
@@ -256,7 +256,7 @@ phylino_status enqueue_finalize(phylino_ctx *ctx, int P, const double *params, c
     f.hist = hist;
     f.nll = nll;
     if (ctx->timing) CU(cudaEventRecord(ctx->ev[2], ctx->stream));
-    CU(launch_finalize(f, mode, ctx->stream));
+    CU(launch_finalize(f, mode, ctx->stream, !ctx->timing));
     ctx->launches += 1;
     if (ctx->timing) CU(cudaEventRecord(ctx->ev[3], ctx->stream));
     return PHYLINO_OK;
@@ -447,7 +447,7 @@ phylino_status enqueue_cached(phylino_ctx *ctx, int P, const double *h_params, c
     if (ctx->timing) CU(cudaEventRecord(ctx->ev[0], ctx->stream));
     if (a.n_items > 0) { CU(launch_setup(a, S, ctx->stream)); ctx->launches += 1; }
     if (ctx->timing) CU(cudaEventRecord(ctx->ev[1], ctx->stream));
-    if (a.n_items > 0) { CU(launch_spectra(a, S, ctx->stream)); ctx->launches += 1; }
+    if (a.n_items > 0) { CU(launch_spectra(a, S, ctx->stream, !ctx->timing)); ctx->launches += 1; }
 
     FinalizeArgs f = ctx->fin;
     f.P = P; f.params = d_params; f.acc = ctx->d_acc; f.flags = ctx->d_flags;
@@ -455,7 +455,7 @@ phylino_status enqueue_cached(phylino_ctx *ctx, int P, const double *h_params, c
     f.comp = 1; f.n_terms = S; f.osc = a.osc;
     f.pt_comp = ctx->d_plan + V + (int64_t)V * S + pl.C;
     if (ctx->timing) CU(cudaEventRecord(ctx->ev[2], ctx->stream));
-    CU(launch_finalize(f, d_nll ? 2 : 0, ctx->stream));
+    CU(launch_finalize(f, d_nll ? 2 : 0, ctx->stream, !ctx->timing));
     ctx->launches += 1;
     if (ctx->timing) CU(cudaEventRecord(ctx->ev[3], ctx->stream));
     /* the cells are shared between points: cleared here, not by the finalize kernel */

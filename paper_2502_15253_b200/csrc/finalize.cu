@@ -40,6 +40,8 @@ __device__ __forceinline__ double half_deviance(double n, double mu)
 template <int MODE>   /* 0 = spectra H, 1 = expectation mu, 2 = NLL */
 __global__ void __launch_bounds__(FIN_THREADS) finalize_kernel(const __grid_constant__ FinalizeArgs a)
 {
+    /* launched as a programmatic dependent of the spectra kernel: wait for its accumulators */
+    asm volatile("griddepcontrol.wait;" ::: "memory");
     const int p = blockIdx.x;
     const double *theta = a.params + (size_t)p * a.n_params;
     const size_t row = (size_t)p * a.total_bins;
@@ -127,13 +129,21 @@ __global__ void __launch_bounds__(FIN_THREADS) finalize_kernel(const __grid_cons
 
 } // namespace
 
-cudaError_t launch_finalize(const FinalizeArgs &a, int mode, cudaStream_t st)
+cudaError_t launch_finalize(const FinalizeArgs &a, int mode, cudaStream_t st, bool pdl)
 {
     if (a.P <= 0) return cudaSuccess;
-    if (mode == 2)      finalize_kernel<2><<<a.P, FIN_THREADS, 0, st>>>(a);
-    else if (mode == 1) finalize_kernel<1><<<a.P, FIN_THREADS, 0, st>>>(a);
-    else                finalize_kernel<0><<<a.P, FIN_THREADS, 0, st>>>(a);
-    return cudaGetLastError();
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(a.P);
+    cfg.blockDim = dim3(FIN_THREADS);
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = pdl ? 1 : 0;
+    if (mode == 2) return cudaLaunchKernelEx(&cfg, finalize_kernel<2>, a);
+    if (mode == 1) return cudaLaunchKernelEx(&cfg, finalize_kernel<1>, a);
+    return cudaLaunchKernelEx(&cfg, finalize_kernel<0>, a);
 }
 
 } // namespace phylino

@@ -126,8 +126,8 @@ struct FinalizeArgs {
 /* kernel launchers (spectra.cu, finalize.cu, peaks.cu) */
 cudaError_t launch_setup(const SpectraArgs &a, int S, cudaStream_t st);
 cudaError_t spectra_max_warps(int S, int sm_count, int *warps);
-cudaError_t launch_spectra(const SpectraArgs &a, int S, cudaStream_t st);
-cudaError_t launch_finalize(const FinalizeArgs &a, int mode /*0 H, 1 mu, 2 nll*/, cudaStream_t st);
+cudaError_t launch_spectra(const SpectraArgs &a, int S, cudaStream_t st, bool pdl);
+cudaError_t launch_finalize(const FinalizeArgs &a, int mode /*0 H, 1 mu, 2 nll*/, cudaStream_t st, bool pdl);
 cudaError_t launch_event_bins(const SpectraArgs &a, int d, const int32_t *perm, long long n, long long ev_off,
                               long long total_events, int32_t *bins, cudaStream_t st);
 cudaError_t run_peak_fp64(int iters, cudaStream_t st, double *dfma_per_s);

@@ -144,6 +144,9 @@ __device__ __forceinline__ int locate_bin(const DatasetDev &ds, const float *thr
 template <int S>
 __global__ void __launch_bounds__(SETUP_THREADS) setup_kernel(const __grid_constant__ SpectraArgs a, int rec_blocks)
 {
+    /* programmatic dependent launch: the spectra kernel may start its prologue (barriers, first copy of
+     * event data) now; it waits for this grid to finish before it reads anything written here */
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     if ((int)blockIdx.x < rec_blocks) {
         const int p = blockIdx.x * SETUP_THREADS + threadIdx.x;
         if (p == 0) *a.counter = 2u * (unsigned)a.n_warps;     /* see spectra_kernel */
@@ -473,6 +476,10 @@ __global__ void __launch_bounds__(WARPS * 32, 4) spectra_kernel(const __grid_con
         decode_item(a, cur, d, b0, b1, chunk);
         bulk_load(buf0, a.ds[d].ev + b0, (unsigned)(b1 - b0) * (unsigned)sizeof(EventBatch), &bars[wib][0]);
     }
+    /* everything above touched only kernel parameters and the event store; the records, thresholds
+     * and the work counter come from the setup kernel (no-op unless launched as its dependent) */
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
 #pragma unroll 1
     while (cur < n_items) {
         const unsigned ticket = take_ticket(a.counter, lane);
@@ -503,10 +510,19 @@ __global__ void __launch_bounds__(WARPS * 32, 4) spectra_kernel(const __grid_con
 /* dynamic shared memory of one CTA: two unit buffers per warp, sized for the largest unit */
 constexpr size_t STAGE_BYTES = (size_t)WARPS * 2 * MAX_UNIT_BATCHES * sizeof(EventBatch);
 
-template <int S> cudaError_t launch_t(const SpectraArgs &a, cudaStream_t st)
+template <int S> cudaError_t launch_t(const SpectraArgs &a, cudaStream_t st, bool pdl)
 {
-    spectra_kernel<S><<<a.n_warps / WARPS, WARPS * 32, STAGE_BYTES, st>>>(a);
-    return cudaGetLastError();
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(a.n_warps / WARPS);
+    cfg.blockDim = dim3(WARPS * 32);
+    cfg.dynamicSmemBytes = STAGE_BYTES;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = pdl ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, spectra_kernel<S>, a);
 }
 
 template <int S> cudaError_t max_warps_t(int sm_count, int *warps)
@@ -539,10 +555,10 @@ cudaError_t launch_setup(const SpectraArgs &a, int S, cudaStream_t st)
 }
 
 /* persistent grid of a.n_warps warps (a multiple of WARPS) that claim the a.n_items work items */
-cudaError_t launch_spectra(const SpectraArgs &a, int S, cudaStream_t st)
+cudaError_t launch_spectra(const SpectraArgs &a, int S, cudaStream_t st, bool pdl)
 {
     if (a.n_items <= 0 || a.P <= 0 || a.n_warps < WARPS) return cudaSuccess;
-    return S == 2 ? launch_t<2>(a, st) : launch_t<3>(a, st);
+    return S == 2 ? launch_t<2>(a, st, pdl) : launch_t<3>(a, st, pdl);
 }
 
 /* ---- diagnostic: bin index of every event at every point (bit-exact parity of row a3) ----
