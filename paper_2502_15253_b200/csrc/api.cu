@@ -160,6 +160,7 @@ void fill_datasets(const phylino_ctx *ctx, SpectraArgs &a)
         v.per_point = (h.idx_a[0] >= 0 || h.idx_a[1] >= 0 || h.idx_a[2] >= 0) ? 1 : 0;
         v.n_batches = (int32_t)(h.n_pad / EB);
         for (int j = 0; j < 3; ++j) v.idx_a[j] = h.idx_a[j];
+        v.unit_w = h.unit_w ? 1 : 0;
         v.v_pos_min = h.v_pos_min;
         v.v_max = h.v_max;
         v.fx_scale = std::ldexp(1.0, h.fx_exp);
@@ -655,6 +656,7 @@ phylino_status phylino_load_events(phylino_ctx *ctx, int dataset, int64_t n, con
     for (int j = 0; j < EB; ++j) blank.v[j] = std::nanf("");
     std::vector<EventBatch> ev((size_t)(n_pad / EB), blank);
     double wsum = 0.0;
+    bool unit_w = true;
     float v_pos_min = INFINITY, v_max = -INFINITY;
     for (int64_t i = 0; i < n; ++i) {
         int32_t s = perm[i];
@@ -668,6 +670,7 @@ phylino_status phylino_load_events(phylino_ctx *ctx, int dataset, int64_t n, con
         if (j == 0)                             /* where a lane starts looking for its bin (a hint, never trusted) */
             b.bin0 = vi == vi ? (int32_t)(std::upper_bound(edges, edges + n_bins + 1, (double)vi) - edges) - 1 : n_bins;
         wsum += std::fabs(b.w[j]);
+        unit_w = unit_w && b.w[j] == 1.0;
         if (std::isfinite(vi)) {
             if (vi > 0.0f && vi < v_pos_min) v_pos_min = vi;
             if (vi > v_max) v_max = vi;
@@ -690,7 +693,7 @@ phylino_status phylino_load_events(phylino_ctx *ctx, int dataset, int64_t n, con
     CU(cudaMemcpyAsync((void *)(ctx->fin.inv_scale + dataset), &inv, sizeof(double), cudaMemcpyHostToDevice, st));
     CU(cudaStreamSynchronize(st));
     h.n = n; h.n_pad = n_pad; h.wsum_abs = wsum; h.fx_exp = fx; h.loaded = true;
-    h.v_pos_min = v_pos_min; h.v_max = v_max;
+    h.v_pos_min = v_pos_min; h.v_max = v_max; h.unit_w = unit_w;
     ctx->err.clear();
     return PHYLINO_OK;
 }

@@ -48,6 +48,7 @@ struct DatasetDev {
     int32_t bin_off;        /* offset of this dataset inside a point's total_bins */
     int32_t thr_off;        /* offset of this dataset inside a threshold row: sum of (n_bins+1) before it */
     int32_t per_point;      /* the energy scale of this dataset depends on theta */
+    int32_t unit_w;         /* every event weight of the dataset is exactly 1 */
     int32_t n_batches;
     int32_t unit_begin;     /* first global unit of this dataset (units never straddle datasets) */
     int32_t idx_a[3];       /* energy-scale indices into theta, -1 => (0,1,0) */
@@ -149,6 +150,7 @@ struct phylino_dataset_host {
     int64_t  n = 0, n_pad = 0;
     double   wsum_abs = 0.0;
     float    v_pos_min = 0.f, v_max = 0.f;
+    bool     unit_w = false;
     int      fx_exp = 0;
     phylino::EventBatch *d_ev = nullptr;
     double  *d_edges = nullptr;

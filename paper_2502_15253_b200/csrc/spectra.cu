@@ -328,7 +328,7 @@ __device__ __forceinline__ void walk_batch(const SpectraArgs &a, const DatasetDe
 
 /* Two consecutive batches known to lie inside the lane's open run (the store is sorted: the last
  * event of the second batch is below r.hi): rows a2 + a4 only, straight-line. */
-template <int S>
+template <int S, bool UW>
 __device__ __forceinline__ void walk_pair_inside(const EventBatch *bp, const double (&h)[S], Run<S> &r)
 {
 #pragma unroll
@@ -336,19 +336,29 @@ __device__ __forceinline__ void walk_pair_inside(const EventBatch *bp, const dou
         const double2 *q = reinterpret_cast<const double2 *>(bp + u);
 #pragma unroll
         for (int j = 0; j < EB / 2; ++j) {
-            const double2 t = q[j], w = q[EB / 2 + j];
+            const double2 t = q[j];
+            if (UW) {
+                /* every weight of the dataset is exactly 1 (the padding, weight 0, sits behind a NaN E_vis
+                 * and never reaches this path): 1 * g + C == g + C bit for bit, and w is not loaded */
 #pragma unroll
-            for (int k = 0; k < S; ++k) r.C[k] = fma(w.x, half_cos_halfturns(h[k], t.x), r.C[k]);
+                for (int k = 0; k < S; ++k) r.C[k] += half_cos_halfturns(h[k], t.x);
 #pragma unroll
-            for (int k = 0; k < S; ++k) r.C[k] = fma(w.y, half_cos_halfturns(h[k], t.y), r.C[k]);
+                for (int k = 0; k < S; ++k) r.C[k] += half_cos_halfturns(h[k], t.y);
+            } else {
+                const double2 w = q[EB / 2 + j];
+#pragma unroll
+                for (int k = 0; k < S; ++k) r.C[k] = fma(w.x, half_cos_halfturns(h[k], t.x), r.C[k]);
+#pragma unroll
+                for (int k = 0; k < S; ++k) r.C[k] = fma(w.y, half_cos_halfturns(h[k], t.y), r.C[k]);
+            }
         }
-        r.W += bp[u].wsum;
+        r.W += UW ? (double)EB : bp[u].wsum;
     }
 }
 
 /* One warp, the nb batches of one unit of dataset ds staged at `unit` (SHARED memory), point group g
  * (points 32 g ... 32 g + 31).  FULL: the group has 32 points, every lane walks all batches. */
-template <int S, bool FULL>
+template <int S, bool FULL, bool UW>
 __device__ __forceinline__ void walk_unit(const SpectraArgs &a, const DatasetDev &ds, int d, const EventBatch *unit,
                                           int nb, int g, int lane)
 {
@@ -406,7 +416,7 @@ __device__ __forceinline__ void walk_unit(const SpectraArgs &a, const DatasetDev
 #pragma unroll 1
         while (i < nb) {
             if (i + 2 <= nb && bp[1].v[EB - 1] < r.hi) {
-                walk_pair_inside<S>(bp, h, r);
+                walk_pair_inside<S, UW>(bp, h, r);
                 i += 2;
                 bp += 2;
             } else {
@@ -498,8 +508,10 @@ __global__ void __launch_bounds__(WARPS * 32, 4) spectra_kernel(const __grid_con
         const int g1 = min((chunk + 1) * a.chunk_groups, n_groups);
 #pragma unroll 1
         for (int g = chunk * a.chunk_groups; g < g1; ++g) {
-            if (32 * g + 32 <= a.P) walk_unit<S, true>(a, ds, d, buf0 + b * a.unit_batches, b1 - b0, g, lane);
-            else                    walk_unit<S, false>(a, ds, d, buf0 + b * a.unit_batches, b1 - b0, g, lane);
+            const EventBatch *unit = buf0 + b * a.unit_batches;
+            if (32 * g + 32 > a.P) walk_unit<S, false, false>(a, ds, d, unit, b1 - b0, g, lane);
+            else if (ds.unit_w)    walk_unit<S, true, true>(a, ds, d, unit, b1 - b0, g, lane);
+            else                   walk_unit<S, true, false>(a, ds, d, unit, b1 - b0, g, lane);
         }
         cur = nxt;
         nxt = __shfl_sync(0xffffffffu, ticket, 0);      /* also orders this item's reads before the next copy */

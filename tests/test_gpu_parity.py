@@ -69,6 +69,16 @@ def test_tiny_inputs(gpu, oracle_mod, osc, n_datasets):
     _run_case(gpu, oracle_mod, wl)
 
 
+@pytest.mark.parametrize("osc", [OSC_EQ1, OSC_STERILE4])
+def test_weighted_events_full_point_groups(gpu, oracle_mod, osc):
+    """Random weights U(0.5, 1.5) with 70 points: two full groups of 32 lanes (the weighted straight-line
+    path; the BASELINE configs all have weight 1 and take the unit-weight one) plus a ragged group of 6."""
+    wl = workloads.make_tiny(seed=91 + osc, osc_model=osc, n_events=3001, n_points=70, n_datasets=2)
+    assert any(np.any(e.w != 1.0) for e in wl.events)
+    _run_case(gpu, oracle_mod, wl)
+    _run_case(gpu, oracle_mod, wl, tuning=(64, 1, 0))
+
+
 # scaled-down copies of the five BASELINE.json configs: several CTA tiles (2048 events) per dataset
 # and a ragged tail, a point count that is not a multiple of the point chunk
 @pytest.mark.parametrize("k,scale,n_points", [(1, 0.137, 3), (2, 0.0123, 19), (3, 0.0051, 41),
