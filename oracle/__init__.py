@@ -46,10 +46,15 @@ class _Dataset(C.Structure):
                 ("bkg", C.POINTER(_Bkg))]
 
 
+class _PriorBlock(C.Structure):
+    _fields_ = [("n", C.c_int32), ("idx", C.c_void_p), ("mean", C.c_void_p), ("inv_cov", C.c_void_p)]
+
+
 class _Model(C.Structure):
     _fields_ = [("osc_model", C.c_int32), ("ordering", C.c_int32), ("n_params", C.c_int32),
                 ("n_datasets", C.c_int32), ("idx_osc", C.c_int32 * 6), ("fixed_osc", C.c_double * 6),
-                ("datasets", C.POINTER(_Dataset)), ("prior_mean", C.c_void_p), ("prior_sigma", C.c_void_p)]
+                ("datasets", C.POINTER(_Dataset)), ("prior_mean", C.c_void_p), ("prior_sigma", C.c_void_p),
+                ("n_prior_blocks", C.c_int32), ("prior_blocks", C.POINTER(_PriorBlock))]
 
 
 _lib = None
@@ -139,6 +144,18 @@ class Oracle:
         m.datasets = C.cast(ds_arr, C.POINTER(_Dataset))
         m.prior_mean = None if model.prior_mean is None else self._arr(model.prior_mean, np.float64)
         m.prior_sigma = None if model.prior_sigma is None else self._arr(model.prior_sigma, np.float64)
+        blocks = list(getattr(model, "prior_blocks", None) or [])
+        pb = (_PriorBlock * max(1, len(blocks)))()
+        for k, b in enumerate(blocks):
+            n = len(b.idx)
+            assert np.shape(b.mean) == (n,) and np.shape(b.inv_cov) == (n, n)
+            pb[k].n = n
+            pb[k].idx = self._arr(b.idx, np.int32)
+            pb[k].mean = self._arr(b.mean, np.float64)
+            pb[k].inv_cov = self._arr(b.inv_cov, np.float64)
+        self._keep.append(pb)
+        m.n_prior_blocks = len(blocks)
+        m.prior_blocks = C.cast(pb, C.POINTER(_PriorBlock)) if blocks else None
         return m
 
     def _marshal_events(self, events):

@@ -274,6 +274,18 @@ int orc_nll_from_mu(const orc_model *m, int32_t P, const double *params, const d
                 nsum(&s, &c, 0.5 * z * z);
             }
         }
+        /* correlated constraints G((b - b0)^T V^-1 (b - b0)) (Eq. 9):
+         * -ln G = 1/2 (b - b0)^T V^-1 (b - b0) + const, the plain double sum over i, j */
+        for (int32_t k = 0; k < m->n_prior_blocks; ++k) {
+            const orc_prior_block *B = &m->prior_blocks[k];
+            for (int32_t i = 0; i < B->n; ++i) {
+                double di = theta[B->idx[i]] - B->mean[i];
+                for (int32_t j = 0; j < B->n; ++j) {
+                    double dj = theta[B->idx[j]] - B->mean[j];
+                    nsum(&s, &c, 0.5 * di * B->inv_cov[(int64_t)i * B->n + j] * dj);
+                }
+            }
+        }
         nll[p] = s + c;
     }
     return 0;

@@ -56,6 +56,15 @@ typedef struct {
     const orc_bkg *bkg;
 } orc_dataset;
 
+/* One correlated Gaussian constraint: (b - b0)^T V^-1 (b - b0) over the parameters idx
+ * (third factor of Eq. 9; "multiple parameters with correlations"). */
+typedef struct {
+    int32_t        n;
+    const int32_t *idx;        /* [n] indices into theta */
+    const double  *mean;       /* [n] b0 */
+    const double  *inv_cov;    /* [n*n] V^-1, row-major */
+} orc_prior_block;
+
 typedef struct {
     int32_t            osc_model;    /* ORC_EQ1 / ORC_FULL3 / ORC_STERILE4 */
     int32_t            ordering;     /* +1 normal, -1 inverted (FULL3) */
@@ -66,6 +75,8 @@ typedef struct {
     const orc_dataset *datasets;
     const double      *prior_mean;   /* [n_params] or NULL */
     const double      *prior_sigma;  /* [n_params] or NULL; <=0, inf or NaN => unconstrained */
+    int32_t                n_prior_blocks;
+    const orc_prior_block *prior_blocks; /* [n_prior_blocks] or NULL */
 } orc_model;
 
 /* O1-O2: amplitudes A_k and mass splittings m_k [eV^2] of the oscillation terms at one point.
@@ -98,7 +109,8 @@ int orc_expectation(const orc_model *m, int32_t P, const double *params, const d
 /* Half-deviance of one bin, mu - n + n ln(n/mu)  (PAPER.md:67 Eq. 3, :96 Eq. 8; R9-R10). */
 double orc_dev(double n, double mu);
 
-/* O5: nll[p] = sum_bins dev(n, mu) + 1/2 sum_j ((theta_j - mean_j)/sigma_j)^2  (PAPER.md:82 Eq. 6, :119 Eq. 9). */
+/* O5: nll[p] = sum_bins dev(n, mu) + 1/2 sum_j ((theta_j - mean_j)/sigma_j)^2
+ *             + 1/2 sum_blocks (b - b0)^T V^-1 (b - b0)            (PAPER.md:82 Eq. 6, :119-123 Eq. 9). */
 int orc_nll_from_mu(const orc_model *m, int32_t P, const double *params, const double *mu,
                     const double *data, double *nll);
 

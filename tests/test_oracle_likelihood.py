@@ -127,3 +127,80 @@ def test_infinite_and_nan_bins_propagate(oracle_mod):
     th = np.array([1.0, 1.0, 1.0, 1.0, 1.0, 1.0, 0.0])
     assert o.nll_from_mu(th, np.array([[0.0, 6.0]]), np.array([2.0, 6.0]))[0] == math.inf
     assert math.isnan(o.nll_from_mu(th, np.array([[np.nan, 6.0]]), np.array([2.0, 6.0]))[0])
+
+
+# ---- correlated prior blocks (third factor of Eq. 9) ---------------------
+
+def _toy_with_blocks(blocks, sigma=None):
+    m = _toy_model()
+    m.prior_sigma = np.zeros(7) if sigma is None else sigma      # diagonal priors off unless asked for
+    m.prior_blocks = blocks
+    return m
+
+
+def test_prior_block_diagonal_reduces_to_uncorrelated_gaussians(oracle_mod):
+    """V = diag(sigma^2): the block term is the plain sum of 1/2 z^2 (the routine pinned above)."""
+    sig = np.array([0.1, 0.02, 0.02, 0.0, 0.05, np.inf, 0.3])
+    idx = np.array([0, 1, 2, 4, 6], np.int32)
+    mean = _toy_model().prior_mean
+    blk = W.PriorBlock(idx=idx, mean=mean[idx], inv_cov=np.diag(1.0 / sig[idx] ** 2))
+    a = oracle_mod.Oracle(_toy_model())                           # diagonal priors
+    b = oracle_mod.Oracle(_toy_with_blocks([blk]))                # the same constraint as one block
+    rng = np.random.default_rng(5)
+    mu, n = np.array([[4.0, 6.0]]), np.array([3.0, 9.0])
+    for _ in range(20):
+        th = mean + rng.normal(0, 0.1, 7)
+        assert b.nll_from_mu(th, mu, n)[0] == pytest.approx(a.nll_from_mu(th, mu, n)[0], rel=1e-13)
+
+
+def test_prior_block_bivariate_closed_form(oracle_mod):
+    """2 x 2 block: q = (z1^2 - 2 rho z1 z2 + z2^2) / (1 - rho^2), the textbook bivariate normal exponent."""
+    s1, s2, rho = 0.03, 0.2, -0.6
+    V = np.array([[s1 * s1, rho * s1 * s2], [rho * s1 * s2, s2 * s2]])
+    blk = W.PriorBlock(idx=np.array([4, 1], np.int32), mean=np.array([1.0, 0.9]), inv_cov=np.linalg.inv(V))
+    o = oracle_mod.Oracle(_toy_with_blocks([blk]))
+    th = np.array([1.0, 0.95, 1.0, 1.0, 1.04, 1.0, 0.0])
+    z1, z2 = (1.04 - 1.0) / s1, (0.95 - 0.9) / s2
+    want = 0.5 * (z1 * z1 - 2 * rho * z1 * z2 + z2 * z2) / (1 - rho * rho)
+    got = o.nll_from_mu(th, np.array([[4.0, 6.0]]), np.array([4.0, 6.0]))[0]
+    assert got == pytest.approx(want, rel=1e-12)
+
+
+def test_prior_blocks_against_scipy_multivariate_normal(oracle_mod):
+    """nll(theta) - nll(b0) = -[ln N(theta; b0, V) - ln N(b0; b0, V)] for two blocks of size 3 and 41."""
+    from scipy.stats import multivariate_normal
+    rng = np.random.default_rng(11)
+    n_par = 50
+    ds = DatasetSpec(n_bins=2, norm=1.0)
+    A3, A41 = rng.normal(size=(3, 3)), rng.normal(size=(41, 41))
+    V3, V41 = A3 @ A3.T + 0.5 * np.eye(3), A41 @ A41.T / 41 + 0.2 * np.eye(41)   # the paper's 41 x 41 flux block size
+    i3 = np.array([47, 2, 45], np.int32)
+    i41 = np.arange(3, 44, dtype=np.int32)
+    m3, m41 = rng.normal(size=3), rng.normal(size=41)
+    model = ModelSpec(osc_model=OSC_EQ1, n_params=n_par, idx_osc=(-1,) * 6, fixed_osc=(0,) * 6, datasets=[ds],
+                      prior_blocks=[W.PriorBlock(i3, m3, np.linalg.inv(V3)), W.PriorBlock(i41, m41, np.linalg.inv(V41))])
+    o = oracle_mod.Oracle(model)
+    mu, n = np.array([[4.0, 6.0]]), np.array([4.0, 6.0])
+    th0 = np.zeros(n_par)
+    th0[i3], th0[i41] = m3, m41
+    assert o.nll_from_mu(th0, mu, n)[0] == 0.0
+    for _ in range(10):
+        th = th0 + rng.normal(0, 0.3, n_par)
+        want = -(multivariate_normal(m3, V3).logpdf(th[i3]) - multivariate_normal(m3, V3).logpdf(m3)) \
+               - (multivariate_normal(m41, V41).logpdf(th[i41]) - multivariate_normal(m41, V41).logpdf(m41))
+        assert o.nll_from_mu(th, mu, n)[0] == pytest.approx(want, rel=1e-9)
+
+
+def test_prior_block_order_and_asymmetry(oracle_mod):
+    """Relabelling the parameters of a block (with the matrix permuted alike) changes nothing; an
+    unsymmetrised matrix M counts as (M + M^T)/2 -- the double sum is taken as written."""
+    rng = np.random.default_rng(3)
+    M = rng.normal(size=(4, 4))
+    idx, mean = np.array([0, 2, 4, 5], np.int32), rng.normal(size=4)
+    perm = np.array([2, 0, 3, 1])
+    th = rng.normal(size=7)
+    mu, n = np.array([[4.0, 6.0]]), np.array([4.0, 6.0])
+    f = lambda blk: oracle_mod.Oracle(_toy_with_blocks([blk])).nll_from_mu(th, mu, n)[0]
+    base = f(W.PriorBlock(idx, mean, M))
+    assert f(W.PriorBlock(idx[perm], mean[perm], M[np.ix_(perm, perm)])) == pytest.approx(base, rel=1e-12, abs=1e-14)
+    assert f(W.PriorBlock(idx, mean, 0.5 * (M + M.T))) == pytest.approx(base, rel=1e-12, abs=1e-14)

@@ -58,6 +58,15 @@ class DatasetEvents:
 
 
 @dataclass
+class PriorBlock:
+    """One correlated Gaussian constraint (Eq. 9 third factor): parameters idx with
+    central values mean and INVERSE covariance inv_cov (row-major [n, n], symmetric)."""
+    idx: np.ndarray           # int32 [n] indices into theta
+    mean: np.ndarray          # float64 [n]
+    inv_cov: np.ndarray       # float64 [n, n]
+
+
+@dataclass
 class ModelSpec:
     osc_model: int
     n_params: int
@@ -67,6 +76,7 @@ class ModelSpec:
     ordering: int = +1                      # +1 normal, -1 inverted (FULL3 only)
     prior_mean: Optional[np.ndarray] = None   # float64 [n_params]
     prior_sigma: Optional[np.ndarray] = None  # float64 [n_params]; <= 0 or inf => unconstrained
+    prior_blocks: List[PriorBlock] = field(default_factory=list)
 
     @property
     def total_bins(self) -> int:
