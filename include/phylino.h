@@ -13,6 +13,7 @@
  *   H[p,d,b]  = sum over MC events e of dataset d with edges[b] <= E' < edges[b+1] of w(e) P_ee(e,p)
  *   mu[p,d,b] = eps_d norm_d f_db H[p,d,b] + sum_k r_dk s_dkb T_dkb
  *   nll[p]    = sum_{d,b} [mu - n + n ln(n/mu)] + 1/2 sum_j ((theta_j - mean_j)/sigma_j)^2
+ *               + 1/2 sum_blocks (b - b0)^T V^-1 (b - b0)     (phylino_set_prior_blocks)
  *               (PAPER.md:67-83 Eq. 3-6, :96 Eq. 8, :119-125 Eq. 9; R9, R10)
  *
  * Conventions
@@ -107,6 +108,18 @@ typedef struct {
                                     (sin^2 2th13 is left free) */
 } phylino_model_desc;
 
+/* One correlated Gaussian constraint over several parameters ("multiple parameters with
+ * correlations", third factor of Eq. 9): G((b - b0)^T V^-1 (b - b0)) with b = theta[idx].
+ * HOST pointers, deep-copied. */
+typedef struct {
+    int32_t        n;          /* parameters in the block, 1 ... PHYLINO_MAX_BLOCK */
+    const int32_t *idx;        /* HOST [n] indices into theta, each 0 ... n_params-1 */
+    const double  *mean;       /* HOST [n] central values b0 */
+    const double  *inv_cov;    /* HOST [n*n] INVERSE covariance V^-1, row-major; used as written (an
+                                  unsymmetric matrix counts as its symmetric part) */
+} phylino_prior_block;
+#define PHYLINO_MAX_BLOCK 1024
+
 /* Create a context on CUDA device `device`.  `cuda_stream` is a cudaStream_t (0 = default stream)
  * on which all later work of this context is enqueued.  Fails with PHYLINO_ERR_CUDA when there is
  * no such device (there is no CPU fallback). */
@@ -162,6 +175,14 @@ PHYLINO_API phylino_status phylino_event_bins(phylino_ctx *ctx, int P, const dou
 PHYLINO_API phylino_status phylino_nll_host(phylino_ctx *ctx, int P, const double *params_host,
                                 const double *data_host, double *nll_host);
 PHYLINO_API phylino_status phylino_spectra_host(phylino_ctx *ctx, int P, const double *params_host, double *hist_host);
+
+/* Correlated prior blocks: phylino_nll / phylino_nll_host add 1/2 (b - b0)^T V^-1 (b - b0) per block and
+ * point (constants dropped, R9), on top of the uncorrelated priors of the model descriptor (a parameter of
+ * a block normally has prior_sigma <= 0 there).  Call after phylino_set_model, which clears the blocks;
+ * n_blocks = 0 clears them too.  Synchronises the stream.  PHYLINO_ERR_STATE before set_model,
+ * PHYLINO_ERR_SHAPE for n or an index out of range, PHYLINO_ERR_ARG for NULL arrays or non-finite
+ * mean / inv_cov entries. */
+PHYLINO_API phylino_status phylino_set_prior_blocks(phylino_ctx *ctx, int n_blocks, const phylino_prior_block *blocks);
 
 /* Sizes the caller needs for its buffers. */
 PHYLINO_API int64_t phylino_total_bins(const phylino_ctx *ctx);     /* sum_d n_bins, 0 before set_model */

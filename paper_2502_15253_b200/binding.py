@@ -21,7 +21,7 @@ abi_symbols = (
     "phylino_spectra_host", "phylino_total_bins", "phylino_total_events",
     "phylino_set_tuning", "phylino_launch_count", "phylino_last_error", "phylino_peak_fp64",
     "phylino_expectation", "phylino_set_timing", "phylino_last_kernel_ms",
-    "phylino_set_caching", "phylino_last_plan",
+    "phylino_set_caching", "phylino_last_plan", "phylino_set_prior_blocks",
 )
 
 _STATUS = {0: "OK", 1: "ERR_ARG", 2: "ERR_SHAPE", 3: "ERR_STATE", 4: "ERR_OOM", 5: "ERR_CUDA"}
@@ -41,6 +41,10 @@ class _Dataset(C.Structure):
     _fields_ = [("n_bins", C.c_int32), ("idx_a", C.c_int32 * 3), ("idx_signorm", C.c_int32),
                 ("norm", C.c_double), ("idx_flux", C.c_void_p), ("n_bkg", C.c_int32),
                 ("bkg", C.POINTER(_Bkg))]
+
+
+class _PriorBlock(C.Structure):
+    _fields_ = [("n", C.c_int32), ("idx", C.c_void_p), ("mean", C.c_void_p), ("inv_cov", C.c_void_p)]
 
 
 class _Model(C.Structure):
@@ -96,6 +100,8 @@ def load_library():
     lib.phylino_total_bins.argtypes = [vp]
     lib.phylino_total_events.restype = i64
     lib.phylino_total_events.argtypes = [vp]
+    lib.phylino_set_prior_blocks.restype = i32
+    lib.phylino_set_prior_blocks.argtypes = [vp, i32, C.POINTER(_PriorBlock)]
     lib.phylino_set_caching.restype = i32
     lib.phylino_set_caching.argtypes = [vp, i32]
     lib.phylino_last_plan.restype = i32
@@ -226,6 +232,9 @@ class Phylino:
     def load_workload(self, wl):
         """set_model + load_events for every dataset of a `workloads.Workload`."""
         self.set_model(wl.model)
+        blocks = list(getattr(wl.model, "prior_blocks", None) or [])
+        if blocks:
+            self.set_prior_blocks(blocks)
         for d, e in enumerate(wl.events):
             self.load_events(d, e.e_nu, e.e_vis, e.w, e.core, e.L_m, e.edges)
 
@@ -278,6 +287,20 @@ class Phylino:
             and out.numel() == p.shape[0] * self.total_bins
         self._check(self._lib.phylino_expectation(self._ctx, int(p.shape[0]), p.data_ptr(), out.data_ptr()))
         return out
+
+    def set_prior_blocks(self, blocks: Sequence = ()):
+        """blocks: objects with .idx [n], .mean [n], .inv_cov [n, n] (workloads.PriorBlock)."""
+        keep = []
+        arr = (_PriorBlock * max(1, len(blocks)))()
+        for k, b in enumerate(blocks):
+            i = np.ascontiguousarray(b.idx, dtype=np.int32)
+            m = np.ascontiguousarray(b.mean, dtype=np.float64)
+            v = np.ascontiguousarray(b.inv_cov, dtype=np.float64)
+            if m.shape != i.shape or v.shape != (i.size, i.size):
+                raise ValueError("prior block: idx [n], mean [n], inv_cov [n, n]")
+            keep += [i, m, v]
+            arr[k].n, arr[k].idx, arr[k].mean, arr[k].inv_cov = int(i.size), i.ctypes.data, m.ctypes.data, v.ctypes.data
+        self._check(self._lib.phylino_set_prior_blocks(self._ctx, len(blocks), arr if blocks else None))
 
     def set_caching(self, on: bool = True):
         self._check(self._lib.phylino_set_caching(self._ctx, int(bool(on))))

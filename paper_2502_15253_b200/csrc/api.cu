@@ -76,6 +76,8 @@ void free_tables(phylino_ctx *c)
     cudaFree((void *)f.norm); cudaFree((void *)f.idx_signorm); cudaFree((void *)f.n_bkg);
     cudaFree((void *)f.idx_rate); cudaFree((void *)f.idx_shape); cudaFree((void *)f.tmpl);
     cudaFree((void *)f.prior_mean); cudaFree((void *)f.prior_sigma);
+    cudaFree((void *)f.blk_off); cudaFree((void *)f.blk_moff); cudaFree((void *)f.blk_idx);
+    cudaFree((void *)f.blk_mean); cudaFree((void *)f.blk_inv);
     f = FinalizeArgs{};
 }
 
@@ -802,6 +804,51 @@ phylino_status phylino_spectra_host(phylino_ctx *ctx, int P, const double *param
     CU(cudaMemcpyAsync(ctx->h_pin + np, ctx->d_stage + np, nh * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
     CU(cudaStreamSynchronize(ctx->stream));
     std::memcpy(hist_host, ctx->h_pin + np, nh * sizeof(double));
+    return PHYLINO_OK;
+}
+
+phylino_status phylino_set_prior_blocks(phylino_ctx *ctx, int n_blocks, const phylino_prior_block *blocks)
+{
+    if (!ctx) return PHYLINO_ERR_ARG;
+    if (!ctx->have_model) return fail(ctx, PHYLINO_ERR_STATE, "phylino_set_model must come before phylino_set_prior_blocks");
+    if (n_blocks < 0 || (n_blocks > 0 && !blocks)) return fail(ctx, PHYLINO_ERR_ARG, "n_blocks = %d with NULL blocks", n_blocks);
+    std::vector<int32_t> off(1, 0), idx;
+    std::vector<int64_t> moff;
+    std::vector<double> mean, inv;
+    for (int k = 0; k < n_blocks; ++k) {
+        const phylino_prior_block &b = blocks[k];
+        if (b.n < 1 || b.n > PHYLINO_MAX_BLOCK) return fail(ctx, PHYLINO_ERR_SHAPE, "block %d: n = %d not in 1..%d", k, b.n, PHYLINO_MAX_BLOCK);
+        if (!b.idx || !b.mean || !b.inv_cov) return fail(ctx, PHYLINO_ERR_ARG, "block %d: NULL array", k);
+        for (int i = 0; i < b.n; ++i) {
+            if (b.idx[i] < 0 || b.idx[i] >= ctx->n_params) return fail(ctx, PHYLINO_ERR_SHAPE, "block %d: idx[%d] = %d out of range", k, i, b.idx[i]);
+            if (!std::isfinite(b.mean[i])) return fail(ctx, PHYLINO_ERR_ARG, "block %d: mean[%d] is not finite", k, i);
+        }
+        for (int64_t i = 0; i < (int64_t)b.n * b.n; ++i)
+            if (!std::isfinite(b.inv_cov[i])) return fail(ctx, PHYLINO_ERR_ARG, "block %d: inv_cov[%lld] is not finite", k, (long long)i);
+        moff.push_back((int64_t)inv.size());
+        idx.insert(idx.end(), b.idx, b.idx + b.n);
+        mean.insert(mean.end(), b.mean, b.mean + b.n);
+        inv.insert(inv.end(), b.inv_cov, b.inv_cov + (size_t)b.n * b.n);
+        off.push_back((int32_t)idx.size());
+    }
+    DeviceGuard g(ctx->device);
+    CU(cudaStreamSynchronize(ctx->stream));
+    FinalizeArgs &f = ctx->fin;
+    cudaFree((void *)f.blk_off); cudaFree((void *)f.blk_moff); cudaFree((void *)f.blk_idx);
+    cudaFree((void *)f.blk_mean); cudaFree((void *)f.blk_inv);
+    f.blk_off = nullptr; f.blk_moff = nullptr; f.blk_idx = nullptr; f.blk_mean = nullptr; f.blk_inv = nullptr;
+    f.n_blocks = 0;
+    if (n_blocks > 0) {
+        cudaStream_t st = ctx->stream;
+        CU(upload((int32_t **)&f.blk_off, off, st));
+        CU(upload((int64_t **)&f.blk_moff, moff, st));
+        CU(upload((int32_t **)&f.blk_idx, idx, st));
+        CU(upload((double **)&f.blk_mean, mean, st));
+        CU(upload((double **)&f.blk_inv, inv, st));
+        CU(cudaStreamSynchronize(st));
+        f.n_blocks = n_blocks;
+    }
+    ctx->err.clear();
     return PHYLINO_OK;
 }
 

@@ -114,6 +114,19 @@ __global__ void __launch_bounds__(FIN_THREADS) finalize_kernel(const __grid_cons
         }
     }
 
+    /* correlated blocks: thread i takes rows i, i + FIN_THREADS, ... of every block */
+    for (int k = 0; k < a.n_blocks; ++k) {
+        const int o = a.blk_off[k], n = a.blk_off[k + 1] - o;
+        const double *M = a.blk_inv + a.blk_moff[k];
+        for (int i = threadIdx.x; i < n; i += FIN_THREADS) {
+            const double di = theta[a.blk_idx[o + i]] - a.blk_mean[o + i];
+            double row = 0.0;
+            for (int j = 0; j < n; ++j)
+                row = fma(M[(size_t)i * n + j], theta[a.blk_idx[o + j]] - a.blk_mean[o + j], row);
+            part += 0.5 * di * row;
+        }
+    }
+
     __shared__ double wsum[FIN_THREADS / 32];
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) part += __shfl_xor_sync(0xffffffffu, part, o);

@@ -115,6 +115,13 @@ struct FinalizeArgs {
     const double  *tmpl;          /* [max_bkg x total_bins] */
     const double  *prior_mean;    /* [n_params] or NULL */
     const double  *prior_sigma;   /* [n_params] or NULL */
+    /* correlated prior blocks (phylino_set_prior_blocks), flattened */
+    int32_t        n_blocks;
+    const int32_t *blk_off;       /* [n_blocks + 1] offsets into blk_idx / blk_mean */
+    const int64_t *blk_moff;      /* [n_blocks] offsets into blk_inv */
+    const int32_t *blk_idx;
+    const double  *blk_mean;
+    const double  *blk_inv;
     const double  *data;          /* [total_bins] (NLL mode) */
     double        *hist;          /* [P x total_bins] (spectra / expectation mode) */
     double        *nll;           /* [P] (NLL mode) */

@@ -348,3 +348,69 @@ def test_peak_fp64_microbenchmark_runs(gpu):
     with gpu.Phylino() as ph:
         r = ph.peak_fp64(2048)
     assert 1e12 < r < 1e14
+
+
+def test_correlated_prior_blocks(gpu, oracle_mod):
+    """PAPER.md:121-123 (Eq. 9, third factor): blocks of 3 and 41 parameters (the size of the paper's flux
+    covariance) on config 3's 301-parameter model, dense and cached entry points, against the oracle."""
+    wl = workloads.make_config(3, scale=0.003, n_points=75)
+    rng = np.random.default_rng(77)
+    A3, A41 = rng.normal(size=(3, 3)), rng.normal(size=(41, 41))
+    V3 = (A3 @ A3.T + 0.5 * np.eye(3)) * 1e-4
+    V41 = (A41 @ A41.T / 41 + 0.2 * np.eye(41)) * 4e-4
+    i3 = np.array([4, 7, 10], np.int32)                    # energy-scale a0 of the three datasets
+    i41 = np.arange(13, 54, dtype=np.int32)                # 41 flux parameters
+    wl.model.prior_sigma = wl.model.prior_sigma.copy()
+    wl.model.prior_sigma[i3] = 0.0
+    wl.model.prior_sigma[i41] = 0.0
+    wl.model.prior_blocks = [workloads.PriorBlock(i3, wl.theta0[i3], np.linalg.inv(V3)),
+                             workloads.PriorBlock(i41, wl.theta0[i41], np.linalg.inv(V41))]
+    params = wl.params.copy()
+    params[:, i41] += rng.normal(0, 0.02, (params.shape[0], 41))
+    params[:, i3] += rng.normal(0, 0.01, (params.shape[0], 3))
+    orc = oracle_mod.Oracle(wl.model, wl.events)
+    data = _data_for(orc, wl, oracle_mod)
+    nll_o = orc.nll(params, data)
+    with gpu.Phylino() as ph:
+        ph.load_workload(wl)
+        nll = ph.nll(_dev(params), _dev(data)).cpu().numpy()
+        nll_h = ph.nll_host(params, data)
+        ph.set_caching(True)
+        nll_c = ph.nll_host(params, data)
+        ph.set_prior_blocks([])                            # cleared: back to the plain model
+        nll_plain = ph.nll(_dev(params), _dev(data)).cpu().numpy()
+    assert np.abs(nll - nll_o).max() <= ABS_NLL
+    assert np.array_equal(nll, nll_h)
+    assert np.abs(nll_c - nll_o).max() <= ABS_NLL
+    wl.model.prior_blocks = []
+    assert np.abs(nll_plain - oracle_mod.Oracle(wl.model, wl.events).nll(params, data)).max() <= ABS_NLL
+    assert np.abs(nll_plain - nll).max() > 1.0             # the blocks did contribute
+
+
+def test_reactor_off_rate_only_dataset(gpu, oracle_mod):
+    """PAPER.md:109, :121 (Eq. 9, second factor P(n_off, mu_off)): the reactor-off period is a dataset of ONE
+    bin with no MC signal events and background templates only; mu_off = sum_k r_k T_k."""
+    from workloads.spec import BkgSpec, DatasetSpec, ModelSpec, Workload
+    edges = 1.0 + 0.5 * np.arange(9)
+    rng = np.random.default_rng(8)
+    on = _events(rng.uniform(2.0, 7.0, 500), rng.uniform(0.5, 6.0, 500), np.ones(500), edges)
+    off = _events([], [], [], np.array([1.0, 20.0]))
+    # theta = (s13, mee, s12, m21, r_li, r_acc)
+    ds_on = DatasetSpec(n_bins=8, norm=0.3, bkg=[BkgSpec(tmpl=np.full(8, 2.0), idx_rate=4)])
+    ds_off = DatasetSpec(n_bins=1, norm=1.0, bkg=[BkgSpec(tmpl=np.array([6.5]), idx_rate=4),
+                                                  BkgSpec(tmpl=np.array([1.25]), idx_rate=5)])
+    model = ModelSpec(osc_model=OSC_EQ1, n_params=6, idx_osc=(0, 1, 2, 3, -1, -1), fixed_osc=(0,) * 6,
+                      datasets=[ds_on, ds_off], prior_mean=np.array([0, 0, 0, 0, 1.0, 1.0]),
+                      prior_sigma=np.array([0, 0, 0, 0, 0.0, 0.3]))
+    params = np.array([[0.1, 2.5e-3, 0.85, 7.5e-5, r1, r2] for r1, r2 in ((1.0, 1.0), (0.7, 1.4), (1.3, 0.2))])
+    wl = Workload(name="off", model=model, events=[on, off], params=params, theta0=params[0], seed=1)
+    orc = oracle_mod.Oracle(model, wl.events)
+    data = np.concatenate([np.round(orc.expectation(params[:1], orc.spectra(params[:1]))[0][:8]), [7.0]])
+    with gpu.Phylino() as ph:
+        ph.load_workload(wl)
+        mu = ph.expectation(_dev(params)).cpu().numpy()
+        nll = ph.nll(_dev(params), _dev(data)).cpu().numpy()
+    assert np.allclose(mu[:, 8], 6.5 * params[:, 4] + 1.25 * params[:, 5], rtol=1e-15)
+    assert np.abs(nll - orc.nll(params, data)).max() <= ABS_NLL
+    # the off term alone: dev(7, mu_off) is what distinguishes the points beyond the on-data and the prior
+    assert np.isfinite(nll).all()
