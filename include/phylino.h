@@ -176,6 +176,14 @@ PHYLINO_API phylino_status phylino_nll_host(phylino_ctx *ctx, int P, const doubl
                                 const double *data_host, double *nll_host);
 PHYLINO_API phylino_status phylino_spectra_host(phylino_ctx *ctx, int P, const double *params_host, double *hist_host);
 
+/* Pseudo-experiment ensembles ("test statistics derived from large ensembles of
+ * pseudo-experiments"): nll[p * E + e] = the NLL of phylino_nll at point p against the observed counts
+ * data[e * total_bins ...], for all P points and E experiments.  The spectra and expectations are computed once
+ * per point; only the deviance sums are per experiment.  params DEVICE [P x n_params], data DEVICE
+ * [E x total_bins], nll DEVICE [P x E] row-major.  Asynchronous on the context's stream like phylino_nll. */
+PHYLINO_API phylino_status phylino_nll_ensemble(phylino_ctx *ctx, int P, const double *params, int E,
+                                                const double *data, double *nll);
+
 /* Correlated prior blocks: phylino_nll / phylino_nll_host add 1/2 (b - b0)^T V^-1 (b - b0) per block and
  * point (constants dropped, R9), on top of the uncorrelated priors of the model descriptor (a parameter of
  * a block normally has prior_sigma <= 0 there).  Call after phylino_set_model, which clears the blocks;

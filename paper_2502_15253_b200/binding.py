@@ -22,6 +22,7 @@ abi_symbols = (
     "phylino_set_tuning", "phylino_launch_count", "phylino_last_error", "phylino_peak_fp64",
     "phylino_expectation", "phylino_set_timing", "phylino_last_kernel_ms",
     "phylino_set_caching", "phylino_last_plan", "phylino_set_prior_blocks",
+    "phylino_nll_ensemble",
 )
 
 _STATUS = {0: "OK", 1: "ERR_ARG", 2: "ERR_SHAPE", 3: "ERR_STATE", 4: "ERR_OOM", 5: "ERR_CUDA"}
@@ -100,6 +101,8 @@ def load_library():
     lib.phylino_total_bins.argtypes = [vp]
     lib.phylino_total_events.restype = i64
     lib.phylino_total_events.argtypes = [vp]
+    lib.phylino_nll_ensemble.restype = i32
+    lib.phylino_nll_ensemble.argtypes = [vp, i32, vp, i32, vp, vp]
     lib.phylino_set_prior_blocks.restype = i32
     lib.phylino_set_prior_blocks.argtypes = [vp, i32, C.POINTER(_PriorBlock)]
     lib.phylino_set_caching.restype = i32
@@ -276,6 +279,21 @@ class Phylino:
         assert out.is_cuda and out.dtype == t.float64 and out.is_contiguous() and out.numel() == p.shape[0]
         self._check(self._lib.phylino_nll(self._ctx, int(p.shape[0]), p.data_ptr(), data.data_ptr(),
                                           out.data_ptr()))
+        return out
+
+    def nll_ensemble(self, params, data, out=None):
+        """data: float64 CUDA tensor [E, total_bins] -> nll [P, E]."""
+        t = self._torch
+        p = self._dev_params(params)
+        if not (isinstance(data, t.Tensor) and data.is_cuda and data.dtype == t.float64 and data.is_contiguous()
+                and data.dim() == 2 and data.shape[1] == self.total_bins):
+            raise TypeError(f"data must be a contiguous float64 CUDA tensor [E, {self.total_bins}]")
+        E = int(data.shape[0])
+        if out is None:
+            out = t.empty((p.shape[0], E), dtype=t.float64, device=p.device)
+        assert out.is_cuda and out.dtype == t.float64 and out.is_contiguous() and out.numel() == p.shape[0] * E
+        self._check(self._lib.phylino_nll_ensemble(self._ctx, int(p.shape[0]), p.data_ptr(), E, data.data_ptr(),
+                                                   out.data_ptr()))
         return out
 
     def expectation(self, params, out=None):

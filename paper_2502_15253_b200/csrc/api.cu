@@ -91,6 +91,7 @@ void free_all(phylino_ctx *c)
     cudaFree(c->d_rec); cudaFree(c->d_thr); cudaFree(c->d_safe); cudaFree(c->d_counter);
     c->d_rec = nullptr; c->d_thr = nullptr; c->d_safe = nullptr; c->d_counter = nullptr; c->point_capacity = 0;
     cudaFree(c->d_plan); c->d_plan = nullptr; c->plan_capacity = 0;
+    cudaFree(c->d_mu); c->d_mu = nullptr; c->mu_capacity = 0;
     cudaFree(c->d_stage); c->d_stage = nullptr;
     if (c->h_pin) cudaFreeHost(c->h_pin);
     c->h_pin = nullptr; c->stage_capacity = 0;
@@ -719,6 +720,32 @@ phylino_status phylino_nll(phylino_ctx *ctx, int P, const double *params, const 
     if ((s = ensure_acc(ctx, P)) != PHYLINO_OK) return s;
     if ((s = enqueue_spectra(ctx, P, params)) != PHYLINO_OK) return s;
     return enqueue_finalize(ctx, P, params, data, nullptr, nll);
+}
+
+phylino_status phylino_nll_ensemble(phylino_ctx *ctx, int P, const double *params, int E, const double *data,
+                                    double *nll)
+{
+    phylino_status s = check_ready(ctx, P, params, nll);
+    if (s != PHYLINO_OK) return s;
+    if (E < 0) return fail(ctx, PHYLINO_ERR_SHAPE, "E = %d is negative", E);
+    if (P == 0 || E == 0) return PHYLINO_OK;
+    if (!data) return fail(ctx, PHYLINO_ERR_ARG, "NULL data pointer");
+    DeviceGuard g(ctx->device);
+    if ((s = ensure_acc(ctx, P)) != PHYLINO_OK) return s;
+    const int64_t need = (int64_t)P * ctx->total_bins;
+    if (need > ctx->mu_capacity) {
+        CU(cudaStreamSynchronize(ctx->stream));
+        cudaFree(ctx->d_mu); ctx->d_mu = nullptr; ctx->mu_capacity = 0;
+        CU(cudaMalloc((void **)&ctx->d_mu, need * sizeof(double)));
+        ctx->mu_capacity = need;
+    }
+    if ((s = enqueue_spectra(ctx, P, params)) != PHYLINO_OK) return s;
+    if ((s = enqueue_finalize(ctx, P, params, nullptr, ctx->d_mu, nullptr, 1)) != PHYLINO_OK) return s;
+    FinalizeArgs f = ctx->fin;
+    f.P = P; f.params = params; f.data = data; f.hist = ctx->d_mu; f.nll = nll;
+    CU(launch_ensemble(f, E, ctx->stream));
+    ctx->launches += 1;
+    return PHYLINO_OK;
 }
 
 phylino_status phylino_expectation(phylino_ctx *ctx, int P, const double *params, double *mu)

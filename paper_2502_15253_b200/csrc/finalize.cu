@@ -17,6 +17,8 @@
  * (Eq. 1; the paper's own "caching").  Cells are shared between points, so
  * the caller clears them after this kernel.
  */
+#include <algorithm>
+
 #include "devmath.cuh"
 
 namespace phylino {
@@ -35,6 +37,37 @@ __device__ __forceinline__ double half_deviance(double n, double mu)
     }
     if (n == 0.0) return mu;
     return __longlong_as_double(0x7ff8000000000000ll);     /* negative counts are not data */
+}
+
+/* this thread's share of the prior terms of one point: a fixed strided subset of the parameters and
+ * of the rows of every correlated block */
+__device__ __forceinline__ double prior_part(const FinalizeArgs &a, const double *theta)
+{
+    double part = 0.0;
+    if (a.prior_mean && a.prior_sigma) {
+        /* uncorrelated Gaussian priors (PAPER.md:80-83 Eq. 6), constants dropped (R9) */
+        for (int j = threadIdx.x; j < a.n_params; j += FIN_THREADS) {
+            double sg = a.prior_sigma[j];
+            if (!(sg > 0.0) || sg > 1.79769313486231570e308) continue;
+            double z = (theta[j] - a.prior_mean[j]) / sg;
+            part += 0.5 * z * z;
+        }
+    }
+
+    /* correlated blocks (PAPER.md:121-123): thread i takes rows i, i + FIN_THREADS, ... of every block */
+    for (int k = 0; k < a.n_blocks; ++k) {
+        const int o = a.blk_off[k], n = a.blk_off[k + 1] - o;
+        const double *M = a.blk_inv + a.blk_moff[k];
+        for (int i = threadIdx.x; i < n; i += FIN_THREADS) {
+            const double di = theta[a.blk_idx[o + i]] - a.blk_mean[o + i];
+            double row = 0.0;
+            for (int j = 0; j < n; ++j)
+                row = fma(M[(size_t)i * n + j], theta[a.blk_idx[o + j]] - a.blk_mean[o + j], row);
+            part += 0.5 * di * row;
+        }
+    }
+
+    return part;
 }
 
 template <int MODE>   /* 0 = spectra H, 1 = expectation mu, 2 = NLL */
@@ -104,28 +137,7 @@ __global__ void __launch_bounds__(FIN_THREADS) finalize_kernel(const __grid_cons
     }
     if (MODE != 2) return;
 
-    if (a.prior_mean && a.prior_sigma) {
-        /* uncorrelated Gaussian priors (PAPER.md:80-83 Eq. 6), constants dropped (R9) */
-        for (int j = threadIdx.x; j < a.n_params; j += FIN_THREADS) {
-            double sg = a.prior_sigma[j];
-            if (!(sg > 0.0) || sg > 1.79769313486231570e308) continue;
-            double z = (theta[j] - a.prior_mean[j]) / sg;
-            part += 0.5 * z * z;
-        }
-    }
-
-    /* correlated blocks (PAPER.md:121-123): thread i takes rows i, i + FIN_THREADS, ... of every block */
-    for (int k = 0; k < a.n_blocks; ++k) {
-        const int o = a.blk_off[k], n = a.blk_off[k + 1] - o;
-        const double *M = a.blk_inv + a.blk_moff[k];
-        for (int i = threadIdx.x; i < n; i += FIN_THREADS) {
-            const double di = theta[a.blk_idx[o + i]] - a.blk_mean[o + i];
-            double row = 0.0;
-            for (int j = 0; j < n; ++j)
-                row = fma(M[(size_t)i * n + j], theta[a.blk_idx[o + j]] - a.blk_mean[o + j], row);
-            part += 0.5 * di * row;
-        }
-    }
+    part += prior_part(a, theta);
 
     __shared__ double wsum[FIN_THREADS / 32];
 #pragma unroll
@@ -140,7 +152,50 @@ __global__ void __launch_bounds__(FIN_THREADS) finalize_kernel(const __grid_cons
     }
 }
 
+/* Pseudo-experiment ensembles: nll[p, e] for E observed-count vectors
+ * against the SAME expectations mu[p, .] (written by finalize_kernel<1>).  One CTA per (point, slice of
+ * experiments): the CTA forms the point's prior term once, then every warp takes experiments
+ * e = slice start + warp, + ENS_WARPS, ...; lanes stride the bins, fixed shuffle tree => reproducible. */
+constexpr int ENS_WARPS = FIN_THREADS / 32;
+
+__global__ void __launch_bounds__(FIN_THREADS) ensemble_kernel(const __grid_constant__ FinalizeArgs a, int E,
+                                                               int e_per_cta)
+{
+    const int p = blockIdx.x, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const double *theta = a.params + (size_t)p * a.n_params;
+    const double *mu = a.hist + (size_t)p * a.total_bins;
+    __shared__ double wsum[ENS_WARPS];
+    double part = prior_part(a, theta);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) part += __shfl_xor_sync(0xffffffffu, part, o);
+    if (lane == 0) wsum[warp] = part;
+    __syncthreads();
+    double prior = 0.0;
+#pragma unroll
+    for (int i = 0; i < ENS_WARPS; ++i) prior += wsum[i];
+    const int e0 = blockIdx.y * e_per_cta, e1 = min(E, e0 + e_per_cta);
+    for (int e = e0 + warp; e < e1; e += ENS_WARPS) {
+        const double *n = a.data + (size_t)e * a.total_bins;
+        double dev = 0.0;
+        for (int g = lane; g < a.total_bins; g += 32) dev += half_deviance(n[g], mu[g]);
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) dev += __shfl_xor_sync(0xffffffffu, dev, o);
+        if (lane == 0) a.nll[(size_t)p * E + e] = dev + prior;
+    }
+}
+
 } // namespace
+
+cudaError_t launch_ensemble(const FinalizeArgs &a, int E, cudaStream_t st)
+{
+    if (a.P <= 0 || E <= 0) return cudaSuccess;
+    /* enough CTAs to fill the chip a few times over, at least 4 experiments per warp */
+    int slices = (int)std::min<long long>((E + 4 * ENS_WARPS - 1) / (4 * ENS_WARPS), std::max(1, 4 * 148 * 8 / a.P));
+    slices = std::max(1, std::min(slices, 65535));
+    const int e_per_cta = (E + slices - 1) / slices;
+    ensemble_kernel<<<dim3(a.P, (E + e_per_cta - 1) / e_per_cta), FIN_THREADS, 0, st>>>(a, E, e_per_cta);
+    return cudaGetLastError();
+}
 
 cudaError_t launch_finalize(const FinalizeArgs &a, int mode, cudaStream_t st, bool pdl)
 {

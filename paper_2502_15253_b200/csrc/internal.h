@@ -136,6 +136,7 @@ cudaError_t launch_setup(const SpectraArgs &a, int S, cudaStream_t st);
 cudaError_t spectra_max_warps(int S, int sm_count, int *warps);
 cudaError_t launch_spectra(const SpectraArgs &a, int S, cudaStream_t st, bool pdl);
 cudaError_t launch_finalize(const FinalizeArgs &a, int mode /*0 H, 1 mu, 2 nll*/, cudaStream_t st, bool pdl);
+cudaError_t launch_ensemble(const FinalizeArgs &a, int E, cudaStream_t st);
 cudaError_t launch_event_bins(const SpectraArgs &a, int d, const int32_t *perm, long long n, long long ev_off,
                               long long total_events, int32_t *bins, cudaStream_t st);
 cudaError_t run_peak_fp64(int iters, cudaStream_t st, double *dfma_per_s);
@@ -192,6 +193,8 @@ struct phylino_ctx {
     int32_t *d_plan = nullptr;                     /* vp_class | vp_src | class_rep | pt_comp */
     int64_t plan_capacity = 0;                     /* int32 entries */
     int64_t last_virtual_points = 0, last_classes = 0;
+    double *d_mu = nullptr;                        /* [mu_capacity] expectations of an ensemble call */
+    int64_t mu_capacity = 0;
     /* host-buffer entry points: pinned + device staging */
     double *h_pin = nullptr, *d_stage = nullptr;
     int64_t stage_capacity = 0;                    /* doubles */

@@ -414,3 +414,39 @@ def test_reactor_off_rate_only_dataset(gpu, oracle_mod):
     assert np.abs(nll - orc.nll(params, data)).max() <= ABS_NLL
     # the off term alone: dev(7, mu_off) is what distinguishes the points beyond the on-data and the prior
     assert np.isfinite(nll).all()
+
+
+def test_pseudo_experiment_ensemble(gpu, oracle_mod):
+    """nll[p, e] for E pseudo-experiments against one batch of expectations == the plain NLL
+    call per experiment (oracle), including priors, an E that is not a multiple of anything, and E = 1."""
+    import torch
+    wl = workloads.make_config(5, scale=0.004, n_points=45)
+    orc = oracle_mod.Oracle(wl.model, wl.events)
+    mu0 = orc.expectation(wl.theta0[None, :], orc.spectra(wl.theta0[None, :]))[0]
+    E = 131
+    data = np.stack([workloads.poisson_counts(mu0, 500 + e) for e in range(E)])
+    want = np.stack([orc.nll(wl.params, data[e]) for e in range(E)], axis=1)            # [P, E]
+    with gpu.Phylino() as ph:
+        ph.load_workload(wl)
+        got = ph.nll_ensemble(_dev(wl.params), _dev(data)).cpu().numpy()
+        one = ph.nll_ensemble(_dev(wl.params), _dev(data[:1])).cpu().numpy()
+        again = ph.nll_ensemble(_dev(wl.params), _dev(data)).cpu().numpy()
+        plain = ph.nll(_dev(wl.params), _dev(data[7])).cpu().numpy()
+        torch.cuda.synchronize()
+    assert got.shape == (45, E)
+    assert np.abs(got - want).max() <= ABS_NLL
+    assert np.array_equal(got, again)                      # reproducible
+    assert np.abs(one[:, 0] - want[:, 0]).max() <= ABS_NLL
+    assert np.abs(plain - got[:, 7]).max() <= 1e-9         # same expectations, another summation tree
+
+
+def test_ensemble_with_priors_config3(gpu, oracle_mod):
+    wl = workloads.make_config(3, scale=0.002, n_points=9)
+    orc = oracle_mod.Oracle(wl.model, wl.events)
+    mu0 = orc.expectation(wl.theta0[None, :], orc.spectra(wl.theta0[None, :]))[0]
+    data = np.stack([workloads.poisson_counts(mu0, 900 + e) for e in range(5)])
+    want = np.stack([orc.nll(wl.params, data[e]) for e in range(5)], axis=1)
+    with gpu.Phylino() as ph:
+        ph.load_workload(wl)
+        got = ph.nll_ensemble(_dev(wl.params), _dev(data)).cpu().numpy()
+    assert np.abs(got - want).max() <= ABS_NLL
