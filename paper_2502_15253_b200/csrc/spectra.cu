@@ -326,13 +326,13 @@ __device__ __forceinline__ void walk_batch(const SpectraArgs &a, const DatasetDe
     }
 }
 
-/* Two consecutive batches known to lie inside the lane's open run (the store is sorted: the last
- * event of the second batch is below r.hi): rows a2 + a4 only, straight-line. */
-template <int S, bool UW>
-__device__ __forceinline__ void walk_pair_inside(const EventBatch *bp, const double (&h)[S], Run<S> &r)
+/* K consecutive batches known to lie inside the lane's open run (the store is sorted: the last
+ * event of the last batch is below r.hi): rows a2 + a4 only, straight-line. */
+template <int S, bool UW, int K>
+__device__ __forceinline__ void walk_inside(const EventBatch *bp, const double (&h)[S], Run<S> &r)
 {
 #pragma unroll
-    for (int u = 0; u < 2; ++u) {
+    for (int u = 0; u < K; ++u) {
         const double2 *q = reinterpret_cast<const double2 *>(bp + u);
 #pragma unroll
         for (int j = 0; j < EB / 2; ++j) {
@@ -415,8 +415,12 @@ __device__ __forceinline__ void walk_unit(const SpectraArgs &a, const DatasetDev
         int i = 0;
 #pragma unroll 1
         while (i < nb) {
-            if (i + 2 <= nb && bp[1].v[EB - 1] < r.hi) {
-                walk_pair_inside<S, UW>(bp, h, r);
+            if (i + 4 <= nb && bp[3].v[EB - 1] < r.hi) {
+                walk_inside<S, UW, 4>(bp, h, r);
+                i += 4;
+                bp += 4;
+            } else if (i + 2 <= nb && bp[1].v[EB - 1] < r.hi) {
+                walk_inside<S, UW, 2>(bp, h, r);
                 i += 2;
                 bp += 2;
             } else {
