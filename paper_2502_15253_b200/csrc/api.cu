@@ -206,17 +206,34 @@ void fill_batch(const phylino_ctx *ctx, SpectraArgs &a, int P, const double *par
     U = std::min<int64_t>(U, MAX_UNIT_BATCHES);         /* a unit must fit the warp's staging buffer */
     int64_t G = std::max<int64_t>(1, std::min<int64_t>(std::min<int64_t>(work, 512) / U, n_groups));
     if (ctx->chunk_groups > 0) G = std::min<int64_t>(ctx->chunk_groups, n_groups);
-    int64_t units, chunks;
+    int64_t units, chunks, tail_unit, tail_b0, Us;
+    const int last = ctx->n_datasets - 1;
     for (;;) {
+        chunks = (n_groups + G - 1) / G;
+        /* fine tail: about the last 1.5 items of every warp's share, at most a quarter of the work and
+         * never more than the last dataset, in units of U/4 */
+        const int64_t per_warp = std::max<int64_t>(1, (batches + U - 1) / U * chunks / cap);
+        const int64_t nb_last = ctx->ds[last].n_pad / EB;
+        int64_t fine = std::min<int64_t>(batches / 4, batches * 3 / (2 * per_warp));
+        fine = std::min(fine, nb_last);
+        Us = std::max<int64_t>(std::max<int64_t>(4, streams), U / 4);
+        if (ctx->unit_events > 0 || Us >= U || fine < 2 * U) fine = 0;     /* explicit tuning: uniform units */
+        tail_b0 = (nb_last - fine) / U * U;
+        if (fine == 0) tail_b0 = nb_last;
         units = 0;
         for (int d = 0; d < ctx->n_datasets; ++d) {
             a.ds[d].unit_begin = (int32_t)units;
-            units += (ctx->ds[d].n_pad / EB + U - 1) / U;
+            const int64_t nb = d == last ? tail_b0 : ctx->ds[d].n_pad / EB;
+            units += (nb + U - 1) / U;
         }
-        chunks = (n_groups + G - 1) / G;
+        tail_unit = units;
+        units += (nb_last - tail_b0 + Us - 1) / Us;
         if (units * chunks < (1ll << 31) - 2ll * cap) break;
         if (G < n_groups) G *= 2; else U *= 2;          /* keep items and tickets inside 32 bits */
     }
+    a.tail_unit = (int32_t)tail_unit;
+    a.tail_b0 = (int32_t)tail_b0;
+    a.tail_batches = (int32_t)Us;
     a.unit_batches = (int32_t)U;
     a.chunk_groups = (int32_t)G;
     a.n_units = (int32_t)units;

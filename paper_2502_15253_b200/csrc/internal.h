@@ -77,6 +77,11 @@ struct SpectraArgs {
     int32_t chunk_groups;   /* G: point groups per work item */
     int32_t n_chunks;       /* ceil(n_groups / G) */
     int32_t n_items;        /* n_units x n_chunks; item = unit * n_chunks + chunk */
+    /* fine tail: the last stretch of the last dataset is cut into shorter units, so that the warps of
+     * the persistent grid run out of work within a fraction of a full item of each other */
+    int32_t tail_unit;      /* first global unit of the fine tail (= n_units if there is none) */
+    int32_t tail_b0;        /* its first batch inside the last dataset */
+    int32_t tail_batches;   /* batches per unit of the fine tail */
     int32_t n_warps;        /* warps of the persistent grid (a multiple of WARPS) */
     unsigned *counter;      /* DEVICE work counter; the setup kernel sets it to 2 n_warps */
     int32_t thr_stride;     /* floats per threshold row: total_bins + n_datasets */

@@ -455,6 +455,12 @@ __device__ __forceinline__ void decode_item(const SpectraArgs &a, unsigned item,
 {
     const int unit = (int)(item / (unsigned)a.n_chunks);
     chunk = (int)(item - (unsigned)unit * (unsigned)a.n_chunks);
+    if (unit >= a.tail_unit) {
+        d = a.n_datasets - 1;
+        b0 = a.tail_b0 + (unit - a.tail_unit) * a.tail_batches;
+        b1 = min(b0 + a.tail_batches, a.ds[d].n_batches);
+        return;
+    }
     d = 0;
     for (int i = 1; i < a.n_datasets; ++i)
         if (unit >= a.ds[i].unit_begin) d = i;
