@@ -357,15 +357,18 @@ __device__ __forceinline__ void walk_inside(const EventBatch *bp, const double (
 }
 
 /* One warp, the nb batches of one unit of dataset ds staged at `unit` (SHARED memory), point group g
- * (points 32 g ... 32 g + 31).  FULL: the group has 32 points, every lane walks all batches. */
+ * (points 32 g ... 32 g + 31).  FULL: the group has more than 16 points, every lane walks all batches. */
 template <int S, bool FULL, bool UW>
 __device__ __forceinline__ void walk_unit(const SpectraArgs &a, const DatasetDev &ds, int d, const EventBatch *unit,
                                           int nb, int g, int lane)
 {
     /* lane -> (point, sub-stream): a group of np < 32 points uses PL = 2^ceil(log2 np) point lanes
      * and splits the batches into NS = 32 / PL contiguous sub-streams */
-    int my0 = 0, mine = nb, iters = nb, p = 32 * g + lane;
-    bool active = true;
+    /* FULL: more than 16 points, so every lane walks all batches; lanes past the last point shadow point
+     * 32 g and never flush */
+    int my0 = 0, mine = nb, iters = nb;
+    bool active = 32 * g + lane < a.P;
+    int p = 32 * g + (active ? lane : 0);
     if (!FULL) {
         const int np = min(32, a.P - 32 * g);
         int PL = 1;
@@ -519,7 +522,7 @@ __global__ void __launch_bounds__(WARPS * 32, 4) spectra_kernel(const __grid_con
 #pragma unroll 1
         for (int g = chunk * a.chunk_groups; g < g1; ++g) {
             const EventBatch *unit = buf0 + b * a.unit_batches;
-            if (32 * g + 32 > a.P) walk_unit<S, false, false>(a, ds, d, unit, b1 - b0, g, lane);
+            if (32 * g + 16 >= a.P) walk_unit<S, false, false>(a, ds, d, unit, b1 - b0, g, lane);
             else if (ds.unit_w)    walk_unit<S, true, true>(a, ds, d, unit, b1 - b0, g, lane);
             else                   walk_unit<S, true, false>(a, ds, d, unit, b1 - b0, g, lane);
         }
