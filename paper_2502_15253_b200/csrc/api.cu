@@ -184,7 +184,7 @@ void fill_datasets(const phylino_ctx *ctx, SpectraArgs &a)
 }
 
 /* Cut of the batch into work items (spectra.cu): U batches per unit, G point groups per item.
- * Aim: about 12 items per resident warp (dynamic balance, short tail) of at least 16 batch-groups
+ * Aim: at least 12 items per resident warp (dynamic balance, short tail) of at least 16 batch-groups
  * each (the per-item cost -- first bin search, one flush per point -- stays a few percent). */
 void fill_batch(const phylino_ctx *ctx, SpectraArgs &a, int P, const double *params)
 {
@@ -204,7 +204,10 @@ void fill_batch(const phylino_ctx *ctx, SpectraArgs &a, int P, const double *par
     U = std::max<int64_t>(U, 4 * streams);
     if (ctx->unit_events > 0) U = std::max(1, ctx->unit_events / EB);
     U = std::min<int64_t>(U, MAX_UNIT_BATCHES);         /* a unit must fit the warp's staging buffer */
-    int64_t G = std::max<int64_t>(1, std::min<int64_t>(std::min<int64_t>(work, 512) / U, n_groups));
+    /* two point groups per item measured best for units of 64 batches (short items balance better and the
+     * unit is re-read from L2, not DRAM); chunks of equal size */
+    int64_t G = std::max<int64_t>(1, std::min<int64_t>(std::min<int64_t>(work, 128) / U, n_groups));
+    G = (n_groups + (n_groups + G - 1) / G - 1) / ((n_groups + G - 1) / G);
     if (ctx->chunk_groups > 0) G = std::min<int64_t>(ctx->chunk_groups, n_groups);
     int64_t units, chunks, tail_unit, tail_b0, Us;
     const int last = ctx->n_datasets - 1;
@@ -217,7 +220,7 @@ void fill_batch(const phylino_ctx *ctx, SpectraArgs &a, int P, const double *par
         int64_t fine = std::min<int64_t>(batches / 4, batches * 3 / (2 * per_warp));
         fine = std::min(fine, nb_last);
         Us = std::max<int64_t>(std::max<int64_t>(4, streams), U / 4);
-        if (ctx->unit_events > 0 || Us >= U || fine < 2 * U) fine = 0;     /* explicit tuning: uniform units */
+        if (Us >= U || fine < 2 * U) fine = 0;
         tail_b0 = (nb_last - fine) / U * U;
         if (fine == 0) tail_b0 = nb_last;
         units = 0;
