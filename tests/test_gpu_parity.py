@@ -450,3 +450,19 @@ def test_ensemble_with_priors_config3(gpu, oracle_mod):
         ph.load_workload(wl)
         got = ph.nll_ensemble(_dev(wl.params), _dev(data)).cpu().numpy()
     assert np.abs(got - want).max() <= ABS_NLL
+
+
+def test_infinite_reconstructed_energies(gpu, oracle_mod):
+    """E_vis = +-inf (and NaN) land in no bin on both sides, with a fixed and with a per-point energy scale,
+    at the start, in the middle and at the end of the sorted store."""
+    edges = np.array([1.0, 1.5, 2.25, 3.0, 3.5, 4.75, 6.0, 9.0])
+    rng = np.random.default_rng(4)
+    e_vis = np.concatenate([rng.uniform(0.5, 10.0, 300), [np.inf, -np.inf, np.nan, np.inf, -np.inf]]).astype(np.float32)
+    rng.shuffle(e_vis)
+    n = len(e_vis)
+    evs = [_events(rng.uniform(2.0, 8.0, n), e_vis, rng.uniform(0.5, 1.5, n), edges)]
+    h, h_o = _both(gpu, oracle_mod, _one_dataset_model(7), evs, THETA)
+    _check_hist(h, h_o)
+    params = np.array([[0.1, 2.5e-3, 0.85, 7.5e-5, 0.02, 1.01, -0.001], [0.1, 2.5e-3, 0.85, 7.5e-5, -0.03, 0.98, 0.002]])
+    h, h_o = _both(gpu, oracle_mod, _one_dataset_model(7, idx_a=(4, 5, 6), n_params=7), evs, params)
+    _check_hist(h, h_o)
