@@ -50,6 +50,11 @@ class _PriorBlock(C.Structure):
     _fields_ = [("n", C.c_int32), ("idx", C.c_void_p), ("mean", C.c_void_p), ("inv_cov", C.c_void_p)]
 
 
+class _TransformBlock(C.Structure):
+    _fields_ = [("n_out", C.c_int32), ("n_in", C.c_int32), ("idx_out", C.c_void_p), ("idx_in", C.c_void_p),
+                ("offset", C.c_void_p), ("centre", C.c_void_p), ("matrix", C.c_void_p)]
+
+
 class _Model(C.Structure):
     _fields_ = [("osc_model", C.c_int32), ("ordering", C.c_int32), ("n_params", C.c_int32),
                 ("n_datasets", C.c_int32), ("idx_osc", C.c_int32 * 6), ("fixed_osc", C.c_double * 6),
@@ -86,6 +91,9 @@ def _load():
         lib.orc_nll_from_mu.argtypes = [C.POINTER(_Model), C.c_int32, dp, dp, dp, dp]
         lib.orc_nll.restype = C.c_int
         lib.orc_nll.argtypes = [C.POINTER(_Model), C.POINTER(_Events), C.c_int32, dp, dp, dp, C.c_int]
+        lib.orc_transform.restype = C.c_int
+        lib.orc_transform.argtypes = [C.c_int32, C.c_int32, C.c_void_p, C.c_void_p, C.c_int32,
+                                      C.POINTER(_TransformBlock), C.c_int32, dp, dp]
         lib.orc_max_threads.restype = C.c_int
         _lib = lib
     return _lib
@@ -251,6 +259,37 @@ def bin_index(edges, e: float) -> int:
 
 def dev(n: float, mu: float) -> float:
     return float(_load().orc_dev(float(n), float(mu)))
+
+
+def transform(spec, n_params: int, u) -> np.ndarray:
+    """theta [P, n_params] from the minimiser's parameters u [P, n_u] through a workloads.TransformSpec
+    (PAPER.md:171, :141)."""
+    lib = _load()
+    u = np.ascontiguousarray(np.atleast_2d(u), dtype=np.float64)
+    assert u.shape[1] == spec.n_u
+    keep = []
+
+    def arr(a, dt):
+        a = np.ascontiguousarray(a, dtype=dt)
+        keep.append(a)
+        return a.ctypes.data
+    src = np.ascontiguousarray(spec.copy_src, dtype=np.int32)
+    cst = np.ascontiguousarray(spec.copy_const, dtype=np.float64)
+    assert src.shape == (n_params,) and cst.shape == (n_params,)
+    blocks = list(spec.blocks)
+    tb = (_TransformBlock * max(1, len(blocks)))()
+    for k, b in enumerate(blocks):
+        n_out, n_in = len(b.idx_out), len(b.idx_in)
+        assert np.shape(b.matrix) == (n_out, n_in) and np.shape(b.offset) == (n_out,) and np.shape(b.centre) == (n_in,)
+        tb[k].n_out, tb[k].n_in = n_out, n_in
+        tb[k].idx_out, tb[k].idx_in = arr(b.idx_out, np.int32), arr(b.idx_in, np.int32)
+        tb[k].offset, tb[k].centre, tb[k].matrix = arr(b.offset, np.float64), arr(b.centre, np.float64), arr(b.matrix, np.float64)
+    theta = np.empty((u.shape[0], n_params), dtype=np.float64)
+    rc = lib.orc_transform(n_params, spec.n_u, src.ctypes.data, cst.ctypes.data, len(blocks), tb, u.shape[0],
+                           _dp(u), _dp(theta))
+    if rc != 0:
+        raise ValueError(f"orc_transform failed ({rc})")
+    return theta
 
 
 def max_threads() -> int:

@@ -304,3 +304,28 @@ int orc_nll(const orc_model *m, const orc_events *ev, int32_t P, const double *p
     free(hist);
     return rc;
 }
+
+/* the affine map written out; the sum over j in index order with fma (the same
+ * correctly rounded sequence on any machine). */
+int orc_transform(int32_t n_params, int32_t n_u, const int32_t *copy_src, const double *copy_const,
+                  int32_t n_blocks, const orc_transform_block *blocks, int32_t P, const double *u, double *theta)
+{
+    for (int32_t p = 0; p < P; ++p) {
+        const double *up = u + (int64_t)p * n_u;
+        double *tp = theta + (int64_t)p * n_params;
+        for (int32_t j = 0; j < n_params; ++j) {
+            if (copy_src[j] >= n_u) return -1;
+            tp[j] = copy_src[j] >= 0 ? up[copy_src[j]] : (copy_const ? copy_const[j] : 0.0);
+        }
+        for (int32_t k = 0; k < n_blocks; ++k) {
+            const orc_transform_block *B = &blocks[k];
+            for (int32_t i = 0; i < B->n_out; ++i) {
+                double acc = B->offset[i];
+                for (int32_t j = 0; j < B->n_in; ++j)
+                    acc = fma(B->matrix[(int64_t)i * B->n_in + j], up[B->idx_in[j]] - B->centre[j], acc);
+                tp[B->idx_out[i]] = acc;
+            }
+        }
+    }
+    return 0;
+}

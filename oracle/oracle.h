@@ -118,6 +118,23 @@ int orc_nll_from_mu(const orc_model *m, int32_t P, const double *params, const d
 int orc_nll(const orc_model *m, const orc_events *ev, int32_t P, const double *params,
             const double *data, double *nll, int n_threads);
 
+/* Transformation layer between the minimiser's parameters u and the model parameters theta (PAPER.md:171
+ * "A transformation layer applies the covariance of any changed model parameter"; "the 9 polynomial
+ * coefficients can be expressed by 7 independent parameters"):
+ *   theta_j = u[copy_src[j]]  (or copy_const[j] where copy_src[j] < 0), then for every block, in order,
+ *   theta[idx_out[i]] = offset[i] + sum_j matrix[i][j] (u[idx_in[j]] - centre[j]). */
+typedef struct {
+    int32_t        n_out, n_in;
+    const int32_t *idx_out;
+    const int32_t *idx_in;
+    const double  *offset;     /* [n_out] */
+    const double  *centre;     /* [n_in] */
+    const double  *matrix;     /* [n_out * n_in] row-major */
+} orc_transform_block;
+
+int orc_transform(int32_t n_params, int32_t n_u, const int32_t *copy_src, const double *copy_const,
+                  int32_t n_blocks, const orc_transform_block *blocks, int32_t P, const double *u, double *theta);
+
 /* Number of threads orc_spectra would use for n_threads <= 0. */
 int orc_max_threads(void);
 

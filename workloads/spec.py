@@ -67,6 +67,26 @@ class PriorBlock:
 
 
 @dataclass
+class TransformBlock:
+    """theta[idx_out] = offset + matrix (u[idx_in] - centre): one block of the transformation layer between the
+    minimiser's parameters u and the model parameters theta (the 9 <- 7 energy-response map of
+    PAPER.md:141 is a 9 x 7 block, a Cholesky factor of a covariance a square one)."""
+    idx_out: np.ndarray       # int32 [n_out] indices into theta
+    idx_in: np.ndarray        # int32 [n_in] indices into u
+    offset: np.ndarray        # float64 [n_out]
+    centre: np.ndarray        # float64 [n_in]
+    matrix: np.ndarray        # float64 [n_out, n_in]
+
+
+@dataclass
+class TransformSpec:
+    n_u: int                  # length of the minimiser's parameter vector
+    copy_src: np.ndarray      # int32 [n_params]: theta_j = u[copy_src[j]], or copy_const[j] where copy_src[j] < 0
+    copy_const: np.ndarray    # float64 [n_params]
+    blocks: List[TransformBlock] = field(default_factory=list)
+
+
+@dataclass
 class ModelSpec:
     osc_model: int
     n_params: int
