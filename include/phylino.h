@@ -120,6 +120,20 @@ typedef struct {
 } phylino_prior_block;
 #define PHYLINO_MAX_BLOCK 1024
 
+/* One block of the transformation layer between the minimiser's parameters u and the model parameters theta
+ * ("A transformation layer applies the covariance of any changed model parameter within the
+ * calculation of the likelihood"; "the 9 polynomial coefficients can be expressed by 7 independent
+ * parameters"): theta[idx_out[i]] = offset[i] + sum_j matrix[i][j] (u[idx_in[j]] - centre[j]).  A Cholesky factor
+ * of a covariance is a square block, the 9 <- 7 energy-response map a 9 x 7 one.  HOST pointers, deep-copied. */
+typedef struct {
+    int32_t        n_out, n_in;   /* 1 ... PHYLINO_MAX_BLOCK each */
+    const int32_t *idx_out;       /* HOST [n_out] indices into theta */
+    const int32_t *idx_in;        /* HOST [n_in] indices into u */
+    const double  *offset;        /* HOST [n_out] */
+    const double  *centre;        /* HOST [n_in] */
+    const double  *matrix;        /* HOST [n_out * n_in] row-major */
+} phylino_transform_block;
+
 /* Create a context on CUDA device `device`.  `cuda_stream` is a cudaStream_t (0 = default stream)
  * on which all later work of this context is enqueued.  Fails with PHYLINO_ERR_CUDA when there is
  * no such device (there is no CPU fallback). */
@@ -191,6 +205,20 @@ PHYLINO_API phylino_status phylino_nll_ensemble(phylino_ctx *ctx, int P, const d
  * PHYLINO_ERR_SHAPE for n or an index out of range, PHYLINO_ERR_ARG for NULL arrays or non-finite
  * mean / inv_cov entries. */
 PHYLINO_API phylino_status phylino_set_prior_blocks(phylino_ctx *ctx, int n_blocks, const phylino_prior_block *blocks);
+
+/* Transformation layer.  After this call every `params` argument (DEVICE or HOST) is a batch of the minimiser's
+ * vectors u, [P x n_u] row-major, and the library forms theta itself before anything else:
+ *   theta_j = u[copy_src[j]]  (copy_const[j] where copy_src[j] < 0; copy_src HOST [n_params], copy_const HOST
+ *   [n_params], may be NULL if no entry of copy_src is negative), then for every block, in order,
+ *   theta[idx_out] = offset + matrix (u[idx_in] - centre); the sums run over j in index order with fma, on the
+ *   device for the DEVICE entry points (one extra kernel), on the host for the HOST ones (identical bits).
+ * Priors (diagonal and blocks) and every index of the model descriptor keep referring to theta.  n_u = 0 with
+ * n_blocks = 0 removes the layer; phylino_set_model removes it too.  Synchronises the stream.
+ * phylino_param_width: n_u if a layer is set, else n_params (0 before set_model). */
+PHYLINO_API phylino_status phylino_set_transform(phylino_ctx *ctx, int n_u, const int32_t *copy_src,
+                                                 const double *copy_const, int n_blocks,
+                                                 const phylino_transform_block *blocks);
+PHYLINO_API int64_t phylino_param_width(const phylino_ctx *ctx);
 
 /* Sizes the caller needs for its buffers. */
 PHYLINO_API int64_t phylino_total_bins(const phylino_ctx *ctx);     /* sum_d n_bins, 0 before set_model */

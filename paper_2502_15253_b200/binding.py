@@ -22,7 +22,7 @@ abi_symbols = (
     "phylino_set_tuning", "phylino_launch_count", "phylino_last_error", "phylino_peak_fp64",
     "phylino_expectation", "phylino_set_timing", "phylino_last_kernel_ms",
     "phylino_set_caching", "phylino_last_plan", "phylino_set_prior_blocks",
-    "phylino_nll_ensemble",
+    "phylino_nll_ensemble", "phylino_set_transform", "phylino_param_width",
 )
 
 _STATUS = {0: "OK", 1: "ERR_ARG", 2: "ERR_SHAPE", 3: "ERR_STATE", 4: "ERR_OOM", 5: "ERR_CUDA"}
@@ -46,6 +46,11 @@ class _Dataset(C.Structure):
 
 class _PriorBlock(C.Structure):
     _fields_ = [("n", C.c_int32), ("idx", C.c_void_p), ("mean", C.c_void_p), ("inv_cov", C.c_void_p)]
+
+
+class _TransformBlock(C.Structure):
+    _fields_ = [("n_out", C.c_int32), ("n_in", C.c_int32), ("idx_out", C.c_void_p), ("idx_in", C.c_void_p),
+                ("offset", C.c_void_p), ("centre", C.c_void_p), ("matrix", C.c_void_p)]
 
 
 class _Model(C.Structure):
@@ -101,6 +106,10 @@ def load_library():
     lib.phylino_total_bins.argtypes = [vp]
     lib.phylino_total_events.restype = i64
     lib.phylino_total_events.argtypes = [vp]
+    lib.phylino_set_transform.restype = i32
+    lib.phylino_set_transform.argtypes = [vp, i32, vp, vp, i32, C.POINTER(_TransformBlock)]
+    lib.phylino_param_width.restype = i64
+    lib.phylino_param_width.argtypes = [vp]
     lib.phylino_nll_ensemble.restype = i32
     lib.phylino_nll_ensemble.argtypes = [vp, i32, vp, i32, vp, vp]
     lib.phylino_set_prior_blocks.restype = i32
@@ -174,8 +183,8 @@ class Phylino:
         if not (isinstance(params, t.Tensor) and params.is_cuda and params.dtype == t.float64
                 and params.is_contiguous() and params.device.index == self.device):
             raise TypeError("params must be a contiguous float64 CUDA tensor on the context's device")
-        if params.dim() != 2 or params.shape[1] != self.n_params:
-            raise ValueError(f"params must be [P, {self.n_params}], got {tuple(params.shape)}")
+        if params.dim() != 2 or params.shape[1] != self.param_width:
+            raise ValueError(f"params must be [P, {self.param_width}], got {tuple(params.shape)}")
         return params
 
     # -- phylino_set_model ---------------------------------------------------------------------
@@ -320,6 +329,34 @@ class Phylino:
             arr[k].n, arr[k].idx, arr[k].mean, arr[k].inv_cov = int(i.size), i.ctypes.data, m.ctypes.data, v.ctypes.data
         self._check(self._lib.phylino_set_prior_blocks(self._ctx, len(blocks), arr if blocks else None))
 
+    def set_transform(self, spec=None):
+        """spec: workloads.TransformSpec (n_u, copy_src, copy_const, blocks) or None to remove the layer."""
+        if spec is None:
+            self._check(self._lib.phylino_set_transform(self._ctx, 0, None, None, 0, None))
+            return
+        keep = []
+
+        def arr(a, dt):
+            a = np.ascontiguousarray(a, dtype=dt)
+            keep.append(a)
+            return a.ctypes.data
+        blocks = list(spec.blocks)
+        tb = (_TransformBlock * max(1, len(blocks)))()
+        for k, b in enumerate(blocks):
+            tb[k].n_out, tb[k].n_in = len(b.idx_out), len(b.idx_in)
+            if np.shape(b.matrix) != (tb[k].n_out, tb[k].n_in):
+                raise ValueError("transform block: matrix must be [n_out, n_in]")
+            tb[k].idx_out, tb[k].idx_in = arr(b.idx_out, np.int32), arr(b.idx_in, np.int32)
+            tb[k].offset, tb[k].centre = arr(b.offset, np.float64), arr(b.centre, np.float64)
+            tb[k].matrix = arr(b.matrix, np.float64)
+        self._check(self._lib.phylino_set_transform(self._ctx, int(spec.n_u), arr(spec.copy_src, np.int32),
+                                                    arr(spec.copy_const, np.float64), len(blocks),
+                                                    tb if blocks else None))
+
+    @property
+    def param_width(self) -> int:
+        return int(self._lib.phylino_param_width(self._ctx))
+
     def set_caching(self, on: bool = True):
         self._check(self._lib.phylino_set_caching(self._ctx, int(bool(on))))
 
@@ -349,7 +386,7 @@ class Phylino:
     def nll_host(self, params: np.ndarray, data: np.ndarray, out: Optional[np.ndarray] = None) -> np.ndarray:
         p = np.ascontiguousarray(params, dtype=np.float64)
         d = np.ascontiguousarray(data, dtype=np.float64)
-        if p.ndim != 2 or p.shape[1] != self.n_params or d.shape != (self.total_bins,):
+        if p.ndim != 2 or p.shape[1] != self.param_width or d.shape != (self.total_bins,):
             raise ValueError("bad shapes")
         if out is None:
             out = np.empty(p.shape[0], dtype=np.float64)
@@ -359,7 +396,7 @@ class Phylino:
 
     def spectra_host(self, params: np.ndarray, out: Optional[np.ndarray] = None) -> np.ndarray:
         p = np.ascontiguousarray(params, dtype=np.float64)
-        if p.ndim != 2 or p.shape[1] != self.n_params:
+        if p.ndim != 2 or p.shape[1] != self.param_width:
             raise ValueError("bad shapes")
         if out is None:
             out = np.empty((p.shape[0], self.total_bins), dtype=np.float64)

@@ -81,6 +81,17 @@ void free_tables(phylino_ctx *c)
     f = FinalizeArgs{};
 }
 
+void free_transform(phylino_ctx *c)
+{
+    TransformArgs &t = c->tf;
+    cudaFree((void *)t.copy_src); cudaFree((void *)t.copy_const); cudaFree((void *)t.row_off);
+    cudaFree((void *)t.col_off); cudaFree((void *)t.mat_off); cudaFree((void *)t.idx_out);
+    cudaFree((void *)t.idx_in); cudaFree((void *)t.offset); cudaFree((void *)t.centre); cudaFree((void *)t.matrix);
+    t = TransformArgs{};
+    c->have_tf = false;
+    c->n_u = 0;
+}
+
 void free_all(phylino_ctx *c)
 {
     for (auto &d : c->ds) free_events(d);
@@ -92,6 +103,8 @@ void free_all(phylino_ctx *c)
     c->d_rec = nullptr; c->d_thr = nullptr; c->d_safe = nullptr; c->d_counter = nullptr; c->point_capacity = 0;
     cudaFree(c->d_plan); c->d_plan = nullptr; c->plan_capacity = 0;
     cudaFree(c->d_mu); c->d_mu = nullptr; c->mu_capacity = 0;
+    free_transform(c);
+    cudaFree(c->d_theta); c->d_theta = nullptr; c->theta_capacity = 0;
     cudaFree(c->d_stage); c->d_stage = nullptr;
     if (c->h_pin) cudaFreeHost(c->h_pin);
     c->h_pin = nullptr; c->stage_capacity = 0;
@@ -296,6 +309,52 @@ phylino_status ensure_stage(phylino_ctx *ctx, int64_t doubles)
     CU(cudaMalloc((void **)&ctx->d_stage, doubles * sizeof(double)));
     CU(cudaHostAlloc((void **)&ctx->h_pin, doubles * sizeof(double), cudaHostAllocDefault));
     ctx->stage_capacity = doubles;
+    return PHYLINO_OK;
+}
+
+/* width of one row of the caller's parameter batch: the minimiser's vector if a transformation layer is set */
+int64_t param_width(const phylino_ctx *ctx) { return ctx->have_tf ? ctx->n_u : ctx->n_params; }
+
+/* the transformation layer on the host: the same fma sequence as transform.cu */
+void host_transform(const phylino_ctx *ctx, int P, const double *u, double *theta)
+{
+    const int NP = ctx->n_params, NU = ctx->n_u;
+    const int n_blocks = (int)ctx->tf_mat_off.size();
+    for (int p = 0; p < P; ++p) {
+        const double *up = u + (size_t)p * NU;
+        double *tp = theta + (size_t)p * NP;
+        for (int j = 0; j < NP; ++j) tp[j] = ctx->tf_src[j] >= 0 ? up[ctx->tf_src[j]] : ctx->tf_const[j];
+        for (int k = 0; k < n_blocks; ++k) {
+            const int ro = ctx->tf_row_off[k], n_out = ctx->tf_row_off[k + 1] - ro;
+            const int co = ctx->tf_col_off[k], n_in = ctx->tf_col_off[k + 1] - co;
+            const double *M = ctx->tf_matrix.data() + ctx->tf_mat_off[k];
+            for (int i = 0; i < n_out; ++i) {
+                double acc = ctx->tf_offset[ro + i];
+                for (int j = 0; j < n_in; ++j)
+                    acc = std::fma(M[(size_t)i * n_in + j], up[ctx->tf_idx_in[co + j]] - ctx->tf_centre[co + j], acc);
+                tp[ctx->tf_idx_out[ro + i]] = acc;
+            }
+        }
+    }
+}
+
+/* DEVICE batch of a device entry point -> model parameters: the caller's pointer, or the transformed copy */
+phylino_status resolve_params(phylino_ctx *ctx, int P, const double *params, const double **theta)
+{
+    *theta = params;
+    if (!ctx->have_tf || P == 0) return PHYLINO_OK;
+    const int64_t need = (int64_t)P * ctx->n_params;
+    if (need > ctx->theta_capacity) {
+        CU(cudaStreamSynchronize(ctx->stream));
+        cudaFree(ctx->d_theta); ctx->d_theta = nullptr; ctx->theta_capacity = 0;
+        CU(cudaMalloc((void **)&ctx->d_theta, need * sizeof(double)));
+        ctx->theta_capacity = need;
+    }
+    TransformArgs t = ctx->tf;
+    t.P = P; t.u = params; t.theta = ctx->d_theta;
+    CU(launch_transform(t, ctx->stream));
+    ctx->launches += 1;
+    *theta = ctx->d_theta;
     return PHYLINO_OK;
 }
 
@@ -726,6 +785,7 @@ phylino_status phylino_spectra(phylino_ctx *ctx, int P, const double *params, do
     phylino_status s = check_ready(ctx, P, params, hist);
     if (s != PHYLINO_OK || P == 0) return s;
     DeviceGuard g(ctx->device);
+    if ((s = resolve_params(ctx, P, params, &params)) != PHYLINO_OK) return s;
     if ((s = ensure_acc(ctx, P)) != PHYLINO_OK) return s;
     if ((s = enqueue_spectra(ctx, P, params)) != PHYLINO_OK) return s;
     return enqueue_finalize(ctx, P, params, nullptr, hist, nullptr);
@@ -737,6 +797,7 @@ phylino_status phylino_nll(phylino_ctx *ctx, int P, const double *params, const 
     if (s != PHYLINO_OK || P == 0) return s;
     if (!data) return fail(ctx, PHYLINO_ERR_ARG, "NULL data pointer");
     DeviceGuard g(ctx->device);
+    if ((s = resolve_params(ctx, P, params, &params)) != PHYLINO_OK) return s;
     if ((s = ensure_acc(ctx, P)) != PHYLINO_OK) return s;
     if ((s = enqueue_spectra(ctx, P, params)) != PHYLINO_OK) return s;
     return enqueue_finalize(ctx, P, params, data, nullptr, nll);
@@ -751,6 +812,7 @@ phylino_status phylino_nll_ensemble(phylino_ctx *ctx, int P, const double *param
     if (P == 0 || E == 0) return PHYLINO_OK;
     if (!data) return fail(ctx, PHYLINO_ERR_ARG, "NULL data pointer");
     DeviceGuard g(ctx->device);
+    if ((s = resolve_params(ctx, P, params, &params)) != PHYLINO_OK) return s;
     if ((s = ensure_acc(ctx, P)) != PHYLINO_OK) return s;
     const int64_t need = (int64_t)P * ctx->total_bins;
     if (need > ctx->mu_capacity) {
@@ -773,6 +835,7 @@ phylino_status phylino_expectation(phylino_ctx *ctx, int P, const double *params
     phylino_status s = check_ready(ctx, P, params, mu);
     if (s != PHYLINO_OK || P == 0) return s;
     DeviceGuard g(ctx->device);
+    if ((s = resolve_params(ctx, P, params, &params)) != PHYLINO_OK) return s;
     if ((s = ensure_acc(ctx, P)) != PHYLINO_OK) return s;
     if ((s = enqueue_spectra(ctx, P, params)) != PHYLINO_OK) return s;
     return enqueue_finalize(ctx, P, params, nullptr, mu, nullptr, 1);
@@ -783,6 +846,7 @@ phylino_status phylino_event_bins(phylino_ctx *ctx, int P, const double *params,
     phylino_status s = check_ready(ctx, P, params, bins);
     if (s != PHYLINO_OK || P == 0) return s;
     DeviceGuard g(ctx->device);
+    if ((s = resolve_params(ctx, P, params, &params)) != PHYLINO_OK) return s;
     if ((s = ensure_acc(ctx, P)) != PHYLINO_OK) return s;
     SpectraArgs a{};
     fill_datasets(ctx, a);
@@ -813,12 +877,13 @@ phylino_status phylino_nll_host(phylino_ctx *ctx, int P, const double *params_ho
     const int64_t np = (int64_t)P * ctx->n_params, tb = ctx->total_bins;
     if ((s = ensure_stage(ctx, np + tb + P)) != PHYLINO_OK) return s;
     if ((s = ensure_acc(ctx, P)) != PHYLINO_OK) return s;
-    std::memcpy(ctx->h_pin, params_host, np * sizeof(double));
+    if (ctx->have_tf) host_transform(ctx, P, params_host, ctx->h_pin);
+    else std::memcpy(ctx->h_pin, params_host, np * sizeof(double));
     std::memcpy(ctx->h_pin + np, data_host, tb * sizeof(double));
     CU(cudaMemcpyAsync(ctx->d_stage, ctx->h_pin, (np + tb) * sizeof(double), cudaMemcpyHostToDevice, ctx->stream));
     bool cached = false;
     if (ctx->caching &&
-        (s = enqueue_cached(ctx, P, params_host, ctx->d_stage, ctx->d_stage + np, nullptr, ctx->d_stage + np + tb, &cached)) != PHYLINO_OK)
+        (s = enqueue_cached(ctx, P, ctx->h_pin, ctx->d_stage, ctx->d_stage + np, nullptr, ctx->d_stage + np + tb, &cached)) != PHYLINO_OK)
         return s;
     if (!cached) {
         if ((s = enqueue_spectra(ctx, P, ctx->d_stage)) != PHYLINO_OK) return s;
@@ -838,11 +903,12 @@ phylino_status phylino_spectra_host(phylino_ctx *ctx, int P, const double *param
     const int64_t np = (int64_t)P * ctx->n_params, nh = (int64_t)P * ctx->total_bins;
     if ((s = ensure_stage(ctx, np + nh)) != PHYLINO_OK) return s;
     if ((s = ensure_acc(ctx, P)) != PHYLINO_OK) return s;
-    std::memcpy(ctx->h_pin, params_host, np * sizeof(double));
+    if (ctx->have_tf) host_transform(ctx, P, params_host, ctx->h_pin);
+    else std::memcpy(ctx->h_pin, params_host, np * sizeof(double));
     CU(cudaMemcpyAsync(ctx->d_stage, ctx->h_pin, np * sizeof(double), cudaMemcpyHostToDevice, ctx->stream));
     bool cached = false;
     if (ctx->caching &&
-        (s = enqueue_cached(ctx, P, params_host, ctx->d_stage, nullptr, ctx->d_stage + np, nullptr, &cached)) != PHYLINO_OK)
+        (s = enqueue_cached(ctx, P, ctx->h_pin, ctx->d_stage, nullptr, ctx->d_stage + np, nullptr, &cached)) != PHYLINO_OK)
         return s;
     if (!cached) {
         if ((s = enqueue_spectra(ctx, P, ctx->d_stage)) != PHYLINO_OK) return s;
@@ -853,6 +919,73 @@ phylino_status phylino_spectra_host(phylino_ctx *ctx, int P, const double *param
     std::memcpy(hist_host, ctx->h_pin + np, nh * sizeof(double));
     return PHYLINO_OK;
 }
+
+phylino_status phylino_set_transform(phylino_ctx *ctx, int n_u, const int32_t *copy_src, const double *copy_const,
+                                     int n_blocks, const phylino_transform_block *blocks)
+{
+    if (!ctx) return PHYLINO_ERR_ARG;
+    if (!ctx->have_model) return fail(ctx, PHYLINO_ERR_STATE, "phylino_set_model must come before phylino_set_transform");
+    DeviceGuard g(ctx->device);
+    CU(cudaStreamSynchronize(ctx->stream));
+    if (n_u == 0 && n_blocks == 0) { free_transform(ctx); ctx->err.clear(); return PHYLINO_OK; }
+    if (n_u < 1 || n_blocks < 0) return fail(ctx, PHYLINO_ERR_SHAPE, "n_u = %d, n_blocks = %d", n_u, n_blocks);
+    if (!copy_src || (n_blocks > 0 && !blocks)) return fail(ctx, PHYLINO_ERR_ARG, "NULL copy_src or blocks");
+    const int NP = ctx->n_params;
+    std::vector<int32_t> src(copy_src, copy_src + NP), row_off(1, 0), col_off(1, 0), idx_out, idx_in;
+    std::vector<double> cst(NP, 0.0), offset, centre, matrix;
+    std::vector<int64_t> mat_off;
+    for (int j = 0; j < NP; ++j) {
+        if (src[j] >= n_u) return fail(ctx, PHYLINO_ERR_SHAPE, "copy_src[%d] = %d out of range", j, src[j]);
+        if (src[j] < 0) {
+            if (!copy_const || !std::isfinite(copy_const[j])) return fail(ctx, PHYLINO_ERR_ARG, "copy_const[%d] missing or not finite", j);
+            cst[j] = copy_const[j];
+        }
+    }
+    for (int k = 0; k < n_blocks; ++k) {
+        const phylino_transform_block &b = blocks[k];
+        if (b.n_out < 1 || b.n_in < 1 || b.n_out > PHYLINO_MAX_BLOCK || b.n_in > PHYLINO_MAX_BLOCK)
+            return fail(ctx, PHYLINO_ERR_SHAPE, "transform block %d: %d x %d not in 1..%d", k, b.n_out, b.n_in, PHYLINO_MAX_BLOCK);
+        if (!b.idx_out || !b.idx_in || !b.offset || !b.centre || !b.matrix) return fail(ctx, PHYLINO_ERR_ARG, "transform block %d: NULL array", k);
+        for (int i = 0; i < b.n_out; ++i)
+            if (b.idx_out[i] < 0 || b.idx_out[i] >= NP || !std::isfinite(b.offset[i])) return fail(ctx, PHYLINO_ERR_SHAPE, "transform block %d: idx_out/offset[%d]", k, i);
+        for (int j = 0; j < b.n_in; ++j)
+            if (b.idx_in[j] < 0 || b.idx_in[j] >= n_u || !std::isfinite(b.centre[j])) return fail(ctx, PHYLINO_ERR_SHAPE, "transform block %d: idx_in/centre[%d]", k, j);
+        for (int64_t i = 0; i < (int64_t)b.n_out * b.n_in; ++i)
+            if (!std::isfinite(b.matrix[i])) return fail(ctx, PHYLINO_ERR_ARG, "transform block %d: matrix[%lld] is not finite", k, (long long)i);
+        mat_off.push_back((int64_t)matrix.size());
+        idx_out.insert(idx_out.end(), b.idx_out, b.idx_out + b.n_out);
+        offset.insert(offset.end(), b.offset, b.offset + b.n_out);
+        idx_in.insert(idx_in.end(), b.idx_in, b.idx_in + b.n_in);
+        centre.insert(centre.end(), b.centre, b.centre + b.n_in);
+        matrix.insert(matrix.end(), b.matrix, b.matrix + (size_t)b.n_out * b.n_in);
+        row_off.push_back((int32_t)idx_out.size());
+        col_off.push_back((int32_t)idx_in.size());
+    }
+    free_transform(ctx);
+    TransformArgs &t = ctx->tf;
+    cudaStream_t st = ctx->stream;
+    CU(upload((int32_t **)&t.copy_src, src, st));
+    CU(upload((double **)&t.copy_const, cst, st));
+    CU(upload((int32_t **)&t.row_off, row_off, st));
+    CU(upload((int32_t **)&t.col_off, col_off, st));
+    CU(upload((int64_t **)&t.mat_off, mat_off, st));
+    CU(upload((int32_t **)&t.idx_out, idx_out, st));
+    CU(upload((int32_t **)&t.idx_in, idx_in, st));
+    CU(upload((double **)&t.offset, offset, st));
+    CU(upload((double **)&t.centre, centre, st));
+    CU(upload((double **)&t.matrix, matrix, st));
+    CU(cudaStreamSynchronize(st));
+    t.n_params = NP; t.n_u = n_u; t.n_blocks = n_blocks;
+    ctx->tf_src = src; ctx->tf_const = cst; ctx->tf_row_off = row_off; ctx->tf_col_off = col_off;
+    ctx->tf_mat_off = mat_off; ctx->tf_idx_out = idx_out; ctx->tf_idx_in = idx_in;
+    ctx->tf_offset = offset; ctx->tf_centre = centre; ctx->tf_matrix = matrix;
+    ctx->n_u = n_u;
+    ctx->have_tf = true;
+    ctx->err.clear();
+    return PHYLINO_OK;
+}
+
+int64_t phylino_param_width(const phylino_ctx *ctx) { return ctx && ctx->have_model ? param_width(ctx) : 0; }
 
 phylino_status phylino_set_prior_blocks(phylino_ctx *ctx, int n_blocks, const phylino_prior_block *blocks)
 {

@@ -136,7 +136,22 @@ struct FinalizeArgs {
     const int32_t *pt_comp;       /* [P x (n_terms + 1)] accumulator rows: W, then the row of each term's C */
 };
 
-/* kernel launchers (spectra.cu, finalize.cu, peaks.cu) */
+/* transformation layer (transform.cu), all DEVICE pointers except P-dependent u / theta set per call */
+struct TransformArgs {
+    int32_t P, n_params, n_u, n_blocks;
+    const int32_t *copy_src;      /* [n_params] */
+    const double  *copy_const;    /* [n_params] */
+    const int32_t *row_off;       /* [n_blocks + 1] offsets into idx_out / offset */
+    const int32_t *col_off;       /* [n_blocks + 1] offsets into idx_in / centre */
+    const int64_t *mat_off;       /* [n_blocks] offsets into matrix */
+    const int32_t *idx_out, *idx_in;
+    const double  *offset, *centre, *matrix;
+    const double  *u;             /* [P x n_u] */
+    double        *theta;         /* [P x n_params] */
+};
+
+/* kernel launchers (spectra.cu, finalize.cu, transform.cu, peaks.cu) */
+cudaError_t launch_transform(const TransformArgs &a, cudaStream_t st);
 cudaError_t launch_setup(const SpectraArgs &a, int S, cudaStream_t st);
 cudaError_t spectra_max_warps(int S, int sm_count, int *warps);
 cudaError_t launch_spectra(const SpectraArgs &a, int S, cudaStream_t st, bool pdl);
@@ -198,6 +213,15 @@ struct phylino_ctx {
     int32_t *d_plan = nullptr;                     /* vp_class | vp_src | class_rep | pt_comp */
     int64_t plan_capacity = 0;                     /* int32 entries */
     int64_t last_virtual_points = 0, last_classes = 0;
+    /* transformation layer (phylino_set_transform): host copy for the host entry points, device tables */
+    bool have_tf = false;
+    int32_t n_u = 0;
+    std::vector<int32_t> tf_src, tf_row_off, tf_col_off, tf_idx_out, tf_idx_in;
+    std::vector<int64_t> tf_mat_off;
+    std::vector<double>  tf_const, tf_offset, tf_centre, tf_matrix;
+    phylino::TransformArgs tf{};                   /* device table pointers */
+    double *d_theta = nullptr;                     /* [theta_capacity] transformed batch of a device call */
+    int64_t theta_capacity = 0;
     double *d_mu = nullptr;                        /* [mu_capacity] expectations of an ensemble call */
     int64_t mu_capacity = 0;
     /* host-buffer entry points: pinned + device staging */

@@ -466,3 +466,69 @@ def test_infinite_reconstructed_energies(gpu, oracle_mod):
     params = np.array([[0.1, 2.5e-3, 0.85, 7.5e-5, 0.02, 1.01, -0.001], [0.1, 2.5e-3, 0.85, 7.5e-5, -0.03, 0.98, 0.002]])
     h, h_o = _both(gpu, oracle_mod, _one_dataset_model(7, idx_a=(4, 5, 6), n_params=7), evs, params)
     _check_hist(h, h_o)
+
+
+def _transform_for_config3(wl, rng):
+    """u = (4 oscillation, 7 energy-response, the other 288 parameters): the 9 energy-scale coefficients of the
+    three datasets come from 7 parameters, a 41-parameter flux block goes through the Cholesky
+    factor of its covariance, everything else is copied."""
+    NP = wl.model.n_params
+    n_u = NP - 2
+    copy_src = np.full(NP, -1, np.int32)
+    copy_src[:4] = np.arange(4)
+    copy_src[13:] = np.arange(11, n_u)                   # theta[13:] <- u[11:]
+    M97 = np.zeros((9, 7))
+    for d in range(3):
+        M97[3 * d + 2, 0] = 1.0
+        M97[3 * d + 0, 1 + 2 * d] = 1.0
+        M97[3 * d + 1, 2 + 2 * d] = 1.0
+    M97 += 0.05 * rng.normal(size=M97.shape)
+    A = rng.normal(size=(41, 41))
+    L = np.linalg.cholesky((A @ A.T / 41 + 0.2 * np.eye(41)) * 4e-4)
+    flux_out = np.arange(13, 54, dtype=np.int32)
+    flux_in = flux_out - 2
+    blocks = [workloads.TransformBlock(np.arange(4, 13, dtype=np.int32), np.arange(4, 11, dtype=np.int32),
+                                       np.tile([0.0, 1.0, 0.0], 3), np.zeros(7), M97),
+              workloads.TransformBlock(flux_out, flux_in, np.ones(41), np.zeros(41), L)]
+    return workloads.TransformSpec(n_u=n_u, copy_src=copy_src, copy_const=np.zeros(NP), blocks=blocks)
+
+
+def test_transformation_layer(gpu, oracle_mod):
+    """batches of the minimiser's vectors u through the device and the host entry points,
+    dense and cached, against oracle.transform followed by the oracle's NLL; then the layer removed."""
+    wl = workloads.make_config(3, scale=0.003, n_points=40)
+    rng = np.random.default_rng(21)
+    spec = _transform_for_config3(wl, rng)
+    P = 40
+    u = np.zeros((P, spec.n_u))
+    u[:, :4] = wl.params[:P, :4]
+    u[:, 4:11] = rng.normal(0, 0.004, (P, 7))            # energy-response parameters
+    u[:, 11:] = wl.params[:P, 13:]
+    u[:, 11:52] = rng.normal(0, 1.0, (P, 41))            # whitened flux parameters
+    u[20:] = u[:20]                                      # repeated energy scales: something for the cache
+    u[20:, 0] *= 1.05
+    theta = oracle_mod.transform(spec, wl.model.n_params, u)
+    orc = oracle_mod.Oracle(wl.model, wl.events)
+    data = _data_for(orc, wl, oracle_mod)
+    nll_o = orc.nll(theta, data)
+    with gpu.Phylino() as ph:
+        ph.load_workload(wl)
+        assert ph.param_width == wl.model.n_params
+        ph.set_transform(spec)
+        assert ph.param_width == spec.n_u
+        nll_d = ph.nll(_dev(u), _dev(data)).cpu().numpy()
+        h_d = ph.spectra(_dev(u)).cpu().numpy()
+        nll_h = ph.nll_host(u, data)
+        ph.set_caching(True)
+        nll_c = ph.nll_host(u, data)
+        cached_vp = ph.last_plan()[0]
+        ph.set_caching(False)
+        with pytest.raises(ValueError):
+            ph.nll(_dev(theta), _dev(data))              # theta-wide batches are refused while the layer is set
+        ph.set_transform(None)
+        nll_plain = ph.nll(_dev(theta), _dev(data)).cpu().numpy()
+    assert np.abs(nll_d - nll_o).max() <= ABS_NLL
+    assert np.array_equal(nll_d, nll_h)                  # host and device transform: identical bits
+    assert np.array_equal(nll_d, nll_plain)              # and identical to handing in the oracle's theta
+    assert cached_vp > 0 and np.abs(nll_c - nll_o).max() <= ABS_NLL
+    _check_hist(h_d, orc.spectra(theta))
