@@ -116,6 +116,39 @@ def traffic_from_profile(config: int):
         return None
 
 
+def gradient_step_wall(pkg, torch, local, flush, steps=10):
+    """north_star: "wall time for a full gradient step" -- BASELINE.json configs[2] (3 x 2e6 events, 301
+    parameters, 603 central-difference points) through the host call a minimiser makes (H2D + kernels + D2H),
+    dense and with cross-point caching; a fresh batch every step, L2 flushed in between."""
+    wl = workloads.make_config(3)
+    ph = pkg.Phylino(device=local)
+    ph.load_workload(wl)
+    mu0 = ph.expectation(torch.as_tensor(wl.theta0[None, :].copy(), device="cuda")).cpu().numpy()[0]
+    data = workloads.poisson_counts(mu0, wl.seed + 7)
+    out = np.empty(wl.n_points)
+    res = {"workload": f"{wl.name} (BASELINE.json configs[2])", "events": wl.n_events, "points": wl.n_points,
+           "n_params": wl.model.n_params, "steps": steps}
+    for key, on in (("dense_ms", False), ("cached_ms", True)):
+        ph.set_caching(on)
+        h = wl.params.copy()
+        for _ in range(3):
+            ph.nll_host(h, data, out)
+        torch.cuda.synchronize()
+        t = 0.0
+        for i in range(steps):
+            h[:, 0] = wl.params[:, 0] * (1.0 + 1e-9 * (i + 1))
+            flush.zero_()
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            ph.nll_host(h, data, out)
+            t += time.perf_counter() - t0
+        res[key] = t / steps * 1e3
+        if on:
+            res["virtual_points"], res["energy_scale_classes"] = ph.last_plan()
+    ph.close()
+    return res
+
+
 def run_reference(args, wl, rank):
     """--impl reference: the CPU oracle, as it stands, on the host cores (bounded sample per step)."""
     if rank != 0:
@@ -157,6 +190,8 @@ def main():
     ap.add_argument("--max-warps", type=int, default=0, help="tuning: cap on the persistent grid's warps")
     ap.add_argument("--ref-points", type=int, default=16, help="points per step of --impl reference")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-gradient-step", action="store_true",
+                    help="skip the wall time of config 3's 603-point gradient step that the default run adds")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
 
@@ -343,6 +378,8 @@ def main():
         }
         if cached is not None:
             line["cached"] = cached
+        if world == 1 and args.config == 2 and not args.no_gradient_step:
+            line["gradient_step"] = gradient_step_wall(pkg, torch, local, flush)
         if world == 1 and not args.no_cpu_baseline:
             import oracle                                   # the cpu_baseline leg (test infrastructure)
             orc = oracle.Oracle(wl.model, wl.events)
