@@ -5,13 +5,16 @@
  * Layout of the work: ONE PARAMETER POINT PER LANE.  The E_vis-sorted events of a dataset are cut
  * into 96-byte batches of EB events and the batches into units; a work item is one unit x a chunk
  * of point groups (32 points each).  The warps of a persistent grid claim items from a global
- * counter (dynamic balance: units that contain bin edges cost more) and walk the unit once per
- * group: the event data (x = L/E, w, E_vis) are warp-uniform broadcast loads from one pointer,
- * everything that depends on the point (half-turn coefficients h_k, the run accumulators, the
- * current bin and its fp32 upper threshold) lives in the lane's registers.  No shared memory, no
- * shuffles in the loop, no barriers.  The next item's unit is prefetched into L2 while the current
- * one is walked.  A group of fewer than 32 points splits the unit into 32/PL sub-streams (PL =
- * points rounded up to a power of two), so that a batch of 1 point still uses all 32 lanes.
+ * counter (dynamic balance: units that contain bin edges cost more; the last stretch of the store is
+ * cut into quarter-size units so the warps run out of work together) and walk the unit once per group.
+ *
+ * Staging.  Each warp owns two unit-sized buffers in shared memory and one mbarrier per buffer; lane 0
+ * starts ONE bulk async copy (cp.async.bulk global -> shared, completion on the mbarrier) of the NEXT
+ * item's unit while the current one is walked.  The hot loop reads warp-uniform LDS.128 broadcasts;
+ * everything that depends on the point (half-turn coefficients h_k, the run accumulators, the current
+ * bin, its fp32 upper threshold and the one after it) lives in the lane's registers.  No shuffles in
+ * the loop, no block barriers.  A group of fewer than 17 points splits the unit into 32/PL sub-streams
+ * (PL = points rounded up to a power of two), so that a batch of 1 point still uses all 32 lanes.
  *
  * Oscillation weight (row a2).  P_ee = P0 + sum_k A_k g_k with g = 1/2 cos(2 phase) (devmath.cuh):
  * the lane accumulates C_k = sum_e w_e g_k(e) and W = sum_e w_e over a run of events that share a
@@ -22,9 +25,11 @@
  * the fp32 values of a dataset (checked per point by the setup kernel), so bin(E'(v)) >= b <=>
  * v >= T[b] with T[b] the smallest fp32 value whose E' reaches edges[b].  T is found by bisection
  * with the SAME fp64 fma sequence, hence the fp32 comparison decides exactly what the fp64
- * comparison E' >= edges[b] decides: bit-exact bins.  Events are sorted, so a batch lies inside the
- * lane's current bin iff its LAST event is below the bin's upper threshold: one fp32 compare per
- * batch.  Events outside the interval on which a table is proven (and points that fail the
+ * comparison E' >= edges[b] decides: bit-exact bins.  Events are sorted, so 4, 2 or 1 batches lie
+ * inside the lane's current bin iff the LAST event of the last one is below the bin's upper threshold:
+ * one fp32 compare, then a straight-line stretch of rows a2 + a4 (datasets whose weights are all exactly
+ * 1 skip the weight loads).  A lane opens its run at the first event of a unit from the load-time hint
+ * bin0 of the batch.  Events outside the interval on which a table is proven (and points that fail the
  * monotonicity check) take the per-event fp64 map.
  *
  * Histogram (rows a4, a5).  When a run ends (bin edge, end of the unit) its fp64 total is converted
@@ -32,6 +37,13 @@
  * Integer addition is associative: the result depends neither on which warp walks an item nor on
  * the order of arrival, i.e. bitwise reproducible with no float atomics anywhere (the cut of the
  * events into items is a function of the sizes only).
+ *
+ * Component mode (cross-point caching): the launch's points are virtual points (an energy-scale class
+ * plus S splittings) and a run is flushed as S + 1 separate sums; finalize.cu combines them per point.
+ *
+ * Launch.  The spectra kernel is a programmatic dependent of the setup kernel: barriers and the first
+ * event copy are set up while the setup kernel runs; griddepcontrol.wait precedes the first read of a
+ * record, a threshold or the work counter.
  */
 #include "devmath.cuh"
 
