@@ -86,3 +86,33 @@ def test_blocks_apply_in_order(oracle_mod):
         W.TransformBlock(np.array([1], np.int32), np.array([0], np.int32), np.array([1.0]), np.array([0.0]), np.array([[2.0]])),
         W.TransformBlock(np.array([1], np.int32), np.array([0], np.int32), np.array([5.0]), np.array([0.0]), np.array([[3.0]]))])
     assert np.array_equal(oracle_mod.transform(sp, 2, np.array([[2.0]])), [[2.0, 11.0]])
+
+
+def test_flux_rebinning_41_to_38_conserves_area(oracle_mod):
+    """41 flux parameters on uniform 0.25 MeV bins from 1 to 11.25 MeV, "transformed back to the
+    original binning".  The piecewise-constant, area-conserving version of that map is a 38 x 41 block of the
+    transformation layer: f_b = sum_j overlap(b, j) F_j / width_b (the analysis bins above 11.25 MeV keep 1).
+    Pin: the integral of the flux correction over any union of analysis bins equals the integral of the 41-bin
+    step function over the same range (R6 edges)."""
+    edges = W.dc_edges()
+    fine = 1.0 + 0.25 * np.arange(42)
+    M = np.zeros((38, 41))
+    off = np.zeros(38)
+    for b in range(38):
+        lo, hi = edges[b], edges[b + 1]
+        for j in range(41):
+            M[b, j] = max(0.0, min(hi, fine[j + 1]) - max(lo, fine[j])) / (hi - lo)
+        off[b] = 1.0 - M[b].sum()                      # the part of the bin above 11.25 MeV keeps the nominal 1
+    sp = W.TransformSpec(n_u=41, copy_src=np.full(38, -1, np.int32), copy_const=np.zeros(38),
+                         blocks=[W.TransformBlock(np.arange(38, dtype=np.int32), np.arange(41, dtype=np.int32),
+                                                  off, np.zeros(41), M)])
+    rng = np.random.default_rng(9)
+    F = 1.0 + 0.02 * rng.normal(size=(6, 41))
+    f = oracle_mod.transform(sp, 38, F)
+    widths = np.diff(edges)
+    for p in range(6):
+        # whole range 1-20 MeV, and 1-8 MeV where analysis and fine bins coincide
+        assert (f[p] * widths).sum() == pytest.approx((F[p] * 0.25).sum() + (20.0 - 11.25), rel=1e-13)
+        assert np.allclose(f[p, :28], F[p, :28], rtol=1e-14)
+        assert f[p, -1] == 1.0                         # 18-20 MeV: beyond the flux parametrisation
+    assert np.array_equal(oracle_mod.transform(sp, 38, np.ones((1, 41))), np.ones((1, 38)))
