@@ -268,6 +268,62 @@ __device__ __forceinline__ void flush_run(const SpectraArgs &a, const DatasetDev
     r.W = 0.0;
 }
 
+/* The flush at the end of a unit when the group has at most 16 points: the 32 / PL sub-streams of a point
+ * usually end in the same bin, and 32 lanes of every resident warp adding to the same one or two cells
+ * would queue at the L2 atomic unit (same-address atomics: a 6e6-event, 1-point call spent 0.45 ms there).
+ * Every lane converts its run to fixed point as usual; the integers of the lanes that share a cell are
+ * summed over the sub-streams with shuffles (exact, so the bits are those of the separate REDs) and the
+ * first lane of each cell issues one RED.  All 32 lanes call this together. */
+template <int S>
+__device__ __forceinline__ void flush_run_substreams(const SpectraArgs &a, const DatasetDev &ds, int p, bool active,
+                                                     int lg, int lane, Run<S> &r)
+{
+    const bool live = active && r.cur >= 0 && r.cur < ds.n_bins;
+    const int nq = a.comp ? S + 1 : 1;
+    long long q[S + 1];
+    unsigned fl[S + 1];
+#pragma unroll
+    for (int j = 0; j <= S; ++j) { q[j] = 0; fl[j] = 0; }
+    unsigned long long cell = ~0ull;
+    if (live) {
+        if (a.comp) {
+            cell = (unsigned long long)p * (S + 1) * a.total_bins + ds.bin_off + r.cur;
+#pragma unroll
+            for (int j = 0; j <= S; ++j) q[j] = to_fixed(j == 0 ? r.W : r.C[j - 1], ds.fx_scale, false, fl[j]);
+        } else {
+            double tot = a.rec[(size_t)(2 * S) * a.P + p] * r.W;
+#pragma unroll
+            for (int k = 0; k < S; ++k) tot = fma(a.rec[(size_t)(S + k) * a.P + p], r.C[k], tot);
+            cell = (unsigned long long)p * a.total_bins + ds.bin_off + r.cur;
+            q[0] = to_fixed(tot, ds.fx_scale, a.rec[(size_t)(2 * S + 1) * a.P + p] != 0.0, fl[0]);
+        }
+    }
+    long long sum[S + 1];
+#pragma unroll
+    for (int j = 0; j <= S; ++j) sum[j] = 0;
+    bool first = true;
+    const int pl = lane & ((1 << lg) - 1);
+    for (int src = pl; src < 32; src += 1 << lg) {              /* the sub-streams of this lane's point */
+        const unsigned long long c = __shfl_sync(0xffffffffu, cell, src);
+        const bool same = live && c == cell;
+        if (same && src < lane) first = false;
+#pragma unroll
+        for (int j = 0; j <= S; ++j) {
+            const long long v = __shfl_sync(0xffffffffu, q[j], src);
+            if (same && j < nq) sum[j] += v;
+        }
+    }
+    if (live) {
+        for (int j = 0; j < nq; ++j) {
+            if (first && sum[j]) atomicAdd((unsigned long long *)a.acc + cell + (size_t)j * a.total_bins, (unsigned long long)sum[j]);
+            if (fl[j]) atomicOr(a.flags + cell + (size_t)j * a.total_bins, fl[j]);
+        }
+    }
+#pragma unroll
+    for (int k = 0; k < S; ++k) r.C[k] = 0.0;
+    r.W = 0.0;
+}
+
 /* threshold row entry with the conventions thr[-1] = -inf, thr[B + 1] = +inf */
 __device__ __forceinline__ float thr_at(const float *thr, int B, int i)
 {
@@ -378,13 +434,14 @@ __device__ __forceinline__ void walk_unit(const SpectraArgs &a, const DatasetDev
      * and splits the batches into NS = 32 / PL contiguous sub-streams */
     /* FULL: more than 16 points, so every lane walks all batches; lanes past the last point shadow point
      * 32 g and never flush */
-    int my0 = 0, mine = nb, iters = nb;
+    int my0 = 0, mine = nb, iters = nb, lg = 5;
     bool active = 32 * g + lane < a.P;
     int p = 32 * g + (active ? lane : 0);
     if (!FULL) {
         const int np = min(32, a.P - 32 * g);
         int PL = 1;
-        while (PL < np) PL <<= 1;
+        lg = 0;
+        while (PL < np) { PL <<= 1; ++lg; }
         const int NS = 32 / PL;
         const int pl = lane & (PL - 1), s = lane / PL;
         active = pl < np;
@@ -451,7 +508,8 @@ __device__ __forceinline__ void walk_unit(const SpectraArgs &a, const DatasetDev
             walk_batch<S>(a, ds, bp, h, thr, safe, p, active, r);
         }
     }
-    flush_run<S>(a, ds, p, active, r);
+    if (FULL) flush_run<S>(a, ds, p, active, r);
+    else      flush_run_substreams<S>(a, ds, p, active, lg, lane, r);
 }
 
 /* lane 0 takes the next ticket of the work counter; the value is needed one item later */
