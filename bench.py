@@ -378,6 +378,11 @@ def main():
         }
         if cached is not None:
             line["cached"] = cached
+        if wl.n_events * P <= 10_000_000:
+            # launch-latency-bound workload (config 1): one host call against the empty-kernel floor
+            line["latency"] = {"host_call_us": e2e_s / args.steps * 1e6, "device_step_us": ms_per_step * 1e3,
+                               "launch_plus_sync_floor_us": ph.launch_floor(200),
+                               "note": "a call is 1 H2D + 3 kernels + 1 D2H + 1 synchronise"}
         if world == 1 and args.config == 2 and not args.no_gradient_step:
             line["gradient_step"] = gradient_step_wall(pkg, torch, local, flush)
         if world == 1 and not args.no_cpu_baseline:

@@ -265,6 +265,12 @@ PHYLINO_API const char *phylino_last_error(const phylino_ctx *ctx);
  * returns the achieved fp64 FMA instructions per second (lane-operations/s) in *dfma_per_s. */
 PHYLINO_API phylino_status phylino_peak_fp64(phylino_ctx *ctx, int iters, double *dfma_per_s_host);
 
+/* Microbenchmark: host wall time, in microseconds per repetition (HOST pointer), of launching an empty
+ * kernel on the context's stream and synchronising it -- the floor under any call whose result the host
+ * waits for.  Launch-latency-bound workloads (one parameter point over a small event store) are reported
+ * against it. */
+PHYLINO_API phylino_status phylino_launch_floor(phylino_ctx *ctx, int reps, double *us_per_call_host);
+
 #ifdef __cplusplus
 }
 #endif

@@ -23,6 +23,7 @@ abi_symbols = (
     "phylino_expectation", "phylino_set_timing", "phylino_last_kernel_ms",
     "phylino_set_caching", "phylino_last_plan", "phylino_set_prior_blocks",
     "phylino_nll_ensemble", "phylino_set_transform", "phylino_param_width",
+    "phylino_launch_floor",
 )
 
 _STATUS = {0: "OK", 1: "ERR_ARG", 2: "ERR_SHAPE", 3: "ERR_STATE", 4: "ERR_OOM", 5: "ERR_CUDA"}
@@ -124,6 +125,8 @@ def load_library():
     lib.phylino_launch_count.argtypes = [vp]
     lib.phylino_last_error.restype = C.c_char_p
     lib.phylino_last_error.argtypes = [vp]
+    lib.phylino_launch_floor.restype = i32
+    lib.phylino_launch_floor.argtypes = [vp, i32, C.POINTER(dbl)]
     lib.phylino_peak_fp64.restype = i32
     lib.phylino_peak_fp64.argtypes = [vp, i32, C.POINTER(dbl)]
     _lib = lib
@@ -402,6 +405,12 @@ class Phylino:
             out = np.empty((p.shape[0], self.total_bins), dtype=np.float64)
         self._check(self._lib.phylino_spectra_host(self._ctx, int(p.shape[0]), p.ctypes.data, out.ctypes.data))
         return out
+
+    def launch_floor(self, reps: int = 200) -> float:
+        """microseconds per (empty-kernel launch + stream synchronise) on this context's stream."""
+        v = C.c_double(0.0)
+        self._check(self._lib.phylino_launch_floor(self._ctx, int(reps), C.byref(v)))
+        return float(v.value)
 
     def peak_fp64(self, iters: int = 4096) -> float:
         v = C.c_double(0.0)

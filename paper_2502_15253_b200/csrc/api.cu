@@ -1090,6 +1090,16 @@ int64_t phylino_launch_count(const phylino_ctx *ctx) { return ctx ? ctx->launche
 
 const char *phylino_last_error(const phylino_ctx *ctx) { return ctx ? ctx->err.c_str() : ""; }
 
+phylino_status phylino_launch_floor(phylino_ctx *ctx, int reps, double *us_per_call_host)
+{
+    if (!ctx || !us_per_call_host || reps < 1) return PHYLINO_ERR_ARG;
+    DeviceGuard g(ctx->device);
+    CU(cudaStreamSynchronize(ctx->stream));
+    CU(run_launch_floor(reps, ctx->stream, us_per_call_host));
+    ctx->launches += reps + 1;
+    return PHYLINO_OK;
+}
+
 phylino_status phylino_peak_fp64(phylino_ctx *ctx, int iters, double *dfma_per_s_host)
 {
     if (!ctx || !dfma_per_s_host || iters < 1) return PHYLINO_ERR_ARG;

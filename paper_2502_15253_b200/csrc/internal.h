@@ -160,6 +160,7 @@ cudaError_t launch_ensemble(const FinalizeArgs &a, int E, cudaStream_t st);
 cudaError_t launch_event_bins(const SpectraArgs &a, int d, const int32_t *perm, long long n, long long ev_off,
                               long long total_events, int32_t *bins, cudaStream_t st);
 cudaError_t run_peak_fp64(int iters, cudaStream_t st, double *dfma_per_s);
+cudaError_t run_launch_floor(int reps, cudaStream_t st, double *us_per_call);
 
 } // namespace phylino
 

@@ -3,6 +3,8 @@
  * the whole chip (the hot loop is ~90 % DFMA/DADD/DMUL, all of which go
  * through the same 64-lane/clk/SM fp64 pipe).  Reported next to the nominal figure by bench.py.
  */
+#include <time.h>
+
 #include "internal.h"
 
 namespace phylino {
@@ -30,7 +32,29 @@ __global__ void __launch_bounds__(256) dfma_kernel(int iters, double seed, doubl
     if (s == 123.456) sink[0] = s;               /* never true; keeps the chains alive */
 }
 
+__global__ void empty_kernel() {}
+
 } // namespace
+
+/* Host wall time of `reps` x (launch of an empty kernel + stream synchronise), in microseconds per
+ * repetition: the floor under any single call whose result the host waits for (config 1 is
+ * reported against it, not against HBM). */
+cudaError_t run_launch_floor(int reps, cudaStream_t st, double *us_per_call)
+{
+    empty_kernel<<<1, 32, 0, st>>>();
+    cudaError_t e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) return e;
+    timespec t0, t1;
+    clock_gettime(CLOCK_MONOTONIC, &t0);
+    for (int i = 0; i < reps; ++i) {
+        empty_kernel<<<1, 32, 0, st>>>();
+        e = cudaStreamSynchronize(st);
+        if (e != cudaSuccess) return e;
+    }
+    clock_gettime(CLOCK_MONOTONIC, &t1);
+    *us_per_call = ((double)(t1.tv_sec - t0.tv_sec) * 1e6 + (double)(t1.tv_nsec - t0.tv_nsec) * 1e-3) / reps;
+    return cudaGetLastError();
+}
 
 cudaError_t run_peak_fp64(int iters, cudaStream_t st, double *dfma_per_s)
 {

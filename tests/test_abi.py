@@ -66,6 +66,7 @@ def test_null_context_is_rejected(phylino_lib):
     assert lib.phylino_last_error(None) == b""
     assert lib.phylino_set_tuning(None, 512, 0, 0) == 1               # PHYLINO_ERR_ARG
     assert lib.phylino_set_caching(None, 1) == 1
+    assert lib.phylino_launch_floor(None, 1, None) == 1
     assert lib.phylino_set_transform(None, 0, None, None, 0, None) == 1
     assert lib.phylino_param_width(None) == 0
     assert lib.phylino_nll_ensemble(None, 1, None, 1, None, None) == 1
