@@ -420,8 +420,9 @@ __device__ __forceinline__ void walk_inside(const EventBatch *bp, const double (
                 for (int k = 0; k < S; ++k) r.C[k] = fma(w.y, half_cos_halfturns(h[k], t.y), r.C[k]);
             }
         }
-        r.W += UW ? (double)EB : bp[u].wsum;
+        if (!UW) r.W += bp[u].wsum;
     }
+    if (UW) r.W += (double)(EB * K);                /* whole numbers: the same bits as K separate adds */
 }
 
 /* One warp, the nb batches of one unit of dataset ds staged at `unit` (SHARED memory), point group g
