@@ -224,7 +224,8 @@ PHYLINO_API int64_t phylino_param_width(const phylino_ctx *ctx);
 PHYLINO_API int64_t phylino_total_bins(const phylino_ctx *ctx);     /* sum_d n_bins, 0 before set_model */
 PHYLINO_API int64_t phylino_total_events(const phylino_ctx *ctx);   /* sum_d n over loaded datasets */
 
-/* Tuning knobs (0 => library default).  unit_events: events per unit of the event store;
+/* Tuning knobs (0 => library default).  unit_events: events per unit of the event store (a unit is staged in
+ * shared memory: values above 256 are clamped to 256; the last stretch of the store is always cut finer);
  * chunk_groups: groups of 32 parameter points per work item (a warp of the spectra kernel walks one
  * unit for every group of an item, then claims the next item); max_warps: cap on the warps of the
  * persistent grid.  Results are bit-identical from call to call for fixed knobs; other values
