@@ -242,8 +242,10 @@ PHYLINO_API phylino_status phylino_set_tuning(phylino_ctx *ctx, int unit_events,
  * rates share all of the event work: a 603-point central-difference batch of a 301-parameter fit needs 21
  * virtual points.  Results agree with the dense path to rounding (within the same per-bin and NLL tolerances) and
  * are bitwise reproducible; a cell that left the fixed-point domain reads NaN (the dense path tells +-inf
- * apart).  If the batch does not shrink to at most half, the dense path runs.  Off by default; the
- * DEVICE-pointer entry points are always dense.  phylino_last_plan: virtual points and energy-scale classes
+ * apart).  If the batch does not shrink to at most half, the dense path runs.  Off by default.  With caching
+ * on, phylino_spectra and phylino_nll (DEVICE pointers) use it too, at the price of ONE device-to-host copy of the
+ * batch and ONE stream synchronisation per call (the plan is made on the host) -- the "never synchronise" rule
+ * above holds only with caching off; phylino_expectation, phylino_nll_ensemble and phylino_event_bins are always dense.  phylino_last_plan: virtual points and energy-scale classes
  * of the last host call that used the cache (0, 0 if it ran dense). */
 PHYLINO_API phylino_status phylino_set_caching(phylino_ctx *ctx, int on);
 PHYLINO_API phylino_status phylino_last_plan(const phylino_ctx *ctx, int64_t *virtual_points, int64_t *classes);

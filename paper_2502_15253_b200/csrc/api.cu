@@ -551,6 +551,20 @@ phylino_status enqueue_cached(phylino_ctx *ctx, int P, const double *h_params, c
     return PHYLINO_OK;
 }
 
+/* Caching for a DEVICE-resident batch: the plan is made on the host, so theta comes back once (one
+ * device -> host copy of the batch and one stream synchronisation per call -- the price stated in phylino.h). */
+phylino_status cached_from_device(phylino_ctx *ctx, int P, const double *d_theta, const double *d_data,
+                                  double *d_hist, double *d_nll, bool *used)
+{
+    *used = false;
+    const int64_t np = (int64_t)P * ctx->n_params;
+    phylino_status s;
+    if ((s = ensure_stage(ctx, np)) != PHYLINO_OK) return s;
+    CU(cudaMemcpyAsync(ctx->h_pin, d_theta, np * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    return enqueue_cached(ctx, P, ctx->h_pin, d_theta, d_data, d_hist, d_nll, used);
+}
+
 } // namespace
 
 extern "C" {
@@ -786,6 +800,12 @@ phylino_status phylino_spectra(phylino_ctx *ctx, int P, const double *params, do
     if (s != PHYLINO_OK || P == 0) return s;
     DeviceGuard g(ctx->device);
     if ((s = resolve_params(ctx, P, params, &params)) != PHYLINO_OK) return s;
+    if (ctx->caching) {
+        bool cached = false;
+        if ((s = cached_from_device(ctx, P, params, nullptr, hist, nullptr, &cached)) != PHYLINO_OK || cached) return s;
+    } else {
+        ctx->last_virtual_points = ctx->last_classes = 0;
+    }
     if ((s = ensure_acc(ctx, P)) != PHYLINO_OK) return s;
     if ((s = enqueue_spectra(ctx, P, params)) != PHYLINO_OK) return s;
     return enqueue_finalize(ctx, P, params, nullptr, hist, nullptr);
@@ -798,6 +818,12 @@ phylino_status phylino_nll(phylino_ctx *ctx, int P, const double *params, const 
     if (!data) return fail(ctx, PHYLINO_ERR_ARG, "NULL data pointer");
     DeviceGuard g(ctx->device);
     if ((s = resolve_params(ctx, P, params, &params)) != PHYLINO_OK) return s;
+    if (ctx->caching) {
+        bool cached = false;
+        if ((s = cached_from_device(ctx, P, params, data, nullptr, nll, &cached)) != PHYLINO_OK || cached) return s;
+    } else {
+        ctx->last_virtual_points = ctx->last_classes = 0;
+    }
     if ((s = ensure_acc(ctx, P)) != PHYLINO_OK) return s;
     if ((s = enqueue_spectra(ctx, P, params)) != PHYLINO_OK) return s;
     return enqueue_finalize(ctx, P, params, data, nullptr, nll);

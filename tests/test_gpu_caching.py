@@ -113,3 +113,28 @@ def test_unphysical_point_in_cached_batch(gpu, oracle_mod):
     assert np.isnan(nll[7]) and np.isnan(nll_o[7])
     keep = np.arange(256) != 7
     assert np.abs(nll[keep] - nll_o[keep]).max() <= ABS_NLL
+
+
+def test_device_pointer_entry_points_use_the_cache_when_asked(gpu, oracle_mod):
+    """phylino_nll / phylino_spectra on DEVICE batches with caching on: same plan, same bits as the host calls."""
+    import torch
+    wl = workloads.make_config(3, scale=0.004)
+    orc = oracle_mod.Oracle(wl.model, wl.events)
+    data = _data(orc, wl)
+    with gpu.Phylino() as ph:
+        ph.load_workload(wl)
+        dp = torch.as_tensor(wl.params, device="cuda")
+        dense = ph.nll(dp, torch.as_tensor(data, device="cuda")).cpu().numpy()
+        assert ph.last_plan() == (0, 0)
+        ph.set_caching(True)
+        nll_d = ph.nll(dp, torch.as_tensor(data, device="cuda")).cpu().numpy()
+        plan = ph.last_plan()
+        h_d = ph.spectra(dp).cpu().numpy()
+        nll_h = ph.nll_host(wl.params, data)
+        h_h = ph.spectra_host(wl.params)
+        ph.set_caching(False)
+        again = ph.nll(dp, torch.as_tensor(data, device="cuda")).cpu().numpy()
+    assert plan == (21, 19)
+    assert np.array_equal(nll_d, nll_h) and np.array_equal(h_d, h_h)
+    assert np.abs(nll_d - orc.nll(wl.params, data)).max() <= ABS_NLL
+    assert np.array_equal(dense, again)                    # the dense path is untouched by a cached call in between
