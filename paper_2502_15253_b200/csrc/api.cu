@@ -307,7 +307,8 @@ phylino_status ensure_stage(phylino_ctx *ctx, int64_t doubles)
     if (ctx->h_pin) cudaFreeHost(ctx->h_pin);
     ctx->h_pin = nullptr; ctx->stage_capacity = 0;
     CU(cudaMalloc((void **)&ctx->d_stage, doubles * sizeof(double)));
-    CU(cudaHostAlloc((void **)&ctx->h_pin, doubles * sizeof(double), cudaHostAllocDefault));
+    CU(cudaHostAlloc((void **)&ctx->h_pin, doubles * sizeof(double), cudaHostAllocMapped));
+    CU(cudaHostGetDevicePointer((void **)&ctx->d_pin, ctx->h_pin, 0));      /* the kernels' view of the pinned block */
     ctx->stage_capacity = doubles;
     return PHYLINO_OK;
 }
@@ -907,15 +908,16 @@ phylino_status phylino_nll_host(phylino_ctx *ctx, int P, const double *params_ho
     else std::memcpy(ctx->h_pin, params_host, np * sizeof(double));
     std::memcpy(ctx->h_pin + np, data_host, tb * sizeof(double));
     CU(cudaMemcpyAsync(ctx->d_stage, ctx->h_pin, (np + tb) * sizeof(double), cudaMemcpyHostToDevice, ctx->stream));
+    /* the finalize kernel writes nll[P] straight into the pinned block (8 P bytes over PCIe): no copy back */
+    double *d_out = ctx->d_pin + np + tb;
     bool cached = false;
     if (ctx->caching &&
-        (s = enqueue_cached(ctx, P, ctx->h_pin, ctx->d_stage, ctx->d_stage + np, nullptr, ctx->d_stage + np + tb, &cached)) != PHYLINO_OK)
+        (s = enqueue_cached(ctx, P, ctx->h_pin, ctx->d_stage, ctx->d_stage + np, nullptr, d_out, &cached)) != PHYLINO_OK)
         return s;
     if (!cached) {
         if ((s = enqueue_spectra(ctx, P, ctx->d_stage)) != PHYLINO_OK) return s;
-        if ((s = enqueue_finalize(ctx, P, ctx->d_stage, ctx->d_stage + np, nullptr, ctx->d_stage + np + tb)) != PHYLINO_OK) return s;
+        if ((s = enqueue_finalize(ctx, P, ctx->d_stage, ctx->d_stage + np, nullptr, d_out)) != PHYLINO_OK) return s;
     }
-    CU(cudaMemcpyAsync(ctx->h_pin + np + tb, ctx->d_stage + np + tb, P * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
     CU(cudaStreamSynchronize(ctx->stream));
     std::memcpy(nll_host, ctx->h_pin + np + tb, P * sizeof(double));
     return PHYLINO_OK;

@@ -226,7 +226,7 @@ struct phylino_ctx {
     double *d_mu = nullptr;                        /* [mu_capacity] expectations of an ensemble call */
     int64_t mu_capacity = 0;
     /* host-buffer entry points: pinned + device staging */
-    double *h_pin = nullptr, *d_stage = nullptr;
+    double *h_pin = nullptr, *d_stage = nullptr, *d_pin = nullptr;   /* d_pin: device alias of h_pin */
     int64_t stage_capacity = 0;                    /* doubles */
     unsigned *d_counter = nullptr;                 /* work counter of the spectra kernel */
     /* tuning knobs, 0 => default (phylino_set_tuning) */
