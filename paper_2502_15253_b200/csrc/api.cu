@@ -257,6 +257,18 @@ void fill_batch(const phylino_ctx *ctx, SpectraArgs &a, int P, const double *par
     a.n_items = (int32_t)(units * chunks);
     const int64_t warps = std::min<int64_t>(cap, (a.n_items + WARPS - 1) / WARPS * WARPS);
     a.n_warps = (int32_t)std::max<int64_t>(warps, WARPS);
+    /* batches of at most 16 points (the minimiser's single evaluations) are bound by per-item latency chains,
+     * not by arithmetic: they take the static schedule -- one contiguous range of at least one unit per warp,
+     * runs carried across its units (spectra.cu, spectra_static_kernel).  Measured on 6e6 events: 1 / 4 / 16
+     * points 0.098 / 0.123 / 0.204 ms -> 0.062 / 0.082 / 0.178 ms (two-term models); on config 4's store (three
+     * terms, 410 bins) 1 / 2 points 0.142 / 0.143 -> 0.084 / 0.114 ms, even at 4, slower from 8.  Larger batches
+     * are faster with the tickets (config 2: 0.21 ms against 0.29 ms static). */
+    a.sched = P <= (ctx->n_terms == 2 ? 16 : 4) ? 1 : 0;
+    if (a.sched == 1) {
+        a.unit_batches = (int32_t)MAX_UNIT_BATCHES;
+        const int64_t want = (batches + MAX_UNIT_BATCHES - 1) / MAX_UNIT_BATCHES;
+        a.n_warps = (int32_t)std::max<int64_t>(WARPS, std::min<int64_t>(cap, (want + WARPS - 1) / WARPS * WARPS));
+    }
 }
 
 /* enqueue the setup and spectra kernels (rows a1-a4) for P points */

@@ -83,6 +83,7 @@ struct SpectraArgs {
     int32_t tail_b0;        /* its first batch inside the last dataset */
     int32_t tail_batches;   /* batches per unit of the fine tail */
     int32_t n_warps;        /* warps of the persistent grid (a multiple of WARPS) */
+    int32_t sched;          /* 0: items claimed from the counter; 1: one contiguous range of batches per warp */
     unsigned *counter;      /* DEVICE work counter; the setup kernel sets it to 2 n_warps */
     int32_t thr_stride;     /* floats per threshold row: total_bins + n_datasets */
     int32_t thr_rows;       /* P if some dataset's energy scale depends on theta, else 1 */

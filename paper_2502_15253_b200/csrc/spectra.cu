@@ -513,6 +513,179 @@ __device__ __forceinline__ void walk_unit(const SpectraArgs &a, const DatasetDev
     else      flush_run_substreams<S>(a, ds, p, active, lg, lane, r);
 }
 
+/* ---- static schedule: ONE contiguous range of batches per warp, runs carried across units ------------
+ * A run is "the events of one bin at one point", not "adjacent events": a lane may keep its run open
+ * across consecutive units (its events stay sorted), so a warp that owns a contiguous range pays the
+ * group prologue and the flush once per (range, group) instead of once per (unit, group), and there is
+ * no ticket, no tail of unequal items: every warp holds the same number of batches.  The units of the
+ * range stream through the warp's two buffers; the copy of the next unit (of this range, or the first
+ * unit of what the warp walks next) is in flight while a unit is walked. */
+struct Pipe {
+    EventBatch *buf0;               /* the warp's two unit buffers */
+    unsigned long long *bars;       /* its two mbarriers */
+    int b;                          /* buffer that holds (or will hold) the unit walked next */
+    unsigned phase;
+};
+
+/* one segment [B0, B1) of dataset d for point group g; (nd, n0, n1): the unit to copy when the last unit of
+ * this segment is being walked (n0 < 0: nothing follows) */
+template <int S, bool FULL, bool UW>
+__device__ __forceinline__ void walk_range(const SpectraArgs &a, int d, int B0, int B1, int g, int lane, Pipe &pp,
+                                           int nd, int n0, int n1)
+{
+    const DatasetDev &ds = a.ds[d];
+    int lg = 5;
+    bool active = 32 * g + lane < a.P;
+    int p = 32 * g + (active ? lane : 0), s = 0;
+    if (!FULL) {
+        const int np = min(32, a.P - 32 * g);
+        lg = np <= 1 ? 0 : 32 - __clz(np - 1);
+        const int pl = lane & ((1 << lg) - 1);
+        s = lane >> lg;
+        active = pl < np;
+        p = 32 * g + (active ? pl : 0);
+    }
+    double h[S];
+#pragma unroll
+    for (int k = 0; k < S; ++k) h[k] = a.rec[(size_t)k * a.P + p];
+    const int row = row_of(a, p);
+    const float *thr = a.thr + (size_t)row * a.thr_stride + ds.thr_off;
+    const float2 safe = a.safe[(size_t)row * a.n_datasets + d];
+    const int B = ds.n_bins, U = a.unit_batches;
+
+    Run<S> r;
+#pragma unroll
+    for (int k = 0; k < S; ++k) r.C[k] = 0.0;
+    r.W = 0.0;
+    r.cur = -1;
+    r.hi = -pos_inf();
+    r.hi2 = pos_inf();
+
+#pragma unroll 1
+    for (int off = B0; off < B1; off += U) {
+        const int nb = min(U, B1 - off);
+        if (lane == 0) {
+            /* the other buffer was last read one unit ago (every lane has passed the __syncwarp below) */
+            int cd = d, c0 = off + U, c1 = min(off + 2 * U, B1);
+            if (c0 >= B1) { cd = nd; c0 = n0; c1 = n1; }
+            if (c0 >= 0)
+                bulk_load(pp.buf0 + (pp.b ^ 1) * U, a.ds[cd].ev + c0, (unsigned)(c1 - c0) * (unsigned)sizeof(EventBatch),
+                          pp.bars + (pp.b ^ 1));
+        }
+        mbar_wait(pp.bars + pp.b, (pp.phase >> pp.b) & 1u);
+        pp.phase ^= 1u << pp.b;
+        int my0 = 0, mine = nb;
+        if (!FULL) {
+            my0 = (nb * s) >> (5 - lg);
+            mine = ((nb * (s + 1)) >> (5 - lg)) - my0;
+        }
+        const EventBatch *bp = pp.buf0 + pp.b * U + my0;
+        if (off == B0 && mine > 0) {
+            /* open the run at the lane's first event from the load-time hint (see walk_unit) */
+            const float v0 = bp->v[0];
+            if (v0 >= safe.x && v0 <= safe.y) {
+                int bb = max(-1, min(bp->bin0, B));
+                float lo = thr_at(thr, B, bb), hi = thr_at(thr, B, bb + 1);
+                while (bb >= 0 && v0 < lo) { --bb; hi = lo; lo = thr_at(thr, B, bb); }
+                while (bb < B && !(v0 < hi)) { ++bb; hi = thr_at(thr, B, bb + 1); }
+                r.cur = bb;
+                r.hi = hi;
+                r.hi2 = thr_at(thr, B, bb + 2);
+            }
+        }
+        int i = 0;
+#pragma unroll 1
+        while (i < mine) {
+            if (i + 4 <= mine && bp[3].v[EB - 1] < r.hi) {
+                walk_inside<S, UW, 4>(bp, h, r);
+                i += 4;
+                bp += 4;
+            } else if (i + 2 <= mine && bp[1].v[EB - 1] < r.hi) {
+                walk_inside<S, UW, 2>(bp, h, r);
+                i += 2;
+                bp += 2;
+            } else {
+                walk_batch<S>(a, ds, bp, h, thr, safe, p, active, r);
+                ++i;
+                ++bp;
+            }
+        }
+        __syncwarp();                                   /* this unit's reads are over before its buffer is refilled */
+        pp.b ^= 1;
+    }
+    if (FULL) flush_run<S>(a, ds, p, active, r);
+    else      flush_run_substreams<S>(a, ds, p, active, lg, lane, r);
+}
+
+/* first (dataset, segment) at or after dataset d0 that the global batch range [G0, G1) touches */
+__device__ __forceinline__ bool next_segment(const SpectraArgs &a, long long G0, long long G1, int d0, int &d, int &B0,
+                                             int &B1)
+{
+    long long off = 0;
+    for (int i = 0; i < a.n_datasets; ++i) {
+        const long long nb = a.ds[i].n_batches;
+        if (i >= d0) {
+            const long long lo = max(G0, off), hi = min(G1, off + nb);
+            if (lo < hi) { d = i; B0 = (int)(lo - off); B1 = (int)(hi - off); return true; }
+        }
+        off += nb;
+    }
+    return false;
+}
+
+template <int S>
+__global__ void __launch_bounds__(WARPS * 32, 4) spectra_static_kernel(const __grid_constant__ SpectraArgs a)
+{
+    extern __shared__ __align__(128) unsigned char stage[];       /* [WARPS][2][unit_batches] EventBatch */
+    __shared__ unsigned long long bars[WARPS][2];
+    const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+    const long long nW = (long long)gridDim.x * WARPS, w = (long long)blockIdx.x * WARPS + wib;
+    const int n_groups = (a.P + 31) >> 5, U = a.unit_batches;
+    long long total = 0;
+    for (int i = 0; i < a.n_datasets; ++i) total += a.ds[i].n_batches;
+    const long long G0 = total * w / nW, G1 = total * (w + 1) / nW;       /* this warp's batches, all datasets */
+    Pipe pp;
+    pp.buf0 = reinterpret_cast<EventBatch *>(stage) + (size_t)(2 * wib) * U;
+    pp.bars = &bars[wib][0];
+    pp.b = 0;
+    pp.phase = 0u;
+    if (lane == 0) {
+        mbar_init(&bars[wib][0], 1);
+        mbar_init(&bars[wib][1], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncwarp();
+    int fd, f0, f1;
+    const bool any = next_segment(a, G0, G1, 0, fd, f0, f1);
+    if (any && lane == 0)
+        bulk_load(pp.buf0, a.ds[fd].ev + f0, (unsigned)(min(f0 + U, f1) - f0) * (unsigned)sizeof(EventBatch), pp.bars);
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    if (!any) return;
+#pragma unroll 1
+    for (int g = 0; g < n_groups; ++g) {
+        int d, B0, B1;
+        bool more = next_segment(a, G0, G1, 0, d, B0, B1);
+#pragma unroll 1
+        while (more) {
+            /* what follows this segment: the next dataset's segment, else the first segment again for the
+             * next group, else nothing */
+            int nd, n0, n1, e1;
+            const bool nxt = next_segment(a, G0, G1, d + 1, nd, n0, e1);
+            if (!nxt) {
+                if (g + 1 < n_groups) { nd = fd; n0 = f0; e1 = f1; } else { nd = 0; n0 = -1; e1 = -1; }
+            }
+            n1 = n0 < 0 ? -1 : min(n0 + U, e1);
+            const DatasetDev &ds = a.ds[d];
+            if (32 * g + 16 >= a.P) walk_range<S, false, false>(a, d, B0, B1, g, lane, pp, nd, n0, n1);
+            else if (ds.unit_w)    walk_range<S, true, true>(a, d, B0, B1, g, lane, pp, nd, n0, n1);
+            else                   walk_range<S, true, false>(a, d, B0, B1, g, lane, pp, nd, n0, n1);
+            more = nxt;
+            if (nxt) { d = nd; B0 = n0; B1 = e1; }
+        }
+    }
+}
+
 /* lane 0 takes the next ticket of the work counter; the value is needed one item later */
 __device__ __forceinline__ unsigned take_ticket(unsigned *counter, int lane)
 {
@@ -618,6 +791,7 @@ template <int S> cudaError_t launch_t(const SpectraArgs &a, cudaStream_t st, boo
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr;
     cfg.numAttrs = pdl ? 1 : 0;
+    if (a.sched == 1) return cudaLaunchKernelEx(&cfg, spectra_static_kernel<S>, a);
     return cudaLaunchKernelEx(&cfg, spectra_kernel<S>, a);
 }
 
@@ -626,6 +800,8 @@ template <int S> cudaError_t max_warps_t(int sm_count, int *warps)
     int per_sm = 0;
     cudaError_t e = cudaFuncSetAttribute(spectra_kernel<S>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          (int)STAGE_BYTES);
+    if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(spectra_static_kernel<S>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)STAGE_BYTES);
     if (e != cudaSuccess) return e;
     e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, spectra_kernel<S>, WARPS * 32, STAGE_BYTES);
     if (e != cudaSuccess) return e;
