@@ -29,3 +29,27 @@ def test_reference_arm_other_ranks_stay_silent(oracle_mod):
                           "--steps", "1", "--warmup", "0", "--gpus", "2"], capture_output=True, text=True, cwd=ROOT,
                          env=env, timeout=600)
     assert out.returncode == 0 and out.stdout.strip() == ""
+
+
+import pytest  # noqa: E402
+
+
+@pytest.mark.gpu
+def test_own_arm_line_has_roofline_cpu_baseline_and_e2e(gpu, oracle_mod):
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--steps", "3", "--warmup", "3",
+                          "--no-gradient-step"], capture_output=True, text=True, cwd=ROOT, timeout=900)
+    assert out.returncode == 0, out.stderr[-2000:]
+    lines = [l for l in out.stdout.splitlines() if l.strip()]
+    assert len(lines) == 1
+    j = json.loads(lines[0])
+    assert "impl" not in j and j["n_gpus"] == 1 and j["steps"] == 3 and j["scaling"] == "weak" and j["dtype"] == "f64"
+    assert "configs[1]" in j["config"]["workload"] and "l2" in j["config"]
+    assert j["gpu_launches"] == 9                                   # setup, spectra, finalize per timed step
+    r = j["roofline"]
+    assert r["bound"] == "alu" and r["unit"] and 0.3 < r["frac"] < 1.05 and abs(r["frac"] - r["achieved"] / r["peak"]) < 1e-9
+    assert r["traffic"] is None or r["traffic"] > 24 * j["config"]["events"] * 0.9
+    cb = j["cpu_baseline"]
+    assert cb["kind"] == "oracle" and cb["cores"] >= 1 and cb["value"] > 0 and cb["max_abs_nll_diff_vs_gpu"] <= 1e-6
+    e = j["e2e"]
+    assert 0 < e["value"] <= j["value"] * 1.05 and e["h2d_bytes_per_step"] > 0 and e["d2h_bytes_per_step"] > 0
+    assert "sm_mhz" in j["clocks"] and "reasons" in j["clocks"]
