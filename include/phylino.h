@@ -23,14 +23,22 @@
  *               phylino_load_events and owns all device memory it allocates.  The caller owns
  *               `params`, `data` and the outputs; they must stay alive until the stream has
  *               passed the call.
- *   Async     : phylino_spectra / phylino_nll / phylino_event_bins only enqueue work on the
- *               context's stream and return; they never synchronise and never touch host-visible
- *               output.  phylino_load_events / phylino_set_model synchronise the stream.
+ *   Async     : phylino_spectra / phylino_nll / phylino_expectation / phylino_nll_ensemble /
+ *               phylino_event_bins only enqueue work on the context's stream and return; they
+ *               never touch host-visible output, and they synchronise the stream in ONE case only:
+ *               when a batch is larger than any before it on this context, the per-point work
+ *               buffers grow (stream synchronise + cudaMalloc).  phylino_reserve(ctx, max_points)
+ *               sizes them once, after which these calls never synchronise (required before the
+ *               stream is captured into a CUDA graph).  phylino_load_events / phylino_set_model /
+ *               phylino_set_transform / phylino_set_prior_blocks synchronise the stream.
  *   Errors    : every entry point returns a phylino_status; nothing throws across the ABI.
  *               Shape / state problems are detected on the host before any launch.  The text of
  *               the last error of a context is kept in phylino_last_error().  VALUE problems in
- *               device-resident `params` (NaN, sin^2 2theta outside [0,1]) are not errors: they
- *               propagate as NaN into that point's outputs, as sqrt of a negative does.
+ *               device-resident `params` (NaN, sin^2 2theta above 1) are not errors: they
+ *               propagate as NaN into that point's outputs, as sqrt of a negative does.  One more
+ *               value rule: a point whose oscillation amplitudes have sum_k |A_k| > 3 (reachable only
+ *               with sin^2 2theta far below 0, e.g. -2: cos^4 theta > 2) reads NaN in every bin --
+ *               the 64-bit fixed-point bin accumulators are scaled for |P_ee| <= 4 (R19).
  *   Threads   : one context must not be used from two host threads at once; any number of
  *               contexts may coexist (independent fits).
  *   Determinism: identical inputs give bit-identical outputs on every call (64-bit fixed-point
@@ -154,8 +162,8 @@ PHYLINO_API phylino_status phylino_set_model(phylino_ctx *ctx, const phylino_mod
  *   baseline_m[n_cores] L in metres (finite, >= 0)
  *   edges     [n_bins+1] strictly ascending reco-energy bin edges; n_bins must equal the model's.
  * The store is sorted by reconstructed energy ("sorted according to their energy";
- * R14) and cut into 96-byte records of 4 events: x = L_core/E_nu and w as fp64, E_vis as fp32
- * (DESIGN.md "Event store").
+ * R14) and cut into records of 4 events: x = L_core/E_nu as fp64 and E_vis as fp32 -- 12 bytes per event
+ * when every weight is exactly 1 (or NULL), else 24 with the weights as fp64.
  * n = 0 is allowed (empty dataset).  Reloading a dataset replaces it. */
 PHYLINO_API phylino_status phylino_load_events(phylino_ctx *ctx, int dataset, int64_t n,
                                    const float *e_nu_MeV, const float *e_vis_MeV, const float *weight,
@@ -179,7 +187,10 @@ PHYLINO_API phylino_status phylino_expectation(phylino_ctx *ctx, int P, const do
 
 /* Diagnostic for the bit-exact bin-assignment parity test: bins[p, i] = bin index b (within its
  * dataset) of event i at point p, -1 if E' falls outside [edges[0], edges[n_bins]) or is NaN.
- * i runs over the datasets' events concatenated in the CALLER's original order.
+ * i runs over the datasets' events concatenated in the CALLER's original order.  The call runs the
+ * PRODUCTION kernels of this batch size (same schedule, same work cut as phylino_spectra) in a
+ * diagnostic instantiation that also records, for every event a lane accumulates, the bin the hot
+ * loop put it in; nothing else is written (the accumulators are cleared).
  *   params DEVICE [P x n_params]; bins DEVICE int32 [P x total_events]. */
 PHYLINO_API phylino_status phylino_event_bins(phylino_ctx *ctx, int P, const double *params, int32_t *bins);
 
@@ -223,6 +234,19 @@ PHYLINO_API int64_t phylino_param_width(const phylino_ctx *ctx);
 /* Sizes the caller needs for its buffers. */
 PHYLINO_API int64_t phylino_total_bins(const phylino_ctx *ctx);     /* sum_d n_bins, 0 before set_model */
 PHYLINO_API int64_t phylino_total_events(const phylino_ctx *ctx);   /* sum_d n over loaded datasets */
+
+/* Pre-size every per-batch work buffer of the context for batches of up to max_points points (accumulators,
+ * per-point records and bin thresholds, pinned staging of the HOST entry points, the transformed batch).  After
+ * it, calls with P <= max_points allocate nothing and the DEVICE entry points never synchronise.  Synchronises
+ * the stream if anything grows.  PHYLINO_ERR_STATE before the model and all events are loaded. */
+PHYLINO_API phylino_status phylino_reserve(phylino_ctx *ctx, int max_points);
+
+/* Which kernels evaluate a batch: 0 (default) the library chooses -- ONE launch of the single-launch kernel for
+ * small batches (at most 16 points with two oscillation terms, 4 with three: the minimiser's single evaluations;
+ * setup, event walk and likelihood in one kernel), else the setup / spectra / finalize kernels with the work-item
+ * tickets; 1 always the three kernels; 2 the single launch for every batch of at most 16 points.  Results agree
+ * to rounding (another grouping of the fp64 partial sums); for tests and measurements. */
+PHYLINO_API phylino_status phylino_set_schedule(phylino_ctx *ctx, int mode);
 
 /* Tuning knobs (0 => library default).  unit_events: events per unit of the event store (a unit is staged in
  * shared memory: values above 256 are clamped to 256; the last stretch of the store is always cut finer);

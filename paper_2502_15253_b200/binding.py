@@ -23,7 +23,7 @@ abi_symbols = (
     "phylino_expectation", "phylino_set_timing", "phylino_last_kernel_ms",
     "phylino_set_caching", "phylino_last_plan", "phylino_set_prior_blocks",
     "phylino_nll_ensemble", "phylino_set_transform", "phylino_param_width",
-    "phylino_launch_floor",
+    "phylino_launch_floor", "phylino_set_schedule", "phylino_reserve",
 )
 
 _STATUS = {0: "OK", 1: "ERR_ARG", 2: "ERR_SHAPE", 3: "ERR_STATE", 4: "ERR_OOM", 5: "ERR_CUDA"}
@@ -121,6 +121,10 @@ def load_library():
     lib.phylino_last_plan.argtypes = [vp, C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
     lib.phylino_set_tuning.restype = i32
     lib.phylino_set_tuning.argtypes = [vp, i32, i32, i32]
+    lib.phylino_set_schedule.restype = i32
+    lib.phylino_set_schedule.argtypes = [vp, i32]
+    lib.phylino_reserve.restype = i32
+    lib.phylino_reserve.argtypes = [vp, i32]
     lib.phylino_launch_count.restype = i64
     lib.phylino_launch_count.argtypes = [vp]
     lib.phylino_last_error.restype = C.c_char_p
@@ -227,6 +231,7 @@ class Phylino:
         m.prior_sigma = None if model.prior_sigma is None else arr(model.prior_sigma, np.float64)
         self._check(self._lib.phylino_set_model(self._ctx, C.byref(m)))
         self.n_params = int(model.n_params)
+        self._sizes = None
         del keep
 
     # -- phylino_load_events -------------------------------------------------------------------
@@ -254,9 +259,16 @@ class Phylino:
             self.load_events(d, e.e_nu, e.e_vis, e.w, e.core, e.L_m, e.edges)
 
     # -- sizes ---------------------------------------------------------------------------------
+    def _size_cache(self):
+        # (total_bins, param_width): fixed between set_model / set_transform calls; asked once, because a
+        # single-point host call is short enough for two extra library calls to show
+        if getattr(self, "_sizes", None) is None:
+            self._sizes = (int(self._lib.phylino_total_bins(self._ctx)), int(self._lib.phylino_param_width(self._ctx)))
+        return self._sizes
+
     @property
     def total_bins(self) -> int:
-        return int(self._lib.phylino_total_bins(self._ctx))
+        return self._size_cache()[0]
 
     @property
     def total_events(self) -> int:
@@ -268,6 +280,13 @@ class Phylino:
 
     def set_tuning(self, unit_events: int = 0, chunk_groups: int = 0, max_warps: int = 0):
         self._check(self._lib.phylino_set_tuning(self._ctx, int(unit_events), int(chunk_groups), int(max_warps)))
+
+    def set_schedule(self, mode: int = 0):
+        """0 library's choice, 1 always setup/spectra/finalize kernels, 2 single launch for <= 16 points."""
+        self._check(self._lib.phylino_set_schedule(self._ctx, int(mode)))
+
+    def reserve(self, max_points: int):
+        self._check(self._lib.phylino_reserve(self._ctx, int(max_points)))
 
     # -- phylino_spectra / phylino_nll / phylino_event_bins (device buffers, asynchronous) -------
     def spectra(self, params, out=None):
@@ -334,6 +353,7 @@ class Phylino:
 
     def set_transform(self, spec=None):
         """spec: workloads.TransformSpec (n_u, copy_src, copy_const, blocks) or None to remove the layer."""
+        self._sizes = None
         if spec is None:
             self._check(self._lib.phylino_set_transform(self._ctx, 0, None, None, 0, None))
             return
@@ -358,7 +378,7 @@ class Phylino:
 
     @property
     def param_width(self) -> int:
-        return int(self._lib.phylino_param_width(self._ctx))
+        return self._size_cache()[1]
 
     def set_caching(self, on: bool = True):
         self._check(self._lib.phylino_set_caching(self._ctx, int(bool(on))))

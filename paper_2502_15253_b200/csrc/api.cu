@@ -64,8 +64,8 @@ template <class T> cudaError_t upload(T **dst, const std::vector<T> &src, cudaSt
 
 void free_events(phylino_dataset_host &d)
 {
-    cudaFree(d.d_ev); cudaFree(d.d_edges); cudaFree(d.d_perm);
-    d.d_ev = nullptr; d.d_edges = nullptr; d.d_perm = nullptr;
+    cudaFree(d.d_ev); cudaFree(d.d_edges); cudaFree(d.d_perm); cudaFree(d.d_hint);
+    d.d_ev = nullptr; d.d_edges = nullptr; d.d_perm = nullptr; d.d_hint = nullptr;
     d.loaded = false; d.n = d.n_pad = 0;
 }
 
@@ -99,8 +99,9 @@ void free_all(phylino_ctx *c)
     free_tables(c);
     cudaFree(c->d_acc); cudaFree(c->d_flags);
     c->d_acc = nullptr; c->d_flags = nullptr; c->acc_capacity = 0;
-    cudaFree(c->d_rec); cudaFree(c->d_thr); cudaFree(c->d_safe); cudaFree(c->d_counter);
-    c->d_rec = nullptr; c->d_thr = nullptr; c->d_safe = nullptr; c->d_counter = nullptr; c->point_capacity = 0;
+    cudaFree(c->d_rec); cudaFree(c->d_thr); cudaFree(c->d_safe); cudaFree(c->d_counter); cudaFree(c->d_done);
+    c->d_rec = nullptr; c->d_thr = nullptr; c->d_safe = nullptr; c->d_counter = nullptr; c->d_done = nullptr;
+    c->point_capacity = 0;
     cudaFree(c->d_plan); c->d_plan = nullptr; c->plan_capacity = 0;
     cudaFree(c->d_mu); c->d_mu = nullptr; c->mu_capacity = 0;
     free_transform(c);
@@ -108,6 +109,8 @@ void free_all(phylino_ctx *c)
     cudaFree(c->d_stage); c->d_stage = nullptr;
     if (c->h_pin) cudaFreeHost(c->h_pin);
     c->h_pin = nullptr; c->stage_capacity = 0;
+    c->resident_warps = c->fused_warps = 0;     /* occupancy of the kernels of the model's n_terms: asked again */
+    c->fused_tables = 0;
     c->have_model = false;
 }
 
@@ -149,6 +152,10 @@ phylino_status ensure_acc(phylino_ctx *ctx, int P)
         CU(cudaMalloc((void **)&ctx->d_counter, sizeof(unsigned)));
         CU(cudaMemsetAsync(ctx->d_counter, 0, sizeof(unsigned), ctx->stream));
     }
+    if (!ctx->d_done) {
+        CU(cudaMalloc((void **)&ctx->d_done, sizeof(unsigned)));
+        CU(cudaMemsetAsync(ctx->d_done, 0, sizeof(unsigned), ctx->stream));
+    }
     if (P > ctx->point_capacity) {
         /* per-point records and threshold rows written by the setup kernel of every call */
         CU(cudaStreamSynchronize(ctx->stream));
@@ -169,7 +176,9 @@ void fill_datasets(const phylino_ctx *ctx, SpectraArgs &a)
     for (int d = 0; d < ctx->n_datasets; ++d) {
         const phylino_dataset_host &h = ctx->ds[d];
         DatasetDev &v = a.ds[d];
-        v.ev = h.d_ev; v.edges = h.d_edges;
+        v.ev = h.d_ev; v.edges = h.d_edges; v.hint = h.d_hint; v.perm = h.d_perm;
+        v.ev_off = d == 0 ? 0 : a.ds[d - 1].ev_off + a.ds[d - 1].n_events;
+        v.n_events = (int32_t)h.n;
         v.n_bins = h.n_bins;
         v.bin_off = d == 0 ? 0 : a.ds[d - 1].bin_off + a.ds[d - 1].n_bins;
         v.thr_off = v.bin_off + d;
@@ -194,21 +203,86 @@ void fill_datasets(const phylino_ctx *ctx, SpectraArgs &a)
     a.acc = ctx->d_acc;
     a.flags = ctx->d_flags;
     a.counter = ctx->d_counter;
+    a.done = ctx->d_done;
 }
 
 /* Cut of the batch into work items (spectra.cu): U batches per unit, G point groups per item.
  * Aim: at least 12 items per resident warp (dynamic balance, short tail) of at least 16 batch-groups
  * each (the per-item cost -- first bin search, one flush per point -- stays a few percent). */
-void fill_batch(const phylino_ctx *ctx, SpectraArgs &a, int P, const double *params)
+/* small batches (the minimiser's single evaluations) are bound by launch latency and HBM bytes, not by
+ * arithmetic: they take ONE launch of the single-launch kernel (spectra.cu, spectra_fused_kernel).  Measured in
+ * round 1 with the then separate static-range kernel on 6e6 events: 1 / 4 / 16 points 0.098 / 0.123 / 0.204 ms
+ * (tickets) -> 0.062 / 0.082 / 0.178 ms (two-term models); on config 4's store (three terms, 410 bins) 1 / 2 points
+ * 0.142 / 0.143 -> 0.084 / 0.114 ms, even at 4, slower from 8.  Larger batches are faster with the tickets
+ * (config 2: 0.21 ms against 0.29 ms static). */
+bool wants_single_launch(const phylino_ctx *ctx, int P)
 {
+    if (ctx->schedule == 1) return false;
+    if (ctx->schedule == 2) return P <= FUSED_MAX_POINTS;
+    return P <= (ctx->n_terms == 2 ? FUSED_MAX_POINTS : 4);
+}
+
+phylino_status fill_batch(phylino_ctx *ctx, SpectraArgs &a, int P, const double *params, int thr_rows = 0)
+{
+    if (ctx->resident_warps == 0)
+        CU(spectra_max_warps(ctx->n_terms, ctx->sm_count, false, 0, &ctx->resident_warps));
     a.P = P;
     a.params = params;
-    a.thr_rows = ctx->per_point_binning ? P : 1;
+    a.thr_rows = thr_rows > 0 ? thr_rows : (ctx->per_point_binning ? P : 1);
     const int64_t n_groups = (P + 31) / 32;
     int streams = 1;                                    /* sub-streams per warp when P < 32 */
     if (P < 32) { int pl = 1; while (pl < P) pl <<= 1; streams = 32 / pl; }
     int64_t batches = 0;
-    for (int d = 0; d < ctx->n_datasets; ++d) batches += ctx->ds[d].n_pad / EB;
+    bool all_slim = true;
+    for (int d = 0; d < ctx->n_datasets; ++d) {
+        batches += ctx->ds[d].n_pad / EB;
+        all_slim = all_slim && (ctx->ds[d].unit_w || ctx->ds[d].n_pad == 0);
+    }
+    const int last = ctx->n_datasets - 1;
+    const int64_t nb_last = ctx->ds[last].n_pad / EB;
+
+    a.sched = 0;
+    if (wants_single_launch(ctx, P)) {
+        const size_t tables = fused_table_bytes(ctx->n_terms, P, a.thr_rows, a.thr_stride, ctx->n_datasets);
+        if (fused_fits(tables)) {
+            if (ctx->fused_warps == 0 || ctx->fused_tables != tables) {
+                CU(spectra_max_warps(ctx->n_terms, ctx->sm_count, true, tables, &ctx->fused_warps));
+                ctx->fused_tables = tables;
+            }
+            a.sched = 1;
+        }
+    }
+    if (a.sched == 1) {
+        /* single launch: bound by the event bytes over HBM, so units as long as a staging buffer holds (6 KB: 128
+         * slim or 64 weighted batches), shorter only where the store is too small to give every SM a few of them */
+        /* the finalize CTAs (one per point) must find room beside the persistent grid to work ahead */
+        int fcap = std::max(ctx->fused_warps - WARPS * P, WARPS);
+        if (ctx->max_warps > 0) fcap = std::max(WARPS, std::min(fcap, ctx->max_warps / WARPS * WARPS));
+        int64_t U = STAGE_BUF_BYTES / (int64_t)(all_slim ? sizeof(EventBatchU) : sizeof(EventBatchW));
+        while (U > 32 && (batches + U - 1) / U < 4ll * ctx->sm_count) U /= 2;
+        if (ctx->unit_events > 0)
+            U = std::max<int64_t>(1, std::min<int64_t>(ctx->unit_events / EB, STAGE_BUF_BYTES / (int64_t)sizeof(EventBatchW)));
+        U = std::max<int64_t>(U, streams);              /* every sub-stream of a unit holds a batch */
+        int64_t units = 0;
+        for (int d = 0; d < ctx->n_datasets; ++d) {
+            a.ds[d].unit_begin = (int32_t)units;
+            units += (ctx->ds[d].n_pad / EB + U - 1) / U;
+        }
+        a.tail_unit = (int32_t)units;                   /* no fine tail */
+        a.tail_b0 = (int32_t)nb_last;
+        a.tail_batches = (int32_t)U;
+        a.unit_batches = (int32_t)U;
+        a.chunk_groups = 1;
+        a.n_units = (int32_t)units;
+        a.n_chunks = 1;
+        a.n_items = (int32_t)units;
+        a.n_warps = (int32_t)std::max<int64_t>(WARPS, std::min<int64_t>(fcap, (units + WARPS - 1) / WARPS * WARPS));
+        return PHYLINO_OK;
+    }
+
+    /* Cut of the batch into work items (spectra.cu): U batches per unit, G point groups per item.
+     * Aim: at least 12 items per resident warp (dynamic balance, short tail) of at least 16 batch-groups
+     * each (the per-item cost -- first bin search, one flush per point -- stays a few percent). */
     int cap = std::max(ctx->resident_warps, WARPS);
     if (ctx->max_warps > 0) cap = std::max(WARPS, std::min(cap, ctx->max_warps / WARPS * WARPS));
     const int64_t work = std::max<int64_t>(1, batches * n_groups / (12ll * cap));
@@ -223,13 +297,11 @@ void fill_batch(const phylino_ctx *ctx, SpectraArgs &a, int P, const double *par
     G = (n_groups + (n_groups + G - 1) / G - 1) / ((n_groups + G - 1) / G);
     if (ctx->chunk_groups > 0) G = std::min<int64_t>(ctx->chunk_groups, n_groups);
     int64_t units, chunks, tail_unit, tail_b0, Us;
-    const int last = ctx->n_datasets - 1;
     for (;;) {
         chunks = (n_groups + G - 1) / G;
         /* fine tail: about the last 1.5 items of every warp's share, at most a quarter of the work and
          * never more than the last dataset, in units of U/4 */
         const int64_t per_warp = std::max<int64_t>(1, (batches + U - 1) / U * chunks / cap);
-        const int64_t nb_last = ctx->ds[last].n_pad / EB;
         int64_t fine = std::min<int64_t>(batches / 4, batches * 3 / (2 * per_warp));
         fine = std::min(fine, nb_last);
         Us = std::max<int64_t>(std::max<int64_t>(4, streams), U / 4);
@@ -257,45 +329,22 @@ void fill_batch(const phylino_ctx *ctx, SpectraArgs &a, int P, const double *par
     a.n_items = (int32_t)(units * chunks);
     const int64_t warps = std::min<int64_t>(cap, (a.n_items + WARPS - 1) / WARPS * WARPS);
     a.n_warps = (int32_t)std::max<int64_t>(warps, WARPS);
-    /* batches of at most 16 points (the minimiser's single evaluations) are bound by per-item latency chains,
-     * not by arithmetic: they take the static schedule -- one contiguous range of at least one unit per warp,
-     * runs carried across its units (spectra.cu, spectra_static_kernel).  Measured on 6e6 events: 1 / 4 / 16
-     * points 0.098 / 0.123 / 0.204 ms -> 0.062 / 0.082 / 0.178 ms (two-term models); on config 4's store (three
-     * terms, 410 bins) 1 / 2 points 0.142 / 0.143 -> 0.084 / 0.114 ms, even at 4, slower from 8.  Larger batches
-     * are faster with the tickets (config 2: 0.21 ms against 0.29 ms static). */
-    a.sched = P <= (ctx->n_terms == 2 ? 16 : 4) ? 1 : 0;
-    if (a.sched == 1) {
-        a.unit_batches = (int32_t)MAX_UNIT_BATCHES;
-        const int64_t want = (batches + MAX_UNIT_BATCHES - 1) / MAX_UNIT_BATCHES;
-        a.n_warps = (int32_t)std::max<int64_t>(WARPS, std::min<int64_t>(cap, (want + WARPS - 1) / WARPS * WARPS));
-    }
-}
-
-/* enqueue the setup and spectra kernels (rows a1-a4) for P points */
-phylino_status enqueue_spectra(phylino_ctx *ctx, int P, const double *params)
-{
-    if (ctx->resident_warps == 0)
-        CU(spectra_max_warps(ctx->n_terms, ctx->sm_count, &ctx->resident_warps));
-    SpectraArgs a{};
-    fill_datasets(ctx, a);
-    fill_batch(ctx, a, P, params);
-    if (ctx->timing) CU(cudaEventRecord(ctx->ev[0], ctx->stream));
-    if (a.n_items > 0 && P > 0) {
-        CU(launch_setup(a, ctx->n_terms, ctx->stream));
-        ctx->launches += 1;
-    }
-    if (ctx->timing) CU(cudaEventRecord(ctx->ev[1], ctx->stream));
-    if (a.n_items > 0 && P > 0) {
-        CU(launch_spectra(a, ctx->n_terms, ctx->stream, !ctx->timing));
-        ctx->launches += 1;
-    }
     return PHYLINO_OK;
 }
 
-phylino_status enqueue_finalize(phylino_ctx *ctx, int P, const double *params, const double *data,
-                                double *hist, double *nll, int mode = -1)
+/* enqueue rows a1-a7 for P points: one launch of the single-launch kernel for small batches, else the
+ * setup, spectra (tickets) and finalize kernels.  mode: 0 spectra H -> hist, 1 expectation mu -> hist, 2 NLL -> nll;
+ * bins != NULL: the diagnostic instantiation (bin of every event), accumulators cleared, no other output. */
+phylino_status enqueue_eval(phylino_ctx *ctx, int P, const double *params, const double *data, double *hist,
+                            double *nll, int mode, int32_t *bins = nullptr, const double *host_copy = nullptr)
 {
-    if (mode < 0) mode = nll ? 2 : 0;
+    SpectraArgs a{};
+    fill_datasets(ctx, a);
+    phylino_status s = fill_batch(ctx, a, P, params);
+    if (s != PHYLINO_OK) return s;
+    const bool dbg = bins != nullptr;
+    a.dbg_bins = bins;
+    a.total_events = phylino_total_events(ctx);
     FinalizeArgs f = ctx->fin;
     f.P = P;
     f.params = params;
@@ -304,8 +353,41 @@ phylino_status enqueue_finalize(phylino_ctx *ctx, int P, const double *params, c
     f.data = data;
     f.hist = hist;
     f.nll = nll;
+    if (dbg) mode = 3;
+    const bool pdl = !ctx->timing;
+    if (ctx->timing) { CU(cudaEventRecord(ctx->ev[0], ctx->stream)); }
+    if (a.sched == 1) {
+        /* small batch: setup fused into the spectra kernel, the finalize kernel (its programmatic dependent, one
+         * CTA per point) does its table work while the events are walked and zeroes the work counter */
+        if (ctx->timing) CU(cudaEventRecord(ctx->ev[1], ctx->stream));
+        /* host_copy: the same batch in host memory, small enough to ride with the kernel arguments -- the walk then
+         * never touches `params` (which may be the device alias of pinned host memory: only the few finalize CTAs
+         * read it, in their prologue) */
+        ParamBlob &blob = ctx->blob;                    /* contents matter only when a.params == NULL */
+        if (host_copy && (int64_t)P * ctx->n_params <= PARAM_BLOB_DOUBLES) {
+            std::memcpy(blob.v, host_copy, (size_t)P * ctx->n_params * sizeof(double));
+            a.params = nullptr;
+        }
+        CU(launch_fused(a, blob, ctx->n_terms, ctx->stream, pdl, dbg));
+        ctx->launches += 1;
+        if (ctx->timing) CU(cudaEventRecord(ctx->ev[2], ctx->stream));
+        f.reset_counter = ctx->d_done;
+        CU(launch_finalize(f, mode, ctx->stream, pdl));
+        ctx->launches += 1;
+        if (ctx->timing) CU(cudaEventRecord(ctx->ev[3], ctx->stream));
+        return PHYLINO_OK;
+    }
+    if (a.n_items > 0 && P > 0) {
+        CU(launch_setup(a, ctx->n_terms, ctx->stream));
+        ctx->launches += 1;
+    }
+    if (ctx->timing) CU(cudaEventRecord(ctx->ev[1], ctx->stream));
+    if (a.n_items > 0 && P > 0) {
+        CU(launch_spectra(a, ctx->n_terms, ctx->stream, pdl, dbg));
+        ctx->launches += 1;
+    }
     if (ctx->timing) CU(cudaEventRecord(ctx->ev[2], ctx->stream));
-    CU(launch_finalize(f, mode, ctx->stream, !ctx->timing));
+    CU(launch_finalize(f, mode, ctx->stream, pdl));
     ctx->launches += 1;
     if (ctx->timing) CU(cudaEventRecord(ctx->ev[3], ctx->stream));
     return PHYLINO_OK;
@@ -424,6 +506,7 @@ struct IdTable {
 bool plan_components(const phylino_ctx *ctx, int P, const double *params, ComponentPlan &pl)
 {
     const int S = ctx->n_terms, NP = ctx->n_params;
+    if (P >= (1 << 29)) return false;                   /* (point, term) is packed as p * 4 + k in an int32 */
     /* columns of the parameter vector that enter the energy scale of any dataset */
     std::vector<int32_t> acols;
     for (int d = 0; d < ctx->n_datasets; ++d)
@@ -531,25 +614,30 @@ phylino_status enqueue_cached(phylino_ctx *ctx, int P, const double *h_params, c
     /* pageable source: the copy is staged by the driver before the call returns */
     CU(cudaMemcpyAsync(ctx->d_plan, blob.data(), n_int * sizeof(int32_t), cudaMemcpyHostToDevice, ctx->stream));
 
-    if (ctx->resident_warps == 0) CU(spectra_max_warps(ctx->n_terms, ctx->sm_count, &ctx->resident_warps));
     SpectraArgs a{};
     fill_datasets(ctx, a);
-    fill_batch(ctx, a, V, d_params);
     a.comp = 1;
-    a.thr_rows = pl.C;
+    if ((s = fill_batch(ctx, a, V, d_params, pl.C)) != PHYLINO_OK) return s;
     a.vp_class = ctx->d_plan;
     a.vp_src = ctx->d_plan + V;
     a.class_rep = ctx->d_plan + V + (int64_t)V * S;
-    if (ctx->timing) CU(cudaEventRecord(ctx->ev[0], ctx->stream));
-    if (a.n_items > 0) { CU(launch_setup(a, S, ctx->stream)); ctx->launches += 1; }
-    if (ctx->timing) CU(cudaEventRecord(ctx->ev[1], ctx->stream));
-    if (a.n_items > 0) { CU(launch_spectra(a, S, ctx->stream, !ctx->timing)); ctx->launches += 1; }
-
     FinalizeArgs f = ctx->fin;
     f.P = P; f.params = d_params; f.acc = ctx->d_acc; f.flags = ctx->d_flags;
     f.data = d_data; f.hist = d_hist; f.nll = d_nll;
     f.comp = 1; f.n_terms = S; f.osc = a.osc;
     f.pt_comp = ctx->d_plan + V + (int64_t)V * S + pl.C;
+    if (ctx->timing) CU(cudaEventRecord(ctx->ev[0], ctx->stream));
+    if (a.sched == 1) {
+        /* few virtual points: setup and walk in one launch; the per-point combination stays a launch of its own */
+        if (ctx->timing) CU(cudaEventRecord(ctx->ev[1], ctx->stream));
+        CU(launch_fused(a, ctx->blob, S, ctx->stream, !ctx->timing, false));
+        ctx->launches += 1;
+        f.reset_counter = ctx->d_done;
+    } else {
+        if (a.n_items > 0) { CU(launch_setup(a, S, ctx->stream)); ctx->launches += 1; }
+        if (ctx->timing) CU(cudaEventRecord(ctx->ev[1], ctx->stream));
+        if (a.n_items > 0) { CU(launch_spectra(a, S, ctx->stream, !ctx->timing, false)); ctx->launches += 1; }
+    }
     if (ctx->timing) CU(cudaEventRecord(ctx->ev[2], ctx->stream));
     CU(launch_finalize(f, d_nll ? 2 : 0, ctx->stream, !ctx->timing));
     ctx->launches += 1;
@@ -704,6 +792,7 @@ phylino_status phylino_set_model(phylino_ctx *ctx, const phylino_model_desc *m)
     FinalizeArgs &f = ctx->fin;
     f.n_params = m->n_params;
     f.total_bins = (int32_t)tb;
+    f.staged = tb <= FIN_STAGE_MAX_BINS ? 1 : 0;
     f.n_datasets = m->n_datasets;
     f.max_bkg = max_bkg;
     cudaStream_t st = ctx->stream;
@@ -760,30 +849,52 @@ phylino_status phylino_load_events(phylino_ctx *ctx, int dataset, int64_t n, con
         if (y != y) return true;
         return x < y;
     });
-    const int64_t n_pad = (n + EB - 1) / EB * EB;
-    EventBatch blank{};
-    for (int j = 0; j < EB; ++j) blank.v[j] = std::nanf("");
-    std::vector<EventBatch> ev((size_t)(n_pad / EB), blank);
+    const int64_t n_pad = (n + EB - 1) / EB * EB, n_batches = n_pad / EB;
     double wsum = 0.0;
     bool unit_w = true;
     float v_pos_min = INFINITY, v_max = -INFINITY;
     for (int64_t i = 0; i < n; ++i) {
-        int32_t s = perm[i];
-        EventBatch &b = ev[(size_t)(i / EB)];
-        const int j = (int)(i % EB);
-        const float vi = e_vis[s];
-        b.x[j] = baseline_m[core ? core[s] : 0] / (double)e_nu[s];
-        b.v[j] = vi;
-        b.w[j] = weight ? (double)weight[s] : 1.0;
-        b.wsum += b.w[j];                       /* in event order: the batch total the hot kernel adds */
-        if (j == 0)                             /* where a lane starts looking for its bin (a hint, never trusted) */
-            b.bin0 = vi == vi ? (int32_t)(std::upper_bound(edges, edges + n_bins + 1, (double)vi) - edges) - 1 : n_bins;
-        wsum += std::fabs(b.w[j]);
-        unit_w = unit_w && b.w[j] == 1.0;
+        const float vi = e_vis[i];
+        const double wi = weight ? (double)weight[i] : 1.0;
+        wsum += std::fabs(wi);
+        unit_w = unit_w && wi == 1.0;
         if (std::isfinite(vi)) {
             if (vi > 0.0f && vi < v_pos_min) v_pos_min = vi;
             if (vi > v_max) v_max = vi;
         }
+    }
+    /* records of EB consecutive sorted events: 48 bytes (x, v) when every weight is exactly 1, else 96 (x, w, v,
+     * batch weight sum); padding: x = 0, w = 0, v = NaN (lands in no bin) */
+    std::vector<EventBatchU> ev_u;
+    std::vector<EventBatchW> ev_w;
+    {
+        EventBatchU bu{};
+        EventBatchW bw{};
+        for (int j = 0; j < EB; ++j) { bu.v[j] = std::nanf(""); bw.v[j] = std::nanf(""); }
+        if (unit_w) ev_u.assign((size_t)n_batches, bu); else ev_w.assign((size_t)n_batches, bw);
+    }
+    /* where a lane starts looking for its bin (a hint, never trusted): the bin of the first event of every
+     * HINT_BATCHES-th batch under the identity energy scale */
+    std::vector<int32_t> hint((size_t)((n_batches + HINT_BATCHES - 1) / HINT_BATCHES), n_bins);
+    for (int64_t i = 0; i < n; ++i) {
+        const int32_t s = perm[i];
+        const int64_t b = i / EB;
+        const int j = (int)(i % EB);
+        const float vi = e_vis[s];
+        const double xi = baseline_m[core ? core[s] : 0] / (double)e_nu[s];
+        if (unit_w) {
+            ev_u[(size_t)b].x[j] = xi;
+            ev_u[(size_t)b].v[j] = vi;
+        } else {
+            EventBatchW &r = ev_w[(size_t)b];
+            r.x[j] = xi;
+            r.v[j] = vi;
+            r.w[j] = (double)weight[s];
+            r.wsum += r.w[j];                   /* in event order: the batch total the hot kernel adds */
+        }
+        if (j == 0 && b % HINT_BATCHES == 0)
+            hint[(size_t)(b / HINT_BATCHES)] =
+                vi == vi ? (int32_t)(std::upper_bound(edges, edges + n_bins + 1, (double)vi) - edges) - 1 : n_bins;
     }
     /* fixed-point scale 2^e with 8 * sum|w| * 2^e <= 2^62 (|P_ee| <= 4 is enforced per point) */
     int ex = 0;
@@ -795,9 +906,11 @@ phylino_status phylino_load_events(phylino_ctx *ctx, int dataset, int64_t n, con
     free_events(h);
     cudaStream_t st = ctx->stream;
     std::vector<double> ed(edges, edges + n_bins + 1);
-    CU(upload(&h.d_ev, ev, st));
+    if (unit_w) { EventBatchU *d = nullptr; CU(upload(&d, ev_u, st)); h.d_ev = d; }
+    else        { EventBatchW *d = nullptr; CU(upload(&d, ev_w, st)); h.d_ev = d; }
     CU(upload(&h.d_edges, ed, st));
     CU(upload(&h.d_perm, perm, st));
+    CU(upload(&h.d_hint, hint, st));
     double inv = std::ldexp(1.0, -fx);
     CU(cudaMemcpyAsync((void *)(ctx->fin.inv_scale + dataset), &inv, sizeof(double), cudaMemcpyHostToDevice, st));
     CU(cudaStreamSynchronize(st));
@@ -813,15 +926,14 @@ phylino_status phylino_spectra(phylino_ctx *ctx, int P, const double *params, do
     if (s != PHYLINO_OK || P == 0) return s;
     DeviceGuard g(ctx->device);
     if ((s = resolve_params(ctx, P, params, &params)) != PHYLINO_OK) return s;
-    if (ctx->caching) {
+    if (ctx->caching && !wants_single_launch(ctx, P)) {
         bool cached = false;
         if ((s = cached_from_device(ctx, P, params, nullptr, hist, nullptr, &cached)) != PHYLINO_OK || cached) return s;
     } else {
         ctx->last_virtual_points = ctx->last_classes = 0;
     }
     if ((s = ensure_acc(ctx, P)) != PHYLINO_OK) return s;
-    if ((s = enqueue_spectra(ctx, P, params)) != PHYLINO_OK) return s;
-    return enqueue_finalize(ctx, P, params, nullptr, hist, nullptr);
+    return enqueue_eval(ctx, P, params, nullptr, hist, nullptr, 0);
 }
 
 phylino_status phylino_nll(phylino_ctx *ctx, int P, const double *params, const double *data, double *nll)
@@ -831,15 +943,14 @@ phylino_status phylino_nll(phylino_ctx *ctx, int P, const double *params, const 
     if (!data) return fail(ctx, PHYLINO_ERR_ARG, "NULL data pointer");
     DeviceGuard g(ctx->device);
     if ((s = resolve_params(ctx, P, params, &params)) != PHYLINO_OK) return s;
-    if (ctx->caching) {
+    if (ctx->caching && !wants_single_launch(ctx, P)) {
         bool cached = false;
         if ((s = cached_from_device(ctx, P, params, data, nullptr, nll, &cached)) != PHYLINO_OK || cached) return s;
     } else {
         ctx->last_virtual_points = ctx->last_classes = 0;
     }
     if ((s = ensure_acc(ctx, P)) != PHYLINO_OK) return s;
-    if ((s = enqueue_spectra(ctx, P, params)) != PHYLINO_OK) return s;
-    return enqueue_finalize(ctx, P, params, data, nullptr, nll);
+    return enqueue_eval(ctx, P, params, data, nullptr, nll, 2);
 }
 
 phylino_status phylino_nll_ensemble(phylino_ctx *ctx, int P, const double *params, int E, const double *data,
@@ -860,11 +971,10 @@ phylino_status phylino_nll_ensemble(phylino_ctx *ctx, int P, const double *param
         CU(cudaMalloc((void **)&ctx->d_mu, need * sizeof(double)));
         ctx->mu_capacity = need;
     }
-    if ((s = enqueue_spectra(ctx, P, params)) != PHYLINO_OK) return s;
-    if ((s = enqueue_finalize(ctx, P, params, nullptr, ctx->d_mu, nullptr, 1)) != PHYLINO_OK) return s;
+    if ((s = enqueue_eval(ctx, P, params, nullptr, ctx->d_mu, nullptr, 1)) != PHYLINO_OK) return s;
     FinalizeArgs f = ctx->fin;
     f.P = P; f.params = params; f.data = data; f.hist = ctx->d_mu; f.nll = nll;
-    CU(launch_ensemble(f, E, ctx->stream));
+    CU(launch_ensemble(f, E, ctx->sm_count, ctx->stream));
     ctx->launches += 1;
     return PHYLINO_OK;
 }
@@ -876,8 +986,7 @@ phylino_status phylino_expectation(phylino_ctx *ctx, int P, const double *params
     DeviceGuard g(ctx->device);
     if ((s = resolve_params(ctx, P, params, &params)) != PHYLINO_OK) return s;
     if ((s = ensure_acc(ctx, P)) != PHYLINO_OK) return s;
-    if ((s = enqueue_spectra(ctx, P, params)) != PHYLINO_OK) return s;
-    return enqueue_finalize(ctx, P, params, nullptr, mu, nullptr, 1);
+    return enqueue_eval(ctx, P, params, nullptr, mu, nullptr, 1);
 }
 
 phylino_status phylino_event_bins(phylino_ctx *ctx, int P, const double *params, int32_t *bins)
@@ -887,23 +996,9 @@ phylino_status phylino_event_bins(phylino_ctx *ctx, int P, const double *params,
     DeviceGuard g(ctx->device);
     if ((s = resolve_params(ctx, P, params, &params)) != PHYLINO_OK) return s;
     if ((s = ensure_acc(ctx, P)) != PHYLINO_OK) return s;
-    SpectraArgs a{};
-    fill_datasets(ctx, a);
-    fill_batch(ctx, a, P, params);
-    if (a.n_items > 0) {                        /* the threshold rows the hot kernel would use */
-        CU(launch_setup(a, ctx->n_terms, ctx->stream));
-        ctx->launches += 1;
-    }
-    int64_t total = phylino_total_events(ctx), off = 0;
-    for (int d = 0; d < ctx->n_datasets; ++d) {
-        const phylino_dataset_host &h = ctx->ds[d];
-        if (h.n > 0) {
-            CU(launch_event_bins(a, d, h.d_perm, h.n, off, total, bins, ctx->stream));
-            ctx->launches += 1;
-        }
-        off += h.n;
-    }
-    return PHYLINO_OK;
+    /* the production kernels of this batch size in their diagnostic instantiation */
+    CU(cudaMemsetAsync(bins, 0xff, (size_t)P * phylino_total_events(ctx) * sizeof(int32_t), ctx->stream));
+    return enqueue_eval(ctx, P, params, nullptr, nullptr, nullptr, 3, bins);
 }
 
 phylino_status phylino_nll_host(phylino_ctx *ctx, int P, const double *params_host, const double *data_host,
@@ -919,16 +1014,25 @@ phylino_status phylino_nll_host(phylino_ctx *ctx, int P, const double *params_ho
     if (ctx->have_tf) host_transform(ctx, P, params_host, ctx->h_pin);
     else std::memcpy(ctx->h_pin, params_host, np * sizeof(double));
     std::memcpy(ctx->h_pin + np, data_host, tb * sizeof(double));
-    CU(cudaMemcpyAsync(ctx->d_stage, ctx->h_pin, (np + tb) * sizeof(double), cudaMemcpyHostToDevice, ctx->stream));
-    /* the finalize kernel writes nll[P] straight into the pinned block (8 P bytes over PCIe): no copy back */
+    /* the likelihood stage writes nll[P] straight into the pinned block (8 P bytes over PCIe): no copy back */
     double *d_out = ctx->d_pin + np + tb;
-    bool cached = false;
-    if (ctx->caching &&
-        (s = enqueue_cached(ctx, P, ctx->h_pin, ctx->d_stage, ctx->d_stage + np, nullptr, d_out, &cached)) != PHYLINO_OK)
-        return s;
-    if (!cached) {
-        if ((s = enqueue_spectra(ctx, P, ctx->d_stage)) != PHYLINO_OK) return s;
-        if ((s = enqueue_finalize(ctx, P, ctx->d_stage, ctx->d_stage + np, nullptr, d_out)) != PHYLINO_OK) return s;
+    if (wants_single_launch(ctx, P) && np <= PARAM_BLOB_DOUBLES) {
+        /* a single evaluation: no copy engine.  The parameters ride with the kernel arguments of the walk; the
+         * finalize CTAs read parameters and data from the pinned block through its device alias while the events
+         * are walked, and write nll[P] into it */
+        ctx->last_virtual_points = ctx->last_classes = 0;
+        if ((s = enqueue_eval(ctx, P, ctx->d_pin, ctx->d_pin + np, nullptr, d_out, 2, nullptr, ctx->h_pin)) != PHYLINO_OK)
+            return s;
+    } else {
+        CU(cudaMemcpyAsync(ctx->d_stage, ctx->h_pin, (np + tb) * sizeof(double), cudaMemcpyHostToDevice, ctx->stream));
+        bool cached = false;
+        if (ctx->caching && !wants_single_launch(ctx, P) &&
+            (s = enqueue_cached(ctx, P, ctx->h_pin, ctx->d_stage, ctx->d_stage + np, nullptr, d_out, &cached)) != PHYLINO_OK)
+            return s;
+        if (!cached) {
+            ctx->last_virtual_points = ctx->last_classes = 0;
+            if ((s = enqueue_eval(ctx, P, ctx->d_stage, ctx->d_stage + np, nullptr, d_out, 2)) != PHYLINO_OK) return s;
+        }
     }
     CU(cudaStreamSynchronize(ctx->stream));
     std::memcpy(nll_host, ctx->h_pin + np + tb, P * sizeof(double));
@@ -947,12 +1051,12 @@ phylino_status phylino_spectra_host(phylino_ctx *ctx, int P, const double *param
     else std::memcpy(ctx->h_pin, params_host, np * sizeof(double));
     CU(cudaMemcpyAsync(ctx->d_stage, ctx->h_pin, np * sizeof(double), cudaMemcpyHostToDevice, ctx->stream));
     bool cached = false;
-    if (ctx->caching &&
+    if (ctx->caching && !wants_single_launch(ctx, P) &&
         (s = enqueue_cached(ctx, P, ctx->h_pin, ctx->d_stage, nullptr, ctx->d_stage + np, nullptr, &cached)) != PHYLINO_OK)
         return s;
     if (!cached) {
-        if ((s = enqueue_spectra(ctx, P, ctx->d_stage)) != PHYLINO_OK) return s;
-        if ((s = enqueue_finalize(ctx, P, ctx->d_stage, nullptr, ctx->d_stage + np, nullptr)) != PHYLINO_OK) return s;
+        ctx->last_virtual_points = ctx->last_classes = 0;
+        if ((s = enqueue_eval(ctx, P, ctx->d_stage, nullptr, ctx->d_stage + np, nullptr, 0)) != PHYLINO_OK) return s;
     }
     CU(cudaMemcpyAsync(ctx->h_pin + np, ctx->d_stage + np, nh * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
     CU(cudaStreamSynchronize(ctx->stream));
@@ -1088,6 +1192,34 @@ phylino_status phylino_set_tuning(phylino_ctx *ctx, int unit_events, int chunk_g
     ctx->unit_events = unit_events;
     ctx->chunk_groups = chunk_groups;
     ctx->max_warps = max_warps;
+    return PHYLINO_OK;
+}
+
+phylino_status phylino_set_schedule(phylino_ctx *ctx, int mode)
+{
+    if (!ctx) return PHYLINO_ERR_ARG;
+    if (mode < 0 || mode > 2) return fail(ctx, PHYLINO_ERR_ARG, "schedule %d not in 0..2", mode);
+    ctx->schedule = mode;
+    return PHYLINO_OK;
+}
+
+phylino_status phylino_reserve(phylino_ctx *ctx, int max_points)
+{
+    phylino_status s = check_ready(ctx, max_points, nullptr, nullptr);
+    if (s != PHYLINO_OK && !(s == PHYLINO_ERR_ARG && ctx && max_points > 0)) return s;   /* no buffers to check here */
+    if (max_points == 0) return PHYLINO_OK;
+    DeviceGuard g(ctx->device);
+    if ((s = ensure_acc(ctx, max_points)) != PHYLINO_OK) return s;
+    const int64_t width = std::max<int64_t>(ctx->n_params, param_width(ctx));
+    if ((s = ensure_stage(ctx, (int64_t)max_points * (width + ctx->total_bins) + ctx->total_bins)) != PHYLINO_OK) return s;
+    const int64_t need = (int64_t)max_points * ctx->n_params;
+    if (ctx->have_tf && need > ctx->theta_capacity) {
+        CU(cudaStreamSynchronize(ctx->stream));
+        cudaFree(ctx->d_theta); ctx->d_theta = nullptr; ctx->theta_capacity = 0;
+        CU(cudaMalloc((void **)&ctx->d_theta, need * sizeof(double)));
+        ctx->theta_capacity = need;
+    }
+    ctx->err.clear();
     return PHYLINO_OK;
 }
 

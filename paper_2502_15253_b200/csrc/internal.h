@@ -16,34 +16,54 @@
 namespace phylino {
 
 /* ---- layout of the event store and of a launch -------------------------------------------------
- * The events of a dataset, sorted by E_vis, are cut into batches of EB consecutive events, one
- * 96-byte record each; `unit_batches` consecutive batches form a unit.  A work item is one unit x
- * `chunk_groups` groups of 32 parameter points; the warps of a persistent grid claim items from a
- * global counter and walk the unit once per group, ONE POINT PER LANE (spectra.cu). */
+ * The events of a dataset, sorted by E_vis, are cut into batches of EB consecutive events, one record
+ * each (48 bytes when every MC weight of the dataset is exactly 1, else 96); `unit_batches` consecutive
+ * batches form a unit.  Large batches of points: a work item is one unit x `chunk_groups` groups of 32
+ * parameter points; the warps of a persistent grid claim items from a global counter and walk the unit
+ * once per group, ONE POINT PER LANE.  Small batches: every warp owns one contiguous range of batches and
+ * setup, walk and likelihood run in ONE launch (spectra.cu). */
 constexpr int EB          = 4;                      /* events per batch; every dataset is padded to a multiple */
-constexpr int WARPS       = 4;                      /* warps per CTA of the spectra kernel */
-constexpr int MAX_UNIT_BATCHES = 64;                /* a unit is staged in shared memory: <= 6 KB */
+constexpr int WARPS       = 4;                      /* warps per CTA of the spectra kernels */
+constexpr int STAGE_BUF_BYTES = 6144;               /* one staging buffer of a warp: a unit is at most this long */
+constexpr int MAX_UNIT_BATCHES = 64;                /* ticket schedule: batches per unit (<= 6 KB of 96-byte records) */
+constexpr int HINT_BATCHES = 16;                    /* one bin hint per this many batches of a dataset */
 constexpr int MAX_TERMS   = 3;
 constexpr int SETUP_THREADS = 128;
+constexpr int FIN_THREADS = 128;                    /* = WARPS * 32: the last CTA of the fused kernel runs the likelihood stage */
+constexpr int FUSED_MAX_POINTS = 16;                /* largest batch the single-launch kernel takes */
+constexpr int FIN_STAGE_MAX_BINS = 2000;            /* 3 doubles per bin of shared memory in the finalize kernel */
 
 /* flag bits of a (point, bin) accumulator whose value left the fixed-point domain */
 enum : unsigned { FLAG_NAN = 1u, FLAG_PINF = 2u, FLAG_NINF = 4u };
 
-/* EB consecutive events of the E_vis-sorted store: everything the hot loop reads, behind one pointer */
-struct __align__(16) EventBatch {
+/* EB consecutive events of the E_vis-sorted store: everything the hot loop reads, behind one pointer.
+ * Weighted datasets (some w != 1): */
+struct __align__(16) EventBatchW {
     double x[EB];           /* L_core/E_nu  [m/MeV], fp64 (phase range reduction needs it) */
     double w[EB];           /* MC weight as fp64 (exact copy of the fp32 input); padding = 0 */
     float  v[EB];           /* E_vis [MeV]; padding = NaN */
     double wsum;            /* w[0] + ... + w[EB-1], summed in that order */
-    int32_t bin0;           /* hint: bin of v[0] under the identity energy scale, -1 below, n_bins above / NaN */
-    int32_t reserved;
+    int32_t reserved[2];
 };
-static_assert(sizeof(EventBatch) == 96, "EventBatch is read with fixed 16-byte offsets");
+/* Unit-weight datasets (every BASELINE.json config): 12 bytes per event */
+struct __align__(16) EventBatchU {
+    double x[EB];
+    float  v[EB];
+};
+static_assert(sizeof(EventBatchW) == 96 && sizeof(EventBatchU) == 48, "records are read with fixed 16-byte offsets");
+template <bool UW> struct RecOf { typedef EventBatchW type; };
+template <> struct RecOf<true> { typedef EventBatchU type; };
 
 /* Per-dataset entry of the table that travels by value in the kernel parameters. */
 struct DatasetDev {
-    const EventBatch *ev;   /* [n_batches] */
+    const void *ev;         /* [n_batches] EventBatchU if unit_w else EventBatchW */
     const double *edges;    /* [n_bins+1] */
+    const int32_t *hint;    /* [ceil(n_batches / HINT_BATCHES)] bin of the first event of batch HINT_BATCHES i under the
+                               identity energy scale (-1 below the first edge, n_bins above the last / NaN): where a
+                               lane starts looking for its bin, never trusted */
+    const int32_t *perm;    /* [n] caller's index of sorted event i (diagnostic instantiation only) */
+    long long ev_off;       /* events of the datasets before this one (diagnostic instantiation only) */
+    int32_t n_events;       /* events before padding */
     int32_t n_bins;
     int32_t bin_off;        /* offset of this dataset inside a point's total_bins */
     int32_t thr_off;        /* offset of this dataset inside a threshold row: sum of (n_bins+1) before it */
@@ -83,12 +103,15 @@ struct SpectraArgs {
     int32_t tail_b0;        /* its first batch inside the last dataset */
     int32_t tail_batches;   /* batches per unit of the fine tail */
     int32_t n_warps;        /* warps of the persistent grid (a multiple of WARPS) */
-    int32_t sched;          /* 0: items claimed from the counter; 1: one contiguous range of batches per warp */
-    unsigned *counter;      /* DEVICE work counter; the setup kernel sets it to 2 n_warps */
+    int32_t sched;          /* 0: items claimed from the counter; 1: one contiguous range of batches per warp, single launch */
+    unsigned *counter;      /* DEVICE work counter of the ticket kernel; the setup kernel zeroes it */
+    unsigned *done;         /* DEVICE work counter of the single-launch kernel; the finalize kernel behind it zeroes it */
+    int32_t  *dbg_bins;     /* DEVICE [P x total_events] diagnostic instantiation: bin the hot loop gave every event */
+    long long total_events;
     int32_t thr_stride;     /* floats per threshold row: total_bins + n_datasets */
     int32_t thr_rows;       /* P if some dataset's energy scale depends on theta, else 1 */
     int32_t total_bins;
-    const double *params;   /* DEVICE [P x n_params] */
+    const double *params;   /* DEVICE [P x n_params]; NULL: the batch is in the ParamBlob argument (small-batch kernel) */
     double       *rec;      /* DEVICE [rec_fields x P] per-point records (setup kernel) */
     float        *thr;      /* DEVICE [thr_rows x thr_stride] fp32 bin thresholds (setup kernel) */
     float2       *safe;     /* DEVICE [thr_rows x n_datasets] fp32 interval on which a row holds */
@@ -104,9 +127,15 @@ struct SpectraArgs {
     const int32_t *class_rep;   /* DEVICE [thr_rows] real point whose energy scale defines the row */
 };
 
+/* a small batch of parameter points travelling BY VALUE with the arguments of the small-batch kernel */
+constexpr int PARAM_BLOB_DOUBLES = 448;
+struct ParamBlob { double v[PARAM_BLOB_DOUBLES]; };
+
 /* Model tables of the expectation / NLL stage, all DEVICE pointers. */
 struct FinalizeArgs {
     int32_t P, n_params, total_bins, n_datasets, max_bkg;
+    int32_t staged;               /* total_bins <= FIN_STAGE_MAX_BINS: per-bin model values staged in shared memory */
+    unsigned *reset_counter;      /* DEVICE word zeroed at the end (the work counter of the single-launch kernel), or NULL */
     const double  *params;        /* [P x n_params] */
     long long     *acc;           /* [P x total_bins]; re-zeroed by the kernel */
     unsigned      *flags;         /* [P x total_bins]; re-zeroed by the kernel */
@@ -154,12 +183,13 @@ struct TransformArgs {
 /* kernel launchers (spectra.cu, finalize.cu, transform.cu, peaks.cu) */
 cudaError_t launch_transform(const TransformArgs &a, cudaStream_t st);
 cudaError_t launch_setup(const SpectraArgs &a, int S, cudaStream_t st);
-cudaError_t spectra_max_warps(int S, int sm_count, int *warps);
-cudaError_t launch_spectra(const SpectraArgs &a, int S, cudaStream_t st, bool pdl);
-cudaError_t launch_finalize(const FinalizeArgs &a, int mode /*0 H, 1 mu, 2 nll*/, cudaStream_t st, bool pdl);
-cudaError_t launch_ensemble(const FinalizeArgs &a, int E, cudaStream_t st);
-cudaError_t launch_event_bins(const SpectraArgs &a, int d, const int32_t *perm, long long n, long long ev_off,
-                              long long total_events, int32_t *bins, cudaStream_t st);
+size_t      fused_table_bytes(int S, int P, int thr_rows, int thr_stride, int n_datasets);
+bool        fused_fits(size_t table_bytes);
+cudaError_t spectra_max_warps(int S, int sm_count, bool fused, size_t table_bytes, int *warps);
+cudaError_t launch_spectra(const SpectraArgs &a, int S, cudaStream_t st, bool pdl, bool dbg);
+cudaError_t launch_fused(const SpectraArgs &a, const ParamBlob &blob, int S, cudaStream_t st, bool pdl, bool dbg);
+cudaError_t launch_finalize(const FinalizeArgs &a, int mode /*0 H, 1 mu, 2 nll, 3 clear*/, cudaStream_t st, bool pdl);
+cudaError_t launch_ensemble(const FinalizeArgs &a, int E, int sm_count, cudaStream_t st);
 cudaError_t run_peak_fp64(int iters, cudaStream_t st, double *dfma_per_s);
 cudaError_t run_launch_floor(int reps, cudaStream_t st, double *us_per_call);
 
@@ -182,7 +212,8 @@ struct phylino_dataset_host {
     float    v_pos_min = 0.f, v_max = 0.f;
     bool     unit_w = false;
     int      fx_exp = 0;
-    phylino::EventBatch *d_ev = nullptr;
+    void    *d_ev = nullptr;                        /* EventBatchU[] if unit_w else EventBatchW[] */
+    int32_t *d_hint = nullptr;
     double  *d_edges = nullptr;
     int32_t *d_perm = nullptr;
 };
@@ -232,7 +263,12 @@ struct phylino_ctx {
     unsigned *d_counter = nullptr;                 /* work counter of the spectra kernel */
     /* tuning knobs, 0 => default (phylino_set_tuning) */
     int unit_events = 0, chunk_groups = 0, max_warps = 0;
-    int resident_warps = 0;                        /* warps of the spectra kernel the chip holds at once */
+    int resident_warps = 0;                        /* warps of the ticket kernel the chip holds at once */
+    int fused_warps = 0;                           /* ... of the single-launch kernel with fused_tables bytes of tables */
+    size_t fused_tables = 0;
+    int schedule = 0;                              /* phylino_set_schedule: 0 auto, 1 tickets, 2 single launch */
+    unsigned *d_done = nullptr;                    /* work counter of the small-batch kernel */
+    phylino::ParamBlob blob{};                     /* a small host batch on its way into the kernel arguments */
     /* optional device timing of the three kernels of a call (phylino_set_timing) */
     bool timing = false;
     cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};

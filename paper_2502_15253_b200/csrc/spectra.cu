@@ -3,18 +3,28 @@
  * PAPER.md:177 signal step 1, :183 "the most time-demanding computational step").
  *
  * Layout of the work: ONE PARAMETER POINT PER LANE.  The E_vis-sorted events of a dataset are cut
- * into 96-byte batches of EB events and the batches into units; a work item is one unit x a chunk
- * of point groups (32 points each).  The warps of a persistent grid claim items from a global
- * counter (dynamic balance: units that contain bin edges cost more; the last stretch of the store is
- * cut into quarter-size units so the warps run out of work together) and walk the unit once per group.
+ * into batches of EB events (48-byte records when every MC weight is 1, else 96-byte ones) and the
+ * batches into units.
+ *
+ * Large batches of points (spectra_kernel, "tickets").  A work item is one unit x a chunk of point
+ * groups (32 points each).  The warps of a persistent grid claim items from a global counter (dynamic
+ * balance: units that contain bin edges cost more; the last stretch of the store is cut into
+ * quarter-size units so the warps run out of work together) and walk the unit once per group.
+ *
+ * Small batches (spectra_fused_kernel: at most FUSED_MAX_POINTS points -- the minimiser's single
+ * evaluations).  ONE launch does rows a1-a7: every CTA derives the per-point records and the
+ * bin thresholds it needs into its own shared memory, every warp walks ONE contiguous range of batches
+ * with its lanes split into 32 / PL sub-streams (PL = points rounded up to a power of two) and the runs
+ * carried across the units of the range, and the CTA that finishes last runs the expectation / likelihood
+ * stage (finalize.cuh) on the accumulators.  No setup launch, no finalize launch, no host copy of the
+ * parameters: the call is bound by the event bytes over HBM (12 B/event for unit-weight datasets).
  *
  * Staging.  Each warp owns two unit-sized buffers in shared memory and one mbarrier per buffer; lane 0
  * starts ONE bulk async copy (cp.async.bulk global -> shared, completion on the mbarrier) of the NEXT
- * item's unit while the current one is walked.  The hot loop reads warp-uniform LDS.128 broadcasts;
+ * unit while the current one is walked.  The hot loop reads warp-uniform LDS.128 broadcasts;
  * everything that depends on the point (half-turn coefficients h_k, the run accumulators, the current
  * bin, its fp32 upper threshold and the one after it) lives in the lane's registers.  No shuffles in
- * the loop, no block barriers.  A group of fewer than 17 points splits the unit into 32/PL sub-streams
- * (PL = points rounded up to a power of two), so that a batch of 1 point still uses all 32 lanes.
+ * the loop, no block barriers.
  *
  * Oscillation weight (row a2).  P_ee = P0 + sum_k A_k g_k with g = 1/2 cos(2 phase) (devmath.cuh):
  * the lane accumulates C_k = sum_e w_e g_k(e) and W = sum_e w_e over a run of events that share a
@@ -22,18 +32,18 @@
  * 11 fp64 instructions and one integer instruction per oscillation term.
  *
  * Binning (row a3).  For one point the map v -> E' = fma(fma(a2,v,a1),v,a0) is non-decreasing over
- * the fp32 values of a dataset (checked per point by the setup kernel), so bin(E'(v)) >= b <=>
- * v >= T[b] with T[b] the smallest fp32 value whose E' reaches edges[b].  T is found by bisection
- * with the SAME fp64 fma sequence, hence the fp32 comparison decides exactly what the fp64
- * comparison E' >= edges[b] decides: bit-exact bins.  Events are sorted, so 4, 2 or 1 batches lie
- * inside the lane's current bin iff the LAST event of the last one is below the bin's upper threshold:
- * one fp32 compare, then a straight-line stretch of rows a2 + a4 (datasets whose weights are all exactly
- * 1 skip the weight loads).  A lane opens its run at the first event of a unit from the load-time hint
- * bin0 of the batch.  Events outside the interval on which a table is proven (and points that fail the
- * monotonicity check) take the per-event fp64 map.
+ * the fp32 values of a dataset (checked per point), so bin(E'(v)) >= b <=> v >= T[b] with T[b] the
+ * smallest fp32 value whose E' reaches edges[b].  T is found with the SAME fp64 fma sequence and the
+ * SAME fp64 edges, hence the fp32 comparison decides exactly what the fp64 comparison E' >= edges[b]
+ * decides: bit-exact bins.  Events are sorted, so 4, 2 or 1 batches lie inside the lane's current bin
+ * iff the LAST event of the last one is below the bin's upper threshold: one fp32 compare, then a
+ * straight-line stretch of rows a2 + a4 (unit-weight datasets carry no weights at all).  A lane opens its
+ * run at its first event from a load-time hint (one per HINT_BATCHES batches).  Events outside the
+ * interval on which a table is proven (and points that fail the monotonicity check) take the per-event
+ * fp64 map.
  *
- * Histogram (rows a4, a5).  When a run ends (bin edge, end of the unit) its fp64 total is converted
- * once to 64-bit fixed point and added to the (point, bin) accumulator with an integer RED.
+ * Histogram (rows a4, a5).  When a run ends (bin edge, end of the unit or range) its fp64 total is
+ * converted once to 64-bit fixed point and added to the (point, bin) accumulator with an integer RED.
  * Integer addition is associative: the result depends neither on which warp walks an item nor on
  * the order of arrival, i.e. bitwise reproducible with no float atomics anywhere (the cut of the
  * events into items is a function of the sizes only).
@@ -41,7 +51,11 @@
  * Component mode (cross-point caching): the launch's points are virtual points (an energy-scale class
  * plus S splittings) and a run is flushed as S + 1 separate sums; finalize.cu combines them per point.
  *
- * Launch.  The spectra kernel is a programmatic dependent of the setup kernel: barriers and the first
+ * Diagnostic instantiation (template flag DBG, phylino_event_bins): the SAME kernels additionally write,
+ * for every event a lane accumulates, the bin it put it in -- through the hint walk, the forward scan, the
+ * whole-batch test, the 2-/4-batch paths and the sub-stream split -- for the bit-exact bin parity test.
+ *
+ * Launch.  The ticket kernel is a programmatic dependent of the setup kernel: barriers and the first
  * event copy are set up while the setup kernel runs; griddepcontrol.wait precedes the first read of a
  * record, a threshold or the work counter.
  */
@@ -52,6 +66,27 @@ namespace phylino {
 namespace {
 
 __device__ __forceinline__ float pos_inf() { return __int_as_float(0x7f800000); }
+
+/* -DPHYLINO_TRACE (never in the shipped build): phase timestamps of the single-launch kernel for timeline work */
+#ifdef PHYLINO_TRACE
+__device__ unsigned long long g_trace[8];
+__device__ unsigned long long g_wtrace[4][256];     /* per-unit timestamps of four sample warps */
+__device__ int g_wn[4];
+__device__ long long g_sub[64][4];                 /* walk_unit sub-phases of the first 64 lanes-0 */
+__device__ unsigned long long g_wend[4096];
+__device__ int g_wunits[4096];
+__device__ __forceinline__ unsigned long long gtime()
+{
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
+#define TRACE_MIN(i) do { if (threadIdx.x == 0) atomicMin(&g_trace[i], gtime()); } while (0)
+#define TRACE_MAX(i) do { if (threadIdx.x == 0) atomicMax(&g_trace[i], gtime()); } while (0)
+#else
+#define TRACE_MIN(i) do { } while (0)
+#define TRACE_MAX(i) do { } while (0)
+#endif
 
 /* ---- per-warp staging of a unit in shared memory: one bulk async copy (TMA engine, no tensor map),
  * completion signalled on an mbarrier that the 32 lanes poll.  (PTX ISA cp.async.bulk / mbarrier.) */
@@ -81,6 +116,26 @@ __device__ __forceinline__ void mbar_wait(unsigned long long *bar, unsigned pari
     } while (!done);
 }
 
+__device__ __forceinline__ unsigned rec_bytes(const DatasetDev &ds)
+{
+    return ds.unit_w ? (unsigned)sizeof(EventBatchU) : (unsigned)sizeof(EventBatchW);
+}
+
+/* address of batch b of the dataset's store */
+__device__ __forceinline__ const void *batch_ptr(const DatasetDev &ds, int b)
+{
+    return static_cast<const char *>(ds.ev) + (size_t)b * rec_bytes(ds);
+}
+
+/* one warp asks L2 for [p, p + bytes): the lines are on their way while the events are walked */
+__device__ __forceinline__ void prefetch_l2(const void *p, size_t bytes, int lane)
+{
+    if (!p) return;
+    const char *c = static_cast<const char *>(p);
+    for (size_t off = (size_t)lane * 128; off < bytes; off += 32 * 128)
+        asm volatile("prefetch.global.L2 [%0];" ::"l"(c + off));
+}
+
 /* run total -> fixed point; values outside the domain become flag bits */
 __device__ __forceinline__ long long to_fixed(double s, double scale, bool bad, unsigned &fl)
 {
@@ -93,13 +148,38 @@ __device__ __forceinline__ long long to_fixed(double s, double scale, bool bad, 
     return __double2ll_rn(y);
 }
 
-/* smallest fp32 v in [safe_lo, safe_hi] (positive, normal) with E'(v) >= edge, +inf if none */
+/* smallest fp32 v in [safe_lo, safe_hi] (positive, normal) with E'(v) >= edge, +inf if none.  E' is
+ * non-decreasing over the fp32 values of the interval (the caller checked), so the answer is unique and any
+ * bracketing search finds it: a Newton guess of the root in fp64, a galloping bracket around it, bisection
+ * inside (a handful of evaluations instead of the ~30 of a bisection over the whole interval). */
 __device__ float threshold_search(double a0, double a1, double a2, double edge, float safe_lo, float safe_hi)
 {
     if (!(safe_lo <= safe_hi)) return pos_inf();
     if (!(escale(a0, a1, a2, (double)safe_hi) >= edge)) return pos_inf();
     if (escale(a0, a1, a2, (double)safe_lo) >= edge) return safe_lo;
     int lo = __float_as_int(safe_lo), hi = __float_as_int(safe_hi);   /* E'(lo) < edge <= E'(hi) */
+    double g = (edge - a0) / a1;
+#pragma unroll
+    for (int it = 0; it < 2; ++it) g -= (escale(a0, a1, a2, g) - edge) / fma(2.0 * a2, g, a1);
+    if (g > (double)safe_lo && g < (double)safe_hi) {
+        const int gi = min(max(__float_as_int(__double2float_rn(g)), lo + 1), hi);
+        int step = 1;
+        if (escale(a0, a1, a2, (double)__int_as_float(gi)) >= edge) {
+            hi = gi;
+            for (;;) {
+                const int c = hi - step;
+                if (c <= lo) break;
+                if (escale(a0, a1, a2, (double)__int_as_float(c)) >= edge) { hi = c; step <<= 1; } else { lo = c; break; }
+            }
+        } else {
+            lo = gi;
+            for (;;) {
+                const int c = lo + step;
+                if (c >= hi) break;
+                if (escale(a0, a1, a2, (double)__int_as_float(c)) >= edge) { hi = c; break; } else { lo = c; step <<= 1; }
+            }
+        }
+    }
     while (hi - lo > 1) {
         int mid = lo + ((hi - lo) >> 1);
         if (escale(a0, a1, a2, (double)__int_as_float(mid)) >= edge) hi = mid; else lo = mid;
@@ -121,9 +201,94 @@ __device__ __forceinline__ int row_of(const SpectraArgs &a, int p)
     return a.comp ? a.vp_class[p] : (a.thr_rows > 1 ? p : 0);
 }
 
-__device__ __forceinline__ const double *theta_of(const SpectraArgs &a, int p)
+__device__ __forceinline__ const double *theta_of(const SpectraArgs &a, const double *params, int p)
 {
-    return a.params + (size_t)(a.comp ? a.class_rep[a.vp_class[p]] : p) * a.n_params;
+    return params + (size_t)(a.comp ? a.class_rep[a.vp_class[p]] : p) * a.n_params;
+}
+
+/* The per-call tables the walk reads: in global memory behind the setup kernel (tickets), in the CTA's own
+ * shared memory in the single-launch kernel. */
+struct Tables {
+    const double *params;   /* [P x n_params]: a.params, or the copy that came with the kernel arguments */
+    const double *rec;      /* [rec_fields x P]: h_k, A_k, P0, bad */
+    const float  *thr;      /* [thr_rows x thr_stride] */
+    const float2 *safe;     /* [thr_rows x n_datasets] */
+};
+
+/* row a1: record of launch point p -> rec[field * P + p] */
+template <int S>
+__device__ __forceinline__ void point_record(const SpectraArgs &a, const double *params, int p, double *rec)
+{
+    if (a.comp) {
+        /* virtual point: slot s computes the half-turn coefficient of (real point, term) vp_src */
+#pragma unroll
+        for (int k = 0; k < S; ++k) {
+            const int src = a.vp_src[(size_t)p * S + k];
+            double A[MAX_TERMS], dm2[MAX_TERMS];
+            osc_terms(a.osc, params + (size_t)(src >> 2) * a.n_params, A, dm2);
+            rec[(size_t)k * a.P + p] = halfturn_coeff(dm2[src & 3]);
+        }
+        return;
+    }
+    const double *theta = params + (size_t)p * a.n_params;
+    double A[MAX_TERMS], dm2[MAX_TERMS];
+    osc_terms(a.osc, theta, A, dm2);
+    double asum = 0.0, half = 0.0;
+#pragma unroll
+    for (int k = 0; k < S; ++k) {
+        rec[(size_t)k * a.P + p] = halfturn_coeff(dm2[k]);
+        rec[(size_t)(S + k) * a.P + p] = A[k];
+        asum += fabs(A[k]);
+        half += A[k];
+    }
+    rec[(size_t)(2 * S) * a.P + p] = 1.0 - 0.5 * half;            /* P0 */
+    /* |P0| + 1/2 sum|A_k| <= 1 + sum|A_k| <= 4 keeps every run total inside the fixed-point range
+     * (phylino.h "Errors": a point beyond this bound reads NaN) */
+    rec[(size_t)(2 * S + 1) * a.P + p] = (asum <= 3.0) ? 0.0 : 1.0;
+}
+
+/* tables of row a3: entry e of threshold row `row` (and the row's validity interval per dataset) */
+__device__ __forceinline__ void threshold_entry(const SpectraArgs &a, const double *params, int row, int e, float *thr,
+                                                float2 *safe)
+{
+    /* only read where idx_a >= 0 */
+    const double *theta = params + (size_t)(a.comp ? a.class_rep[row] : row) * a.n_params;
+    int d = 0;
+    for (int i = 1; i < a.n_datasets; ++i)
+        if (e >= a.ds[i].thr_off) d = i;
+    const DatasetDev &ds = a.ds[d];
+    const int b = e - ds.thr_off;
+    const double edge = ds.edges[b];
+    float slo, shi, t;
+    if (!ds.per_point) {
+        slo = -pos_inf(); shi = pos_inf();      /* E' = v exactly: the table holds for every float */
+        t = __double2float_ru(edge);            /* v >= edge <=> v >= ru(edge) */
+    } else {
+        /* E'(v) computed with the two fma is non-decreasing over the fp32 values of
+         * [v_pos_min, v_max] if the Horner inner value t = a2 v + a1 is positive and the
+         * derivative a1 + 2 a2 v exceeds 2^-20 t at both ends (both are linear in v): between
+         * fp32 neighbours the exact increase then outweighs the rounding of t 2^8-fold
+         * (DESIGN.md "Bit-exact binning with fp32 thresholds"). */
+        double a0, a1, a2;
+        energy_scale_of(ds, theta, a0, a1, a2);
+        double vl = (double)ds.v_pos_min, vh = (double)ds.v_max;
+        double t_lo = fma(a2, vl, a1), t_hi = fma(a2, vh, a1);
+        double g_lo = fma(2.0 * a2, vl, a1), g_hi = fma(2.0 * a2, vh, a1);
+        double tm = fmax(t_lo, t_hi) * 0x1p-20;
+        bool ok = t_lo > 0.0 && t_hi > 0.0 && g_lo >= tm && g_hi >= tm && fabs(a0) < 1.0e300 &&
+                  t_hi < 1.0e300 && ds.v_pos_min >= 1.17549435e-38f && ds.v_pos_min <= ds.v_max;
+        slo = ok ? ds.v_pos_min : pos_inf();
+        shi = ok ? ds.v_max : -pos_inf();
+        t = threshold_search(a0, a1, a2, edge, slo, shi);
+    }
+    thr[(size_t)row * a.thr_stride + e] = t;
+    if (b == 0) safe[(size_t)row * a.n_datasets + d] = make_float2(slo, shi);
+}
+
+/* threshold row entry with the conventions thr[-1] = -inf, thr[B + 1] = +inf */
+__device__ __forceinline__ float thr_at(const float *thr, int B, int i)
+{
+    return i < 0 ? -pos_inf() : (i > B ? pos_inf() : thr[i]);
 }
 
 /* Bin of one event of dataset ds at one point, and the fp32 bound `hi` below which later (larger)
@@ -139,9 +304,9 @@ __device__ __forceinline__ int locate_bin(const DatasetDev &ds, const float *thr
         int lo = -1, up = B + 1;                    /* thr[lo] <= v < thr[up], thr[-1] = -inf, thr[B+1] = +inf */
         while (up - lo > 1) {
             int mid = (lo + up) >> 1;
-            if (__ldg(thr + mid) <= v) lo = mid; else up = mid;
+            if (thr[mid] <= v) lo = mid; else up = mid;
         }
-        hi = lo < B ? __ldg(thr + lo + 1) : pos_inf();
+        hi = lo < B ? thr[lo + 1] : pos_inf();
         return lo;
     }
     double a0, a1, a2;
@@ -150,8 +315,8 @@ __device__ __forceinline__ int locate_bin(const DatasetDev &ds, const float *thr
     return bin_search(ds.edges, B, escale(a0, a1, a2, (double)v));
 }
 
-/* ---- setup kernel: per-point records and threshold rows (row a1 and the tables of row a3) ---------
- * blocks [0, rec_blocks): one thread per point writes rec[field * P + p] = h_k, A_k, P0, bad;
+/* ---- setup kernel (tickets): per-point records and threshold rows (row a1 and the tables of row a3) ----
+ * blocks [0, rec_blocks): one thread per point writes its record;
  * blocks [rec_blocks, rec_blocks + thr_rows): one CTA per threshold row. */
 template <int S>
 __global__ void __launch_bounds__(SETUP_THREADS) setup_kernel(const __grid_constant__ SpectraArgs a, int rec_blocks)
@@ -161,73 +326,15 @@ __global__ void __launch_bounds__(SETUP_THREADS) setup_kernel(const __grid_const
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     if ((int)blockIdx.x < rec_blocks) {
         const int p = blockIdx.x * SETUP_THREADS + threadIdx.x;
-        if (p == 0) *a.counter = 2u * (unsigned)a.n_warps;     /* see spectra_kernel */
-        if (p >= a.P) return;
-        if (a.comp) {
-            /* virtual point: slot s computes the half-turn coefficient of (real point, term) vp_src */
-#pragma unroll
-            for (int k = 0; k < S; ++k) {
-                const int src = a.vp_src[(size_t)p * S + k];
-                double A[MAX_TERMS], dm2[MAX_TERMS];
-                osc_terms(a.osc, a.params + (size_t)(src >> 2) * a.n_params, A, dm2);
-                a.rec[(size_t)k * a.P + p] = halfturn_coeff(dm2[src & 3]);
-            }
-            return;
-        }
-        const double *theta = a.params + (size_t)p * a.n_params;
-        double A[MAX_TERMS], dm2[MAX_TERMS];
-        osc_terms(a.osc, theta, A, dm2);
-        double asum = 0.0, half = 0.0;
-#pragma unroll
-        for (int k = 0; k < S; ++k) {
-            a.rec[(size_t)k * a.P + p] = halfturn_coeff(dm2[k]);
-            a.rec[(size_t)(S + k) * a.P + p] = A[k];
-            asum += fabs(A[k]);
-            half += A[k];
-        }
-        a.rec[(size_t)(2 * S) * a.P + p] = 1.0 - 0.5 * half;            /* P0 */
-        /* |P0| + 1/2 sum|A_k| <= 1 + sum|A_k| <= 4 keeps every run total inside the fixed-point range */
-        a.rec[(size_t)(2 * S + 1) * a.P + p] = (asum <= 3.0) ? 0.0 : 1.0;
+        if (p == 0) *a.counter = 0u;                            /* the work counter of ticket_loop */
+        if (p < a.P) point_record<S>(a, a.params, p, a.rec);
         return;
     }
     const int row = blockIdx.x - rec_blocks;
-    /* only read where idx_a >= 0 */
-    const double *theta = a.params + (size_t)(a.comp ? a.class_rep[row] : row) * a.n_params;
-    for (int e = threadIdx.x; e < a.thr_stride; e += SETUP_THREADS) {
-        int d = 0;
-        for (int i = 1; i < a.n_datasets; ++i)
-            if (e >= a.ds[i].thr_off) d = i;
-        const DatasetDev &ds = a.ds[d];
-        const int b = e - ds.thr_off;
-        const double edge = ds.edges[b];
-        float slo, shi, t;
-        if (!ds.per_point) {
-            slo = -pos_inf(); shi = pos_inf();      /* E' = v exactly: the table holds for every float */
-            t = __double2float_ru(edge);            /* v >= edge <=> v >= ru(edge) */
-        } else {
-            /* E'(v) computed with the two fma is non-decreasing over the fp32 values of
-             * [v_pos_min, v_max] if the Horner inner value t = a2 v + a1 is positive and the
-             * derivative a1 + 2 a2 v exceeds 2^-20 t at both ends (both are linear in v): between
-             * fp32 neighbours the exact increase then outweighs the rounding of t 2^8-fold
-             * (DESIGN.md "Bit-exact binning with fp32 thresholds"). */
-            double a0, a1, a2;
-            energy_scale_of(ds, theta, a0, a1, a2);
-            double vl = (double)ds.v_pos_min, vh = (double)ds.v_max;
-            double t_lo = fma(a2, vl, a1), t_hi = fma(a2, vh, a1);
-            double g_lo = fma(2.0 * a2, vl, a1), g_hi = fma(2.0 * a2, vh, a1);
-            double tm = fmax(t_lo, t_hi) * 0x1p-20;
-            bool ok = t_lo > 0.0 && t_hi > 0.0 && g_lo >= tm && g_hi >= tm && fabs(a0) < 1.0e300 &&
-                      t_hi < 1.0e300 && ds.v_pos_min >= 1.17549435e-38f && ds.v_pos_min <= ds.v_max;
-            slo = ok ? ds.v_pos_min : pos_inf();
-            shi = ok ? ds.v_max : -pos_inf();
-            t = threshold_search(a0, a1, a2, edge, slo, shi);
-        }
-        a.thr[(size_t)row * a.thr_stride + e] = t;
-        if (b == 0) a.safe[(size_t)row * a.n_datasets + d] = make_float2(slo, shi);
-    }
+    for (int e = threadIdx.x; e < a.thr_stride; e += SETUP_THREADS) threshold_entry(a, a.params, row, e, a.thr, a.safe);
 }
 
-/* ---- the hot kernel ---------------------------------------------------------------------------- */
+/* ---- the hot loop ------------------------------------------------------------------------------ */
 
 /* the lane's open run: events of ONE bin seen since the last flush */
 template <int S> struct Run {
@@ -239,8 +346,30 @@ template <int S> struct Run {
                      * end of the run does not wait for it; meaningful only while hi is a table threshold */
 };
 
+template <int S> __device__ __forceinline__ void run_reset(Run<S> &r)
+{
+#pragma unroll
+    for (int k = 0; k < S; ++k) r.C[k] = 0.0;
+    r.W = 0.0;
+    r.cur = -1;
+    r.hi = -pos_inf();
+    r.hi2 = pos_inf();
+}
+
+/* diagnostic instantiation: the bin the hot loop gave event j of dataset batch gb at point p */
+template <bool DBG>
+__device__ __forceinline__ void dbg_mark(const SpectraArgs &a, const DatasetDev &ds, int p, bool active, int gb, int j,
+                                         int cur)
+{
+    if (!DBG) return;
+    const long long i = (long long)gb * EB + j;
+    if (!active || i >= ds.n_events) return;
+    a.dbg_bins[(size_t)p * a.total_events + ds.ev_off + ds.perm[i]] = (cur >= 0 && cur < ds.n_bins) ? cur : -1;
+}
+
 template <int S>
-__device__ __forceinline__ void flush_run(const SpectraArgs &a, const DatasetDev &ds, int p, bool active, Run<S> &r)
+__device__ __forceinline__ void flush_run(const SpectraArgs &a, const Tables &T, const DatasetDev &ds, int p,
+                                          bool active, Run<S> &r)
 {
     if (a.comp && active && r.cur >= 0 && r.cur < ds.n_bins) {
         /* component mode: W and every C_k go to cells of their own (the amplitudes come later) */
@@ -253,10 +382,10 @@ __device__ __forceinline__ void flush_run(const SpectraArgs &a, const DatasetDev
             if (fl) atomicOr(a.flags + cell + (size_t)j * a.total_bins, fl);
         }
     } else if (active && r.cur >= 0 && r.cur < ds.n_bins) {
-        double tot = a.rec[(size_t)(2 * S) * a.P + p] * r.W;                 /* P0 W */
+        double tot = T.rec[(size_t)(2 * S) * a.P + p] * r.W;                 /* P0 W */
 #pragma unroll
-        for (int k = 0; k < S; ++k) tot = fma(a.rec[(size_t)(S + k) * a.P + p], r.C[k], tot);
-        const bool bad = a.rec[(size_t)(2 * S + 1) * a.P + p] != 0.0;
+        for (int k = 0; k < S; ++k) tot = fma(T.rec[(size_t)(S + k) * a.P + p], r.C[k], tot);
+        const bool bad = T.rec[(size_t)(2 * S + 1) * a.P + p] != 0.0;
         unsigned fl;
         const long long q = to_fixed(tot, ds.fx_scale, bad, fl);
         const size_t cell = (size_t)p * a.total_bins + ds.bin_off + r.cur;
@@ -268,55 +397,98 @@ __device__ __forceinline__ void flush_run(const SpectraArgs &a, const DatasetDev
     r.W = 0.0;
 }
 
-/* The flush at the end of a unit when the group has at most 16 points: the 32 / PL sub-streams of a point
- * usually end in the same bin, and 32 lanes of every resident warp adding to the same one or two cells
+/* the rare flush: sub-streams of a point end in different cells (a bin edge inside the unit).  For every lane the
+ * sum over the sub-streams of its point that share its cell, and whether it is the first of them.  Not inlined
+ * (see walk_batch_slow). */
+template <int S> struct SubSums { long long sum[S + 1]; bool first; };
+
+template <int S>
+__device__ __noinline__ SubSums<S> substream_sums_general(unsigned long long cell, bool live, int lg, int lane, int nq,
+                                                          SubSums<S> q)
+{
+    SubSums<S> out;
+#pragma unroll
+    for (int j = 0; j <= S; ++j) out.sum[j] = 0;
+    out.first = true;
+    const int pl = lane & ((1 << lg) - 1);
+#pragma unroll 1
+    for (int src = pl; src < 32; src += 1 << lg) {              /* the sub-streams of this lane's point */
+        const unsigned long long c = __shfl_sync(0xffffffffu, cell, src);
+        const bool same = live && c == cell;
+        if (same && src < lane) out.first = false;
+#pragma unroll
+        for (int j = 0; j <= S; ++j) {
+            if (j < nq) {                                        /* nq is warp-uniform */
+                const long long v = __shfl_sync(0xffffffffu, q.sum[j], src);
+                if (same) out.sum[j] += v;
+            }
+        }
+    }
+    return out;
+}
+
+/* The flush at the end of a unit / range when the group has at most 16 points: the 32 / PL sub-streams of a
+ * point usually end in the same bin, and 32 lanes of every resident warp adding to the same one or two cells
  * would queue at the L2 atomic unit (same-address atomics: a 6e6-event, 1-point call spent 0.45 ms there).
  * Every lane converts its run to fixed point as usual; the integers of the lanes that share a cell are
  * summed over the sub-streams with shuffles (exact, so the bits are those of the separate REDs) and the
  * first lane of each cell issues one RED.  All 32 lanes call this together. */
 template <int S>
-__device__ __forceinline__ void flush_run_substreams(const SpectraArgs &a, const DatasetDev &ds, int p, bool active,
-                                                     int lg, int lane, Run<S> &r)
+__device__ __forceinline__ void flush_run_substreams(const SpectraArgs &a, const Tables &T, const DatasetDev &ds, int p,
+                                                     bool active, int lg, int lane, Run<S> &r)
 {
     const bool live = active && r.cur >= 0 && r.cur < ds.n_bins;
-    const int nq = a.comp ? S + 1 : 1;
+    const bool comp = a.comp != 0;                              /* warp-uniform */
+    const int pl = lane & ((1 << lg) - 1);
+    /* the usual case: the sub-streams of every point end in the same bin (the cell is a function of point and bin) */
+    const int my_bin = live ? r.cur : -1;
+    const bool uniform = __all_sync(0xffffffffu, my_bin == __shfl_sync(0xffffffffu, my_bin, pl));
     long long q[S + 1];
     unsigned fl[S + 1];
 #pragma unroll
     for (int j = 0; j <= S; ++j) { q[j] = 0; fl[j] = 0; }
     unsigned long long cell = ~0ull;
     if (live) {
-        if (a.comp) {
+        if (comp) {
             cell = (unsigned long long)p * (S + 1) * a.total_bins + ds.bin_off + r.cur;
 #pragma unroll
             for (int j = 0; j <= S; ++j) q[j] = to_fixed(j == 0 ? r.W : r.C[j - 1], ds.fx_scale, false, fl[j]);
         } else {
-            double tot = a.rec[(size_t)(2 * S) * a.P + p] * r.W;
+            double tot = T.rec[(size_t)(2 * S) * a.P + p] * r.W;
 #pragma unroll
-            for (int k = 0; k < S; ++k) tot = fma(a.rec[(size_t)(S + k) * a.P + p], r.C[k], tot);
+            for (int k = 0; k < S; ++k) tot = fma(T.rec[(size_t)(S + k) * a.P + p], r.C[k], tot);
             cell = (unsigned long long)p * a.total_bins + ds.bin_off + r.cur;
-            q[0] = to_fixed(tot, ds.fx_scale, a.rec[(size_t)(2 * S + 1) * a.P + p] != 0.0, fl[0]);
+            q[0] = to_fixed(tot, ds.fx_scale, T.rec[(size_t)(2 * S + 1) * a.P + p] != 0.0, fl[0]);
         }
     }
-    long long sum[S + 1];
+    bool first;
+    if (uniform) {
+        /* a butterfly over the sub-stream bits of the lane index (exact integers: any order gives the same bits) */
+        for (int o = 16; o >= (1 << lg); o >>= 1) {
+            q[0] += __shfl_xor_sync(0xffffffffu, q[0], o);
+            if (comp) {
 #pragma unroll
-    for (int j = 0; j <= S; ++j) sum[j] = 0;
-    bool first = true;
-    const int pl = lane & ((1 << lg) - 1);
-    for (int src = pl; src < 32; src += 1 << lg) {              /* the sub-streams of this lane's point */
-        const unsigned long long c = __shfl_sync(0xffffffffu, cell, src);
-        const bool same = live && c == cell;
-        if (same && src < lane) first = false;
-#pragma unroll
-        for (int j = 0; j <= S; ++j) {
-            const long long v = __shfl_sync(0xffffffffu, q[j], src);
-            if (same && j < nq) sum[j] += v;
+                for (int j = 1; j <= S; ++j) q[j] += __shfl_xor_sync(0xffffffffu, q[j], o);
+            }
         }
+        first = lane == pl;
+    } else {
+        SubSums<S> qs;
+#pragma unroll
+        for (int j = 0; j <= S; ++j) qs.sum[j] = q[j];
+        qs.first = true;
+        const SubSums<S> g = substream_sums_general<S>(cell, live, lg, lane, comp ? S + 1 : 1, qs);
+#pragma unroll
+        for (int j = 0; j <= S; ++j) q[j] = g.sum[j];
+        first = g.first;
     }
     if (live) {
-        for (int j = 0; j < nq; ++j) {
-            if (first && sum[j]) atomicAdd((unsigned long long *)a.acc + cell + (size_t)j * a.total_bins, (unsigned long long)sum[j]);
-            if (fl[j]) atomicOr(a.flags + cell + (size_t)j * a.total_bins, fl[j]);
+#pragma unroll
+        for (int j = 0; j <= S; ++j) {
+            if (j == 0 || comp) {
+                if (first && q[j]) atomicAdd((unsigned long long *)a.acc + cell + (size_t)j * a.total_bins, (unsigned long long)q[j]);
+                if (fl[j]) atomicOr(a.flags + cell + (size_t)j * a.total_bins, fl[j]);
+            }
         }
     }
 #pragma unroll
@@ -324,80 +496,34 @@ __device__ __forceinline__ void flush_run_substreams(const SpectraArgs &a, const
     r.W = 0.0;
 }
 
-/* threshold row entry with the conventions thr[-1] = -inf, thr[B + 1] = +inf */
-__device__ __forceinline__ float thr_at(const float *thr, int B, int i)
-{
-    return i < 0 ? -pos_inf() : (i > B ? pos_inf() : __ldg(thr + i));
-}
-
-/* One batch of the lane's stream (rows a2-a4). */
+/* Open the lane's run at its first event v0 (dataset batch gb): start from the load-time hint (the bin, under
+ * the identity energy scale, of an event at most HINT_BATCHES batches earlier; loaded by the caller one item
+ * ahead, off the critical path) and step to the bin the lane's
+ * own thresholds give -- the same decision as the binary search of locate_bin, usually with two independent
+ * loads and no dependent one; a lane whose bin lies far from the hint falls back to the search. */
 template <int S>
-__device__ __forceinline__ void walk_batch(const SpectraArgs &a, const DatasetDev &ds, const EventBatch *bp,
-                                           const double (&h)[S], const float *thr, float2 safe, int p, bool active,
-                                           Run<S> &r)
+__device__ __forceinline__ void open_run(const DatasetDev &ds, const float *thr, float2 safe, float v0, int hint,
+                                         Run<S> &r)
 {
+    if (!(v0 >= safe.x && v0 <= safe.y)) return;        /* the first walk_batch locates it in fp64 */
     const int B = ds.n_bins;
-    double x[EB], w[EB];
-    {
-        const double2 *q = reinterpret_cast<const double2 *>(bp);
-#pragma unroll
-        for (int j = 0; j < EB / 2; ++j) {
-            double2 t = q[j], u = q[EB / 2 + j];
-            x[2 * j] = t.x; x[2 * j + 1] = t.y;
-            w[2 * j] = u.x; w[2 * j + 1] = u.y;
-        }
-    }
-    const float v_last = bp->v[EB - 1];
-
-    /* row a2: g_k of every event of the batch */
-    double gk[S][EB];
-#pragma unroll
-    for (int j = 0; j < EB; ++j)
-#pragma unroll
-        for (int k = 0; k < S; ++k) gk[k][j] = half_cos_halfturns(h[k], x[j]);
-
-    if (v_last < r.hi) {
-        /* rows a3 + a4: the store is sorted, so the whole batch lies in the run's bin */
-#pragma unroll
-        for (int j = 0; j < EB; ++j)
-#pragma unroll
-            for (int k = 0; k < S; ++k) r.C[k] = fma(w[j], gk[k][j], r.C[k]);
-        r.W += bp->wsum;
-    } else {
-        /* a run ends inside the batch (or none is open yet): walk its events one by one */
-        const float4 v4 = *reinterpret_cast<const float4 *>(bp->v);
-        const float v[EB] = {v4.x, v4.y, v4.z, v4.w};
-#pragma unroll
-        for (int j = 0; j < EB; ++j) {
-            if (!(v[j] < r.hi)) {
-                int b;
-                float nhi;
-                if (r.hi > -pos_inf() && r.hi < pos_inf() && v[j] <= safe.y) {
-                    /* r.hi = thr[cur + 1] <= v inside the table's interval: scan forward */
-                    b = r.cur + 1;
-                    nhi = r.hi2;
-                    while (b < B && !(v[j] < nhi)) { ++b; nhi = thr_at(thr, B, b + 1); }
-                } else {
-                    b = locate_bin(ds, thr, safe, theta_of(a, p), v[j], nhi);
-                }
-                if (b != r.cur) {
-                    flush_run<S>(a, ds, p, active, r);
-                    r.cur = b;
-                }
-                r.hi = nhi;
-                r.hi2 = thr_at(thr, B, b + 2);
-            }
-#pragma unroll
-            for (int k = 0; k < S; ++k) r.C[k] = fma(w[j], gk[k][j], r.C[k]);
-            r.W += w[j];
-        }
-    }
+    int b = max(-1, min(hint, B));
+    float lo = thr_at(thr, B, b), hi = thr_at(thr, B, b + 1);
+    int steps = 0;
+    while (b >= 0 && v0 < lo && steps < 8) { --b; hi = lo; lo = thr_at(thr, B, b); ++steps; }
+    while (b < B && !(v0 < hi) && steps < 8) { ++b; hi = thr_at(thr, B, b + 1); ++steps; }
+    if (steps >= 8) b = locate_bin(ds, thr, safe, nullptr, v0, hi);     /* inside the table's interval: theta unused */
+    r.cur = b;
+    r.hi = hi;
+    r.hi2 = thr_at(thr, B, b + 2);
 }
 
 /* K consecutive batches known to lie inside the lane's open run (the store is sorted: the last
  * event of the last batch is below r.hi): rows a2 + a4 only, straight-line. */
-template <int S, bool UW, int K>
-__device__ __forceinline__ void walk_inside(const EventBatch *bp, const double (&h)[S], Run<S> &r)
+template <int S, bool UW, int K, bool DBG>
+__device__ __forceinline__ void walk_inside(const SpectraArgs &a, const DatasetDev &ds,
+                                            const typename RecOf<UW>::type *bp, int gb, const double (&h)[S], int p,
+                                            bool active, Run<S> &r)
 {
 #pragma unroll
     for (int u = 0; u < K; ++u) {
@@ -406,8 +532,8 @@ __device__ __forceinline__ void walk_inside(const EventBatch *bp, const double (
         for (int j = 0; j < EB / 2; ++j) {
             const double2 t = q[j];
             if (UW) {
-                /* every weight of the dataset is exactly 1 (the padding, weight 0, sits behind a NaN E_vis
-                 * and never reaches this path): 1 * g + C == g + C bit for bit, and w is not loaded */
+                /* every weight of the dataset is exactly 1 (the padding sits behind a NaN E_vis and never
+                 * reaches this path): 1 * g + C == g + C bit for bit, and no weight is stored */
 #pragma unroll
                 for (int k = 0; k < S; ++k) r.C[k] += half_cos_halfturns(h[k], t.x);
 #pragma unroll
@@ -420,270 +546,182 @@ __device__ __forceinline__ void walk_inside(const EventBatch *bp, const double (
                 for (int k = 0; k < S; ++k) r.C[k] = fma(w.y, half_cos_halfturns(h[k], t.y), r.C[k]);
             }
         }
-        if (!UW) r.W += bp[u].wsum;
+        if (!UW) r.W += reinterpret_cast<const EventBatchW *>(bp + u)->wsum;
+        if (DBG)
+            for (int j = 0; j < EB; ++j) dbg_mark<DBG>(a, ds, p, active, gb + u, j, r.cur);
     }
     if (UW) r.W += (double)(EB * K);                /* whole numbers: the same bits as K separate adds */
 }
 
-/* One warp, the nb batches of one unit of dataset ds staged at `unit` (SHARED memory), point group g
- * (points 32 g ... 32 g + 31).  FULL: the group has more than 16 points, every lane walks all batches. */
-template <int S, bool FULL, bool UW>
-__device__ __forceinline__ void walk_unit(const SpectraArgs &a, const DatasetDev &ds, int d, const EventBatch *unit,
-                                          int nb, int g, int lane)
+/* the half-turn coefficients of the lane's point, by value (they travel to the non-inlined slow path) */
+template <int S> struct Coef { double h[S]; };
+
+/* A batch in which a run ends (or none is open yet): its events one by one (rows a2-a4).  Rare -- once per
+ * bin edge and lane -- and therefore NOT inlined and not unrolled: the hot loop stays small, and a warp that
+ * meets an edge fetches few instruction lines it has not seen before (a cold instruction line costs as much as
+ * a DRAM access; round 2 timeline: warps that met an edge finished 20 us late).  Everything by value: the run
+ * must stay in registers in the caller. */
+template <int S, bool UW, bool DBG>
+__device__ __noinline__ Run<S> walk_batch_slow(const SpectraArgs &a, Tables T, const DatasetDev &ds,
+                                               const typename RecOf<UW>::type *bp, int gb, Coef<S> c,
+                                               const float *thr, float2 safe, int p, bool active, Run<S> r)
 {
-    /* lane -> (point, sub-stream): a group of np < 32 points uses PL = 2^ceil(log2 np) point lanes
-     * and splits the batches into NS = 32 / PL contiguous sub-streams */
-    /* FULL: more than 16 points, so every lane walks all batches; lanes past the last point shadow point
-     * 32 g and never flush */
-    int my0 = 0, mine = nb, iters = nb, lg = 5;
+    const int B = ds.n_bins;
+#pragma unroll 1
+    for (int j = 0; j < EB; ++j) {
+        const float v = bp->v[j];
+        if (!(v < r.hi)) {
+            int b;
+            float nhi;
+            if (r.hi > -pos_inf() && r.hi < pos_inf() && v <= safe.y) {
+                /* r.hi = thr[cur + 1] <= v inside the table's interval: scan forward */
+                b = r.cur + 1;
+                nhi = r.hi2;
+                while (b < B && !(v < nhi)) { ++b; nhi = thr_at(thr, B, b + 1); }
+            } else {
+                b = locate_bin(ds, thr, safe, theta_of(a, T.params, p), v, nhi);
+            }
+            if (b != r.cur) {
+                flush_run<S>(a, T, ds, p, active, r);
+                r.cur = b;
+            }
+            r.hi = nhi;
+            r.hi2 = thr_at(thr, B, b + 2);
+        }
+        /* the padding of the last batch (E_vis = NaN, so it is in no bin): weight 0 in a weighted store,
+         * skipped by index in a unit-weight one */
+        const bool pad = UW && (long long)gb * EB + j >= ds.n_events;
+        const double x = bp->x[j];
+        double w = 1.0;
+        if (!UW) w = reinterpret_cast<const EventBatchW *>(bp)->w[j];
+#pragma unroll
+        for (int k = 0; k < S; ++k) {
+            const double g = half_cos_halfturns(c.h[k], x);
+            if (UW) { if (!pad) r.C[k] += g; }          /* 1 * g + C == g + C bit for bit */
+            else    r.C[k] = fma(w, g, r.C[k]);
+        }
+        if (UW) { if (!pad) r.W += 1.0; }
+        else    r.W += w;
+        dbg_mark<DBG>(a, ds, p, active, gb, j, r.cur);
+    }
+    return r;
+}
+
+/* One batch of the lane's stream (rows a2-a4); gb: its index in the dataset. */
+template <int S, bool UW, bool DBG>
+__device__ __forceinline__ void walk_batch(const SpectraArgs &a, const Tables &T, const DatasetDev &ds,
+                                           const typename RecOf<UW>::type *bp, int gb, const double (&h)[S],
+                                           const float *thr, float2 safe, int p, bool active, Run<S> &r)
+{
+    if (bp->v[EB - 1] < r.hi) {
+        /* rows a3 + a4: the store is sorted, so the whole batch lies in the run's bin (a padding event has
+         * E_vis = NaN and fails the test: it never comes here) */
+        walk_inside<S, UW, 1, DBG>(a, ds, bp, gb, h, p, active, r);
+    } else {
+        Coef<S> c;
+#pragma unroll
+        for (int k = 0; k < S; ++k) c.h[k] = h[k];
+        r = walk_batch_slow<S, UW, DBG>(a, T, ds, bp, gb, c, thr, safe, p, active, r);
+    }
+}
+
+/* `mine` consecutive batches of the lane's stream starting at bp (dataset batch gb): 4, 2 or 1 at a time */
+template <int S, bool UW, bool DBG>
+__device__ __forceinline__ void walk_stretch(const SpectraArgs &a, const Tables &T, const DatasetDev &ds,
+                                             const typename RecOf<UW>::type *bp, int gb, int mine, const double (&h)[S],
+                                             const float *thr, float2 safe, int p, bool active, Run<S> &r)
+{
+    int i = 0;
+#pragma unroll 1
+    while (i < mine) {
+        if (i + 4 <= mine && bp[3].v[EB - 1] < r.hi) {
+            walk_inside<S, UW, 4, DBG>(a, ds, bp, gb + i, h, p, active, r);
+            i += 4;
+            bp += 4;
+        } else if (i + 2 <= mine && bp[1].v[EB - 1] < r.hi) {
+            walk_inside<S, UW, 2, DBG>(a, ds, bp, gb + i, h, p, active, r);
+            i += 2;
+            bp += 2;
+        } else {
+            walk_batch<S, UW, DBG>(a, T, ds, bp, gb + i, h, thr, safe, p, active, r);
+            ++i;
+            ++bp;
+        }
+    }
+}
+
+/* One warp, the nb batches [b0, b0 + nb) of dataset ds staged at `unit` (SHARED memory), point group g
+ * (points 32 g ... 32 g + 31).  FULL: the group has more than 16 points, every lane walks all batches. */
+/* lane -> (point, sub-stream) for a group of np <= 16 points: PL = 2^lg >= np point lanes, the nb batches of a
+ * unit split into NS = 32 / PL contiguous sub-streams; this lane's is [my0, my0 + mine) */
+__device__ __forceinline__ void substream_of(int np, int lane, int nb, int &lg, int &pl, int &my0, int &mine)
+{
+    lg = np <= 1 ? 0 : 32 - __clz(np - 1);
+    pl = lane & ((1 << lg) - 1);
+    const int s = lane >> lg;
+    my0 = (nb * s) >> (5 - lg);
+    mine = ((nb * (s + 1)) >> (5 - lg)) - my0;
+}
+
+/* the hint a lane needs to open its run in unit [b0, b0 + nb) of dataset ds (group of np points; np > 16: all
+ * lanes start at b0) */
+__device__ __forceinline__ int load_hint(const DatasetDev &ds, int np, int lane, int b0, int nb)
+{
+    int my0 = 0;
+    if (np <= 16) {
+        int lg, pl, mine;
+        substream_of(np, lane, nb, lg, pl, my0, mine);
+    }
+    return __ldg(ds.hint + (b0 + my0) / HINT_BATCHES);
+}
+
+/* One warp, the nb batches [b0, b0 + nb) of dataset ds staged at `unit` (SHARED memory), point group g
+ * (points 32 g ... 32 g + 31).  FULL: the group has more than 16 points, every lane walks all batches; lanes past
+ * the last point shadow point 32 g and never flush.  hint: load_hint() of this lane for this unit and group. */
+template <int S, bool FULL, bool UW, bool DBG>
+__device__ __forceinline__ void walk_unit(const SpectraArgs &a, const Tables &T, const DatasetDev &ds, int d,
+                                          const void *unit, int b0, int nb, int g, int lane, int hint)
+{
+    typedef typename RecOf<UW>::type Rec;
+    int my0 = 0, mine = nb, lg = 5;
     bool active = 32 * g + lane < a.P;
     int p = 32 * g + (active ? lane : 0);
     if (!FULL) {
         const int np = min(32, a.P - 32 * g);
-        int PL = 1;
-        lg = 0;
-        while (PL < np) { PL <<= 1; ++lg; }
-        const int NS = 32 / PL;
-        const int pl = lane & (PL - 1), s = lane / PL;
+        int pl;
+        substream_of(np, lane, nb, lg, pl, my0, mine);
         active = pl < np;
         p = 32 * g + (active ? pl : 0);
-        my0 = nb * s / NS;
-        mine = nb * (s + 1) / NS - my0;
-        iters = (nb + NS - 1) / NS;                        /* >= mine for every lane */
     }
 
     double h[S];
 #pragma unroll
-    for (int k = 0; k < S; ++k) h[k] = a.rec[(size_t)k * a.P + p];
+    for (int k = 0; k < S; ++k) h[k] = T.rec[(size_t)k * a.P + p];
     const int row = row_of(a, p);
-    const float *thr = a.thr + (size_t)row * a.thr_stride + ds.thr_off;
-    const float2 safe = a.safe[(size_t)row * a.n_datasets + d];
-    const int B = ds.n_bins;
+    const float *thr = T.thr + (size_t)row * a.thr_stride + ds.thr_off;
+    const float2 safe = T.safe[(size_t)row * a.n_datasets + d];
 
+#ifdef PHYLINO_TRACE
+    const long long q0 = clock64();
+#endif
     Run<S> r;
-#pragma unroll
-    for (int k = 0; k < S; ++k) r.C[k] = 0.0;
-    r.W = 0.0;
-    r.cur = -1;
-    r.hi = -pos_inf();
-    r.hi2 = pos_inf();
-
-    const EventBatch *bp = unit + my0;
-    if (mine > 0) {
-        /* open the run at the lane's first event: start from the load-time hint (its bin under the
-         * identity energy scale) and step to the bin the lane's own thresholds give -- the same
-         * decision as the binary search of locate_bin, usually without a single dependent load */
-        const float v0 = bp->v[0];
-        if (v0 >= safe.x && v0 <= safe.y) {
-            int b = max(-1, min(bp->bin0, B));
-            float lo = thr_at(thr, B, b), hi = thr_at(thr, B, b + 1);
-            while (b >= 0 && v0 < lo) { --b; hi = lo; lo = thr_at(thr, B, b); }
-            while (b < B && !(v0 < hi)) { ++b; hi = thr_at(thr, B, b + 1); }
-            r.cur = b;
-            r.hi = hi;
-            r.hi2 = thr_at(thr, B, b + 2);
-        }
-    }
-    if (FULL) {
-        int i = 0;
-#pragma unroll 1
-        while (i < nb) {
-            if (i + 4 <= nb && bp[3].v[EB - 1] < r.hi) {
-                walk_inside<S, UW, 4>(bp, h, r);
-                i += 4;
-                bp += 4;
-            } else if (i + 2 <= nb && bp[1].v[EB - 1] < r.hi) {
-                walk_inside<S, UW, 2>(bp, h, r);
-                i += 2;
-                bp += 2;
-            } else {
-                walk_batch<S>(a, ds, bp, h, thr, safe, p, active, r);
-                ++i;
-                ++bp;
-            }
-        }
-    } else {
-#pragma unroll 1
-        for (int i = 0; i < iters; ++i, ++bp) {
-            if (i >= mine) continue;
-            walk_batch<S>(a, ds, bp, h, thr, safe, p, active, r);
-        }
-    }
-    if (FULL) flush_run<S>(a, ds, p, active, r);
-    else      flush_run_substreams<S>(a, ds, p, active, lg, lane, r);
-}
-
-/* ---- static schedule: ONE contiguous range of batches per warp, runs carried across units ------------
- * A run is "the events of one bin at one point", not "adjacent events": a lane may keep its run open
- * across consecutive units (its events stay sorted), so a warp that owns a contiguous range pays the
- * group prologue and the flush once per (range, group) instead of once per (unit, group), and there is
- * no ticket, no tail of unequal items: every warp holds the same number of batches.  The units of the
- * range stream through the warp's two buffers; the copy of the next unit (of this range, or the first
- * unit of what the warp walks next) is in flight while a unit is walked. */
-struct Pipe {
-    EventBatch *buf0;               /* the warp's two unit buffers */
-    unsigned long long *bars;       /* its two mbarriers */
-    int b;                          /* buffer that holds (or will hold) the unit walked next */
-    unsigned phase;
-};
-
-/* one segment [B0, B1) of dataset d for point group g; (nd, n0, n1): the unit to copy when the last unit of
- * this segment is being walked (n0 < 0: nothing follows) */
-template <int S, bool FULL, bool UW>
-__device__ __forceinline__ void walk_range(const SpectraArgs &a, int d, int B0, int B1, int g, int lane, Pipe &pp,
-                                           int nd, int n0, int n1)
-{
-    const DatasetDev &ds = a.ds[d];
-    int lg = 5;
-    bool active = 32 * g + lane < a.P;
-    int p = 32 * g + (active ? lane : 0), s = 0;
-    if (!FULL) {
-        const int np = min(32, a.P - 32 * g);
-        lg = np <= 1 ? 0 : 32 - __clz(np - 1);
-        const int pl = lane & ((1 << lg) - 1);
-        s = lane >> lg;
-        active = pl < np;
-        p = 32 * g + (active ? pl : 0);
-    }
-    double h[S];
-#pragma unroll
-    for (int k = 0; k < S; ++k) h[k] = a.rec[(size_t)k * a.P + p];
-    const int row = row_of(a, p);
-    const float *thr = a.thr + (size_t)row * a.thr_stride + ds.thr_off;
-    const float2 safe = a.safe[(size_t)row * a.n_datasets + d];
-    const int B = ds.n_bins, U = a.unit_batches;
-
-    Run<S> r;
-#pragma unroll
-    for (int k = 0; k < S; ++k) r.C[k] = 0.0;
-    r.W = 0.0;
-    r.cur = -1;
-    r.hi = -pos_inf();
-    r.hi2 = pos_inf();
-
-#pragma unroll 1
-    for (int off = B0; off < B1; off += U) {
-        const int nb = min(U, B1 - off);
-        if (lane == 0) {
-            /* the other buffer was last read one unit ago (every lane has passed the __syncwarp below) */
-            int cd = d, c0 = off + U, c1 = min(off + 2 * U, B1);
-            if (c0 >= B1) { cd = nd; c0 = n0; c1 = n1; }
-            if (c0 >= 0)
-                bulk_load(pp.buf0 + (pp.b ^ 1) * U, a.ds[cd].ev + c0, (unsigned)(c1 - c0) * (unsigned)sizeof(EventBatch),
-                          pp.bars + (pp.b ^ 1));
-        }
-        mbar_wait(pp.bars + pp.b, (pp.phase >> pp.b) & 1u);
-        pp.phase ^= 1u << pp.b;
-        int my0 = 0, mine = nb;
-        if (!FULL) {
-            my0 = (nb * s) >> (5 - lg);
-            mine = ((nb * (s + 1)) >> (5 - lg)) - my0;
-        }
-        const EventBatch *bp = pp.buf0 + pp.b * U + my0;
-        if (off == B0 && mine > 0) {
-            /* open the run at the lane's first event from the load-time hint (see walk_unit) */
-            const float v0 = bp->v[0];
-            if (v0 >= safe.x && v0 <= safe.y) {
-                int bb = max(-1, min(bp->bin0, B));
-                float lo = thr_at(thr, B, bb), hi = thr_at(thr, B, bb + 1);
-                while (bb >= 0 && v0 < lo) { --bb; hi = lo; lo = thr_at(thr, B, bb); }
-                while (bb < B && !(v0 < hi)) { ++bb; hi = thr_at(thr, B, bb + 1); }
-                r.cur = bb;
-                r.hi = hi;
-                r.hi2 = thr_at(thr, B, bb + 2);
-            }
-        }
-        int i = 0;
-#pragma unroll 1
-        while (i < mine) {
-            if (i + 4 <= mine && bp[3].v[EB - 1] < r.hi) {
-                walk_inside<S, UW, 4>(bp, h, r);
-                i += 4;
-                bp += 4;
-            } else if (i + 2 <= mine && bp[1].v[EB - 1] < r.hi) {
-                walk_inside<S, UW, 2>(bp, h, r);
-                i += 2;
-                bp += 2;
-            } else {
-                walk_batch<S>(a, ds, bp, h, thr, safe, p, active, r);
-                ++i;
-                ++bp;
-            }
-        }
-        __syncwarp();                                   /* this unit's reads are over before its buffer is refilled */
-        pp.b ^= 1;
-    }
-    if (FULL) flush_run<S>(a, ds, p, active, r);
-    else      flush_run_substreams<S>(a, ds, p, active, lg, lane, r);
-}
-
-/* first (dataset, segment) at or after dataset d0 that the global batch range [G0, G1) touches */
-__device__ __forceinline__ bool next_segment(const SpectraArgs &a, long long G0, long long G1, int d0, int &d, int &B0,
-                                             int &B1)
-{
-    long long off = 0;
-    for (int i = 0; i < a.n_datasets; ++i) {
-        const long long nb = a.ds[i].n_batches;
-        if (i >= d0) {
-            const long long lo = max(G0, off), hi = min(G1, off + nb);
-            if (lo < hi) { d = i; B0 = (int)(lo - off); B1 = (int)(hi - off); return true; }
-        }
-        off += nb;
-    }
-    return false;
-}
-
-template <int S>
-__global__ void __launch_bounds__(WARPS * 32, 4) spectra_static_kernel(const __grid_constant__ SpectraArgs a)
-{
-    extern __shared__ __align__(128) unsigned char stage[];       /* [WARPS][2][unit_batches] EventBatch */
-    __shared__ unsigned long long bars[WARPS][2];
-    const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
-    const long long nW = (long long)gridDim.x * WARPS, w = (long long)blockIdx.x * WARPS + wib;
-    const int n_groups = (a.P + 31) >> 5, U = a.unit_batches;
-    long long total = 0;
-    for (int i = 0; i < a.n_datasets; ++i) total += a.ds[i].n_batches;
-    const long long G0 = total * w / nW, G1 = total * (w + 1) / nW;       /* this warp's batches, all datasets */
-    Pipe pp;
-    pp.buf0 = reinterpret_cast<EventBatch *>(stage) + (size_t)(2 * wib) * U;
-    pp.bars = &bars[wib][0];
-    pp.b = 0;
-    pp.phase = 0u;
-    if (lane == 0) {
-        mbar_init(&bars[wib][0], 1);
-        mbar_init(&bars[wib][1], 1);
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    }
-    __syncwarp();
-    int fd, f0, f1;
-    const bool any = next_segment(a, G0, G1, 0, fd, f0, f1);
-    if (any && lane == 0)
-        bulk_load(pp.buf0, a.ds[fd].ev + f0, (unsigned)(min(f0 + U, f1) - f0) * (unsigned)sizeof(EventBatch), pp.bars);
-    asm volatile("griddepcontrol.wait;" ::: "memory");
-    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
-    if (!any) return;
-#pragma unroll 1
-    for (int g = 0; g < n_groups; ++g) {
-        int d, B0, B1;
-        bool more = next_segment(a, G0, G1, 0, d, B0, B1);
-#pragma unroll 1
-        while (more) {
-            /* what follows this segment: the next dataset's segment, else the first segment again for the
-             * next group, else nothing */
-            int nd, n0, n1, e1;
-            const bool nxt = next_segment(a, G0, G1, d + 1, nd, n0, e1);
-            if (!nxt) {
-                if (g + 1 < n_groups) { nd = fd; n0 = f0; e1 = f1; } else { nd = 0; n0 = -1; e1 = -1; }
-            }
-            n1 = n0 < 0 ? -1 : min(n0 + U, e1);
-            const DatasetDev &ds = a.ds[d];
-            if (32 * g + 16 >= a.P) walk_range<S, false, false>(a, d, B0, B1, g, lane, pp, nd, n0, n1);
-            else if (ds.unit_w)    walk_range<S, true, true>(a, d, B0, B1, g, lane, pp, nd, n0, n1);
-            else                   walk_range<S, true, false>(a, d, B0, B1, g, lane, pp, nd, n0, n1);
-            more = nxt;
-            if (nxt) { d = nd; B0 = n0; B1 = e1; }
-        }
-    }
+    run_reset<S>(r);
+    const Rec *bp = static_cast<const Rec *>(unit) + my0;
+    if (mine > 0) open_run<S>(ds, thr, safe, bp->v[0], hint, r);
+#ifdef PHYLINO_TRACE
+    const long long q1 = clock64();
+#endif
+    walk_stretch<S, UW, DBG>(a, T, ds, bp, b0 + my0, mine, h, thr, safe, p, active, r);
+#ifdef PHYLINO_TRACE
+    const long long q2 = clock64();
+#endif
+    if (FULL) flush_run<S>(a, T, ds, p, active, r);
+    else      flush_run_substreams<S>(a, T, ds, p, active, lg, lane, r);
+#ifdef PHYLINO_TRACE
+    const long long q3 = clock64();
+    const unsigned wid = blockIdx.x * WARPS + (threadIdx.x >> 5);
+    if (lane == 0 && wid < 64) { g_sub[wid][0] += q1 - q0; g_sub[wid][1] += q2 - q1; g_sub[wid][2] += q3 - q2; g_sub[wid][3] += 1; }
+#endif
 }
 
 /* lane 0 takes the next ticket of the work counter; the value is needed one item later */
@@ -697,12 +735,13 @@ __device__ __forceinline__ unsigned take_ticket(unsigned *counter, int lane)
     return t;
 }
 
-/* item -> (dataset, batches [b0, b1), chunk) */
+/* item -> (dataset, batches [b0, b1), chunk); SMALL: one chunk, no fine tail (an item is a unit) */
+template <bool SMALL>
 __device__ __forceinline__ void decode_item(const SpectraArgs &a, unsigned item, int &d, int &b0, int &b1, int &chunk)
 {
-    const int unit = (int)(item / (unsigned)a.n_chunks);
-    chunk = (int)(item - (unsigned)unit * (unsigned)a.n_chunks);
-    if (unit >= a.tail_unit) {
+    const int unit = SMALL ? (int)item : (int)(item / (unsigned)a.n_chunks);
+    chunk = SMALL ? 0 : (int)(item - (unsigned)unit * (unsigned)a.n_chunks);
+    if (!SMALL && unit >= a.tail_unit) {
         d = a.n_datasets - 1;
         b0 = a.tail_b0 + (unit - a.tail_unit) * a.tail_batches;
         b1 = min(b0 + a.tail_batches, a.ds[d].n_batches);
@@ -715,71 +754,198 @@ __device__ __forceinline__ void decode_item(const SpectraArgs &a, unsigned item,
     b1 = min(b0 + a.unit_batches, a.ds[d].n_batches);
 }
 
-template <int S>
+/* The persistent warp: its first two items are static (warp index, + number of warps), later ones come from
+ * the counter (zero at kernel start; ticket t is item 2 nW + t): warps that meet expensive units (bin edges) or
+ * slow memory simply claim fewer.  The unit of item i + 1 is copied into the warp's other buffer while item i
+ * is walked.  first_item_loading(): the copy of the first item was started before the tables were ready. */
+struct WarpPipe {
+    unsigned char *buf0;            /* the warp's two unit buffers */
+    unsigned long long *bars;       /* its two mbarriers */
+};
+
+struct Item { int d, b0, b1, chunk; };
+
+template <bool SMALL>
+__device__ __forceinline__ void start_first_item(const SpectraArgs &a, const WarpPipe &wp, unsigned cur, int lane)
+{
+    if (lane == 0) {
+        mbar_init(wp.bars, 1);
+        mbar_init(wp.bars + 1, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        if (cur < (unsigned)a.n_items) {
+            Item it;
+            decode_item<SMALL>(a, cur, it.d, it.b0, it.b1, it.chunk);
+            bulk_load(wp.buf0, batch_ptr(a.ds[it.d], it.b0), (unsigned)(it.b1 - it.b0) * rec_bytes(a.ds[it.d]), wp.bars);
+        }
+    }
+    __syncwarp();
+}
+
+/* the hint of the item's first group (its other groups, and the short last group of a large batch, load theirs
+ * when they get there) */
+__device__ __forceinline__ int item_hint(const SpectraArgs &a, const Item &it, int lane)
+{
+    const int np = min(32, a.P - 32 * it.chunk * a.chunk_groups);
+    return load_hint(a.ds[it.d], np, lane, it.b0, it.b1 - it.b0);
+}
+
+/* SMALL: at most 16 points (one group of sub-streams): the full-group code is not even instantiated */
+template <int S, bool DBG, bool SMALL>
+__device__ __forceinline__ void ticket_loop(const SpectraArgs &a, const Tables &T, unsigned *counter, const WarpPipe &wp,
+                                            unsigned cur, unsigned nW, int lane)
+{
+    const int n_groups = (a.P + 31) >> 5;
+    const unsigned n_items = (unsigned)a.n_items;
+    unsigned nxt = cur + nW;
+    unsigned phase = 0u;                                /* bit b: parity of the next completion of buffer b */
+    int b = 0;
+#ifdef PHYLINO_TRACE
+    const unsigned wme = cur;
+    int wcount = 0;
+    long long kacc[4] = {0, 0, 0, 0};
+#endif
+    Item it, nit;
+    int hint = 0, nhint = 0;
+    if (cur < n_items) {
+        decode_item<SMALL>(a, cur, it.d, it.b0, it.b1, it.chunk);
+        hint = item_hint(a, it, lane);
+    }
+#pragma unroll 1
+    while (cur < n_items) {
+#ifdef PHYLINO_TRACE
+        const long long k0 = clock64();
+#endif
+        const unsigned ticket = take_ticket(counter, lane);
+        if (nxt < n_items) {
+            /* the other buffer was last read one item ago; every lane has passed the shuffle below */
+            decode_item<SMALL>(a, nxt, nit.d, nit.b0, nit.b1, nit.chunk);
+            if (lane == 0)
+                bulk_load(wp.buf0 + (b ^ 1) * STAGE_BUF_BYTES, batch_ptr(a.ds[nit.d], nit.b0),
+                          (unsigned)(nit.b1 - nit.b0) * rec_bytes(a.ds[nit.d]), wp.bars + (b ^ 1));
+            nhint = item_hint(a, nit, lane);            /* needed one item from now */
+        }
+#ifdef PHYLINO_TRACE
+        const long long k1 = clock64();
+#endif
+        mbar_wait(wp.bars + b, (phase >> b) & 1u);
+#ifdef PHYLINO_TRACE
+        const long long k2 = clock64();
+#endif
+        phase ^= 1u << b;
+        const DatasetDev &ds = a.ds[it.d];
+        const int nb = it.b1 - it.b0;
+        const int g0 = it.chunk * a.chunk_groups, g1 = min(g0 + a.chunk_groups, n_groups);
+#pragma unroll 1
+        for (int g = g0; g < g1; ++g) {
+            const void *unit = wp.buf0 + b * STAGE_BUF_BYTES;
+            const bool full = !SMALL && 32 * g + 16 < a.P;
+            /* the prefetched hint fits the item's first group, and every full group (all lanes start at b0) */
+            int hg = hint;
+            if (!SMALL && g > g0 && !full) hg = load_hint(ds, a.P - 32 * g, lane, it.b0, nb);
+            if (ds.unit_w) {
+                if (full) { if (!SMALL) walk_unit<S, true, true, DBG>(a, T, ds, it.d, unit, it.b0, nb, g, lane, hg); }
+                else      walk_unit<S, false, true, DBG>(a, T, ds, it.d, unit, it.b0, nb, g, lane, hg);
+            } else {
+                if (full) { if (!SMALL) walk_unit<S, true, false, DBG>(a, T, ds, it.d, unit, it.b0, nb, g, lane, hg); }
+                else      walk_unit<S, false, false, DBG>(a, T, ds, it.d, unit, it.b0, nb, g, lane, hg);
+            }
+        }
+#ifdef PHYLINO_TRACE
+        const long long k3 = clock64();
+        ++wcount;
+#endif
+        cur = nxt;
+        it = nit;
+        hint = nhint;
+        nxt = 2u * nW + __shfl_sync(0xffffffffu, ticket, 0);    /* also orders this item's reads before the next copy */
+#ifdef PHYLINO_TRACE
+        const long long k4 = clock64();
+        kacc[0] += k1 - k0; kacc[1] += k2 - k1; kacc[2] += k3 - k2; kacc[3] += k4 - k3;
+#endif
+        b ^= 1;
+    }
+#ifdef PHYLINO_TRACE
+    if (lane == 0 && wme < 4096) {
+        g_wend[wme] = gtime(); g_wunits[wme] = wcount;
+        if (wme < 64) for (int i = 0; i < 4; ++i) g_wtrace[0][4 * wme + i] = (unsigned long long)kacc[i];
+    }
+#endif
+}
+
+template <int S, bool DBG>
 __global__ void __launch_bounds__(WARPS * 32, 4) spectra_kernel(const __grid_constant__ SpectraArgs a)
 {
     static_assert(EB == 4, "the batch loads are written for EB = 4");
-    extern __shared__ __align__(128) unsigned char stage[];       /* [WARPS][2][unit_batches] EventBatch */
+    extern __shared__ __align__(128) unsigned char stage[];       /* [WARPS][2][STAGE_BUF_BYTES] */
     __shared__ unsigned long long bars[WARPS][2];
     const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
-    const unsigned nW = gridDim.x * WARPS;
-    const int n_groups = (a.P + 31) >> 5;
-    const unsigned n_items = (unsigned)a.n_items;
-    EventBatch *const buf0 = reinterpret_cast<EventBatch *>(stage) + (size_t)(2 * wib) * a.unit_batches;
-    if (lane == 0) {
-        mbar_init(&bars[wib][0], 1);
-        mbar_init(&bars[wib][1], 1);
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    }
-    __syncwarp();
-    /* the first two items of a warp are static, later ones come from the counter (which the setup
-     * kernel left at 2 nW): warps that meet expensive units (bin edges) simply claim fewer.  The
-     * unit of item i + 1 is copied into the warp's other buffer while item i is walked. */
-    unsigned cur = blockIdx.x * WARPS + wib, nxt = cur + nW;
-    unsigned phase = 0u;                                /* bit b: parity of the next completion of buffer b */
-    int b = 0;
-    if (cur < n_items && lane == 0) {
-        int d, b0, b1, chunk;
-        decode_item(a, cur, d, b0, b1, chunk);
-        bulk_load(buf0, a.ds[d].ev + b0, (unsigned)(b1 - b0) * (unsigned)sizeof(EventBatch), &bars[wib][0]);
-    }
+    const unsigned nW = gridDim.x * WARPS, cur = blockIdx.x * WARPS + wib;
+    WarpPipe wp;
+    wp.buf0 = stage + (size_t)(2 * wib) * STAGE_BUF_BYTES;
+    wp.bars = &bars[wib][0];
+    start_first_item<false>(a, wp, cur, lane);
     /* everything above touched only kernel parameters and the event store; the records, thresholds
      * and the work counter come from the setup kernel (no-op unless launched as its dependent) */
     asm volatile("griddepcontrol.wait;" ::: "memory");
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
-#pragma unroll 1
-    while (cur < n_items) {
-        const unsigned ticket = take_ticket(a.counter, lane);
-        int d, b0, b1, chunk;
-        decode_item(a, cur, d, b0, b1, chunk);
-        if (nxt < n_items && lane == 0) {
-            /* the other buffer was last read one item ago; every lane has passed the __syncwarp below */
-            int nd, nb0, nb1, nc;
-            decode_item(a, nxt, nd, nb0, nb1, nc);
-            bulk_load(buf0 + (b ^ 1) * a.unit_batches, a.ds[nd].ev + nb0, (unsigned)(nb1 - nb0) * (unsigned)sizeof(EventBatch),
-                      &bars[wib][b ^ 1]);
-        }
-        mbar_wait(&bars[wib][b], (phase >> b) & 1u);
-        phase ^= 1u << b;
-        const DatasetDev &ds = a.ds[d];
-        const int g1 = min((chunk + 1) * a.chunk_groups, n_groups);
-#pragma unroll 1
-        for (int g = chunk * a.chunk_groups; g < g1; ++g) {
-            const EventBatch *unit = buf0 + b * a.unit_batches;
-            if (32 * g + 16 >= a.P) walk_unit<S, false, false>(a, ds, d, unit, b1 - b0, g, lane);
-            else if (ds.unit_w)    walk_unit<S, true, true>(a, ds, d, unit, b1 - b0, g, lane);
-            else                   walk_unit<S, true, false>(a, ds, d, unit, b1 - b0, g, lane);
-        }
-        cur = nxt;
-        nxt = __shfl_sync(0xffffffffu, ticket, 0);      /* also orders this item's reads before the next copy */
-        b ^= 1;
-    }
+    Tables T;
+    T.params = a.params;
+    T.rec = a.rec;
+    T.thr = a.thr;
+    T.safe = a.safe;
+    ticket_loop<S, DBG, false>(a, T, a.counter, wp, cur, nW, lane);
 }
 
-/* dynamic shared memory of one CTA: two unit buffers per warp, sized for the largest unit */
-constexpr size_t STAGE_BYTES = (size_t)WARPS * 2 * MAX_UNIT_BATCHES * sizeof(EventBatch);
+/* ---- small batches (at most FUSED_MAX_POINTS points: one group of sub-streams) ----
+ * Rows a1 and the tables of a3 per CTA in shared memory -- no setup launch -- then the same ticket loop over the
+ * units.  The finalize kernel behind it is its programmatic dependent and does its table work meanwhile; it also
+ * zeroes the work counter a.done again.  A batch of at most PARAM_BLOB_DOUBLES parameters may travel by value
+ * with the kernel arguments (blob): a host call then needs no copy engine at all. */
+template <int S, bool DBG>
+__global__ void __launch_bounds__(WARPS * 32, 4) spectra_fused_kernel(const __grid_constant__ SpectraArgs a,
+                                                                      const __grid_constant__ ParamBlob blob)
+{
+    /* [WARPS][2][STAGE_BUF_BYTES] stage | rec [rec_fields x P] | safe [thr_rows x D] | thr [thr_rows x thr_stride] */
+    extern __shared__ __align__(128) unsigned char stage[];
+    __shared__ unsigned long long bars[WARPS][2];
+    const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+    const unsigned nW = gridDim.x * WARPS, cur = blockIdx.x * WARPS + wib;
+    TRACE_MIN(0);
+    TRACE_MAX(1);
+    WarpPipe wp;
+    wp.buf0 = stage + (size_t)(2 * wib) * STAGE_BUF_BYTES;
+    wp.bars = &bars[wib][0];
+    start_first_item<true>(a, wp, cur, lane);
+    /* the event copy above touched only the event store; the parameters may come from a kernel before us, and
+     * the accumulators and the work counter must have been left clean by the finalize kernel of the call before */
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
 
-template <int S> cudaError_t launch_t(const SpectraArgs &a, cudaStream_t st, bool pdl)
+    double *rec_s = reinterpret_cast<double *>(stage + (size_t)WARPS * 2 * STAGE_BUF_BYTES);
+    float2 *safe_s = reinterpret_cast<float2 *>(rec_s + (size_t)(2 * S + 2) * a.P);
+    float *thr_s = reinterpret_cast<float *>(safe_s + (size_t)a.thr_rows * a.n_datasets);
+    /* a.params == NULL: the batch came by value with the kernel arguments (host entry points, small batches) */
+    const double *params = a.params ? a.params : blob.v;
+    if ((int)threadIdx.x < a.P) point_record<S>(a, params, threadIdx.x, rec_s);
+    for (int e = threadIdx.x; e < a.thr_rows * a.thr_stride; e += WARPS * 32)
+        threshold_entry(a, params, e / a.thr_stride, e % a.thr_stride, thr_s, safe_s);
+    __syncthreads();
+    TRACE_MAX(2);
+    Tables T;
+    T.params = params;
+    T.rec = rec_s;
+    T.thr = thr_s;
+    T.safe = safe_s;
+    ticket_loop<S, DBG, true>(a, T, a.done, wp, cur, nW, lane);
+    TRACE_MIN(3);
+    TRACE_MAX(4);
+}
+
+/* dynamic shared memory of one CTA: two unit buffers per warp */
+constexpr size_t STAGE_BYTES = (size_t)WARPS * 2 * STAGE_BUF_BYTES;
+constexpr size_t FUSED_TABLE_MAX = 160 * 1024;          /* records + thresholds of the single-launch kernel */
+
+template <int S, bool DBG> cudaError_t launch_t(const SpectraArgs &a, cudaStream_t st, bool pdl)
 {
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(a.n_warps / WARPS);
@@ -791,30 +957,107 @@ template <int S> cudaError_t launch_t(const SpectraArgs &a, cudaStream_t st, boo
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr;
     cfg.numAttrs = pdl ? 1 : 0;
-    if (a.sched == 1) return cudaLaunchKernelEx(&cfg, spectra_static_kernel<S>, a);
-    return cudaLaunchKernelEx(&cfg, spectra_kernel<S>, a);
+    return cudaLaunchKernelEx(&cfg, spectra_kernel<S, DBG>, a);
 }
 
-template <int S> cudaError_t max_warps_t(int sm_count, int *warps)
+template <int S, bool DBG>
+cudaError_t launch_fused_t(const SpectraArgs &a, const ParamBlob &blob, cudaStream_t st, bool pdl)
 {
-    int per_sm = 0;
-    cudaError_t e = cudaFuncSetAttribute(spectra_kernel<S>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(a.n_warps / WARPS);
+    cfg.blockDim = dim3(WARPS * 32);
+    cfg.dynamicSmemBytes = STAGE_BYTES + fused_table_bytes(S, a.P, a.thr_rows, a.thr_stride, a.n_datasets);
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = pdl ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, spectra_fused_kernel<S, DBG>, a, blob);
+}
+
+/* the dynamic shared memory sits above the 48 KB default: opt every instantiation in (the attribute is per
+ * function, so a context that changes its oscillation model finds the other S ready too) */
+template <int S, bool DBG> cudaError_t allow_stage_t()
+{
+    cudaError_t e = cudaFuncSetAttribute(spectra_kernel<S, DBG>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          (int)STAGE_BYTES);
     if (e != cudaSuccess) return e;
-    e = cudaFuncSetAttribute(spectra_static_kernel<S>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)STAGE_BYTES);
-    if (e != cudaSuccess) return e;
-    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, spectra_kernel<S>, WARPS * 32, STAGE_BYTES);
-    if (e != cudaSuccess) return e;
-    if (per_sm < 1) return cudaErrorLaunchOutOfResources;
-    *warps = sm_count * per_sm * WARPS;
-    return cudaSuccess;
+    return cudaFuncSetAttribute(spectra_fused_kernel<S, DBG>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                (int)(STAGE_BYTES + FUSED_TABLE_MAX));
+}
+
+cudaError_t allow_stage_all()
+{
+    cudaError_t e = allow_stage_t<2, false>();
+    if (e == cudaSuccess) e = allow_stage_t<3, false>();
+    if (e == cudaSuccess) e = allow_stage_t<2, true>();
+    if (e == cudaSuccess) e = allow_stage_t<3, true>();
+    return e;
 }
 
 } // namespace
 
-cudaError_t spectra_max_warps(int S, int sm_count, int *warps)
+#ifdef PHYLINO_TRACE
+extern "C" __attribute__((visibility("default"))) int phylino_debug_trace(unsigned long long *out, int reset)
 {
-    return S == 2 ? max_warps_t<2>(sm_count, warps) : max_warps_t<3>(sm_count, warps);
+    if (out && cudaMemcpyFromSymbol(out, g_trace, sizeof(unsigned long long) * 8) != cudaSuccess) return 1;
+    if (out && reset == 2) {        /* out: [8 + 4 * 256 + 4] */
+        if (cudaMemcpyFromSymbol(out + 8, g_wtrace, sizeof(unsigned long long) * 1024) != cudaSuccess) return 1;
+        int n[4];
+        if (cudaMemcpyFromSymbol(n, g_wn, sizeof n) != cudaSuccess) return 1;
+        for (int i = 0; i < 4; ++i) out[8 + 1024 + i] = (unsigned long long)n[i];
+        return 0;
+    }
+    if (out && reset == 4) return cudaMemcpyFromSymbol(out, g_sub, sizeof(long long) * 256) != cudaSuccess;
+    if (out && reset == 3) {        /* out: [4096 end times | 4096 unit counts] */
+        if (cudaMemcpyFromSymbol(out, g_wend, sizeof(unsigned long long) * 4096) != cudaSuccess) return 1;
+        static int u[4096];
+        if (cudaMemcpyFromSymbol(u, g_wunits, sizeof u) != cudaSuccess) return 1;
+        for (int i = 0; i < 4096; ++i) out[4096 + i] = (unsigned long long)u[i];
+        return 0;
+    }
+    if (reset) {
+        static long long zs[256];
+        if (cudaMemcpyToSymbol(g_sub, zs, sizeof zs) != cudaSuccess) return 1;
+        int zn[4] = {0, 0, 0, 0};
+        if (cudaMemcpyToSymbol(g_wn, zn, sizeof zn) != cudaSuccess) return 1;
+        unsigned long long z[8] = {~0ull, 0, 0, ~0ull, 0, 0, 0, 0};
+        if (cudaMemcpyToSymbol(g_trace, z, sizeof z) != cudaSuccess) return 1;
+    }
+    return 0;
+}
+#endif
+
+size_t fused_table_bytes(int S, int P, int thr_rows, int thr_stride, int n_datasets)
+{
+    const size_t b = (size_t)rec_fields(S) * P * sizeof(double) + (size_t)thr_rows * n_datasets * sizeof(float2) +
+                     (size_t)thr_rows * thr_stride * sizeof(float);
+    return (b + 15) / 16 * 16;
+}
+
+bool fused_fits(size_t table_bytes) { return table_bytes <= FUSED_TABLE_MAX; }
+
+/* warps of a persistent grid the chip holds at once: the ticket kernel (fused = false) or the single-launch
+ * kernel with `table_bytes` of tables */
+cudaError_t spectra_max_warps(int S, int sm_count, bool fused, size_t table_bytes, int *warps)
+{
+    int per_sm = 0;
+    cudaError_t e = allow_stage_all();
+    if (e != cudaSuccess) return e;
+    if (fused) {
+        e = S == 2 ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, spectra_fused_kernel<2, false>, WARPS * 32,
+                                                                   STAGE_BYTES + table_bytes)
+                   : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, spectra_fused_kernel<3, false>, WARPS * 32,
+                                                                   STAGE_BYTES + table_bytes);
+    } else {
+        e = S == 2 ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, spectra_kernel<2, false>, WARPS * 32, STAGE_BYTES)
+                   : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, spectra_kernel<3, false>, WARPS * 32, STAGE_BYTES);
+    }
+    if (e != cudaSuccess) return e;
+    if (per_sm < 1) return cudaErrorLaunchOutOfResources;
+    *warps = sm_count * per_sm * WARPS;
+    return cudaSuccess;
 }
 
 cudaError_t launch_setup(const SpectraArgs &a, int S, cudaStream_t st)
@@ -827,39 +1070,19 @@ cudaError_t launch_setup(const SpectraArgs &a, int S, cudaStream_t st)
 }
 
 /* persistent grid of a.n_warps warps (a multiple of WARPS) that claim the a.n_items work items */
-cudaError_t launch_spectra(const SpectraArgs &a, int S, cudaStream_t st, bool pdl)
+cudaError_t launch_spectra(const SpectraArgs &a, int S, cudaStream_t st, bool pdl, bool dbg)
 {
     if (a.n_items <= 0 || a.P <= 0 || a.n_warps < WARPS) return cudaSuccess;
-    return S == 2 ? launch_t<2>(a, st, pdl) : launch_t<3>(a, st, pdl);
+    if (dbg) return S == 2 ? launch_t<2, true>(a, st, pdl) : launch_t<3, true>(a, st, pdl);
+    return S == 2 ? launch_t<2, false>(a, st, pdl) : launch_t<3, false>(a, st, pdl);
 }
 
-/* ---- diagnostic: bin index of every event at every point (bit-exact parity of row a3) ----
- * Reads the threshold rows the setup kernel wrote and assigns bins with the same locate_bin() as
- * the hot kernel, so the test covers the production binning. */
-namespace {
-__global__ void __launch_bounds__(256) event_bins_kernel(const __grid_constant__ SpectraArgs a, int d,
-                                                         const int32_t *perm, long long n, long long ev_off,
-                                                         long long total_events, int32_t *bins)
+/* the kernel for at most FUSED_MAX_POINTS points (setup fused in): a.n_warps warps */
+cudaError_t launch_fused(const SpectraArgs &a, const ParamBlob &blob, int S, cudaStream_t st, bool pdl, bool dbg)
 {
-    const DatasetDev &ds = a.ds[d];
-    const int p = blockIdx.y;
-    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n) return;
-    const int row = row_of(a, p);
-    float hi;
-    int b = locate_bin(ds, a.thr + (size_t)row * a.thr_stride + ds.thr_off, a.safe[(size_t)row * a.n_datasets + d],
-                       theta_of(a, p), ds.ev[i / EB].v[i % EB], hi);
-    bins[(size_t)p * total_events + ev_off + perm[i]] = (b >= 0 && b < ds.n_bins) ? b : -1;
-}
-} // namespace
-
-cudaError_t launch_event_bins(const SpectraArgs &a, int d, const int32_t *perm, long long n, long long ev_off,
-                              long long total_events, int32_t *bins, cudaStream_t st)
-{
-    if (n <= 0 || a.P <= 0) return cudaSuccess;
-    dim3 grid((unsigned)((n + 255) / 256), a.P);
-    event_bins_kernel<<<grid, 256, 0, st>>>(a, d, perm, n, ev_off, total_events, bins);
-    return cudaGetLastError();
+    if (a.P <= 0 || a.n_warps < WARPS) return cudaSuccess;
+    if (dbg) return S == 2 ? launch_fused_t<2, true>(a, blob, st, pdl) : launch_fused_t<3, true>(a, blob, st, pdl);
+    return S == 2 ? launch_fused_t<2, false>(a, blob, st, pdl) : launch_fused_t<3, false>(a, blob, st, pdl);
 }
 
 } // namespace phylino
