@@ -19,12 +19,13 @@ sys.path.insert(0, os.path.dirname(os.path.dirname(HERE)))
 import oracle  # noqa: E402
 import workloads  # noqa: E402
 
-CASES = {"eq1": (0, 611), "full3": (1, 612), "sterile4": (2, 613)}      # name -> (osc_model, seed)
+# name -> (osc_model, seed, mass ordering); full3_inv: PAPER.md:226 (section 4.3), the inverted-ordering branch
+CASES = {"eq1": (0, 611, +1), "full3": (1, 612, +1), "sterile4": (2, 613, +1), "full3_inv": (1, 614, -1)}
 
 
 def case_inputs(name):
-    osc, seed = CASES[name]
-    wl = workloads.make_tiny(seed=seed, osc_model=osc, n_events=100, n_points=5, n_datasets=2)
+    osc, seed, ordering = CASES[name]
+    wl = workloads.make_tiny(seed=seed, osc_model=osc, n_events=100, n_points=5, n_datasets=2, ordering=ordering)
     data = np.arange(wl.model.total_bins, dtype=np.float64) * 3.0 + 2.0
     return wl, data
 
@@ -39,7 +40,8 @@ def main():
         path = os.path.join(HERE, f"tiny_{name}.txt")
         with open(path, "w") as f:
             f.write(f"# oracle results, workloads.make_tiny(seed={CASES[name][1]}, osc_model={CASES[name][0]}, "
-                    f"n_events=100, n_points=5, n_datasets=2); data[i] = 3 i + 2\n")
+                    f"n_events=100, n_points=5, n_datasets=2"
+                    + (f", ordering={CASES[name][2]}" if CASES[name][2] != 1 else "") + "); data[i] = 3 i + 2\n")
             f.write("# written by tests/golden/make_golden.py (oracle only); P_ee: PAPER.md:34 Eq. 1 / DESIGN.md R2, R15;\n")
             f.write("# NLL: PAPER.md:67-83 Eq. 3-6, :119-125 Eq. 9.  Rows: 'hist p' then total_bins values; 'nll' then P values\n")
             for p in range(hist.shape[0]):

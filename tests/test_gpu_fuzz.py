@@ -2,7 +2,8 @@
 
 Random event counts (including 0 and counts that leave ragged batches and units), 1-3 datasets, 1-70 points
 (all lane mappings: sub-streams for <= 16 points, full groups, ragged last group), unit or random weights,
-the three oscillation models, random work cuts, dense / host / cached entry points.  Same bars as everywhere:
+the three oscillation models (FULL3 in both mass orderings), random work cuts, the three schedules,
+dense / host / cached entry points.  Same bars as everywhere:
 bit-exact bins, per-bin relative error <= 1e-7, |dNLL| <= 1e-6.
 """
 import numpy as np
@@ -22,7 +23,9 @@ def _case(i):
     n_ds = int(rng.integers(1, 4))
     n_ev = int(rng.choice([0, 1, 3, 4, 5, 63, 64, 65, 255, 257, 1000, 2049, 3001]))
     n_pt = int(rng.choice([1, 2, 3, 5, 8, 15, 16, 17, 31, 32, 33, 47, 64, 70]))
-    wl = workloads.make_tiny(seed=20_000 + i, osc_model=osc, n_events=n_ev, n_points=n_pt, n_datasets=n_ds)
+    ordering = -1 if (osc == 1 and rng.random() < 0.5) else +1      # FULL3: both mass orderings
+    wl = workloads.make_tiny(seed=20_000 + i, osc_model=osc, n_events=n_ev, n_points=n_pt, n_datasets=n_ds,
+                             ordering=ordering)
     if rng.random() < 0.5:                        # the unit-weight paths
         for e in wl.events:
             e.w[:] = 1.0
@@ -30,18 +33,19 @@ def _case(i):
         wl.params[n_pt // 2:] = wl.params[: n_pt - n_pt // 2]
         wl.params[n_pt // 2:, 0] *= 0.97
     tuning = (int(rng.choice([0, 16, 64, 128, 256])), int(rng.choice([0, 1, 2])), int(rng.choice([0, 0, 8, 148, 1000])))
-    return wl, tuning, bool(rng.random() < 0.5)
+    return wl, tuning, bool(rng.random() < 0.5), int(rng.choice([0, 0, 1, 2]))
 
 
 @pytest.mark.parametrize("i", range(N_CASES))
 def test_random_small_workload(gpu, oracle_mod, i):
     import torch
-    wl, tuning, cache = _case(i)
+    wl, tuning, cache, schedule = _case(i)
     orc = oracle_mod.Oracle(wl.model, wl.events)
     data = np.arange(orc.total_bins, dtype=np.float64) * 2.0 + 1.0
     with gpu.Phylino() as ph:
         ph.load_workload(wl)
         ph.set_tuning(*tuning)
+        ph.set_schedule(schedule)                 # library's choice / always tickets / small-batch kernel up to 16 points
         dp = torch.as_tensor(wl.params, device="cuda")
         h = ph.spectra(dp).cpu().numpy()
         nll = ph.nll(dp, torch.as_tensor(data, device="cuda")).cpu().numpy()

@@ -1,0 +1,280 @@
+"""-m gpu: the launch schedules, the hot loop's own bin assignment, contexts side by side, sharding on one GPU.
+
+Bars as everywhere: bins bit-exact, per-bin relative error <= 1e-7, |dNLL| <= 1e-6 against the oracle."""
+import numpy as np
+import pytest
+
+import workloads
+from workloads.spec import OSC_EQ1, OSC_FULL3, OSC_STERILE4
+
+pytestmark = pytest.mark.gpu
+
+REL_BIN = 1e-7
+ABS_NLL = 1e-6
+
+
+def _dev(a):
+    import torch
+    return torch.as_tensor(np.ascontiguousarray(a, dtype=np.float64), device="cuda")
+
+
+def _check_hist(h_gpu, h_orc):
+    zero = h_orc == 0.0
+    assert np.array_equal(h_gpu[zero], h_orc[zero])
+    rel = np.abs(h_gpu[~zero] - h_orc[~zero]) / np.abs(h_orc[~zero])
+    assert rel.size == 0 or rel.max() <= REL_BIN, rel.max()
+
+
+def _data(orc, wl):
+    mu0 = orc.expectation(wl.theta0[None, :], orc.spectra(wl.theta0[None, :]))[0]
+    return workloads.poisson_counts(mu0, wl.seed + 7)
+
+
+# ---- bit-exact bins FROM THE HOT LOOP (north_star "bin assignment bit-exact") ------------------------------------
+# phylino_event_bins runs the production kernels of the batch size in their diagnostic instantiation: every
+# event is reported with the bin the lane that accumulated it put it in -- through the hint walk, the forward
+# scan, the whole-batch test, the 2-/4-batch straight-line paths, the per-event path and the sub-stream split.
+# 1 / 5 points: small-batch kernel (32 / 4 sub-streams); 17: one full group with 15 shadow lanes; 33: a full group
+# and a 1-point group of 32 sub-streams; 70: two full groups and a ragged one of 6.
+@pytest.mark.parametrize("k,scale", [(2, 0.02), (3, 0.004), (4, 0.004), (5, 0.02)])
+@pytest.mark.parametrize("n_points", [1, 5, 17, 33, 70])
+def test_hot_loop_bins_scaled_configs(gpu, oracle_mod, k, scale, n_points):
+    import torch
+    wl = workloads.make_config(k, scale=scale)
+    rng = np.random.default_rng(7 * k + n_points)
+    sel = rng.choice(wl.n_points, size=n_points, replace=wl.n_points < n_points)
+    params = wl.params[sel].copy()
+    orc = oracle_mod.Oracle(wl.model, wl.events)
+    want = orc.event_bins(params)
+    with gpu.Phylino() as ph:
+        ph.load_workload(wl)
+        for schedule in ((0, 1, 2) if n_points <= 16 else (0,)):
+            ph.set_schedule(schedule)
+            got = ph.event_bins(_dev(params)).cpu().numpy()
+            assert np.array_equal(got, want), (schedule, int((got != want).sum()))
+            # the diagnostic pass left the accumulators clean
+            _check_hist(ph.spectra(_dev(params)).cpu().numpy(), orc.spectra(params))
+        torch.cuda.synchronize()
+
+
+@pytest.mark.parametrize("n_points", [1, 5, 17, 33, 70])
+@pytest.mark.parametrize("osc", [OSC_EQ1, OSC_FULL3])
+def test_hot_loop_bins_weighted_store(gpu, oracle_mod, osc, n_points):
+    """random weights (the 96-byte records), per-point energy scales, three datasets, ragged event counts"""
+    wl = workloads.make_tiny(seed=300 + n_points + osc, osc_model=osc, n_events=2500 + 37 * n_points, n_points=n_points,
+                             n_datasets=3, ordering=-1 if osc == OSC_FULL3 else +1)
+    orc = oracle_mod.Oracle(wl.model, wl.events)
+    with gpu.Phylino() as ph:
+        ph.load_workload(wl)
+        for tuning in ((0, 0, 0), (64, 1, 0), (256, 2, 16)):
+            ph.set_tuning(*tuning)
+            assert np.array_equal(ph.event_bins(_dev(wl.params)).cpu().numpy(), orc.event_bins(wl.params)), tuning
+
+
+# ---- schedules -----------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("k,scale,n_points", [(1, 1.0, 1), (2, 0.05, 3), (3, 0.01, 16), (4, 0.01, 2), (5, 0.05, 4), (5, 0.05, 11)])
+def test_small_batches_every_schedule(gpu, oracle_mod, k, scale, n_points):
+    """the small-batch kernel (setup fused in, finalize prologue overlapped) and the three-kernel ticket path
+    against the oracle, device and host entry points; the schedules differ from each other by rounding only"""
+    wl = workloads.make_config(k, scale=scale, n_points=n_points)
+    orc = oracle_mod.Oracle(wl.model, wl.events)
+    data = _data(orc, wl)
+    h_o, nll_o = orc.spectra(wl.params), orc.nll(wl.params, data)
+    mu_o = orc.expectation(wl.params, h_o)
+    out = {}
+    with gpu.Phylino() as ph:
+        ph.load_workload(wl)
+        for schedule in (0, 1, 2):
+            ph.set_schedule(schedule)
+            n0 = ph.launch_count
+            h = ph.spectra(_dev(wl.params)).cpu().numpy()
+            launches = ph.launch_count - n0
+            assert launches == (3 if schedule == 1 else 2) or schedule == 0
+            nll = ph.nll(_dev(wl.params), _dev(data)).cpu().numpy()
+            mu = ph.expectation(_dev(wl.params)).cpu().numpy()
+            nll_h = ph.nll_host(wl.params, data)
+            h_h = ph.spectra_host(wl.params)
+            _check_hist(h, h_o)
+            _check_hist(mu, mu_o)
+            assert np.abs(nll - nll_o).max() <= ABS_NLL
+            assert np.array_equal(nll, nll_h) and np.array_equal(h, h_h)     # same kernels, same bits
+            out[schedule] = (h, nll)
+    assert np.allclose(out[1][0], out[2][0], rtol=1e-12, atol=0) and np.allclose(out[1][1], out[2][1], rtol=0, atol=1e-8)
+
+
+def test_model_switch_on_one_context(gpu, oracle_mod):
+    """A context that goes from a two-term model to a three-term one and back (the cached occupancy
+    and the shared-memory opt-in belonged to the first model's kernels)."""
+    with gpu.Phylino() as ph:
+        for k, scale, n_points in ((2, 0.01, 40), (4, 0.002, 40), (2, 0.01, 3), (5, 0.01, 3), (2, 0.01, 40)):
+            wl = workloads.make_config(k, scale=scale, n_points=n_points)
+            orc = oracle_mod.Oracle(wl.model, wl.events)
+            data = _data(orc, wl)
+            ph.load_workload(wl)
+            nll = ph.nll(_dev(wl.params), _dev(data)).cpu().numpy()
+            assert np.abs(nll - orc.nll(wl.params, data)).max() <= ABS_NLL, k
+
+
+def test_unphysical_amplitudes_near_the_fixed_point_bound(gpu, oracle_mod):
+    """phylino.h "Errors": finite but unphysical mixings.  sin^2 2theta13 = -1 gives cos^4 theta13 = 1.457 and
+    sum |A_k| = 2.24 <= 3: still inside the fixed-point range, parity with the oracle holds.  sin^2 2theta13 = -3
+    gives sum |A_k| = 4.9 > 3: the documented NaN (the oracle, which has no fixed point, stays finite)."""
+    wl = workloads.make_tiny(seed=83, osc_model=OSC_EQ1, n_events=400, n_points=4)
+    wl.params[1, 0] = -1.0
+    wl.params[2, 0] = -3.0
+    orc = oracle_mod.Oracle(wl.model, wl.events)
+    A, _ = orc.terms(wl.params[1])
+    assert 2.0 < np.abs(A).sum() <= 3.0
+    A, _ = orc.terms(wl.params[2])
+    assert np.abs(A).sum() > 3.0
+    h_o = orc.spectra(wl.params)
+    assert np.isfinite(h_o).all()
+    for schedule in (1, 2):
+        with gpu.Phylino() as ph:
+            ph.load_workload(wl)
+            ph.set_schedule(schedule)
+            h = ph.spectra(_dev(wl.params)).cpu().numpy()
+        ok = [0, 1, 3]
+        _check_hist(h[ok], h_o[ok])
+        assert np.isnan(h[2]).all()
+
+
+def test_two_contexts_on_two_streams(gpu, oracle_mod):
+    """phylino.h "Threads": any number of contexts may coexist (independent fits).  Two contexts on
+    two streams, calls interleaved with no synchronisation in between, each against the oracle."""
+    import torch
+    wls = [workloads.make_config(2, scale=0.05, n_points=40), workloads.make_config(5, scale=0.05, n_points=70)]
+    orcs = [oracle_mod.Oracle(w.model, w.events) for w in wls]
+    datas = [_data(o, w) for o, w in zip(orcs, wls)]
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    ctxs, outs = [], [[], []]
+    for w, st in zip(wls, streams):
+        ph = gpu.Phylino(stream=st.cuda_stream)
+        ph.load_workload(w)
+        ctxs.append(ph)
+    dev = []
+    for w, d, st in zip(wls, datas, streams):
+        with torch.cuda.stream(st):
+            dev.append((_dev(w.params), _dev(d)))
+    torch.cuda.synchronize()
+    for rep in range(3):
+        for i in (0, 1):
+            with torch.cuda.stream(streams[i]):
+                outs[i].append((ctxs[i].nll(*dev[i]), ctxs[i].spectra(dev[i][0])))
+    torch.cuda.synchronize()
+    for i in (0, 1):
+        nll_o, h_o = orcs[i].nll(wls[i].params, datas[i]), orcs[i].spectra(wls[i].params)
+        for nll, h in outs[i]:
+            assert np.abs(nll.cpu().numpy() - nll_o).max() <= ABS_NLL
+            _check_hist(h.cpu().numpy(), h_o)
+        assert all(np.array_equal(outs[i][0][0].cpu().numpy(), o[0].cpu().numpy()) for o in outs[i][1:])
+    for ph in ctxs:
+        ph.close()
+
+
+def test_reserve_then_cuda_graph(gpu, oracle_mod):
+    """phylino.h "Async": after phylino_reserve the device entry points neither allocate nor synchronise, so a
+    call can be captured into a CUDA graph and replayed (the launch-bound inner loop of a minimiser)."""
+    import torch
+    for k, scale, n_points in ((2, 0.02, 64), (2, 0.02, 1)):
+        wl = workloads.make_config(k, scale=scale, n_points=n_points)
+        orc = oracle_mod.Oracle(wl.model, wl.events)
+        data = _data(orc, wl)
+        st = torch.cuda.Stream()
+        with torch.cuda.stream(st):
+            ph = gpu.Phylino(stream=st.cuda_stream)
+            ph.load_workload(wl)
+            ph.reserve(n_points)
+            dp, dd = _dev(wl.params), _dev(data)
+            out = torch.zeros(n_points, dtype=torch.float64, device="cuda")
+            ph.nll(dp, dd, out)                       # warm: occupancy queries and attributes are set
+            st.synchronize()
+            first = out.cpu().numpy().copy()
+            g = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g, stream=st):
+                ph.nll(dp, dd, out)
+            for shift in (0.0, 1e-3):
+                dp[:, 0] = torch.as_tensor(wl.params[:, 0] * (1.0 + shift), device="cuda")
+                out.zero_()
+                g.replay()
+                st.synchronize()
+                p = wl.params.copy()
+                p[:, 0] *= 1.0 + shift
+                assert np.abs(out.cpu().numpy() - orc.nll(p, data)).max() <= ABS_NLL
+                if shift == 0.0:
+                    assert np.array_equal(out.cpu().numpy(), first)
+        ph.close()
+
+
+# ---- the multi-GPU split, with the REAL library, on one GPU -------------
+@pytest.mark.parametrize("k,scale,n_points", [(2, 0.05, 64), (3, 0.01, 603)])
+@pytest.mark.parametrize("world", [2, 3, 8])
+def test_point_shards_agree_with_the_unsharded_batch(gpu, oracle_mod, k, scale, n_points, world):
+    """Every rank evaluates a contiguous slice of the batch (sharding.shard_points).  A slice is another batch
+    size, hence possibly another schedule and another grouping of the fp64 partial sums before the exact integer
+    accumulation: the slices agree with the unsharded call to rounding (<= 1e-13 relative per bin, <= 1e-9 in the
+    NLL), not bit for bit -- and each meets the parity bars against the oracle on its own."""
+    from paper_2502_15253_b200 import sharding
+    wl = workloads.make_config(k, scale=scale, n_points=n_points)
+    orc = oracle_mod.Oracle(wl.model, wl.events)
+    data = _data(orc, wl)
+    with gpu.Phylino() as ph:
+        ph.load_workload(wl)
+        h_all = ph.spectra(_dev(wl.params)).cpu().numpy()
+        nll_all = ph.nll(_dev(wl.params), _dev(data)).cpu().numpy()
+        h_parts, nll_parts = [], []
+        for rank in range(world):
+            lo, hi = sharding.shard_points(n_points, world, rank)
+            h_parts.append(ph.spectra(_dev(wl.params[lo:hi])).cpu().numpy())
+            nll_parts.append(ph.nll(_dev(wl.params[lo:hi]), _dev(data)).cpu().numpy())
+    h_sh, nll_sh = np.concatenate(h_parts), np.concatenate(nll_parts)
+    assert h_sh.shape == h_all.shape
+    assert np.allclose(h_sh, h_all, rtol=1e-13, atol=0.0)
+    assert np.abs(nll_sh - nll_all).max() <= 1e-9
+    _check_hist(h_sh, orc.spectra(wl.params))
+    assert np.abs(nll_sh - orc.nll(wl.params, data)).max() <= ABS_NLL
+
+
+# ---- the 41 -> 38 flux block through the transformation layer --------------------------------------
+def test_flux_rebinning_block_through_set_transform(gpu, oracle_mod):
+    """41 flux parameters on uniform 0.25-MeV bins (1-11.25 MeV) drive the 38 per-bin flux scales of each of config
+    3's datasets through one 38 x 41 area-conserving block per dataset of phylino_set_transform; NLL and
+    expectations against oracle.transform followed by the oracle."""
+    wl = workloads.make_config(3, scale=0.004, n_points=24)
+    NP = wl.model.n_params
+    edges = workloads.dc_edges()
+    fine = 1.0 + 0.25 * np.arange(42)
+    M = np.zeros((38, 41))
+    off = np.zeros(38)
+    for b in range(38):
+        lo, hi = edges[b], edges[b + 1]
+        for j in range(41):
+            M[b, j] = max(0.0, min(hi, fine[j + 1]) - max(lo, fine[j])) / (hi - lo)
+        off[b] = 1.0 - M[b].sum()
+    # u = theta without the 3 x 38 flux scales (theta[13:127]) + 3 x 41 flux-model parameters at the end
+    keep = np.r_[0:13, 127:NP]
+    n_keep = keep.size
+    n_u = n_keep + 3 * 41
+    copy_src = np.full(NP, -1, np.int32)
+    copy_src[keep] = np.arange(n_keep)
+    blocks = [workloads.TransformBlock(np.arange(13 + 38 * d, 13 + 38 * (d + 1), dtype=np.int32),
+                                       np.arange(n_keep + 41 * d, n_keep + 41 * (d + 1), dtype=np.int32),
+                                       off, np.zeros(41), M) for d in range(3)]
+    spec = workloads.TransformSpec(n_u=n_u, copy_src=copy_src, copy_const=np.zeros(NP), blocks=blocks)
+    rng = np.random.default_rng(12)
+    u = np.zeros((24, n_u))
+    u[:, :n_keep] = wl.params[:, keep]
+    u[:, n_keep:] = 1.0 + 0.02 * rng.normal(size=(24, 123))
+    theta = oracle_mod.transform(spec, NP, u)
+    assert np.allclose(theta[:, 13:13 + 28], u[:, n_keep:n_keep + 28], rtol=1e-14)     # 1-8 MeV: bins coincide
+    orc = oracle_mod.Oracle(wl.model, wl.events)
+    data = _data(orc, wl)
+    with gpu.Phylino() as ph:
+        ph.load_workload(wl)
+        ph.set_transform(spec)
+        nll = ph.nll(_dev(u), _dev(data)).cpu().numpy()
+        mu = ph.expectation(_dev(u)).cpu().numpy()
+        nll_h = ph.nll_host(u, data)
+    assert np.abs(nll - orc.nll(theta, data)).max() <= ABS_NLL
+    assert np.array_equal(nll, nll_h)
+    _check_hist(mu, orc.expectation(theta, orc.spectra(theta)))

@@ -223,14 +223,14 @@ def _config3(rng, scale, n_points):
     return model, evs, params, theta0
 
 
-def _config4(rng, scale, n_points):
+def _config4(rng, scale, n_points, ordering=+1):
     edges = 0.8 + np.arange(411, dtype=np.float64) * 0.02
     L = [52_000.0 + 100.0 * i for i in range(9)] + [215_000.0, 265_000.0]
     prob = [0.1] * 9 + [0.05, 0.05]
     ev = reactor_events(rng, _n(10_000_000, scale), L, prob, 0.03, edges)
     theta0 = np.array([THETA0["s13"], THETA0["mee"], THETA0["s12"], THETA0["m21"]])
     sig = np.array([SIGMA0["s13"], SIGMA0["mee"], SIGMA0["s12"], SIGMA0["m21"]])
-    model = ModelSpec(osc_model=OSC_FULL3, ordering=+1, n_params=4, idx_osc=(0, 1, 2, 3, -1, -1),
+    model = ModelSpec(osc_model=OSC_FULL3, ordering=ordering, n_params=4, idx_osc=(0, 1, 2, 3, -1, -1),
                       fixed_osc=(0, 0, 0, 0, 0.0, 0.0),
                       datasets=[DatasetSpec(n_bins=410, norm=0.05)],
                       prior_mean=theta0.copy(), prior_sigma=np.zeros(4))   # no systematics
@@ -265,12 +265,19 @@ _BUILDERS = {1: _config1, 2: _config2, 3: _config3, 4: _config4, 5: _config5}
 
 
 def make_config(k: int, seed: int | None = None, scale: float = 1.0,
-                n_points: int | None = None) -> Workload:
+                n_points: int | None = None, ordering: int = +1) -> Workload:
     """BASELINE.json config k (1-based).  `scale` shrinks the event counts and `n_points`
-    truncates the batch, for parity cases the oracle finishes in seconds."""
+    truncates the batch, for parity cases the oracle finishes in seconds.  `ordering` = -1 turns
+    config 4 (the only one with the full 3-flavour P_ee) to the inverted mass ordering (PAPER.md:226);
+    the same events and points, BASELINE.json's config 4 itself is the normal ordering."""
     seed = DEFAULT_SEEDS[k] if seed is None else seed
     rng = np.random.Generator(np.random.PCG64(seed))
-    model, evs, params, theta0 = _BUILDERS[k](rng, scale, n_points)
+    if k == 4:
+        model, evs, params, theta0 = _config4(rng, scale, n_points, ordering)
+    else:
+        if ordering != +1:
+            raise ValueError("only config 4 (FULL3) has a mass ordering")
+        model, evs, params, theta0 = _BUILDERS[k](rng, scale, n_points)
     return Workload(name=CONFIG_NAMES[k], model=model, events=evs,
                     params=np.ascontiguousarray(params, dtype=np.float64),
                     theta0=np.asarray(theta0, dtype=np.float64), seed=seed,
@@ -278,7 +285,7 @@ def make_config(k: int, seed: int | None = None, scale: float = 1.0,
 
 
 def make_tiny(seed: int, osc_model: int = OSC_EQ1, n_events: int = 100, n_points: int = 5,
-              n_datasets: int = 1) -> Workload:
+              n_datasets: int = 1, ordering: int = +1) -> Workload:
     """<= 100 events per dataset, U(0.5,1.5) weights, 3 cores, 7 non-uniform bins: brute-force size."""
     rng = np.random.Generator(np.random.PCG64(seed))
     edges = np.array([1.0, 1.5, 2.25, 3.0, 3.5, 4.75, 6.0, 9.0])
@@ -309,7 +316,7 @@ def make_tiny(seed: int, osc_model: int = OSC_EQ1, n_events: int = 100, n_points
     prior_sigma = sig.copy()
     prior_sigma[0] = 0.0
     model = ModelSpec(osc_model=osc_model, n_params=npar, idx_osc=(0, 1, 2, 3, 4, 5),
-                      fixed_osc=(0,) * 6, datasets=dsets, prior_mean=theta0.copy(),
+                      fixed_osc=(0,) * 6, datasets=dsets, ordering=ordering, prior_mean=theta0.copy(),
                       prior_sigma=prior_sigma)
     params = theta0[None, :] + rng.standard_normal((n_points, npar)) * sig[None, :]
     params[0] = theta0
