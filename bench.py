@@ -3,10 +3,17 @@
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config k] [--impl ours|reference]
 
-A step = one phylino_nll call over the whole batch of parameter points of the workload (all rows of
+A step = one phylino_nll call over the whole batch of parameter points of a workload (all rows of
 SURVEY.md 8(a): per-point derivation, oscillation weights, energy scale + binning, scatter-add,
-deterministic reduction, expectation assembly, NLL reduction).  Default workload: BASELINE.json
-configs[1] (Double Chooz FD+ND, 2 x 1e6 events, 64 points).  Prints ONE JSON line (rank 0).
+deterministic reduction, expectation assembly, NLL reduction).
+
+Headline workload (`value`, `roofline`, `e2e`, `clocks`): BASELINE.json names no config for its metric, so
+it is the LARGEST single-GPU one, configs[4] (sterile grid scan: 2 x 1e6 events x 4096 points = 8.19e9
+event x point per step), timed for exactly K steps.  At one GPU the line also carries `configs`: all five
+BASELINE.json configs measured in the same run, each with value, median / min / mean ms per step, the spectra
+kernel's own duration and roofline fraction, dram traffic and end-to-end numbers; config 1 (one point, 1e5
+events: launch-latency bound) with its single-call latencies; config 3 with the wall time of the 603-point
+gradient step, dense and with cross-point caching.  `--config k` makes config k the headline and skips the rest.
 
 N > 1 (torchrun): the path shards by parameter point with no data-path collective -- every rank
 holds the event store and evaluates its own batch of points ("weak" scaling).
@@ -32,14 +39,17 @@ import workloads  # noqa: E402
 
 METRIC = "oscillated event x param-point/s (batched spectra+NLL)"
 UNIT = "event*point/s"
+HEADLINE_CONFIG = 5
 # ALGORITHMIC fp64-pipe instructions per event x point: per oscillation term
 # 10 for 1/2 cos(2 phase) (3 range reduction, 1 square, 6 Horner) + 1 multiply-accumulate into the run;
-# the SASS of the hot loop has exactly these (9 DFMA + 1 DADD + 1 DMUL per event x point x term).
-# The bin/weight bookkeeping is per batch of events and per run, not per event x point.
+# the SASS of the hot loop has exactly these (9 DFMA + 1 DADD + 1 DMUL per event x point x term,
+# profiles/r2_hot_loop_sass.md).  The bin/weight bookkeeping is per batch of events and per run, not per event x point.
 FP64_PER_TERM = 11
-# nominal fp64 pipe: 64 lanes/clk/SM x 148 SMs x 1.965 GHz (B200_PROFILING.md table)
-PEAK_FP64_INST = 64 * 148 * 1.965e9
+# nominal fp64 pipe, derived in DESIGN.md section 7 (the guide has no fp64 row): 64 fp64 lanes/clk/SM (one DFMA
+# per lane and clock) x SMs x the SM clock nvidia-smi reports as maximum
+FP64_LANES_PER_SM = 64
 L2_FLUSH_BYTES = 256 << 20
+EVENT_BYTES = 12            # unit-weight store: x fp64 + E_vis fp32 (every BASELINE.json config)
 
 
 def fp64_inst_per_evpt(model) -> int:
@@ -105,15 +115,251 @@ def physical_gpu_index(local: int) -> int:
 
 
 def traffic_from_profile(config: int):
-    """dram bytes (read + write) per launch of the spectra kernel for this config, from the committed
-    summary of the ncu --set full capture (profiles/spectra_kernel_traffic.csv), or None."""
+    """(dram bytes read + written per launch of the spectra kernel, where the number comes from) for this config,
+    from the committed summary of the `ncu --set full` captures (profiles/spectra_kernel_traffic.csv); (None, why)
+    if there is no row.  A number taken under a profiler is never a bench value: this is the ONE quantity of the
+    line that is not measured in this run, and `traffic_source` says so."""
     import csv
     p = os.path.join(ROOT, "profiles", "spectra_kernel_traffic.csv")
     try:
         rows = [r for r in csv.DictReader(open(p)) if int(r["config"]) == config]
-        return int(rows[-1]["dram_bytes_read"]) + int(rows[-1]["dram_bytes_write"])
+        r = rows[-1]
+        return (int(r["dram_bytes_read"]) + int(r["dram_bytes_write"]),
+                f"profiles/spectra_kernel_traffic.csv, capture {r['capture']} ({r['kernel']}; ncu --set full, one launch; "
+                "not measured in this run)")
     except Exception:
-        return None
+        return None, "no ncu capture of this config under profiles/"
+
+
+def stats_ms(ms):
+    return {"mean": sum(ms) / len(ms), "median": statistics.median(ms), "min": min(ms), "max": max(ms)}
+
+
+def oracle_rates(wl, data, n_all=64, n_one=4):
+    """The CPU oracle as it stands, on a bounded sample of this workload: all host cores (OpenMP over points) and
+    one thread.  Test infrastructure: only the cpu_baseline leg comes here."""
+    import oracle
+    orc = oracle.Oracle(wl.model, wl.events)
+    P = wl.n_points
+    n_all = min(P, n_all)
+    t0 = time.perf_counter()
+    nll_o = orc.nll(wl.params[:n_all], data)
+    dt_all = time.perf_counter() - t0
+    n_one = min(P, n_one)
+    t0 = time.perf_counter()
+    orc.nll(wl.params[:n_one], data, n_threads=1)
+    dt_one = time.perf_counter() - t0
+    return {"value": wl.n_events * n_all / dt_all, "unit": UNIT, "cores": oracle.max_threads(), "kind": "oracle",
+            "sample": f"all {wl.n_events} events x first {n_all} of {P} points, one call, {dt_all:.2f} s",
+            "single_thread": {"value": wl.n_events * n_one / dt_one, "unit": UNIT, "cores": 1,
+                              "sample": f"all {wl.n_events} events x first {n_one} of {P} points, one call, {dt_one:.2f} s"}}, nll_o
+
+
+def measure(pkg, torch, dist, k, steps, warmup, local, rank, world, flush, tuning, sample_clocks, measured_peak,
+            with_oracle):
+    """All numbers of one config: K device-timed steps (CUDA events per step, L2 flushed in between), the same K steps
+    with the library's events around each kernel, the end-to-end host-buffer call, the cached host call."""
+    wl = workloads.make_config(k)
+    params = wl.params.copy()
+    if rank > 0:    # every rank: the same event store, its own batch of points (sharded by parameter point)
+        rng = np.random.Generator(np.random.PCG64(wl.seed + 1000 * rank))
+        spread = np.abs(wl.params - wl.theta0[None, :]).max(axis=0)
+        params = wl.theta0[None, :] + rng.uniform(-1, 1, wl.params.shape) * spread[None, :]
+    ph = pkg.Phylino(device=local)
+    ph.load_workload(wl)
+    if any(tuning):
+        ph.set_tuning(*tuning)
+    P, NPAR, TB = wl.n_points, wl.model.n_params, ph.total_bins
+    ph.reserve(P)
+    d_params = torch.as_tensor(params, device="cuda")
+    # pseudo-data: Poisson counts around the product's own expectation at theta0 (input synthesis only)
+    mu0 = ph.expectation(torch.as_tensor(wl.theta0[None, :].copy(), device="cuda")).cpu().numpy()[0]
+    data = workloads.poisson_counts(mu0, wl.seed + 7)
+    d_data = torch.as_tensor(data, device="cuda")
+    d_nll = torch.empty(P, dtype=torch.float64, device="cuda")
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+
+    # ---- device-resident timed region: K steps, CUDA events per step, L2 flushed in between.  The library's
+    # own per-kernel events are OFF here (with them off the kernels of a call go out as programmatic dependent
+    # launches) ----
+    ph.set_timing(False)
+    for _ in range(warmup):
+        ph.nll(d_params, d_data, d_nll)
+        flush.zero_()
+    starts = [torch.cuda.Event(enable_timing=True) for _ in range(steps)]
+    ends = [torch.cuda.Event(enable_timing=True) for _ in range(steps)]
+    sampler = ClockSampler(physical_gpu_index(local)) if sample_clocks else None
+    launches0 = ph.launch_count
+    barrier()
+    torch.cuda.synchronize()
+    if sampler:
+        sampler.start()
+    for i in range(steps):
+        starts[i].record()
+        ph.nll(d_params, d_data, d_nll)
+        ends[i].record()
+        flush.zero_()
+    torch.cuda.synchronize()
+    launches = ph.launch_count - launches0
+    barrier()
+    step_ms = [s.elapsed_time(e) for s, e in zip(starts, ends)]
+    total_ms = sum(step_ms)
+    # ---- the same K steps with the library's events around each of the kernels of a call (recorded on the
+    # stream the kernels run on): the per-kernel durations the roofline uses ----
+    ph.set_timing(True)
+    su_ms, sp_ms, fin_ms, inst_ms = [], [], [], []
+    for i in range(steps):
+        s0, e0 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        s0.record()
+        ph.nll(d_params, d_data, d_nll)
+        e0.record()
+        a, b, c = ph.last_kernel_ms()       # waits for this step; per-kernel device times
+        su_ms.append(a)
+        sp_ms.append(b)
+        fin_ms.append(c)
+        inst_ms.append(s0.elapsed_time(e0))
+        flush.zero_()
+    torch.cuda.synchronize()
+    clocks = sampler.stop() if sampler else None
+    barrier()
+    if world > 1:
+        t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+    ms_per_step = total_ms / steps
+    evpt_step = wl.n_events * P
+    value = world * evpt_step / (ms_per_step * 1e-3)
+
+    # ---- end to end through the host-buffer entry point: params + data in, kernels, nll out, every step ----
+    ph.set_timing(False)
+    h_params = params.copy()
+    out = np.empty(P)
+    for _ in range(warmup):
+        ph.nll_host(h_params, data, out)
+    barrier()
+    torch.cuda.synchronize()
+    e2e_ms = []
+    for i in range(steps):
+        h_params[:, 0] = params[:, 0] * (1.0 + 1e-9 * i)     # a fresh batch every step
+        flush.zero_()
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        ph.nll_host(h_params, data, out)
+        e2e_ms.append((time.perf_counter() - t0) * 1e3)
+    e2e_s = sum(e2e_ms) * 1e-3
+    if world > 1:
+        t = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_s = float(t.item())
+    e2e_value = world * evpt_step * steps / e2e_s
+
+    # ---- cross-point caching (SURVEY.md 8(f) NEXT-1), reported beside the dense numbers, never instead of
+    # them: the same host-buffer call with phylino_set_caching(1); wall time of one whole batch (config 3: one
+    # central-difference gradient step; config 5: one grid scan), every step a fresh batch.
+    cached = None
+    ph.set_caching(True)
+    ph.nll_host(h_params, data, out)
+    vp, classes = ph.last_plan()
+    if vp > 0:
+        for _ in range(warmup):
+            ph.nll_host(h_params, data, out)
+        torch.cuda.synchronize()
+        c_ms = []
+        for i in range(steps):
+            h_params[:, 0] = params[:, 0] * (1.0 + 1e-9 * (i + 1))
+            flush.zero_()
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            ph.nll_host(h_params, data, out)
+            c_ms.append((time.perf_counter() - t0) * 1e3)
+        dense_ref = np.empty(P)
+        ph.set_caching(False)
+        ph.nll_host(h_params, data, dense_ref)
+        cached = {"ms_per_step": stats_ms(c_ms), "virtual_points": vp, "energy_scale_classes": classes,
+                  "points": P, "max_abs_nll_diff_vs_dense": float(np.nanmax(np.abs(out - dense_ref))),
+                  "note": "phylino_nll_host with phylino_set_caching(1): H2D + plan + kernels + D2H, host wall time; "
+                          "not comparable with the dense roofline (fewer event x point evaluations are executed)"}
+    ph.set_caching(False)
+
+    res = None
+    if rank == 0:
+        inst = fp64_inst_per_evpt(wl.model)
+        small = P <= 16 and not (inst == 33 and P > 4)      # the small-batch kernel (setup fused in) ran
+        sp = stats_ms(sp_ms)
+        sm_max_mhz = (clocks or {}).get("sm_max_mhz") or 1965.0
+        sm_count = torch.cuda.get_device_properties(local).multi_processor_count
+        peak_nominal = FP64_LANES_PER_SM * sm_count * sm_max_mhz * 1e6
+        achieved = inst * evpt_step / (sp["mean"] * 1e-3)
+        traffic, traffic_source = traffic_from_profile(k)
+        hbm_bytes = EVENT_BYTES * wl.n_events + 8 * P * NPAR + 8 * P
+        roofline = {
+            "bound": "alu", "kernel": "spectra_fused_kernel" if small else "spectra_kernel",
+            "achieved": achieved / 1e9, "peak": peak_nominal / 1e9, "unit": "fp64 Ginst/s",
+            "frac": achieved / peak_nominal, "frac_of": "nominal fp64 pipe",
+            "peak_source": f"nominal: {FP64_LANES_PER_SM} fp64 lanes/clk/SM x {sm_count} SMs x {sm_max_mhz:.0f} MHz "
+                           "(derived in DESIGN.md section 7; MEASURED_PEAKS.json and the profiling guide hold no fp64 figure)",
+            "measured_dfma_peak": None if measured_peak is None else measured_peak / 1e9,
+            "frac_of_measured_dfma_peak": None if not measured_peak else achieved / measured_peak,
+            "traffic": traffic, "traffic_source": traffic_source,
+            "fp64_inst_per_event_point": inst, "kernel_ms": sp["mean"], "kernel_ms_median": sp["median"],
+            "kernel_ms_min": sp["min"],
+            "kernel_share_of_step": sp["mean"] / (sum(inst_ms) / steps),
+            "kernel_timing": f"second pass of {steps} steps with CUDA events around each kernel on the library's "
+                             f"stream ({sum(inst_ms) / steps:.4f} ms per instrumented step)",
+            "setup_kernel_ms": sum(su_ms) / steps, "finalize_kernel_ms": sum(fin_ms) / steps,
+            "hbm_bytes_per_launch": hbm_bytes,
+            "hbm_frac_if_bandwidth_bound": None,
+        }
+        if small:
+            # one point over the store is bound by the event bytes (and, at 1e5 events, by launch latency): the same
+            # kernel time against the HBM roofline of MEASURED_PEAKS.json
+            hbm_gbs = measured_hbm_gbs()
+            roofline["hbm_frac_if_bandwidth_bound"] = hbm_bytes / (sp["mean"] * 1e-3) / (hbm_gbs * 1e9)
+            roofline["hbm_peak_gbs"] = hbm_gbs
+        st = stats_ms(step_ms)
+        res = {
+            "config": k, "workload": f"{wl.name} (BASELINE.json configs[{k - 1}])", "events": wl.n_events,
+            "points_per_gpu": P, "n_params": NPAR, "total_bins": TB, "steps": steps, "warmup": warmup,
+            "value": value, "unit": UNIT, "ms_per_step": ms_per_step, "ms_per_step_median": st["median"],
+            "ms_per_step_min": st["min"], "gpu_launches": launches,
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 8 * (P * NPAR + TB),
+                    "d2h_bytes_per_step": 8 * P, "ms_per_step": e2e_s / steps * 1e3,
+                    "ms_per_step_median": statistics.median(e2e_ms), "ms_per_step_min": min(e2e_ms),
+                    "call": "phylino_nll_host: pinned staging, parameters + data to the device, kernels, nll[P] back, "
+                            "one synchronise; host wall clock, L2 flushed before every call"},
+            "roofline": roofline, "clocks": clocks,
+        }
+        if cached is not None:
+            res["cached"] = cached
+        if evpt_step <= 10_000_000:
+            # launch-latency-bound workload (config 1): one host call against the empty-kernel floor, cold (L2
+            # flushed before the call: the e2e numbers above) and warm (back to back, as a minimiser calls it)
+            warm = []
+            for i in range(max(steps, 50)):
+                t0 = time.perf_counter()
+                ph.nll_host(h_params, data, out)
+                warm.append((time.perf_counter() - t0) * 1e6)
+            res["latency"] = {"host_call_us_cold_median": statistics.median(e2e_ms) * 1e3, "host_call_us_cold_min": min(e2e_ms) * 1e3,
+                              "host_call_us_warm_median": statistics.median(warm), "host_call_us_warm_min": min(warm),
+                              "device_step_us_median": st["median"] * 1e3, "device_step_us_min": st["min"] * 1e3,
+                              "launch_plus_sync_floor_us": ph.launch_floor(200),
+                              "note": "a call is 2 launches (spectra with the setup fused in; finalize, overlapped) "
+                                      "+ 1 synchronise; no copy engine (parameters ride with the kernel arguments)"}
+        if with_oracle:
+            res["cpu_baseline"], nll_o = oracle_rates(wl, data)
+            res["cpu_baseline"]["max_abs_nll_diff_vs_gpu"] = float(np.abs(nll_o - d_nll.cpu().numpy()[:len(nll_o)]).max())
+    ph.close()
+    return res
+
+
+def measured_hbm_gbs() -> float:
+    try:
+        return float(json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"])
+    except Exception:
+        return 6553.6       # the profiling guide's fallback for this pool's B200s
 
 
 def gradient_step_wall(pkg, torch, local, flush, steps=10):
@@ -134,15 +380,17 @@ def gradient_step_wall(pkg, torch, local, flush, steps=10):
         for _ in range(3):
             ph.nll_host(h, data, out)
         torch.cuda.synchronize()
-        t = 0.0
+        ts = []
         for i in range(steps):
             h[:, 0] = wl.params[:, 0] * (1.0 + 1e-9 * (i + 1))
             flush.zero_()
             torch.cuda.synchronize()
             t0 = time.perf_counter()
             ph.nll_host(h, data, out)
-            t += time.perf_counter() - t0
-        res[key] = t / steps * 1e3
+            ts.append((time.perf_counter() - t0) * 1e3)
+        res[key] = sum(ts) / steps
+        res[key + "_median"] = statistics.median(ts)
+        res[key + "_min"] = min(ts)
         if on:
             res["virtual_points"], res["energy_scale_classes"] = ph.last_plan()
     ph.close()
@@ -172,7 +420,8 @@ def run_reference(args, wl, rank):
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
-        "data": "synthetic", "config": {"workload": wl.name, "events": wl.n_events, "points": n_pts},
+        "data": "synthetic", "config": {"workload": f"{wl.name} (BASELINE.json configs[{args.config - 1}])",
+                                        "events": wl.n_events, "points": n_pts},
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0}))
@@ -181,10 +430,13 @@ def run_reference(args, wl, rank):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--steps", type=int, default=100)
     ap.add_argument("--warmup", type=int, default=5)
-    ap.add_argument("--config", type=int, default=2, help="BASELINE.json config, 1-based (default 2 = configs[1])")
+    ap.add_argument("--config", type=int, default=0,
+                    help="BASELINE.json config, 1-based, as the headline and only workload (default: config 5 as the "
+                         "headline plus all five in `configs`)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--other-steps", type=int, default=20, help="steps per config of the `configs` array")
     ap.add_argument("--unit-events", type=int, default=0, help="tuning: events per unit of the event store")
     ap.add_argument("--chunk-groups", type=int, default=0, help="tuning: groups of 32 points per work item")
     ap.add_argument("--max-warps", type=int, default=0, help="tuning: cap on the persistent grid's warps")
@@ -194,14 +446,16 @@ def main():
                     help="skip the wall time of config 3's 603-point gradient step that the default run adds")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    all_configs = args.config == 0
+    if all_configs:
+        args.config = HEADLINE_CONFIG
 
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
-    wl = workloads.make_config(args.config)
 
     if args.impl == "reference":
-        run_reference(args, wl, rank)
+        run_reference(args, workloads.make_config(args.config), rank)
         return
 
     import torch
@@ -213,191 +467,49 @@ def main():
     torch.cuda.set_device(local)
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-
-    # every rank: the same event store, its own batch of points (sharded by parameter point)
-    params = wl.params.copy()
-    if rank > 0:
-        rng = np.random.Generator(np.random.PCG64(wl.seed + 1000 * rank))
-        spread = np.abs(wl.params - wl.theta0[None, :]).max(axis=0)
-        params = wl.theta0[None, :] + rng.uniform(-1, 1, wl.params.shape) * spread[None, :]
-    ph = pkg.Phylino(device=local)
-    ph.load_workload(wl)
-    if args.unit_events or args.chunk_groups or args.max_warps:
-        ph.set_tuning(args.unit_events, args.chunk_groups, args.max_warps)
-    P, NPAR, TB = wl.n_points, wl.model.n_params, ph.total_bins
-    d_params = torch.as_tensor(params, device="cuda")
-    # pseudo-data: Poisson counts around the product's own expectation at theta0 (input synthesis only)
-    mu0 = ph.expectation(torch.as_tensor(wl.theta0[None, :].copy(), device="cuda")).cpu().numpy()[0]
-    data = workloads.poisson_counts(mu0, wl.seed + 7)
-    d_data = torch.as_tensor(data, device="cuda")
-    d_nll = torch.empty(P, dtype=torch.float64, device="cuda")
     flush = torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device="cuda")
+    tuning = (args.unit_events, args.chunk_groups, args.max_warps)
 
-    def barrier():
-        if world > 1:
-            dist.barrier()
-
-    for _ in range(args.warmup):
-        ph.nll(d_params, d_data, d_nll)
-        flush.zero_()
-    torch.cuda.synchronize()
-
-    # ---- device-resident timed region: K steps, CUDA events per step, L2 flushed in between.  The library's
-    # own per-kernel events are OFF here (they sit between the three launches and cost ~10 us per step; with
-    # them off the spectra and finalize kernels go out as programmatic dependent launches) ----
-    starts = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps)]
-    ends = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps)]
-    sampler = ClockSampler(physical_gpu_index(local))
-    ph.set_timing(False)
-    for _ in range(2):
-        ph.nll(d_params, d_data, d_nll)
-        flush.zero_()
-    launches0 = ph.launch_count
-    barrier()
-    torch.cuda.synchronize()
-    sampler.start()
-    for i in range(args.steps):
-        starts[i].record()
-        ph.nll(d_params, d_data, d_nll)
-        ends[i].record()
-        flush.zero_()
-    torch.cuda.synchronize()
-    launches = ph.launch_count - launches0
-    barrier()
-    total_ms = sum(s.elapsed_time(e) for s, e in zip(starts, ends))
-    # ---- same K steps again with the library's events around each of the three kernels (recorded on the
-    # stream the kernels run on): the per-kernel durations the roofline uses ----
-    ph.set_timing(True)
-    su_ms, sp_ms, fin_ms = [], [], []
-    inst_ms = 0.0
-    for i in range(args.steps):
-        s0, e0 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        s0.record()
-        ph.nll(d_params, d_data, d_nll)
-        e0.record()
-        a, b, c = ph.last_kernel_ms()       # waits for this step; per-kernel device times
-        su_ms.append(a)
-        sp_ms.append(b)
-        fin_ms.append(c)
-        inst_ms += s0.elapsed_time(e0)
-        flush.zero_()
-    torch.cuda.synchronize()
-    clocks = sampler.stop()
-    barrier()
-    if world > 1:
-        t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
-    ms_per_step = total_ms / args.steps
-    evpt_step = wl.n_events * P
-    value = world * evpt_step / (ms_per_step * 1e-3)
-
-    # ---- end to end through the host-buffer entry point: H2D params+data, kernels, D2H nll ----
-    ph.set_timing(False)
-    h_params = params.copy()
-    out = np.empty(P)
-    for _ in range(args.warmup):
-        ph.nll_host(h_params, data, out)
-    barrier()
-    torch.cuda.synchronize()
-    e2e_s = 0.0
-    for i in range(args.steps):
-        h_params[:, 0] = params[:, 0] * (1.0 + 1e-9 * i)     # a fresh batch every step
-        t0 = time.perf_counter()
-        ph.nll_host(h_params, data, out)
-        e2e_s += time.perf_counter() - t0
-        flush.zero_()
-        torch.cuda.synchronize()
-    if world > 1:
-        t = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_s = float(t.item())
-    e2e_value = world * evpt_step * args.steps / e2e_s
-
-    # ---- cross-point caching, reported beside the dense numbers, never instead of
-    # them: the same host-buffer call with phylino_set_caching(1); wall time of one whole batch (config 3: one
-    # central-difference gradient step; config 5: one grid scan), every step a fresh batch.
-    cached = None
-    ph.set_caching(True)
-    ph.nll_host(h_params, data, out)
-    vp, classes = ph.last_plan()
-    if vp > 0:
-        for _ in range(args.warmup):
-            ph.nll_host(h_params, data, out)
-        torch.cuda.synchronize()
-        c_s = 0.0
-        for i in range(args.steps):
-            h_params[:, 0] = params[:, 0] * (1.0 + 1e-9 * (i + 1))
-            t0 = time.perf_counter()
-            ph.nll_host(h_params, data, out)
-            c_s += time.perf_counter() - t0
-            flush.zero_()
-            torch.cuda.synchronize()
-        dense_ref = np.empty(P)
-        ph.set_caching(False)
-        ph.nll_host(h_params, data, dense_ref)
-        cached = {"ms_per_step": c_s / args.steps * 1e3, "virtual_points": vp, "energy_scale_classes": classes,
-                  "points": P, "max_abs_nll_diff_vs_dense": float(np.nanmax(np.abs(out - dense_ref))),
-                  "note": "phylino_nll_host with phylino_set_caching(1): H2D + plan + kernels + D2H; "
-                          "not comparable with the dense roofline (fewer event x point evaluations are executed)"}
-    ph.set_caching(False)
-
+    measured_peak = None
     if rank == 0:
-        inst = fp64_inst_per_evpt(wl.model)
-        sp_avg = sum(sp_ms) / len(sp_ms)
-        achieved = inst * evpt_step / (sp_avg * 1e-3)
         try:
-            measured_peak = ph.peak_fp64(8192)
+            with pkg.Phylino(device=local) as ph0:
+                measured_peak = ph0.peak_fp64(8192)
         except Exception:
             measured_peak = None
-        roofline = {
-            "bound": "alu", "kernel": "spectra_kernel", "achieved": achieved / 1e9, "peak": PEAK_FP64_INST / 1e9,
-            "unit": "fp64 Ginst/s", "frac": achieved / PEAK_FP64_INST, "traffic": traffic_from_profile(args.config),
-            "peak_source": "nominal: 64 fp64 lanes/clk/SM x 148 SMs x 1.965 GHz (DESIGN.md)",
-            "measured_dfma_peak": None if measured_peak is None else measured_peak / 1e9,
-            "frac_of_measured": None if not measured_peak else achieved / measured_peak,
-            "fp64_inst_per_event_point": inst, "kernel_ms": sp_avg,
-            "kernel_share_of_step": sp_avg / (inst_ms / args.steps),
-            "kernel_timing": f"second pass of {args.steps} steps with CUDA events around each kernel on the library's "
-                             f"stream ({inst_ms / args.steps:.4f} ms per instrumented step)",
-            "setup_kernel_ms": sum(su_ms) / len(su_ms), "finalize_kernel_ms": sum(fin_ms) / len(fin_ms),
-            "hbm_bytes_per_launch": 24 * wl.n_events + 8 * P * TB,
-        }
+
+    with_oracle = world == 1 and not args.no_cpu_baseline
+    head = measure(pkg, torch, dist, args.config, args.steps, args.warmup, local, rank, world, flush, tuning, True,
+                   measured_peak, with_oracle)
+    others = []
+    if all_configs and world == 1:
+        for k in (1, 2, 3, 4):
+            others.append(measure(pkg, torch, dist, k, args.other_steps, args.warmup, local, rank, world, flush, tuning,
+                                  False, measured_peak, with_oracle))
+
+    if rank == 0:
         line = {
-            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+            "metric": METRIC, "value": head["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": head["ms_per_step"], "ms_per_step_median": head["ms_per_step_median"],
+            "ms_per_step_min": head["ms_per_step_min"], "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": f"{wl.name} (BASELINE.json configs[{args.config - 1}])",
-                       "events": wl.n_events, "points_per_gpu": P, "n_params": NPAR, "total_bins": TB,
+            "config": {"workload": head["workload"] + (": the largest single-GPU config (BASELINE.json's metric names none)"
+                                                       if all_configs else ""),
+                       "events": head["events"], "points_per_gpu": head["points_per_gpu"], "n_params": head["n_params"],
+                       "total_bins": head["total_bins"],
                        "l2": f"flushed between timed iterations ({L2_FLUSH_BYTES >> 20} MiB write)",
                        "sharding": "by parameter point, event store replicated, no collective"},
-            "clocks": clocks, "gpu_launches": launches,
-            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": 8 * (P * NPAR + TB),
-                    "d2h_bytes_per_step": 8 * P, "ms_per_step": e2e_s / args.steps * 1e3},
-            "roofline": roofline,
+            "clocks": head["clocks"], "gpu_launches": head["gpu_launches"],
+            "e2e": head["e2e"], "roofline": head["roofline"],
         }
-        if cached is not None:
-            line["cached"] = cached
-        if wl.n_events * P <= 10_000_000:
-            # launch-latency-bound workload (config 1): one host call against the empty-kernel floor
-            line["latency"] = {"host_call_us": e2e_s / args.steps * 1e6, "device_step_us": ms_per_step * 1e3,
-                               "launch_plus_sync_floor_us": ph.launch_floor(200),
-                               "note": "a call is 1 H2D + 3 kernels + 1 D2H + 1 synchronise"}
-        if world == 1 and args.config == 2 and not args.no_gradient_step:
+        for key in ("cached", "latency", "cpu_baseline"):
+            if key in head:
+                line[key] = head[key]
+        if others:
+            line["configs"] = sorted(others + [head], key=lambda r: r["config"])
+        if world == 1 and all_configs and not args.no_gradient_step:
             line["gradient_step"] = gradient_step_wall(pkg, torch, local, flush)
-        if world == 1 and not args.no_cpu_baseline:
-            import oracle                                   # the cpu_baseline leg (test infrastructure)
-            orc = oracle.Oracle(wl.model, wl.events)
-            n_pts = min(P, 64)
-            t0 = time.perf_counter()
-            nll_o = orc.nll(wl.params[:n_pts], data)
-            dt = time.perf_counter() - t0
-            line["cpu_baseline"] = {
-                "value": wl.n_events * n_pts / dt, "unit": UNIT, "cores": oracle.max_threads(), "kind": "oracle",
-                "sample": f"all {wl.n_events} events x first {n_pts} of {P} points, one call, {dt:.2f} s",
-                "max_abs_nll_diff_vs_gpu": float(np.abs(nll_o - d_nll.cpu().numpy()[:n_pts]).max())}
         print(json.dumps(line))
-    ph.close()
     if world > 1:
         dist.destroy_process_group()
 
