@@ -94,6 +94,16 @@ def _load():
         lib.orc_transform.restype = C.c_int
         lib.orc_transform.argtypes = [C.c_int32, C.c_int32, C.c_void_p, C.c_void_p, C.c_int32,
                                       C.POINTER(_TransformBlock), C.c_int32, dp, dp]
+        lib.orc_philox4x32_10.restype = None
+        lib.orc_philox4x32_10.argtypes = [C.POINTER(C.c_uint32), C.POINTER(C.c_uint32), C.POINTER(C.c_uint32)]
+        lib.orc_uniform53.restype = C.c_double
+        lib.orc_uniform53.argtypes = [C.c_uint64, C.c_uint32, C.c_uint32]
+        lib.orc_poisson_norm.restype = C.c_double
+        lib.orc_poisson_norm.argtypes = [C.c_double]
+        lib.orc_poisson_inv.restype = C.c_double
+        lib.orc_poisson_inv.argtypes = [C.c_double, C.c_double, C.c_double]
+        lib.orc_draw_pseudo_data.restype = C.c_int
+        lib.orc_draw_pseudo_data.argtypes = [C.c_int64, dp, C.c_int32, C.c_uint64, dp]
         lib.orc_max_threads.restype = C.c_int
         _lib = lib
     return _lib
@@ -294,3 +304,34 @@ def transform(spec, n_params: int, u) -> np.ndarray:
 
 def max_threads() -> int:
     return int(_load().orc_max_threads())
+
+
+# -- pseudo-experiments (R26) ---------------------------------------------
+def philox4x32_10(ctr, key):
+    c = (C.c_uint32 * 4)(*[int(x) for x in ctr])
+    k = (C.c_uint32 * 2)(*[int(x) for x in key])
+    out = (C.c_uint32 * 4)()
+    _load().orc_philox4x32_10(c, k, out)
+    return [int(x) for x in out]
+
+
+def uniform53(seed: int, bin_index: int, experiment: int) -> float:
+    return float(_load().orc_uniform53(int(seed), int(bin_index), int(experiment)))
+
+
+def poisson_norm(mu: float) -> float:
+    return float(_load().orc_poisson_norm(float(mu)))
+
+
+def poisson_inv(mu: float, Z: float, u: float) -> float:
+    return float(_load().orc_poisson_inv(float(mu), float(Z), float(u)))
+
+
+def draw_pseudo_data(mu, n_experiments: int, seed: int) -> np.ndarray:
+    """data [E, total_bins]: Poisson-fluctuated counts around mu [total_bins]."""
+    mu = _f64(mu)
+    data = np.zeros((int(n_experiments), mu.shape[0]))
+    rc = _load().orc_draw_pseudo_data(mu.shape[0], _dp(mu), int(n_experiments), int(seed), _dp(data))
+    assert rc == 0, rc
+    return data
+

@@ -329,3 +329,103 @@ int orc_transform(int32_t n_params, int32_t n_u, const int32_t *copy_src, const 
     }
     return 0;
 }
+
+/* ---- pseudo-experiments (section 4.1: "test statistics derived from large ensembles of
+ * pseudo-experiments"): Poisson-fluctuated counts n[e][i] ~ Poisson(mu[i]).  The paper names no generator and no
+ * sampler; R26 fixes both so that the counts are a function of (seed, experiment, bin, mu) alone:
+ *
+ *   uniform   Philox4x32-10 (Salmon et al., SC'11), counter (bin, experiment, 0, 0), key = the 64-bit seed;
+ *             u = (x0 * 2^21 + (x1 >> 11)) * 2^-53 in [0, 1), x0, x1 the first two output words;
+ *   sampler   exact inversion of the Poisson distribution from its mode outwards, using only +, *, / (every
+ *             operation correctly rounded, hence the same bits on any IEEE machine):
+ *               weights relative to the mode m = floor(mu):  w_m = 1,  w_{k+1} = w_k * (mu / (k+1)),
+ *                                                            w_{k-1} = w_k * (k / mu)     (pmf ratios)
+ *               Z = (sum of the left weights, outwards until a term no longer changes the sum)
+ *                   + 1 + (the same to the right)                                  [orc_poisson_norm]
+ *               the interval [0, Z) is cut into pieces of length w_k in the order m, m+1, m-1, m+2, m-2, ...;
+ *               the count is the k whose piece holds u * Z                          [orc_poisson_inv]
+ *             P(k) = w_k / Z = the Poisson pmf up to the rounding of ~10 sqrt(mu) additions (1e-13).
+ * Cost O(sqrt(mu)) per draw. */
+static void mulhilo32(uint32_t a, uint32_t b, uint32_t *hi, uint32_t *lo)
+{
+    uint64_t p = (uint64_t)a * (uint64_t)b;
+    *hi = (uint32_t)(p >> 32);
+    *lo = (uint32_t)p;
+}
+
+void orc_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4])
+{
+    uint32_t c0 = ctr[0], c1 = ctr[1], c2 = ctr[2], c3 = ctr[3], k0 = key[0], k1 = key[1];
+    for (int r = 0; r < 10; ++r) {
+        uint32_t hi0, lo0, hi1, lo1;
+        mulhilo32(0xD2511F53u, c0, &hi0, &lo0);
+        mulhilo32(0xCD9E8D57u, c2, &hi1, &lo1);
+        uint32_t n0 = hi1 ^ c1 ^ k0, n1 = lo1, n2 = hi0 ^ c3 ^ k1, n3 = lo0;
+        c0 = n0; c1 = n1; c2 = n2; c3 = n3;
+        k0 += 0x9E3779B9u;                       /* golden-ratio Weyl sequence on the key */
+        k1 += 0xBB67AE85u;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+double orc_uniform53(uint64_t seed, uint32_t bin, uint32_t experiment)
+{
+    uint32_t ctr[4] = {bin, experiment, 0u, 0u}, key[2] = {(uint32_t)seed, (uint32_t)(seed >> 32)}, x[4];
+    orc_philox4x32_10(ctr, key, x);
+    return (double)(((uint64_t)x[0] << 21) | (uint64_t)(x[1] >> 11)) * 0x1p-53;
+}
+
+double orc_poisson_norm(double mu)
+{
+    if (!(mu > 0.0) || isinf(mu)) return 1.0;
+    const double m = floor(mu);
+    double L = 0.0, R = 0.0, t = 1.0;
+    for (double k = m; k >= 1.0; k -= 1.0) {     /* w_{k-1} = w_k * (k / mu) */
+        t = t * (k / mu);
+        if (L + t == L) break;
+        L += t;
+    }
+    t = 1.0;
+    for (double k = m + 1.0;; k += 1.0) {        /* w_k = w_{k-1} * (mu / k) */
+        t = t * (mu / k);
+        if (R + t == R) break;
+        R += t;
+    }
+    return (L + 1.0) + R;
+}
+
+double orc_poisson_inv(double mu, double Z, double u)
+{
+    if (!(mu > 0.0) || isinf(mu)) return 0.0;
+    const double m = floor(mu), target = u * Z;
+    double acc = 1.0, tr = 1.0, tl = 1.0, kr = m, kl = m;
+    if (target < acc) return m;
+    for (;;) {
+        kr += 1.0;
+        tr = tr * (mu / kr);
+        acc += tr;
+        if (target < acc) return kr;
+        int left_done = 1;
+        if (kl >= 1.0) {
+            tl = tl * (kl / mu);
+            kl -= 1.0;
+            const double before = acc;
+            acc += tl;
+            if (target < acc) return kl;
+            left_done = acc == before;
+        }
+        /* both tails exhausted and u * Z still not reached (it can sit within rounding of Z): the last piece */
+        if (acc + tr == acc && left_done) return kr;
+    }
+}
+
+int orc_draw_pseudo_data(int64_t total_bins_, const double *mu, int32_t E, uint64_t seed, double *data)
+{
+    for (int64_t i = 0; i < total_bins_; ++i) {
+        const double Z = orc_poisson_norm(mu[i]);
+        for (int32_t e = 0; e < E; ++e)
+            data[(int64_t)e * total_bins_ + i] = orc_poisson_inv(mu[i], Z, orc_uniform53(seed, (uint32_t)i, (uint32_t)e));
+    }
+    return 0;
+}
+

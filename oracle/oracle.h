@@ -11,7 +11,8 @@
  * and DESIGN.md reading numbers (R1...).
  *
  * Pins (tests/test_oracle_*.py): every function below is pinned by closed forms, invariants,
- * mpmath / exact-rational brute force and textbook identities; none is "parity unpinned".
+ * mpmath / exact-rational brute force, textbook identities, published known-answer vectors (Philox) and
+ * goodness of fit against scipy.stats (Poisson sampler); none is "parity unpinned".
  * End-to-end numeric values are NOT pinned against the paper: it prints no spectrum or
  * likelihood value and its inputs are not public ("What pins the oracle").
  */
@@ -134,6 +135,19 @@ typedef struct {
 
 int orc_transform(int32_t n_params, int32_t n_u, const int32_t *copy_src, const double *copy_const,
                   int32_t n_blocks, const orc_transform_block *blocks, int32_t P, const double *u, double *theta);
+
+/* Pseudo-experiments (R26): Philox4x32-10 counter-based uniforms and the exact
+ * mode-outward inversion of the Poisson distribution built from +, *, / only (see oracle.c).
+ *   orc_philox4x32_10   one block of the generator (Random123 reference algorithm)
+ *   orc_uniform53       u in [0,1) of (seed, bin, experiment): counter (bin, experiment, 0, 0), key = seed
+ *   orc_poisson_norm    Z(mu) = sum of the pmf weights relative to the mode
+ *   orc_poisson_inv     the count for uniform u
+ *   orc_draw_pseudo_data  data[e][i] = orc_poisson_inv(mu[i], Z(mu[i]), orc_uniform53(seed, i, e)) */
+void   orc_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]);
+double orc_uniform53(uint64_t seed, uint32_t bin, uint32_t experiment);
+double orc_poisson_norm(double mu);
+double orc_poisson_inv(double mu, double Z, double u);
+int    orc_draw_pseudo_data(int64_t total_bins, const double *mu, int32_t E, uint64_t seed, double *data);
 
 /* Number of threads orc_spectra would use for n_threads <= 0. */
 int orc_max_threads(void);
