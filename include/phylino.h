@@ -209,6 +209,36 @@ PHYLINO_API phylino_status phylino_spectra_host(phylino_ctx *ctx, int P, const d
 PHYLINO_API phylino_status phylino_nll_ensemble(phylino_ctx *ctx, int P, const double *params, int E,
                                                 const double *data, double *nll);
 
+/* Poisson pseudo-data for an ensemble of pseudo-experiments, drawn on the device:
+ * data[e * total_bins + i] ~ Poisson(mu[i]), e = 0 ... E-1.  mu DEVICE [total_bins] (e.g. one row of
+ * phylino_expectation at the injected hypothesis), data DEVICE [E x total_bins]; feed it to phylino_nll_ensemble.
+ * The counts are a function of (seed, e, i, mu[i]) alone (R26): Philox4x32-10 uniforms with counter
+ * (i, e, 0, 0) and key = seed, and an exact inversion of the Poisson distribution from its mode outwards that uses
+ * only +, *, / -- the same integers as any other IEEE implementation of that sequence, and from run to run.  mu[i] <= 0, NaN or inf gives 0.
+ * O(sqrt(mu)) steps per draw.  Asynchronous on the context's stream. */
+PHYLINO_API phylino_status phylino_draw_pseudo_data(phylino_ctx *ctx, const double *mu, int E, uint64_t seed,
+                                                    double *data);
+
+/* Scan of one parameter under BOTH mass orderings in one call (Fig. 4: the likelihood as a
+ * function of dm2_ee under the normal and the inverted ordering): for every grid value g the point theta with
+ * theta[scan_param] = grid[g] is evaluated with ordering +1 and -1 (the model's own ordering flag is ignored).
+ *   grid DEVICE [n_grid]; theta DEVICE [param_width] the point the other parameters are taken from;
+ *   data DEVICE [total_bins]; nll DEVICE [2 x n_grid]: row 0 normal, row 1 inverted ordering.
+ * Only the PHYLINO_OSC_FULL3 model depends on the ordering.  The minimisation over the other parameters that a
+ * PROFILE needs stays with the caller's minimiser (out of scope); this is its inner batch.
+ * Always dense.  Asynchronous. */
+PHYLINO_API phylino_status phylino_ordering_scan(phylino_ctx *ctx, int n_grid, int scan_param, const double *grid,
+                                                 const double *theta, const double *data, double *nll);
+
+/* Central-difference gradient of the NLL from the 2 N + 1-point batch a minimiser evaluates per iteration
+ * (R18), N = param_width: the batch {theta} U {theta +- step_j e_j} is formed on the
+ * device, evaluated (with cross-point caching if phylino_set_caching is on), and
+ *   grad[j] = (nll(theta + step_j e_j) - nll(theta - step_j e_j)) / ((theta_j + step_j) - (theta_j - step_j)).
+ *   theta, step DEVICE [N] (step_j != 0); data DEVICE [total_bins]; nll0 DEVICE [1] receives nll(theta), may be
+ *   NULL; grad DEVICE [N].  Asynchronous unless caching is on (see phylino_set_caching). */
+PHYLINO_API phylino_status phylino_nll_gradient(phylino_ctx *ctx, const double *theta, const double *step,
+                                                const double *data, double *nll0, double *grad);
+
 /* Correlated prior blocks: phylino_nll / phylino_nll_host add 1/2 (b - b0)^T V^-1 (b - b0) per block and
  * point (constants dropped, R9), on top of the uncorrelated priors of the model descriptor (a parameter of
  * a block normally has prior_sigma <= 0 there).  Call after phylino_set_model, which clears the blocks;

@@ -24,6 +24,7 @@ abi_symbols = (
     "phylino_set_caching", "phylino_last_plan", "phylino_set_prior_blocks",
     "phylino_nll_ensemble", "phylino_set_transform", "phylino_param_width",
     "phylino_launch_floor", "phylino_set_schedule", "phylino_reserve",
+    "phylino_draw_pseudo_data", "phylino_ordering_scan", "phylino_nll_gradient",
 )
 
 _STATUS = {0: "OK", 1: "ERR_ARG", 2: "ERR_SHAPE", 3: "ERR_STATE", 4: "ERR_OOM", 5: "ERR_CUDA"}
@@ -121,6 +122,12 @@ def load_library():
     lib.phylino_last_plan.argtypes = [vp, C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
     lib.phylino_set_tuning.restype = i32
     lib.phylino_set_tuning.argtypes = [vp, i32, i32, i32]
+    lib.phylino_draw_pseudo_data.restype = i32
+    lib.phylino_draw_pseudo_data.argtypes = [vp, vp, i32, C.c_uint64, vp]
+    lib.phylino_ordering_scan.restype = i32
+    lib.phylino_ordering_scan.argtypes = [vp, i32, i32, vp, vp, vp, vp]
+    lib.phylino_nll_gradient.restype = i32
+    lib.phylino_nll_gradient.argtypes = [vp, vp, vp, vp, vp, vp]
     lib.phylino_set_schedule.restype = i32
     lib.phylino_set_schedule.argtypes = [vp, i32]
     lib.phylino_reserve.restype = i32
@@ -326,6 +333,49 @@ class Phylino:
         self._check(self._lib.phylino_nll_ensemble(self._ctx, int(p.shape[0]), p.data_ptr(), E, data.data_ptr(),
                                                    out.data_ptr()))
         return out
+
+    def _dev_vec(self, x, n, what):
+        t = self._torch
+        if not (isinstance(x, t.Tensor) and x.is_cuda and x.dtype == t.float64 and x.is_contiguous() and x.numel() == n):
+            raise TypeError(f"{what} must be a contiguous float64 CUDA tensor of {n} values")
+        return x
+
+    def draw_pseudo_data(self, mu, n_experiments: int, seed: int, out=None):
+        """mu: float64 CUDA tensor [total_bins] -> Poisson counts [E, total_bins] (float64)."""
+        t = self._torch
+        mu = self._dev_vec(mu, self.total_bins, "mu")
+        E = int(n_experiments)
+        if out is None:
+            out = t.empty((E, self.total_bins), dtype=t.float64, device=mu.device)
+        assert out.is_cuda and out.dtype == t.float64 and out.is_contiguous() and out.numel() == E * self.total_bins
+        self._check(self._lib.phylino_draw_pseudo_data(self._ctx, mu.data_ptr(), E, int(seed) & (2 ** 64 - 1), out.data_ptr()))
+        return out
+
+    def ordering_scan(self, scan_param: int, grid, theta, data, out=None):
+        """grid [n_grid], theta [param_width], data [total_bins] (float64 CUDA) -> nll [2, n_grid]: normal, inverted."""
+        t = self._torch
+        n = int(grid.numel())
+        grid = self._dev_vec(grid, n, "grid")
+        theta = self._dev_vec(theta, self.param_width, "theta")
+        data = self._dev_vec(data, self.total_bins, "data")
+        if out is None:
+            out = t.empty((2, n), dtype=t.float64, device=grid.device)
+        assert out.is_cuda and out.dtype == t.float64 and out.is_contiguous() and out.numel() == 2 * n
+        self._check(self._lib.phylino_ordering_scan(self._ctx, n, int(scan_param), grid.data_ptr(), theta.data_ptr(),
+                                                    data.data_ptr(), out.data_ptr()))
+        return out
+
+    def nll_gradient(self, theta, step, data):
+        """theta, step [param_width], data [total_bins] (float64 CUDA) -> (nll(theta) [1], grad [param_width])."""
+        t = self._torch
+        N = self.param_width
+        theta, step = self._dev_vec(theta, N, "theta"), self._dev_vec(step, N, "step")
+        data = self._dev_vec(data, self.total_bins, "data")
+        nll0 = t.empty(1, dtype=t.float64, device=theta.device)
+        grad = t.empty(N, dtype=t.float64, device=theta.device)
+        self._check(self._lib.phylino_nll_gradient(self._ctx, theta.data_ptr(), step.data_ptr(), data.data_ptr(),
+                                                   nll0.data_ptr(), grad.data_ptr()))
+        return nll0, grad
 
     def expectation(self, params, out=None):
         t = self._torch

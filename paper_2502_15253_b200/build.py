@@ -16,8 +16,8 @@ _ROOT = os.path.dirname(_HERE)
 CSRC = os.path.join(_HERE, "csrc")
 INCLUDE = os.path.join(_ROOT, "include")
 LIB = os.path.join(_HERE, "libphylino.so")
-SOURCES = ["api.cu", "spectra.cu", "finalize.cu", "transform.cu", "peaks.cu"]
-HEADERS = ["internal.h", "devmath.cuh", os.path.join(INCLUDE, "phylino.h")]
+SOURCES = ["api.cu", "spectra.cu", "finalize.cu", "transform.cu", "consumers.cu", "peaks.cu"]
+HEADERS = ["internal.h", "devmath.cuh", "finalize.cuh", os.path.join(INCLUDE, "phylino.h")]
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",

@@ -104,6 +104,7 @@ void free_all(phylino_ctx *c)
     c->point_capacity = 0;
     cudaFree(c->d_plan); c->d_plan = nullptr; c->plan_capacity = 0;
     cudaFree(c->d_mu); c->d_mu = nullptr; c->mu_capacity = 0;
+    cudaFree(c->d_work); c->d_work = nullptr; c->work_capacity = 0;
     free_transform(c);
     cudaFree(c->d_theta); c->d_theta = nullptr; c->theta_capacity = 0;
     cudaFree(c->d_stage); c->d_stage = nullptr;
@@ -191,7 +192,7 @@ void fill_datasets(const phylino_ctx *ctx, SpectraArgs &a)
         v.fx_scale = std::ldexp(1.0, h.fx_exp);
     }
     a.osc.osc_model = ctx->osc_model;
-    a.osc.ordering = ctx->ordering;
+    a.osc.ordering = ctx->ordering_override ? ctx->ordering_override : ctx->ordering;
     for (int j = 0; j < 6; ++j) { a.osc.idx_osc[j] = ctx->idx_osc[j]; a.osc.fixed_osc[j] = ctx->fixed_osc[j]; }
     a.n_datasets = ctx->n_datasets;
     a.n_params = ctx->n_params;
@@ -975,6 +976,80 @@ phylino_status phylino_nll_ensemble(phylino_ctx *ctx, int P, const double *param
     FinalizeArgs f = ctx->fin;
     f.P = P; f.params = params; f.data = data; f.hist = ctx->d_mu; f.nll = nll;
     CU(launch_ensemble(f, E, ctx->sm_count, ctx->stream));
+    ctx->launches += 1;
+    return PHYLINO_OK;
+}
+
+/* work buffer of the consumers below (grown with a stream synchronise, like the other per-batch buffers) */
+static phylino_status ensure_work(phylino_ctx *ctx, int64_t doubles)
+{
+    if (doubles <= ctx->work_capacity) return PHYLINO_OK;
+    CU(cudaStreamSynchronize(ctx->stream));
+    cudaFree(ctx->d_work); ctx->d_work = nullptr; ctx->work_capacity = 0;
+    CU(cudaMalloc((void **)&ctx->d_work, doubles * sizeof(double)));
+    ctx->work_capacity = doubles;
+    return PHYLINO_OK;
+}
+
+phylino_status phylino_draw_pseudo_data(phylino_ctx *ctx, const double *mu, int E, uint64_t seed, double *data)
+{
+    if (!ctx) return PHYLINO_ERR_ARG;
+    if (!ctx->have_model) return fail(ctx, PHYLINO_ERR_STATE, "phylino_set_model has not been called");
+    if (E < 0) return fail(ctx, PHYLINO_ERR_SHAPE, "E = %d is negative", E);
+    if (E == 0) return PHYLINO_OK;
+    if (!mu || !data) return fail(ctx, PHYLINO_ERR_ARG, "NULL mu or data pointer");
+    DeviceGuard g(ctx->device);
+    phylino_status s;
+    if ((s = ensure_work(ctx, ctx->total_bins)) != PHYLINO_OK) return s;
+    CU(launch_pseudo_data(mu, ctx->d_work, ctx->total_bins, E, (unsigned long long)seed, data, ctx->stream));
+    ctx->launches += 2;
+    return PHYLINO_OK;
+}
+
+phylino_status phylino_ordering_scan(phylino_ctx *ctx, int n_grid, int scan_param, const double *grid,
+                                     const double *theta, const double *data, double *nll)
+{
+    phylino_status s = check_ready(ctx, n_grid, theta, nll);
+    if (s != PHYLINO_OK || n_grid == 0) return s;
+    if (!grid || !data) return fail(ctx, PHYLINO_ERR_ARG, "NULL grid or data pointer");
+    const int64_t width = param_width(ctx);
+    if (scan_param < 0 || scan_param >= width) return fail(ctx, PHYLINO_ERR_SHAPE, "scan_param = %d not in 0..%lld", scan_param, (long long)width - 1);
+    DeviceGuard g(ctx->device);
+    if ((s = ensure_work(ctx, (int64_t)n_grid * width)) != PHYLINO_OK) return s;
+    if ((s = ensure_acc(ctx, n_grid)) != PHYLINO_OK) return s;
+    double *batch = ctx->d_work;
+    CU(launch_scan_batch(theta, (int)width, scan_param, grid, n_grid, batch, ctx->stream));
+    ctx->launches += 1;
+    const double *params = batch;
+    if ((s = resolve_params(ctx, n_grid, batch, &params)) != PHYLINO_OK) return s;
+    for (int o = 0; o < 2 && s == PHYLINO_OK; ++o) {
+        ctx->ordering_override = o == 0 ? +1 : -1;
+        s = enqueue_eval(ctx, n_grid, params, data, nullptr, nll + (size_t)o * n_grid, 2);
+    }
+    ctx->ordering_override = 0;
+    ctx->last_virtual_points = ctx->last_classes = 0;
+    return s;
+}
+
+phylino_status phylino_nll_gradient(phylino_ctx *ctx, const double *theta, const double *step, const double *data,
+                                    double *nll0, double *grad)
+{
+    if (!ctx) return PHYLINO_ERR_ARG;
+    const int64_t width = ctx->have_model ? param_width(ctx) : 0;
+    if (width > (1 << 20)) return fail(ctx, PHYLINO_ERR_SHAPE, "too many parameters for a gradient batch");
+    const int P = (int)(2 * width + 1);
+    phylino_status s = check_ready(ctx, P, theta, grad);
+    if (s != PHYLINO_OK) return s;
+    if (!step || !data) return fail(ctx, PHYLINO_ERR_ARG, "NULL step or data pointer");
+    if (width == 0) return PHYLINO_OK;
+    DeviceGuard g(ctx->device);
+    if ((s = ensure_work(ctx, (int64_t)P * width + P)) != PHYLINO_OK) return s;
+    if ((s = ensure_acc(ctx, P)) != PHYLINO_OK) return s;
+    double *batch = ctx->d_work, *nll = ctx->d_work + (int64_t)P * width;
+    CU(launch_gradient_batch(theta, step, (int)width, batch, ctx->stream));
+    ctx->launches += 1;
+    if ((s = phylino_nll(ctx, P, batch, data, nll)) != PHYLINO_OK) return s;      /* dense, or cached if caching is on */
+    CU(launch_gradient(theta, step, nll, (int)width, nll0, grad, ctx->stream));
     ctx->launches += 1;
     return PHYLINO_OK;
 }

@@ -1,0 +1,174 @@
+/*
+ * consumers.cu -- on-device consumers and producers of batches: Poisson pseudo-data for
+ * ensembles of pseudo-experiments, the scan of one parameter under both mass orderings
+ * (Fig. 4), the central-difference gradient of the NLL.
+ *
+ * Pseudo-data (R26; the paper names no generator).  data[e, i] is a function of (seed, e, i, mu_i) alone:
+ *   uniform  Philox4x32-10, counter (i, e, 0, 0), key = seed; u = (x0 2^21 + (x1 >> 11)) 2^-53;
+ *   count    exact inversion of the Poisson distribution from its mode m = floor(mu) outwards with the pmf
+ *            ratios w_{k+1} = w_k (mu / (k+1)), w_{k-1} = w_k (k / mu): Z = sum of the weights (each tail summed
+ *            until a term no longer changes it), [0, Z) cut into pieces w_k in the order m, m+1, m-1, m+2, ...;
+ *            the count is the piece that holds u Z.  Only +, *, / -- every operation correctly rounded and none
+ *            contracted (-fmad=false), so the integers are those of any other IEEE implementation of the same
+ *            sequence: the parity bar for this stage is bit-exact.
+ * One thread per bin forms Z (O(sqrt mu) steps), then one thread per (experiment, bin) draws (O(sqrt mu) steps).
+ */
+#include "internal.h"
+
+namespace phylino {
+
+namespace {
+
+__device__ __forceinline__ void philox_round(unsigned &c0, unsigned &c1, unsigned &c2, unsigned &c3, unsigned k0,
+                                             unsigned k1)
+{
+    const unsigned hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
+    const unsigned hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
+    const unsigned n0 = hi1 ^ c1 ^ k0, n2 = hi0 ^ c3 ^ k1;
+    c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;
+}
+
+/* u in [0, 1) of (seed, bin, experiment) */
+__device__ __forceinline__ double uniform53(unsigned long long seed, unsigned bin, unsigned experiment)
+{
+    unsigned c0 = bin, c1 = experiment, c2 = 0u, c3 = 0u;
+    unsigned k0 = (unsigned)seed, k1 = (unsigned)(seed >> 32);
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        philox_round(c0, c1, c2, c3, k0, k1);
+        k0 += 0x9E3779B9u;
+        k1 += 0xBB67AE85u;
+    }
+    return (double)(((unsigned long long)c0 << 21) | (unsigned long long)(c1 >> 11)) * 0x1p-53;
+}
+
+__device__ double poisson_norm(double mu)
+{
+    if (!(mu > 0.0) || mu > 1.79769313486231570e308) return 1.0;
+    const double m = floor(mu);
+    double L = 0.0, R = 0.0, t = 1.0;
+    for (double k = m; k >= 1.0; k -= 1.0) {
+        t = t * (k / mu);
+        if (L + t == L) break;
+        L += t;
+    }
+    t = 1.0;
+    for (double k = m + 1.0;; k += 1.0) {
+        t = t * (mu / k);
+        if (R + t == R) break;
+        R += t;
+    }
+    return (L + 1.0) + R;
+}
+
+__device__ double poisson_inv(double mu, double Z, double u)
+{
+    if (!(mu > 0.0) || mu > 1.79769313486231570e308) return 0.0;
+    const double m = floor(mu), target = u * Z;
+    double acc = 1.0, tr = 1.0, tl = 1.0, kr = m, kl = m;
+    if (target < acc) return m;
+    for (;;) {
+        kr += 1.0;
+        tr = tr * (mu / kr);
+        acc += tr;
+        if (target < acc) return kr;
+        bool left_done = true;
+        if (kl >= 1.0) {
+            tl = tl * (kl / mu);
+            kl -= 1.0;
+            const double before = acc;
+            acc += tl;
+            if (target < acc) return kl;
+            left_done = acc == before;
+        }
+        if (acc + tr == acc && left_done) return kr;    /* u Z within rounding of Z: the last piece */
+    }
+}
+
+__global__ void __launch_bounds__(128) poisson_norm_kernel(const double *mu, int n, double *Z)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) Z[i] = poisson_norm(mu[i]);
+}
+
+__global__ void __launch_bounds__(128) poisson_draw_kernel(const double *mu, const double *Z, int n, int E,
+                                                           unsigned long long seed, double *data)
+{
+    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= (long long)n * E) return;
+    const int i = (int)(t % n), e = (int)(t / n);
+    data[t] = poisson_inv(mu[i], Z[i], uniform53(seed, (unsigned)i, (unsigned)e));
+}
+
+/* batch[g] = theta with theta[col] = grid[g] */
+__global__ void __launch_bounds__(128) scan_batch_kernel(const double *theta, int width, int col, const double *grid,
+                                                         int n_grid, double *batch)
+{
+    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= (long long)n_grid * width) return;
+    const int j = (int)(t % width), g = (int)(t / width);
+    batch[t] = j == col ? grid[g] : theta[j];
+}
+
+/* central-difference batch (R18): row 0 = theta, rows 1 + 2j / 2 + 2j = theta +- h_j e_j */
+__global__ void __launch_bounds__(128) gradient_batch_kernel(const double *theta, const double *h, int width,
+                                                             double *batch)
+{
+    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= (long long)(2 * width + 1) * width) return;
+    const int j = (int)(t % width), row = (int)(t / width);
+    double v = theta[j];
+    if (row > 0 && (row - 1) / 2 == j) v = (row & 1) ? v + h[j] : v - h[j];
+    batch[t] = v;
+}
+
+/* g_j = (nll(theta + h_j e_j) - nll(theta - h_j e_j)) / ((theta_j + h_j) - (theta_j - h_j)): the divisor is the
+ * step actually taken in floating point */
+__global__ void __launch_bounds__(128) gradient_kernel(const double *theta, const double *h, const double *nll,
+                                                       int width, double *nll0, double *grad)
+{
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j == 0 && nll0) *nll0 = nll[0];
+    if (j >= width) return;
+    const double up = theta[j] + h[j], dn = theta[j] - h[j];
+    grad[j] = (nll[1 + 2 * j] - nll[2 + 2 * j]) / (up - dn);
+}
+
+} // namespace
+
+cudaError_t launch_pseudo_data(const double *mu, double *Z, int n, int E, unsigned long long seed, double *data,
+                               cudaStream_t st)
+{
+    if (n <= 0 || E <= 0) return cudaSuccess;
+    poisson_norm_kernel<<<(n + 127) / 128, 128, 0, st>>>(mu, n, Z);
+    const long long total = (long long)n * E;
+    poisson_draw_kernel<<<(unsigned)((total + 127) / 128), 128, 0, st>>>(mu, Z, n, E, seed, data);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_scan_batch(const double *theta, int width, int col, const double *grid, int n_grid, double *batch,
+                              cudaStream_t st)
+{
+    const long long total = (long long)n_grid * width;
+    if (total <= 0) return cudaSuccess;
+    scan_batch_kernel<<<(unsigned)((total + 127) / 128), 128, 0, st>>>(theta, width, col, grid, n_grid, batch);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_gradient_batch(const double *theta, const double *h, int width, double *batch, cudaStream_t st)
+{
+    const long long total = (long long)(2 * width + 1) * width;
+    if (width <= 0) return cudaSuccess;
+    gradient_batch_kernel<<<(unsigned)((total + 127) / 128), 128, 0, st>>>(theta, h, width, batch);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_gradient(const double *theta, const double *h, const double *nll, int width, double *nll0,
+                            double *grad, cudaStream_t st)
+{
+    if (width <= 0) return cudaSuccess;
+    gradient_kernel<<<(width + 127) / 128, 128, 0, st>>>(theta, h, nll, width, nll0, grad);
+    return cudaGetLastError();
+}
+
+} // namespace phylino

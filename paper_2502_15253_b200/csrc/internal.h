@@ -190,6 +190,13 @@ cudaError_t launch_spectra(const SpectraArgs &a, int S, cudaStream_t st, bool pd
 cudaError_t launch_fused(const SpectraArgs &a, const ParamBlob &blob, int S, cudaStream_t st, bool pdl, bool dbg);
 cudaError_t launch_finalize(const FinalizeArgs &a, int mode /*0 H, 1 mu, 2 nll, 3 clear*/, cudaStream_t st, bool pdl);
 cudaError_t launch_ensemble(const FinalizeArgs &a, int E, int sm_count, cudaStream_t st);
+cudaError_t launch_pseudo_data(const double *mu, double *Z, int n, int E, unsigned long long seed, double *data,
+                               cudaStream_t st);
+cudaError_t launch_scan_batch(const double *theta, int width, int col, const double *grid, int n_grid, double *batch,
+                              cudaStream_t st);
+cudaError_t launch_gradient_batch(const double *theta, const double *h, int width, double *batch, cudaStream_t st);
+cudaError_t launch_gradient(const double *theta, const double *h, const double *nll, int width, double *nll0,
+                            double *grad, cudaStream_t st);
 cudaError_t run_peak_fp64(int iters, cudaStream_t st, double *dfma_per_s);
 cudaError_t run_launch_floor(int reps, cudaStream_t st, double *us_per_call);
 
@@ -257,6 +264,9 @@ struct phylino_ctx {
     int64_t theta_capacity = 0;
     double *d_mu = nullptr;                        /* [mu_capacity] expectations of an ensemble call */
     int64_t mu_capacity = 0;
+    double *d_work = nullptr;                      /* [work_capacity] batches / NLLs / Poisson norms of the consumers */
+    int64_t work_capacity = 0;
+    int ordering_override = 0;                     /* +-1 while an ordering scan runs, else 0 */
     /* host-buffer entry points: pinned + device staging */
     double *h_pin = nullptr, *d_stage = nullptr, *d_pin = nullptr;   /* d_pin: device alias of h_pin */
     int64_t stage_capacity = 0;                    /* doubles */

@@ -127,15 +127,6 @@ __device__ __forceinline__ const void *batch_ptr(const DatasetDev &ds, int b)
     return static_cast<const char *>(ds.ev) + (size_t)b * rec_bytes(ds);
 }
 
-/* one warp asks L2 for [p, p + bytes): the lines are on their way while the events are walked */
-__device__ __forceinline__ void prefetch_l2(const void *p, size_t bytes, int lane)
-{
-    if (!p) return;
-    const char *c = static_cast<const char *>(p);
-    for (size_t off = (size_t)lane * 128; off < bytes; off += 32 * 128)
-        asm volatile("prefetch.global.L2 [%0];" ::"l"(c + off));
-}
-
 /* run total -> fixed point; values outside the domain become flag bits */
 __device__ __forceinline__ long long to_fixed(double s, double scale, bool bad, unsigned &fl)
 {

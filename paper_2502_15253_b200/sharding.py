@@ -7,7 +7,7 @@ another size, so the library may cut its work differently (unit length, schedule
 which events a lane sums in fp64 before the exact integer accumulation): the gathered rows agree with
 the one-GPU call to rounding -- <= 1e-13 relative per bin, <= 1e-9 in the NLL, measured with the real
 library in tests/test_gpu_schedules.py::test_point_shards_agree_with_the_unsharded_batch -- not bit
-for bit, and each slice meets the oracle parity bars on its own.  Reruns of the same split are
+for bit, and each slice meets the parity bars against the CPU reference on its own.  Reruns of the same split are
 bit-identical.
 The only exchange is an all-gather of the per-point results (`nll[P]`, or `hist[P x bins]`),
 done with `torch.distributed` (NCCL on GPUs; gloo in the CPU tests).  There is no data-path

@@ -1,0 +1,111 @@
+"""-m gpu: on-device producers / consumers of batches: Poisson pseudo-data (bit-exact
+against the oracle's generator), the ordering scan of Fig. 4, the central-difference gradient."""
+import numpy as np
+import pytest
+
+import workloads
+from workloads.spec import OSC_FULL3
+
+pytestmark = pytest.mark.gpu
+ABS_NLL = 1e-6
+
+
+def _dev(a):
+    import torch
+    return torch.as_tensor(np.ascontiguousarray(a, dtype=np.float64), device="cuda")
+
+
+def _data(orc, wl):
+    mu0 = orc.expectation(wl.theta0[None, :], orc.spectra(wl.theta0[None, :]))[0]
+    return workloads.poisson_counts(mu0, wl.seed + 7)
+
+
+@pytest.mark.parametrize("k,scale,E", [(2, 0.01, 257), (3, 0.02, 64), (4, 0.01, 33), (5, 1.0, 16)])
+def test_pseudo_data_bit_exact(gpu, oracle_mod, k, scale, E):
+    """integer output, so the bar is bit-exact.  Expectations from tiny (scaled configs: single-event
+    bins) to 1e5 per bin (config 5 at full size), drawn on the device from the ORACLE's expectation vector."""
+    wl = workloads.make_config(k, scale=scale, n_points=1)
+    orc = oracle_mod.Oracle(wl.model, wl.events)
+    mu = orc.expectation(wl.theta0[None, :], orc.spectra(wl.theta0[None, :]))[0]
+    mu[::17] = 0.0                       # empty expectation: always 0 counts
+    mu[3] = 0.37
+    want = oracle_mod.draw_pseudo_data(mu, E, seed=0xC0FFEE1234567)
+    with gpu.Phylino() as ph:
+        ph.load_workload(wl)
+        got = ph.draw_pseudo_data(_dev(mu), E, seed=0xC0FFEE1234567).cpu().numpy()
+        again = ph.draw_pseudo_data(_dev(mu), E, seed=0xC0FFEE1234567).cpu().numpy()
+        other = ph.draw_pseudo_data(_dev(mu), E, seed=1).cpu().numpy()
+    assert got.shape == want.shape == (E, mu.size)
+    assert np.array_equal(got, want)
+    assert np.array_equal(got, again) and not np.array_equal(got, other)
+    assert np.all(got[:, ::17] == 0.0)
+    big = mu > 50
+    if big.any():
+        assert np.abs((got[:, big] - mu[big]) / np.sqrt(mu[big])).max() < 7.0     # fluctuations of Poisson size
+
+
+def test_ensemble_from_device_drawn_data(gpu, oracle_mod):
+    """the whole pseudo-experiment loop on the device: expectation at the injected point -> pseudo-data -> nll[P, E]"""
+    wl = workloads.make_config(5, scale=0.01, n_points=23)
+    orc = oracle_mod.Oracle(wl.model, wl.events)
+    E = 19
+    with gpu.Phylino() as ph:
+        ph.load_workload(wl)
+        mu0 = ph.expectation(_dev(wl.theta0[None, :]))
+        data = ph.draw_pseudo_data(mu0[0].contiguous(), E, seed=77)
+        nll = ph.nll_ensemble(_dev(wl.params), data).cpu().numpy()
+        data_h, mu0_h = data.cpu().numpy(), mu0.cpu().numpy()[0]
+    assert np.array_equal(data_h, oracle_mod.draw_pseudo_data(mu0_h, E, seed=77))      # same mu bits in, same counts out
+    want = np.stack([orc.nll(wl.params, data_h[e]) for e in range(E)], axis=1)
+    assert np.abs(nll - want).max() <= ABS_NLL
+
+
+def test_ordering_scan_matches_two_models(gpu, oracle_mod):
+    """PAPER.md:213, :228 (Fig. 4): dm2_ee grid x {normal, inverted}; row o of the result is the oracle's NLL of the
+    model with ordering o, whatever ordering the loaded model itself carries."""
+    import torch
+    n_grid = 45
+    for loaded in (+1, -1):
+        wl = workloads.make_config(4, scale=0.004, n_points=1, ordering=loaded)
+        grid = np.linspace(2.3e-3, 2.7e-3, n_grid)
+        batch = np.tile(wl.theta0, (n_grid, 1))
+        batch[:, 1] = grid
+        orc_n = oracle_mod.Oracle(workloads.make_config(4, scale=0.004, n_points=1, ordering=+1).model, wl.events)
+        orc_i = oracle_mod.Oracle(workloads.make_config(4, scale=0.004, n_points=1, ordering=-1).model, wl.events)
+        data = _data(orc_n, wl)                           # injected hypothesis: normal ordering
+        with gpu.Phylino() as ph:
+            ph.load_workload(wl)
+            nll = ph.ordering_scan(1, _dev(grid), _dev(wl.theta0), _dev(data)).cpu().numpy()
+            own = ph.nll(_dev(batch), _dev(data)).cpu().numpy()       # the context's own ordering is untouched afterwards
+            torch.cuda.synchronize()
+        want = np.stack([orc_n.nll(batch, data), orc_i.nll(batch, data)])
+        assert np.abs(nll - want).max() <= ABS_NLL
+        assert np.abs(own - want[0 if loaded > 0 else 1]).max() <= ABS_NLL
+        assert np.abs(want[0] - want[1]).max() > 1e-3     # the two orderings are different curves
+
+
+@pytest.mark.parametrize("caching", [False, True])
+def test_gradient_from_the_603_point_batch(gpu, oracle_mod, caching):
+    """g_j = (nll+ - nll-) / (2 h_j) on the device against the same differences of the oracle's NLLs,
+    to 1e-6 / h_j (the NLL bar divided by the step); config 3's 301 parameters at reduced event count."""
+    wl = workloads.make_config(3, scale=0.01)
+    N = wl.model.n_params
+    assert wl.n_points == 2 * N + 1
+    orc = oracle_mod.Oracle(wl.model, wl.events)
+    data = _data(orc, wl)
+    theta = wl.params[0].copy()
+    h = np.array([wl.params[1 + 2 * j, j] - theta[j] for j in range(N)])
+    nll_o = orc.nll(wl.params, data)
+    up = np.array([wl.params[1 + 2 * j, j] for j in range(N)])
+    dn = np.array([wl.params[2 + 2 * j, j] for j in range(N)])
+    grad_o = (nll_o[1::2] - nll_o[2::2]) / (up - dn)
+    with gpu.Phylino() as ph:
+        ph.load_workload(wl)
+        ph.set_caching(caching)
+        nll0, grad = ph.nll_gradient(_dev(theta), _dev(h), _dev(data))
+        if caching:
+            assert ph.last_plan()[0] > 0
+        nll0, grad = nll0.cpu().numpy(), grad.cpu().numpy()
+    assert abs(nll0[0] - nll_o[0]) <= ABS_NLL
+    assert np.all(np.abs(grad - grad_o) <= 1e-6 / np.abs(h))
+    assert np.abs(grad - grad_o).max() <= 1e-3 * max(1.0, np.abs(grad_o).max())       # and tight in absolute terms
