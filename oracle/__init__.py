@@ -43,7 +43,8 @@ class _Bkg(C.Structure):
 class _Dataset(C.Structure):
     _fields_ = [("n_bins", C.c_int32), ("idx_a", C.c_int32 * 3), ("idx_signorm", C.c_int32),
                 ("norm", C.c_double), ("idx_flux", C.c_void_p), ("n_bkg", C.c_int32),
-                ("bkg", C.POINTER(_Bkg))]
+                ("bkg", C.POINTER(_Bkg)), ("n_flux_par", C.c_int32), ("idx_flux_par", C.c_void_p),
+                ("flux_lo", C.c_double), ("flux_width", C.c_double)]
 
 
 class _PriorBlock(C.Structure):
@@ -59,7 +60,8 @@ class _Model(C.Structure):
     _fields_ = [("osc_model", C.c_int32), ("ordering", C.c_int32), ("n_params", C.c_int32),
                 ("n_datasets", C.c_int32), ("idx_osc", C.c_int32 * 6), ("fixed_osc", C.c_double * 6),
                 ("datasets", C.POINTER(_Dataset)), ("prior_mean", C.c_void_p), ("prior_sigma", C.c_void_p),
-                ("n_prior_blocks", C.c_int32), ("prior_blocks", C.POINTER(_PriorBlock))]
+                ("n_prior_blocks", C.c_int32), ("prior_blocks", C.POINTER(_PriorBlock)),
+                ("energy_correction", C.c_int32)]
 
 
 _lib = None
@@ -86,7 +88,15 @@ def _load():
         lib.orc_event_bins.argtypes = [C.POINTER(_Model), C.POINTER(_Events), C.c_int32, dp,
                                        C.POINTER(C.c_int32)]
         lib.orc_expectation.restype = C.c_int
-        lib.orc_expectation.argtypes = [C.POINTER(_Model), C.c_int32, dp, dp, dp]
+        lib.orc_expectation.argtypes = [C.POINTER(_Model), C.POINTER(dp), C.c_int32, dp, dp, dp]
+        lib.orc_correct_spectra.restype = C.c_int
+        lib.orc_correct_spectra.argtypes = [C.POINTER(_Model), C.POINTER(dp), C.c_int32, dp, dp, dp]
+        lib.orc_escale_inverse.restype = C.c_double
+        lib.orc_escale_inverse.argtypes = [C.c_double] * 4
+        lib.orc_rebin_quadratic.restype = C.c_int
+        lib.orc_rebin_quadratic.argtypes = [C.c_int32, dp, dp, C.c_int32, dp, dp]
+        lib.orc_flux_scales.restype = C.c_int
+        lib.orc_flux_scales.argtypes = [C.POINTER(_Dataset), dp, dp, dp]
         lib.orc_nll_from_mu.restype = C.c_int
         lib.orc_nll_from_mu.argtypes = [C.POINTER(_Model), C.c_int32, dp, dp, dp, dp]
         lib.orc_nll.restype = C.c_int
@@ -128,6 +138,13 @@ class Oracle:
         self.n_params = model.n_params
         self.total_bins = sum(d.n_bins for d in model.datasets)
         self.n_events = sum(e.n for e in events)
+        self.bin_level = int(getattr(model, "energy_correction", 0)) == 1
+        # bin edges per dataset (the bin-level steps need them): from the events if given
+        self._edges = None
+        if len(events):
+            arrs = [np.ascontiguousarray(e.edges, dtype=np.float64) for e in events]
+            self._keep.extend(arrs)
+            self._edges = (C.POINTER(C.c_double) * len(arrs))(*[_dp(a) for a in arrs])
 
     # -- marshalling ---------------------------------------------------------------------------
     def _arr(self, a, dtype):
@@ -151,7 +168,13 @@ class Oracle:
             ds_arr[d].idx_flux = None if ds.idx_flux is None else self._arr(ds.idx_flux, np.int32)
             ds_arr[d].n_bkg = len(ds.bkg)
             ds_arr[d].bkg = C.cast(bk_arr, C.POINTER(_Bkg))
+            fm = getattr(ds, "flux_model", None)
+            if fm is not None:
+                ds_arr[d].n_flux_par = len(fm.idx_par)
+                ds_arr[d].idx_flux_par = self._arr(fm.idx_par, np.int32)
+                ds_arr[d].flux_lo, ds_arr[d].flux_width = float(fm.lo), float(fm.width)
         self._keep.append(ds_arr)
+        self._ds_arr = ds_arr
         m = _Model()
         m.osc_model = int(model.osc_model)
         m.ordering = int(model.ordering)
@@ -174,6 +197,7 @@ class Oracle:
         self._keep.append(pb)
         m.n_prior_blocks = len(blocks)
         m.prior_blocks = C.cast(pb, C.POINTER(_PriorBlock)) if blocks else None
+        m.energy_correction = int(getattr(model, "energy_correction", 0))
         return m
 
     def _marshal_events(self, events):
@@ -207,12 +231,25 @@ class Oracle:
         return A[:S].copy(), m[:S].copy()
 
     # -- O3 ------------------------------------------------------------------------------------
-    def spectra(self, params, n_threads: int = 0) -> np.ndarray:
+    def spectra_raw(self, params, n_threads: int = 0) -> np.ndarray:
+        """step 1 of PAPER.md:177; with energy_correction = 1 binned under the identity energy scale"""
         p = self._params(params)
         hist = np.zeros((p.shape[0], self.total_bins))
         rc = _load().orc_spectra(C.byref(self._m), self._ev, p.shape[0], _dp(p), _dp(hist), n_threads)
         assert rc == 0, rc
         return hist
+
+    def spectra(self, params, n_threads: int = 0) -> np.ndarray:
+        """the signal spectrum the product's spectra call returns: step 1, plus the bin-level energy correction
+        (step 3, no flux re-scaling) when energy_correction = 1"""
+        hist = self.spectra_raw(params, n_threads)
+        if not self.bin_level:
+            return hist
+        p = self._params(params)
+        out = np.zeros_like(hist)
+        rc = _load().orc_correct_spectra(C.byref(self._m), self._edges, p.shape[0], _dp(p), _dp(hist), _dp(out))
+        assert rc == 0, rc
+        return out
 
     def event_bins(self, params) -> np.ndarray:
         p = self._params(params)
@@ -224,12 +261,25 @@ class Oracle:
 
     # -- O4 / O5 -------------------------------------------------------------------------------
     def expectation(self, params, hist) -> np.ndarray:
+        """hist: the step-1 spectra (with energy_correction = 1: spectra_raw, not spectra)"""
         p = self._params(params)
         h = _f64(hist).reshape(p.shape[0], self.total_bins)
         mu = np.zeros_like(h)
-        rc = _load().orc_expectation(C.byref(self._m), p.shape[0], _dp(p), _dp(h), _dp(mu))
+        rc = _load().orc_expectation(C.byref(self._m), self._edges, p.shape[0], _dp(p), _dp(h), _dp(mu))
         assert rc == 0, rc
         return mu
+
+    def flux_scales(self, dataset: int, theta) -> np.ndarray:
+        th = _f64(theta)
+        f = np.zeros(self.model.datasets[dataset].n_bins)
+        ed = np.ascontiguousarray(self._keep_edges(dataset))
+        rc = _load().orc_flux_scales(C.byref(self._ds_arr[dataset]), _dp(ed), _dp(th), _dp(f))
+        assert rc == 0, rc
+        return f
+
+    def _keep_edges(self, dataset: int) -> np.ndarray:
+        n = self.model.datasets[dataset].n_bins
+        return np.ctypeslib.as_array(self._edges[dataset], shape=(n + 1,)).copy()
 
     def nll_from_mu(self, params, mu, data) -> np.ndarray:
         p = self._params(params)
@@ -334,4 +384,18 @@ def draw_pseudo_data(mu, n_experiments: int, seed: int) -> np.ndarray:
     rc = _load().orc_draw_pseudo_data(mu.shape[0], _dp(mu), int(n_experiments), int(seed), _dp(data))
     assert rc == 0, rc
     return data
+
+
+# -- bin-level steps (R27) ----------------------------------------------------------------
+def escale_inverse(a0: float, a1: float, a2: float, t: float) -> float:
+    return float(_load().orc_escale_inverse(a0, a1, a2, t))
+
+
+def rebin_quadratic(src_edges, src_int, x) -> np.ndarray:
+    e, h, x = _f64(src_edges), _f64(src_int), _f64(x)
+    assert e.shape[0] == h.shape[0] + 1
+    out = np.zeros(x.shape[0] - 1)
+    rc = _load().orc_rebin_quadratic(h.shape[0], _dp(e), _dp(h), out.shape[0], _dp(x), _dp(out))
+    assert rc == 0, rc
+    return out
 

@@ -155,6 +155,7 @@ static void spectra_point(const orc_model *m, const orc_events *ev, const double
         const orc_dataset *ds = &m->datasets[d];
         double a[3];
         get_a(ds, theta, a);
+        if (m->energy_correction == 1) { a[0] = 0.0; a[1] = 1.0; a[2] = 0.0; }    /* step 3 acts on the bins instead */
         for (int b = 0; b < e->n_bins; ++b) { hist[off + b] = 0.0; comp[off + b] = 0.0; }
         for (int64_t i = 0; i < e->n; ++i) {
             double E = (double)e->e_nu[i];
@@ -216,7 +217,89 @@ int orc_event_bins(const orc_model *m, const orc_events *ev, int32_t P, const do
     return 0;
 }
 
-int orc_expectation(const orc_model *m, int32_t P, const double *params, const double *hist, double *mu)
+/* ---- PAPER.md:177 steps 2-3 on the binned spectrum (R27, R28) -------------------------------------- */
+double orc_escale_inverse(double a0, double a1, double a2, double t)
+{
+    const double c = t - a0;
+    if (a2 == 0.0) return c / a1;
+    return (2.0 * c) / (a1 + sqrt(a1 * a1 + 4.0 * a2 * c));
+}
+
+/* cumulative integral, from src_edges[t0], of the smoothed density that belongs to source bin b */
+static double cumulative(int32_t n, const double *e, const double *h, int32_t b, double E)
+{
+    if (n == 1) return h[0] / (e[1] - e[0]) * (E - e[0]);
+    int32_t t0 = b - 1;
+    if (t0 < 0) t0 = 0;
+    if (t0 > n - 3) t0 = n - 3;
+    if (n == 2) {
+        /* quadratic cumulative through (e0, 0), (e1, h0), (e2, h0 + h1): a straight-line density */
+        const double d1 = h[0] / (e[1] - e[0]);
+        const double d1b = h[1] / (e[2] - e[1]);
+        const double d2 = (d1b - d1) / (e[2] - e[0]);
+        return d1 * (E - e[0]) + d2 * (E - e[0]) * (E - e[1]);
+    }
+    /* Newton form of the cubic through the four cumulative points of bins t0, t0+1, t0+2 */
+    const double *x = e + t0, *y = h + t0;
+    const double f01 = y[0] / (x[1] - x[0]), f12 = y[1] / (x[2] - x[1]), f23 = y[2] / (x[3] - x[2]);
+    const double f012 = (f12 - f01) / (x[2] - x[0]), f123 = (f23 - f12) / (x[3] - x[1]);
+    const double f0123 = (f123 - f012) / (x[3] - x[0]);
+    return f01 * (E - x[0]) + f012 * (E - x[0]) * (E - x[1]) + f0123 * (E - x[0]) * (E - x[1]) * (E - x[2]);
+}
+
+int orc_rebin_quadratic(int32_t n_src, const double *e, const double *h, int32_t n_tgt, const double *x, double *out)
+{
+    if (n_src < 1 || n_tgt < 0) return -1;
+    for (int32_t c = 0; c < n_tgt; ++c) {
+        const double lo = x[c], hi = x[c + 1];
+        if (isnan(lo) || isnan(hi)) { out[c] = NAN; continue; }
+        double s = 0.0;
+        for (int32_t b = 0; b < n_src; ++b) {
+            const double a = lo > e[b] ? lo : e[b], z = hi < e[b + 1] ? hi : e[b + 1];
+            if (a < z) s += cumulative(n_src, e, h, b, z) - cumulative(n_src, e, h, b, a);
+        }
+        out[c] = s;
+    }
+    return 0;
+}
+
+/* pre-images of the bin edges under the energy scale of dataset ds at theta */
+static void preimages(const orc_dataset *ds, const double *edges, const double *theta, double *x)
+{
+    double a[3];
+    get_a(ds, theta, a);
+    for (int32_t b = 0; b <= ds->n_bins; ++b) x[b] = orc_escale_inverse(a[0], a[1], a[2], edges[b]);
+}
+
+int orc_flux_scales(const orc_dataset *ds, const double *edges, const double *theta, double *f)
+{
+    const int32_t B = ds->n_bins, n = ds->n_flux_par;
+    if (n <= 0) {
+        for (int32_t b = 0; b < B; ++b) f[b] = (ds->idx_flux && ds->idx_flux[b] >= 0) ? theta[ds->idx_flux[b]] : 1.0;
+        return 0;
+    }
+    /* the n parameters are bin averages on the uniform fine grid; "area conserving spline ... energy
+     * corrected and later transformed into the original binning" (R28) */
+    double *fe = (double *)malloc(sizeof(double) * (size_t)(2 * n + 1 + 2 * (B + 1)));
+    if (!fe) return -3;
+    double *fi = fe + n + 1, *x = fi + n, *in = x + B + 1;
+    for (int32_t j = 0; j <= n; ++j) fe[j] = ds->flux_lo + ds->flux_width * (double)j;
+    for (int32_t j = 0; j < n; ++j) fi[j] = theta[ds->idx_flux_par[j]] * ds->flux_width;
+    preimages(ds, edges, theta, x);
+    orc_rebin_quadratic(n, fe, fi, B, x, in);
+    for (int32_t b = 0; b < B; ++b) {
+        /* average over the pre-image: the part inside the fine grid from the spline, the rest at the nominal 1 */
+        const double lo = x[b], hi = x[b + 1];
+        const double a = lo > fe[0] ? lo : fe[0], z = hi < fe[n] ? hi : fe[n];
+        const double inside = a < z ? z - a : 0.0;
+        f[b] = (in[b] + ((hi - lo) - inside)) / (hi - lo);
+    }
+    free(fe);
+    return 0;
+}
+
+int orc_correct_spectra(const orc_model *m, const double *const *edges, int32_t P, const double *params,
+                        const double *hist, double *out)
 {
     int64_t TB = total_bins(m);
     for (int32_t p = 0; p < P; ++p) {
@@ -224,10 +307,46 @@ int orc_expectation(const orc_model *m, int32_t P, const double *params, const d
         int64_t off = 0;
         for (int d = 0; d < m->n_datasets; ++d) {
             const orc_dataset *ds = &m->datasets[d];
+            double *x = (double *)malloc(sizeof(double) * (size_t)(ds->n_bins + 1));
+            if (!x) return -3;
+            preimages(ds, edges[d], theta, x);
+            orc_rebin_quadratic(ds->n_bins, edges[d], hist + p * TB + off, ds->n_bins, x, out + p * TB + off);
+            free(x);
+            off += ds->n_bins;
+        }
+    }
+    return 0;
+}
+
+int orc_expectation(const orc_model *m, const double *const *edges, int32_t P, const double *params,
+                    const double *hist, double *mu)
+{
+    int64_t TB = total_bins(m);
+    for (int32_t p = 0; p < P; ++p) {
+        const double *theta = params + (int64_t)p * m->n_params;
+        int64_t off = 0;
+        for (int d = 0; d < m->n_datasets; ++d) {
+            const orc_dataset *ds = &m->datasets[d];
+            const int32_t B = ds->n_bins;
             double eps = ds->idx_signorm >= 0 ? theta[ds->idx_signorm] : 1.0;
-            for (int b = 0; b < ds->n_bins; ++b) {
-                double f = (ds->idx_flux && ds->idx_flux[b] >= 0) ? theta[ds->idx_flux[b]] : 1.0;
-                double v = eps * ds->norm * f * hist[p * TB + off + b];      /* signal */
+            double *f = (double *)malloc(sizeof(double) * (size_t)(3 * B + 1));
+            if (!f) return -3;
+            double *g = f + B, *x = g + B;
+            if ((ds->n_flux_par > 0 || m->energy_correction == 1) && !edges) { free(f); return -4; }
+            orc_flux_scales(ds, edges ? edges[d] : NULL, theta, f);
+            if (m->energy_correction == 1) {
+                /* step 2 (bin re-scaling) on the raw spectrum, then step 3 (energy correction of the bins) */
+                for (int32_t b = 0; b < B; ++b) g[b] = f[b] * hist[p * TB + off + b];
+                preimages(ds, edges[d], theta, x);
+                double *gc = (double *)malloc(sizeof(double) * (size_t)B);
+                if (!gc) { free(f); return -3; }
+                orc_rebin_quadratic(B, edges[d], g, B, x, gc);
+                for (int32_t b = 0; b < B; ++b) g[b] = gc[b];
+                free(gc);
+            }
+            for (int b = 0; b < B; ++b) {
+                double v = m->energy_correction == 1 ? eps * ds->norm * g[b]
+                                                     : eps * ds->norm * f[b] * hist[p * TB + off + b];   /* signal */
                 for (int k = 0; k < ds->n_bkg; ++k) {                        /* + backgrounds */
                     const orc_bkg *bk = &ds->bkg[k];
                     double r = bk->idx_rate >= 0 ? theta[bk->idx_rate] : 1.0;
@@ -236,7 +355,8 @@ int orc_expectation(const orc_model *m, int32_t P, const double *params, const d
                 }
                 mu[p * TB + off + b] = v;
             }
-            off += ds->n_bins;
+            free(f);
+            off += B;
         }
     }
     return 0;
@@ -299,7 +419,11 @@ int orc_nll(const orc_model *m, const orc_events *ev, int32_t P, const double *p
     if (!hist) return -3;
     double *mu = hist + (size_t)TB * (size_t)P;
     int rc = orc_spectra(m, ev, P, params, hist, n_threads);
-    if (!rc) rc = orc_expectation(m, P, params, hist, mu);
+    const double **edges = (const double **)malloc(sizeof(double *) * (size_t)m->n_datasets);
+    if (!edges) { free(hist); return -3; }
+    for (int d = 0; d < m->n_datasets; ++d) edges[d] = ev[d].edges;
+    if (!rc) rc = orc_expectation(m, edges, P, params, hist, mu);
+    free(edges);
     if (!rc) rc = orc_nll_from_mu(m, P, params, mu, data, nll);
     free(hist);
     return rc;

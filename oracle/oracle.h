@@ -55,6 +55,11 @@ typedef struct {
     const int32_t *idx_flux;     /* [n_bins] or NULL => 1 */
     int32_t        n_bkg;
     const orc_bkg *bkg;
+    /* reactor-flux model on a uniform fine grid (R28): n_flux_par > 0 replaces idx_flux.
+     * theta[idx_flux_par[j]] is the average flux correction on [flux_lo + j flux_width, flux_lo + (j+1) flux_width) */
+    int32_t        n_flux_par;
+    const int32_t *idx_flux_par; /* [n_flux_par] */
+    double         flux_lo, flux_width;
 } orc_dataset;
 
 /* One correlated Gaussian constraint: (b - b0)^T V^-1 (b - b0) over the parameters idx
@@ -78,6 +83,8 @@ typedef struct {
     const double      *prior_sigma;  /* [n_params] or NULL; <=0, inf or NaN => unconstrained */
     int32_t                n_prior_blocks;
     const orc_prior_block *prior_blocks; /* [n_prior_blocks] or NULL */
+    int32_t            energy_correction; /* 0: per event before binning (north_star; R8);
+                                             1: on the binned spectrum (PAPER.md:177 step 3; R27) */
 } orc_model;
 
 /* O1-O2: amplitudes A_k and mass splittings m_k [eV^2] of the oscillation terms at one point.
@@ -104,8 +111,12 @@ int orc_spectra(const orc_model *m, const orc_events *ev, int32_t P, const doubl
 int orc_event_bins(const orc_model *m, const orc_events *ev, int32_t P, const double *params,
                    int32_t *bins);
 
-/* O4: mu[p][off_d+b] = eps_d norm_d f_db H + sum_k r_dk s_dkb T_dkb. */
-int orc_expectation(const orc_model *m, int32_t P, const double *params, const double *hist, double *mu);
+/* O4: mu[p][off_d+b] = eps_d norm_d f_db H + sum_k r_dk s_dkb T_dkb.
+ * energy_correction = 1: hist is the RAW (identity-binned) step-1 spectrum, and the signal part is
+ * eps_d norm_d C_a(f_d . H)_b with C_a the bin-level correction above (step 2, then step 3).
+ * edges: per dataset [n_bins + 1]; needed only with energy_correction = 1 or a flux model, else may be NULL. */
+int orc_expectation(const orc_model *m, const double *const *edges, int32_t P, const double *params,
+                    const double *hist, double *mu);
 
 /* Half-deviance of one bin, mu - n + n ln(n/mu)  (PAPER.md:67 Eq. 3, :96 Eq. 8; R9-R10). */
 double orc_dev(double n, double mu);
@@ -135,6 +146,28 @@ typedef struct {
 
 int orc_transform(int32_t n_params, int32_t n_u, const int32_t *copy_src, const double *copy_const,
                   int32_t n_blocks, const orc_transform_block *blocks, int32_t P, const double *u, double *theta);
+
+/* ---- the paper's own signal steps 2-3 on the BINNED spectrum (R27, R28) --------------
+ * "The expectation is smoothed using a second-degree polynomial function.  These corrected bins entries are then
+ * integrated over the original binning" -- the paper gives no formula; the reading taken (R27):
+ *   smoothing   inside source bin b the density is the parabola whose integrals over three consecutive bins
+ *               (b-1, b, b+1; the first / last three at the ends) equal their contents, i.e. the derivative of the
+ *               cubic through the four cumulative points of that triple (2 bins: straight line; 1 bin: constant);
+ *   correction  content arriving in [t_c, t_c+1) of the corrected energy E' = a0 + a1 E + a2 E^2 is the integral
+ *               of that density over the pre-image [x_c, x_c+1), x = E'^-1(t) on the branch through (t - a0)/a1.
+ * orc_escale_inverse: x with a0 + a1 x + a2 x^2 = t, as 2 (t - a0) / (a1 + sqrt(a1^2 + 4 a2 (t - a0))).
+ * orc_rebin_quadratic: out[c] = integral over [x[c], x[c+1]) of the smoothed density of (src_edges, src_int);
+ *   x ascending, n_tgt + 1 values; nothing outside the source range; NaN in x gives NaN out.
+ * orc_correct_spectra: applies the correction of the point's energy-scale parameters to every dataset of raw
+ *   (identity-binned) spectra hist [P x total_bins] -> out: what the product's spectra call returns in mode 1.
+ * orc_flux_scales: f[b] of dataset d at theta (R28): the fine-grid flux parameters, smoothed the same way, averaged
+ *   over the pre-image of analysis bin b under the dataset's energy scale; 1 outside the fine grid. */
+double orc_escale_inverse(double a0, double a1, double a2, double t);
+int    orc_rebin_quadratic(int32_t n_src, const double *src_edges, const double *src_int, int32_t n_tgt,
+                           const double *x, double *out);
+int    orc_correct_spectra(const orc_model *m, const double *const *edges, int32_t P, const double *params,
+                           const double *hist, double *out);
+int    orc_flux_scales(const orc_dataset *ds, const double *edges, const double *theta, double *f);
 
 /* Pseudo-experiments (R26): Philox4x32-10 counter-based uniforms and the exact
  * mode-outward inversion of the Poisson distribution built from +, *, / only (see oracle.c).

@@ -28,6 +28,15 @@ class BkgSpec:
 
 
 @dataclass
+class FluxModel:
+    """Reactor-flux nuisance model of one dataset on a uniform fine grid (41 parameters on 0.25-MeV bins
+    from 1 to 11.25 MeV): theta[idx_par[j]] is the average flux correction on [lo + j width, lo + (j+1) width)."""
+    idx_par: np.ndarray       # int32 [n] indices into theta
+    lo: float = 1.0
+    width: float = 0.25
+
+
+@dataclass
 class DatasetSpec:
     """How theta acts on one dataset's signal spectrum and backgrounds."""
     n_bins: int
@@ -36,6 +45,7 @@ class DatasetSpec:
     norm: float = 1.0                      # constant MC -> data normalisation
     idx_flux: Optional[np.ndarray] = None  # int32 [n_bins] per-bin flux scale; None => all 1
     bkg: List[BkgSpec] = field(default_factory=list)
+    flux_model: Optional[FluxModel] = None  # replaces idx_flux: fine-grid parameters -> per-bin scales (R28)
 
 
 @dataclass
@@ -97,6 +107,7 @@ class ModelSpec:
     prior_mean: Optional[np.ndarray] = None   # float64 [n_params]
     prior_sigma: Optional[np.ndarray] = None  # float64 [n_params]; <= 0 or inf => unconstrained
     prior_blocks: List[PriorBlock] = field(default_factory=list)
+    energy_correction: int = 0              # 0: per event before binning (north_star); 1: on the bins (PAPER.md:177 step 3)
 
     @property
     def total_bins(self) -> int:
