@@ -239,6 +239,28 @@ PHYLINO_API phylino_status phylino_ordering_scan(phylino_ctx *ctx, int n_grid, i
 PHYLINO_API phylino_status phylino_nll_gradient(phylino_ctx *ctx, const double *theta, const double *step,
                                                 const double *data, double *nll0, double *grad);
 
+/* Where the energy-scale systematic acts.  mode 0 (default; what BASELINE.json's north_star
+ * asks for, R8): on every event before binning, E' = a0 + a1 E_vis + a2 E_vis^2.  mode 1: on the BINNED
+ * spectrum, the paper's own signal step 3 ("The expectation is smoothed using a second-degree polynomial function.
+ * These corrected bins entries are then integrated over the original binning"; reading R27 of DESIGN.md:
+ * inside a bin the density is the parabola whose integrals over three consecutive bins equal their contents; a bin of
+ * the corrected spectrum is the integral of that density over the bin's pre-image under E'): the events are binned
+ * under the identity scale, then per point and dataset  mu = eps norm C_a(f . H) + backgrounds, i.e. step 2 (the per-bin
+ * re-scaling f) followed by step 3 (C_a).  phylino_spectra returns C_a(H).  With mode 1 no event work depends on the
+ * energy-scale parameters, so cross-point caching merges all of them.  Needs total_bins <= 2000
+ * (PHYLINO_ERR_SHAPE otherwise); PHYLINO_ERR_STATE before set_model, which resets the mode to 0. */
+PHYLINO_API phylino_status phylino_set_energy_correction_mode(phylino_ctx *ctx, int mode);
+
+/* Reactor-flux model of one dataset on a uniform fine grid (41 parameters on 0.25-MeV bins from 1 to
+ * 11.25 MeV, "the basis of an area conserving spline, which is energy corrected and later transformed into the
+ * original binning"; reading R28): theta[idx_par[j]] is the average flux correction on
+ * [lo + j width, lo + (j+1) width); the flux scale f_db of analysis bin b becomes the average, over the bin's
+ * pre-image under the dataset's energy scale, of the same area-conserving parabolic reconstruction as above (1 outside
+ * the grid), replacing theta[idx_flux[b]].  idx_par HOST [n_par], copied; n_par = 0 removes the model; set_model
+ * removes all.  Needs total_bins <= 2000.  Synchronises the stream. */
+PHYLINO_API phylino_status phylino_set_flux_model(phylino_ctx *ctx, int dataset, int n_par, const int32_t *idx_par,
+                                                  double lo, double width);
+
 /* Correlated prior blocks: phylino_nll / phylino_nll_host add 1/2 (b - b0)^T V^-1 (b - b0) per block and
  * point (constants dropped, R9), on top of the uncorrelated priors of the model descriptor (a parameter of
  * a block normally has prior_sigma <= 0 there).  Call after phylino_set_model, which clears the blocks;

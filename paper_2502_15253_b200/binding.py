@@ -25,6 +25,7 @@ abi_symbols = (
     "phylino_nll_ensemble", "phylino_set_transform", "phylino_param_width",
     "phylino_launch_floor", "phylino_set_schedule", "phylino_reserve",
     "phylino_draw_pseudo_data", "phylino_ordering_scan", "phylino_nll_gradient",
+    "phylino_set_energy_correction_mode", "phylino_set_flux_model",
 )
 
 _STATUS = {0: "OK", 1: "ERR_ARG", 2: "ERR_SHAPE", 3: "ERR_STATE", 4: "ERR_OOM", 5: "ERR_CUDA"}
@@ -128,6 +129,10 @@ def load_library():
     lib.phylino_ordering_scan.argtypes = [vp, i32, i32, vp, vp, vp, vp]
     lib.phylino_nll_gradient.restype = i32
     lib.phylino_nll_gradient.argtypes = [vp, vp, vp, vp, vp, vp]
+    lib.phylino_set_energy_correction_mode.restype = i32
+    lib.phylino_set_energy_correction_mode.argtypes = [vp, i32]
+    lib.phylino_set_flux_model.restype = i32
+    lib.phylino_set_flux_model.argtypes = [vp, i32, i32, vp, dbl, dbl]
     lib.phylino_set_schedule.restype = i32
     lib.phylino_set_schedule.argtypes = [vp, i32]
     lib.phylino_reserve.restype = i32
@@ -262,6 +267,12 @@ class Phylino:
         blocks = list(getattr(wl.model, "prior_blocks", None) or [])
         if blocks:
             self.set_prior_blocks(blocks)
+        for d, ds in enumerate(wl.model.datasets):
+            fm = getattr(ds, "flux_model", None)
+            if fm is not None:
+                self.set_flux_model(d, fm.idx_par, fm.lo, fm.width)
+        if int(getattr(wl.model, "energy_correction", 0)):
+            self.set_energy_correction_mode(1)
         for d, e in enumerate(wl.events):
             self.load_events(d, e.e_nu, e.e_vis, e.w, e.core, e.L_m, e.edges)
 
@@ -287,6 +298,16 @@ class Phylino:
 
     def set_tuning(self, unit_events: int = 0, chunk_groups: int = 0, max_warps: int = 0):
         self._check(self._lib.phylino_set_tuning(self._ctx, int(unit_events), int(chunk_groups), int(max_warps)))
+
+    def set_energy_correction_mode(self, mode: int):
+        """0: per event before binning (default); 1: on the binned spectrum (PAPER.md:177 step 3)."""
+        self._check(self._lib.phylino_set_energy_correction_mode(self._ctx, int(mode)))
+
+    def set_flux_model(self, dataset: int, idx_par, lo: float = 1.0, width: float = 0.25):
+        """fine-grid flux parameters of one dataset; idx_par empty removes the model."""
+        idx = np.ascontiguousarray(idx_par, dtype=np.int32)
+        self._check(self._lib.phylino_set_flux_model(self._ctx, int(dataset), int(idx.size),
+                                                     idx.ctypes.data if idx.size else None, float(lo), float(width)))
 
     def set_schedule(self, mode: int = 0):
         """0 library's choice, 1 always setup/spectra/finalize kernels, 2 single launch for <= 16 points."""

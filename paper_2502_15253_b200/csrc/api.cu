@@ -78,6 +78,8 @@ void free_tables(phylino_ctx *c)
     cudaFree((void *)f.prior_mean); cudaFree((void *)f.prior_sigma);
     cudaFree((void *)f.blk_off); cudaFree((void *)f.blk_moff); cudaFree((void *)f.blk_idx);
     cudaFree((void *)f.blk_mean); cudaFree((void *)f.blk_inv);
+    cudaFree((void *)f.edges_all); cudaFree((void *)f.ds_bin_off); cudaFree((void *)f.ds_idx_a);
+    cudaFree((void *)f.fm_off); cudaFree((void *)f.fm_idx); cudaFree((void *)f.fm_grid);
     f = FinalizeArgs{};
 }
 
@@ -162,7 +164,7 @@ phylino_status ensure_acc(phylino_ctx *ctx, int P)
         CU(cudaStreamSynchronize(ctx->stream));
         cudaFree(ctx->d_rec); cudaFree(ctx->d_thr); cudaFree(ctx->d_safe);
         ctx->d_rec = nullptr; ctx->d_thr = nullptr; ctx->d_safe = nullptr; ctx->point_capacity = 0;
-        const int64_t rows = ctx->per_point_binning ? P : 1;
+        const int64_t rows = ctx->per_point_binning ? P : 1;      /* (sized for mode 0 even while mode 1 is on) */
         CU(cudaMalloc((void **)&ctx->d_rec, (size_t)rec_fields(ctx->n_terms) * P * sizeof(double)));
         CU(cudaMalloc((void **)&ctx->d_thr, (size_t)rows * (ctx->total_bins + ctx->n_datasets) * sizeof(float)));
         CU(cudaMalloc((void **)&ctx->d_safe, (size_t)rows * ctx->n_datasets * sizeof(float2)));
@@ -183,9 +185,11 @@ void fill_datasets(const phylino_ctx *ctx, SpectraArgs &a)
         v.n_bins = h.n_bins;
         v.bin_off = d == 0 ? 0 : a.ds[d - 1].bin_off + a.ds[d - 1].n_bins;
         v.thr_off = v.bin_off + d;
-        v.per_point = (h.idx_a[0] >= 0 || h.idx_a[1] >= 0 || h.idx_a[2] >= 0) ? 1 : 0;
+        /* bin-level energy correction (phylino_set_energy_correction_mode): the events are binned under the
+         * identity scale, the finalize stage corrects the bins */
+        v.per_point = (!ctx->ec_mode && (h.idx_a[0] >= 0 || h.idx_a[1] >= 0 || h.idx_a[2] >= 0)) ? 1 : 0;
         v.n_batches = (int32_t)(h.n_pad / EB);
-        for (int j = 0; j < 3; ++j) v.idx_a[j] = h.idx_a[j];
+        for (int j = 0; j < 3; ++j) v.idx_a[j] = ctx->ec_mode ? -1 : h.idx_a[j];
         v.unit_w = h.unit_w ? 1 : 0;
         v.v_pos_min = h.v_pos_min;
         v.v_max = h.v_max;
@@ -229,7 +233,7 @@ phylino_status fill_batch(phylino_ctx *ctx, SpectraArgs &a, int P, const double 
         CU(spectra_max_warps(ctx->n_terms, ctx->sm_count, false, 0, &ctx->resident_warps));
     a.P = P;
     a.params = params;
-    a.thr_rows = thr_rows > 0 ? thr_rows : (ctx->per_point_binning ? P : 1);
+    a.thr_rows = thr_rows > 0 ? thr_rows : (ctx->per_point_binning && !ctx->ec_mode ? P : 1);
     const int64_t n_groups = (P + 31) / 32;
     int streams = 1;                                    /* sub-streams per warp when P < 32 */
     if (P < 32) { int pl = 1; while (pl < P) pl <<= 1; streams = 32 / pl; }
@@ -354,6 +358,7 @@ phylino_status enqueue_eval(phylino_ctx *ctx, int P, const double *params, const
     f.data = data;
     f.hist = hist;
     f.nll = nll;
+    f.ec_mode = ctx->ec_mode;
     if (dbg) mode = 3;
     const bool pdl = !ctx->timing;
     if (ctx->timing) { CU(cudaEventRecord(ctx->ev[0], ctx->stream)); }
@@ -510,7 +515,7 @@ bool plan_components(const phylino_ctx *ctx, int P, const double *params, Compon
     if (P >= (1 << 29)) return false;                   /* (point, term) is packed as p * 4 + k in an int32 */
     /* columns of the parameter vector that enter the energy scale of any dataset */
     std::vector<int32_t> acols;
-    for (int d = 0; d < ctx->n_datasets; ++d)
+    for (int d = 0; d < ctx->n_datasets && !ctx->ec_mode; ++d)     /* bin-level correction: the walk ignores the scale */
         for (int j = 0; j < 3; ++j)
             if (ctx->ds[d].idx_a[j] >= 0) acols.push_back(ctx->ds[d].idx_a[j]);
     std::vector<int32_t> cls((size_t)P);
@@ -626,6 +631,7 @@ phylino_status enqueue_cached(phylino_ctx *ctx, int P, const double *h_params, c
     f.P = P; f.params = d_params; f.acc = ctx->d_acc; f.flags = ctx->d_flags;
     f.data = d_data; f.hist = d_hist; f.nll = d_nll;
     f.comp = 1; f.n_terms = S; f.osc = a.osc;
+    f.ec_mode = ctx->ec_mode;
     f.pt_comp = ctx->d_plan + V + (int64_t)V * S + pl.C;
     if (ctx->timing) CU(cudaEventRecord(ctx->ev[0], ctx->stream));
     if (a.sched == 1) {
@@ -794,6 +800,24 @@ phylino_status phylino_set_model(phylino_ctx *ctx, const phylino_model_desc *m)
     f.n_params = m->n_params;
     f.total_bins = (int32_t)tb;
     f.staged = tb <= FIN_STAGE_MAX_BINS ? 1 : 0;
+    ctx->ec_mode = 0;
+    ctx->fm_idx.assign(m->n_datasets, std::vector<int32_t>());
+    ctx->fm_lo.assign(m->n_datasets, 0.0);
+    ctx->fm_width.assign(m->n_datasets, 0.0);
+    {
+        std::vector<int32_t> ds_off(m->n_datasets + 1, 0), ds_a((size_t)m->n_datasets * 3, -1);
+        for (int d = 0; d < m->n_datasets; ++d) {
+            ds_off[d + 1] = ds_off[d] + m->datasets[d].n_bins;
+            for (int j = 0; j < 3; ++j) ds_a[(size_t)3 * d + j] = m->datasets[d].idx_a[j];
+        }
+        std::vector<double> edges0((size_t)tb + m->n_datasets, 0.0);
+        std::vector<int32_t> fm_off(m->n_datasets + 1, 0);
+        CU(upload((int32_t **)&f.ds_bin_off, ds_off, ctx->stream));
+        CU(upload((int32_t **)&f.ds_idx_a, ds_a, ctx->stream));
+        CU(upload((double **)&f.edges_all, edges0, ctx->stream));
+        CU(upload((int32_t **)&f.fm_off, fm_off, ctx->stream));
+        CU(cudaStreamSynchronize(ctx->stream));
+    }
     f.n_datasets = m->n_datasets;
     f.max_bkg = max_bkg;
     cudaStream_t st = ctx->stream;
@@ -914,6 +938,11 @@ phylino_status phylino_load_events(phylino_ctx *ctx, int dataset, int64_t n, con
     CU(upload(&h.d_hint, hint, st));
     double inv = std::ldexp(1.0, -fx);
     CU(cudaMemcpyAsync((void *)(ctx->fin.inv_scale + dataset), &inv, sizeof(double), cudaMemcpyHostToDevice, st));
+    {
+        int64_t off = dataset;                  /* dataset d's edges start at (bins before it) + d */
+        for (int d = 0; d < dataset; ++d) off += ctx->ds[d].n_bins;
+        CU(cudaMemcpyAsync((void *)(ctx->fin.edges_all + off), ed.data(), ed.size() * sizeof(double), cudaMemcpyHostToDevice, st));
+    }
     CU(cudaStreamSynchronize(st));
     h.n = n; h.n_pad = n_pad; h.wsum_abs = wsum; h.fx_exp = fx; h.loaded = true;
     h.v_pos_min = v_pos_min; h.v_max = v_max; h.unit_w = unit_w;
@@ -975,6 +1004,7 @@ phylino_status phylino_nll_ensemble(phylino_ctx *ctx, int P, const double *param
     if ((s = enqueue_eval(ctx, P, params, nullptr, ctx->d_mu, nullptr, 1)) != PHYLINO_OK) return s;
     FinalizeArgs f = ctx->fin;
     f.P = P; f.params = params; f.data = data; f.hist = ctx->d_mu; f.nll = nll;
+    f.ec_mode = ctx->ec_mode;
     CU(launch_ensemble(f, E, ctx->sm_count, ctx->stream));
     ctx->launches += 1;
     return PHYLINO_OK;
@@ -1267,6 +1297,57 @@ phylino_status phylino_set_tuning(phylino_ctx *ctx, int unit_events, int chunk_g
     ctx->unit_events = unit_events;
     ctx->chunk_groups = chunk_groups;
     ctx->max_warps = max_warps;
+    return PHYLINO_OK;
+}
+
+phylino_status phylino_set_energy_correction_mode(phylino_ctx *ctx, int mode)
+{
+    if (!ctx) return PHYLINO_ERR_ARG;
+    if (!ctx->have_model) return fail(ctx, PHYLINO_ERR_STATE, "phylino_set_model must come before phylino_set_energy_correction_mode");
+    if (mode != 0 && mode != 1) return fail(ctx, PHYLINO_ERR_ARG, "mode %d not 0 or 1", mode);
+    if (mode == 1 && !ctx->fin.staged)
+        return fail(ctx, PHYLINO_ERR_SHAPE, "the bin-level correction needs total_bins <= %d", FIN_STAGE_MAX_BINS);
+    ctx->ec_mode = mode;
+    ctx->fused_warps = 0;               /* the threshold tables of the small-batch kernel change size */
+    return PHYLINO_OK;
+}
+
+phylino_status phylino_set_flux_model(phylino_ctx *ctx, int dataset, int n_par, const int32_t *idx_par, double lo,
+                                      double width)
+{
+    if (!ctx) return PHYLINO_ERR_ARG;
+    if (!ctx->have_model) return fail(ctx, PHYLINO_ERR_STATE, "phylino_set_model must come before phylino_set_flux_model");
+    if (dataset < 0 || dataset >= ctx->n_datasets) return fail(ctx, PHYLINO_ERR_SHAPE, "dataset %d not in 0..%d", dataset, ctx->n_datasets - 1);
+    if (n_par < 0 || n_par > PHYLINO_MAX_BLOCK) return fail(ctx, PHYLINO_ERR_SHAPE, "n_par = %d not in 0..%d", n_par, PHYLINO_MAX_BLOCK);
+    if (n_par > 0) {
+        if (!idx_par) return fail(ctx, PHYLINO_ERR_ARG, "NULL idx_par");
+        if (!std::isfinite(lo) || !(width > 0.0) || !std::isfinite(width)) return fail(ctx, PHYLINO_ERR_ARG, "fine grid: lo must be finite, width finite > 0");
+        if (!ctx->fin.staged) return fail(ctx, PHYLINO_ERR_SHAPE, "a flux model needs total_bins <= %d", FIN_STAGE_MAX_BINS);
+        for (int j = 0; j < n_par; ++j)
+            if (idx_par[j] < 0 || idx_par[j] >= ctx->n_params) return fail(ctx, PHYLINO_ERR_SHAPE, "idx_par[%d] = %d out of range", j, idx_par[j]);
+    }
+    ctx->fm_idx[dataset].assign(idx_par, idx_par + n_par);
+    ctx->fm_lo[dataset] = lo;
+    ctx->fm_width[dataset] = width;
+    std::vector<int32_t> off(ctx->n_datasets + 1, 0), idx;
+    std::vector<double> grid((size_t)ctx->n_datasets * 2, 0.0);
+    for (int d = 0; d < ctx->n_datasets; ++d) {
+        idx.insert(idx.end(), ctx->fm_idx[d].begin(), ctx->fm_idx[d].end());
+        off[d + 1] = (int32_t)idx.size();
+        grid[2 * d] = ctx->fm_lo[d];
+        grid[2 * d + 1] = ctx->fm_width[d];
+    }
+    DeviceGuard g(ctx->device);
+    CU(cudaStreamSynchronize(ctx->stream));
+    FinalizeArgs &f = ctx->fin;
+    cudaFree((void *)f.fm_off); cudaFree((void *)f.fm_idx); cudaFree((void *)f.fm_grid);
+    f.fm_off = nullptr; f.fm_idx = nullptr; f.fm_grid = nullptr;
+    CU(upload((int32_t **)&f.fm_off, off, ctx->stream));
+    CU(upload((int32_t **)&f.fm_idx, idx, ctx->stream));
+    CU(upload((double **)&f.fm_grid, grid, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    f.have_fm = idx.empty() ? 0 : 1;
+    ctx->err.clear();
     return PHYLINO_OK;
 }
 

@@ -39,7 +39,7 @@ __global__ void __launch_bounds__(FIN_THREADS) finalize_kernel(const __grid_cons
     finalize_pre<MODE>(a, blockIdx.x, a.staged ? stage : nullptr, pre);
     if (a.staged) __syncthreads();
     asm volatile("griddepcontrol.wait;" ::: "memory");  /* the accumulators of the whole spectra grid are in */
-    finalize_post<MODE>(a, blockIdx.x, a.staged ? stage : nullptr, pre, wsum);
+    finalize_post<MODE>(a, blockIdx.x, a.staged ? stage : nullptr, pre, wsum);   /* ec_mode implies staged (api.cu) */
     if (a.reset_counter && blockIdx.x == 0 && threadIdx.x == 0) *a.reset_counter = 0u;
 }
 

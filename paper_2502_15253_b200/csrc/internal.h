@@ -160,6 +160,16 @@ struct FinalizeArgs {
     const double  *data;          /* [total_bins] (NLL mode) */
     double        *hist;          /* [P x total_bins] (spectra / expectation mode) */
     double        *nll;           /* [P] (NLL mode) */
+    /* the paper's bin-level steps (PAPER.md:177 steps 2-3, :129; R27, R28) */
+    int32_t        ec_mode;       /* 1: the energy correction acts on the binned spectrum (the events were binned under
+                                     the identity scale); 0: it acted per event */
+    int32_t        have_fm;       /* some dataset takes its flux scales from a fine-grid flux model */
+    const double  *edges_all;     /* [total_bins + n_datasets] bin edges, dataset d at ds_bin_off[d] + d */
+    const int32_t *ds_bin_off;    /* [n_datasets + 1] */
+    const int32_t *ds_idx_a;      /* [n_datasets x 3] energy-scale indices into theta, -1 => (0,1,0) */
+    const int32_t *fm_off;        /* [n_datasets + 1] offsets into fm_idx (equal => no flux model for the dataset) */
+    const int32_t *fm_idx;        /* indices into theta of the fine-grid parameters */
+    const double  *fm_grid;       /* [n_datasets x 2] lower end and bin width of the fine grid */
     /* component mode: H[p,b] = P0(p) W[b] + sum_k A_k(p) C_k[b] from the cells pt_comp names */
     int32_t comp, n_terms;
     OscDev  osc;
@@ -267,6 +277,9 @@ struct phylino_ctx {
     double *d_work = nullptr;                      /* [work_capacity] batches / NLLs / Poisson norms of the consumers */
     int64_t work_capacity = 0;
     int ordering_override = 0;                     /* +-1 while an ordering scan runs, else 0 */
+    int ec_mode = 0;                               /* phylino_set_energy_correction_mode */
+    std::vector<std::vector<int32_t>> fm_idx;      /* per dataset: fine-grid flux parameters (phylino_set_flux_model) */
+    std::vector<double> fm_lo, fm_width;
     /* host-buffer entry points: pinned + device staging */
     double *h_pin = nullptr, *d_stage = nullptr, *d_pin = nullptr;   /* d_pin: device alias of h_pin */
     int64_t stage_capacity = 0;                    /* doubles */
