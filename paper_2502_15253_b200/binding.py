@@ -12,7 +12,8 @@ from typing import Optional, Sequence
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_LIB_PATH = os.path.join(_HERE, "libphylino.so")
+# PHYLINO_LIBRARY: another build of the same library (e.g. libphylino_checked.so, python -m ...build --checked)
+_LIB_PATH = os.environ.get("PHYLINO_LIBRARY") or os.path.join(_HERE, "libphylino.so")
 
 # every symbol include/phylino.h declares
 abi_symbols = (

@@ -1,6 +1,6 @@
 """Builds libphylino.so (the C-ABI CUDA library) in-tree with nvcc for sm_100a.
 
-    python -m paper_2502_15253_b200.build [--force]
+    python -m paper_2502_15253_b200.build [--force] [--verbose] [--checked]
 
 The library links the CUDA runtime statically and has no Python or torch dependency.
 """
@@ -45,11 +45,17 @@ def _stale() -> bool:
     return any(os.path.getmtime(d) > t for d in deps)
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
-    if not (force or _stale()):
+LIB_CHECKED = os.path.join(_HERE, "libphylino_checked.so")
+
+
+def build(force: bool = False, verbose: bool = False, checked: bool = False) -> str:
+    """checked: the same sources with -DPHYLINO_CHECKED (device-side bounds / invariant checks that trap) into
+    libphylino_checked.so; load it with PHYLINO_LIBRARY=<path> (binding.py).  Never the shipped library."""
+    lib = LIB_CHECKED if checked else LIB
+    if not checked and not (force or _stale()):
         return LIB
-    tmp = LIB + f".tmp{os.getpid()}"
-    cmd = [nvcc(), *NVCC_FLAGS, "-I", INCLUDE, "-I", CSRC,
+    tmp = lib + f".tmp{os.getpid()}"
+    cmd = [nvcc(), *NVCC_FLAGS, *(["-DPHYLINO_CHECKED"] if checked else []), "-I", INCLUDE, "-I", CSRC,
            *[os.path.join(CSRC, s) for s in SOURCES], "-o", tmp]
     res = subprocess.run(cmd, capture_output=True, text=True)
     if res.returncode != 0:
@@ -57,11 +63,12 @@ def build(force: bool = False, verbose: bool = False) -> str:
         raise RuntimeError("nvcc failed building libphylino.so")
     if verbose:
         sys.stderr.write(res.stderr)
-    with open(os.path.join(_HERE, "ptxas_info.log"), "w") as f:
-        f.write(" ".join(cmd) + "\n" + res.stdout + res.stderr)
-    os.replace(tmp, LIB)
-    return LIB
+    if not checked:
+        with open(os.path.join(_HERE, "ptxas_info.log"), "w") as f:
+            f.write(" ".join(cmd) + "\n" + res.stdout + res.stderr)
+    os.replace(tmp, lib)
+    return lib
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose=True))
+    print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv, checked="--checked" in sys.argv))

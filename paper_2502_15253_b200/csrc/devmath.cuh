@@ -8,6 +8,23 @@
 
 #include "internal.h"
 
+/* -DPHYLINO_CHECKED (python -m paper_2502_15253_b200.build --checked -> libphylino_checked.so): device-side bounds
+ * and invariant checks that trap with a message; compiled out of the shipped library.  compute-sanitizer is not
+ * available on the measurement pool, so these stand in for memcheck on the indices the kernels compute themselves. */
+#ifdef PHYLINO_CHECKED
+#include <cstdio>
+#define PHYLINO_ASSERT(cond)                                                                          \
+    do {                                                                                              \
+        if (!(cond)) {                                                                                \
+            printf("PHYLINO_CHECKED %s:%d: %s (block %d thread %d)\n", __FILE__, __LINE__, #cond,     \
+                   (int)blockIdx.x, (int)threadIdx.x);                                                \
+            __trap();                                                                                 \
+        }                                                                                             \
+    } while (0)
+#else
+#define PHYLINO_ASSERT(cond) do { } while (0)
+#endif
+
 namespace phylino {
 
 /* first-octant branch theta < pi/4 (R4): cos 2theta = +sqrt(1 - sin^2 2theta) */

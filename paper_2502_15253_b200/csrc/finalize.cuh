@@ -112,6 +112,7 @@ __device__ __forceinline__ double rebin_quadratic(int n, const double *e, const 
         if (e[mid + 1] > lo) top = mid; else b = mid + 1;
     }
     double s = 0.0;
+    PHYLINO_ASSERT(b >= 0 && b <= n);
     for (; b < n && e[b] < hi; ++b) {
         const double a = fmax(lo, e[b]), z = fmin(hi, e[b + 1]);
         if (a < z) s += cumulative_quadratic(n, e, h, b, z) - cumulative_quadratic(n, e, h, b, a);
@@ -143,6 +144,7 @@ __device__ __forceinline__ double flux_scale_of_bin(const FinalizeArgs &a, const
             const int t0 = n >= 3 ? min(max(j - 1, 0), n - 3) : 0;
             double e4[4], h3[3];
             const int m = min(n, 3);
+            PHYLINO_ASSERT(t0 >= 0 && t0 + m <= n && j - t0 >= 0 && j - t0 < m);
             for (int i = 0; i <= m; ++i) e4[i] = g0 + w * (double)(t0 + i);
             for (int i = 0; i < m; ++i) h3[i] = theta[a.fm_idx[o + t0 + i]] * w;
             s += cumulative_quadratic(m, e4, h3, j - t0, hi_j) - cumulative_quadratic(m, e4, h3, j - t0, lo_j);

@@ -279,6 +279,7 @@ __device__ __forceinline__ void threshold_entry(const SpectraArgs &a, const doub
 /* threshold row entry with the conventions thr[-1] = -inf, thr[B + 1] = +inf */
 __device__ __forceinline__ float thr_at(const float *thr, int B, int i)
 {
+    PHYLINO_ASSERT(i >= -2 && i <= B + 3);
     return i < 0 ? -pos_inf() : (i > B ? pos_inf() : thr[i]);
 }
 
@@ -355,6 +356,7 @@ __device__ __forceinline__ void dbg_mark(const SpectraArgs &a, const DatasetDev 
     if (!DBG) return;
     const long long i = (long long)gb * EB + j;
     if (!active || i >= ds.n_events) return;
+    PHYLINO_ASSERT(ds.perm[i] >= 0 && ds.perm[i] < ds.n_events && ds.ev_off + ds.perm[i] < a.total_events);
     a.dbg_bins[(size_t)p * a.total_events + ds.ev_off + ds.perm[i]] = (cur >= 0 && cur < ds.n_bins) ? cur : -1;
 }
 
@@ -365,6 +367,7 @@ __device__ __forceinline__ void flush_run(const SpectraArgs &a, const Tables &T,
     if (a.comp && active && r.cur >= 0 && r.cur < ds.n_bins) {
         /* component mode: W and every C_k go to cells of their own (the amplitudes come later) */
         const size_t cell = (size_t)p * (S + 1) * a.total_bins + ds.bin_off + r.cur;
+        PHYLINO_ASSERT(cell + (size_t)S * a.total_bins < (size_t)a.P * (S + 1) * a.total_bins);
 #pragma unroll
         for (int j = 0; j <= S; ++j) {
             unsigned fl;
@@ -380,6 +383,7 @@ __device__ __forceinline__ void flush_run(const SpectraArgs &a, const Tables &T,
         unsigned fl;
         const long long q = to_fixed(tot, ds.fx_scale, bad, fl);
         const size_t cell = (size_t)p * a.total_bins + ds.bin_off + r.cur;
+        PHYLINO_ASSERT(cell < (size_t)a.P * a.total_bins);
         if (q) atomicAdd((unsigned long long *)a.acc + cell, (unsigned long long)q);
         if (fl) atomicOr(a.flags + cell, fl);
     }
@@ -663,6 +667,7 @@ __device__ __forceinline__ int load_hint(const DatasetDev &ds, int np, int lane,
         int lg, pl, mine;
         substream_of(np, lane, nb, lg, pl, my0, mine);
     }
+    PHYLINO_ASSERT(b0 + my0 >= 0 && (b0 + my0 < ds.n_batches || (nb == 0 && b0 + my0 <= ds.n_batches)));
     return __ldg(ds.hint + (b0 + my0) / HINT_BATCHES);
 }
 
@@ -697,6 +702,8 @@ __device__ __forceinline__ void walk_unit(const SpectraArgs &a, const Tables &T,
 #endif
     Run<S> r;
     run_reset<S>(r);
+    PHYLINO_ASSERT(my0 >= 0 && mine >= 0 && my0 + mine <= nb && p >= 0 && p < a.P);
+    PHYLINO_ASSERT(row >= 0 && row < a.thr_rows);
     const Rec *bp = static_cast<const Rec *>(unit) + my0;
     if (mine > 0) open_run<S>(ds, thr, safe, bp->v[0], hint, r);
 #ifdef PHYLINO_TRACE
@@ -736,6 +743,7 @@ __device__ __forceinline__ void decode_item(const SpectraArgs &a, unsigned item,
         d = a.n_datasets - 1;
         b0 = a.tail_b0 + (unit - a.tail_unit) * a.tail_batches;
         b1 = min(b0 + a.tail_batches, a.ds[d].n_batches);
+        PHYLINO_ASSERT(b0 >= 0 && b0 < b1 && (unsigned)(b1 - b0) * rec_bytes(a.ds[d]) <= (unsigned)STAGE_BUF_BYTES);
         return;
     }
     d = 0;
@@ -743,6 +751,9 @@ __device__ __forceinline__ void decode_item(const SpectraArgs &a, unsigned item,
         if (unit >= a.ds[i].unit_begin) d = i;
     b0 = (unit - a.ds[d].unit_begin) * a.unit_batches;
     b1 = min(b0 + a.unit_batches, a.ds[d].n_batches);
+    PHYLINO_ASSERT(item < (unsigned)a.n_items && d >= 0 && d < a.n_datasets);
+    PHYLINO_ASSERT(b0 >= 0 && b0 < b1 && b1 <= a.ds[d].n_batches);
+    PHYLINO_ASSERT((unsigned)(b1 - b0) * rec_bytes(a.ds[d]) <= (unsigned)STAGE_BUF_BYTES);
 }
 
 /* The persistent warp: its first two items are static (warp index, + number of warps), later ones come from
@@ -915,6 +926,14 @@ __global__ void __launch_bounds__(WARPS * 32, 4) spectra_fused_kernel(const __gr
     double *rec_s = reinterpret_cast<double *>(stage + (size_t)WARPS * 2 * STAGE_BUF_BYTES);
     float2 *safe_s = reinterpret_cast<float2 *>(rec_s + (size_t)(2 * S + 2) * a.P);
     float *thr_s = reinterpret_cast<float *>(safe_s + (size_t)a.thr_rows * a.n_datasets);
+#ifdef PHYLINO_CHECKED
+    {
+        unsigned dyn;
+        asm volatile("mov.u32 %0, %%dynamic_smem_size;" : "=r"(dyn));
+        PHYLINO_ASSERT((size_t)((unsigned char *)(thr_s + (size_t)a.thr_rows * a.thr_stride) - stage) <= dyn);
+        PHYLINO_ASSERT(a.P >= 1 && a.P <= FUSED_MAX_POINTS && a.n_chunks == 1 && a.tail_unit == a.n_units);
+    }
+#endif
     /* a.params == NULL: the batch came by value with the kernel arguments (host entry points, small batches) */
     const double *params = a.params ? a.params : blob.v;
     if ((int)threadIdx.x < a.P) point_record<S>(a, params, threadIdx.x, rec_s);
