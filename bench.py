@@ -45,6 +45,10 @@ HEADLINE_CONFIG = 5
 # the SASS of the hot loop has exactly these (9 DFMA + 1 DADD + 1 DMUL per event x point x term,
 # profiles/r2_hot_loop_sass.md).  The bin/weight bookkeeping is per batch of events and per run, not per event x point.
 FP64_PER_TERM = 11
+# ... and 7 for the LAST term where its phase stays below an eighth of a half-turn for every event and point of a
+# group (no range reduction, a cubic instead of a quintic: devmath.cuh half_cos_small); the library reports the
+# fraction of event x point evaluations that took it (phylino_last_small_phase), the roofline counts what ran
+FP64_SMALL_TERM = 7
 # nominal fp64 pipe, derived in DESIGN.md section 7 (the guide has no fp64 row): 64 fp64 lanes/clk/SM (one DFMA
 # per lane and clock) x SMs x the SM clock nvidia-smi reports as maximum
 FP64_LANES_PER_SM = 64
@@ -223,6 +227,7 @@ def measure(pkg, torch, dist, k, steps, warmup, local, rank, world, flush, tunin
         inst_ms.append(s0.elapsed_time(e0))
         flush.zero_()
     torch.cuda.synchronize()
+    small_frac = ph.last_small_phase()
     clocks = sampler.stop() if sampler else None
     barrier()
     if world > 1:
@@ -286,8 +291,9 @@ def measure(pkg, torch, dist, k, steps, warmup, local, rank, world, flush, tunin
 
     res = None
     if rank == 0:
-        inst = fp64_inst_per_evpt(wl.model)
-        small = P <= 16 and not (inst == 33 and P > 4)      # the small-batch kernel (setup fused in) ran
+        inst_general = fp64_inst_per_evpt(wl.model)
+        inst = inst_general - (FP64_PER_TERM - FP64_SMALL_TERM) * small_frac      # fp64 instructions executed
+        small = P <= 16 and not (inst_general == 33 and P > 4)      # the small-batch kernel (setup fused in) ran
         sp = stats_ms(sp_ms)
         sm_max_mhz = (clocks or {}).get("sm_max_mhz") or 1965.0
         sm_count = torch.cuda.get_device_properties(local).multi_processor_count
@@ -304,7 +310,8 @@ def measure(pkg, torch, dist, k, steps, warmup, local, rank, world, flush, tunin
             "measured_dfma_peak": None if measured_peak is None else measured_peak / 1e9,
             "frac_of_measured_dfma_peak": None if not measured_peak else achieved / measured_peak,
             "traffic": traffic, "traffic_source": traffic_source,
-            "fp64_inst_per_event_point": inst, "kernel_ms": sp["mean"], "kernel_ms_median": sp["median"],
+            "fp64_inst_per_event_point": inst, "fp64_inst_general_form": inst_general,
+            "small_phase_fraction": small_frac, "kernel_ms": sp["mean"], "kernel_ms_median": sp["median"],
             "kernel_ms_min": sp["min"],
             "kernel_share_of_step": sp["mean"] / (sum(inst_ms) / steps),
             "kernel_timing": f"second pass of {steps} steps with CUDA events around each kernel on the library's "

@@ -333,6 +333,13 @@ PHYLINO_API phylino_status phylino_last_plan(const phylino_ctx *ctx, int64_t *vi
 PHYLINO_API phylino_status phylino_set_timing(phylino_ctx *ctx, int on);
 PHYLINO_API phylino_status phylino_last_kernel_ms(phylino_ctx *ctx, float *ms);
 
+/* Which arithmetic the last spectra launch of this context ran (for the roofline accounting of bench.py): the
+ * fraction, weighted by events x points, of (point group, dataset) pairs whose LAST oscillation term took the
+ * small-phase form of 1/2 cos(2 phase) -- 7 fp64 instructions per event x point instead of 11.  The kernels pick it
+ * per group of 32 points and dataset where |1.267 dm2 (2/pi) L/E| <= 1/8 for every event and point (the solar term
+ * at Double-Chooz baselines).  fraction HOST; synchronises the stream. */
+PHYLINO_API phylino_status phylino_last_small_phase(phylino_ctx *ctx, double *fraction_host);
+
 /* Kernel launches enqueued by this context so far (bench.py's `gpu_launches`). */
 PHYLINO_API int64_t phylino_launch_count(const phylino_ctx *ctx);
 

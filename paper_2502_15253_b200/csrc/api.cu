@@ -102,7 +102,9 @@ void free_all(phylino_ctx *c)
     cudaFree(c->d_acc); cudaFree(c->d_flags);
     c->d_acc = nullptr; c->d_flags = nullptr; c->acc_capacity = 0;
     cudaFree(c->d_rec); cudaFree(c->d_thr); cudaFree(c->d_safe); cudaFree(c->d_counter); cudaFree(c->d_done);
+    cudaFree(c->d_small);
     c->d_rec = nullptr; c->d_thr = nullptr; c->d_safe = nullptr; c->d_counter = nullptr; c->d_done = nullptr;
+    c->d_small = nullptr;
     c->point_capacity = 0;
     cudaFree(c->d_plan); c->d_plan = nullptr; c->plan_capacity = 0;
     cudaFree(c->d_mu); c->d_mu = nullptr; c->mu_capacity = 0;
@@ -162,12 +164,13 @@ phylino_status ensure_acc(phylino_ctx *ctx, int P)
     if (P > ctx->point_capacity) {
         /* per-point records and threshold rows written by the setup kernel of every call */
         CU(cudaStreamSynchronize(ctx->stream));
-        cudaFree(ctx->d_rec); cudaFree(ctx->d_thr); cudaFree(ctx->d_safe);
-        ctx->d_rec = nullptr; ctx->d_thr = nullptr; ctx->d_safe = nullptr; ctx->point_capacity = 0;
+        cudaFree(ctx->d_rec); cudaFree(ctx->d_thr); cudaFree(ctx->d_safe); cudaFree(ctx->d_small);
+        ctx->d_rec = nullptr; ctx->d_thr = nullptr; ctx->d_safe = nullptr; ctx->d_small = nullptr; ctx->point_capacity = 0;
         const int64_t rows = ctx->per_point_binning ? P : 1;      /* (sized for mode 0 even while mode 1 is on) */
         CU(cudaMalloc((void **)&ctx->d_rec, (size_t)rec_fields(ctx->n_terms) * P * sizeof(double)));
         CU(cudaMalloc((void **)&ctx->d_thr, (size_t)rows * (ctx->total_bins + ctx->n_datasets) * sizeof(float)));
         CU(cudaMalloc((void **)&ctx->d_safe, (size_t)rows * ctx->n_datasets * sizeof(float2)));
+        CU(cudaMalloc((void **)&ctx->d_small, (size_t)((P + 31) / 32 + 4) * ctx->n_datasets));
         ctx->point_capacity = P;
     }
     return PHYLINO_OK;
@@ -194,6 +197,7 @@ void fill_datasets(const phylino_ctx *ctx, SpectraArgs &a)
         v.v_pos_min = h.v_pos_min;
         v.v_max = h.v_max;
         v.fx_scale = std::ldexp(1.0, h.fx_exp);
+        v.x_max = h.x_max;
     }
     a.osc.osc_model = ctx->osc_model;
     a.osc.ordering = ctx->ordering_override ? ctx->ordering_override : ctx->ordering;
@@ -205,6 +209,7 @@ void fill_datasets(const phylino_ctx *ctx, SpectraArgs &a)
     a.rec = ctx->d_rec;
     a.thr = ctx->d_thr;
     a.safe = ctx->d_safe;
+    a.small = ctx->d_small;
     a.acc = ctx->d_acc;
     a.flags = ctx->d_flags;
     a.counter = ctx->d_counter;
@@ -348,6 +353,7 @@ phylino_status enqueue_eval(phylino_ctx *ctx, int P, const double *params, const
     phylino_status s = fill_batch(ctx, a, P, params);
     if (s != PHYLINO_OK) return s;
     const bool dbg = bins != nullptr;
+    ctx->last_points = P;
     a.dbg_bins = bins;
     a.total_events = phylino_total_events(ctx);
     FinalizeArgs f = ctx->fin;
@@ -479,7 +485,7 @@ int term_deps(int osc_model, int k, int slots[3])
 {
     if (osc_model == PHYLINO_OSC_EQ1) { slots[0] = k == 0 ? PHYLINO_MEE : PHYLINO_M21; return 1; }
     if (osc_model == PHYLINO_OSC_STERILE4) { slots[0] = k == 0 ? PHYLINO_MEE : (k == 1 ? PHYLINO_M41 : PHYLINO_M21); return 1; }
-    if (k == 0) { slots[0] = PHYLINO_M21; return 1; }
+    if (k == 2) { slots[0] = PHYLINO_M21; return 1; }            /* FULL3: (31, 32, 21) */
     slots[0] = PHYLINO_MEE; slots[1] = PHYLINO_S12; slots[2] = PHYLINO_M21;
     return 3;
 }
@@ -624,6 +630,7 @@ phylino_status enqueue_cached(phylino_ctx *ctx, int P, const double *h_params, c
     fill_datasets(ctx, a);
     a.comp = 1;
     if ((s = fill_batch(ctx, a, V, d_params, pl.C)) != PHYLINO_OK) return s;
+    ctx->last_points = V;
     a.vp_class = ctx->d_plan;
     a.vp_src = ctx->d_plan + V;
     a.class_rep = ctx->d_plan + V + (int64_t)V * S;
@@ -901,12 +908,14 @@ phylino_status phylino_load_events(phylino_ctx *ctx, int dataset, int64_t n, con
     /* where a lane starts looking for its bin (a hint, never trusted): the bin of the first event of every
      * HINT_BATCHES-th batch under the identity energy scale */
     std::vector<int32_t> hint((size_t)((n_batches + HINT_BATCHES - 1) / HINT_BATCHES), n_bins);
+    double x_max = 0.0;
     for (int64_t i = 0; i < n; ++i) {
         const int32_t s = perm[i];
         const int64_t b = i / EB;
         const int j = (int)(i % EB);
         const float vi = e_vis[s];
         const double xi = baseline_m[core ? core[s] : 0] / (double)e_nu[s];
+        x_max = std::max(x_max, xi);
         if (unit_w) {
             ev_u[(size_t)b].x[j] = xi;
             ev_u[(size_t)b].v[j] = vi;
@@ -945,7 +954,7 @@ phylino_status phylino_load_events(phylino_ctx *ctx, int dataset, int64_t n, con
     }
     CU(cudaStreamSynchronize(st));
     h.n = n; h.n_pad = n_pad; h.wsum_abs = wsum; h.fx_exp = fx; h.loaded = true;
-    h.v_pos_min = v_pos_min; h.v_max = v_max; h.unit_w = unit_w;
+    h.v_pos_min = v_pos_min; h.v_max = v_max; h.unit_w = unit_w; h.x_max = x_max;
     ctx->err.clear();
     return PHYLINO_OK;
 }
@@ -1391,6 +1400,30 @@ phylino_status phylino_last_plan(const phylino_ctx *ctx, int64_t *virtual_points
     if (!ctx || !virtual_points || !classes) return PHYLINO_ERR_ARG;
     *virtual_points = ctx->last_virtual_points;
     *classes = ctx->last_classes;
+    return PHYLINO_OK;
+}
+
+phylino_status phylino_last_small_phase(phylino_ctx *ctx, double *fraction_host)
+{
+    if (!ctx || !fraction_host) return PHYLINO_ERR_ARG;
+    *fraction_host = 0.0;
+    const int P = ctx->last_points;
+    if (!ctx->have_model || P <= 0 || !ctx->d_small) return PHYLINO_OK;
+    DeviceGuard g(ctx->device);
+    const int n_groups = (P + 31) / 32, D = ctx->n_datasets;
+    std::vector<unsigned char> flags((size_t)n_groups * D);
+    CU(cudaMemcpyAsync(flags.data(), ctx->d_small, flags.size(), cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    double small = 0.0, total = 0.0;
+    for (int gi = 0; gi < n_groups; ++gi) {
+        const double np = std::min(32, P - 32 * gi);
+        for (int d = 0; d < D; ++d) {
+            const double w = np * (double)ctx->ds[d].n;
+            total += w;
+            if (flags[(size_t)gi * D + d]) small += w;
+        }
+    }
+    *fraction_host = total > 0.0 ? small / total : 0.0;
     return PHYLINO_OK;
 }
 

@@ -23,7 +23,14 @@ namespace phylino {
  * once per group, ONE POINT PER LANE.  Small batches: every warp owns one contiguous range of batches and
  * setup, walk and likelihood run in ONE launch (spectra.cu). */
 constexpr int EB          = 4;                      /* events per batch; every dataset is padded to a multiple */
-constexpr int WARPS       = 4;                      /* warps per CTA of the spectra kernels */
+#ifndef PHYLINO_WARPS
+#define PHYLINO_WARPS 4
+#endif
+#ifndef PHYLINO_CTAS_PER_SM
+#define PHYLINO_CTAS_PER_SM 4
+#endif
+constexpr int WARPS       = PHYLINO_WARPS;          /* warps per CTA of the spectra kernels */
+constexpr int CTAS_PER_SM = PHYLINO_CTAS_PER_SM;    /* ... and CTAs per SM their register budget is set for */
 constexpr int STAGE_BUF_BYTES = 6144;               /* one staging buffer of a warp: a unit is at most this long */
 constexpr int MAX_UNIT_BATCHES = 64;                /* ticket schedule: batches per unit (<= 6 KB of 96-byte records) */
 constexpr int HINT_BATCHES = 16;                    /* one bin hint per this many batches of a dataset */
@@ -75,6 +82,7 @@ struct DatasetDev {
     float   v_pos_min;      /* smallest positive finite E_vis of the dataset (+inf if none) */
     float   v_max;          /* largest finite E_vis (-inf if none) */
     double  fx_scale;       /* 2^e: fixed-point scale of the bin accumulators */
+    double  x_max;          /* largest L/E_nu of the dataset (0 if empty) */
 };
 
 struct OscDev {
@@ -115,6 +123,7 @@ struct SpectraArgs {
     double       *rec;      /* DEVICE [rec_fields x P] per-point records (setup kernel) */
     float        *thr;      /* DEVICE [thr_rows x thr_stride] fp32 bin thresholds (setup kernel) */
     float2       *safe;     /* DEVICE [thr_rows x n_datasets] fp32 interval on which a row holds */
+    unsigned char *small;   /* DEVICE [n_groups x n_datasets] small-phase flag of the last term (setup kernel) */
     long long    *acc;      /* DEVICE [P x total_bins] fixed-point accumulators (zero on entry) */
     unsigned     *flags;    /* DEVICE [P x total_bins] FLAG_* (zero on entry) */
     /* component mode (cross-point caching; api.cu plan_components): the P
@@ -229,6 +238,7 @@ struct phylino_dataset_host {
     float    v_pos_min = 0.f, v_max = 0.f;
     bool     unit_w = false;
     int      fx_exp = 0;
+    double   x_max = 0.0;
     void    *d_ev = nullptr;                        /* EventBatchU[] if unit_w else EventBatchW[] */
     int32_t *d_hint = nullptr;
     double  *d_edges = nullptr;
@@ -258,6 +268,7 @@ struct phylino_ctx {
     double   *d_rec = nullptr;                     /* [rec_fields x point_capacity] */
     float    *d_thr = nullptr;                     /* [thr_rows x (total_bins + n_datasets)] */
     float2   *d_safe = nullptr;                    /* [thr_rows x n_datasets] */
+    unsigned char *d_small = nullptr;              /* [ceil(point_capacity / 32) x n_datasets] */
     /* cross-point caching of the host-buffer entry points (phylino_set_caching) */
     bool caching = false;
     int32_t *d_plan = nullptr;                     /* vp_class | vp_src | class_rep | pt_comp */
@@ -278,6 +289,7 @@ struct phylino_ctx {
     int64_t work_capacity = 0;
     int ordering_override = 0;                     /* +-1 while an ordering scan runs, else 0 */
     int ec_mode = 0;                               /* phylino_set_energy_correction_mode */
+    int last_points = 0;                           /* launch points of the last spectra launch (phylino_last_small_phase) */
     std::vector<std::vector<int32_t>> fm_idx;      /* per dataset: fine-grid flux parameters (phylino_set_flux_model) */
     std::vector<double> fm_lo, fm_width;
     /* host-buffer entry points: pinned + device staging */

@@ -204,11 +204,13 @@ struct Tables {
     const double *rec;      /* [rec_fields x P]: h_k, A_k, P0, bad */
     const float  *thr;      /* [thr_rows x thr_stride] */
     const float2 *safe;     /* [thr_rows x n_datasets] */
+    const unsigned char *small;     /* [n_groups x n_datasets] the last term takes half_cos_small for this group and dataset */
 };
 
 /* row a1: record of launch point p -> rec[field * P + p] */
+/* returns the half-turn coefficient of the point's last term */
 template <int S>
-__device__ __forceinline__ void point_record(const SpectraArgs &a, const double *params, int p, double *rec)
+__device__ __forceinline__ double point_record(const SpectraArgs &a, const double *params, int p, double *rec)
 {
     if (a.comp) {
         /* virtual point: slot s computes the half-turn coefficient of (real point, term) vp_src */
@@ -219,7 +221,7 @@ __device__ __forceinline__ void point_record(const SpectraArgs &a, const double 
             osc_terms(a.osc, params + (size_t)(src >> 2) * a.n_params, A, dm2);
             rec[(size_t)k * a.P + p] = halfturn_coeff(dm2[src & 3]);
         }
-        return;
+        return rec[(size_t)(S - 1) * a.P + p];
     }
     const double *theta = params + (size_t)p * a.n_params;
     double A[MAX_TERMS], dm2[MAX_TERMS];
@@ -236,6 +238,18 @@ __device__ __forceinline__ void point_record(const SpectraArgs &a, const double 
     /* |P0| + 1/2 sum|A_k| <= 1 + sum|A_k| <= 4 keeps every run total inside the fixed-point range
      * (phylino.h "Errors": a point beyond this bound reads NaN) */
     rec[(size_t)(2 * S + 1) * a.P + p] = (asum <= 3.0) ? 0.0 : 1.0;
+    return rec[(size_t)(S - 1) * a.P + p];
+}
+
+/* One warp, its lane's last coefficient (0 for a lane without a point): small[d] = the phase of the last term stays
+ * within SMALL_PHASE over dataset d for all 32 lanes.  A NaN coefficient compares false and lands on the cheap form,
+ * where it is as much a NaN as on the other. */
+__device__ __forceinline__ void group_flags(const SpectraArgs &a, double h_last, unsigned char *small)
+{
+    for (int d = 0; d < a.n_datasets; ++d) {
+        const bool big = __any_sync(0xffffffffu, fabs(h_last) * a.ds[d].x_max > SMALL_PHASE);
+        if ((threadIdx.x & 31) == 0) small[d] = big ? 0 : 1;
+    }
 }
 
 /* tables of row a3: entry e of threshold row `row` (and the row's validity interval per dataset) */
@@ -319,7 +333,8 @@ __global__ void __launch_bounds__(SETUP_THREADS) setup_kernel(const __grid_const
     if ((int)blockIdx.x < rec_blocks) {
         const int p = blockIdx.x * SETUP_THREADS + threadIdx.x;
         if (p == 0) *a.counter = 0u;                            /* the work counter of ticket_loop */
-        if (p < a.P) point_record<S>(a, a.params, p, a.rec);
+        const double h_last = p < a.P ? point_record<S>(a, a.params, p, a.rec) : 0.0;
+        group_flags(a, h_last, a.small + (size_t)(p >> 5) * a.n_datasets);      /* SETUP_THREADS is a multiple of 32 */
         return;
     }
     const int row = blockIdx.x - rec_blocks;
@@ -515,7 +530,7 @@ __device__ __forceinline__ void open_run(const DatasetDev &ds, const float *thr,
 
 /* K consecutive batches known to lie inside the lane's open run (the store is sorted: the last
  * event of the last batch is below r.hi): rows a2 + a4 only, straight-line. */
-template <int S, bool UW, int K, bool DBG>
+template <int S, bool UW, int K, bool DBG, bool SM>
 __device__ __forceinline__ void walk_inside(const SpectraArgs &a, const DatasetDev &ds,
                                             const typename RecOf<UW>::type *bp, int gb, const double (&h)[S], int p,
                                             bool active, Run<S> &r)
@@ -530,15 +545,15 @@ __device__ __forceinline__ void walk_inside(const SpectraArgs &a, const DatasetD
                 /* every weight of the dataset is exactly 1 (the padding sits behind a NaN E_vis and never
                  * reaches this path): 1 * g + C == g + C bit for bit, and no weight is stored */
 #pragma unroll
-                for (int k = 0; k < S; ++k) r.C[k] += half_cos_halfturns(h[k], t.x);
+                for (int k = 0; k < S; ++k) r.C[k] += half_cos_term<S, SM>(k, h[k], t.x);
 #pragma unroll
-                for (int k = 0; k < S; ++k) r.C[k] += half_cos_halfturns(h[k], t.y);
+                for (int k = 0; k < S; ++k) r.C[k] += half_cos_term<S, SM>(k, h[k], t.y);
             } else {
                 const double2 w = q[EB / 2 + j];
 #pragma unroll
-                for (int k = 0; k < S; ++k) r.C[k] = fma(w.x, half_cos_halfturns(h[k], t.x), r.C[k]);
+                for (int k = 0; k < S; ++k) r.C[k] = fma(w.x, half_cos_term<S, SM>(k, h[k], t.x), r.C[k]);
 #pragma unroll
-                for (int k = 0; k < S; ++k) r.C[k] = fma(w.y, half_cos_halfturns(h[k], t.y), r.C[k]);
+                for (int k = 0; k < S; ++k) r.C[k] = fma(w.y, half_cos_term<S, SM>(k, h[k], t.y), r.C[k]);
             }
         }
         if (!UW) r.W += reinterpret_cast<const EventBatchW *>(bp + u)->wsum;
@@ -603,7 +618,7 @@ __device__ __noinline__ Run<S> walk_batch_slow(const SpectraArgs &a, Tables T, c
 }
 
 /* One batch of the lane's stream (rows a2-a4); gb: its index in the dataset. */
-template <int S, bool UW, bool DBG>
+template <int S, bool UW, bool DBG, bool SM>
 __device__ __forceinline__ void walk_batch(const SpectraArgs &a, const Tables &T, const DatasetDev &ds,
                                            const typename RecOf<UW>::type *bp, int gb, const double (&h)[S],
                                            const float *thr, float2 safe, int p, bool active, Run<S> &r)
@@ -611,7 +626,7 @@ __device__ __forceinline__ void walk_batch(const SpectraArgs &a, const Tables &T
     if (bp->v[EB - 1] < r.hi) {
         /* rows a3 + a4: the store is sorted, so the whole batch lies in the run's bin (a padding event has
          * E_vis = NaN and fails the test: it never comes here) */
-        walk_inside<S, UW, 1, DBG>(a, ds, bp, gb, h, p, active, r);
+        walk_inside<S, UW, 1, DBG, SM>(a, ds, bp, gb, h, p, active, r);
     } else {
         Coef<S> c;
 #pragma unroll
@@ -621,7 +636,7 @@ __device__ __forceinline__ void walk_batch(const SpectraArgs &a, const Tables &T
 }
 
 /* `mine` consecutive batches of the lane's stream starting at bp (dataset batch gb): 4, 2 or 1 at a time */
-template <int S, bool UW, bool DBG>
+template <int S, bool UW, bool DBG, bool SM>
 __device__ __forceinline__ void walk_stretch(const SpectraArgs &a, const Tables &T, const DatasetDev &ds,
                                              const typename RecOf<UW>::type *bp, int gb, int mine, const double (&h)[S],
                                              const float *thr, float2 safe, int p, bool active, Run<S> &r)
@@ -630,15 +645,15 @@ __device__ __forceinline__ void walk_stretch(const SpectraArgs &a, const Tables 
 #pragma unroll 1
     while (i < mine) {
         if (i + 4 <= mine && bp[3].v[EB - 1] < r.hi) {
-            walk_inside<S, UW, 4, DBG>(a, ds, bp, gb + i, h, p, active, r);
+            walk_inside<S, UW, 4, DBG, SM>(a, ds, bp, gb + i, h, p, active, r);
             i += 4;
             bp += 4;
         } else if (i + 2 <= mine && bp[1].v[EB - 1] < r.hi) {
-            walk_inside<S, UW, 2, DBG>(a, ds, bp, gb + i, h, p, active, r);
+            walk_inside<S, UW, 2, DBG, SM>(a, ds, bp, gb + i, h, p, active, r);
             i += 2;
             bp += 2;
         } else {
-            walk_batch<S, UW, DBG>(a, T, ds, bp, gb + i, h, thr, safe, p, active, r);
+            walk_batch<S, UW, DBG, SM>(a, T, ds, bp, gb + i, h, thr, safe, p, active, r);
             ++i;
             ++bp;
         }
@@ -709,7 +724,9 @@ __device__ __forceinline__ void walk_unit(const SpectraArgs &a, const Tables &T,
 #ifdef PHYLINO_TRACE
     const long long q1 = clock64();
 #endif
-    walk_stretch<S, UW, DBG>(a, T, ds, bp, b0 + my0, mine, h, thr, safe, p, active, r);
+    /* the last term's phase stays small over this dataset for every point of the group: its cheap form */
+    if (T.small[g * a.n_datasets + d]) walk_stretch<S, UW, DBG, true>(a, T, ds, bp, b0 + my0, mine, h, thr, safe, p, active, r);
+    else                               walk_stretch<S, UW, DBG, false>(a, T, ds, bp, b0 + my0, mine, h, thr, safe, p, active, r);
 #ifdef PHYLINO_TRACE
     const long long q2 = clock64();
 #endif
@@ -875,7 +892,7 @@ __device__ __forceinline__ void ticket_loop(const SpectraArgs &a, const Tables &
 }
 
 template <int S, bool DBG>
-__global__ void __launch_bounds__(WARPS * 32, 4) spectra_kernel(const __grid_constant__ SpectraArgs a)
+__global__ void __launch_bounds__(WARPS * 32, CTAS_PER_SM) spectra_kernel(const __grid_constant__ SpectraArgs a)
 {
     static_assert(EB == 4, "the batch loads are written for EB = 4");
     extern __shared__ __align__(128) unsigned char stage[];       /* [WARPS][2][STAGE_BUF_BYTES] */
@@ -895,6 +912,7 @@ __global__ void __launch_bounds__(WARPS * 32, 4) spectra_kernel(const __grid_con
     T.rec = a.rec;
     T.thr = a.thr;
     T.safe = a.safe;
+    T.small = a.small;
     ticket_loop<S, DBG, false>(a, T, a.counter, wp, cur, nW, lane);
 }
 
@@ -904,12 +922,13 @@ __global__ void __launch_bounds__(WARPS * 32, 4) spectra_kernel(const __grid_con
  * zeroes the work counter a.done again.  A batch of at most PARAM_BLOB_DOUBLES parameters may travel by value
  * with the kernel arguments (blob): a host call then needs no copy engine at all. */
 template <int S, bool DBG>
-__global__ void __launch_bounds__(WARPS * 32, 4) spectra_fused_kernel(const __grid_constant__ SpectraArgs a,
+__global__ void __launch_bounds__(WARPS * 32, CTAS_PER_SM) spectra_fused_kernel(const __grid_constant__ SpectraArgs a,
                                                                       const __grid_constant__ ParamBlob blob)
 {
     /* [WARPS][2][STAGE_BUF_BYTES] stage | rec [rec_fields x P] | safe [thr_rows x D] | thr [thr_rows x thr_stride] */
     extern __shared__ __align__(128) unsigned char stage[];
     __shared__ unsigned long long bars[WARPS][2];
+    __shared__ unsigned char small_s[PHYLINO_MAX_DATASETS];
     const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
     const unsigned nW = gridDim.x * WARPS, cur = blockIdx.x * WARPS + wib;
     TRACE_MIN(0);
@@ -936,16 +955,21 @@ __global__ void __launch_bounds__(WARPS * 32, 4) spectra_fused_kernel(const __gr
 #endif
     /* a.params == NULL: the batch came by value with the kernel arguments (host entry points, small batches) */
     const double *params = a.params ? a.params : blob.v;
-    if ((int)threadIdx.x < a.P) point_record<S>(a, params, threadIdx.x, rec_s);
+    if (threadIdx.x < 32) {             /* at most FUSED_MAX_POINTS <= 32 points: the first warp */
+        const double h_last = (int)threadIdx.x < a.P ? point_record<S>(a, params, threadIdx.x, rec_s) : 0.0;
+        group_flags(a, h_last, small_s);
+    }
     for (int e = threadIdx.x; e < a.thr_rows * a.thr_stride; e += WARPS * 32)
         threshold_entry(a, params, e / a.thr_stride, e % a.thr_stride, thr_s, safe_s);
     __syncthreads();
     TRACE_MAX(2);
+    if (blockIdx.x == 0 && (int)threadIdx.x < a.n_datasets) a.small[threadIdx.x] = small_s[threadIdx.x];   /* for phylino_last_small_phase */
     Tables T;
     T.params = params;
     T.rec = rec_s;
     T.thr = thr_s;
     T.safe = safe_s;
+    T.small = small_s;
     ticket_loop<S, DBG, true>(a, T, a.done, wp, cur, nW, lane);
     TRACE_MIN(3);
     TRACE_MAX(4);
@@ -953,7 +977,8 @@ __global__ void __launch_bounds__(WARPS * 32, 4) spectra_fused_kernel(const __gr
 
 /* dynamic shared memory of one CTA: two unit buffers per warp */
 constexpr size_t STAGE_BYTES = (size_t)WARPS * 2 * STAGE_BUF_BYTES;
-constexpr size_t FUSED_TABLE_MAX = 160 * 1024;          /* records + thresholds of the single-launch kernel */
+/* records + thresholds of the small-batch kernel: what 227 KB of shared memory per CTA leave beside the staging */
+constexpr size_t FUSED_TABLE_MAX = (227 * 1024 - 1024 - STAGE_BYTES) < 160 * 1024 ? (227 * 1024 - 1024 - STAGE_BYTES) : 160 * 1024;
 
 template <int S, bool DBG> cudaError_t launch_t(const SpectraArgs &a, cudaStream_t st, bool pdl)
 {
