@@ -400,6 +400,46 @@ def gradient_step_wall(pkg, torch, local, flush, steps=10):
         res[key + "_min"] = min(ts)
         if on:
             res["virtual_points"], res["energy_scale_classes"] = ph.last_plan()
+    ph.set_caching(False)
+    # a minimiser's SINGLE evaluation on the same store (one point over 6e6 events): bound by the event bytes over
+    # HBM, not by arithmetic -- the small-batch kernel (setup fused in) + the overlapped finalize kernel
+    d_data = torch.as_tensor(data, device="cuda")
+    single = {}
+    for n_pts in (1, 4, 16):
+        dp = torch.as_tensor(wl.params[:n_pts].copy(), device="cuda")
+        d_out = torch.empty(n_pts, dtype=torch.float64, device="cuda")
+        for _ in range(3):
+            ph.nll(dp, d_data, d_out)
+        ts = []
+        for i in range(max(steps, 20)):
+            flush.zero_()
+            s0, e0 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            s0.record()
+            ph.nll(dp, d_data, d_out)
+            e0.record()
+            torch.cuda.synchronize()
+            ts.append(s0.elapsed_time(e0) * 1e3)
+        hs = []
+        hp, ho = wl.params[:n_pts].copy(), np.empty(n_pts)
+        for i in range(max(steps, 20)):
+            flush.zero_()
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            ph.nll_host(hp, data, ho)
+            hs.append((time.perf_counter() - t0) * 1e6)
+        single[str(n_pts)] = {"device_step_us_median": statistics.median(ts), "device_step_us_min": min(ts),
+                              "host_call_us_median": statistics.median(hs), "host_call_us_min": min(hs)}
+    store_bytes = EVENT_BYTES * wl.n_events
+    floor_us = ph.hbm_read_floor(store_bytes, 10)
+    hbm = measured_hbm_gbs()
+    res["single_evaluation"] = {
+        "points": single, "event_store_bytes": store_bytes, "l2": "flushed before every call",
+        "hbm_time_at_measured_peak_us": store_bytes / (hbm * 1e9) * 1e6, "hbm_peak_gbs": hbm,
+        "hbm_read_floor_us": floor_us,
+        "hbm_read_floor_note": "device time of one kernel that only reads the store's bytes from HBM (L2 flushed), "
+                               "launch ramp included (phylino_hbm_read_floor)",
+        "frac_of_hbm_roofline_1pt": store_bytes / (hbm * 1e9) * 1e6 / single["1"]["device_step_us_median"],
+        "frac_of_read_floor_1pt": floor_us / single["1"]["device_step_us_median"]}
     ph.close()
     return res
 

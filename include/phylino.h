@@ -351,6 +351,12 @@ PHYLINO_API const char *phylino_last_error(const phylino_ctx *ctx);
  * returns the achieved fp64 FMA instructions per second (lane-operations/s) in *dfma_per_s. */
 PHYLINO_API phylino_status phylino_peak_fp64(phylino_ctx *ctx, int iters, double *dfma_per_s_host);
 
+/* Microbenchmark: device time in microseconds (HOST pointer; CUDA events, best of `reps`, L2 flushed before each) of
+ * one kernel that does nothing but read `bytes` from HBM with coalesced loads.  The practical floor, launch ramp
+ * included, under a call bound by its event bytes (one parameter point over a large event store): reported beside
+ * bytes / peak bandwidth.  Allocates bytes + 256 MiB for the duration of the call; synchronises. */
+PHYLINO_API phylino_status phylino_hbm_read_floor(phylino_ctx *ctx, int64_t bytes, int reps, double *us_host);
+
 /* Microbenchmark: host wall time, in microseconds per repetition (HOST pointer), of launching an empty
  * kernel on the context's stream and synchronising it -- the floor under any call whose result the host
  * waits for.  Launch-latency-bound workloads (one parameter point over a small event store) are reported

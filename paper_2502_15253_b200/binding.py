@@ -27,6 +27,7 @@ abi_symbols = (
     "phylino_launch_floor", "phylino_set_schedule", "phylino_reserve",
     "phylino_draw_pseudo_data", "phylino_ordering_scan", "phylino_nll_gradient",
     "phylino_set_energy_correction_mode", "phylino_set_flux_model", "phylino_last_small_phase",
+    "phylino_hbm_read_floor",
 )
 
 _STATUS = {0: "OK", 1: "ERR_ARG", 2: "ERR_SHAPE", 3: "ERR_STATE", 4: "ERR_OOM", 5: "ERR_CUDA"}
@@ -146,6 +147,8 @@ def load_library():
     lib.phylino_last_error.argtypes = [vp]
     lib.phylino_launch_floor.restype = i32
     lib.phylino_launch_floor.argtypes = [vp, i32, C.POINTER(dbl)]
+    lib.phylino_hbm_read_floor.restype = i32
+    lib.phylino_hbm_read_floor.argtypes = [vp, i64, i32, C.POINTER(dbl)]
     lib.phylino_peak_fp64.restype = i32
     lib.phylino_peak_fp64.argtypes = [vp, i32, C.POINTER(dbl)]
     _lib = lib
@@ -510,6 +513,12 @@ class Phylino:
         """microseconds per (empty-kernel launch + stream synchronise) on this context's stream."""
         v = C.c_double(0.0)
         self._check(self._lib.phylino_launch_floor(self._ctx, int(reps), C.byref(v)))
+        return float(v.value)
+
+    def hbm_read_floor(self, nbytes: int, reps: int = 10) -> float:
+        """microseconds of one kernel that only reads nbytes from HBM (L2 flushed), best of reps"""
+        v = C.c_double(0.0)
+        self._check(self._lib.phylino_hbm_read_floor(self._ctx, int(nbytes), int(reps), C.byref(v)))
         return float(v.value)
 
     def peak_fp64(self, iters: int = 4096) -> float:

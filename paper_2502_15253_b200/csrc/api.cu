@@ -1461,6 +1461,16 @@ phylino_status phylino_launch_floor(phylino_ctx *ctx, int reps, double *us_per_c
     return PHYLINO_OK;
 }
 
+phylino_status phylino_hbm_read_floor(phylino_ctx *ctx, int64_t bytes, int reps, double *us_host)
+{
+    if (!ctx || !us_host || reps < 1 || bytes < 16 || bytes > ((int64_t)1 << 36)) return PHYLINO_ERR_ARG;
+    DeviceGuard g(ctx->device);
+    CU(cudaStreamSynchronize(ctx->stream));
+    CU(run_hbm_read_floor((size_t)bytes, reps, ctx->stream, us_host));
+    ctx->launches += reps + 2;
+    return PHYLINO_OK;
+}
+
 phylino_status phylino_peak_fp64(phylino_ctx *ctx, int iters, double *dfma_per_s_host)
 {
     if (!ctx || !dfma_per_s_host || iters < 1) return PHYLINO_ERR_ARG;

@@ -218,6 +218,7 @@ cudaError_t launch_gradient(const double *theta, const double *h, const double *
                             double *grad, cudaStream_t st);
 cudaError_t run_peak_fp64(int iters, cudaStream_t st, double *dfma_per_s);
 cudaError_t run_launch_floor(int reps, cudaStream_t st, double *us_per_call);
+cudaError_t run_hbm_read_floor(size_t bytes, int reps, cudaStream_t st, double *us_best);
 
 } // namespace phylino
 
