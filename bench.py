@@ -40,15 +40,18 @@ import workloads  # noqa: E402
 METRIC = "oscillated event x param-point/s (batched spectra+NLL)"
 UNIT = "event*point/s"
 HEADLINE_CONFIG = 5
-# ALGORITHMIC fp64-pipe instructions per event x point: per oscillation term
-# 10 for 1/2 cos(2 phase) (3 range reduction, 1 square, 6 Horner) + 1 multiply-accumulate into the run;
-# the SASS of the hot loop has exactly these (9 DFMA + 1 DADD + 1 DMUL per event x point x term,
-# profiles/r2_hot_loop_sass.md).  The bin/weight bookkeeping is per batch of events and per run, not per event x point.
-FP64_PER_TERM = 11
-# ... and 7 for the LAST term where its phase stays below an eighth of a half-turn for every event and point of a
-# group (no range reduction, a cubic instead of a quintic: devmath.cuh half_cos_small); the library reports the
-# fraction of event x point evaluations that took it (phylino_last_small_phase), the roofline counts what ran
-FP64_SMALL_TERM = 7
+# ALGORITHMIC fp64-pipe instructions per event x point, unit-weight datasets (every
+# BASELINE.json config).  Per oscillation term: 3 range reduction + 1 square + 5 Horner + the last Horner step; the
+# two-term model accumulates with that last step itself (devmath.cuh half_cos_accumulate: 10), the three-term models
+# form g and add it (11).  The SASS of the hot loop has exactly these (profiles/r2a_hot_loop_sass.md, r2c_*).  The
+# bin/weight bookkeeping is per batch of events and per run, not per event x point.
+def fp64_per_general_term(S: int) -> int:
+    return 10 if S == 2 else 11
+# ... and 6 for the LAST term where its phase stays below an eighth of a half-turn for every event and point of a
+# group (no range reduction, a cubic instead of a quintic, accumulated with its last Horner step: devmath.cuh
+# half_cos_small_accumulate); the library reports the fraction of event x point evaluations that took it
+# (phylino_last_small_phase), the roofline counts what ran
+FP64_SMALL_TERM = 6
 # nominal fp64 pipe, derived in DESIGN.md section 7 (the guide has no fp64 row): 64 fp64 lanes/clk/SM (one DFMA
 # per lane and clock) x SMs x the SM clock nvidia-smi reports as maximum
 FP64_LANES_PER_SM = 64
@@ -56,9 +59,13 @@ L2_FLUSH_BYTES = 256 << 20
 EVENT_BYTES = 12            # unit-weight store: x fp64 + E_vis fp32 (every BASELINE.json config)
 
 
+def n_terms(model) -> int:
+    return 2 if model.osc_model == 0 else 3
+
+
 def fp64_inst_per_evpt(model) -> int:
-    S = 2 if model.osc_model == 0 else 3
-    return FP64_PER_TERM * S
+    S = n_terms(model)
+    return fp64_per_general_term(S) * S
 
 
 class ClockSampler(threading.Thread):
@@ -292,8 +299,8 @@ def measure(pkg, torch, dist, k, steps, warmup, local, rank, world, flush, tunin
     res = None
     if rank == 0:
         inst_general = fp64_inst_per_evpt(wl.model)
-        inst = inst_general - (FP64_PER_TERM - FP64_SMALL_TERM) * small_frac      # fp64 instructions executed
-        small = P <= 16 and not (inst_general == 33 and P > 4)      # the small-batch kernel (setup fused in) ran
+        inst = inst_general - (fp64_per_general_term(n_terms(wl.model)) - FP64_SMALL_TERM) * small_frac   # executed
+        small = P <= 16 and not (n_terms(wl.model) == 3 and P > 4)      # the small-batch kernel (setup fused in) ran
         sp = stats_ms(sp_ms)
         sm_max_mhz = (clocks or {}).get("sm_max_mhz") or 1965.0
         sm_count = torch.cuda.get_device_properties(local).multi_processor_count

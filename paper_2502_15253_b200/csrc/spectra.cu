@@ -345,7 +345,10 @@ __global__ void __launch_bounds__(SETUP_THREADS) setup_kernel(const __grid_const
 
 /* the lane's open run: events of ONE bin seen since the last flush */
 template <int S> struct Run {
-    double C[S];    /* sum of w g_k over the run */
+    double C[S];    /* sum of w g_k over the run; a FOLDED term (see folded()) holds only its oscillating part C'
+                     * (devmath.cuh, half_cos_accumulate), the rest is 1/2 W - odd[k] */
+    int    odd[S];  /* folded terms: events of the run whose half-turn count n_k is odd */
+    bool   sm;      /* the run's last term takes the small-phase form (fixed per group and dataset) */
     double W;       /* sum of w over the run */
     int    cur;     /* its bin; < 0 or >= n_bins: events that land in no bin (never flushed) */
     float  hi;      /* later events below hi stay in the run (-inf: re-locate at the next event) */
@@ -356,11 +359,26 @@ template <int S> struct Run {
 template <int S> __device__ __forceinline__ void run_reset(Run<S> &r)
 {
 #pragma unroll
-    for (int k = 0; k < S; ++k) r.C[k] = 0.0;
+    for (int k = 0; k < S; ++k) { r.C[k] = 0.0; r.odd[k] = 0; }
     r.W = 0.0;
     r.cur = -1;
     r.hi = -pos_inf();
     r.hi2 = pos_inf();
+    r.sm = false;
+}
+
+/* Which terms of a UNIT-WEIGHT run are accumulated in the folded form (devmath.cuh, half_cos_accumulate): the
+ * small-phase last term always (no sign, so the fold costs nothing: 6 fp64 instructions instead of 7); the general
+ * terms of the two-term model (10 + 2 integer instead of 11 + 1: config 3 +4 %).  Not the general terms of the
+ * three-term models: measured in round 2, config 4 lost 5.6 % (128 registers, fp64 pipe 91.7 -> 78.8 % busy, top stall
+ * "wait": the two extra integer instructions per term sit in the dependency chains of three terms at once). */
+template <int S> __device__ __forceinline__ bool folded(bool sm, int k) { return S == 2 || (sm && k == S - 1); }
+
+/* sum of w g_k over the run, whichever way it was accumulated */
+template <int S>
+__device__ __forceinline__ double run_sum(const DatasetDev &ds, const Run<S> &r, int k)
+{
+    return (ds.unit_w && folded<S>(r.sm, k)) ? r.C[k] + (0.5 * r.W - (double)r.odd[k]) : r.C[k];
 }
 
 /* diagnostic instantiation: the bin the hot loop gave event j of dataset batch gb at point p */
@@ -386,14 +404,14 @@ __device__ __forceinline__ void flush_run(const SpectraArgs &a, const Tables &T,
 #pragma unroll
         for (int j = 0; j <= S; ++j) {
             unsigned fl;
-            const long long q = to_fixed(j == 0 ? r.W : r.C[j - 1], ds.fx_scale, false, fl);
+            const long long q = to_fixed(j == 0 ? r.W : run_sum<S>(ds, r, j - 1), ds.fx_scale, false, fl);
             if (q) atomicAdd((unsigned long long *)a.acc + cell + (size_t)j * a.total_bins, (unsigned long long)q);
             if (fl) atomicOr(a.flags + cell + (size_t)j * a.total_bins, fl);
         }
     } else if (active && r.cur >= 0 && r.cur < ds.n_bins) {
         double tot = T.rec[(size_t)(2 * S) * a.P + p] * r.W;                 /* P0 W */
 #pragma unroll
-        for (int k = 0; k < S; ++k) tot = fma(T.rec[(size_t)(S + k) * a.P + p], r.C[k], tot);
+        for (int k = 0; k < S; ++k) tot = fma(T.rec[(size_t)(S + k) * a.P + p], run_sum<S>(ds, r, k), tot);
         const bool bad = T.rec[(size_t)(2 * S + 1) * a.P + p] != 0.0;
         unsigned fl;
         const long long q = to_fixed(tot, ds.fx_scale, bad, fl);
@@ -403,7 +421,7 @@ __device__ __forceinline__ void flush_run(const SpectraArgs &a, const Tables &T,
         if (fl) atomicOr(a.flags + cell, fl);
     }
 #pragma unroll
-    for (int k = 0; k < S; ++k) r.C[k] = 0.0;
+    for (int k = 0; k < S; ++k) { r.C[k] = 0.0; r.odd[k] = 0; }
     r.W = 0.0;
 }
 
@@ -462,11 +480,11 @@ __device__ __forceinline__ void flush_run_substreams(const SpectraArgs &a, const
         if (comp) {
             cell = (unsigned long long)p * (S + 1) * a.total_bins + ds.bin_off + r.cur;
 #pragma unroll
-            for (int j = 0; j <= S; ++j) q[j] = to_fixed(j == 0 ? r.W : r.C[j - 1], ds.fx_scale, false, fl[j]);
+            for (int j = 0; j <= S; ++j) q[j] = to_fixed(j == 0 ? r.W : run_sum<S>(ds, r, j - 1), ds.fx_scale, false, fl[j]);
         } else {
             double tot = T.rec[(size_t)(2 * S) * a.P + p] * r.W;
 #pragma unroll
-            for (int k = 0; k < S; ++k) tot = fma(T.rec[(size_t)(S + k) * a.P + p], r.C[k], tot);
+            for (int k = 0; k < S; ++k) tot = fma(T.rec[(size_t)(S + k) * a.P + p], run_sum<S>(ds, r, k), tot);
             cell = (unsigned long long)p * a.total_bins + ds.bin_off + r.cur;
             q[0] = to_fixed(tot, ds.fx_scale, T.rec[(size_t)(2 * S + 1) * a.P + p] != 0.0, fl[0]);
         }
@@ -502,7 +520,7 @@ __device__ __forceinline__ void flush_run_substreams(const SpectraArgs &a, const
         }
     }
 #pragma unroll
-    for (int k = 0; k < S; ++k) r.C[k] = 0.0;
+    for (int k = 0; k < S; ++k) { r.C[k] = 0.0; r.odd[k] = 0; }
     r.W = 0.0;
 }
 
@@ -535,6 +553,10 @@ __device__ __forceinline__ void walk_inside(const SpectraArgs &a, const DatasetD
                                             const typename RecOf<UW>::type *bp, int gb, const double (&h)[S], int p,
                                             bool active, Run<S> &r)
 {
+    unsigned parity[S];                             /* unit weights: parity bits of this stretch's events, per term */
+#pragma unroll
+    for (int k = 0; k < S; ++k) parity[k] = 0u;
+    static_assert(EB * K <= 32, "one parity register per term and stretch");
 #pragma unroll
     for (int u = 0; u < K; ++u) {
         const double2 *q = reinterpret_cast<const double2 *>(bp + u);
@@ -543,11 +565,17 @@ __device__ __forceinline__ void walk_inside(const SpectraArgs &a, const DatasetD
             const double2 t = q[j];
             if (UW) {
                 /* every weight of the dataset is exactly 1 (the padding sits behind a NaN E_vis and never
-                 * reaches this path): 1 * g + C == g + C bit for bit, and no weight is stored */
+                 * reaches this path): no weight is stored, and the run sum takes the accumulating form */
 #pragma unroll
-                for (int k = 0; k < S; ++k) r.C[k] += half_cos_term<S, SM>(k, h[k], t.x);
+                for (int k = 0; k < S; ++k) {
+                    if (folded<S>(SM, k)) half_cos_term_accumulate<S, SM>(k, h[k], t.x, r.C[k], parity[k]);
+                    else                  r.C[k] += half_cos_halfturns(h[k], t.x);      /* 1 * g + C == g + C bit for bit */
+                }
 #pragma unroll
-                for (int k = 0; k < S; ++k) r.C[k] += half_cos_term<S, SM>(k, h[k], t.y);
+                for (int k = 0; k < S; ++k) {
+                    if (folded<S>(SM, k)) half_cos_term_accumulate<S, SM>(k, h[k], t.y, r.C[k], parity[k]);
+                    else                  r.C[k] += half_cos_halfturns(h[k], t.y);
+                }
             } else {
                 const double2 w = q[EB / 2 + j];
 #pragma unroll
@@ -560,7 +588,12 @@ __device__ __forceinline__ void walk_inside(const SpectraArgs &a, const DatasetD
         if (DBG)
             for (int j = 0; j < EB; ++j) dbg_mark<DBG>(a, ds, p, active, gb + u, j, r.cur);
     }
-    if (UW) r.W += (double)(EB * K);                /* whole numbers: the same bits as K separate adds */
+    if (UW) {
+        r.W += (double)(EB * K);                    /* whole numbers: the same bits as K separate adds */
+#pragma unroll
+        for (int k = 0; k < S; ++k)
+            if (folded<S>(SM, k) && !(SM && k == S - 1)) r.odd[k] += __popc(parity[k]);
+    }
 }
 
 /* the half-turn coefficients of the lane's point, by value (they travel to the non-inlined slow path) */
@@ -606,9 +639,18 @@ __device__ __noinline__ Run<S> walk_batch_slow(const SpectraArgs &a, Tables T, c
         if (!UW) w = reinterpret_cast<const EventBatchW *>(bp)->w[j];
 #pragma unroll
         for (int k = 0; k < S; ++k) {
-            const double g = half_cos_halfturns(c.h[k], x);
-            if (UW) { if (!pad) r.C[k] += g; }          /* 1 * g + C == g + C bit for bit */
-            else    r.C[k] = fma(w, g, r.C[k]);
+            if (UW) {
+                if (pad) continue;
+                if (folded<S>(r.sm, k)) {               /* the accumulating form of walk_inside, one event at a time */
+                    unsigned parity = 0u;
+                    half_cos_accumulate(c.h[k], x, r.C[k], parity);
+                    r.odd[k] += (int)(parity >> 31);
+                } else {
+                    r.C[k] += half_cos_halfturns(c.h[k], x);
+                }
+            } else {
+                r.C[k] = fma(w, half_cos_halfturns(c.h[k], x), r.C[k]);
+            }
         }
         if (UW) { if (!pad) r.W += 1.0; }
         else    r.W += w;
@@ -717,6 +759,7 @@ __device__ __forceinline__ void walk_unit(const SpectraArgs &a, const Tables &T,
 #endif
     Run<S> r;
     run_reset<S>(r);
+    r.sm = T.small[g * a.n_datasets + d] != 0;
     PHYLINO_ASSERT(my0 >= 0 && mine >= 0 && my0 + mine <= nb && p >= 0 && p < a.P);
     PHYLINO_ASSERT(row >= 0 && row < a.thr_rows);
     const Rec *bp = static_cast<const Rec *>(unit) + my0;
@@ -725,7 +768,7 @@ __device__ __forceinline__ void walk_unit(const SpectraArgs &a, const Tables &T,
     const long long q1 = clock64();
 #endif
     /* the last term's phase stays small over this dataset for every point of the group: its cheap form */
-    if (T.small[g * a.n_datasets + d]) walk_stretch<S, UW, DBG, true>(a, T, ds, bp, b0 + my0, mine, h, thr, safe, p, active, r);
+    if (r.sm) walk_stretch<S, UW, DBG, true>(a, T, ds, bp, b0 + my0, mine, h, thr, safe, p, active, r);
     else                               walk_stretch<S, UW, DBG, false>(a, T, ds, bp, b0 + my0, mine, h, thr, safe, p, active, r);
 #ifdef PHYLINO_TRACE
     const long long q2 = clock64();
