@@ -52,6 +52,9 @@ def fp64_per_general_term(S: int) -> int:
 # half_cos_small_accumulate); the library reports the fraction of event x point evaluations that took it
 # (phylino_last_small_phase), the roofline counts what ran
 FP64_SMALL_TERM = 6
+# ... and 8 for the FIRST term where its phase cannot wrap for any event of a work item and any point of the group (no
+# range reduction, no sign: devmath.cuh half_cos_medium_accumulate; phylino_last_medium_phase reports the fraction)
+FP64_MEDIUM_TERM = 8
 # nominal fp64 pipe, derived in DESIGN.md section 7 (the guide has no fp64 row): 64 fp64 lanes/clk/SM (one DFMA
 # per lane and clock) x SMs x the SM clock nvidia-smi reports as maximum
 FP64_LANES_PER_SM = 64
@@ -235,6 +238,7 @@ def measure(pkg, torch, dist, k, steps, warmup, local, rank, world, flush, tunin
         flush.zero_()
     torch.cuda.synchronize()
     small_frac = ph.last_small_phase()
+    medium_frac = ph.last_medium_phase()
     clocks = sampler.stop() if sampler else None
     barrier()
     if world > 1:
@@ -299,7 +303,8 @@ def measure(pkg, torch, dist, k, steps, warmup, local, rank, world, flush, tunin
     res = None
     if rank == 0:
         inst_general = fp64_inst_per_evpt(wl.model)
-        inst = inst_general - (fp64_per_general_term(n_terms(wl.model)) - FP64_SMALL_TERM) * small_frac   # executed
+        gen = fp64_per_general_term(n_terms(wl.model))
+        inst = inst_general - (gen - FP64_SMALL_TERM) * small_frac - (gen - FP64_MEDIUM_TERM) * medium_frac   # executed
         small = P <= 16 and not (n_terms(wl.model) == 3 and P > 4)      # the small-batch kernel (setup fused in) ran
         sp = stats_ms(sp_ms)
         sm_max_mhz = (clocks or {}).get("sm_max_mhz") or 1965.0
@@ -318,7 +323,7 @@ def measure(pkg, torch, dist, k, steps, warmup, local, rank, world, flush, tunin
             "frac_of_measured_dfma_peak": None if not measured_peak else achieved / measured_peak,
             "traffic": traffic, "traffic_source": traffic_source,
             "fp64_inst_per_event_point": inst, "fp64_inst_general_form": inst_general,
-            "small_phase_fraction": small_frac, "kernel_ms": sp["mean"], "kernel_ms_median": sp["median"],
+            "small_phase_fraction": small_frac, "medium_phase_fraction": medium_frac, "kernel_ms": sp["mean"], "kernel_ms_median": sp["median"],
             "kernel_ms_min": sp["min"],
             "kernel_share_of_step": sp["mean"] / (sum(inst_ms) / steps),
             "kernel_timing": f"second pass of {steps} steps with CUDA events around each kernel on the library's "

@@ -339,6 +339,11 @@ PHYLINO_API phylino_status phylino_last_kernel_ms(phylino_ctx *ctx, float *ms);
  * per group of 32 points and dataset where |1.267 dm2 (2/pi) L/E| <= 1/8 for every event and point (the solar term
  * at Double-Chooz baselines).  fraction HOST; synchronises the stream. */
 PHYLINO_API phylino_status phylino_last_small_phase(phylino_ctx *ctx, double *fraction_host);
+/* fraction_host (HOST, out): share of the event x point evaluations of the last spectra launch on this context whose
+ * FIRST term took the no-reduction form (its phase stayed within half a half-turn for every event of a work item and
+ * every point of the group: DESIGN.md section 6.1; bit-identical results, fewer instructions).  With cross-point
+ * caching on the count is over virtual points.  Synchronises the stream. */
+PHYLINO_API phylino_status phylino_last_medium_phase(phylino_ctx *ctx, double *fraction_host);
 
 /* Kernel launches enqueued by this context so far (bench.py's `gpu_launches`). */
 PHYLINO_API int64_t phylino_launch_count(const phylino_ctx *ctx);

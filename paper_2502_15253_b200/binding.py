@@ -27,7 +27,7 @@ abi_symbols = (
     "phylino_launch_floor", "phylino_set_schedule", "phylino_reserve",
     "phylino_draw_pseudo_data", "phylino_ordering_scan", "phylino_nll_gradient",
     "phylino_set_energy_correction_mode", "phylino_set_flux_model", "phylino_last_small_phase",
-    "phylino_hbm_read_floor",
+    "phylino_hbm_read_floor", "phylino_last_medium_phase",
 )
 
 _STATUS = {0: "OK", 1: "ERR_ARG", 2: "ERR_SHAPE", 3: "ERR_STATE", 4: "ERR_OOM", 5: "ERR_CUDA"}
@@ -137,6 +137,8 @@ def load_library():
     lib.phylino_set_flux_model.argtypes = [vp, i32, i32, vp, dbl, dbl]
     lib.phylino_last_small_phase.restype = i32
     lib.phylino_last_small_phase.argtypes = [vp, C.POINTER(dbl)]
+    lib.phylino_last_medium_phase.restype = i32
+    lib.phylino_last_medium_phase.argtypes = [vp, C.POINTER(dbl)]
     lib.phylino_set_schedule.restype = i32
     lib.phylino_set_schedule.argtypes = [vp, i32]
     lib.phylino_reserve.restype = i32
@@ -466,8 +468,14 @@ class Phylino:
         self._check(self._lib.phylino_last_plan(self._ctx, C.byref(v), C.byref(c)))
         return int(v.value), int(c.value)
 
+    def last_medium_phase(self) -> float:
+        """fraction of the last call's event x point evaluations whose first term took the no-reduction form"""
+        v = C.c_double(0.0)
+        self._check(self._lib.phylino_last_medium_phase(self._ctx, C.byref(v)))
+        return float(v.value)
+
     def last_small_phase(self) -> float:
-        """fraction of the last call's event x point evaluations whose last term took the 7-instruction form"""
+        """fraction of the last call's event x point evaluations whose last term took the small-phase form"""
         v = C.c_double(0.0)
         self._check(self._lib.phylino_last_small_phase(self._ctx, C.byref(v)))
         return float(v.value)

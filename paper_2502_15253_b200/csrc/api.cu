@@ -101,9 +101,9 @@ void free_all(phylino_ctx *c)
     free_tables(c);
     cudaFree(c->d_acc); cudaFree(c->d_flags);
     c->d_acc = nullptr; c->d_flags = nullptr; c->acc_capacity = 0;
-    cudaFree(c->d_rec); cudaFree(c->d_thr); cudaFree(c->d_safe); cudaFree(c->d_counter); cudaFree(c->d_done);
+    cudaFree(c->d_rec); cudaFree(c->d_thr); cudaFree(c->d_safe); cudaFree(c->d_counter); cudaFree(c->d_done); cudaFree(c->d_med);
     cudaFree(c->d_small);
-    c->d_rec = nullptr; c->d_thr = nullptr; c->d_safe = nullptr; c->d_counter = nullptr; c->d_done = nullptr;
+    c->d_rec = nullptr; c->d_thr = nullptr; c->d_safe = nullptr; c->d_counter = nullptr; c->d_done = nullptr; c->d_med = nullptr;
     c->d_small = nullptr;
     c->point_capacity = 0;
     cudaFree(c->d_plan); c->d_plan = nullptr; c->plan_capacity = 0;
@@ -161,6 +161,10 @@ phylino_status ensure_acc(phylino_ctx *ctx, int P)
         CU(cudaMalloc((void **)&ctx->d_done, sizeof(unsigned)));
         CU(cudaMemsetAsync(ctx->d_done, 0, sizeof(unsigned), ctx->stream));
     }
+    if (!ctx->d_med) {
+        CU(cudaMalloc((void **)&ctx->d_med, sizeof(unsigned long long)));
+        CU(cudaMemsetAsync(ctx->d_med, 0, sizeof(unsigned long long), ctx->stream));
+    }
     if (P > ctx->point_capacity) {
         /* per-point records and threshold rows written by the setup kernel of every call */
         CU(cudaStreamSynchronize(ctx->stream));
@@ -214,6 +218,7 @@ void fill_datasets(const phylino_ctx *ctx, SpectraArgs &a)
     a.flags = ctx->d_flags;
     a.counter = ctx->d_counter;
     a.done = ctx->d_done;
+    a.med_count = ctx->d_med;
 }
 
 /* Cut of the batch into work items (spectra.cu): U batches per unit, G point groups per item.
@@ -354,6 +359,7 @@ phylino_status enqueue_eval(phylino_ctx *ctx, int P, const double *params, const
     if (s != PHYLINO_OK) return s;
     const bool dbg = bins != nullptr;
     ctx->last_points = P;
+    ctx->last_fused = a.sched == 1;
     a.dbg_bins = bins;
     a.total_events = phylino_total_events(ctx);
     FinalizeArgs f = ctx->fin;
@@ -631,6 +637,7 @@ phylino_status enqueue_cached(phylino_ctx *ctx, int P, const double *h_params, c
     a.comp = 1;
     if ((s = fill_batch(ctx, a, V, d_params, pl.C)) != PHYLINO_OK) return s;
     ctx->last_points = V;
+    ctx->last_fused = a.sched == 1;
     a.vp_class = ctx->d_plan;
     a.vp_src = ctx->d_plan + V;
     a.class_rep = ctx->d_plan + V + (int64_t)V * S;
@@ -907,7 +914,8 @@ phylino_status phylino_load_events(phylino_ctx *ctx, int dataset, int64_t n, con
     }
     /* where a lane starts looking for its bin (a hint, never trusted): the bin of the first event of every
      * HINT_BATCHES-th batch under the identity energy scale */
-    std::vector<int32_t> hint((size_t)((n_batches + HINT_BATCHES - 1) / HINT_BATCHES), n_bins);
+    std::vector<HintEntry> hint((size_t)((n_batches + HINT_BATCHES - 1) / HINT_BATCHES), HintEntry{n_bins, 0.0f});
+    std::vector<double> x_blk(hint.size(), 0.0);       /* largest L/E_nu of each block of HINT_BATCHES batches */
     double x_max = 0.0;
     for (int64_t i = 0; i < n; ++i) {
         const int32_t s = perm[i];
@@ -916,6 +924,7 @@ phylino_status phylino_load_events(phylino_ctx *ctx, int dataset, int64_t n, con
         const float vi = e_vis[s];
         const double xi = baseline_m[core ? core[s] : 0] / (double)e_nu[s];
         x_max = std::max(x_max, xi);
+        x_blk[(size_t)(b / HINT_BATCHES)] = std::max(x_blk[(size_t)(b / HINT_BATCHES)], xi);
         if (unit_w) {
             ev_u[(size_t)b].x[j] = xi;
             ev_u[(size_t)b].v[j] = vi;
@@ -927,8 +936,19 @@ phylino_status phylino_load_events(phylino_ctx *ctx, int dataset, int64_t n, con
             r.wsum += r.w[j];                   /* in event order: the batch total the hot kernel adds */
         }
         if (j == 0 && b % HINT_BATCHES == 0)
-            hint[(size_t)(b / HINT_BATCHES)] =
+            hint[(size_t)(b / HINT_BATCHES)].bin =
                 vi == vi ? (int32_t)(std::upper_bound(edges, edges + n_bins + 1, (double)vi) - edges) - 1 : n_bins;
+    }
+    /* envelope of L/E_nu from a block to the end of the store, as a float rounded up: the store is sorted by E_vis, and
+     * L/E_nu falls with it, so the envelope stays close to the block's own largest value */
+    {
+        double env = 0.0;
+        for (size_t i = hint.size(); i-- > 0;) {
+            env = std::max(env, x_blk[i]);
+            float f = (float)env;
+            if ((double)f < env) f = std::nextafter(f, INFINITY);
+            hint[i].x_env = f;
+        }
     }
     /* fixed-point scale 2^e with 8 * sum|w| * 2^e <= 2^62 (|P_ee| <= 4 is enforced per point) */
     int ex = 0;
@@ -1424,6 +1444,22 @@ phylino_status phylino_last_small_phase(phylino_ctx *ctx, double *fraction_host)
         }
     }
     *fraction_host = total > 0.0 ? small / total : 0.0;
+    return PHYLINO_OK;
+}
+
+phylino_status phylino_last_medium_phase(phylino_ctx *ctx, double *fraction_host)
+{
+    if (!ctx || !fraction_host) return PHYLINO_ERR_ARG;
+    *fraction_host = 0.0;
+    const int P = ctx->last_points;
+    if (!ctx->have_model || P <= 0 || !ctx->d_med || ctx->last_fused) return PHYLINO_OK;   /* the single-launch kernel has no such form */
+    DeviceGuard g(ctx->device);
+    unsigned long long n = 0;
+    CU(cudaMemcpyAsync(&n, ctx->d_med, sizeof n, cudaMemcpyDeviceToHost, ctx->stream));
+    CU(cudaStreamSynchronize(ctx->stream));
+    double total = 0.0;
+    for (int d = 0; d < ctx->n_datasets; ++d) total += (double)ctx->ds[d].n_pad * P;
+    *fraction_host = total > 0.0 ? std::min(1.0, (double)n / total) : 0.0;
     return PHYLINO_OK;
 }
 

@@ -173,10 +173,31 @@ __device__ __forceinline__ void half_cos_small_accumulate(double h, double x, do
     C = fma(q, z, C);
 }
 
-template <int S, bool SM>
+/* ... and where |h x| <= MEDIUM_PHASE = 1/2 for every event a lane meets in a work item: n = 0, f = h x exactly as the
+ * general form computes it (fma(h, x, -0) is the rounded product), so the range reduction and the sign drop out and
+ * the result is BIT-IDENTICAL to the general form: 8 fp64 instructions, no integer one.  That is the first term
+ * (dm2_ee) at a near detector (1.267 x 2.5e-3 x 469 m / 1.9 MeV = 0.78 rad = 0.5 half-turns) and above 4 - 4.5 MeV at
+ * the far one; decided per work item and group from the load-time envelope of L/E (HintEntry::x_env). */
+constexpr double MEDIUM_PHASE = 0.5;
+__device__ __forceinline__ void half_cos_medium_accumulate(double h, double x, double &C)
+{
+    const double f = h * x;
+    const double z = f * f;
+    double q =  0x1.e2a4cab0973aep-11;
+    q = fma(q, z, -0x1.a65598e5b8576p-7);
+    q = fma(q, z,  0x1.e1f273f3e9df0p-4);
+    q = fma(q, z, -0x1.55d3c0fdef250p-1);
+    q = fma(q, z,  0x1.03c1f070b1413p+1);
+    q = fma(q, z, -0x1.3bd3cc9bac6fep+1);
+    C = fma(q, z, C);
+}
+
+/* term k of S in accumulating form: SM: the last term is small; MED: the first term never wraps */
+template <int S, bool SM, bool MED>
 __device__ __forceinline__ void half_cos_term_accumulate(int k, double h, double x, double &C, unsigned &parity)
 {
     if (SM && k == S - 1) half_cos_small_accumulate(h, x, C);
+    else if (MED && k == 0) half_cos_medium_accumulate(h, x, C);
     else                  half_cos_accumulate(h, x, C, parity);
 }
 

@@ -61,13 +61,20 @@ static_assert(sizeof(EventBatchW) == 96 && sizeof(EventBatchU) == 48, "records a
 template <bool UW> struct RecOf { typedef EventBatchW type; };
 template <> struct RecOf<true> { typedef EventBatchU type; };
 
+/* One entry per HINT_BATCHES batches of a dataset's store, read once per work item and lane. */
+struct HintEntry {
+    int32_t bin;            /* bin of the first event of batch HINT_BATCHES i under the identity energy scale (-1 below the
+                               first edge, n_bins above the last / NaN): where a lane starts looking for its bin, never
+                               trusted */
+    float   x_env;          /* >= L/E_nu of every event of the batches HINT_BATCHES i, ... to the end of the dataset
+                               (rounded up): decides per item whether the first term's phase can wrap at all */
+};
+
 /* Per-dataset entry of the table that travels by value in the kernel parameters. */
 struct DatasetDev {
     const void *ev;         /* [n_batches] EventBatchU if unit_w else EventBatchW */
     const double *edges;    /* [n_bins+1] */
-    const int32_t *hint;    /* [ceil(n_batches / HINT_BATCHES)] bin of the first event of batch HINT_BATCHES i under the
-                               identity energy scale (-1 below the first edge, n_bins above the last / NaN): where a
-                               lane starts looking for its bin, never trusted */
+    const HintEntry *hint;  /* [ceil(n_batches / HINT_BATCHES)] */
     const int32_t *perm;    /* [n] caller's index of sorted event i (diagnostic instantiation only) */
     long long ev_off;       /* events of the datasets before this one (diagnostic instantiation only) */
     int32_t n_events;       /* events before padding */
@@ -114,6 +121,8 @@ struct SpectraArgs {
     int32_t sched;          /* 0: items claimed from the counter; 1: one contiguous range of batches per warp, single launch */
     unsigned *counter;      /* DEVICE work counter of the ticket kernel; the setup kernel zeroes it */
     unsigned *done;         /* DEVICE work counter of the single-launch kernel; the finalize kernel behind it zeroes it */
+    unsigned long long *med_count;  /* DEVICE event x point evaluations whose first term took the no-reduction form
+                                       (phylino_last_medium_phase); the setup kernel zeroes it */
     int32_t  *dbg_bins;     /* DEVICE [P x total_events] diagnostic instantiation: bin the hot loop gave every event */
     long long total_events;
     int32_t thr_stride;     /* floats per threshold row: total_bins + n_datasets */
@@ -241,7 +250,7 @@ struct phylino_dataset_host {
     int      fx_exp = 0;
     double   x_max = 0.0;
     void    *d_ev = nullptr;                        /* EventBatchU[] if unit_w else EventBatchW[] */
-    int32_t *d_hint = nullptr;
+    phylino::HintEntry *d_hint = nullptr;
     double  *d_edges = nullptr;
     int32_t *d_perm = nullptr;
 };
@@ -304,6 +313,8 @@ struct phylino_ctx {
     size_t fused_tables = 0;
     int schedule = 0;                              /* phylino_set_schedule: 0 auto, 1 tickets, 2 single launch */
     unsigned *d_done = nullptr;                    /* work counter of the small-batch kernel */
+    unsigned long long *d_med = nullptr;           /* medium-phase evaluations of the last ticket launch */
+    bool last_fused = false;                       /* the last spectra launch was the single-launch kernel */
     phylino::ParamBlob blob{};                     /* a small host batch on its way into the kernel arguments */
     /* optional device timing of the three kernels of a call (phylino_set_timing) */
     bool timing = false;

@@ -332,7 +332,10 @@ __global__ void __launch_bounds__(SETUP_THREADS) setup_kernel(const __grid_const
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     if ((int)blockIdx.x < rec_blocks) {
         const int p = blockIdx.x * SETUP_THREADS + threadIdx.x;
-        if (p == 0) *a.counter = 0u;                            /* the work counter of ticket_loop */
+        if (p == 0) {
+            *a.counter = 0u;                                    /* the work counter of ticket_loop */
+            *a.med_count = 0ull;                                /* phylino_last_medium_phase */
+        }
         const double h_last = p < a.P ? point_record<S>(a, a.params, p, a.rec) : 0.0;
         group_flags(a, h_last, a.small + (size_t)(p >> 5) * a.n_datasets);      /* SETUP_THREADS is a multiple of 32 */
         return;
@@ -347,8 +350,11 @@ __global__ void __launch_bounds__(SETUP_THREADS) setup_kernel(const __grid_const
 template <int S> struct Run {
     double C[S];    /* sum of w g_k over the run; a FOLDED term (see folded()) holds only its oscillating part C'
                      * (devmath.cuh, half_cos_accumulate), the rest is 1/2 W - odd[k] */
-    int    odd[S];  /* folded terms: events of the run whose half-turn count n_k is odd */
+    int    odd[S];  /* folded GENERAL terms (two-term model only): events of the run whose half-turn count n_k is odd;
+                     * the small-phase and the no-reduction form have n = 0, so three-term models never touch it */
     bool   sm;      /* the run's last term takes the small-phase form (fixed per group and dataset) */
+    bool   med;     /* the run's first term takes the no-reduction form (fixed per work item and group) */
+    bool   fo;      /* the kernel folds at all (the large-batch kernel does, the single-launch one does not) */
     double W;       /* sum of w over the run */
     int    cur;     /* its bin; < 0 or >= n_bins: events that land in no bin (never flushed) */
     float  hi;      /* later events below hi stay in the run (-inf: re-locate at the next event) */
@@ -365,20 +371,27 @@ template <int S> __device__ __forceinline__ void run_reset(Run<S> &r)
     r.hi = -pos_inf();
     r.hi2 = pos_inf();
     r.sm = false;
+    r.med = false;
+    r.fo = false;
 }
 
 /* Which terms of a UNIT-WEIGHT run are accumulated in the folded form (devmath.cuh, half_cos_accumulate): the
  * small-phase last term always (no sign, so the fold costs nothing: 6 fp64 instructions instead of 7); the general
  * terms of the two-term model (10 + 2 integer instead of 11 + 1: config 3 +4 %).  Not the general terms of the
  * three-term models: measured in round 2, config 4 lost 5.6 % (128 registers, fp64 pipe 91.7 -> 78.8 % busy, top stall
- * "wait": the two extra integer instructions per term sit in the dependency chains of three terms at once). */
-template <int S> __device__ __forceinline__ bool folded(bool sm, int k) { return S == 2 || (sm && k == S - 1); }
+ * "wait": the two extra integer instructions per term sit in the dependency chains of three terms at once).
+ * Not in the single-launch kernel for at most 16 points either (fo = false): that call is bound by latency and by the
+ * instruction lines it has to fetch, not by the fp64 pipe, and was 3 us slower per call with the folded flush. */
+template <int S> __device__ __forceinline__ bool folded(bool fo, bool sm, bool med, int k)
+{
+    return fo && (S == 2 || (sm && k == S - 1) || (med && k == 0));     /* the no-reduction form has no sign either */
+}
 
 /* sum of w g_k over the run, whichever way it was accumulated */
 template <int S>
 __device__ __forceinline__ double run_sum(const DatasetDev &ds, const Run<S> &r, int k)
 {
-    return (ds.unit_w && folded<S>(r.sm, k)) ? r.C[k] + (0.5 * r.W - (double)r.odd[k]) : r.C[k];
+    return (ds.unit_w && folded<S>(r.fo, r.sm, r.med, k)) ? r.C[k] + (0.5 * r.W - (S == 2 ? (double)r.odd[k] : 0.0)) : r.C[k];
 }
 
 /* diagnostic instantiation: the bin the hot loop gave event j of dataset batch gb at point p */
@@ -548,7 +561,7 @@ __device__ __forceinline__ void open_run(const DatasetDev &ds, const float *thr,
 
 /* K consecutive batches known to lie inside the lane's open run (the store is sorted: the last
  * event of the last batch is below r.hi): rows a2 + a4 only, straight-line. */
-template <int S, bool UW, int K, bool DBG, bool SM>
+template <int S, bool UW, int K, bool DBG, bool SM, bool MED, bool FO>
 __device__ __forceinline__ void walk_inside(const SpectraArgs &a, const DatasetDev &ds,
                                             const typename RecOf<UW>::type *bp, int gb, const double (&h)[S], int p,
                                             bool active, Run<S> &r)
@@ -568,13 +581,13 @@ __device__ __forceinline__ void walk_inside(const SpectraArgs &a, const DatasetD
                  * reaches this path): no weight is stored, and the run sum takes the accumulating form */
 #pragma unroll
                 for (int k = 0; k < S; ++k) {
-                    if (folded<S>(SM, k)) half_cos_term_accumulate<S, SM>(k, h[k], t.x, r.C[k], parity[k]);
-                    else                  r.C[k] += half_cos_halfturns(h[k], t.x);      /* 1 * g + C == g + C bit for bit */
+                    if (folded<S>(FO, SM, MED, k)) half_cos_term_accumulate<S, SM, MED>(k, h[k], t.x, r.C[k], parity[k]);
+                    else                       r.C[k] += half_cos_term<S, SM>(k, h[k], t.x);    /* 1 * g + C == g + C bit for bit */
                 }
 #pragma unroll
                 for (int k = 0; k < S; ++k) {
-                    if (folded<S>(SM, k)) half_cos_term_accumulate<S, SM>(k, h[k], t.y, r.C[k], parity[k]);
-                    else                  r.C[k] += half_cos_halfturns(h[k], t.y);
+                    if (folded<S>(FO, SM, MED, k)) half_cos_term_accumulate<S, SM, MED>(k, h[k], t.y, r.C[k], parity[k]);
+                    else                       r.C[k] += half_cos_term<S, SM>(k, h[k], t.y);
                 }
             } else {
                 const double2 w = q[EB / 2 + j];
@@ -592,7 +605,7 @@ __device__ __forceinline__ void walk_inside(const SpectraArgs &a, const DatasetD
         r.W += (double)(EB * K);                    /* whole numbers: the same bits as K separate adds */
 #pragma unroll
         for (int k = 0; k < S; ++k)
-            if (folded<S>(SM, k) && !(SM && k == S - 1)) r.odd[k] += __popc(parity[k]);
+            if (FO && S == 2 && !(SM && k == S - 1) && !(MED && k == 0)) r.odd[k] += __popc(parity[k]);
     }
 }
 
@@ -641,10 +654,10 @@ __device__ __noinline__ Run<S> walk_batch_slow(const SpectraArgs &a, Tables T, c
         for (int k = 0; k < S; ++k) {
             if (UW) {
                 if (pad) continue;
-                if (folded<S>(r.sm, k)) {               /* the accumulating form of walk_inside, one event at a time */
-                    unsigned parity = 0u;
+                if (folded<S>(r.fo, r.sm, r.med, k)) {        /* the accumulating form of walk_inside, one event at a time */
+                    unsigned parity = 0u;               /* (n = 0 wherever a three-term model folds a term) */
                     half_cos_accumulate(c.h[k], x, r.C[k], parity);
-                    r.odd[k] += (int)(parity >> 31);
+                    if (S == 2) r.odd[k] += (int)(parity >> 31);
                 } else {
                     r.C[k] += half_cos_halfturns(c.h[k], x);
                 }
@@ -660,7 +673,7 @@ __device__ __noinline__ Run<S> walk_batch_slow(const SpectraArgs &a, Tables T, c
 }
 
 /* One batch of the lane's stream (rows a2-a4); gb: its index in the dataset. */
-template <int S, bool UW, bool DBG, bool SM>
+template <int S, bool UW, bool DBG, bool SM, bool MED, bool FO>
 __device__ __forceinline__ void walk_batch(const SpectraArgs &a, const Tables &T, const DatasetDev &ds,
                                            const typename RecOf<UW>::type *bp, int gb, const double (&h)[S],
                                            const float *thr, float2 safe, int p, bool active, Run<S> &r)
@@ -668,7 +681,7 @@ __device__ __forceinline__ void walk_batch(const SpectraArgs &a, const Tables &T
     if (bp->v[EB - 1] < r.hi) {
         /* rows a3 + a4: the store is sorted, so the whole batch lies in the run's bin (a padding event has
          * E_vis = NaN and fails the test: it never comes here) */
-        walk_inside<S, UW, 1, DBG, SM>(a, ds, bp, gb, h, p, active, r);
+        walk_inside<S, UW, 1, DBG, SM, MED, FO>(a, ds, bp, gb, h, p, active, r);
     } else {
         Coef<S> c;
 #pragma unroll
@@ -678,7 +691,7 @@ __device__ __forceinline__ void walk_batch(const SpectraArgs &a, const Tables &T
 }
 
 /* `mine` consecutive batches of the lane's stream starting at bp (dataset batch gb): 4, 2 or 1 at a time */
-template <int S, bool UW, bool DBG, bool SM>
+template <int S, bool UW, bool DBG, bool SM, bool MED, bool FO>
 __device__ __forceinline__ void walk_stretch(const SpectraArgs &a, const Tables &T, const DatasetDev &ds,
                                              const typename RecOf<UW>::type *bp, int gb, int mine, const double (&h)[S],
                                              const float *thr, float2 safe, int p, bool active, Run<S> &r)
@@ -687,15 +700,15 @@ __device__ __forceinline__ void walk_stretch(const SpectraArgs &a, const Tables 
 #pragma unroll 1
     while (i < mine) {
         if (i + 4 <= mine && bp[3].v[EB - 1] < r.hi) {
-            walk_inside<S, UW, 4, DBG, SM>(a, ds, bp, gb + i, h, p, active, r);
+            walk_inside<S, UW, 4, DBG, SM, MED, FO>(a, ds, bp, gb + i, h, p, active, r);
             i += 4;
             bp += 4;
         } else if (i + 2 <= mine && bp[1].v[EB - 1] < r.hi) {
-            walk_inside<S, UW, 2, DBG, SM>(a, ds, bp, gb + i, h, p, active, r);
+            walk_inside<S, UW, 2, DBG, SM, MED, FO>(a, ds, bp, gb + i, h, p, active, r);
             i += 2;
             bp += 2;
         } else {
-            walk_batch<S, UW, DBG, SM>(a, T, ds, bp, gb + i, h, thr, safe, p, active, r);
+            walk_batch<S, UW, DBG, SM, MED, FO>(a, T, ds, bp, gb + i, h, thr, safe, p, active, r);
             ++i;
             ++bp;
         }
@@ -717,7 +730,7 @@ __device__ __forceinline__ void substream_of(int np, int lane, int nb, int &lg, 
 
 /* the hint a lane needs to open its run in unit [b0, b0 + nb) of dataset ds (group of np points; np > 16: all
  * lanes start at b0) */
-__device__ __forceinline__ int load_hint(const DatasetDev &ds, int np, int lane, int b0, int nb)
+__device__ __forceinline__ HintEntry load_hint(const DatasetDev &ds, int np, int lane, int b0, int nb)
 {
     int my0 = 0;
     if (np <= 16) {
@@ -725,15 +738,19 @@ __device__ __forceinline__ int load_hint(const DatasetDev &ds, int np, int lane,
         substream_of(np, lane, nb, lg, pl, my0, mine);
     }
     PHYLINO_ASSERT(b0 + my0 >= 0 && (b0 + my0 < ds.n_batches || (nb == 0 && b0 + my0 <= ds.n_batches)));
-    return __ldg(ds.hint + (b0 + my0) / HINT_BATCHES);
+    const int2 e = __ldg(reinterpret_cast<const int2 *>(ds.hint + (b0 + my0) / HINT_BATCHES));
+    HintEntry he;
+    he.bin = e.x;
+    he.x_env = __int_as_float(e.y);
+    return he;
 }
 
 /* One warp, the nb batches [b0, b0 + nb) of dataset ds staged at `unit` (SHARED memory), point group g
  * (points 32 g ... 32 g + 31).  FULL: the group has more than 16 points, every lane walks all batches; lanes past
  * the last point shadow point 32 g and never flush.  hint: load_hint() of this lane for this unit and group. */
-template <int S, bool FULL, bool UW, bool DBG>
+template <int S, bool FULL, bool UW, bool DBG, bool FO>
 __device__ __forceinline__ void walk_unit(const SpectraArgs &a, const Tables &T, const DatasetDev &ds, int d,
-                                          const void *unit, int b0, int nb, int g, int lane, int hint)
+                                          const void *unit, int b0, int nb, int g, int lane, HintEntry hint)
 {
     typedef typename RecOf<UW>::type Rec;
     int my0 = 0, mine = nb, lg = 5;
@@ -760,16 +777,27 @@ __device__ __forceinline__ void walk_unit(const SpectraArgs &a, const Tables &T,
     Run<S> r;
     run_reset<S>(r);
     r.sm = T.small[g * a.n_datasets + d] != 0;
+    r.fo = FO;
     PHYLINO_ASSERT(my0 >= 0 && mine >= 0 && my0 + mine <= nb && p >= 0 && p < a.P);
     PHYLINO_ASSERT(row >= 0 && row < a.thr_rows);
     const Rec *bp = static_cast<const Rec *>(unit) + my0;
-    if (mine > 0) open_run<S>(ds, thr, safe, bp->v[0], hint, r);
+    if (mine > 0) open_run<S>(ds, thr, safe, bp->v[0], hint.bin, r);
 #ifdef PHYLINO_TRACE
     const long long q1 = clock64();
 #endif
     /* the last term's phase stays small over this dataset for every point of the group: its cheap form */
-    if (r.sm) walk_stretch<S, UW, DBG, true>(a, T, ds, bp, b0 + my0, mine, h, thr, safe, p, active, r);
-    else                               walk_stretch<S, UW, DBG, false>(a, T, ds, bp, b0 + my0, mine, h, thr, safe, p, active, r);
+    /* the first term's phase cannot wrap for any event this lane meets in this item (unit-weight stores only: the
+     * weighted ones keep the one form; neither does the single-launch kernel); a NaN coefficient compares false */
+    constexpr bool ME = UW && FO;
+    r.med = ME && __all_sync(0xffffffffu, fabs(h[0]) * (double)hint.x_env <= MEDIUM_PHASE);
+    if (ME && r.med) {
+        if (lane == 0) atomicAdd(a.med_count, (unsigned long long)nb * EB * (unsigned)min(32, a.P - 32 * g));
+        if (r.sm) walk_stretch<S, UW, DBG, true, ME, FO>(a, T, ds, bp, b0 + my0, mine, h, thr, safe, p, active, r);
+        else      walk_stretch<S, UW, DBG, false, ME, FO>(a, T, ds, bp, b0 + my0, mine, h, thr, safe, p, active, r);
+    } else {
+        if (r.sm) walk_stretch<S, UW, DBG, true, false, FO>(a, T, ds, bp, b0 + my0, mine, h, thr, safe, p, active, r);
+        else      walk_stretch<S, UW, DBG, false, false, FO>(a, T, ds, bp, b0 + my0, mine, h, thr, safe, p, active, r);
+    }
 #ifdef PHYLINO_TRACE
     const long long q2 = clock64();
 #endif
@@ -845,7 +873,7 @@ __device__ __forceinline__ void start_first_item(const SpectraArgs &a, const War
 
 /* the hint of the item's first group (its other groups, and the short last group of a large batch, load theirs
  * when they get there) */
-__device__ __forceinline__ int item_hint(const SpectraArgs &a, const Item &it, int lane)
+__device__ __forceinline__ HintEntry item_hint(const SpectraArgs &a, const Item &it, int lane)
 {
     const int np = min(32, a.P - 32 * it.chunk * a.chunk_groups);
     return load_hint(a.ds[it.d], np, lane, it.b0, it.b1 - it.b0);
@@ -867,7 +895,9 @@ __device__ __forceinline__ void ticket_loop(const SpectraArgs &a, const Tables &
     long long kacc[4] = {0, 0, 0, 0};
 #endif
     Item it, nit;
-    int hint = 0, nhint = 0;
+    HintEntry hint, nhint;
+    hint.bin = 0; hint.x_env = pos_inf();
+    nhint = hint;
     if (cur < n_items) {
         decode_item<SMALL>(a, cur, it.d, it.b0, it.b1, it.chunk);
         hint = item_hint(a, it, lane);
@@ -902,14 +932,14 @@ __device__ __forceinline__ void ticket_loop(const SpectraArgs &a, const Tables &
             const void *unit = wp.buf0 + b * STAGE_BUF_BYTES;
             const bool full = !SMALL && 32 * g + 16 < a.P;
             /* the prefetched hint fits the item's first group, and every full group (all lanes start at b0) */
-            int hg = hint;
+            HintEntry hg = hint;
             if (!SMALL && g > g0 && !full) hg = load_hint(ds, a.P - 32 * g, lane, it.b0, nb);
             if (ds.unit_w) {
-                if (full) { if (!SMALL) walk_unit<S, true, true, DBG>(a, T, ds, it.d, unit, it.b0, nb, g, lane, hg); }
-                else      walk_unit<S, false, true, DBG>(a, T, ds, it.d, unit, it.b0, nb, g, lane, hg);
+                if (full) { if (!SMALL) walk_unit<S, true, true, DBG, !SMALL>(a, T, ds, it.d, unit, it.b0, nb, g, lane, hg); }
+                else      walk_unit<S, false, true, DBG, !SMALL>(a, T, ds, it.d, unit, it.b0, nb, g, lane, hg);
             } else {
-                if (full) { if (!SMALL) walk_unit<S, true, false, DBG>(a, T, ds, it.d, unit, it.b0, nb, g, lane, hg); }
-                else      walk_unit<S, false, false, DBG>(a, T, ds, it.d, unit, it.b0, nb, g, lane, hg);
+                if (full) { if (!SMALL) walk_unit<S, true, false, DBG, !SMALL>(a, T, ds, it.d, unit, it.b0, nb, g, lane, hg); }
+                else      walk_unit<S, false, false, DBG, !SMALL>(a, T, ds, it.d, unit, it.b0, nb, g, lane, hg);
             }
         }
 #ifdef PHYLINO_TRACE
