@@ -296,18 +296,24 @@ phylino_status fill_batch(phylino_ctx *ctx, SpectraArgs &a, int P, const double 
     }
 
     /* Cut of the batch into work items (spectra.cu): U batches per unit, G point groups per item.
-     * Aim: at least 12 items per resident warp (dynamic balance, short tail) of at least 16 batch-groups
-     * each (the per-item cost -- first bin search, one flush per point -- stays a few percent). */
+     * Aim: at least 6 items per resident warp (dynamic balance; the fine tail below evens out the end) of at least
+     * 16 batch-groups each, units as long as the staging buffer allows: an item costs about 500 instructions that
+     * the hot loop keeps evicting from the instruction cache (ticket, decode, opening and flushing the run),
+     * against 300 per 16 events x 32 points of work -- round 2, ncu source view of config 2: 22 % of all warp
+     * instructions with units of 32 batches.  Measured (unit batches x groups per item): config 2 32 x 1 7.3e11,
+     * 64 x 1 7.7e11, 128 x 1 6.8e11 event x point/s; config 3 64 x 2 0.997e12, 128 x 1 1.014e12; config 5 64 x 2
+     * 6.21e11, 128 x 2 6.27e11, 128 x 1 6.25e11. */
     int cap = std::max(ctx->resident_warps, WARPS);
     if (ctx->max_warps > 0) cap = std::max(WARPS, std::min(cap, ctx->max_warps / WARPS * WARPS));
-    const int64_t work = std::max<int64_t>(1, batches * n_groups / (12ll * cap));
+    const int64_t work = std::max<int64_t>(1, batches * n_groups / (6ll * cap));
+    /* a unit must fit the warp's staging buffer: 64 weighted or 128 unit-weight batches */
+    const int64_t u_max = STAGE_BUF_BYTES / (int64_t)(all_slim ? sizeof(EventBatchU) : sizeof(EventBatchW));
     int64_t U = 16;
-    while (U < 64 && U * 2 <= work) U *= 2;
+    while (U < u_max && U * 2 <= work) U *= 2;
     U = std::max<int64_t>(U, 4 * streams);
     if (ctx->unit_events > 0) U = std::max(1, ctx->unit_events / EB);
-    U = std::min<int64_t>(U, MAX_UNIT_BATCHES);         /* a unit must fit the warp's staging buffer */
-    /* two point groups per item measured best for units of 64 batches (short items balance better and the
-     * unit is re-read from L2, not DRAM); chunks of equal size */
+    U = std::min<int64_t>(U, u_max);
+    /* point groups per item: one once the units are long; chunks of equal size */
     int64_t G = std::max<int64_t>(1, std::min<int64_t>(std::min<int64_t>(work, 128) / U, n_groups));
     G = (n_groups + (n_groups + G - 1) / G - 1) / ((n_groups + G - 1) / G);
     if (ctx->chunk_groups > 0) G = std::min<int64_t>(ctx->chunk_groups, n_groups);

@@ -32,7 +32,6 @@ constexpr int EB          = 4;                      /* events per batch; every d
 constexpr int WARPS       = PHYLINO_WARPS;          /* warps per CTA of the spectra kernels */
 constexpr int CTAS_PER_SM = PHYLINO_CTAS_PER_SM;    /* ... and CTAs per SM their register budget is set for */
 constexpr int STAGE_BUF_BYTES = 6144;               /* one staging buffer of a warp: a unit is at most this long */
-constexpr int MAX_UNIT_BATCHES = 64;                /* ticket schedule: batches per unit (<= 6 KB of 96-byte records) */
 constexpr int HINT_BATCHES = 16;                    /* one bin hint per this many batches of a dataset */
 constexpr int MAX_TERMS   = 3;
 constexpr int SETUP_THREADS = 128;
