@@ -559,12 +559,12 @@ __device__ __forceinline__ void open_run(const DatasetDev &ds, const float *thr,
     r.hi2 = thr_at(thr, B, b + 2);
 }
 
-/* K consecutive batches known to lie inside the lane's open run (the store is sorted: the last
- * event of the last batch is below r.hi): rows a2 + a4 only, straight-line. */
+/* K batches of the lane's stream (bp, bp + st, ...; dataset batches gb, gb + st, ...) known to lie inside the lane's
+ * open run (the store is sorted: the last event of the last batch is below r.hi): rows a2 + a4 only, straight-line. */
 template <int S, bool UW, int K, bool DBG, bool SM, bool MED, bool FO>
 __device__ __forceinline__ void walk_inside(const SpectraArgs &a, const DatasetDev &ds,
-                                            const typename RecOf<UW>::type *bp, int gb, const double (&h)[S], int p,
-                                            bool active, Run<S> &r)
+                                            const typename RecOf<UW>::type *bp, int gb, int st, const double (&h)[S],
+                                            int p, bool active, Run<S> &r)
 {
     unsigned parity[S];                             /* unit weights: parity bits of this stretch's events, per term */
 #pragma unroll
@@ -572,7 +572,7 @@ __device__ __forceinline__ void walk_inside(const SpectraArgs &a, const DatasetD
     static_assert(EB * K <= 32, "one parity register per term and stretch");
 #pragma unroll
     for (int u = 0; u < K; ++u) {
-        const double2 *q = reinterpret_cast<const double2 *>(bp + u);
+        const double2 *q = reinterpret_cast<const double2 *>(bp + u * st);
 #pragma unroll
         for (int j = 0; j < EB / 2; ++j) {
             const double2 t = q[j];
@@ -597,9 +597,9 @@ __device__ __forceinline__ void walk_inside(const SpectraArgs &a, const DatasetD
                 for (int k = 0; k < S; ++k) r.C[k] = fma(w.y, half_cos_term<S, SM>(k, h[k], t.y), r.C[k]);
             }
         }
-        if (!UW) r.W += reinterpret_cast<const EventBatchW *>(bp + u)->wsum;
+        if (!UW) r.W += reinterpret_cast<const EventBatchW *>(bp + u * st)->wsum;
         if (DBG)
-            for (int j = 0; j < EB; ++j) dbg_mark<DBG>(a, ds, p, active, gb + u, j, r.cur);
+            for (int j = 0; j < EB; ++j) dbg_mark<DBG>(a, ds, p, active, gb + u * st, j, r.cur);
     }
     if (UW) {
         r.W += (double)(EB * K);                    /* whole numbers: the same bits as K separate adds */
@@ -681,7 +681,7 @@ __device__ __forceinline__ void walk_batch(const SpectraArgs &a, const Tables &T
     if (bp->v[EB - 1] < r.hi) {
         /* rows a3 + a4: the store is sorted, so the whole batch lies in the run's bin (a padding event has
          * E_vis = NaN and fails the test: it never comes here) */
-        walk_inside<S, UW, 1, DBG, SM, MED, FO>(a, ds, bp, gb, h, p, active, r);
+        walk_inside<S, UW, 1, DBG, SM, MED, FO>(a, ds, bp, gb, 1, h, p, active, r);
     } else {
         Coef<S> c;
 #pragma unroll
@@ -690,42 +690,49 @@ __device__ __forceinline__ void walk_batch(const SpectraArgs &a, const Tables &T
     }
 }
 
-/* `mine` consecutive batches of the lane's stream starting at bp (dataset batch gb): 4, 2 or 1 at a time */
+/* `mine` batches of the lane's stream, bp, bp + st, bp + 2 st, ... (dataset batches gb, gb + st, ...): 4, 2 or 1 at a
+ * time.  st = 1: every lane walks the whole unit; st = NS: the lane's sub-stream of a small batch of points. */
 template <int S, bool UW, bool DBG, bool SM, bool MED, bool FO>
 __device__ __forceinline__ void walk_stretch(const SpectraArgs &a, const Tables &T, const DatasetDev &ds,
-                                             const typename RecOf<UW>::type *bp, int gb, int mine, const double (&h)[S],
-                                             const float *thr, float2 safe, int p, bool active, Run<S> &r)
+                                             const typename RecOf<UW>::type *bp, int gb, int mine, int st,
+                                             const double (&h)[S], const float *thr, float2 safe, int p, bool active,
+                                             Run<S> &r)
 {
     int i = 0;
 #pragma unroll 1
     while (i < mine) {
-        if (i + 4 <= mine && bp[3].v[EB - 1] < r.hi) {
-            walk_inside<S, UW, 4, DBG, SM, MED, FO>(a, ds, bp, gb + i, h, p, active, r);
+        if (i + 4 <= mine && bp[3 * st].v[EB - 1] < r.hi) {
+            walk_inside<S, UW, 4, DBG, SM, MED, FO>(a, ds, bp, gb + i * st, st, h, p, active, r);
             i += 4;
-            bp += 4;
-        } else if (i + 2 <= mine && bp[1].v[EB - 1] < r.hi) {
-            walk_inside<S, UW, 2, DBG, SM, MED, FO>(a, ds, bp, gb + i, h, p, active, r);
+            bp += 4 * st;
+        } else if (i + 2 <= mine && bp[st].v[EB - 1] < r.hi) {
+            walk_inside<S, UW, 2, DBG, SM, MED, FO>(a, ds, bp, gb + i * st, st, h, p, active, r);
             i += 2;
-            bp += 2;
+            bp += 2 * st;
         } else {
-            walk_batch<S, UW, DBG, SM, MED, FO>(a, T, ds, bp, gb + i, h, thr, safe, p, active, r);
+            walk_batch<S, UW, DBG, SM, MED, FO>(a, T, ds, bp, gb + i * st, h, thr, safe, p, active, r);
             ++i;
-            ++bp;
+            bp += st;
         }
     }
 }
 
 /* One warp, the nb batches [b0, b0 + nb) of dataset ds staged at `unit` (SHARED memory), point group g
  * (points 32 g ... 32 g + 31).  FULL: the group has more than 16 points, every lane walks all batches. */
-/* lane -> (point, sub-stream) for a group of np <= 16 points: PL = 2^lg >= np point lanes, the nb batches of a
- * unit split into NS = 32 / PL contiguous sub-streams; this lane's is [my0, my0 + mine) */
-__device__ __forceinline__ void substream_of(int np, int lane, int nb, int &lg, int &pl, int &my0, int &mine)
+/* lane -> (point, sub-stream) for a group of np <= 16 points: PL = 2^lg >= np point lanes, the nb batches of a unit
+ * dealt out to NS = 32 / PL sub-streams in turn: this lane's are my0, my0 + NS, my0 + 2 NS, ... (`mine` of them).
+ * Dealt out, not cut into contiguous pieces: the lanes of a warp then read NEIGHBOURING 48-byte records of the staged
+ * unit with every 128-bit load -- eight lanes of a quarter-warp, eight different 16-byte bank groups -- where the
+ * contiguous pieces (4 records = 192 bytes apart for one point) put four lanes on each group: ncu counted 1.49e6
+ * bank-conflict wavefronts of 2.23e6 in a one-point call over 6e6 events.  A lane's events stay sorted, which is all
+ * the run logic needs. */
+__device__ __forceinline__ void substream_of(int np, int lane, int nb, int &lg, int &pl, int &my0, int &mine, int &st)
 {
     lg = np <= 1 ? 0 : 32 - __clz(np - 1);
     pl = lane & ((1 << lg) - 1);
-    const int s = lane >> lg;
-    my0 = (nb * s) >> (5 - lg);
-    mine = ((nb * (s + 1)) >> (5 - lg)) - my0;
+    st = 32 >> lg;
+    my0 = lane >> lg;
+    mine = my0 < nb ? (nb - my0 + st - 1) >> (5 - lg) : 0;
 }
 
 /* the hint a lane needs to open its run in unit [b0, b0 + nb) of dataset ds (group of np points; np > 16: all
@@ -734,8 +741,9 @@ __device__ __forceinline__ HintEntry load_hint(const DatasetDev &ds, int np, int
 {
     int my0 = 0;
     if (np <= 16) {
-        int lg, pl, mine;
-        substream_of(np, lane, nb, lg, pl, my0, mine);
+        int lg, pl, mine, st;
+        substream_of(np, lane, nb, lg, pl, my0, mine, st);
+        if (mine == 0) my0 = 0;                         /* a lane without a batch opens no run */
     }
     PHYLINO_ASSERT(b0 + my0 >= 0 && (b0 + my0 < ds.n_batches || (nb == 0 && b0 + my0 <= ds.n_batches)));
     const int2 e = __ldg(reinterpret_cast<const int2 *>(ds.hint + (b0 + my0) / HINT_BATCHES));
@@ -753,13 +761,13 @@ __device__ __forceinline__ void walk_unit(const SpectraArgs &a, const Tables &T,
                                           const void *unit, int b0, int nb, int g, int lane, HintEntry hint)
 {
     typedef typename RecOf<UW>::type Rec;
-    int my0 = 0, mine = nb, lg = 5;
+    int my0 = 0, mine = nb, lg = 5, st = 1;
     bool active = 32 * g + lane < a.P;
     int p = 32 * g + (active ? lane : 0);
     if (!FULL) {
         const int np = min(32, a.P - 32 * g);
         int pl;
-        substream_of(np, lane, nb, lg, pl, my0, mine);
+        substream_of(np, lane, nb, lg, pl, my0, mine, st);
         active = pl < np;
         p = 32 * g + (active ? pl : 0);
     }
@@ -778,7 +786,7 @@ __device__ __forceinline__ void walk_unit(const SpectraArgs &a, const Tables &T,
     run_reset<S>(r);
     r.sm = T.small[g * a.n_datasets + d] != 0;
     r.fo = FO;
-    PHYLINO_ASSERT(my0 >= 0 && mine >= 0 && my0 + mine <= nb && p >= 0 && p < a.P);
+    PHYLINO_ASSERT(my0 >= 0 && mine >= 0 && (mine == 0 || my0 + (mine - 1) * st < nb) && p >= 0 && p < a.P);
     PHYLINO_ASSERT(row >= 0 && row < a.thr_rows);
     const Rec *bp = static_cast<const Rec *>(unit) + my0;
     if (mine > 0) open_run<S>(ds, thr, safe, bp->v[0], hint.bin, r);
@@ -792,11 +800,11 @@ __device__ __forceinline__ void walk_unit(const SpectraArgs &a, const Tables &T,
     r.med = ME && __all_sync(0xffffffffu, fabs(h[0]) * (double)hint.x_env <= MEDIUM_PHASE);
     if (ME && r.med) {
         if (lane == 0) atomicAdd(a.med_count, (unsigned long long)nb * EB * (unsigned)min(32, a.P - 32 * g));
-        if (r.sm) walk_stretch<S, UW, DBG, true, ME, FO>(a, T, ds, bp, b0 + my0, mine, h, thr, safe, p, active, r);
-        else      walk_stretch<S, UW, DBG, false, ME, FO>(a, T, ds, bp, b0 + my0, mine, h, thr, safe, p, active, r);
+        if (r.sm) walk_stretch<S, UW, DBG, true, ME, FO>(a, T, ds, bp, b0 + my0, mine, st, h, thr, safe, p, active, r);
+        else      walk_stretch<S, UW, DBG, false, ME, FO>(a, T, ds, bp, b0 + my0, mine, st, h, thr, safe, p, active, r);
     } else {
-        if (r.sm) walk_stretch<S, UW, DBG, true, false, FO>(a, T, ds, bp, b0 + my0, mine, h, thr, safe, p, active, r);
-        else      walk_stretch<S, UW, DBG, false, false, FO>(a, T, ds, bp, b0 + my0, mine, h, thr, safe, p, active, r);
+        if (r.sm) walk_stretch<S, UW, DBG, true, false, FO>(a, T, ds, bp, b0 + my0, mine, st, h, thr, safe, p, active, r);
+        else      walk_stretch<S, UW, DBG, false, false, FO>(a, T, ds, bp, b0 + my0, mine, st, h, thr, safe, p, active, r);
     }
 #ifdef PHYLINO_TRACE
     const long long q2 = clock64();
