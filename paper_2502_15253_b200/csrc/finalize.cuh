@@ -1,7 +1,6 @@
 /*
- * finalize.cuh -- the likelihood stage of one parameter point as a device function of one 128-thread CTA
- * (SURVEY.md 8(a) rows a5-a7), shared by finalize_kernel (finalize.cu) and by the last CTA of the
- * single-launch kernel for small batches (spectra.cu).
+ * finalize.cuh -- the likelihood stage of one parameter point as device functions of one 128-thread CTA
+ * (SURVEY.md 8(a) rows a5-a7), called by finalize_kernel and ensemble_kernel (finalize.cu).
  *
  *   mu[p,d,b] = eps_d norm_d f_db H[p,d,b] + sum_k r_dk s_dkb T_dkb
  *   nll[p]    = sum_{d,b} dev(n, mu) + 1/2 sum_j ((theta_j - mean_j)/sigma_j)^2

@@ -12,12 +12,14 @@
  * quarter-size units so the warps run out of work together) and walk the unit once per group.
  *
  * Small batches (spectra_fused_kernel: at most FUSED_MAX_POINTS points -- the minimiser's single
- * evaluations).  ONE launch does rows a1-a7: every CTA derives the per-point records and the
- * bin thresholds it needs into its own shared memory, every warp walks ONE contiguous range of batches
- * with its lanes split into 32 / PL sub-streams (PL = points rounded up to a power of two) and the runs
- * carried across the units of the range, and the CTA that finishes last runs the expectation / likelihood
- * stage (finalize.cuh) on the accumulators.  No setup launch, no finalize launch, no host copy of the
- * parameters: the call is bound by the event bytes over HBM (12 B/event for unit-weight datasets).
+ * evaluations).  ONE launch does rows a1-a5: every CTA derives the per-point records and the
+ * bin thresholds it needs into its own shared memory, then the same ticket loop runs over units as long as a
+ * staging buffer holds, the lanes of a warp split into 32 / PL sub-streams (PL = points rounded up to a power of
+ * two) that are dealt the batches of a unit in turn.  No setup launch and no host copy of the parameters (a small
+ * host batch rides with the kernel arguments); the finalize kernel behind it is a programmatic dependent that
+ * does its table work while the events are walked.  The call is bound by the event bytes over HBM (12 B/event
+ * for unit-weight datasets) and by latency -- launch, per-CTA setup, the instruction lines of everything that is
+ * not the hot loop -- not by arithmetic.
  *
  * Staging.  Each warp owns two unit-sized buffers in shared memory and one mbarrier per buffer; lane 0
  * starts ONE bulk async copy (cp.async.bulk global -> shared, completion on the mbarrier) of the NEXT
@@ -28,8 +30,11 @@
  *
  * Oscillation weight (row a2).  P_ee = P0 + sum_k A_k g_k with g = 1/2 cos(2 phase) (devmath.cuh):
  * the lane accumulates C_k = sum_e w_e g_k(e) and W = sum_e w_e over a run of events that share a
- * bin; the run's total is P0 W + sum_k A_k C_k, formed once per run.  Per event x point that is
- * 11 fp64 instructions and one integer instruction per oscillation term.
+ * bin; the run's total is P0 W + sum_k A_k C_k, formed once per run.  Per event x point and term that is
+ * 11 fp64 instructions and one integer instruction in the general form; unit-weight datasets take cheaper
+ * forms where they are exact: the run sum formed by the last Horner step itself (10 + 2 integer; two-term
+ * model), no range reduction where the first term's phase cannot wrap within a work item (8), a cubic for a
+ * last term that stays below an eighth of a half-turn over a dataset (6): see folded() below.
  *
  * Binning (row a3).  For one point the map v -> E' = fma(fma(a2,v,a1),v,a0) is non-decreasing over
  * the fp32 values of a dataset (checked per point), so bin(E'(v)) >= b <=> v >= T[b] with T[b] the

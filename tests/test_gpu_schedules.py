@@ -278,3 +278,32 @@ def test_flux_rebinning_block_through_set_transform(gpu, oracle_mod):
     assert np.abs(nll - orc.nll(theta, data)).max() <= ABS_NLL
     assert np.array_equal(nll, nll_h)
     _check_hist(mu, orc.expectation(theta, orc.spectra(theta)))
+
+
+# ---- the cheaper forms of a term where they are exact (devmath.cuh: folded / no-reduction / small-phase) ----------
+# The kernel may take them only where the result is the general form's: the first term without range reduction where
+# |phase| <= 1/2 half-turn for every event of a work item and every point of the group, the last term as a cubic where
+# it stays below 1/8 over a dataset.  Checked here: the forms are actually reached on the Double-Chooz-like stores and
+# not on the 52-km one, batches of at most 16 points (single-launch kernel) never take the first, and every one of these
+# batches matches the oracle far inside the per-bin bar (a dropped parity count or constant part would be O(1)).
+@pytest.mark.parametrize("k,scale,n_points", [(2, 0.05, 64), (3, 0.02, 40), (5, 0.05, 96), (4, 0.01, 64), (2, 0.05, 8)])
+def test_cheaper_forms_are_reached_and_exact(gpu, oracle_mod, k, scale, n_points):
+    wl = workloads.make_config(k, scale=scale, n_points=n_points)
+    orc = oracle_mod.Oracle(wl.model, wl.events)
+    with gpu.Phylino() as ph:
+        ph.load_workload(wl)
+        h = ph.spectra(_dev(wl.params)).cpu().numpy()
+        med, small = ph.last_medium_phase(), ph.last_small_phase()
+        h_o = orc.spectra(wl.params)
+        nz = h_o != 0.0
+        assert np.array_equal(h[~nz], h_o[~nz])
+        assert (np.abs(h - h_o)[nz] / np.abs(h_o[nz])).max() <= 1e-10
+        if k == 4:                      # 52 km: the dm2_ee phase is hundreds of radians, the solar term up to 5 rad
+            assert med == 0.0 and small == 0.0
+        elif n_points <= 16:            # single-launch kernel: small-phase form only
+            assert med == 0.0 and small == 1.0
+        else:                           # near detector fully, far detector above 4-4.5 MeV
+            assert 0.25 < med < 0.9 and small == 1.0, (med, small)
+        # determinism of the count and of the bits
+        h2 = ph.spectra(_dev(wl.params)).cpu().numpy()
+        assert np.array_equal(h, h2) and ph.last_medium_phase() == med
