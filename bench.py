@@ -412,6 +412,32 @@ def gradient_step_wall(pkg, torch, local, flush, steps=10):
         res[key + "_min"] = min(ts)
         if on:
             res["virtual_points"], res["energy_scale_classes"] = ph.last_plan()
+    # the same step with the batch formed and differenced ON THE DEVICE (phylino_nll_gradient: theta and steps in,
+    # gradient out; with caching the plan comes from the batch's structure, so nothing is copied back and nothing
+    # synchronises): device time between CUDA events
+    N = wl.model.n_params
+    theta0 = wl.params[0].copy()
+    d_theta = torch.as_tensor(theta0, device="cuda")
+    d_step = torch.as_tensor(np.array([wl.params[1 + 2 * j, j] - theta0[j] for j in range(N)]), device="cuda")
+    d_data0 = torch.as_tensor(data, device="cuda")
+    g0 = torch.empty(1, dtype=torch.float64, device="cuda")
+    gg = torch.empty(N, dtype=torch.float64, device="cuda")
+    for key, on in (("device_gradient_dense_ms", False), ("device_gradient_cached_ms", True)):
+        ph.set_caching(on)
+        for _ in range(3):
+            ph.nll_gradient(d_theta, d_step, d_data0, g0, gg)
+        ts = []
+        for i in range(steps):
+            flush.zero_()
+            s0, e0 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            s0.record()
+            ph.nll_gradient(d_theta, d_step, d_data0, g0, gg)
+            e0.record()
+            torch.cuda.synchronize()
+            ts.append(s0.elapsed_time(e0))
+        res[key] = sum(ts) / steps
+        res[key + "_median"] = statistics.median(ts)
+        res[key + "_min"] = min(ts)
     ph.set_caching(False)
     # a minimiser's SINGLE evaluation on the same store (one point over 6e6 events): bound by the event bytes over
     # HBM, not by arithmetic -- the small-batch kernel (setup fused in) + the overlapped finalize kernel

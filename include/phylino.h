@@ -235,7 +235,11 @@ PHYLINO_API phylino_status phylino_ordering_scan(phylino_ctx *ctx, int n_grid, i
  * device, evaluated (with cross-point caching if phylino_set_caching is on), and
  *   grad[j] = (nll(theta + step_j e_j) - nll(theta - step_j e_j)) / ((theta_j + step_j) - (theta_j - step_j)).
  *   theta, step DEVICE [N] (step_j != 0); data DEVICE [total_bins]; nll0 DEVICE [1] receives nll(theta), may be
- *   NULL; grad DEVICE [N].  Asynchronous unless caching is on (see phylino_set_caching). */
+ *   NULL; grad DEVICE [N].  Asynchronous, also with caching on: which points of a central-difference batch share an
+ *   energy scale or a mass splitting follows from which column each point perturbs, so the plan needs no values and
+ *   nothing is copied back (a step below one ulp of theta_j only loses a merge, never a result).  Exception: caching
+ *   together with a transformation layer goes through the host plan of phylino_set_caching (one copy back, one
+ *   synchronisation). */
 PHYLINO_API phylino_status phylino_nll_gradient(phylino_ctx *ctx, const double *theta, const double *step,
                                                 const double *data, double *nll0, double *grad);
 

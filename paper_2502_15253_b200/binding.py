@@ -394,14 +394,17 @@ class Phylino:
                                                     data.data_ptr(), out.data_ptr()))
         return out
 
-    def nll_gradient(self, theta, step, data):
+    def nll_gradient(self, theta, step, data, nll0=None, grad=None):
         """theta, step [param_width], data [total_bins] (float64 CUDA) -> (nll(theta) [1], grad [param_width])."""
         t = self._torch
         N = self.param_width
         theta, step = self._dev_vec(theta, N, "theta"), self._dev_vec(step, N, "step")
         data = self._dev_vec(data, self.total_bins, "data")
-        nll0 = t.empty(1, dtype=t.float64, device=theta.device)
-        grad = t.empty(N, dtype=t.float64, device=theta.device)
+        if nll0 is None:
+            nll0 = t.empty(1, dtype=t.float64, device=theta.device)
+        if grad is None:
+            grad = t.empty(N, dtype=t.float64, device=theta.device)
+        nll0, grad = self._dev_vec(nll0, 1, "nll0"), self._dev_vec(grad, N, "grad")
         self._check(self._lib.phylino_nll_gradient(self._ctx, theta.data_ptr(), step.data_ptr(), data.data_ptr(),
                                                    nll0.data_ptr(), grad.data_ptr()))
         return nll0, grad

@@ -101,9 +101,9 @@ void free_all(phylino_ctx *c)
     free_tables(c);
     cudaFree(c->d_acc); cudaFree(c->d_flags);
     c->d_acc = nullptr; c->d_flags = nullptr; c->acc_capacity = 0;
-    cudaFree(c->d_rec); cudaFree(c->d_thr); cudaFree(c->d_safe); cudaFree(c->d_counter); cudaFree(c->d_done); cudaFree(c->d_med);
+    cudaFree(c->d_rec); cudaFree(c->d_thr); cudaFree(c->d_safe); cudaFree(c->d_counter); cudaFree(c->d_done); cudaFree(c->d_med); cudaFree(c->d_grad_plan);
     cudaFree(c->d_small);
-    c->d_rec = nullptr; c->d_thr = nullptr; c->d_safe = nullptr; c->d_counter = nullptr; c->d_done = nullptr; c->d_med = nullptr;
+    c->d_rec = nullptr; c->d_thr = nullptr; c->d_safe = nullptr; c->d_counter = nullptr; c->d_done = nullptr; c->d_med = nullptr; c->d_grad_plan = nullptr; c->grad_plan_state = 0;
     c->d_small = nullptr;
     c->point_capacity = 0;
     cudaFree(c->d_plan); c->d_plan = nullptr; c->plan_capacity = 0;
@@ -487,11 +487,6 @@ phylino_status resolve_params(phylino_ctx *ctx, int P, const double *params, con
  * time into virtual points for the spectra kernel, and tells the finalize kernel which cells each
  * real point combines.  A 603-point central-difference batch of config 3 becomes 21 virtual
  * points, the 4096-point grid of config 5 becomes 22. */
-struct ComponentPlan {
-    int V = 0, C = 0;
-    std::vector<int32_t> vp_class, vp_src, class_rep, pt_comp;
-};
-
 /* parameters the half-turn coefficient of term k depends on (devmath.cuh osc_terms) */
 int term_deps(int osc_model, int k, int slots[3])
 {
@@ -609,34 +604,47 @@ bool plan_components(const phylino_ctx *ctx, int P, const double *params, Compon
     return true;
 }
 
+/* the plan as the kernels read it: vp_class | vp_src | class_rep | pt_comp */
+std::vector<int32_t> plan_blob(const ComponentPlan &pl)
+{
+    std::vector<int32_t> blob;
+    blob.reserve(pl.vp_class.size() + pl.vp_src.size() + pl.class_rep.size() + pl.pt_comp.size());
+    blob.insert(blob.end(), pl.vp_class.begin(), pl.vp_class.end());
+    blob.insert(blob.end(), pl.vp_src.begin(), pl.vp_src.end());
+    blob.insert(blob.end(), pl.class_rep.begin(), pl.class_rep.end());
+    blob.insert(blob.end(), pl.pt_comp.begin(), pl.pt_comp.end());
+    return blob;
+}
+
 /* enqueue rows a1-a7 for a host-resident batch already copied to d_params, through the component
  * plan; hist xor nll as in enqueue_finalize */
 phylino_status enqueue_cached(phylino_ctx *ctx, int P, const double *h_params, const double *d_params,
-                              const double *d_data, double *d_hist, double *d_nll, bool *used)
+                              const double *d_data, double *d_hist, double *d_nll, bool *used,
+                              const ComponentPlan *given = nullptr, const int32_t *d_given = nullptr)
 {
     *used = false;
     ctx->last_virtual_points = ctx->last_classes = 0;
-    ComponentPlan pl;
-    if (!plan_components(ctx, P, h_params, pl)) return PHYLINO_OK;
+    ComponentPlan made;
+    if (!given && !plan_components(ctx, P, h_params, made)) return PHYLINO_OK;
+    const ComponentPlan &pl = given ? *given : made;
     const int S = ctx->n_terms, V = pl.V;
     phylino_status s;
     /* accumulator rows: V (S + 1); threshold rows and records: sized by ensure_acc for max(P, .) points */
     if ((s = ensure_acc(ctx, std::max(P, V * (S + 1)))) != PHYLINO_OK) return s;
     const int64_t n_int = (int64_t)V + (int64_t)V * S + pl.C + (int64_t)P * (S + 1);
-    if (n_int > ctx->plan_capacity) {
-        CU(cudaStreamSynchronize(ctx->stream));
-        cudaFree(ctx->d_plan); ctx->d_plan = nullptr; ctx->plan_capacity = 0;
-        CU(cudaMalloc((void **)&ctx->d_plan, n_int * sizeof(int32_t)));
-        ctx->plan_capacity = n_int;
+    const int32_t *d_plan = d_given;            /* a plan that already sits on the device (gradient_plan) */
+    if (!d_plan) {
+        if (n_int > ctx->plan_capacity) {
+            CU(cudaStreamSynchronize(ctx->stream));
+            cudaFree(ctx->d_plan); ctx->d_plan = nullptr; ctx->plan_capacity = 0;
+            CU(cudaMalloc((void **)&ctx->d_plan, n_int * sizeof(int32_t)));
+            ctx->plan_capacity = n_int;
+        }
+        const std::vector<int32_t> blob = plan_blob(pl);
+        /* pageable source: the copy is staged by the driver before the call returns */
+        CU(cudaMemcpyAsync(ctx->d_plan, blob.data(), n_int * sizeof(int32_t), cudaMemcpyHostToDevice, ctx->stream));
+        d_plan = ctx->d_plan;
     }
-    std::vector<int32_t> blob;
-    blob.reserve((size_t)n_int);
-    blob.insert(blob.end(), pl.vp_class.begin(), pl.vp_class.end());
-    blob.insert(blob.end(), pl.vp_src.begin(), pl.vp_src.end());
-    blob.insert(blob.end(), pl.class_rep.begin(), pl.class_rep.end());
-    blob.insert(blob.end(), pl.pt_comp.begin(), pl.pt_comp.end());
-    /* pageable source: the copy is staged by the driver before the call returns */
-    CU(cudaMemcpyAsync(ctx->d_plan, blob.data(), n_int * sizeof(int32_t), cudaMemcpyHostToDevice, ctx->stream));
 
     SpectraArgs a{};
     fill_datasets(ctx, a);
@@ -644,15 +652,15 @@ phylino_status enqueue_cached(phylino_ctx *ctx, int P, const double *h_params, c
     if ((s = fill_batch(ctx, a, V, d_params, pl.C)) != PHYLINO_OK) return s;
     ctx->last_points = V;
     ctx->last_fused = a.sched == 1;
-    a.vp_class = ctx->d_plan;
-    a.vp_src = ctx->d_plan + V;
-    a.class_rep = ctx->d_plan + V + (int64_t)V * S;
+    a.vp_class = d_plan;
+    a.vp_src = d_plan + V;
+    a.class_rep = d_plan + V + (int64_t)V * S;
     FinalizeArgs f = ctx->fin;
     f.P = P; f.params = d_params; f.acc = ctx->d_acc; f.flags = ctx->d_flags;
     f.data = d_data; f.hist = d_hist; f.nll = d_nll;
     f.comp = 1; f.n_terms = S; f.osc = a.osc;
     f.ec_mode = ctx->ec_mode;
-    f.pt_comp = ctx->d_plan + V + (int64_t)V * S + pl.C;
+    f.pt_comp = d_plan + V + (int64_t)V * S + pl.C;
     if (ctx->timing) CU(cudaEventRecord(ctx->ev[0], ctx->stream));
     if (a.sched == 1) {
         /* few virtual points: setup and walk in one launch; the per-point combination stays a launch of its own */
@@ -677,6 +685,40 @@ phylino_status enqueue_cached(phylino_ctx *ctx, int P, const double *h_params, c
     ctx->last_classes = pl.C;
     *used = true;
     return PHYLINO_OK;
+}
+
+/* The plan of a central-difference batch {theta} U {theta +- step_j e_j} needs no values: which points share an
+ * energy-scale tuple or a mass splitting follows from WHICH column a point perturbs.  plan_components only compares
+ * bit patterns, so it is run once per model on a symbolic batch with that equality structure (column j holds j,
+ * perturbed entries j +- 1/4) and the plan is kept.  Points that are structurally different but equal in value
+ * (a step below one ulp) are merely not merged; structurally equal points ARE equal in value, so nothing is merged
+ * wrongly.  Not with a transformation layer (a step in u_j moves several columns of theta by amounts the symbols do
+ * not know).  With this phylino_nll_gradient plans without seeing the batch: no copy back, no synchronisation. */
+const ComponentPlan *gradient_plan(phylino_ctx *ctx, int width)
+{
+    if (ctx->grad_plan_state == 0) {
+        cudaFree(ctx->d_grad_plan);
+        ctx->d_grad_plan = nullptr;
+        const int P = 2 * width + 1;
+        std::vector<double> sym((size_t)P * width);
+        for (int r = 0; r < P; ++r)
+            for (int j = 0; j < width; ++j)
+                sym[(size_t)r * width + j] = (double)j + ((r > 0 && (r - 1) / 2 == j) ? ((r & 1) ? 0.25 : -0.25) : 0.0);
+        ctx->grad_plan = ComponentPlan();
+        ctx->grad_plan_state = plan_components(ctx, P, sym.data(), ctx->grad_plan) ? 1 : -1;
+        if (ctx->grad_plan_state > 0) {
+            /* once per model, outside any capture: the plan stays on the device */
+            const std::vector<int32_t> blob = plan_blob(ctx->grad_plan);
+            if (cudaMalloc((void **)&ctx->d_grad_plan, blob.size() * sizeof(int32_t)) != cudaSuccess ||
+                cudaMemcpy(ctx->d_grad_plan, blob.data(), blob.size() * sizeof(int32_t), cudaMemcpyHostToDevice) != cudaSuccess) {
+                cudaGetLastError();
+                cudaFree(ctx->d_grad_plan);
+                ctx->d_grad_plan = nullptr;
+                ctx->grad_plan_state = -1;
+            }
+        }
+    }
+    return ctx->grad_plan_state > 0 ? &ctx->grad_plan : nullptr;
 }
 
 /* Caching for a DEVICE-resident batch: the plan is made on the host, so theta comes back once (one
@@ -821,6 +863,7 @@ phylino_status phylino_set_model(phylino_ctx *ctx, const phylino_model_desc *m)
     f.total_bins = (int32_t)tb;
     f.staged = tb <= FIN_STAGE_MAX_BINS ? 1 : 0;
     ctx->ec_mode = 0;
+    ctx->grad_plan_state = 0;
     ctx->fm_idx.assign(m->n_datasets, std::vector<int32_t>());
     ctx->fm_lo.assign(m->n_datasets, 0.0);
     ctx->fm_width.assign(m->n_datasets, 0.0);
@@ -1113,7 +1156,13 @@ phylino_status phylino_nll_gradient(phylino_ctx *ctx, const double *theta, const
     double *batch = ctx->d_work, *nll = ctx->d_work + (int64_t)P * width;
     CU(launch_gradient_batch(theta, step, (int)width, batch, ctx->stream));
     ctx->launches += 1;
-    if ((s = phylino_nll(ctx, P, batch, data, nll)) != PHYLINO_OK) return s;      /* dense, or cached if caching is on */
+    bool done = false;
+    if (ctx->caching && !ctx->have_tf && !wants_single_launch(ctx, P)) {
+        /* cached through the structural plan of the batch: asynchronous like the dense call */
+        if (const ComponentPlan *pl = gradient_plan(ctx, (int)width))
+            if ((s = enqueue_cached(ctx, P, nullptr, batch, data, nullptr, nll, &done, pl, ctx->d_grad_plan)) != PHYLINO_OK) return s;
+    }
+    if (!done && (s = phylino_nll(ctx, P, batch, data, nll)) != PHYLINO_OK) return s;   /* dense, or cached via the host plan */
     CU(launch_gradient(theta, step, nll, (int)width, nll0, grad, ctx->stream));
     ctx->launches += 1;
     return PHYLINO_OK;
@@ -1343,6 +1392,7 @@ phylino_status phylino_set_energy_correction_mode(phylino_ctx *ctx, int mode)
     if (mode == 1 && !ctx->fin.staged)
         return fail(ctx, PHYLINO_ERR_SHAPE, "the bin-level correction needs total_bins <= %d", FIN_STAGE_MAX_BINS);
     ctx->ec_mode = mode;
+    ctx->grad_plan_state = 0;
     ctx->fused_warps = 0;               /* the threshold tables of the small-batch kernel change size */
     return PHYLINO_OK;
 }

@@ -207,6 +207,12 @@ struct TransformArgs {
     double        *theta;         /* [P x n_params] */
 };
 
+/* cross-point caching: the plan of a batch (api.cu plan_components) */
+struct ComponentPlan {
+    int V = 0, C = 0;               /* virtual points, energy-scale classes */
+    std::vector<int32_t> vp_class, vp_src, class_rep, pt_comp;
+};
+
 /* kernel launchers (spectra.cu, finalize.cu, transform.cu, peaks.cu) */
 cudaError_t launch_transform(const TransformArgs &a, cudaStream_t st);
 cudaError_t launch_setup(const SpectraArgs &a, int S, cudaStream_t st);
@@ -283,6 +289,9 @@ struct phylino_ctx {
     int32_t *d_plan = nullptr;                     /* vp_class | vp_src | class_rep | pt_comp */
     int64_t plan_capacity = 0;                     /* int32 entries */
     int64_t last_virtual_points = 0, last_classes = 0;
+    phylino::ComponentPlan grad_plan;              /* structural plan of the central-difference batch (phylino_nll_gradient) */
+    int grad_plan_state = 0;                       /* 0: not made for this model yet, 1: made, -1: does not pay */
+    int32_t *d_grad_plan = nullptr;                /* ... on the device: vp_class | vp_src | class_rep | pt_comp */
     /* transformation layer (phylino_set_transform): host copy for the host entry points, device tables */
     bool have_tf = false;
     int32_t n_u = 0;

@@ -109,3 +109,62 @@ def test_gradient_from_the_603_point_batch(gpu, oracle_mod, caching):
     assert abs(nll0[0] - nll_o[0]) <= ABS_NLL
     assert np.all(np.abs(grad - grad_o) <= 1e-6 / np.abs(h))
     assert np.abs(grad - grad_o).max() <= 1e-3 * max(1.0, np.abs(grad_o).max())       # and tight in absolute terms
+
+
+def test_cached_gradient_plans_without_the_values(gpu, oracle_mod):
+    """phylino_nll_gradient with caching on takes the plan of a central-difference batch from its structure (which
+    column each point perturbs), not from the values: the same 21 virtual points as the host plan of the same batch,
+    the same bits, the call can be captured into a CUDA graph (nothing is copied back, nothing synchronises), and a
+    step below one ulp -- structurally different, equal in value -- only loses a merge."""
+    import torch
+    wl = workloads.make_config(3, scale=0.01)
+    N = wl.model.n_params
+    orc = oracle_mod.Oracle(wl.model, wl.events)
+    data = _data(orc, wl)
+    theta = wl.params[0].copy()
+    h = np.array([wl.params[1 + 2 * j, j] - theta[j] for j in range(N)])
+    with gpu.Phylino() as ph:
+        ph.load_workload(wl)
+        ph.reserve(2 * N + 1)
+        ph.set_caching(True)
+        d_theta, d_h, d_data = _dev(theta), _dev(h), _dev(data)
+        nll0, grad = ph.nll_gradient(d_theta, d_h, d_data)
+        plan = ph.last_plan()
+        # the host plan of the very same batch (values seen): same plan, same bits
+        batch = np.tile(theta, (2 * N + 1, 1))
+        for j in range(N):
+            batch[1 + 2 * j, j] = theta[j] + h[j]
+            batch[2 + 2 * j, j] = theta[j] - h[j]
+        nll_host = ph.nll(_dev(batch), d_data).cpu().numpy()
+        assert ph.last_plan() == plan and plan[0] == 21
+        up = batch[1::2][np.arange(N), np.arange(N)]
+        dn = batch[2::2][np.arange(N), np.arange(N)]
+        assert np.array_equal(grad.cpu().numpy(), (nll_host[1::2] - nll_host[2::2]) / (up - dn))
+        assert nll0.cpu().numpy()[0] == nll_host[0]
+        # capture + replay: would fail on any synchronisation or copy back inside the call
+        g = torch.cuda.CUDAGraph()
+        out0 = torch.empty(1, dtype=torch.float64, device="cuda")
+        outg = torch.empty(N, dtype=torch.float64, device="cuda")
+        s = torch.cuda.Stream()
+        with torch.cuda.stream(s):
+            with gpu.Phylino(stream=s.cuda_stream) as ph2:
+                ph2.load_workload(wl)
+                ph2.reserve(2 * N + 1)
+                ph2.set_caching(True)
+                ph2.nll_gradient(d_theta, d_h, d_data, out0, outg)        # warm: plan made, buffers sized
+                s.synchronize()
+                with torch.cuda.graph(g, stream=s):
+                    ph2.nll_gradient(d_theta, d_h, d_data, out0, outg)
+                outg.zero_()
+                g.replay()
+                s.synchronize()
+                assert np.array_equal(outg.cpu().numpy(), grad.cpu().numpy())
+        # a vanishing step: theta_j +- h_j == theta_j bit for bit; the structural plan keeps the points apart, the
+        # values are those of the centre
+        h2 = h.copy()
+        h2[5] = theta[5] * 1e-20 if theta[5] != 0 else 1e-320
+        nll0b, gradb = ph.nll_gradient(d_theta, _dev(h2), d_data)
+        gb = gradb.cpu().numpy()
+        assert np.isnan(gb[5]) or gb[5] == 0.0 or np.isinf(gb[5])       # 0 / 0 or 0 / tiny: no information, no crash
+        keep = np.arange(N) != 5
+        assert np.array_equal(gb[keep], grad.cpu().numpy()[keep])
