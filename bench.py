@@ -303,9 +303,14 @@ def measure(pkg, torch, dist, k, steps, warmup, local, rank, world, flush, tunin
     res = None
     if rank == 0:
         inst_general = fp64_inst_per_evpt(wl.model)
-        gen = fp64_per_general_term(n_terms(wl.model))
-        inst = inst_general - (gen - FP64_SMALL_TERM) * small_frac - (gen - FP64_MEDIUM_TERM) * medium_frac   # executed
         small = P <= 16 and not (n_terms(wl.model) == 3 and P > 4)      # the small-batch kernel (setup fused in) ran
+        if small:
+            # the single-launch kernel keeps the unfolded forms: 11 per general term, 7 for a small-phase last term
+            inst_general = 11 * n_terms(wl.model)
+            inst = inst_general - (11 - 7) * small_frac
+        else:
+            gen = fp64_per_general_term(n_terms(wl.model))
+            inst = inst_general - (gen - FP64_SMALL_TERM) * small_frac - (gen - FP64_MEDIUM_TERM) * medium_frac   # executed
         sp = stats_ms(sp_ms)
         sm_max_mhz = (clocks or {}).get("sm_max_mhz") or 1965.0
         sm_count = torch.cuda.get_device_properties(local).multi_processor_count
