@@ -101,9 +101,9 @@ void free_all(phylino_ctx *c)
     free_tables(c);
     cudaFree(c->d_acc); cudaFree(c->d_flags);
     c->d_acc = nullptr; c->d_flags = nullptr; c->acc_capacity = 0;
-    cudaFree(c->d_rec); cudaFree(c->d_thr); cudaFree(c->d_safe); cudaFree(c->d_counter); cudaFree(c->d_done); cudaFree(c->d_med); cudaFree(c->d_grad_plan);
+    cudaFree(c->d_rec); cudaFree(c->d_thr); cudaFree(c->d_safe); cudaFree(c->d_counter); cudaFree(c->d_done); cudaFree(c->d_med); cudaFree(c->d_grad_plan); cudaFree(c->d_unit_order);
     cudaFree(c->d_small);
-    c->d_rec = nullptr; c->d_thr = nullptr; c->d_safe = nullptr; c->d_counter = nullptr; c->d_done = nullptr; c->d_med = nullptr; c->d_grad_plan = nullptr; c->grad_plan_state = 0;
+    c->d_rec = nullptr; c->d_thr = nullptr; c->d_safe = nullptr; c->d_counter = nullptr; c->d_done = nullptr; c->d_med = nullptr; c->d_grad_plan = nullptr; c->grad_plan_state = 0; c->d_unit_order = nullptr; c->order_U = c->order_units = 0;
     c->d_small = nullptr;
     c->point_capacity = 0;
     cudaFree(c->d_plan); c->d_plan = nullptr; c->plan_capacity = 0;
@@ -230,6 +230,59 @@ void fill_datasets(const phylino_ctx *ctx, SpectraArgs &a)
  * (tickets) -> 0.062 / 0.082 / 0.178 ms (two-term models); on config 4's store (three terms, 410 bins) 1 / 2 points
  * 0.142 / 0.143 -> 0.084 / 0.114 ms, even at 4, slower from 8.  Larger batches are faster with the tickets
  * (config 2: 0.21 ms against 0.29 ms static). */
+/* Order in which the single-launch kernel hands out its units: those nearest a bin edge FIRST, those in the middle of
+ * a bin last.  A call for a few points is as long as its slowest warp, and a warp that meets a bin edge is 1-2.5 us
+ * late (the event-by-event path through cold instruction lines; round-2 timeline: median warp done at 20 us, the last
+ * at 27-30 us, all of the late ones had met an edge).  Met early, the delay is absorbed by the tickets -- a late warp
+ * claims fewer units; met in a warp's last unit, it is the end of the call.  "Nearest" under the identity energy scale,
+ * in units of the local bin width: the real edges move with the energy-scale parameters, by far less than half a bin.
+ * The order changes no result (the accumulators are integers).  One table per (store, unit length), built at the
+ * first small-batch call and kept on the device. */
+phylino_status build_unit_order(phylino_ctx *ctx, int64_t U, int64_t units)
+{
+    std::vector<std::pair<float, int32_t>> key;
+    key.reserve((size_t)units);
+    int32_t unit = 0;
+    for (int d = 0; d < ctx->n_datasets; ++d) {
+        const phylino_dataset_host &h = ctx->ds[d];
+        const int64_t nb = h.n_pad / EB;
+        const int B = h.n_bins;
+        const int64_t n_blk = (int64_t)h.v_blk.size();
+        for (int64_t b0 = 0; b0 < nb; b0 += U, ++unit) {
+            const int64_t b1 = std::min(b0 + U, nb);
+            /* [va, vb] contains every E_vis of the unit: first event of the block b0 falls in, first event of the first
+             * block at or after b1 (the store is sorted; the largest value of the dataset past the last block) */
+            const float va = h.v_blk[(size_t)(b0 / HINT_BATCHES)];
+            const int64_t kb = (b1 + HINT_BATCHES - 1) / HINT_BATCHES;
+            float vb = kb < n_blk ? h.v_blk[(size_t)kb] : h.v_max;
+            if (!(vb == vb)) vb = h.v_max;              /* a block of padding / NaN events */
+            float dist = 1.0e30f;                       /* no finite event: never at an edge */
+            if (va == va && vb == vb) {
+                const double *e = h.edges.data();
+                const int i = (int)(std::upper_bound(e, e + B + 1, (double)va) - e) - 1;     /* -1 ... B */
+                if (i < 0)       dist = (float)((e[0] - (double)vb) / (e[1] - e[0]));
+                else if (i >= B) dist = (float)(((double)va - e[B]) / (e[B] - e[B - 1]));
+                else             dist = (float)(std::min((double)va - e[i], e[i + 1] - (double)vb) / (e[i + 1] - e[i]));
+                if (!(dist > 0.0f)) dist = 0.0f;        /* an edge inside the unit */
+            }
+            key.emplace_back(dist, unit);
+        }
+    }
+    if ((int64_t)key.size() != units) return fail(ctx, PHYLINO_ERR_STATE, "unit order: %lld units expected, %lld found", (long long)units, (long long)key.size());
+    std::stable_sort(key.begin(), key.end(), [](const std::pair<float, int32_t> &x, const std::pair<float, int32_t> &y) { return x.first < y.first; });
+    std::vector<int32_t> order((size_t)units);
+    for (int64_t i = 0; i < units; ++i) order[(size_t)i] = key[(size_t)i].second;
+    CU(cudaStreamSynchronize(ctx->stream));             /* a launch in flight may still read the old table */
+    cudaFree(ctx->d_unit_order);
+    ctx->d_unit_order = nullptr;
+    ctx->order_U = ctx->order_units = 0;
+    CU(cudaMalloc((void **)&ctx->d_unit_order, (size_t)std::max<int64_t>(units, 1) * sizeof(int32_t)));
+    CU(cudaMemcpy(ctx->d_unit_order, order.data(), (size_t)units * sizeof(int32_t), cudaMemcpyHostToDevice));
+    ctx->order_U = U;
+    ctx->order_units = units;
+    return PHYLINO_OK;
+}
+
 bool wants_single_launch(const phylino_ctx *ctx, int P)
 {
     if (ctx->schedule == 1) return false;
@@ -292,6 +345,16 @@ phylino_status fill_batch(phylino_ctx *ctx, SpectraArgs &a, int P, const double 
         a.n_chunks = 1;
         a.n_items = (int32_t)units;
         a.n_warps = (int32_t)std::max<int64_t>(WARPS, std::min<int64_t>(fcap, (units + WARPS - 1) / WARPS * WARPS));
+        /* edge-first order of the units -- where there are tickets at all: with at most two units per warp every
+         * unit is a static first item, the order buys nothing and its look-up sits in front of the first copy */
+        a.unit_order = nullptr;
+        if (units > 2ll * a.n_warps) {
+            if (!ctx->d_unit_order || ctx->order_U != U || ctx->order_units != units) {
+                const phylino_status so = build_unit_order(ctx, U, units);
+                if (so != PHYLINO_OK) return so;
+            }
+            a.unit_order = ctx->d_unit_order;
+        }
         return PHYLINO_OK;
     }
 
@@ -965,6 +1028,7 @@ phylino_status phylino_load_events(phylino_ctx *ctx, int dataset, int64_t n, con
      * HINT_BATCHES-th batch under the identity energy scale */
     std::vector<HintEntry> hint((size_t)((n_batches + HINT_BATCHES - 1) / HINT_BATCHES), HintEntry{n_bins, 0.0f});
     std::vector<double> x_blk(hint.size(), 0.0);       /* largest L/E_nu of each block of HINT_BATCHES batches */
+    std::vector<float> v_blk(hint.size(), std::nanf(""));
     double x_max = 0.0;
     for (int64_t i = 0; i < n; ++i) {
         const int32_t s = perm[i];
@@ -984,6 +1048,7 @@ phylino_status phylino_load_events(phylino_ctx *ctx, int dataset, int64_t n, con
             r.w[j] = (double)weight[s];
             r.wsum += r.w[j];                   /* in event order: the batch total the hot kernel adds */
         }
+        if (j == 0 && b % HINT_BATCHES == 0) v_blk[(size_t)(b / HINT_BATCHES)] = vi;
         if (j == 0 && b % HINT_BATCHES == 0)
             hint[(size_t)(b / HINT_BATCHES)].bin =
                 vi == vi ? (int32_t)(std::upper_bound(edges, edges + n_bins + 1, (double)vi) - edges) - 1 : n_bins;
@@ -1024,6 +1089,11 @@ phylino_status phylino_load_events(phylino_ctx *ctx, int dataset, int64_t n, con
     CU(cudaStreamSynchronize(st));
     h.n = n; h.n_pad = n_pad; h.wsum_abs = wsum; h.fx_exp = fx; h.loaded = true;
     h.v_pos_min = v_pos_min; h.v_max = v_max; h.unit_w = unit_w; h.x_max = x_max;
+    h.v_blk.swap(v_blk);
+    h.edges = ed;
+    cudaFree(ctx->d_unit_order);                /* the single-launch kernel's unit order belongs to the old store */
+    ctx->d_unit_order = nullptr;
+    ctx->order_U = ctx->order_units = 0;
     ctx->err.clear();
     return PHYLINO_OK;
 }

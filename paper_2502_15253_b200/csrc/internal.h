@@ -120,6 +120,8 @@ struct SpectraArgs {
     int32_t sched;          /* 0: items claimed from the counter; 1: one contiguous range of batches per warp, single launch */
     unsigned *counter;      /* DEVICE work counter of the ticket kernel; the setup kernel zeroes it */
     unsigned *done;         /* DEVICE work counter of the single-launch kernel; the finalize kernel behind it zeroes it */
+    const int32_t *unit_order;  /* DEVICE [n_units] single-launch kernel: item -> unit, the units nearest a bin edge
+                                   first (api.cu build_unit_order); NULL: item = unit */
     unsigned long long *med_count;  /* DEVICE event x point evaluations whose first term took the no-reduction form
                                        (phylino_last_medium_phase); the setup kernel zeroes it */
     int32_t  *dbg_bins;     /* DEVICE [P x total_events] diagnostic instantiation: bin the hot loop gave every event */
@@ -256,6 +258,8 @@ struct phylino_dataset_host {
     double   x_max = 0.0;
     void    *d_ev = nullptr;                        /* EventBatchU[] if unit_w else EventBatchW[] */
     phylino::HintEntry *d_hint = nullptr;
+    std::vector<float>  v_blk;                     /* E_vis of the first event of every block of HINT_BATCHES batches */
+    std::vector<double> edges;                     /* host copy of the bin edges */
     double  *d_edges = nullptr;
     int32_t *d_perm = nullptr;
 };
@@ -321,6 +325,8 @@ struct phylino_ctx {
     size_t fused_tables = 0;
     int schedule = 0;                              /* phylino_set_schedule: 0 auto, 1 tickets, 2 single launch */
     unsigned *d_done = nullptr;                    /* work counter of the small-batch kernel */
+    int32_t  *d_unit_order = nullptr;              /* its item -> unit table for units of order_U batches */
+    int64_t   order_U = 0, order_units = 0;
     unsigned long long *d_med = nullptr;           /* medium-phase evaluations of the last ticket launch */
     bool last_fused = false;                       /* the last spectra launch was the single-launch kernel */
     phylino::ParamBlob blob{};                     /* a small host batch on its way into the kernel arguments */

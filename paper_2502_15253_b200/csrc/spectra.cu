@@ -838,7 +838,8 @@ __device__ __forceinline__ unsigned take_ticket(unsigned *counter, int lane)
 template <bool SMALL>
 __device__ __forceinline__ void decode_item(const SpectraArgs &a, unsigned item, int &d, int &b0, int &b1, int &chunk)
 {
-    const int unit = SMALL ? (int)item : (int)(item / (unsigned)a.n_chunks);
+    /* SMALL: the units nearest a bin edge are handed out first (api.cu build_unit_order) */
+    const int unit = SMALL ? (a.unit_order ? __ldg(a.unit_order + item) : (int)item) : (int)(item / (unsigned)a.n_chunks);
     chunk = SMALL ? 0 : (int)(item - (unsigned)unit * (unsigned)a.n_chunks);
     if (!SMALL && unit >= a.tail_unit) {
         d = a.n_datasets - 1;
