@@ -211,7 +211,12 @@ __device__ __forceinline__ void finalize_pre(const FinalizeArgs &a, int p, doubl
     if (MODE >= 1 && stage) {
         for (int g = threadIdx.x; g < a.total_bins; g += FIN_THREADS) {
             double m, bsum;
-            bin_model(a, theta, g, a.bin_ds[g], m, bsum);
+            const int d = a.bin_ds[g];
+            bin_model(a, theta, g, d, m, bsum);
+            /* NLL of the plain (dense, per-event energy scale) path: the fixed-point scale 2^-e of the dataset goes
+             * into the multiplier here -- an exact scaling, so m 2^-e q is the same double as m (q 2^-e) -- and the
+             * second half of the kernel reads nothing but the accumulators (no dataset look-up behind the wait) */
+            if (MODE == 2 && !a.comp && !a.ec_mode) m *= a.inv_scale[d];
             stage[g] = m;
             stage[a.total_bins + g] = bsum;
             if (MODE == 2) stage[2 * a.total_bins + g] = a.data[g];
@@ -283,6 +288,22 @@ __device__ __forceinline__ void finalize_post(const FinalizeArgs &a, int p, doub
         }
     } else {
         for (int g = threadIdx.x; g < a.total_bins; g += FIN_THREADS) {
+            if (MODE == 2 && stage && !a.comp) {
+                /* the staged multiplier carries the fixed-point scale (finalize_pre) */
+                long long q = __ldcg(a.acc + row + g);
+                const unsigned fl = __ldcg(a.flags + row + g);
+                if (q) a.acc[row + g] = 0;
+                if (fl) a.flags[row + g] = 0;
+                double Hq = (double)q;
+                if (fl) {
+                    if ((fl & FLAG_NAN) || ((fl & FLAG_PINF) && (fl & FLAG_NINF)))
+                        Hq = __longlong_as_double(0x7ff8000000000000ll);
+                    else
+                        Hq = __longlong_as_double((fl & FLAG_PINF) ? 0x7ff0000000000000ll : 0xfff0000000000000ll);
+                }
+                part += half_deviance(stage[2 * a.total_bins + g], stage[g] * Hq + stage[a.total_bins + g]);
+                continue;
+            }
             const int d = a.bin_ds[g];
             const double H = load_H(a, p, g, d, pre);
             if (MODE == 3) continue;
