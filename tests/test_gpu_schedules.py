@@ -307,3 +307,49 @@ def test_cheaper_forms_are_reached_and_exact(gpu, oracle_mod, k, scale, n_points
         # determinism of the count and of the bits
         h2 = ph.spectra(_dev(wl.params)).cpu().numpy()
         assert np.array_equal(h, h2) and ph.last_medium_phase() == med
+
+
+# ---- the single-launch kernel's edge-first unit order (api.cu build_unit_order) -----------------------------------
+# The order table exists only where warps claim tickets (more than two units per warp); a cap on the warps forces
+# that on small stores.  The order must change no result: bins bit-exact, spectra and NLL at the usual bars, and the
+# same bits as the uncapped launch (integer accumulators: the walk order is immaterial).
+@pytest.mark.parametrize("k,scale", [(2, 0.05), (3, 0.02), (4, 0.01), (5, 0.05)])
+@pytest.mark.parametrize("n_points", [1, 5])
+def test_edge_first_unit_order_changes_nothing(gpu, oracle_mod, k, scale, n_points):
+    wl = workloads.make_config(k, scale=scale)
+    params = wl.params[:n_points].copy()
+    orc = oracle_mod.Oracle(wl.model, wl.events)
+    data = _data(orc, wl)
+    with gpu.Phylino() as ph:
+        ph.load_workload(wl)
+        h_free = ph.spectra(_dev(params)).cpu().numpy()
+        ph.set_tuning(0, 0, 8)                              # 8 warps: every warp claims dozens of tickets
+        h = ph.spectra(_dev(params)).cpu().numpy()
+        nll = ph.nll(_dev(params), _dev(data)).cpu().numpy()
+        bins = ph.event_bins(_dev(params)).cpu().numpy()
+    assert np.array_equal(bins, orc.event_bins(params))
+    _check_hist(h, orc.spectra(params))
+    assert np.abs(nll - orc.nll(params, data)).max() <= ABS_NLL
+    single_launch = n_points <= (16 if wl.model.osc_model == OSC_EQ1 else 4)
+    if single_launch:       # the same cut into units, another walk order: the same bits
+        assert np.array_equal(h, h_free)
+    else:                   # the ticket schedule cuts the units by the number of warps: rounding only
+        assert np.allclose(h, h_free, rtol=1e-13, atol=0.0)
+
+
+def test_one_point_over_the_full_store(gpu, oracle_mod):
+    """The minimiser's single evaluation at full size (config 3: 6e6 events, 11 721 units for 2 364 warps): the
+    launch configuration bench.py times, order table included, against the oracle."""
+    wl = workloads.make_config(3)
+    params = wl.params[:1].copy()
+    orc = oracle_mod.Oracle(wl.model, wl.events)
+    data = _data(orc, wl)
+    with gpu.Phylino() as ph:
+        ph.load_workload(wl)
+        h = ph.spectra(_dev(params)).cpu().numpy()
+        nll = ph.nll(_dev(params), _dev(data)).cpu().numpy()
+        bins = ph.event_bins(_dev(params)).cpu().numpy()
+        assert ph.launch_count == 6                          # 3 calls x (single launch + finalize)
+    assert np.array_equal(bins, orc.event_bins(params))
+    _check_hist(h, orc.spectra(params))
+    assert np.abs(nll - orc.nll(params, data)).max() <= ABS_NLL
