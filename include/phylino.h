@@ -292,9 +292,10 @@ PHYLINO_API int64_t phylino_total_bins(const phylino_ctx *ctx);     /* sum_d n_b
 PHYLINO_API int64_t phylino_total_events(const phylino_ctx *ctx);   /* sum_d n over loaded datasets */
 
 /* Pre-size every per-batch work buffer of the context for batches of up to max_points points (accumulators,
- * per-point records and bin thresholds, pinned staging of the HOST entry points, the transformed batch).  After
- * it, calls with P <= max_points allocate nothing and the DEVICE entry points never synchronise.  Synchronises
- * the stream if anything grows.  PHYLINO_ERR_STATE before the model and all events are loaded. */
+ * per-point records and bin thresholds, pinned staging of the HOST entry points, the transformed batch) and build
+ * what a first call would otherwise build with a synchronisation (kernel occupancies, the unit order of the
+ * single-launch kernel).  After it, calls with P <= max_points allocate nothing and the DEVICE entry points never
+ * synchronise.  Synchronises the stream if anything grows.  PHYLINO_ERR_STATE before the model and all events are loaded. */
 PHYLINO_API phylino_status phylino_reserve(phylino_ctx *ctx, int max_points);
 
 /* Which kernels evaluate a batch: 0 (default) the library chooses -- ONE launch of the single-launch kernel for

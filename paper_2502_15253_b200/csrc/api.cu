@@ -1530,6 +1530,18 @@ phylino_status phylino_reserve(phylino_ctx *ctx, int max_points)
         CU(cudaMalloc((void **)&ctx->d_theta, need * sizeof(double)));
         ctx->theta_capacity = need;
     }
+    /* everything else a first call would set up with a synchronisation: the occupancy of the kernels, and the
+     * single-launch kernel's edge-first unit order (a function of the store alone at the default unit length) */
+    for (int P = 1; P <= std::min(max_points, FUSED_MAX_POINTS); P *= 2) {
+        SpectraArgs a{};
+        fill_datasets(ctx, a);
+        if ((s = fill_batch(ctx, a, P, nullptr)) != PHYLINO_OK) return s;
+    }
+    {
+        SpectraArgs a{};
+        fill_datasets(ctx, a);
+        if ((s = fill_batch(ctx, a, max_points, nullptr)) != PHYLINO_OK) return s;
+    }
     ctx->err.clear();
     return PHYLINO_OK;
 }

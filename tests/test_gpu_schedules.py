@@ -353,3 +353,30 @@ def test_one_point_over_the_full_store(gpu, oracle_mod):
     assert np.array_equal(bins, orc.event_bins(params))
     _check_hist(h, orc.spectra(params))
     assert np.abs(nll - orc.nll(params, data)).max() <= ABS_NLL
+
+
+def test_reserve_leaves_nothing_to_set_up_for_a_single_evaluation(gpu, oracle_mod):
+    """phylino.h: after phylino_reserve the DEVICE entry points never synchronise -- also not the FIRST one-point call,
+    which needs kernel occupancies and the single-launch kernel's unit order: captured into a CUDA graph cold (a
+    synchronisation or a blocking copy inside the call would fail the capture), replayed, checked against the oracle."""
+    import torch
+    wl = workloads.make_config(2, scale=0.05)
+    orc = oracle_mod.Oracle(wl.model, wl.events)
+    data = _data(orc, wl)
+    params = wl.params[:1].copy()
+    st = torch.cuda.Stream()
+    with torch.cuda.stream(st):
+        ph = gpu.Phylino(stream=st.cuda_stream)
+        ph.load_workload(wl)
+        ph.set_tuning(0, 0, 8)                  # few warps: the unit order table is needed
+        ph.reserve(4)
+        dp, dd = _dev(params), _dev(data)
+        out = torch.zeros(1, dtype=torch.float64, device="cuda")
+        st.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=st):
+            ph.nll(dp, dd, out)                 # the first call of this context
+        g.replay()
+        st.synchronize()
+        assert np.abs(out.cpu().numpy() - orc.nll(params, data)).max() <= ABS_NLL
+    ph.close()
