@@ -298,15 +298,17 @@ PHYLINO_API int64_t phylino_total_events(const phylino_ctx *ctx);   /* sum_d n o
  * synchronise.  Synchronises the stream if anything grows.  PHYLINO_ERR_STATE before the model and all events are loaded. */
 PHYLINO_API phylino_status phylino_reserve(phylino_ctx *ctx, int max_points);
 
-/* Which kernels evaluate a batch: 0 (default) the library chooses -- ONE launch of the single-launch kernel for
- * small batches (at most 16 points with two oscillation terms, 4 with three: the minimiser's single evaluations;
- * setup, event walk and likelihood in one kernel), else the setup / spectra / finalize kernels with the work-item
- * tickets; 1 always the three kernels; 2 the single launch for every batch of at most 16 points.  Results agree
+/* Which kernels evaluate a batch: 0 (default) the library chooses -- the single-launch kernel for small batches
+ * (at most 16 points with two oscillation terms, 4 with three: the minimiser's single evaluations; setup and event
+ * walk in one kernel, the finalize kernel behind it as its programmatic dependent), else the setup / spectra /
+ * finalize kernels with the work-item tickets; 1 always the three kernels; 2 the single-launch kernel for every
+ * batch of at most 16 points.  Results agree
  * to rounding (another grouping of the fp64 partial sums); for tests and measurements. */
 PHYLINO_API phylino_status phylino_set_schedule(phylino_ctx *ctx, int mode);
 
 /* Tuning knobs (0 => library default).  unit_events: events per unit of the event store (a unit is staged in
- * shared memory: values above 256 are clamped to 256; the last stretch of the store is always cut finer);
+ * shared memory: values above 256 -- 512 where every dataset has unit weights -- are clamped; the last stretch of
+ * the store is always cut finer);
  * chunk_groups: groups of 32 parameter points per work item (a warp of the spectra kernel walks one
  * unit for every group of an item, then claims the next item); max_warps: cap on the warps of the
  * persistent grid.  Results are bit-identical from call to call for fixed knobs; other values
@@ -340,7 +342,8 @@ PHYLINO_API phylino_status phylino_last_kernel_ms(phylino_ctx *ctx, float *ms);
 
 /* Which arithmetic the last spectra launch of this context ran (for the roofline accounting of bench.py): the
  * fraction, weighted by events x points, of (point group, dataset) pairs whose LAST oscillation term took the
- * small-phase form of 1/2 cos(2 phase) -- 7 fp64 instructions per event x point instead of 11.  The kernels pick it
+ * small-phase form of 1/2 cos(2 phase) -- 6 fp64 instructions per event x point instead of 10 or 11 (7 in the
+ * single-launch kernel for at most 16 points).  The kernels pick it
  * per group of 32 points and dataset where |1.267 dm2 (2/pi) L/E| <= 1/8 for every event and point (the solar term
  * at Double-Chooz baselines).  fraction HOST; synchronises the stream. */
 PHYLINO_API phylino_status phylino_last_small_phase(phylino_ctx *ctx, double *fraction_host);
