@@ -51,6 +51,14 @@ class _PriorBlock(C.Structure):
     _fields_ = [("n", C.c_int32), ("idx", C.c_void_p), ("mean", C.c_void_p), ("inv_cov", C.c_void_p)]
 
 
+class _Monomial(C.Structure):
+    _fields_ = [("coef", C.c_double), ("n_factors", C.c_int32), ("idx", C.c_void_p), ("power", C.c_void_p)]
+
+
+class _Function(C.Structure):
+    _fields_ = [("offset", C.c_double), ("n_terms", C.c_int32), ("terms", C.POINTER(_Monomial))]
+
+
 class _TransformBlock(C.Structure):
     _fields_ = [("n_out", C.c_int32), ("n_in", C.c_int32), ("idx_out", C.c_void_p), ("idx_in", C.c_void_p),
                 ("offset", C.c_void_p), ("centre", C.c_void_p), ("matrix", C.c_void_p)]
@@ -61,7 +69,8 @@ class _Model(C.Structure):
                 ("n_datasets", C.c_int32), ("idx_osc", C.c_int32 * 6), ("fixed_osc", C.c_double * 6),
                 ("datasets", C.POINTER(_Dataset)), ("prior_mean", C.c_void_p), ("prior_sigma", C.c_void_p),
                 ("n_prior_blocks", C.c_int32), ("prior_blocks", C.POINTER(_PriorBlock)),
-                ("energy_correction", C.c_int32)]
+                ("energy_correction", C.c_int32),
+                ("n_functions", C.c_int32), ("functions", C.POINTER(_Function))]
 
 
 _lib = None
@@ -99,6 +108,8 @@ def _load():
         lib.orc_flux_scales.argtypes = [C.POINTER(_Dataset), dp, dp, dp]
         lib.orc_nll_from_mu.restype = C.c_int
         lib.orc_nll_from_mu.argtypes = [C.POINTER(_Model), C.c_int32, dp, dp, dp, dp]
+        lib.orc_function_value.restype = C.c_double
+        lib.orc_function_value.argtypes = [C.POINTER(_Function), dp]
         lib.orc_nll.restype = C.c_int
         lib.orc_nll.argtypes = [C.POINTER(_Model), C.POINTER(_Events), C.c_int32, dp, dp, dp, C.c_int]
         lib.orc_transform.restype = C.c_int
@@ -198,6 +209,23 @@ class Oracle:
         m.n_prior_blocks = len(blocks)
         m.prior_blocks = C.cast(pb, C.POINTER(_PriorBlock)) if blocks else None
         m.energy_correction = int(getattr(model, "energy_correction", 0))
+        funcs = list(getattr(model, "functions", None) or [])
+        fa = (_Function * max(1, len(funcs)))()
+        for k, f in enumerate(funcs):
+            ta = (_Monomial * max(1, len(f.terms)))()
+            for j, (coef, idx, power) in enumerate(f.terms):
+                assert len(idx) == len(power)
+                ta[j].coef = float(coef)
+                ta[j].n_factors = len(idx)
+                ta[j].idx = self._arr(idx, np.int32)
+                ta[j].power = self._arr(power, np.int32)
+            self._keep.append(ta)
+            fa[k].offset = float(f.offset)
+            fa[k].n_terms = len(f.terms)
+            fa[k].terms = C.cast(ta, C.POINTER(_Monomial))
+        self._keep.append(fa)
+        m.n_functions = len(funcs)
+        m.functions = C.cast(fa, C.POINTER(_Function)) if funcs else None
         return m
 
     def _marshal_events(self, events):
@@ -280,6 +308,13 @@ class Oracle:
     def _keep_edges(self, dataset: int) -> np.ndarray:
         n = self.model.datasets[dataset].n_bins
         return np.ctypeslib.as_array(self._edges[dataset], shape=(n + 1,)).copy()
+
+    def function_values(self, theta) -> np.ndarray:
+        """b_f(theta) of the model's constrained functions (R29) at one point."""
+        th = _f64(theta)
+        assert th.shape == (self.model.n_params,)
+        return np.array([_load().orc_function_value(C.byref(self._m.functions[f]), _dp(th))
+                         for f in range(self._m.n_functions)])
 
     def nll_from_mu(self, params, mu, data) -> np.ndarray:
         p = self._params(params)

@@ -376,6 +376,33 @@ double orc_dev(double n, double mu)
     return NAN;                                  /* negative counts are not data */
 }
 
+/* a constrained quantity b(theta) that is a function of the fitted parameters (R29) */
+double orc_function_value(const orc_function *f, const double *theta)
+{
+    double v = f->offset;
+    for (int32_t m = 0; m < f->n_terms; ++m) {
+        const orc_monomial *t = &f->terms[m];
+        double term = t->coef;
+        for (int32_t i = 0; i < t->n_factors; ++i) {
+            const double x = theta[t->idx[i]];
+            const int32_t pw = t->power[i], n = pw < 0 ? -pw : pw;
+            if (n == 0) continue;
+            double q = x;
+            for (int32_t r = 1; r < n; ++r) q *= x;
+            if (pw > 0) term *= q; else term /= q;
+        }
+        v += term;
+    }
+    return v;
+}
+
+/* value of entry idx of a prior block: a parameter, or a function of the parameters */
+static double constrained_value(const orc_model *m, const double *theta, int32_t idx)
+{
+    if (idx < m->n_params) return theta[idx];
+    return orc_function_value(&m->functions[idx - m->n_params], theta);
+}
+
 int orc_nll_from_mu(const orc_model *m, int32_t P, const double *params, const double *mu,
                     const double *data, double *nll)
 {
@@ -399,9 +426,9 @@ int orc_nll_from_mu(const orc_model *m, int32_t P, const double *params, const d
         for (int32_t k = 0; k < m->n_prior_blocks; ++k) {
             const orc_prior_block *B = &m->prior_blocks[k];
             for (int32_t i = 0; i < B->n; ++i) {
-                double di = theta[B->idx[i]] - B->mean[i];
+                double di = constrained_value(m, theta, B->idx[i]) - B->mean[i];
                 for (int32_t j = 0; j < B->n; ++j) {
-                    double dj = theta[B->idx[j]] - B->mean[j];
+                    double dj = constrained_value(m, theta, B->idx[j]) - B->mean[j];
                     nsum(&s, &c, 0.5 * di * B->inv_cov[(int64_t)i * B->n + j] * dj);
                 }
             }

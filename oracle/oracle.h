@@ -71,6 +71,25 @@ typedef struct {
     const double  *inv_cov;    /* [n*n] V^-1, row-major */
 } orc_prior_block;
 
+/* A constrained quantity that is a FUNCTION of the fitted parameters ("a generalized parametrization
+ * where the constrained parameters b_i(theta) are functions of the actually fitted nuisance parameters"; the paper
+ * names no function family -- DESIGN.md R29: polynomials with integer powers,
+ *     b(theta) = offset + sum_m coef_m prod_i theta[idx_mi]^power_mi,
+ * which covers affine maps, products (rate x efficiency) and ratios).  A prior block refers to function f through the
+ * index n_params + f. */
+typedef struct {
+    double         coef;
+    int32_t        n_factors;
+    const int32_t *idx;        /* [n_factors] indices into theta */
+    const int32_t *power;      /* [n_factors] integer powers, negative = divide */
+} orc_monomial;
+
+typedef struct {
+    double              offset;
+    int32_t             n_terms;
+    const orc_monomial *terms;
+} orc_function;
+
 typedef struct {
     int32_t            osc_model;    /* ORC_EQ1 / ORC_FULL3 / ORC_STERILE4 */
     int32_t            ordering;     /* +1 normal, -1 inverted (FULL3) */
@@ -85,7 +104,13 @@ typedef struct {
     const orc_prior_block *prior_blocks; /* [n_prior_blocks] or NULL */
     int32_t            energy_correction; /* 0: per event before binning (north_star; R8);
                                              1: on the binned spectrum (PAPER.md:177 step 3; R27) */
+    int32_t             n_functions;  /* constrained functions of theta (R29); prior blocks reach function f */
+    const orc_function *functions;    /* through the index n_params + f */
 } orc_model;
+
+/* b(theta) of one function: offset + sum over the terms, in order, of coef x the factors in order, a factor being
+ * theta^|power| by repeated multiplication, multiplied in (power > 0) or divided out (power < 0); power 0 is 1. */
+double orc_function_value(const orc_function *f, const double *theta);
 
 /* O1-O2: amplitudes A_k and mass splittings m_k [eV^2] of the oscillation terms at one point.
  * Returns the number of terms S (2 or 3).  PAPER.md:34 (Eq. 1), :39 (Eq. 2), BASELINE.json config 5. */
@@ -122,7 +147,8 @@ int orc_expectation(const orc_model *m, const double *const *edges, int32_t P, c
 double orc_dev(double n, double mu);
 
 /* O5: nll[p] = sum_bins dev(n, mu) + 1/2 sum_j ((theta_j - mean_j)/sigma_j)^2
- *             + 1/2 sum_blocks (b - b0)^T V^-1 (b - b0)            (PAPER.md:82 Eq. 6, :119-123 Eq. 9). */
+ *             + 1/2 sum_blocks (b - b0)^T V^-1 (b - b0)            (PAPER.md:82 Eq. 6, :119-123 Eq. 9),
+ * b_i = theta[idx_i], or the function idx_i - n_params of theta where idx_i >= n_params (R29). */
 int orc_nll_from_mu(const orc_model *m, int32_t P, const double *params, const double *mu,
                     const double *data, double *nll);
 

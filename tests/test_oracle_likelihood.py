@@ -204,3 +204,92 @@ def test_prior_block_order_and_asymmetry(oracle_mod):
     base = f(W.PriorBlock(idx, mean, M))
     assert f(W.PriorBlock(idx[perm], mean[perm], M[np.ix_(perm, perm)])) == pytest.approx(base, rel=1e-12, abs=1e-14)
     assert f(W.PriorBlock(idx, mean, 0.5 * (M + M.T))) == pytest.approx(base, rel=1e-12, abs=1e-14)
+
+
+# ---- constrained FUNCTIONS of the fitted parameters ("b_i(theta) are functions of the actually fitted
+# nuisance parameters"; R29: polynomials with integer powers; a block reaches function f as n_params + f) --
+
+def _fn(terms, offset=0.0):
+    return W.FunctionSpec(terms=[(c, np.array(i, np.int32), np.array(p, np.int32)) for c, i, p in terms], offset=offset)
+
+
+def _toy_with_functions(functions, blocks):
+    m = _toy_with_blocks(blocks)
+    m.functions = functions
+    return m
+
+
+def test_function_value_exact_rationals(oracle_mod):
+    """b = 3/4 - 5/2 th1^2 th4 + 7 th2^-3 + 1/8 th0 th1^-1 th6^2 on dyadic arguments: every product and sum is exact
+    in binary floating point, so the result must equal the rational arithmetic bit for bit -- a wrong power, a
+    dropped factor, a swapped index or a sign all show."""
+    from fractions import Fraction as F
+    th = np.array([1.5, -0.75, 2.0, 9.0, 0.625, 3.0, -4.0])
+    f = _fn([(-2.5, [1, 4], [2, 1]), (7.0, [2], [-3]), (0.125, [0, 1, 6], [1, -1, 2]), (11.0, [3], [0])], offset=0.75)
+    t = [F(x) for x in th]
+    want = F(3, 4) - F(5, 2) * t[1] ** 2 * t[4] + F(7) / t[2] ** 3 + F(1, 8) * t[0] / t[1] * t[6] ** 2 + 11
+    o = oracle_mod.Oracle(_toy_with_functions([f], []))
+    assert o.function_values(th)[0] == float(want)
+
+
+def test_function_identity_is_the_raw_parameter_prior(oracle_mod):
+    """b(theta) = theta_j: a block over functions must give exactly what the same block over the parameters gives."""
+    s1, s2, rho = 0.03, 0.2, -0.6
+    Vi = np.linalg.inv(np.array([[s1 * s1, rho * s1 * s2], [rho * s1 * s2, s2 * s2]]))
+    mean = np.array([1.0, 0.9])
+    raw = W.PriorBlock(idx=np.array([4, 1], np.int32), mean=mean, inv_cov=Vi)
+    fns = [_fn([(1.0, [4], [1])]), _fn([(1.0, [1], [1])])]
+    via = W.PriorBlock(idx=np.array([7 + 0, 7 + 1], np.int32), mean=mean, inv_cov=Vi)
+    a = oracle_mod.Oracle(_toy_with_blocks([raw]))
+    b = oracle_mod.Oracle(_toy_with_functions(fns, [via]))
+    rng = np.random.default_rng(11)
+    mu, n = np.array([[4.0, 6.0]]), np.array([3.0, 9.0])
+    for _ in range(20):
+        th = _toy_model().prior_mean + rng.normal(0, 0.1, 7)
+        assert b.nll_from_mu(th, mu, n)[0] == a.nll_from_mu(th, mu, n)[0]
+
+
+def test_function_priors_against_mpmath(oracle_mod):
+    """A Gaussian constraint on a product over a ratio, b = th0 th4 / th2, and a correlated pair (b, c) with
+    c = 2 th1 - th5^2 + 1/2, typed here from Eq. 6 / Eq. 9 with 50 digits."""
+    import mpmath as mp
+    mp.mp.dps = 50
+    fb = _fn([(1.0, [0, 4, 2], [1, 1, -1])])
+    fc = _fn([(2.0, [1], [1]), (-1.0, [5], [2])], offset=0.5)
+    sb = 0.07
+    s1, s2, rho = 0.05, 0.3, 0.4
+    V = np.array([[s1 * s1, rho * s1 * s2], [rho * s1 * s2, s2 * s2]])
+    blocks = [W.PriorBlock(idx=np.array([7], np.int32), mean=np.array([1.1]), inv_cov=np.array([[1.0 / sb ** 2]])),
+              W.PriorBlock(idx=np.array([7, 8], np.int32), mean=np.array([1.0, 1.4]), inv_cov=np.linalg.inv(V))]
+    o = oracle_mod.Oracle(_toy_with_functions([fb, fc], blocks))
+    rng = np.random.default_rng(3)
+    for _ in range(10):
+        th = np.array([1.0, 0.95, 1.0, 1.0, 1.04, 1.0, 0.0]) + rng.normal(0, 0.05, 7)
+        t = [mp.mpf(float(x)) for x in th]
+        b = t[0] * t[4] / t[2]
+        c = 2 * t[1] - t[5] ** 2 + mp.mpf("0.5")
+        Vi = mp.matrix(np.linalg.inv(V).tolist())
+        d = mp.matrix([b - 1, c - mp.mpf("1.4")])
+        want = ((b - mp.mpf("1.1")) / mp.mpf(sb)) ** 2 / 2 + (d.T * Vi * d)[0] / 2
+        got = o.nll_from_mu(th, np.array([[4.0, 6.0]]), np.array([4.0, 6.0]))[0]
+        assert got == pytest.approx(float(want), rel=1e-12)
+
+
+def test_function_prior_gradient(oracle_mod):
+    """d/d theta_k of 1/2 ((b - b0)/sigma)^2 = (b - b0)/sigma^2 db/dtheta_k with db/dtheta by hand, against a central
+    difference of the oracle."""
+    f = _fn([(3.0, [0, 4], [2, 1]), (-1.0, [2], [-1])], offset=0.2)          # b = 3 th0^2 th4 - 1/th2 + 0.2
+    b0, sg = 2.0, 0.5
+    blk = W.PriorBlock(idx=np.array([7], np.int32), mean=np.array([b0]), inv_cov=np.array([[1.0 / sg ** 2]]))
+    o = oracle_mod.Oracle(_toy_with_functions([f], [blk]))
+    th = np.array([0.9, 1.0, 1.3, 1.0, 0.8, 1.0, 0.0])
+    mu, n = np.array([[4.0, 6.0]]), np.array([4.0, 6.0])
+    b = 3 * th[0] ** 2 * th[4] - 1 / th[2] + 0.2
+    grad = {0: 6 * th[0] * th[4], 4: 3 * th[0] ** 2, 2: 1 / th[2] ** 2, 1: 0.0}
+    for k, db in grad.items():
+        h = 1e-6
+        up, dn = th.copy(), th.copy()
+        up[k] += h
+        dn[k] -= h
+        num = (o.nll_from_mu(up, mu, n)[0] - o.nll_from_mu(dn, mu, n)[0]) / (2 * h)
+        assert num == pytest.approx((b - b0) / sg ** 2 * db, rel=1e-6, abs=1e-7)

@@ -11,7 +11,7 @@ PAPER.md:228) are not public; the recipes here take their shapes, sizes and valu
 distributions from PAPER.md (§3.2–3.3, §4.1, §4.3) and BASELINE.json `configs` and stand
 in for them.  The recipes are restated in DESIGN.md §"Input recipe".
 """
-from .spec import (BkgSpec, DatasetSpec, DatasetEvents, FluxModel, ModelSpec, PriorBlock, TransformBlock,  # noqa: F401
+from .spec import (BkgSpec, DatasetSpec, DatasetEvents, FluxModel, FunctionSpec, ModelSpec, PriorBlock, TransformBlock,  # noqa: F401
                    TransformSpec, Workload)
 from .generate import (  # noqa: F401
     CONFIG_NAMES,

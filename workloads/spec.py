@@ -77,6 +77,15 @@ class PriorBlock:
 
 
 @dataclass
+class FunctionSpec:
+    """A constrained quantity that is a function of the fitted parameters (R29):
+    b(theta) = offset + sum over terms of coef * prod_i theta[idx_i] ** power_i, integer powers.  A PriorBlock
+    refers to function f of the model through the index n_params + f."""
+    terms: list               # [(coef, idx int32 [k], power int32 [k]), ...]
+    offset: float = 0.0
+
+
+@dataclass
 class TransformBlock:
     """theta[idx_out] = offset + matrix (u[idx_in] - centre): one block of the transformation layer between the
     minimiser's parameters u and the model parameters theta (the 9 <- 7 energy-response map of
@@ -107,6 +116,7 @@ class ModelSpec:
     prior_mean: Optional[np.ndarray] = None   # float64 [n_params]
     prior_sigma: Optional[np.ndarray] = None  # float64 [n_params]; <= 0 or inf => unconstrained
     prior_blocks: List[PriorBlock] = field(default_factory=list)
+    functions: List[FunctionSpec] = field(default_factory=list)   # constrained functions of theta
     energy_correction: int = 0              # 0: per event before binning (north_star); 1: on the bins (PAPER.md:177 step 3)
 
     @property
