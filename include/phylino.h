@@ -121,12 +121,34 @@ typedef struct {
  * HOST pointers, deep-copied. */
 typedef struct {
     int32_t        n;          /* parameters in the block, 1 ... PHYLINO_MAX_BLOCK */
-    const int32_t *idx;        /* HOST [n] indices into theta, each 0 ... n_params-1 */
+    const int32_t *idx;        /* HOST [n] indices into theta, each 0 ... n_params-1; or n_params + f for the
+                                  constrained function f of phylino_set_functions */
     const double  *mean;       /* HOST [n] central values b0 */
     const double  *inv_cov;    /* HOST [n*n] INVERSE covariance V^-1, row-major; used as written (an
                                   unsymmetric matrix counts as its symmetric part) */
 } phylino_prior_block;
 #define PHYLINO_MAX_BLOCK 1024
+
+/* A constrained quantity that is a FUNCTION of the fitted parameters ("a generalized parametrization where
+ * the constrained parameters b_i(theta) are functions of the actually fitted nuisance parameters"; the paper names no
+ * function family -- DESIGN.md R29: polynomials with integer powers),
+ *     b(theta) = offset + sum_m coef_m prod_i theta[idx_mi]^power_mi :
+ * affine maps, products (rate x efficiency), ratios.  Evaluated as written: the terms in order, inside a term the
+ * factors in order, a factor being theta^|power| by repeated multiplication, multiplied in (power > 0) or divided out
+ * (power < 0); power 0 is 1.  HOST pointers, deep-copied. */
+typedef struct {
+    double         coef;
+    int32_t        n_factors;  /* 0 ... PHYLINO_MAX_FACTORS */
+    const int32_t *idx;        /* HOST [n_factors] indices into theta */
+    const int32_t *power;      /* HOST [n_factors], |power| <= PHYLINO_MAX_POWER */
+} phylino_monomial;
+typedef struct {
+    double                  offset;
+    int32_t                 n_terms;
+    const phylino_monomial *terms;   /* HOST [n_terms] */
+} phylino_function;
+#define PHYLINO_MAX_FACTORS 16
+#define PHYLINO_MAX_POWER   16
 
 /* One block of the transformation layer between the minimiser's parameters u and the model parameters theta
  * ("A transformation layer applies the covariance of any changed model parameter within the
@@ -272,6 +294,15 @@ PHYLINO_API phylino_status phylino_set_flux_model(phylino_ctx *ctx, int dataset,
  * PHYLINO_ERR_SHAPE for n or an index out of range, PHYLINO_ERR_ARG for NULL arrays or non-finite
  * mean / inv_cov entries. */
 PHYLINO_API phylino_status phylino_set_prior_blocks(phylino_ctx *ctx, int n_blocks, const phylino_prior_block *blocks);
+
+/* Constrained functions of the parameters (R29).  After this call a prior block may name function f
+ * (0 ... n_functions-1) through the index n_params + f: 1/2 (b - b0)^T V^-1 (b - b0) then runs over b_i = theta[idx_i] or
+ * b_i = function value; a Gaussian constraint on one function is a block of one with inv_cov = 1/sigma^2.  With a
+ * transformation layer the functions are functions of theta = T(u).  Call after phylino_set_model (which clears them)
+ * and BEFORE the blocks that use them; replacing the functions by fewer than the current blocks reference is
+ * PHYLINO_ERR_STATE.  n_functions = 0 clears.  Synchronises the stream.  PHYLINO_ERR_SHAPE for an index or a power out
+ * of range, PHYLINO_ERR_ARG for NULL arrays or non-finite coefficients. */
+PHYLINO_API phylino_status phylino_set_functions(phylino_ctx *ctx, int n_functions, const phylino_function *functions);
 
 /* Transformation layer.  After this call every `params` argument (DEVICE or HOST) is a batch of the minimiser's
  * vectors u, [P x n_u] row-major, and the library forms theta itself before anything else:

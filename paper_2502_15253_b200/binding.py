@@ -27,7 +27,7 @@ abi_symbols = (
     "phylino_launch_floor", "phylino_set_schedule", "phylino_reserve",
     "phylino_draw_pseudo_data", "phylino_ordering_scan", "phylino_nll_gradient",
     "phylino_set_energy_correction_mode", "phylino_set_flux_model", "phylino_last_small_phase",
-    "phylino_hbm_read_floor", "phylino_last_medium_phase",
+    "phylino_hbm_read_floor", "phylino_last_medium_phase", "phylino_set_functions",
 )
 
 _STATUS = {0: "OK", 1: "ERR_ARG", 2: "ERR_SHAPE", 3: "ERR_STATE", 4: "ERR_OOM", 5: "ERR_CUDA"}
@@ -51,6 +51,14 @@ class _Dataset(C.Structure):
 
 class _PriorBlock(C.Structure):
     _fields_ = [("n", C.c_int32), ("idx", C.c_void_p), ("mean", C.c_void_p), ("inv_cov", C.c_void_p)]
+
+
+class _Monomial(C.Structure):
+    _fields_ = [("coef", C.c_double), ("n_factors", C.c_int32), ("idx", C.c_void_p), ("power", C.c_void_p)]
+
+
+class _Function(C.Structure):
+    _fields_ = [("offset", C.c_double), ("n_terms", C.c_int32), ("terms", C.POINTER(_Monomial))]
 
 
 class _TransformBlock(C.Structure):
@@ -119,6 +127,8 @@ def load_library():
     lib.phylino_nll_ensemble.argtypes = [vp, i32, vp, i32, vp, vp]
     lib.phylino_set_prior_blocks.restype = i32
     lib.phylino_set_prior_blocks.argtypes = [vp, i32, C.POINTER(_PriorBlock)]
+    lib.phylino_set_functions.restype = i32
+    lib.phylino_set_functions.argtypes = [vp, i32, C.POINTER(_Function)]
     lib.phylino_set_caching.restype = i32
     lib.phylino_set_caching.argtypes = [vp, i32]
     lib.phylino_last_plan.restype = i32
@@ -272,6 +282,9 @@ class Phylino:
     def load_workload(self, wl):
         """set_model + load_events for every dataset of a `workloads.Workload`."""
         self.set_model(wl.model)
+        functions = list(getattr(wl.model, "functions", None) or [])
+        if functions:
+            self.set_functions(functions)
         blocks = list(getattr(wl.model, "prior_blocks", None) or [])
         if blocks:
             self.set_prior_blocks(blocks)
@@ -418,6 +431,30 @@ class Phylino:
             and out.numel() == p.shape[0] * self.total_bins
         self._check(self._lib.phylino_expectation(self._ctx, int(p.shape[0]), p.data_ptr(), out.data_ptr()))
         return out
+
+    def set_functions(self, functions: Sequence = ()):
+        """constrained functions of theta (PAPER.md:80): each has .offset and .terms = [(coef, idx, power), ...];
+        a prior block names function f as n_params + f.  Empty clears."""
+        functions = list(functions)
+        keep = []
+        arr = (_Function * max(1, len(functions)))()
+        for k, f in enumerate(functions):
+            ta = (_Monomial * max(1, len(f.terms)))()
+            for j, (coef, idx, power) in enumerate(f.terms):
+                idx = np.ascontiguousarray(idx, dtype=np.int32)
+                power = np.ascontiguousarray(power, dtype=np.int32)
+                if idx.shape != power.shape or idx.ndim != 1:
+                    raise ValueError("function term: idx and power must be 1-d arrays of equal length")
+                keep += [idx, power]
+                ta[j].coef = float(coef)
+                ta[j].n_factors = int(idx.shape[0])
+                ta[j].idx = idx.ctypes.data
+                ta[j].power = power.ctypes.data
+            keep.append(ta)
+            arr[k].offset = float(f.offset)
+            arr[k].n_terms = len(f.terms)
+            arr[k].terms = C.cast(ta, C.POINTER(_Monomial))
+        self._check(self._lib.phylino_set_functions(self._ctx, len(functions), arr if functions else None))
 
     def set_prior_blocks(self, blocks: Sequence = ()):
         """blocks: objects with .idx [n], .mean [n], .inv_cov [n, n] (workloads.PriorBlock)."""

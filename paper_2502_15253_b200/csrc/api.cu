@@ -80,7 +80,10 @@ void free_tables(phylino_ctx *c)
     cudaFree((void *)f.blk_mean); cudaFree((void *)f.blk_inv);
     cudaFree((void *)f.edges_all); cudaFree((void *)f.ds_bin_off); cudaFree((void *)f.ds_idx_a);
     cudaFree((void *)f.fm_off); cudaFree((void *)f.fm_idx); cudaFree((void *)f.fm_grid);
+    cudaFree((void *)f.fn_offset); cudaFree((void *)f.fn_term_off); cudaFree((void *)f.term_coef);
+    cudaFree((void *)f.term_fac_off); cudaFree((void *)f.fac_idx); cudaFree((void *)f.fac_pow);
     f = FinalizeArgs{};
+    c->max_block_idx = -1;
 }
 
 void free_transform(phylino_ctx *c)
@@ -1390,6 +1393,68 @@ phylino_status phylino_set_transform(phylino_ctx *ctx, int n_u, const int32_t *c
 
 int64_t phylino_param_width(const phylino_ctx *ctx) { return ctx && ctx->have_model ? param_width(ctx) : 0; }
 
+static void free_functions(phylino_ctx *ctx)
+{
+    FinalizeArgs &f = ctx->fin;
+    cudaFree((void *)f.fn_offset); cudaFree((void *)f.fn_term_off); cudaFree((void *)f.term_coef);
+    cudaFree((void *)f.term_fac_off); cudaFree((void *)f.fac_idx); cudaFree((void *)f.fac_pow);
+    f.fn_offset = nullptr; f.fn_term_off = nullptr; f.term_coef = nullptr;
+    f.term_fac_off = nullptr; f.fac_idx = nullptr; f.fac_pow = nullptr;
+    f.n_functions = 0;
+}
+
+phylino_status phylino_set_functions(phylino_ctx *ctx, int n_functions, const phylino_function *functions)
+{
+    if (!ctx) return PHYLINO_ERR_ARG;
+    if (!ctx->have_model) return fail(ctx, PHYLINO_ERR_STATE, "phylino_set_model must come before phylino_set_functions");
+    if (n_functions < 0 || (n_functions > 0 && !functions)) return fail(ctx, PHYLINO_ERR_ARG, "n_functions = %d with NULL functions", n_functions);
+    if (ctx->max_block_idx >= ctx->n_params + n_functions)
+        return fail(ctx, PHYLINO_ERR_STATE, "a prior block names function %d: clear the blocks before removing functions", ctx->max_block_idx - ctx->n_params);
+    std::vector<double> offset, coef;
+    std::vector<int32_t> term_off(1, 0), fac_off(1, 0), fidx, fpow;
+    for (int k = 0; k < n_functions; ++k) {
+        const phylino_function &fn = functions[k];
+        if (!std::isfinite(fn.offset)) return fail(ctx, PHYLINO_ERR_ARG, "function %d: offset is not finite", k);
+        if (fn.n_terms < 0 || (fn.n_terms > 0 && !fn.terms)) return fail(ctx, PHYLINO_ERR_ARG, "function %d: n_terms = %d with NULL terms", k, fn.n_terms);
+        offset.push_back(fn.offset);
+        for (int m = 0; m < fn.n_terms; ++m) {
+            const phylino_monomial &t = fn.terms[m];
+            if (!std::isfinite(t.coef)) return fail(ctx, PHYLINO_ERR_ARG, "function %d term %d: coef is not finite", k, m);
+            if (t.n_factors < 0 || t.n_factors > PHYLINO_MAX_FACTORS) return fail(ctx, PHYLINO_ERR_SHAPE, "function %d term %d: n_factors = %d not in 0..%d", k, m, t.n_factors, PHYLINO_MAX_FACTORS);
+            if (t.n_factors > 0 && (!t.idx || !t.power)) return fail(ctx, PHYLINO_ERR_ARG, "function %d term %d: NULL idx or power", k, m);
+            for (int i = 0; i < t.n_factors; ++i) {
+                if (t.idx[i] < 0 || t.idx[i] >= ctx->n_params) return fail(ctx, PHYLINO_ERR_SHAPE, "function %d term %d: idx[%d] = %d out of range", k, m, i, t.idx[i]);
+                if (t.power[i] < -PHYLINO_MAX_POWER || t.power[i] > PHYLINO_MAX_POWER) return fail(ctx, PHYLINO_ERR_SHAPE, "function %d term %d: power[%d] = %d out of range", k, m, i, t.power[i]);
+                fidx.push_back(t.idx[i]);
+                fpow.push_back(t.power[i]);
+            }
+            coef.push_back(t.coef);
+            fac_off.push_back((int32_t)fidx.size());
+        }
+        term_off.push_back((int32_t)coef.size());
+    }
+    DeviceGuard g(ctx->device);
+    CU(cudaStreamSynchronize(ctx->stream));
+    free_functions(ctx);
+    if (n_functions > 0) {
+        FinalizeArgs &f = ctx->fin;
+        cudaStream_t st = ctx->stream;
+        /* never empty: a function without terms, a term without factors are legal */
+        if (coef.empty()) coef.push_back(0.0);
+        if (fidx.empty()) { fidx.push_back(0); fpow.push_back(0); }
+        CU(upload((double **)&f.fn_offset, offset, st));
+        CU(upload((int32_t **)&f.fn_term_off, term_off, st));
+        CU(upload((double **)&f.term_coef, coef, st));
+        CU(upload((int32_t **)&f.term_fac_off, fac_off, st));
+        CU(upload((int32_t **)&f.fac_idx, fidx, st));
+        CU(upload((int32_t **)&f.fac_pow, fpow, st));
+        CU(cudaStreamSynchronize(st));
+        f.n_functions = n_functions;
+    }
+    ctx->err.clear();
+    return PHYLINO_OK;
+}
+
 phylino_status phylino_set_prior_blocks(phylino_ctx *ctx, int n_blocks, const phylino_prior_block *blocks)
 {
     if (!ctx) return PHYLINO_ERR_ARG;
@@ -1403,7 +1468,8 @@ phylino_status phylino_set_prior_blocks(phylino_ctx *ctx, int n_blocks, const ph
         if (b.n < 1 || b.n > PHYLINO_MAX_BLOCK) return fail(ctx, PHYLINO_ERR_SHAPE, "block %d: n = %d not in 1..%d", k, b.n, PHYLINO_MAX_BLOCK);
         if (!b.idx || !b.mean || !b.inv_cov) return fail(ctx, PHYLINO_ERR_ARG, "block %d: NULL array", k);
         for (int i = 0; i < b.n; ++i) {
-            if (b.idx[i] < 0 || b.idx[i] >= ctx->n_params) return fail(ctx, PHYLINO_ERR_SHAPE, "block %d: idx[%d] = %d out of range", k, i, b.idx[i]);
+            if (b.idx[i] < 0 || b.idx[i] >= ctx->n_params + ctx->fin.n_functions)
+                return fail(ctx, PHYLINO_ERR_SHAPE, "block %d: idx[%d] = %d out of range (%d parameters, %d functions)", k, i, b.idx[i], ctx->n_params, ctx->fin.n_functions);
             if (!std::isfinite(b.mean[i])) return fail(ctx, PHYLINO_ERR_ARG, "block %d: mean[%d] is not finite", k, i);
         }
         for (int64_t i = 0; i < (int64_t)b.n * b.n; ++i)
@@ -1421,7 +1487,9 @@ phylino_status phylino_set_prior_blocks(phylino_ctx *ctx, int n_blocks, const ph
     cudaFree((void *)f.blk_mean); cudaFree((void *)f.blk_inv);
     f.blk_off = nullptr; f.blk_moff = nullptr; f.blk_idx = nullptr; f.blk_mean = nullptr; f.blk_inv = nullptr;
     f.n_blocks = 0;
+    ctx->max_block_idx = -1;
     if (n_blocks > 0) {
+        for (int32_t i : idx) ctx->max_block_idx = std::max(ctx->max_block_idx, i);
         cudaStream_t st = ctx->stream;
         CU(upload((int32_t **)&f.blk_off, off, st));
         CU(upload((int64_t **)&f.blk_moff, moff, st));

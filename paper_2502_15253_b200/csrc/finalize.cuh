@@ -25,6 +25,30 @@ __device__ __forceinline__ double half_deviance(double n, double mu)
     return __longlong_as_double(0x7ff8000000000000ll);     /* negative counts are not data */
 }
 
+/* entry idx of a prior block: a parameter, or a constrained FUNCTION of the parameters (R29):
+ * offset + the terms in order, a term = coef x its factors in order, a factor = theta^|power| by repeated
+ * multiplication, multiplied in or divided out -- the sequence phylino.h states, in plain (unfused) arithmetic */
+__device__ __forceinline__ double constrained_value(const FinalizeArgs &a, const double *theta, int idx)
+{
+    if (idx < a.n_params) return theta[idx];
+    const int f = idx - a.n_params;
+    PHYLINO_ASSERT(f >= 0 && f < a.n_functions);
+    double v = a.fn_offset[f];
+    for (int m = a.fn_term_off[f]; m < a.fn_term_off[f + 1]; ++m) {
+        double term = a.term_coef[m];
+        for (int i = a.term_fac_off[m]; i < a.term_fac_off[m + 1]; ++i) {
+            const double x = theta[a.fac_idx[i]];
+            const int pw = a.fac_pow[i], n = pw < 0 ? -pw : pw;
+            if (n == 0) continue;
+            double q = x;
+            for (int r = 1; r < n; ++r) q *= x;
+            if (pw > 0) term *= q; else term /= q;
+        }
+        v += term;
+    }
+    return v;
+}
+
 /* this thread's share of the prior terms of one point: a fixed strided subset of the parameters and
  * of the rows of every correlated block */
 __device__ __forceinline__ double prior_part(const FinalizeArgs &a, const double *theta)
@@ -45,10 +69,10 @@ __device__ __forceinline__ double prior_part(const FinalizeArgs &a, const double
         const int o = a.blk_off[k], n = a.blk_off[k + 1] - o;
         const double *M = a.blk_inv + a.blk_moff[k];
         for (int i = threadIdx.x; i < n; i += FIN_THREADS) {
-            const double di = theta[a.blk_idx[o + i]] - a.blk_mean[o + i];
+            const double di = constrained_value(a, theta, a.blk_idx[o + i]) - a.blk_mean[o + i];
             double row = 0.0;
             for (int j = 0; j < n; ++j)
-                row = fma(M[(size_t)i * n + j], theta[a.blk_idx[o + j]] - a.blk_mean[o + j], row);
+                row = fma(M[(size_t)i * n + j], constrained_value(a, theta, a.blk_idx[o + j]) - a.blk_mean[o + j], row);
             part += 0.5 * di * row;
         }
     }

@@ -176,6 +176,15 @@ struct FinalizeArgs {
     const int32_t *blk_idx;
     const double  *blk_mean;
     const double  *blk_inv;
+    /* constrained functions of theta (phylino_set_functions, R29), flattened; a block index
+     * >= n_params names function idx - n_params */
+    int32_t        n_functions;
+    const double  *fn_offset;     /* [n_functions] */
+    const int32_t *fn_term_off;   /* [n_functions + 1] offsets into term_coef / term_fac_off */
+    const double  *term_coef;     /* [terms] */
+    const int32_t *term_fac_off;  /* [terms + 1] offsets into fac_idx / fac_pow */
+    const int32_t *fac_idx;
+    const int32_t *fac_pow;
     const double  *data;          /* [total_bins] (NLL mode) */
     double        *hist;          /* [P x total_bins] (spectra / expectation mode) */
     double        *nll;           /* [P] (NLL mode) */
@@ -295,6 +304,7 @@ struct phylino_ctx {
     int64_t last_virtual_points = 0, last_classes = 0;
     phylino::ComponentPlan grad_plan;              /* structural plan of the central-difference batch (phylino_nll_gradient) */
     int grad_plan_state = 0;                       /* 0: not made for this model yet, 1: made, -1: does not pay */
+    int32_t max_block_idx = -1;                    /* largest index any prior block names (functions must cover it) */
     int32_t *d_grad_plan = nullptr;                /* ... on the device: vp_class | vp_src | class_rep | pt_comp */
     /* transformation layer (phylino_set_transform): host copy for the host entry points, device tables */
     bool have_tf = false;

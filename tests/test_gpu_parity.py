@@ -553,3 +553,61 @@ def test_configs_full_size_all_points(gpu, oracle_mod, k, stride, ordering):
     assert err <= 1e-7, err            # where the shipped kernel actually is: ten times inside the bar
     # properties that hold at any size: every point finite, NLL >= 0 (half-deviance + priors)
     assert np.isfinite(nll).all() and (nll >= 0).all()
+
+
+def test_function_priors(gpu, oracle_mod):
+    """PAPER.md:80 ("the constrained parameters b_i(theta) are functions of the actually fitted nuisance parameters";
+    DESIGN.md R29: polynomials with integer powers): on config 3's 301-parameter model a Gaussian constraint on the
+    product (signal normalisation x background rate) of each dataset, one on a ratio of two energy-scale slopes, and a
+    correlated pair (an affine combination of two flux parameters, a square) in one block together with a raw
+    parameter -- dense, host, cached, single-launch and ensemble entry points against the oracle."""
+    wl = workloads.make_config(3, scale=0.003, n_points=75)
+    NP = wl.model.n_params
+    rng = np.random.default_rng(91)
+    i32 = lambda *a: np.array(a, np.int32)
+    F = workloads.FunctionSpec
+    th0 = wl.theta0
+    fns = [F(terms=[(1.0, i32(127 + d, 130 + 3 * d), i32(1, 1))]) for d in range(3)]         # eps_d x rate_d0
+    fns.append(F(terms=[(1.0, i32(5, 8), i32(1, -1))]))                                      # a1(FD-I) / a1(FD-II)
+    fns.append(F(terms=[(2.0, i32(13), i32(1)), (-1.0, i32(14), i32(1))], offset=0.25))      # 2 f_0 - f_1 + 1/4
+    fns.append(F(terms=[(3.0, i32(20), i32(2))]))                                            # 3 f_7^2
+    wl.model.functions = fns
+    orc0 = oracle_mod.Oracle(wl.model, wl.events)
+    b0 = orc0.function_values(th0)
+    A = rng.normal(size=(3, 3))
+    V = (A @ A.T + 0.5 * np.eye(3)) * 1e-3
+    blocks = [workloads.PriorBlock(i32(NP + k), b0[k:k + 1], np.array([[1.0 / (0.05 * abs(b0[k])) ** 2]])) for k in range(4)]
+    blocks.append(workloads.PriorBlock(i32(NP + 4, 30, NP + 5), np.array([b0[4], th0[30], b0[5]]), np.linalg.inv(V)))
+    wl.model.prior_blocks = blocks
+    params = wl.params.copy()
+    params[:, 13:54] += rng.normal(0, 0.02, (params.shape[0], 41))
+    params[:, 127:139] *= 1.0 + rng.normal(0, 0.03, (params.shape[0], 12))
+    orc = oracle_mod.Oracle(wl.model, wl.events)
+    data = _data_for(orc, wl, oracle_mod)
+    nll_o = orc.nll(params, data)
+    with gpu.Phylino() as ph:
+        ph.load_workload(wl)
+        nll = ph.nll(_dev(params), _dev(data)).cpu().numpy()
+        nll_h = ph.nll_host(params, data)
+        nll_1 = np.concatenate([ph.nll(_dev(params[i:i + 3]), _dev(data)).cpu().numpy() for i in (0, 30)])
+        ens = ph.nll_ensemble(_dev(params[:5]), _dev(np.stack([data, data + 1.0]))).cpu().numpy()
+        ph.set_caching(True)
+        nll_c = ph.nll_host(params, data)
+        ph.set_caching(False)
+        # removing functions that blocks still name is refused; blocks first, then functions
+        with pytest.raises(gpu.PhylinoError):
+            ph.set_functions([])
+        ph.set_prior_blocks([])
+        ph.set_functions([])
+        nll_plain = ph.nll(_dev(params), _dev(data)).cpu().numpy()
+        with pytest.raises(gpu.PhylinoError):                   # no functions any more: the index is out of range
+            ph.set_prior_blocks(blocks[:1])
+    assert np.abs(nll - nll_o).max() <= ABS_NLL
+    assert np.array_equal(nll, nll_h)
+    assert np.abs(nll_1 - nll_o[[0, 1, 2, 30, 31, 32]]).max() <= ABS_NLL
+    assert np.abs(nll_c - nll_o).max() <= ABS_NLL
+    assert np.abs(ens[:, 0] - nll_o[:5]).max() <= ABS_NLL
+    assert np.abs(ens[:, 1] - orc.nll(params[:5], data + 1.0)).max() <= ABS_NLL
+    wl.model.prior_blocks, wl.model.functions = [], []
+    assert np.abs(nll_plain - oracle_mod.Oracle(wl.model, wl.events).nll(params, data)).max() <= ABS_NLL
+    assert np.abs(nll_plain - nll).max() > 0.1              # the constraints did contribute
