@@ -4,8 +4,9 @@
 
 Paths: ticket schedule with full groups, a ragged group and sub-streams (70 points), the small-batch kernel with its
 in-CTA tables (1, 5, 16 points), weighted and unit-weight records, bin edges inside units (per-event slow path, general
-sub-stream flush), component mode (caching), the transformation layer, prior blocks, ensembles, pseudo-data, the
-ordering scan, the gradient, the bin-level energy correction with a flux model, the diagnostic instantiation.
+sub-stream flush), the edge-first unit order of the single-launch kernel (capped warps), component mode (caching),
+prior blocks over parameters and over functions of them, ensembles, pseudo-data, the ordering scan, the gradient (dense
+and through the structural plan), the bin-level energy correction with a flux model, the diagnostic instantiation.
 Results are checked against the oracle so that a sanitizer-clean run is also a correct one."""
 import os
 import sys
@@ -70,6 +71,31 @@ def main():
             torch.cuda.synchronize()
             assert np.isfinite(grad.cpu().numpy()).all() and np.isfinite(scan.cpu().numpy()).all()
             n += 8
+    # prior blocks over parameters and over functions of them; the single-launch kernel with few warps (unit order
+    # table); the cached gradient through its structural plan
+    wl = workloads.make_config(3, scale=0.002, n_points=40)
+    NP0 = wl.model.n_params
+    i32 = lambda *a: np.array(a, np.int32)      # noqa: E731
+    wl.model.functions = [workloads.FunctionSpec(terms=[(1.0, i32(127, 130), i32(1, 1))]),
+                          workloads.FunctionSpec(terms=[(2.0, i32(13), i32(1)), (-1.0, i32(5, 8), i32(2, -1))], offset=0.5)]
+    b0 = oracle.Oracle(wl.model, wl.events).function_values(wl.theta0)
+    wl.model.prior_blocks = [workloads.PriorBlock(i32(NP0, 30, NP0 + 1), np.array([b0[0], 1.0, b0[1]]),
+                                                  np.array([[4e2, 1e1, 0.0], [1e1, 9e2, -2e1], [0.0, -2e1, 1e2]]))]
+    orc = oracle.Oracle(wl.model, wl.events)
+    data = np.full(orc.total_bins, 40.0)
+    with pkg.Phylino() as ph:
+        ph.load_workload(wl)
+        assert np.abs(ph.nll(dev(wl.params), dev(data)).cpu().numpy() - orc.nll(wl.params, data)).max() <= 1e-6
+        ph.set_tuning(0, 0, 8)
+        assert np.abs(ph.nll(dev(wl.params[:3]), dev(data)).cpu().numpy() - orc.nll(wl.params[:3], data)).max() <= 1e-6
+        assert np.array_equal(ph.event_bins(dev(wl.params[:1])).cpu().numpy(), orc.event_bins(wl.params[:1]))
+        ph.set_tuning(0, 0, 0)
+        ph.set_caching(True)
+        step = np.full(NP0, 1e-4)
+        nll0, grad = ph.nll_gradient(dev(wl.theta0), dev(step), dev(data))
+        assert ph.last_plan()[0] > 0
+        assert abs(nll0.cpu().numpy()[0] - orc.nll(wl.theta0[None, :], data)[0]) <= 1e-6
+        n += 5
     # the paper's bin-level steps with a flux model
     wl = workloads.make_config(3, scale=0.001, n_points=20)
     NP0 = wl.model.n_params
