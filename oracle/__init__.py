@@ -108,6 +108,8 @@ def _load():
         lib.orc_flux_scales.argtypes = [C.POINTER(_Dataset), dp, dp, dp]
         lib.orc_nll_from_mu.restype = C.c_int
         lib.orc_nll_from_mu.argtypes = [C.POINTER(_Model), C.c_int32, dp, dp, dp, dp]
+        lib.orc_variable_metric_step.restype = C.c_int
+        lib.orc_variable_metric_step.argtypes = [C.c_int32, dp, dp, dp, dp, dp, dp]
         lib.orc_function_value.restype = C.c_double
         lib.orc_function_value.argtypes = [C.POINTER(_Function), dp]
         lib.orc_nll.restype = C.c_int
@@ -385,6 +387,22 @@ def transform(spec, n_params: int, u) -> np.ndarray:
     if rc != 0:
         raise ValueError(f"orc_transform failed ({rc})")
     return theta
+
+
+def variable_metric_step(V, grad, dx=None, dg=None):
+    """One variable-metric step (R30): returns (V_new, direction, edm, skipped)."""
+    V = np.array(V, dtype=np.float64, order="C", copy=True)
+    N = V.shape[0]
+    assert V.shape == (N, N)
+    g = _f64(grad)
+    d = np.zeros(N)
+    edm = np.zeros(1)
+    has = dx is not None and dg is not None
+    a_dx, a_dg = (_f64(dx), _f64(dg)) if has else (None, None)
+    rc = _load().orc_variable_metric_step(N, _dp(V), _dp(a_dx) if has else None, _dp(a_dg) if has else None, _dp(g),
+                                          _dp(d), _dp(edm))
+    assert rc in (0, 1), rc
+    return V, d, float(edm[0]), bool(rc)
 
 
 def max_threads() -> int:

@@ -580,3 +580,48 @@ int orc_draw_pseudo_data(int64_t total_bins_, const double *mu, int32_t E, uint6
     return 0;
 }
 
+
+/* PAPER.md:155; R30: one variable-metric (MIGRAD-type) step: rank-two update of the inverse Hessian estimate,
+ * Newton direction, estimated distance to the minimum */
+int orc_variable_metric_step(int32_t N, double *V, const double *dx, const double *dg, const double *grad,
+                             double *direction, double *edm)
+{
+    int skipped = 0;
+    if (dx && dg) {
+        double *vg = (double *)malloc(sizeof(double) * (size_t)(N > 0 ? N : 1));
+        if (!vg) return -3;
+        double a = 0.0, b = 0.0;
+        for (int32_t i = 0; i < N; ++i) {
+            double s = 0.0;
+            for (int32_t j = 0; j < N; ++j) s += V[(int64_t)i * N + j] * dg[j];
+            vg[i] = s;
+        }
+        for (int32_t i = 0; i < N; ++i) a += dx[i] * dg[i];
+        for (int32_t i = 0; i < N; ++i) b += dg[i] * vg[i];
+        if (a > 0.0 && b > 0.0) {
+            for (int32_t i = 0; i < N; ++i)
+                for (int32_t j = 0; j < N; ++j) {
+                    double v = V[(int64_t)i * N + j];
+                    v += dx[i] * dx[j] / a;
+                    v -= vg[i] * vg[j] / b;
+                    if (a > b) {
+                        const double ui = dx[i] / a - vg[i] / b, uj = dx[j] / a - vg[j] / b;
+                        v += b * ui * uj;
+                    }
+                    V[(int64_t)i * N + j] = v;
+                }
+        } else {
+            skipped = 1;
+        }
+        free(vg);
+    }
+    double e = 0.0;
+    for (int32_t i = 0; i < N; ++i) {
+        double s = 0.0;
+        for (int32_t j = 0; j < N; ++j) s += V[(int64_t)i * N + j] * grad[j];
+        direction[i] = -s;
+        e += grad[i] * s;
+    }
+    *edm = 0.5 * e;
+    return skipped;
+}

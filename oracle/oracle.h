@@ -208,6 +208,20 @@ double orc_poisson_norm(double mu);
 double orc_poisson_inv(double mu, double Z, double u);
 int    orc_draw_pseudo_data(int64_t total_bins, const double *mu, int32_t E, uint64_t seed, double *data);
 
+/* One variable-metric step of the minimiser's loop ("This function is minimized by iteratively modifying
+ * the model parameters until the estimated distance to the minimum is smaller than a predefined threshold"; the
+ * minimiser is Minuit2's MIGRAD [28], a variable-metric method -- the paper prints no formula; R30 takes the
+ * published rule).  V [N x N] is the current estimate of the INVERSE Hessian of the NLL (symmetric), updated in place
+ * from the last move dx = x_new - x_old and the change of the gradient dg = g_new - g_old (both NULL: no update):
+ *     vg = V dg,  a = dx.dg,  b = dg.vg
+ *     V += dx dx^T / a - vg vg^T / b                                  (Davidon-Fletcher-Powell)
+ *     V += b u u^T,  u = dx / a - vg / b          where a > b        (the rank-one term that makes it BFGS)
+ * skipped (V unchanged, return value 1) unless a > 0 and b > 0.  Then
+ *     direction = -V grad,   edm = 1/2 grad^T V grad   (the estimated distance to the minimum).
+ * All sums run in index order in plain double arithmetic. */
+int orc_variable_metric_step(int32_t N, double *V, const double *dx, const double *dg, const double *grad,
+                             double *direction, double *edm);
+
 /* Number of threads orc_spectra would use for n_threads <= 0. */
 int orc_max_threads(void);
 
