@@ -265,6 +265,22 @@ PHYLINO_API phylino_status phylino_ordering_scan(phylino_ctx *ctx, int n_grid, i
 PHYLINO_API phylino_status phylino_nll_gradient(phylino_ctx *ctx, const double *theta, const double *step,
                                                 const double *data, double *nll0, double *grad);
 
+/* One variable-metric step of the minimiser's loop on the device ("This function is minimized by
+ * iteratively modifying the model parameters until the estimated distance to the minimum is smaller than a predefined
+ * threshold"; the minimiser is Minuit2's MIGRAD, a variable-metric method -- the paper prints no formula, R30
+ * takes the published rule).  V DEVICE [N x N] row-major, in/out: the current estimate of the INVERSE Hessian of the NLL;
+ * dx, dg DEVICE [N]: the last move x_new - x_old and the change of the gradient (both NULL: V is used as it is); grad
+ * DEVICE [N] (e.g. from phylino_nll_gradient); direction DEVICE [N] out; edm DEVICE [2] out.
+ *     vg = V dg, a = dx.dg, b = dg.vg;   V += dx dx^T / a - vg vg^T / b   (+ b u u^T, u = dx / a - vg / b, where a > b)
+ *     -- only if a > 0 and b > 0, else V stays and edm[1] = 1 (edm[1] = 0 otherwise);
+ *     direction = -V grad,   edm[0] = 1/2 grad^T V grad.
+ * All sums in index order in plain double arithmetic.  The line search along `direction`, the convergence test on
+ * edm[0] and the loop itself stay with the caller.  Needs no model; asynchronous on the
+ * context's stream (the scratch grows once with N, as phylino.h "Async" says of the work buffers). */
+PHYLINO_API phylino_status phylino_variable_metric_step(phylino_ctx *ctx, int N, double *V, const double *dx,
+                                                        const double *dg, const double *grad, double *direction,
+                                                        double *edm);
+
 /* Where the energy-scale systematic acts.  mode 0 (default; what BASELINE.json's north_star
  * asks for, R8): on every event before binning, E' = a0 + a1 E_vis + a2 E_vis^2.  mode 1: on the BINNED
  * spectrum, the paper's own signal step 3 ("The expectation is smoothed using a second-degree polynomial function.

@@ -28,6 +28,7 @@ abi_symbols = (
     "phylino_draw_pseudo_data", "phylino_ordering_scan", "phylino_nll_gradient",
     "phylino_set_energy_correction_mode", "phylino_set_flux_model", "phylino_last_small_phase",
     "phylino_hbm_read_floor", "phylino_last_medium_phase", "phylino_set_functions",
+    "phylino_variable_metric_step",
 )
 
 _STATUS = {0: "OK", 1: "ERR_ARG", 2: "ERR_SHAPE", 3: "ERR_STATE", 4: "ERR_OOM", 5: "ERR_CUDA"}
@@ -127,6 +128,8 @@ def load_library():
     lib.phylino_nll_ensemble.argtypes = [vp, i32, vp, i32, vp, vp]
     lib.phylino_set_prior_blocks.restype = i32
     lib.phylino_set_prior_blocks.argtypes = [vp, i32, C.POINTER(_PriorBlock)]
+    lib.phylino_variable_metric_step.restype = i32
+    lib.phylino_variable_metric_step.argtypes = [vp, i32, vp, vp, vp, vp, vp, vp]
     lib.phylino_set_functions.restype = i32
     lib.phylino_set_functions.argtypes = [vp, i32, C.POINTER(_Function)]
     lib.phylino_set_caching.restype = i32
@@ -421,6 +424,26 @@ class Phylino:
         self._check(self._lib.phylino_nll_gradient(self._ctx, theta.data_ptr(), step.data_ptr(), data.data_ptr(),
                                                    nll0.data_ptr(), grad.data_ptr()))
         return nll0, grad
+
+    def variable_metric_step(self, V, grad, dx=None, dg=None):
+        """One variable-metric step: V [N, N] float64 CUDA, updated IN PLACE from the last move dx and
+        gradient change dg (both or neither); returns (direction [N], edm [2] = (edm, update skipped))."""
+        t = self._torch
+        if not (isinstance(V, t.Tensor) and V.is_cuda and V.dtype == t.float64 and V.is_contiguous() and V.dim() == 2
+                and V.shape[0] == V.shape[1]):
+            raise TypeError("V must be a contiguous square float64 CUDA tensor")
+        N = int(V.shape[0])
+        grad = self._dev_vec(grad, N, "grad")
+        if (dx is None) != (dg is None):
+            raise ValueError("dx and dg must both be given or both be None")
+        if dx is not None:
+            dx, dg = self._dev_vec(dx, N, "dx"), self._dev_vec(dg, N, "dg")
+        direction = t.empty(N, dtype=t.float64, device=V.device)
+        edm = t.empty(2, dtype=t.float64, device=V.device)
+        self._check(self._lib.phylino_variable_metric_step(
+            self._ctx, N, V.data_ptr(), dx.data_ptr() if dx is not None else None,
+            dg.data_ptr() if dg is not None else None, grad.data_ptr(), direction.data_ptr(), edm.data_ptr()))
+        return direction, edm
 
     def expectation(self, params, out=None):
         t = self._torch

@@ -1241,6 +1241,22 @@ phylino_status phylino_nll_gradient(phylino_ctx *ctx, const double *theta, const
     return PHYLINO_OK;
 }
 
+phylino_status phylino_variable_metric_step(phylino_ctx *ctx, int N, double *V, const double *dx, const double *dg,
+                                            const double *grad, double *direction, double *edm)
+{
+    if (!ctx) return PHYLINO_ERR_ARG;
+    if (N < 0 || N > (1 << 14)) return fail(ctx, PHYLINO_ERR_SHAPE, "N = %d not in 0..%d", N, 1 << 14);
+    if (N == 0) return PHYLINO_OK;
+    if (!V || !grad || !direction || !edm) return fail(ctx, PHYLINO_ERR_ARG, "NULL V, grad, direction or edm");
+    if ((dx == nullptr) != (dg == nullptr)) return fail(ctx, PHYLINO_ERR_ARG, "dx and dg must both be given or both be NULL");
+    DeviceGuard g(ctx->device);
+    phylino_status s;
+    if ((s = ensure_work(ctx, 2 * (int64_t)N + 2)) != PHYLINO_OK) return s;
+    CU(launch_variable_metric_step(N, V, dx, dg, grad, direction, edm, ctx->d_work, ctx->stream));
+    ctx->launches += (dx && dg) ? 5 : 2;
+    return PHYLINO_OK;
+}
+
 phylino_status phylino_expectation(phylino_ctx *ctx, int P, const double *params, double *mu)
 {
     phylino_status s = check_ready(ctx, P, params, mu);

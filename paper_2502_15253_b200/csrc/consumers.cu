@@ -134,7 +134,79 @@ __global__ void __launch_bounds__(128) gradient_kernel(const double *theta, cons
     grad[j] = (nll[1 + 2 * j] - nll[2 + 2 * j]) / (up - dn);
 }
 
+/* ---- one variable-metric step of the minimiser's loop (R30) ---------------------------------
+ * Every sum runs over j in index order in plain (unfused) double arithmetic -- one thread per row, one thread for the
+ * scalars -- so the result is the oracle's bit for bit; N is a few hundred, the work is nothing beside one gradient. */
+__global__ void __launch_bounds__(128) vm_matvec_kernel(const double *V, const double *x, int N, double *out)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    double s = 0.0;
+    for (int j = 0; j < N; ++j) s += V[(size_t)i * N + j] * x[j];
+    out[i] = s;
+}
+
+/* ab[0] = dx.dg, ab[1] = dg.vg */
+__global__ void vm_scalars_kernel(const double *dx, const double *dg, const double *vg, int N, double *ab)
+{
+    double a = 0.0, b = 0.0;
+    for (int i = 0; i < N; ++i) a += dx[i] * dg[i];
+    for (int i = 0; i < N; ++i) b += dg[i] * vg[i];
+    ab[0] = a;
+    ab[1] = b;
+}
+
+/* V += dx dx^T / a - vg vg^T / b (+ b u u^T, u = dx / a - vg / b, where a > b); nothing unless a > 0 and b > 0 */
+__global__ void __launch_bounds__(128) vm_update_kernel(double *V, const double *dx, const double *vg, const double *ab,
+                                                        int N)
+{
+    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= (long long)N * N) return;
+    const double a = ab[0], b = ab[1];
+    if (!(a > 0.0 && b > 0.0)) return;
+    const int i = (int)(t / N), j = (int)(t % N);
+    double v = V[t];
+    v += dx[i] * dx[j] / a;
+    v -= vg[i] * vg[j] / b;
+    if (a > b) {
+        const double ui = dx[i] / a - vg[i] / b, uj = dx[j] / a - vg[j] / b;
+        v += b * ui * uj;
+    }
+    V[t] = v;
+}
+
+/* direction = -V grad (s = V grad), out[0] = 1/2 grad.s, out[1] = 1 if the update was skipped */
+__global__ void __launch_bounds__(128) vm_finish_kernel(const double *grad, const double *s, const double *ab, int N,
+                                                        double *direction, double *out)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < N) direction[i] = -s[i];
+    if (i == 0) {
+        double e = 0.0;
+        for (int k = 0; k < N; ++k) e += grad[k] * s[k];
+        out[0] = 0.5 * e;
+        out[1] = (ab && !(ab[0] > 0.0 && ab[1] > 0.0)) ? 1.0 : 0.0;
+    }
+}
+
 } // namespace
+
+/* work: DEVICE [2 N + 2] scratch (vg | s | a, b) */
+cudaError_t launch_variable_metric_step(int N, double *V, const double *dx, const double *dg, const double *grad,
+                                        double *direction, double *out, double *work, cudaStream_t st)
+{
+    if (N <= 0) return cudaSuccess;
+    double *vg = work, *s = work + N, *ab = work + 2 * (size_t)N;
+    const int blocks = (N + 127) / 128;
+    if (dx && dg) {
+        vm_matvec_kernel<<<blocks, 128, 0, st>>>(V, dg, N, vg);
+        vm_scalars_kernel<<<1, 1, 0, st>>>(dx, dg, vg, N, ab);
+        vm_update_kernel<<<(unsigned)(((long long)N * N + 127) / 128), 128, 0, st>>>(V, dx, vg, ab, N);
+    }
+    vm_matvec_kernel<<<blocks, 128, 0, st>>>(V, grad, N, s);
+    vm_finish_kernel<<<blocks, 128, 0, st>>>(grad, s, (dx && dg) ? ab : nullptr, N, direction, out);
+    return cudaGetLastError();
+}
 
 cudaError_t launch_pseudo_data(const double *mu, double *Z, int n, int E, unsigned long long seed, double *data,
                                cudaStream_t st)

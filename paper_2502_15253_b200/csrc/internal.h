@@ -241,6 +241,8 @@ cudaError_t launch_scan_batch(const double *theta, int width, int col, const dou
 cudaError_t launch_gradient_batch(const double *theta, const double *h, int width, double *batch, cudaStream_t st);
 cudaError_t launch_gradient(const double *theta, const double *h, const double *nll, int width, double *nll0,
                             double *grad, cudaStream_t st);
+cudaError_t launch_variable_metric_step(int N, double *V, const double *dx, const double *dg, const double *grad,
+                                        double *direction, double *out, double *work, cudaStream_t st);
 cudaError_t run_peak_fp64(int iters, cudaStream_t st, double *dfma_per_s);
 cudaError_t run_launch_floor(int reps, cudaStream_t st, double *us_per_call);
 cudaError_t run_hbm_read_floor(size_t bytes, int reps, cudaStream_t st, double *us_best);

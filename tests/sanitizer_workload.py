@@ -6,7 +6,7 @@ Paths: ticket schedule with full groups, a ragged group and sub-streams (70 poin
 in-CTA tables (1, 5, 16 points), weighted and unit-weight records, bin edges inside units (per-event slow path, general
 sub-stream flush), the edge-first unit order of the single-launch kernel (capped warps), component mode (caching),
 prior blocks over parameters and over functions of them, ensembles, pseudo-data, the ordering scan, the gradient (dense
-and through the structural plan), the bin-level energy correction with a flux model, the diagnostic instantiation.
+and through the structural plan) and the variable-metric step, the bin-level energy correction with a flux model, the diagnostic instantiation.
 Results are checked against the oracle so that a sanitizer-clean run is also a correct one."""
 import os
 import sys
@@ -95,7 +95,13 @@ def main():
         nll0, grad = ph.nll_gradient(dev(wl.theta0), dev(step), dev(data))
         assert ph.last_plan()[0] > 0
         assert abs(nll0.cpu().numpy()[0] - orc.nll(wl.theta0[None, :], data)[0]) <= 1e-6
-        n += 5
+        V = np.diag(np.full(NP0, 1e-4))
+        dV = dev(V)
+        dxs, dgs = np.full(NP0, 1e-3), np.linspace(0.5, 2.0, NP0)
+        d, edm = ph.variable_metric_step(dV, grad, dev(dxs), dev(dgs))
+        V_o, d_o, edm_o, _ = oracle.variable_metric_step(V, grad.cpu().numpy(), dxs, dgs)
+        assert np.array_equal(dV.cpu().numpy(), V_o) and np.array_equal(d.cpu().numpy(), d_o) and edm.cpu().numpy()[0] == edm_o
+        n += 6
     # the paper's bin-level steps with a flux model
     wl = workloads.make_config(3, scale=0.001, n_points=20)
     NP0 = wl.model.n_params

@@ -168,3 +168,65 @@ def test_cached_gradient_plans_without_the_values(gpu, oracle_mod):
         assert np.isnan(gb[5]) or gb[5] == 0.0 or np.isinf(gb[5])       # 0 / 0 or 0 / tiny: no information, no crash
         keep = np.arange(N) != 5
         assert np.array_equal(gb[keep], grad.cpu().numpy()[keep])
+
+
+def test_variable_metric_step_matches_the_oracle_bit_for_bit(gpu, oracle_mod):
+    """PAPER.md:155; R30: the rank-two update of the inverse-Hessian estimate, the Newton direction and the
+    estimated distance to the minimum -- every sum in index order in plain double arithmetic on both sides, so the
+    comparison is bit for bit; both branches of the rule, the no-move call and the skip; then a short minimisation of
+    config 3's NLL (scaled) driven by phylino_nll_gradient + this step, which must go downhill."""
+    import torch
+    rng = np.random.default_rng(17)
+    with gpu.Phylino() as ph:
+        for N, vscale in ((3, 1.0), (37, 1e-3), (301, 1.0), (301, 1e-3)):
+            A = rng.normal(size=(N, N))
+            V = (A @ A.T / N + np.eye(N)) * vscale
+            H = rng.normal(size=(N, N))
+            H = H @ H.T / N + np.eye(N)
+            g = rng.normal(size=N)
+            dx = rng.normal(size=N) * 0.1
+            dg = H @ dx
+            for use_move in (False, True):
+                dV = _dev(V)
+                d, edm = ph.variable_metric_step(dV, _dev(g), _dev(dx) if use_move else None, _dev(dg) if use_move else None)
+                V_o, d_o, edm_o, skipped = oracle_mod.variable_metric_step(V, g, dx if use_move else None, dg if use_move else None)
+                assert np.array_equal(dV.cpu().numpy(), V_o)
+                assert np.array_equal(d.cpu().numpy(), d_o)
+                assert edm.cpu().numpy()[0] == edm_o and edm.cpu().numpy()[1] == float(skipped) == 0.0
+        dV = _dev(np.eye(4))
+        d, edm = ph.variable_metric_step(dV, _dev(np.ones(4)), _dev(np.array([1.0, 0, 0, 0])), _dev(np.array([-1.0, 0, 0, 0])))
+        assert edm.cpu().numpy()[1] == 1.0 and np.array_equal(dV.cpu().numpy(), np.eye(4))       # no positive curvature
+
+    # a few steps of the loop the paper describes, on the device except for the step length
+    wl = workloads.make_config(3, scale=0.01)
+    N = wl.model.n_params
+    orc = oracle_mod.Oracle(wl.model, wl.events)
+    data = _data(orc, wl)
+    sig = np.where(np.isfinite(wl.model.prior_sigma) & (wl.model.prior_sigma > 0), wl.model.prior_sigma, 1e-2)
+    theta = wl.theta0 + 0.5 * sig * np.random.default_rng(4).normal(size=N)
+    h = 0.01 * sig
+    with gpu.Phylino() as ph:
+        ph.load_workload(wl)
+        ph.set_caching(True)
+        dV = _dev(np.diag(sig ** 2))                       # first metric: the prior covariance
+        d_theta, d_h, d_data = _dev(theta), _dev(h), _dev(data)
+        nll0, grad = ph.nll_gradient(d_theta, d_h, d_data)
+        f = [float(nll0.cpu()[0])]
+        dx = dg = None
+        for it in range(4):
+            d, edm = ph.variable_metric_step(dV, grad, dx, dg)
+            assert float(edm.cpu()[0]) >= 0.0
+            t = 1.0
+            while True:                                    # backtracking: the caller's line search
+                trial = d_theta + t * d
+                f_t = float(ph.nll(trial[None, :].contiguous(), d_data).cpu()[0])
+                if f_t < f[-1] or t < 1e-4:
+                    break
+                t *= 0.5
+            nll1, grad1 = ph.nll_gradient(trial.contiguous(), d_h, d_data)
+            dx, dg = (trial - d_theta).contiguous(), (grad1 - grad).contiguous()
+            d_theta, grad = trial.contiguous(), grad1
+            f.append(f_t)
+        torch.cuda.synchronize()
+    assert all(b < a for a, b in zip(f, f[1:])) and f[-1] < f[0] - 1.0, f
+    assert abs(f[-1] - orc.nll(d_theta.cpu().numpy()[None, :], data)[0]) <= ABS_NLL
