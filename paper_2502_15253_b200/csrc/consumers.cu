@@ -136,7 +136,8 @@ __global__ void __launch_bounds__(128) gradient_kernel(const double *theta, cons
 
 /* ---- one variable-metric step of the minimiser's loop (R30) ---------------------------------
  * Every sum runs over j in index order in plain (unfused) double arithmetic -- one thread per row, one thread for the
- * scalars -- so the result is the oracle's bit for bit; N is a few hundred, the work is nothing beside one gradient. */
+ * scalars -- so the result is a function of the inputs alone, the same bits as any other IEEE evaluation of that
+ * sequence; N is a few hundred, the work is nothing beside one gradient. */
 __global__ void __launch_bounds__(128) vm_matvec_kernel(const double *V, const double *x, int N, double *out)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
