@@ -443,36 +443,6 @@ __device__ __forceinline__ void flush_run(const SpectraArgs &a, const Tables &T,
     r.W = 0.0;
 }
 
-/* the rare flush: sub-streams of a point end in different cells (a bin edge inside the unit).  For every lane the
- * sum over the sub-streams of its point that share its cell, and whether it is the first of them.  Not inlined
- * (see walk_batch_slow). */
-template <int S> struct SubSums { long long sum[S + 1]; bool first; };
-
-template <int S>
-__device__ __noinline__ SubSums<S> substream_sums_general(unsigned long long cell, bool live, int lg, int lane, int nq,
-                                                          SubSums<S> q)
-{
-    SubSums<S> out;
-#pragma unroll
-    for (int j = 0; j <= S; ++j) out.sum[j] = 0;
-    out.first = true;
-    const int pl = lane & ((1 << lg) - 1);
-#pragma unroll 1
-    for (int src = pl; src < 32; src += 1 << lg) {              /* the sub-streams of this lane's point */
-        const unsigned long long c = __shfl_sync(0xffffffffu, cell, src);
-        const bool same = live && c == cell;
-        if (same && src < lane) out.first = false;
-#pragma unroll
-        for (int j = 0; j <= S; ++j) {
-            if (j < nq) {                                        /* nq is warp-uniform */
-                const long long v = __shfl_sync(0xffffffffu, q.sum[j], src);
-                if (same) out.sum[j] += v;
-            }
-        }
-    }
-    return out;
-}
-
 /* The flush at the end of a unit / range when the group has at most 16 points: the 32 / PL sub-streams of a
  * point usually end in the same bin, and 32 lanes of every resident warp adding to the same one or two cells
  * would queue at the L2 atomic unit (same-address atomics: a 6e6-event, 1-point call spent 0.45 ms there).
@@ -507,7 +477,7 @@ __device__ __forceinline__ void flush_run_substreams(const SpectraArgs &a, const
             q[0] = to_fixed(tot, ds.fx_scale, T.rec[(size_t)(2 * S + 1) * a.P + p] != 0.0, fl[0]);
         }
     }
-    bool first;
+    bool first = true;
     if (uniform) {
         /* a butterfly over the sub-stream bits of the lane index (exact integers: any order gives the same bits) */
         for (int o = 16; o >= (1 << lg); o >>= 1) {
@@ -518,16 +488,11 @@ __device__ __forceinline__ void flush_run_substreams(const SpectraArgs &a, const
             }
         }
         first = lane == pl;
-    } else {
-        SubSums<S> qs;
-#pragma unroll
-        for (int j = 0; j <= S; ++j) qs.sum[j] = q[j];
-        qs.first = true;
-        const SubSums<S> g = substream_sums_general<S>(cell, live, lg, lane, comp ? S + 1 : 1, qs);
-#pragma unroll
-        for (int j = 0; j <= S; ++j) q[j] = g.sum[j];
-        first = g.first;
     }
+    /* else: a bin edge inside the unit -- the sub-streams of a point end in different cells.  Rare (one unit per
+     * edge and point), so every lane simply adds its own total: the same integers in another order, and nothing
+     * cold to fetch on the way (the shuffle loop that used to sort the lanes by cell was a second cold function
+     * behind the event-by-event path: a warp with an edge ended 5 us after the others in a one-point call) */
     if (live) {
 #pragma unroll
         for (int j = 0; j <= S; ++j) {
