@@ -43,7 +43,7 @@ HEADLINE_CONFIG = 5
 # ALGORITHMIC fp64-pipe instructions per event x point, unit-weight datasets (every
 # BASELINE.json config).  Per oscillation term: 3 range reduction + 1 square + 5 Horner + the last Horner step; the
 # two-term model accumulates with that last step itself (devmath.cuh half_cos_accumulate: 10), the three-term models
-# form g and add it (11).  The SASS of the hot loop has exactly these (profiles/r2e_hot_loop_sass.md).  The
+# form g and add it (11).  The SASS of the hot loop has exactly these (profiles/r2f_hot_loop_sass.md).  The
 # bin/weight bookkeeping is per batch of events and per run, not per event x point.
 def fp64_per_general_term(S: int) -> int:
     return 10 if S == 2 else 11
