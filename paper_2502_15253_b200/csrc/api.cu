@@ -645,20 +645,63 @@ bool plan_components(const phylino_ctx *ctx, int P, const double *params, Compon
             }
         }
     }
-    /* pack the pairs of a class S at a time */
+    /* Pack the pairs of a class into virtual points of S slots.  Two ways, both exact: by TERM -- slot k holds only
+     * pairs that first appeared as term k, so that a virtual point looks like a real one (the slow splitting in the
+     * last slot, dm2_ee in the first) and the kernel's cheaper forms of those terms apply to the whole group -- or
+     * S at a time in order of appearance, which needs fewer virtual points when one term has many more distinct
+     * splittings than the others (config 5's grid: 64 values of dm2_41, one of each other: 22 against 64).  By term
+     * where that costs no extra virtual point (config 3's gradient batch: 21 either way). */
     const int n_pairs = (int)pair_class.size();
-    std::vector<int32_t> fill((size_t)pl.C, 0), open_vp((size_t)pl.C, -1), pair_cell((size_t)n_pairs);
+    std::vector<int32_t> cnt_c((size_t)pl.C, 0), cnt_ck((size_t)pl.C * S, 0), pair_cell((size_t)n_pairs);
     for (int q = 0; q < n_pairs; ++q) {
-        const int c = pair_class[q];
-        if (open_vp[c] < 0 || fill[c] == S) {
-            open_vp[c] = pl.V++;
-            fill[c] = 0;
-            pl.vp_class.push_back(c);
-            for (int s = 0; s < S; ++s) pl.vp_src.push_back(pair_src[q]);   /* unused slots repeat the first pair */
+        ++cnt_c[pair_class[q]];
+        ++cnt_ck[(size_t)pair_class[q] * S + (pair_src[q] & 3)];
+    }
+    int64_t v_free = 0, v_term = 0;
+    for (int c = 0; c < pl.C; ++c) {
+        v_free += (cnt_c[c] + S - 1) / S;
+        int m = 0;
+        for (int k = 0; k < S; ++k) m = std::max(m, (int)cnt_ck[(size_t)c * S + k]);
+        v_term += m;
+    }
+    if (v_term <= v_free) {
+        std::vector<int32_t> base((size_t)pl.C, 0), first_c((size_t)pl.C, -1), first_ck((size_t)pl.C * S, -1);
+        for (int q = n_pairs - 1; q >= 0; --q) {
+            first_c[pair_class[q]] = pair_src[q];
+            first_ck[(size_t)pair_class[q] * S + (pair_src[q] & 3)] = pair_src[q];
         }
-        pl.vp_src[(size_t)open_vp[c] * S + fill[c]] = pair_src[q];
-        pair_cell[q] = open_vp[c] * (S + 1) + 1 + fill[c];
-        ++fill[c];
+        for (int c = 0; c < pl.C; ++c) {
+            int m = 0;
+            for (int k = 0; k < S; ++k) m = std::max(m, (int)cnt_ck[(size_t)c * S + k]);
+            base[c] = pl.V;
+            for (int j = 0; j < m; ++j) {
+                pl.vp_class.push_back(c);
+                for (int k = 0; k < S; ++k)         /* unused slots repeat the first pair of their term (or class) */
+                    pl.vp_src.push_back(first_ck[(size_t)c * S + k] >= 0 ? first_ck[(size_t)c * S + k] : first_c[c]);
+            }
+            pl.V += m;
+        }
+        std::vector<int32_t> seen((size_t)pl.C * S, 0);
+        for (int q = 0; q < n_pairs; ++q) {
+            const int c = pair_class[q], k = pair_src[q] & 3;
+            const int vp = base[c] + seen[(size_t)c * S + k]++;
+            pl.vp_src[(size_t)vp * S + k] = pair_src[q];
+            pair_cell[q] = vp * (S + 1) + 1 + k;
+        }
+    } else {
+        std::vector<int32_t> fill((size_t)pl.C, 0), open_vp((size_t)pl.C, -1);
+        for (int q = 0; q < n_pairs; ++q) {
+            const int c = pair_class[q];
+            if (open_vp[c] < 0 || fill[c] == S) {
+                open_vp[c] = pl.V++;
+                fill[c] = 0;
+                pl.vp_class.push_back(c);
+                for (int s2 = 0; s2 < S; ++s2) pl.vp_src.push_back(pair_src[q]);   /* unused slots repeat the first pair */
+            }
+            pl.vp_src[(size_t)open_vp[c] * S + fill[c]] = pair_src[q];
+            pair_cell[q] = open_vp[c] * (S + 1) + 1 + fill[c];
+            ++fill[c];
+        }
     }
     if (2 * (int64_t)pl.V > P) return false;
     pl.pt_comp.resize((size_t)P * (S + 1));
