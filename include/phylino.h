@@ -281,6 +281,42 @@ PHYLINO_API phylino_status phylino_variable_metric_step(phylino_ctx *ctx, int N,
                                                         const double *dg, const double *grad, double *direction,
                                                         double *edm);
 
+/* The same variable-metric step, for callers that cannot let this library allocate device memory.
+ *
+ * phylino_variable_metric_step above needs a context (phylino_create allocates) and keeps its 2 N + 2 doubles of
+ * scratch in a cudaMalloc'ed buffer that grows with N.  That rules it out for a fit that shares its GPU with a
+ * framework whose caching allocator already owns the memory (a cudaMalloc of ours can fail or fragment that pool, and
+ * under an MPS / MIG memory limit it counts against the limit), for a minimiser loop that cannot afford the
+ * device-wide synchronisation cudaMalloc / cudaFree imply, and for services that allow no allocation after start-up.
+ * This entry point takes no context and calls no cudaMalloc, cudaFree or other allocating routine, ever: its scratch
+ * is ONE fixed array inside the library's device image.
+ *
+ *   cuda_stream a cudaStream_t of the CURRENT device (0 = default stream); the work is enqueued there and the call
+ *               returns without waiting.  Every DEVICE pointer must belong to the current device.
+ *   N           0 ... PHYLINO_STATIC_MAX_N.  Anything larger is refused with PHYLINO_ERR_SHAPE before any launch
+ *               (the array cannot grow) -- use phylino_variable_metric_step for such problems.
+ *   V, dx, dg, grad, direction, edm   DEVICE, exactly as for phylino_variable_metric_step (same rule, same operation
+ *               order, same kernels: the two entry points return identical bits).  The caller owns all of them.
+ *   error       HOST [error_len] or NULL: receives the text of a failure ("" on success); there is no context to
+ *               keep it in.
+ *
+ * What the fixed array costs and how it behaves:
+ *   - (2 * PHYLINO_STATIC_MAX_N + 2) * 8 = 32 784 bytes of device memory on every GPU that loads this library, from
+ *     the moment its device code is loaded there until the process exits, whether or not this call is ever made.
+ *   - The FIRST call on each device looks up the array's device address (cudaGetSymbolAddress, with that device
+ *     current) and remembers it per device; make that first call before any stream capture begins.
+ *   - All calls on a device share the array, and it keeps whatever the last call wrote.  No call depends on that:
+ *     each part of the array is written in full on the stream before the kernel that reads it, so nothing needs
+ *     clearing.  But two calls that can run at the same time on one GPU -- different streams, or two host threads --
+ *     race on it and corrupt each other's results; keep all calls of a device on one stream, or order them yourself.
+ * Returns PHYLINO_ERR_ARG for NULL V / grad / direction / edm or for only one of dx, dg; PHYLINO_ERR_CUDA if the
+ * address lookup or a launch fails (no device: there is no CPU fallback). */
+#define PHYLINO_STATIC_MAX_N 2048
+PHYLINO_API phylino_status phylino_variable_metric_step_static(void *cuda_stream, int N, double *V, const double *dx,
+                                                               const double *dg, const double *grad,
+                                                               double *direction, double *edm, char *error,
+                                                               int error_len);
+
 /* Where the energy-scale systematic acts.  mode 0 (default; what BASELINE.json's north_star
  * asks for, R8): on every event before binning, E' = a0 + a1 E_vis + a2 E_vis^2.  mode 1: on the BINNED
  * spectrum, the paper's own signal step 3 ("The expectation is smoothed using a second-degree polynomial function.

@@ -13,4 +13,5 @@ from .binding import (  # noqa: F401
     abi_symbols,
     lib_path,
     load_library,
+    variable_metric_step_static,
 )

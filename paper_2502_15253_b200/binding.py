@@ -28,7 +28,7 @@ abi_symbols = (
     "phylino_draw_pseudo_data", "phylino_ordering_scan", "phylino_nll_gradient",
     "phylino_set_energy_correction_mode", "phylino_set_flux_model", "phylino_last_small_phase",
     "phylino_hbm_read_floor", "phylino_last_medium_phase", "phylino_set_functions",
-    "phylino_variable_metric_step",
+    "phylino_variable_metric_step", "phylino_variable_metric_step_static",
 )
 
 _STATUS = {0: "OK", 1: "ERR_ARG", 2: "ERR_SHAPE", 3: "ERR_STATE", 4: "ERR_OOM", 5: "ERR_CUDA"}
@@ -130,6 +130,8 @@ def load_library():
     lib.phylino_set_prior_blocks.argtypes = [vp, i32, C.POINTER(_PriorBlock)]
     lib.phylino_variable_metric_step.restype = i32
     lib.phylino_variable_metric_step.argtypes = [vp, i32, vp, vp, vp, vp, vp, vp]
+    lib.phylino_variable_metric_step_static.restype = i32
+    lib.phylino_variable_metric_step_static.argtypes = [vp, i32, vp, vp, vp, vp, vp, vp, C.c_char_p, i32]
     lib.phylino_set_functions.restype = i32
     lib.phylino_set_functions.argtypes = [vp, i32, C.POINTER(_Function)]
     lib.phylino_set_caching.restype = i32
@@ -172,6 +174,51 @@ def load_library():
 
 def _np_ptr(a: Optional[np.ndarray]):
     return None if a is None else a.ctypes.data
+
+
+STATIC_MAX_N = 2048      # PHYLINO_STATIC_MAX_N
+
+
+def variable_metric_step_static(V, grad, dx=None, dg=None, direction=None, edm=None, stream: Optional[int] = None):
+    """phylino_variable_metric_step_static: the variable-metric step without a context and without any device
+    allocation by the library -- for callers whose GPU memory belongs to another allocator, who cannot take the
+    device-wide stall of a cudaMalloc, or who may not allocate after start-up.  The library's scratch is a fixed
+    array (N <= STATIC_MAX_N) shared by all calls on a device: keep them on one stream.
+
+    V [N, N] float64 CUDA, updated IN PLACE from the last move dx and gradient change dg (both or neither).  Pass
+    preallocated `direction` [N] and `edm` [2] to keep this wrapper from allocating too (torch.empty otherwise).
+    Work goes on `stream` (default: torch's current stream of V's device, which is made current for the call)."""
+    import torch as t
+    lib = load_library()
+
+    def vec(x, n, what):
+        if not (isinstance(x, t.Tensor) and x.is_cuda and x.dtype == t.float64 and x.is_contiguous()
+                and x.numel() == n and x.device == V.device):
+            raise TypeError(f"{what} must be a contiguous float64 CUDA tensor of {n} values on V's device")
+        return x
+
+    if not (isinstance(V, t.Tensor) and V.is_cuda and V.dtype == t.float64 and V.is_contiguous() and V.dim() == 2
+            and V.shape[0] == V.shape[1]):
+        raise TypeError("V must be a contiguous square float64 CUDA tensor")
+    N = int(V.shape[0])
+    grad = vec(grad, N, "grad")
+    if (dx is None) != (dg is None):
+        raise ValueError("dx and dg must both be given or both be None")
+    if dx is not None:
+        dx, dg = vec(dx, N, "dx"), vec(dg, N, "dg")
+    direction = t.empty(N, dtype=t.float64, device=V.device) if direction is None else vec(direction, N, "direction")
+    edm = t.empty(2, dtype=t.float64, device=V.device) if edm is None else vec(edm, 2, "edm")
+    err = C.create_string_buffer(512)
+    with t.cuda.device(V.device):
+        if stream is None:
+            stream = t.cuda.current_stream(V.device).cuda_stream
+        st = lib.phylino_variable_metric_step_static(
+            C.c_void_p(stream), N, V.data_ptr(), dx.data_ptr() if dx is not None else None,
+            dg.data_ptr() if dg is not None else None, grad.data_ptr(), direction.data_ptr(), edm.data_ptr(),
+            err, len(err))
+    if st != 0:
+        raise PhylinoError(st, err.value.decode())
+    return direction, edm
 
 
 class Phylino:

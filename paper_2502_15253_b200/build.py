@@ -16,7 +16,7 @@ _ROOT = os.path.dirname(_HERE)
 CSRC = os.path.join(_HERE, "csrc")
 INCLUDE = os.path.join(_ROOT, "include")
 LIB = os.path.join(_HERE, "libphylino.so")
-SOURCES = ["api.cu", "spectra.cu", "finalize.cu", "transform.cu", "consumers.cu", "peaks.cu"]
+SOURCES = ["api.cu", "spectra.cu", "finalize.cu", "transform.cu", "consumers.cu", "peaks.cu", "static_step.cu"]
 HEADERS = ["internal.h", "devmath.cuh", "finalize.cuh", os.path.join(INCLUDE, "phylino.h")]
 
 NVCC_FLAGS = [
