@@ -236,8 +236,9 @@ PHYLINO_API phylino_status phylino_nll_ensemble(phylino_ctx *ctx, int P, const d
  * phylino_expectation at the injected hypothesis), data DEVICE [E x total_bins]; feed it to phylino_nll_ensemble.
  * The counts are a function of (seed, e, i, mu[i]) alone (R26): Philox4x32-10 uniforms with counter
  * (i, e, 0, 0) and key = seed, and an exact inversion of the Poisson distribution from its mode outwards that uses
- * only +, *, / -- the same integers as any other IEEE implementation of that sequence, and from run to run.  mu[i] <= 0, NaN or inf gives 0.
- * O(sqrt(mu)) steps per draw.  Asynchronous on the context's stream. */
+ * only +, *, / -- the same integers as any other IEEE implementation of that sequence, and from run to run.  mu[i] <= 0, NaN or inf gives 0;
+ * a finite mu[i] above 1e9 is outside the sampler's domain and gives NaN (the walk costs O(sqrt(mu)) steps per draw and
+ * every loop is bounded, so no value in `mu` can stall the device).  Asynchronous on the context's stream. */
 PHYLINO_API phylino_status phylino_draw_pseudo_data(phylino_ctx *ctx, const double *mu, int E, uint64_t seed,
                                                     double *data);
 
@@ -374,11 +375,17 @@ PHYLINO_API int64_t phylino_param_width(const phylino_ctx *ctx);
 PHYLINO_API int64_t phylino_total_bins(const phylino_ctx *ctx);     /* sum_d n_bins, 0 before set_model */
 PHYLINO_API int64_t phylino_total_events(const phylino_ctx *ctx);   /* sum_d n over loaded datasets */
 
-/* Pre-size every per-batch work buffer of the context for batches of up to max_points points (accumulators,
- * per-point records and bin thresholds, pinned staging of the HOST entry points, the transformed batch) and build
- * what a first call would otherwise build with a synchronisation (kernel occupancies, the unit order of the
- * single-launch kernel).  After it, calls with P <= max_points allocate nothing and the DEVICE entry points never
- * synchronise.  Synchronises the stream if anything grows.  PHYLINO_ERR_STATE before the model and all events are loaded. */
+/* Pre-size every per-batch work buffer of the context for batches of up to max_points points (accumulators -- also
+ * for the rows of a cached batch --, per-point records and bin thresholds, pinned staging of the HOST entry points,
+ * the transformed batch, the plan of a cached batch, the work buffer of phylino_nll_gradient / _ordering_scan /
+ * _draw_pseudo_data / _variable_metric_step, the expectations of phylino_nll_ensemble) and build what a first call would
+ * otherwise build with a synchronisation (kernel occupancies, the unit order of the single-launch kernel, and -- if
+ * phylino_set_caching is ON at the time of this call -- the structural plan of the central-difference batch).  After it,
+ * calls with P <= max_points allocate nothing and the DEVICE entry points never synchronise (with caching on only
+ * phylino_nll_gradient: see phylino_set_caching).  A batch counts with all its points: phylino_nll_gradient needs
+ * max_points >= 2 W + 1, phylino_ordering_scan max_points >= n_grid (W = phylino_param_width), and
+ * phylino_variable_metric_step N <= W.  Synchronises the stream if anything grows.  PHYLINO_ERR_STATE before the model
+ * and all events are loaded. */
 PHYLINO_API phylino_status phylino_reserve(phylino_ctx *ctx, int max_points);
 
 /* Which kernels evaluate a batch: 0 (default) the library chooses -- the single-launch kernel for small batches

@@ -119,6 +119,7 @@ void free_all(phylino_ctx *c)
     c->h_pin = nullptr; c->stage_capacity = 0;
     c->resident_warps = c->fused_warps = 0;     /* occupancy of the kernels of the model's n_terms: asked again */
     c->fused_tables = 0;
+    c->fused_cache.clear();
     c->have_model = false;
 }
 
@@ -316,10 +317,16 @@ phylino_status fill_batch(phylino_ctx *ctx, SpectraArgs &a, int P, const double 
     if (wants_single_launch(ctx, P)) {
         const size_t tables = fused_table_bytes(ctx->n_terms, P, a.thr_rows, a.thr_stride, ctx->n_datasets);
         if (fused_fits(tables)) {
-            if (ctx->fused_warps == 0 || ctx->fused_tables != tables) {
-                CU(spectra_max_warps(ctx->n_terms, ctx->sm_count, true, tables, &ctx->fused_warps));
-                ctx->fused_tables = tables;
+            /* one occupancy query per distinct table size (the size depends on P): a minimiser that alternates
+             * single evaluations with small line-search batches finds both in the list */
+            int found = 0;
+            for (const auto &kv : ctx->fused_cache) if (kv.first == tables) { found = kv.second; break; }
+            if (found == 0) {
+                CU(spectra_max_warps(ctx->n_terms, ctx->sm_count, true, tables, &found));
+                ctx->fused_cache.emplace_back(tables, found);
             }
+            ctx->fused_warps = found;
+            ctx->fused_tables = tables;
             a.sched = 1;
         }
     }
@@ -477,7 +484,11 @@ phylino_status enqueue_eval(phylino_ctx *ctx, int P, const double *params, const
         ctx->launches += 1;
     }
     if (ctx->timing) CU(cudaEventRecord(ctx->ev[2], ctx->stream));
-    CU(launch_finalize(f, mode, ctx->stream, pdl));
+    /* the finalize prologue reads params and data BEFORE its griddepcontrol.wait, which is safe only behind a spectra
+     * kernel of this call (that kernel waited for its own predecessor before releasing dependents).  With nothing to
+     * walk (every dataset empty) no such kernel was launched: the finalize kernel then follows the caller's
+     * producer of params / data directly and must be an ordinary, fully ordered launch. */
+    CU(launch_finalize(f, mode, ctx->stream, pdl && a.n_items > 0 && P > 0));
     ctx->launches += 1;
     if (ctx->timing) CU(cudaEventRecord(ctx->ev[3], ctx->stream));
     return PHYLINO_OK;
@@ -565,6 +576,9 @@ int term_deps(int osc_model, int k, int slots[3])
 
 uint64_t bits_of(double x) { uint64_t u; std::memcpy(&u, &x, sizeof u); return u; }
 
+/* tags of the symbolic batch of gradient_plan: two disjoint families of bit patterns */
+constexpr uint64_t kSymbolTag = 0xfff8000000000000ull, kFixedTag = 0xfff9000000000000ull;
+
 uint64_t mix64(uint64_t h, uint64_t x)
 {
     h ^= x + 0x9e3779b97f4a7c15ull + (h << 6) + (h >> 2);
@@ -587,8 +601,11 @@ struct IdTable {
     }
 };
 
-/* false: caching would not pay (more than half as many virtual points as points) -- use the dense path */
-bool plan_components(const phylino_ctx *ctx, int P, const double *params, ComponentPlan &pl)
+/* false: caching would not pay (more than half as many virtual points as points) -- use the dense path.
+ * symbolic: `params` holds the symbols of gradient_plan (tags, not values); a FIXED oscillation parameter then
+ * enters the comparison as a tag of its own (fixed slots with equal bits share one) that no symbol can equal, so a
+ * fixed splitting is never merged with a fitted one because its value happens to look like a symbol. */
+bool plan_components(const phylino_ctx *ctx, int P, const double *params, ComponentPlan &pl, bool symbolic = false)
 {
     const int S = ctx->n_terms, NP = ctx->n_params;
     if (P >= (1 << 29)) return false;                   /* (point, term) is packed as p * 4 + k in an int32 */
@@ -622,7 +639,12 @@ bool plan_components(const phylino_ctx *ctx, int P, const double *params, Compon
         auto dep = [&](int p, int k, int j, int n_slots, const int *slots) -> uint64_t {
             (void)k; (void)n_slots;
             const int idx = ctx->idx_osc[slots[j]];
-            return bits_of(idx >= 0 ? params[(size_t)p * NP + idx] : ctx->fixed_osc[slots[j]]);
+            if (idx >= 0) return bits_of(params[(size_t)p * NP + idx]);
+            if (!symbolic) return bits_of(ctx->fixed_osc[slots[j]]);
+            int first = slots[j];                           /* lowest fixed slot with the same bits */
+            for (int q = 0; q < slots[j]; ++q)
+                if (ctx->idx_osc[q] < 0 && bits_of(ctx->fixed_osc[q]) == bits_of(ctx->fixed_osc[slots[j]])) { first = q; break; }
+            return kFixedTag | (uint64_t)first;
         };
         for (int p = 0; p < P; ++p) {
             for (int k = 0; k < S; ++k) {
@@ -783,7 +805,7 @@ phylino_status enqueue_cached(phylino_ctx *ctx, int P, const double *h_params, c
         if (a.n_items > 0) { CU(launch_spectra(a, S, ctx->stream, !ctx->timing, false)); ctx->launches += 1; }
     }
     if (ctx->timing) CU(cudaEventRecord(ctx->ev[2], ctx->stream));
-    CU(launch_finalize(f, d_nll ? 2 : 0, ctx->stream, !ctx->timing));
+    CU(launch_finalize(f, d_nll ? 2 : 0, ctx->stream, !ctx->timing && (a.sched == 1 || a.n_items > 0)));
     ctx->launches += 1;
     if (ctx->timing) CU(cudaEventRecord(ctx->ev[3], ctx->stream));
     /* the cells are shared between points: cleared here, not by the finalize kernel */
@@ -798,10 +820,11 @@ phylino_status enqueue_cached(phylino_ctx *ctx, int P, const double *h_params, c
 
 /* The plan of a central-difference batch {theta} U {theta +- step_j e_j} needs no values: which points share an
  * energy-scale tuple or a mass splitting follows from WHICH column a point perturbs.  plan_components only compares
- * bit patterns, so it is run once per model on a symbolic batch with that equality structure (column j holds j,
- * perturbed entries j +- 1/4) and the plan is kept.  Points that are structurally different but equal in value
- * (a step below one ulp) are merely not merged; structurally equal points ARE equal in value, so nothing is merged
- * wrongly.  Not with a transformation layer (a step in u_j moves several columns of theta by amounts the symbols do
+ * bit patterns, so it is run once per model on a symbolic batch with that equality structure (column j holds the
+ * tag 4 j, perturbed entries 4 j + 1 / 4 j + 2; fixed oscillation parameters get tags of another family, see
+ * plan_components) and the plan is kept.  Points that are structurally different but equal in value (a step below
+ * one ulp, a fixed splitting equal to a fitted one) are merely not merged; structurally equal points ARE equal in
+ * value, so nothing is merged wrongly.  Not with a transformation layer (a step in u_j moves several columns of theta by amounts the symbols do
  * not know).  With this phylino_nll_gradient plans without seeing the batch: no copy back, no synchronisation. */
 const ComponentPlan *gradient_plan(phylino_ctx *ctx, int width)
 {
@@ -811,10 +834,12 @@ const ComponentPlan *gradient_plan(phylino_ctx *ctx, int width)
         const int P = 2 * width + 1;
         std::vector<double> sym((size_t)P * width);
         for (int r = 0; r < P; ++r)
-            for (int j = 0; j < width; ++j)
-                sym[(size_t)r * width + j] = (double)j + ((r > 0 && (r - 1) / 2 == j) ? ((r & 1) ? 0.25 : -0.25) : 0.0);
+            for (int j = 0; j < width; ++j) {
+                const uint64_t tag = kSymbolTag | (4ull * (uint64_t)j + ((r > 0 && (r - 1) / 2 == j) ? ((r & 1) ? 1u : 2u) : 0u));
+                std::memcpy(&sym[(size_t)r * width + j], &tag, sizeof tag);
+            }
         ctx->grad_plan = ComponentPlan();
-        ctx->grad_plan_state = plan_components(ctx, P, sym.data(), ctx->grad_plan) ? 1 : -1;
+        ctx->grad_plan_state = plan_components(ctx, P, sym.data(), ctx->grad_plan, true) ? 1 : -1;
         if (ctx->grad_plan_state > 0) {
             /* once per model, outside any capture: the plan stays on the device */
             const std::vector<int32_t> blob = plan_blob(ctx->grad_plan);
@@ -860,8 +885,10 @@ phylino_status phylino_create(int device, void *cuda_stream, phylino_ctx **out)
     c->device = device;
     c->stream = (cudaStream_t)cuda_stream;
     DeviceGuard g(device);
+    /* allow_stage_all: the shared-memory opt-in of the spectra kernels, once per context (it is a per-device setting) */
     if (!g.ok || cudaFree(0) != cudaSuccess ||
-        cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, device) != cudaSuccess) {
+        cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, device) != cudaSuccess ||
+        allow_stage_all() != cudaSuccess) {
         cudaGetLastError();
         delete c;
         return PHYLINO_ERR_CUDA;
@@ -1591,6 +1618,7 @@ phylino_status phylino_set_energy_correction_mode(phylino_ctx *ctx, int mode)
     ctx->ec_mode = mode;
     ctx->grad_plan_state = 0;
     ctx->fused_warps = 0;               /* the threshold tables of the small-batch kernel change size */
+    ctx->fused_cache.clear();
     return PHYLINO_OK;
 }
 
@@ -1656,6 +1684,37 @@ phylino_status phylino_reserve(phylino_ctx *ctx, int max_points)
         cudaFree(ctx->d_theta); ctx->d_theta = nullptr; ctx->theta_capacity = 0;
         CU(cudaMalloc((void **)&ctx->d_theta, need * sizeof(double)));
         ctx->theta_capacity = need;
+    }
+    /* the buffers of the consumers and of the cached path, so that "allocates nothing, never synchronises" holds for
+     * every DEVICE entry point and not only for spectra / nll / expectation:
+     *   d_work   batch + NLLs of phylino_nll_gradient (2 W + 1 <= max_points) and phylino_ordering_scan
+     *            (n_grid <= max_points), the Poisson norms of phylino_draw_pseudo_data, the 2 W + 2 doubles of
+     *            phylino_variable_metric_step (N <= W);
+     *   d_mu     the expectations of phylino_nll_ensemble;
+     *   d_plan   the largest plan a cached batch of max_points points can have, V + V S + C + P (S + 1) <= P (2 S + 3);
+     *   accumulators for the V (S + 1) <= P (S + 1) / 2 rows of a cached batch (V <= P / 2 or the batch runs dense);
+     *   the structural plan of the central-difference batch, if caching is on now and the batch fits. */
+    {
+        const int64_t W = param_width(ctx), S = ctx->n_terms;
+        const int64_t work = std::max<int64_t>((int64_t)max_points * (W + 1), std::max<int64_t>(ctx->total_bins, 2 * W + 2));
+        if ((s = ensure_work(ctx, work)) != PHYLINO_OK) return s;
+        const int64_t mu_need = (int64_t)max_points * ctx->total_bins;
+        if (mu_need > ctx->mu_capacity) {
+            CU(cudaStreamSynchronize(ctx->stream));
+            cudaFree(ctx->d_mu); ctx->d_mu = nullptr; ctx->mu_capacity = 0;
+            CU(cudaMalloc((void **)&ctx->d_mu, mu_need * sizeof(double)));
+            ctx->mu_capacity = mu_need;
+        }
+        const int64_t plan_need = (int64_t)max_points * (2 * S + 3);
+        if (plan_need > ctx->plan_capacity) {
+            CU(cudaStreamSynchronize(ctx->stream));
+            cudaFree(ctx->d_plan); ctx->d_plan = nullptr; ctx->plan_capacity = 0;
+            CU(cudaMalloc((void **)&ctx->d_plan, plan_need * sizeof(int32_t)));
+            ctx->plan_capacity = plan_need;
+        }
+        const int64_t rows = ((int64_t)max_points * (S + 1) + 1) / 2;
+        if (rows > max_points && rows < (1ll << 30) && (s = ensure_acc(ctx, (int)rows)) != PHYLINO_OK) return s;
+        if (ctx->caching && !ctx->have_tf && W > 0 && 2 * W + 1 <= max_points) gradient_plan(ctx, (int)W);
     }
     /* everything else a first call would set up with a synchronisation: the occupancy of the kernels, and the
      * single-launch kernel's edge-first unit order (a function of the store alone at the default unit length) */

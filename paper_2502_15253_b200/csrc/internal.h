@@ -9,6 +9,7 @@
 #include <stdint.h>
 
 #include <string>
+#include <utility>
 #include <vector>
 
 #include "phylino.h"
@@ -229,6 +230,7 @@ cudaError_t launch_transform(const TransformArgs &a, cudaStream_t st);
 cudaError_t launch_setup(const SpectraArgs &a, int S, cudaStream_t st);
 size_t      fused_table_bytes(int S, int P, int thr_rows, int thr_stride, int n_datasets);
 bool        fused_fits(size_t table_bytes);
+cudaError_t allow_stage_all();      /* shared-memory opt-in of every spectra kernel on the current device (phylino_create) */
 cudaError_t spectra_max_warps(int S, int sm_count, bool fused, size_t table_bytes, int *warps);
 cudaError_t launch_spectra(const SpectraArgs &a, int S, cudaStream_t st, bool pdl, bool dbg);
 cudaError_t launch_fused(const SpectraArgs &a, const ParamBlob &blob, int S, cudaStream_t st, bool pdl, bool dbg);
@@ -335,6 +337,7 @@ struct phylino_ctx {
     int resident_warps = 0;                        /* warps of the ticket kernel the chip holds at once */
     int fused_warps = 0;                           /* ... of the single-launch kernel with fused_tables bytes of tables */
     size_t fused_tables = 0;
+    std::vector<std::pair<size_t, int>> fused_cache;   /* (table bytes, warps) of every table size asked so far */
     int schedule = 0;                              /* phylino_set_schedule: 0 auto, 1 tickets, 2 single launch */
     unsigned *d_done = nullptr;                    /* work counter of the small-batch kernel */
     int32_t  *d_unit_order = nullptr;              /* its item -> unit table for units of order_U batches */

@@ -1074,6 +1074,8 @@ template <int S, bool DBG> cudaError_t allow_stage_t()
                                 (int)(STAGE_BYTES + FUSED_TABLE_MAX));
 }
 
+} // namespace
+
 cudaError_t allow_stage_all()
 {
     cudaError_t e = allow_stage_t<2, false>();
@@ -1082,8 +1084,6 @@ cudaError_t allow_stage_all()
     if (e == cudaSuccess) e = allow_stage_t<3, true>();
     return e;
 }
-
-} // namespace
 
 #ifdef PHYLINO_TRACE
 extern "C" __attribute__((visibility("default"))) int phylino_debug_trace(unsigned long long *out, int reset)
@@ -1130,8 +1130,7 @@ bool fused_fits(size_t table_bytes) { return table_bytes <= FUSED_TABLE_MAX; }
 cudaError_t spectra_max_warps(int S, int sm_count, bool fused, size_t table_bytes, int *warps)
 {
     int per_sm = 0;
-    cudaError_t e = allow_stage_all();
-    if (e != cudaSuccess) return e;
+    cudaError_t e = cudaSuccess;
     if (fused) {
         e = S == 2 ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, spectra_fused_kernel<2, false>, WARPS * 32,
                                                                    STAGE_BYTES + table_bytes)

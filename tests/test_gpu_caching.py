@@ -138,3 +138,44 @@ def test_device_pointer_entry_points_use_the_cache_when_asked(gpu, oracle_mod):
     assert np.array_equal(nll_d, nll_h) and np.array_equal(h_d, h_h)
     assert np.abs(nll_d - orc.nll(wl.params, data)).max() <= ABS_NLL
     assert np.array_equal(dense, again)                    # the dense path is untouched by a cached call in between
+
+
+@pytest.mark.parametrize("k,slot,value", [(5, 5, 1.0), (5, 5, 0.75), (3, 3, 1.0), (3, 3, 1.25)])
+def test_cached_gradient_with_a_fixed_splitting(gpu, oracle_mod, k, slot, value):
+    """phylino_nll_gradient with caching plans from the STRUCTURE of the central-difference batch.
+    A mass splitting that is FIXED (idx_osc = -1) has a value but no column; whatever that value is -- here the very
+    numbers an earlier build used as the symbols of the dm2_ee column (1, 1 +- 1/4) -- its term must never be served
+    from the cell of a fitted splitting.  The cached gradient has to agree with the dense one and with the oracle:
+    3+1 model (config 5) with dm2_41 fixed, two-term model (config 3, 301 parameters) with dm2_21 fixed."""
+    import dataclasses
+    import torch
+    wl = workloads.make_config(k, scale=0.01, n_points=4)
+    idx, fixed = list(wl.model.idx_osc), list(wl.model.fixed_osc)
+    assert idx[1] == 1                                   # dm2_ee is column 1
+    idx[slot], fixed[slot] = -1, value
+    model = dataclasses.replace(wl.model, idx_osc=tuple(idx), fixed_osc=tuple(fixed))
+    wl = dataclasses.replace(wl, model=model)
+    N = model.n_params
+    orc = oracle_mod.Oracle(model, wl.events)
+    data = _data(orc, wl)
+    sig = np.where(np.isfinite(model.prior_sigma) & (model.prior_sigma > 0), model.prior_sigma, 1e-2)
+    theta = wl.theta0.copy()
+    h = 0.05 * sig
+    batch = np.tile(theta, (2 * N + 1, 1))
+    for j in range(N):
+        batch[1 + 2 * j, j] += h[j]
+        batch[2 + 2 * j, j] -= h[j]
+    nll_o = orc.nll(batch, data)
+    grad_o = (nll_o[1::2] - nll_o[2::2]) / (np.array([batch[1 + 2 * j, j] - batch[2 + 2 * j, j] for j in range(N)]))
+    dev = lambda a: torch.as_tensor(np.ascontiguousarray(a, dtype=np.float64), device="cuda")
+    with gpu.Phylino() as ph:
+        ph.load_workload(wl)
+        nll0_d, grad_d = ph.nll_gradient(dev(theta), dev(h), dev(data))
+        assert ph.last_plan()[0] == 0
+        ph.set_caching(True)
+        nll0_c, grad_c = ph.nll_gradient(dev(theta), dev(h), dev(data))
+        assert ph.last_plan()[0] > 0, "the cached path did not run"
+        nll0_d, grad_d, nll0_c, grad_c = (x.cpu().numpy() for x in (nll0_d, grad_d, nll0_c, grad_c))
+    assert abs(nll0_c[0] - nll_o[0]) <= ABS_NLL and abs(nll0_d[0] - nll_o[0]) <= ABS_NLL
+    assert np.all(np.abs(grad_c - grad_o) <= 2 * ABS_NLL / np.abs(2 * h))
+    assert np.all(np.abs(grad_c - grad_d) <= 2 * ABS_NLL / np.abs(2 * h))

@@ -380,3 +380,54 @@ def test_reserve_leaves_nothing_to_set_up_for_a_single_evaluation(gpu, oracle_mo
         st.synchronize()
         assert np.abs(out.cpu().numpy() - orc.nll(params, data)).max() <= ABS_NLL
     ph.close()
+
+
+def test_reserve_covers_the_consumers_and_the_cached_gradient(gpu, oracle_mod):
+    """phylino.h (phylino_reserve): after reserve(2 W + 1) with caching on, the FIRST calls of phylino_nll_gradient (cached
+    through the structural plan, which reserve has built), phylino_nll_ensemble, phylino_draw_pseudo_data and
+    phylino_variable_metric_step allocate nothing and never synchronise: all four are captured cold into one CUDA graph (an
+    allocation, a synchronisation or a blocking copy inside a call would fail the capture), replayed, and checked
+    against the oracle."""
+    import torch
+    wl = workloads.make_config(3, scale=0.01)
+    N = wl.model.n_params
+    orc = oracle_mod.Oracle(wl.model, wl.events)
+    data = _data(orc, wl)
+    theta = wl.params[0].copy()
+    h = np.array([wl.params[1 + 2 * j, j] - theta[j] for j in range(N)])
+    nll_o = orc.nll(wl.params, data)
+    grad_o = (nll_o[1::2] - nll_o[2::2]) / np.array([wl.params[1 + 2 * j, j] - wl.params[2 + 2 * j, j] for j in range(N)])
+    mu0 = orc.expectation(theta[None, :], orc.spectra(theta[None, :]))[0]
+    E = 5
+    st = torch.cuda.Stream()
+    with torch.cuda.stream(st):
+        ph = gpu.Phylino(stream=st.cuda_stream)
+        ph.load_workload(wl)
+        ph.set_caching(True)
+        ph.reserve(2 * N + 1)
+        d_theta, d_h, d_data, d_mu = _dev(theta), _dev(h), _dev(data), _dev(mu0)
+        nll0 = torch.zeros(1, dtype=torch.float64, device="cuda")
+        grad = torch.zeros(N, dtype=torch.float64, device="cuda")
+        pseudo = torch.zeros((E, ph.total_bins), dtype=torch.float64, device="cuda")
+        ens = torch.zeros((3, E), dtype=torch.float64, device="cuda")
+        d_pts = _dev(wl.params[:3])
+        V = _dev(np.eye(N))
+        st.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=st):
+            ph.nll_gradient(d_theta, d_h, d_data, nll0, grad)           # the first calls of this context
+            plan = ph.last_plan()
+            ph.draw_pseudo_data(d_mu, E, seed=9, out=pseudo)
+            ph.nll_ensemble(d_pts, pseudo, out=ens)
+            direction, edm = ph.variable_metric_step(V, grad)
+        g.replay()
+        st.synchronize()
+        assert plan[0] > 0                                              # cached through the structural plan
+        assert abs(nll0.cpu().numpy()[0] - nll_o[0]) <= ABS_NLL
+        assert np.all(np.abs(grad.cpu().numpy() - grad_o) <= 1e-6 / np.abs(h))
+        want = oracle_mod.draw_pseudo_data(mu0, E, seed=9)
+        assert np.array_equal(pseudo.cpu().numpy(), want)
+        ens_o = np.stack([orc.nll(wl.params[:3], want[e]) for e in range(E)], axis=1)
+        assert np.abs(ens.cpu().numpy() - ens_o).max() <= ABS_NLL
+        assert np.array_equal(direction.cpu().numpy(), -grad.cpu().numpy())    # V = 1
+    ph.close()
