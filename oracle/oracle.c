@@ -528,7 +528,7 @@ double orc_uniform53(uint64_t seed, uint32_t bin, uint32_t experiment)
 
 double orc_poisson_norm(double mu)
 {
-    if (!(mu > 0.0) || isinf(mu)) return 1.0;
+    if (!(mu > 0.0) || isinf(mu) || mu > 1e9) return 1.0;     /* outside the domain (R26): Z is not used */
     const double m = floor(mu);
     double L = 0.0, R = 0.0, t = 1.0;
     for (double k = m; k >= 1.0; k -= 1.0) {     /* w_{k-1} = w_k * (k / mu) */
@@ -547,6 +547,7 @@ double orc_poisson_norm(double mu)
 
 double orc_poisson_inv(double mu, double Z, double u)
 {
+    if (mu > 1e9 && !isinf(mu)) return NAN;      /* DESIGN.md R26: a finite mu above 1e9 is outside the domain */
     if (!(mu > 0.0) || isinf(mu)) return 0.0;
     const double m = floor(mu), target = u * Z;
     double acc = 1.0, tr = 1.0, tl = 1.0, kr = m, kl = m;

@@ -42,18 +42,27 @@ __device__ __forceinline__ double uniform53(unsigned long long seed, unsigned bi
     return (double)(((unsigned long long)c0 << 21) | (unsigned long long)(c1 >> 11)) * 0x1p-53;
 }
 
+/* Domain of the sampler (R26): 0 < mu <= POISSON_MAX_MU.  The walk from the mode costs O(sqrt mu) steps --
+ * about 3e5 per side at the limit -- and above 2^53 the step k -> k + 1 no longer moves, so a finite value in a
+ * device buffer could otherwise keep a thread busy for good.  Beyond the limit the count is NaN.  POISSON_MAX_STEPS
+ * bounds every loop as well; inside the domain it is never reached (it is ten times the longest walk). */
+constexpr double POISSON_MAX_MU = 1e9;
+constexpr int POISSON_MAX_STEPS = 1 << 22;
+
 __device__ double poisson_norm(double mu)
 {
-    if (!(mu > 0.0) || mu > 1.79769313486231570e308) return 1.0;
+    if (!(mu > 0.0) || mu > POISSON_MAX_MU) return 1.0;
     const double m = floor(mu);
     double L = 0.0, R = 0.0, t = 1.0;
-    for (double k = m; k >= 1.0; k -= 1.0) {
+    int steps = 0;
+    for (double k = m; k >= 1.0 && steps < POISSON_MAX_STEPS; k -= 1.0, ++steps) {
         t = t * (k / mu);
         if (L + t == L) break;
         L += t;
     }
     t = 1.0;
-    for (double k = m + 1.0;; k += 1.0) {
+    steps = 0;
+    for (double k = m + 1.0; steps < POISSON_MAX_STEPS; k += 1.0, ++steps) {
         t = t * (mu / k);
         if (R + t == R) break;
         R += t;
@@ -63,11 +72,13 @@ __device__ double poisson_norm(double mu)
 
 __device__ double poisson_inv(double mu, double Z, double u)
 {
+    if (mu > POISSON_MAX_MU && mu <= 1.79769313486231570e308) return __longlong_as_double(0x7ff8000000000000ll);
     if (!(mu > 0.0) || mu > 1.79769313486231570e308) return 0.0;
     const double m = floor(mu), target = u * Z;
     double acc = 1.0, tr = 1.0, tl = 1.0, kr = m, kl = m;
     if (target < acc) return m;
-    for (;;) {
+    for (int steps = 0;; ++steps) {
+        if (steps >= POISSON_MAX_STEPS) return kr;
         kr += 1.0;
         tr = tr * (mu / kr);
         acc += tr;

@@ -230,3 +230,83 @@ def test_variable_metric_step_matches_the_oracle_bit_for_bit(gpu, oracle_mod):
         torch.cuda.synchronize()
     assert all(b < a for a, b in zip(f, f[1:])) and f[-1] < f[0] - 1.0, f
     assert abs(f[-1] - orc.nll(d_theta.cpu().numpy()[None, :], data)[0]) <= ABS_NLL
+
+
+def _philox_bigint(ctr, key, rounds=10):
+    """Philox4x32 round function as published (Salmon et al., SC'11, section 3.3) on Python integers -- typed here
+    from the publication, shared with neither the library nor the oracle."""
+    M0, M1, W0, W1 = 0xD2511F53, 0xCD9E8D57, 0x9E3779B9, 0xBB67AE85
+    c, k = list(ctr), list(key)
+    for _ in range(rounds):
+        p0, p1 = M0 * c[0], M1 * c[2]
+        c = [(p1 >> 32) ^ c[1] ^ k[0], p1 & 0xffffffff, (p0 >> 32) ^ c[3] ^ k[1], p0 & 0xffffffff]
+        k = [(k[0] + W0) & 0xffffffff, (k[1] + W1) & 0xffffffff]
+    return c
+
+
+def test_device_draws_are_the_stated_function_of_the_uniforms(gpu):
+    """The INDEPENDENT check of phylino_draw_pseudo_data (R26).  The oracle's sampler and the
+    library's follow the same operation sequence on purpose (that is what makes the bit-exact bar of
+    test_pseudo_data_bit_exact possible), so that comparison cannot find a mistake in the RULE.  This test uses neither:
+    u comes from a big-integer Philox typed from the publication, the Poisson probabilities from scipy.stats, and the
+    rule is R26 as stated in words -- [0, 1) is cut into pieces of length pmf(k) laid out from the mode m = floor(mu)
+    outwards in the order m, m+1, m-1, m+2, m-2, ... (only upwards once 0 is passed), and the count is the piece that
+    holds u.  With ring j = {m-j, ..., m+j} and F(j) = P(|X - m| <= j), the count is in the first ring with u < F(j);
+    inside it m+j if u < F(j-1) + pmf(m+j), else m-j.  Every device count must be that k wherever u is farther than
+    delta from a piece boundary (delta = 1e-11: the rounding of Z, 1e-13, plus scipy's cdf), and one of the two
+    neighbouring pieces otherwise; >= 1e4 (bin, experiment) pairs, mu from 0.3 to 1e5 including integer mu."""
+    from scipy import stats
+    from workloads.spec import DatasetEvents, DatasetSpec, ModelSpec, Workload
+    mu = np.concatenate([np.logspace(np.log10(0.3), 5.0, 688), [0.37, 1.0, 2.0, 2.5, 7.0, 1000.0, 99999.0, 1e5 - 0.5,
+                                                                 1e-3, 0.0, 31.999999999, 32.000000001]])
+    n, E, seed = mu.size, 16, 0x5EED0123456789AB
+    assert n * E >= 10000
+    edges = np.linspace(1.0, 8.0, n + 1)
+    model = ModelSpec(osc_model=0, n_params=4, idx_osc=(0, 1, 2, 3, -1, -1), fixed_osc=(0,) * 6,
+                      datasets=[DatasetSpec(n_bins=n)])
+    ev = DatasetEvents(e_nu=np.zeros(0, np.float32), e_vis=np.zeros(0, np.float32), w=np.zeros(0, np.float32),
+                       core=np.zeros(0, np.int32), L_m=np.array([1050.0]), edges=edges)
+    theta = np.array([[0.1, 2.5e-3, 0.85, 7.5e-5]])
+    with gpu.Phylino() as ph:
+        ph.load_workload(Workload("draw", model, [ev], theta, theta[0], 1))
+        got = ph.draw_pseudo_data(_dev(mu), E, seed=seed).cpu().numpy()
+    assert got.shape == (E, n)
+    key = [seed & 0xffffffff, seed >> 32]
+    delta, exact, near = 1e-11, 0, 0
+    for i in range(n):
+        if not mu[i] > 0.0:
+            assert np.all(got[:, i] == 0.0)
+            continue
+        m = int(np.floor(mu[i]))
+        J = int(12 * np.sqrt(mu[i]) + 40)
+        j = np.arange(J + 1)
+        hi = stats.poisson.cdf(m + j, mu[i])
+        lo = np.where(m - j - 1 >= 0, stats.poisson.cdf(m - j - 1, mu[i]), 0.0)
+        F = hi - lo                                               # mass of rings 0 ... j
+        for e in range(E):
+            x = _philox_bigint([i, e, 0, 0], key)
+            u = ((x[0] << 21) | (x[1] >> 11)) / 2.0 ** 53
+            ring = int(np.searchsorted(F, u, side="right"))
+            assert ring <= J, (mu[i], u)
+            if ring == 0:
+                want, bounds = m, (F[0],)
+            else:
+                cut = F[ring - 1] + stats.poisson.pmf(m + ring, mu[i])
+                want = m + ring if (u < cut or m - ring < 0) else m - ring
+                bounds = (F[ring - 1], cut, F[ring])
+            k = got[e, i]
+            assert k == np.floor(k) and k >= 0
+            if min(abs(u - b) for b in bounds) > delta:
+                assert k == want, (mu[i], e, u, k, want)
+                exact += 1
+            else:
+                assert abs(abs(k - m) - ring) <= 1, (mu[i], e, u, k, want)
+                near += 1
+    assert exact >= 10000 and near <= 5, (exact, near)
+    # outside the domain (R26): a finite mu above 1e9 gives NaN, promptly
+    with gpu.Phylino() as ph:
+        ph.load_workload(Workload("draw", model, [ev], theta, theta[0], 1))
+        wild = np.full(n, 3.0)
+        wild[:4] = [2e9, 1e15, 1e300, np.inf]
+        out = ph.draw_pseudo_data(_dev(wild), 2, seed=1).cpu().numpy()
+    assert np.isnan(out[:, :3]).all() and np.all(out[:, 3] == 0.0) and np.all(out[:, 4:] >= 0.0)
