@@ -186,8 +186,18 @@ def measure(pkg, torch, dist, k, steps, warmup, local, rank, world, flush, tunin
     P, NPAR, TB = wl.n_points, wl.model.n_params, ph.total_bins
     ph.reserve(P)
     d_params = torch.as_tensor(params, device="cuda")
-    # pseudo-data: Poisson counts around the product's own expectation at theta0 (input synthesis only)
-    mu0 = ph.expectation(torch.as_tensor(wl.theta0[None, :].copy(), device="cuda")).cpu().numpy()[0]
+    # pseudo-data: Poisson counts around the expectation at theta0.  Where the oracle leg runs (rank 0 at N = 1, the
+    # only place its NLLs are compared with the library's) the expectation is the ORACLE's, so that no input of the
+    # checker comes from the checked; elsewhere it is the library's own (input synthesis only, nothing is compared).
+    if with_oracle:
+        import oracle
+        orc0 = oracle.Oracle(wl.model, wl.events)
+        th0 = wl.theta0[None, :].copy()
+        mu0 = orc0.expectation(th0, orc0.spectra(th0))[0]
+        data_from = "oracle expectation at theta0"
+    else:
+        mu0 = ph.expectation(torch.as_tensor(wl.theta0[None, :].copy(), device="cuda")).cpu().numpy()[0]
+        data_from = "library expectation at theta0 (no oracle leg in this run)"
     data = workloads.poisson_counts(mu0, wl.seed + 7)
     d_data = torch.as_tensor(data, device="cuda")
     d_nll = torch.empty(P, dtype=torch.float64, device="cuda")
@@ -374,6 +384,7 @@ def measure(pkg, torch, dist, k, steps, warmup, local, rank, world, flush, tunin
                                       "+ 1 synchronise; no copy engine (parameters ride with the kernel arguments)"}
         if with_oracle:
             res["cpu_baseline"], nll_o = oracle_rates(wl, data)
+            res["cpu_baseline"]["pseudo_data_from"] = data_from
             res["cpu_baseline"]["max_abs_nll_diff_vs_gpu"] = float(np.abs(nll_o - d_nll.cpu().numpy()[:len(nll_o)]).max())
     ph.close()
     return res

@@ -79,8 +79,9 @@ def test_random_small_workload(gpu, oracle_mod, i):
     fin = np.isfinite(nll_o)
     assert np.array_equal(np.isfinite(nll), fin) and np.array_equal(np.isfinite(nll_h), fin)
     if fin.any():
-        # the 1e-6 bar is for likelihoods of the paper's size (up to ~1e6); a random constraint on theta^-2 of a
-        # 1e-5-sized parameter makes the NLL 1e10, where ONE ulp is 2e-6: beyond 1e6 the bar scales with the value
+        # DESIGN.md R31: the 1e-6 bar is for likelihoods of the paper's size (up to ~1e6); a random constraint on
+        # theta^-2 of a 1e-5-sized parameter makes the NLL 1e10, where ONE ulp is 2e-6: beyond 1e6 the bar scales with
+        # the value (1e-12 relative)
         tol = 1e-6 * np.maximum(1.0, np.abs(nll_o[fin]) / 1e6)
         assert np.all(np.abs(nll[fin] - nll_o[fin]) <= tol)
         assert np.all(np.abs(nll_h[fin] - nll_o[fin]) <= tol)
