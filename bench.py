@@ -390,6 +390,86 @@ def measure(pkg, torch, dist, k, steps, warmup, local, rank, world, flush, tunin
     return res
 
 
+def sharded_steps(evaluate, params, n_events, steps, warmup, dist, before_step, timer, check_against=None, tol=1e-9):
+    """The STRONG arm of a multi-rank run: ONE batch of points is cut across the ranks
+    with sharding.shard_points, every rank evaluates its slice, and nll[P] is all-gathered INSIDE the timed region
+    (sharding.sharded_eval).  The step time is the maximum over ranks; value = n_events x P / that time.
+    Device-agnostic so that the CPU test can drive it with gloo: `evaluate(slice) -> one row per point`,
+    `before_step()` = flush + synchronise + barrier, `timer` = object with start() / stop() -> milliseconds on the
+    device the evaluator runs on.  check_against: the unsharded result on this rank (rank 0), compared to `tol`
+    (a slice is a batch of another size, so the rows agree to rounding, not bit for bit)."""
+    import torch
+    from paper_2502_15253_b200 import sharding
+    world = dist.get_world_size() if dist.is_initialized() else 1
+    rank = dist.get_rank() if dist.is_initialized() else 0
+    P = int(params.shape[0])
+    ms, out = [], None
+    for it in range(warmup + steps):
+        before_step()
+        timer.start()
+        out = sharding.sharded_eval(evaluate, params)
+        t = torch.tensor([timer.stop()], dtype=torch.float64, device=params.device)
+        if world > 1:
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        if it >= warmup:
+            ms.append(float(t.item()))
+    if tuple(out.shape[:1]) != (P,):
+        raise RuntimeError("the gathered result does not have one row per point")
+    res = {"points": P, "slices": sharding.shard_sizes(P, world), "steps": steps, "warmup": warmup,
+           "ms_per_step": sum(ms) / len(ms), "ms_per_step_min": min(ms),
+           "value": n_events * P / (sum(ms) / len(ms) * 1e-3), "unit": UNIT, "scaling": "strong",
+           "collective": "all_gather of nll[P] inside the timed region (padded to the largest slice)"}
+    if check_against is not None and rank == 0:
+        err = float((out - check_against).abs().max()) if P else 0.0
+        res["max_abs_nll_diff_vs_one_gpu"] = err
+        if not err <= tol:
+            raise RuntimeError(f"sharded NLLs differ from the one-GPU batch by {err} > {tol}")
+    return res
+
+
+class CudaEventTimer:
+    """milliseconds between start() and stop() on torch's current CUDA stream (the library's stream in bench.py)"""
+    def __init__(self, torch):
+        self.torch = torch
+        self.a, self.b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+
+    def start(self):
+        self.a.record()
+
+    def stop(self):
+        self.b.record()
+        self.b.synchronize()
+        return self.a.elapsed_time(self.b)
+
+
+def sharded_arm(pkg, torch, dist, k, steps, warmup, local, rank, world, flush):
+    """config k's whole batch sharded over the ranks (603 points over 8 ranks: 76 / 75, the uneven case)"""
+    wl = workloads.make_config(k)
+    ph = pkg.Phylino(device=local)
+    ph.load_workload(wl)
+    ph.reserve(wl.n_points if rank == 0 else max(1, -(-wl.n_points // world)))
+    d_params = torch.as_tensor(wl.params, device="cuda")
+    mu0 = ph.expectation(torch.as_tensor(wl.theta0[None, :].copy(), device="cuda")).cpu().numpy()[0]
+    d_data = torch.as_tensor(workloads.poisson_counts(mu0, wl.seed + 7), device="cuda")
+    whole = ph.nll(d_params, d_data).clone() if rank == 0 else None     # the one-GPU call, for the check only
+
+    def before_step():
+        flush.fill_(1)
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+
+    def evaluate(p):
+        if p.shape[0] == 0:
+            return torch.empty(0, dtype=torch.float64, device="cuda")
+        return ph.nll(p, d_data)
+
+    res = sharded_steps(evaluate, d_params, wl.n_events, steps, warmup, dist, before_step, CudaEventTimer(torch), whole)
+    res["workload"] = f"{wl.name} (BASELINE.json configs[{k - 1}])"
+    ph.close()
+    return res
+
+
 def measured_hbm_gbs() -> float:
     try:
         return float(json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"])
@@ -543,6 +623,8 @@ def main():
     ap.add_argument("--max-warps", type=int, default=0, help="tuning: cap on the persistent grid's warps")
     ap.add_argument("--ref-points", type=int, default=16, help="points per step of --impl reference")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-sharded-arm", action="store_true", help="N > 1: skip the strong (sharded batch) arm")
+    ap.add_argument("--sharded-arm", action="store_true", help="run the strong arm also at N = 1 (one slice, no collective)")
     ap.add_argument("--no-gradient-step", action="store_true",
                     help="skip the wall time of config 3's 603-point gradient step that the default run adds")
     args = ap.parse_args()
@@ -588,6 +670,13 @@ def main():
             others.append(measure(pkg, torch, dist, k, args.other_steps, args.warmup, local, rank, world, flush, tuning,
                                   False, measured_peak, with_oracle))
 
+    # N > 1: besides the weak arm above (every rank its own batch), the STRONG arm -- the configured batch cut across
+    # the ranks and gathered inside the timed region: config 5's 4096 points and config 3's 603 (uneven slices)
+    sharded = []
+    if (world > 1 and not args.no_sharded_arm) or args.sharded_arm:
+        for k in (HEADLINE_CONFIG, 3):
+            sharded.append(sharded_arm(pkg, torch, dist, k, min(args.steps, args.other_steps), args.warmup, local, rank,
+                                       world, flush))
     if rank == 0:
         line = {
             "metric": METRIC, "value": head["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
@@ -610,6 +699,8 @@ def main():
             line["configs"] = sorted(others + [head], key=lambda r: r["config"])
         if world == 1 and all_configs and not args.no_gradient_step:
             line["gradient_step"] = gradient_step_wall(pkg, torch, local, flush)
+        if sharded:
+            line["sharded"] = sharded
         print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
